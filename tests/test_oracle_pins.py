@@ -1,0 +1,314 @@
+"""Pins for the CPU oracle (oracle/) -- what the paper and the mathematics fix, NOT the oracle re-typed.
+
+Pin numbering follows DESIGN.md section 3 (P1..P11).  None of these tests touches the CUDA path.
+
+  P1  hand-evaluated eq. 1 delays (tests/golden/delays_eq1_hand.txt)
+  P2  closed-form properties + exact rational arithmetic (fractions.Fraction)
+  P3  table checksums computed independently for the survey
+  P4  DM = 0 row is the plain channel sum (numpy.sum)                            eq. 5 with DM = 0
+  P5  impulse response, brute force over (channel, time), all nbits              eq. 3
+  P6  linearity                                                                   eq. 3 is a sum
+  P7  time-shift covariance                                                       eq. 3
+  P8  an injected dispersed pulse peaks at its own DM trial and time             PAPER.md:37 (Fig. 1)
+  P9  C loop == numpy gather == pure-Python triple loop on tiny inputs           eq. 3
+  P10 output statistics of uniform 2-bit noise                                   eq. 3 + CLT
+  P11 packing convention: bytes 0xE4 / 0x21                                      reading R9
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import torch
+
+import dd_workloads as W
+import oracle
+
+
+def _table(cfg):
+    return oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list())
+
+
+def _read_rows(path):
+    rows = []
+    with open(path) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                rows.append(line.split())
+    return rows
+
+
+# ----------------------------------------------------------------------------- P1
+def test_p1_hand_delays(golden_dir):
+    cfg = W.CONFIGS[1]
+    for dm, c, x_hand, delay in _read_rows(os.path.join(golden_dir, "delays_eq1_hand.txt")):
+        dm, c, x_hand, delay = float(dm), int(c), float(x_hand), int(delay)
+        tab = oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, [dm])
+        assert tab[0, c] == delay, (dm, c)
+        assert abs(tab[0, c] - x_hand) <= 0.5 + 0.05
+        assert round(x_hand) == delay
+
+
+# ----------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_p2_closed_form_properties(idx):
+    cfg = W.CONFIGS[idx]
+    tab = _table(cfg)
+    assert tab.shape == (cfg.ndm, cfg.nchans)
+    assert (tab[:, 0] == 0).all(), "delay is relative to the start of the band (PAPER.md:60)"
+    assert (tab[0, :] == 0).all(), "DM = 0 has no delay (eq. 5)"
+    assert (np.diff(tab, axis=1) >= 0).all(), "lower frequency arrives later (eq. 1)"
+    assert (np.diff(tab, axis=0) >= 0).all(), "delay grows with DM (eq. 1)"
+    assert tab.min() >= 0
+
+
+def _exact_delay(cfg, dm: float, c: int) -> int:
+    """floor(x + 1/2) with x evaluated in exact rational arithmetic on the double inputs."""
+    K = Fraction(4148808, 1000)
+    f_top, df, dt = Fraction(cfg.f_top), Fraction(cfg.df), Fraction(cfg.dt)
+    f = f_top + c * df
+    x = K * Fraction(dm) * (1 / (f * f) - 1 / (f_top * f_top)) / dt
+    return math.floor(x + Fraction(1, 2))
+
+
+def test_p2_exact_rational_full_cfg1():
+    cfg = W.CONFIGS[1]
+    tab = _table(cfg)
+    dms = cfg.dm_list()
+    for d in range(cfg.ndm):
+        for c in range(cfg.nchans):
+            assert tab[d, c] == _exact_delay(cfg, float(dms[d]), c), (d, c)
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_p2_exact_rational_sampled(idx):
+    cfg = W.CONFIGS[idx]
+    tab = _table(cfg)
+    dms = cfg.dm_list()
+    rng = np.random.default_rng(idx)
+    ds = np.concatenate([rng.integers(0, cfg.ndm, 1500), [0, 1, cfg.ndm - 1, cfg.ndm - 1]])
+    cs = np.concatenate([rng.integers(0, cfg.nchans, 1500), [cfg.nchans - 1, 1, cfg.nchans - 1, 0]])
+    for d, c in zip(ds, cs):
+        assert tab[d, c] == _exact_delay(cfg, float(dms[d]), int(c)), (d, c)
+
+
+def test_p2_k_dm_is_the_papers_constant():
+    """The common 1/2.41e-4 approximation must NOT be what the oracle uses (reading R3)."""
+    cfg = W.CONFIGS[2]
+    tab = oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, [1000.0])
+    f_lo = cfg.f_top + (cfg.nchans - 1) * cfg.df
+    x_paper = 4.148808e3 * 1000.0 * (f_lo ** -2 - cfg.f_top ** -2) / cfg.dt
+    x_approx = (1.0 / 2.41e-4) * 1000.0 * (f_lo ** -2 - cfg.f_top ** -2) / cfg.dt
+    assert abs(x_paper - x_approx) > 2.0
+    assert abs(tab[0, -1] - x_paper) <= 0.5
+
+
+# ----------------------------------------------------------------------------- P3
+def test_p3_table_checksums(golden_dir):
+    for idx, mx, sm, mid in _read_rows(os.path.join(golden_dir, "table_checksums.txt")):
+        cfg = W.CONFIGS[int(idx)]
+        tab = _table(cfg)
+        assert int(tab.max()) == int(mx)
+        assert int(tab.sum()) == int(sm)
+        if int(mid) >= 0:
+            assert int(tab[cfg.ndm // 2, cfg.nchans // 2]) == int(mid)
+
+
+def test_p3_two_evaluation_orders_agree():
+    """north_star's expression (C oracle) and the paper's LUT order eq. 4 then eq. 5 (numpy) give one table (R2)."""
+    for idx in (1, 2, 3, 4):
+        cfg = W.CONFIGS[idx]
+        assert np.array_equal(_table(cfg), oracle.delay_table_np(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list()))
+
+
+# ----------------------------------------------------------------------- helpers
+def _random_case(nbits, nchans, nsamps, ndm, maxdelay, seed):
+    rng = np.random.default_rng(seed)
+    delays = rng.integers(0, maxdelay + 1, size=(ndm, nchans)).astype(np.int64)
+    delays[0, :] = 0
+    per = 8 // nbits
+    a_len = -(-(nsamps + maxdelay) // (16 * per)) * (16 * per)
+    a = rng.integers(0, 1 << nbits, size=(nchans, a_len)).astype(np.uint8)
+    packed = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+    return a, packed, delays
+
+
+# ----------------------------------------------------------------------------- P4
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_p4_dm0_is_channel_sum(nbits):
+    a, packed, delays = _random_case(nbits, 37, 1000, 3, 50, seed=nbits)
+    out = oracle.dedisperse(packed, nbits, 1000, delays)
+    assert np.array_equal(out[0], a[:, :1000].astype(np.int64).sum(axis=0))
+
+
+def test_p4_dm0_cfg1_real_table():
+    cfg = W.CONFIGS[1]
+    tab = _table(cfg)
+    packed, _ = W.gen_packed(cfg, int(tab.max()))
+    out = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab)
+    assert np.array_equal(out[0], packed[0].numpy()[:, :cfg.nsamps].astype(np.int64).sum(axis=0))
+
+
+# ----------------------------------------------------------------------------- P5
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_p5_impulse_response(nbits):
+    """A single non-zero sample a[c*][tau] = v appears at out[d][tau - delay[d][c*]] and nowhere else."""
+    nchans, nsamps, ndm, maxdelay = 9, 64, 5, 23
+    rng = np.random.default_rng(100 + nbits)
+    delays = rng.integers(0, maxdelay + 1, size=(ndm, nchans)).astype(np.int64)
+    per = 8 // nbits
+    a_len = -(-(nsamps + maxdelay) // (16 * per)) * (16 * per)
+    vmax = (1 << nbits) - 1
+    for cstar in range(nchans):
+        for tau in range(0, nsamps + maxdelay, 7):
+            a = np.zeros((nchans, a_len), np.uint8)
+            a[cstar, tau] = vmax
+            packed = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+            out = oracle.dedisperse(packed, nbits, nsamps, delays)
+            expect = np.zeros((ndm, nsamps), np.uint32)
+            for d in range(ndm):
+                t = tau - delays[d, cstar]
+                if 0 <= t < nsamps:
+                    expect[d, t] = vmax
+            assert np.array_equal(out, expect), (cstar, tau)
+
+
+# ----------------------------------------------------------------------------- P6
+@pytest.mark.parametrize("nbits", [4, 8])
+def test_p6_linearity(nbits):
+    nchans, nsamps, ndm, maxdelay = 21, 500, 6, 40
+    half = (1 << nbits) // 2
+    rng = np.random.default_rng(7)
+    delays = rng.integers(0, maxdelay + 1, size=(ndm, nchans)).astype(np.int64)
+    per = 8 // nbits
+    a_len = -(-(nsamps + maxdelay) // (16 * per)) * (16 * per)
+    A = rng.integers(0, half, size=(nchans, a_len)).astype(np.uint8)
+    B = rng.integers(0, half, size=(nchans, a_len)).astype(np.uint8)
+    pk = lambda x: W.pack_rows(torch.from_numpy(x), nbits).numpy()
+    D = lambda x: oracle.dedisperse(pk(x), nbits, nsamps, delays).astype(np.int64)
+    assert np.array_equal(D(A + B), D(A) + D(B))
+    assert np.array_equal(D((2 * (A // 2)).astype(np.uint8)), 2 * D(A // 2))
+
+
+# ----------------------------------------------------------------------------- P7
+def test_p7_time_shift():
+    nbits, nchans, nsamps, ndm, maxdelay, s = 8, 13, 400, 4, 31, 17
+    a, packed, delays = _random_case(nbits, nchans, nsamps + s, ndm, maxdelay, seed=77)
+    full = oracle.dedisperse(packed, nbits, nsamps + s, delays)
+    shifted = np.zeros_like(a)
+    shifted[:, :a.shape[1] - s] = a[:, s:]
+    out_shift = oracle.dedisperse(shifted, nbits, nsamps, delays)
+    assert np.array_equal(out_shift, full[:, s:s + nsamps])
+
+
+# ----------------------------------------------------------------------------- P8
+def test_p8_injected_pulse_cfg1():
+    cfg = W.CONFIGS[1]
+    tab = _table(cfg)
+    pulses = W.make_pulses(cfg, lambda idx: tab[idx])
+    assert pulses.dm_index[0] == 10 and abs(cfg.dm_list()[10] - 50.0) < 1e-12
+    packed, _ = W.gen_packed(cfg, int(tab.max()), pulses)
+    out = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab)
+    d, t = np.unravel_index(np.argmax(out), out.shape)
+    assert (d, t) == (10, int(pulses.t0[0]))
+    # peak ~ 64*128 + 64*40 = 10752 against noise sigma 16*sqrt(64) = 128
+    assert abs(int(out[d, t]) - 10752) < 6 * 128
+    assert out[d, t] - np.partition(out.ravel(), -2)[-2] > 0
+
+
+def test_p8_injected_pulses_cfg3_reduced():
+    cfg = W.CONFIGS[3].reduced(nsamps=6000, ndm=48, nchans=512)
+    tab = _table(cfg)
+    pulses = W.make_pulses(cfg, lambda idx: tab[idx])
+    packed, _ = W.gen_packed(cfg, int(tab.max()), pulses)
+    out = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab).astype(np.int64)
+    mean = out.mean()
+    for d_i, t_i in zip(pulses.dm_index, pulses.t0):
+        col = out[:, t_i]
+        assert col[d_i] == col.max()
+        assert out[d_i, t_i] - mean >= 0.9 * cfg.pulse_amp * cfg.nchans
+
+
+# ----------------------------------------------------------------------------- P9
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_p9_three_formulations_agree(nbits):
+    nchans, nsamps, ndm, maxdelay = 16, 256, 8, 45
+    a, packed, delays = _random_case(nbits, nchans, nsamps, ndm, maxdelay, seed=900 + nbits)
+    c_out = oracle.dedisperse(packed, nbits, nsamps, delays)
+    assert np.array_equal(oracle.unpack(packed, nbits, a.shape[1]), a)
+    assert np.array_equal(oracle.unpack_np(packed, nbits, a.shape[1]), a)
+    assert np.array_equal(c_out, oracle.dedisperse_gather_np(a, delays, nsamps))
+    assert np.array_equal(c_out[:3, :40], np.asarray(oracle.dedisperse_loops_py(a, delays[:3], 40)))
+    # per-point evaluation agrees too
+    rng = np.random.default_rng(1)
+    d_idx, t_idx = rng.integers(0, ndm, 50), rng.integers(0, nsamps, 50)
+    pts = oracle.dedisperse_points(lambda c, t: a[c, t], delays, d_idx, t_idx)
+    assert np.array_equal(pts, c_out[d_idx, t_idx])
+    # threads do not change the answer
+    assert np.array_equal(c_out, oracle.dedisperse(packed, nbits, nsamps, delays, nthreads=1))
+
+
+def test_p9_hand_worked_transform(golden_dir):
+    spec = {"delay": [], "in": [], "out": []}
+    for row in _read_rows(os.path.join(golden_dir, "tiny_transform.txt")):
+        if row[0] in spec:
+            spec[row[0]].append([int(x) for x in row[1:]])
+    a = np.zeros((3, 16), np.uint8)
+    a[:, :7] = np.asarray(spec["in"], np.uint8)
+    delays = np.asarray(spec["delay"], np.int64)
+    expect = np.asarray(spec["out"], np.uint32)
+    for nbits in (2, 4, 8):
+        packed = np.zeros((3, 16), np.uint8)
+        pk = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+        packed[:, :pk.shape[1]] = pk
+        assert np.array_equal(oracle.dedisperse(packed, nbits, 4, delays), expect)
+    assert np.array_equal(oracle.dedisperse_gather_np(a, delays, 4), expect)
+
+
+# ---------------------------------------------------------------------------- P10
+def test_p10_statistics_cfg2_reduced():
+    cfg = W.CONFIGS[2].reduced(nsamps=4096, ndm=16)
+    tab = _table(cfg)
+    packed, _ = W.gen_packed(cfg, int(tab.max()))
+    out = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab).astype(np.float64)
+    assert out.max() <= 1024 * 3
+    assert abs(out.mean() - 1536.0) < 1.0            # 1024 * 1.5
+    assert abs(out.std() - math.sqrt(1024 * 1.25)) < 0.5
+
+
+def test_p10_output_ranges():
+    assert 1024 * 15 == 15360 < 65536          # cfg4 fits uint16
+    assert 4096 * 255 == 1044480 < (1 << 24)   # cfg3 exact in float32
+    with pytest.raises(AssertionError):
+        oracle.cast_out(np.array([70000]), "u16")
+    with pytest.raises(AssertionError):
+        oracle.cast_out(np.array([1 << 24]), "f32")
+    assert oracle.cast_out(np.array([16777215]), "f32")[0] == 16777215.0
+
+
+# ---------------------------------------------------------------------------- P11
+def test_p11_packing_convention():
+    assert oracle.unpack(np.array([[0xE4]], np.uint8), 2, 4).tolist() == [[0, 1, 2, 3]]
+    assert oracle.unpack(np.array([[0x21]], np.uint8), 4, 2).tolist() == [[1, 2]]
+    assert oracle.unpack(np.array([[0xAB]], np.uint8), 8, 1).tolist() == [[0xAB]]
+    assert W.pack_rows(torch.tensor([[0, 1, 2, 3]], dtype=torch.uint8), 2).tolist() == [[0xE4]]
+    assert W.pack_rows(torch.tensor([[1, 2]], dtype=torch.uint8), 4).tolist() == [[0x21]]
+    rng = np.random.default_rng(5)
+    for nbits in (2, 4, 8):
+        a = rng.integers(0, 1 << nbits, size=(3, 64)).astype(np.uint8)
+        p = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+        assert p.shape == (3, 64 * nbits // 8)
+        assert np.array_equal(oracle.unpack(p, nbits, 64), a)
+
+
+# --------------------------------------------------------------- oracle regression
+def test_oracle_regression_file(golden_dir):
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(golden_dir, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = {r[0]: tuple(int(x) for x in r[1:]) for r in _read_rows(os.path.join(golden_dir, "oracle_regression.txt"))}
+    for name, cfg in mg.cases():
+        assert mg.checksum(mg.run_case(cfg)) == stored[name], name
