@@ -1,0 +1,160 @@
+/*
+ * dd.h -- C ABI of the B200-native direct incoherent dedispersion library (libdd_b200.so).
+ *
+ * The operation is the paper's *direct* dedispersion transform (arXiv:1201.5380; citations are
+ * /root/reference/PAPER.md line numbers):
+ *
+ *     D[d][t] = sum_{c=0}^{nchans-1} A[c][ t + delay[d][c] ]                    eq. 3
+ *     delay[d][c] = floor( k_DM * DM[d] * (f_c^-2 - f_top^-2) / dt + 0.5 )      eq. 1, 4, 5
+ *     f_c = f_top + c*df,  k_DM = 4.148808e3 MHz^2 pc^-1 cm^3 s
+ *
+ * over 2/4/8-bit packed unsigned filterbank input.  The API is a plan object in the
+ * style the paper describes for its own library ("modeled on FFTW"): create a plan
+ * from the observing parameters, give it any list of DM trials, execute it on
+ * device-resident data.  Batching over independent beams follows PAPER.md:388 (footnote 5).
+ *
+ * Conventions
+ *   - Plain C types only.  Every pointer argument says whether it is HOST or DEVICE memory.
+ *   - All functions return a dd_status (0 = DD_OK, negative = error) unless stated; none aborts.
+ *     On error the plan is left unchanged.
+ *   - A plan is not thread-safe; distinct plans are independent.  The library never frees or
+ *     retains caller buffers.  The plan owns its DM list, delay table and tile metadata (host and
+ *     device copies) until dd_plan_destroy.
+ *   - There is NO CPU fallback: dd_execute* return DD_ERR_CUDA when no CUDA device is usable.
+ */
+#ifndef DD_B200_H
+#define DD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dd_plan_s *dd_plan; /* opaque, library-owned */
+typedef int dd_status;
+
+enum {
+    DD_OK = 0,
+    DD_ERR_NULL = -1,             /* a required pointer is NULL                                          */
+    DD_ERR_INVALID_ARG = -2,      /* nchans<=0, dt<=0, f_top<=0, df>=0, lowest frequency<=0, nbits not in
+                                     {2,4,8}, ndm<=0, DM<0 or non-finite, nsamps<=0, out_nbits unknown,
+                                     nbeams<=0, negative beam stride                                      */
+    DD_ERR_NO_DM_LIST = -3,       /* dd_set_dm_list has not succeeded on this plan yet                    */
+    DD_ERR_ALIGNMENT = -4,        /* in_ptr not 16-byte aligned, in_stride or in_beam_stride not a
+                                     multiple of 16, out_ptr not aligned to its element size              */
+    DD_ERR_STRIDE_TOO_SMALL = -5, /* in_stride*8 < (nsamps + max_delay)*nbits, or a beam stride smaller
+                                     than one beam                                                        */
+    DD_ERR_OUT_RANGE = -6,        /* nchans*(2^nbits-1) does not fit the requested output type exactly
+                                     (>65535 for uint16, >=2^24 for float32)                              */
+    DD_ERR_DELAY_OVERFLOW = -7,   /* a delay does not fit int32                                           */
+    DD_ERR_SMEM = -8,             /* the delay spread of one DM block does not fit shared memory          */
+    DD_ERR_CUDA = -9,             /* a CUDA call failed / no device; text via dd_last_cuda_error          */
+    DD_ERR_NOMEM = -10            /* host allocation failed                                               */
+};
+
+/* Output element type codes for `out_nbits` (reading R12 of DESIGN.md): raw sums, no scaling. */
+enum {
+    DD_OUT_F32 = 32,  /* float32 (exact: sums < 2^24)  */
+    DD_OUT_U16 = 16,  /* uint16                         */
+    DD_OUT_U32 = -32  /* uint32                         */
+};
+
+/*
+ * dd_plan_create -- the observing parameters of PAPER.md:55-67 / 384.
+ *   plan    HOST out: receives the new plan.
+ *   nchans  number of frequency channels N_nu (> 0).
+ *   dt      sampling interval in seconds (> 0), e.g. 64e-6.
+ *   f_top   frequency of channel 0 in MHz ("start of the band", nu_0; > 0).
+ *   df      channel width in MHz, < 0 (descending band; reading R6); f_top + (nchans-1)*df must be > 0.
+ *   nbits   bits per input sample: 2, 4 or 8 (unsigned).
+ * Host only; touches no device.
+ */
+dd_status dd_plan_create(dd_plan *plan, int nchans, double dt, double f_top, double df, int nbits);
+
+/* Frees the plan and its host and device tables.  NULL is accepted. */
+dd_status dd_plan_destroy(dd_plan plan);
+
+/*
+ * dd_set_dm_list -- "any list of DMs": finite, >= 0, any order, pc cm^-3.
+ *   dm_list  HOST, ndm doubles; copied.
+ * Computes, in double precision on the host (eq. 4-5), the int32 delay table
+ * [ndm][nchans] and the per-(DM block, channel) span metadata, then uploads them if a CUDA device
+ * is present (may synchronise).  Without a device the host tables are still built (so
+ * dd_get_delay_table works) and the upload is retried by the first dd_execute.
+ * Replaces any previous list.
+ */
+dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm);
+
+/* Copies the delay table to `table` (HOST, ndm*nchans int32, row-major [d][c]).  Host only. */
+dd_status dd_get_delay_table(dd_plan plan, int32_t *table);
+
+/* max over the delay table (>= 0), or DD_ERR_NO_DM_LIST / DD_ERR_NULL (negative).  Host only. */
+int64_t dd_get_max_delay(dd_plan plan);
+
+/*
+ * dd_set_batch -- independent beams processed by ONE dd_execute call.
+ *   nbeams           >= 1 (default 1).
+ *   in_beam_stride   bytes between beam b and b+1 of the input  (multiple of 16; >= nchans*in_stride
+ *                    is checked at execute time).  Ignored when nbeams == 1.
+ *   out_beam_stride  bytes between beam b and b+1 of the output (>= ndm*nsamps*elem, checked at
+ *                    execute time; multiple of the element size).
+ * All beams share the plan's delay table.
+ */
+dd_status dd_set_batch(dd_plan plan, int nbeams, int64_t in_beam_stride, int64_t out_beam_stride);
+
+/*
+ * dd_execute -- the dedispersion transform (eq. 3) on device-resident data, asynchronously.
+ *   nsamps     number of OUTPUT samples per DM trial (> 0) (reading R8).
+ *   in_ptr     DEVICE, 16-byte aligned.  in[beam][c] is a row of at least nsamps + dd_get_max_delay()
+ *              samples packed along time, LSB first: sample t is bits [(t*nbits)&7, +nbits) of byte
+ *              (t*nbits)>>3 (reading R9).  Rows are in_stride bytes apart and must be READABLE out to
+ *              in_stride bytes (the kernel's 16-byte bulk copies may touch the padding).
+ *   in_stride  bytes between channel rows; multiple of 16; in_stride*8 >= (nsamps+max_delay)*nbits.
+ *   out_ptr    DEVICE.  out[beam][d][t], dense rows of nsamps elements, DM-major, time contiguous.
+ *   out_nbits  DD_OUT_F32 (32), DD_OUT_U16 (16) or DD_OUT_U32 (-32).
+ *   stream     a cudaStream_t (NULL = default stream).
+ * Enqueues on `stream` and returns; does not synchronise and does not allocate (except that the first
+ * call after a dd_set_dm_list made without a device uploads the tables).  The caller keeps in/out
+ * alive until the stream has passed the enqueued work.  Launch errors are returned as DD_ERR_CUDA.
+ */
+dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
+                     int out_nbits, void *stream);
+
+/*
+ * dd_execute_host -- the same transform with HOST buffers (end-to-end path).
+ *   in_host / out_host  HOST memory with the layouts of dd_execute (pinned memory gives full PCIe speed).
+ * Copies the input to device staging owned by the plan, runs the kernel over time slabs and copies each
+ * slab's output back, overlapping copies with compute on internal streams; returns after everything
+ * has completed (synchronous).  Staging buffers are (re)allocated when the problem size grows.
+ */
+dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int64_t in_stride,
+                          void *out_host, int out_nbits);
+
+/*
+ * dd_get_launch_info -- how the plan tiles the problem (for benchmarks and tests).  Host only.
+ *   info  HOST out, 8 int64: [0] DMs per CTA (DB), [1] output samples per CTA (TB), [2] channels per
+ *         pipeline stage, [3] dynamic shared memory bytes per CTA, [4] threads per CTA, [5] number of DM
+ *         blocks, [6] kernels launched by the last dd_execute (0 if none yet), [7] kernel variant id.
+ */
+dd_status dd_get_launch_info(dd_plan plan, int64_t *info);
+
+/*
+ * dd_int_add_peak -- measures this GPU's 32-bit integer-add throughput (the ALU roofline denominator
+ * of DESIGN.md section 6) with a register-resident microbenchmark on all SMs.
+ *   mode          0: independent chains of 2-input adds; 1: 3-input adds (two additions per IADD3).
+ *   adds_per_sec  HOST out: additions per second (adds counted, not instructions).
+ *   stream        cudaStream_t.  Synchronises.
+ */
+dd_status dd_int_add_peak(int mode, double *adds_per_sec, void *stream);
+
+/* Static description of a status code. */
+const char *dd_strerror(dd_status s);
+
+/* Text of the last CUDA error seen by this library in the calling thread ("" if none). */
+const char *dd_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DD_B200_H */

@@ -1,0 +1,233 @@
+"""paper_1201_5380_b200 -- B200-native direct incoherent dedispersion (arXiv:1201.5380, eq. 3-5).
+
+Thin Python binding over the C ABI of `include/dd.h` (libdd_b200.so, built in-tree by
+`paper_1201_5380_b200/build.py`).  The functions have the same names as the C entry points and
+only marshal arguments: every step of the hot path runs in the library's CUDA kernels.  PyTorch
+is used by callers for device memory and streams only.
+
+There is NO CPU fallback.  Importing this package does not load the library; the first call
+does, and raises `DDLibraryError` if the CUDA extension has not been built.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+__all__ = [
+    "DDError", "DDLibraryError", "lib", "library_path",
+    "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
+    "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_strerror", "dd_last_cuda_error", "Plan",
+    "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
+]
+
+DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
+
+# every symbol include/dd.h declares (tests check the library exports exactly these)
+EXPORTED_SYMBOLS = (
+    "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
+    "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_strerror", "dd_last_cuda_error",
+)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB: Optional[ctypes.CDLL] = None
+
+
+class DDError(RuntimeError):
+    """A dd_* call returned a negative status."""
+
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = f"{where}: {dd_strerror(status)} (status {status})"
+        if status == -9:
+            msg += f" [{dd_last_cuda_error()}]"
+        super().__init__(msg)
+
+
+class DDLibraryError(ImportError):
+    """libdd_b200.so is missing: build it with `python -m paper_1201_5380_b200.build`."""
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "libdd_b200.so")
+
+
+def lib() -> ctypes.CDLL:
+    """Load the C-ABI library (fails loudly when it has not been built; there is no fallback)."""
+    global _LIB
+    if _LIB is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise DDLibraryError(f"{path} not found -- run `python -m paper_1201_5380_b200.build` "
+                                 f"(nvcc, sm_100a). There is no CPU fallback.")
+        L = ctypes.CDLL(path)
+        vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
+        L.dd_plan_create.argtypes = [ctypes.POINTER(vp), i32, dbl, dbl, dbl, i32]
+        L.dd_plan_destroy.argtypes = [vp]
+        L.dd_set_dm_list.argtypes = [vp, vp, i32]
+        L.dd_get_delay_table.argtypes = [vp, vp]
+        L.dd_get_max_delay.argtypes = [vp]
+        L.dd_get_max_delay.restype = i64
+        L.dd_set_batch.argtypes = [vp, i32, i64, i64]
+        L.dd_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
+        L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
+        L.dd_get_launch_info.argtypes = [vp, vp]
+        L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
+        L.dd_strerror.argtypes = [i32]
+        L.dd_strerror.restype = ctypes.c_char_p
+        L.dd_last_cuda_error.argtypes = []
+        L.dd_last_cuda_error.restype = ctypes.c_char_p
+        for name in ("dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_set_batch",
+                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak"):
+            getattr(L, name).restype = i32
+        _LIB = L
+    return _LIB
+
+
+def _addr(x) -> int:
+    """Address of a buffer: int, torch tensor (host or device), numpy array or None."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return 0
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)          # torch.cuda.Stream
+
+
+def _check(status: int, where: str) -> int:
+    if status < 0:
+        raise DDError(status, where)
+    return status
+
+
+def dd_strerror(status: int) -> str:
+    return lib().dd_strerror(int(status)).decode()
+
+
+def dd_last_cuda_error() -> str:
+    return lib().dd_last_cuda_error().decode()
+
+
+def dd_plan_create(nchans: int, dt: float, f_top: float, df: float, nbits: int) -> int:
+    """-> opaque plan handle (int).  See include/dd.h."""
+    h = ctypes.c_void_p()
+    _check(lib().dd_plan_create(ctypes.byref(h), int(nchans), float(dt), float(f_top), float(df), int(nbits)),
+           "dd_plan_create")
+    return int(h.value)
+
+
+def dd_plan_destroy(plan: int) -> None:
+    _check(lib().dd_plan_destroy(plan), "dd_plan_destroy")
+
+
+def dd_set_dm_list(plan: int, dm_list: Sequence[float]) -> None:
+    dm = np.ascontiguousarray(dm_list, dtype=np.float64)
+    _check(lib().dd_set_dm_list(plan, dm.ctypes.data, int(dm.shape[0])), "dd_set_dm_list")
+
+
+def dd_get_max_delay(plan: int) -> int:
+    return _check(int(lib().dd_get_max_delay(plan)), "dd_get_max_delay")
+
+
+def dd_get_delay_table(plan: int, ndm: int, nchans: int) -> np.ndarray:
+    """-> int32 [ndm][nchans] (host)."""
+    out = np.empty((ndm, nchans), dtype=np.int32)
+    _check(lib().dd_get_delay_table(plan, out.ctypes.data), "dd_get_delay_table")
+    return out
+
+
+def dd_set_batch(plan: int, nbeams: int, in_beam_stride: int, out_beam_stride: int) -> None:
+    _check(lib().dd_set_batch(plan, int(nbeams), int(in_beam_stride), int(out_beam_stride)), "dd_set_batch")
+
+
+def dd_execute(plan: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbits: int, stream=None) -> None:
+    """Asynchronous; in_ptr/out_ptr are DEVICE buffers (tensors or addresses)."""
+    _check(lib().dd_execute(plan, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits),
+                            _stream(stream)), "dd_execute")
+
+
+def dd_execute_host(plan: int, nsamps: int, in_host, in_stride: int, out_host, out_nbits: int) -> None:
+    """Synchronous; in_host/out_host are HOST buffers (pinned tensors, numpy arrays or addresses)."""
+    _check(lib().dd_execute_host(plan, int(nsamps), _addr(in_host), int(in_stride), _addr(out_host), int(out_nbits)),
+           "dd_execute_host")
+
+
+def dd_get_launch_info(plan: int) -> dict:
+    info = np.zeros(8, dtype=np.int64)
+    _check(lib().dd_get_launch_info(plan, info.ctypes.data), "dd_get_launch_info")
+    keys = ("dm_block", "time_block", "chans_per_stage", "smem_bytes", "threads", "n_dm_blocks", "last_launches",
+            "variant")
+    return {k: int(v) for k, v in zip(keys, info)}
+
+
+def dd_int_add_peak(mode: int = 0, stream=None) -> float:
+    """Measured 32-bit integer additions per second on the current device (synchronises)."""
+    v = ctypes.c_double()
+    _check(lib().dd_int_add_peak(int(mode), ctypes.byref(v), _stream(stream)), "dd_int_add_peak")
+    return float(v.value)
+
+
+class Plan:
+    """Owns one dd_plan handle (context manager); argument marshalling only."""
+
+    def __init__(self, nchans: int, dt: float, f_top: float, df: float, nbits: int):
+        self.nchans, self.nbits = int(nchans), int(nbits)
+        self.ndm = 0
+        self.handle = dd_plan_create(nchans, dt, f_top, df, nbits)
+
+    def set_dm_list(self, dm_list) -> "Plan":
+        dd_set_dm_list(self.handle, dm_list)
+        self.ndm = len(dm_list)
+        return self
+
+    def set_batch(self, nbeams: int, in_beam_stride: int, out_beam_stride: int) -> "Plan":
+        dd_set_batch(self.handle, nbeams, in_beam_stride, out_beam_stride)
+        return self
+
+    @property
+    def max_delay(self) -> int:
+        return dd_get_max_delay(self.handle)
+
+    def delay_table(self) -> np.ndarray:
+        return dd_get_delay_table(self.handle, self.ndm, self.nchans)
+
+    def launch_info(self) -> dict:
+        return dd_get_launch_info(self.handle)
+
+    def execute(self, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream=None) -> None:
+        dd_execute(self.handle, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream)
+
+    def execute_host(self, nsamps, in_host, in_stride, out_host, out_nbits) -> None:
+        dd_execute_host(self.handle, nsamps, in_host, in_stride, out_host, out_nbits)
+
+    def close(self) -> None:
+        if self.handle:
+            dd_plan_destroy(self.handle)
+            self.handle = 0
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,473 @@
+// dd_api.cu -- the C ABI of include/dd.h: argument checking, table upload, kernel launch.
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include <cuda_runtime.h>
+
+#include "dd_kernels.cuh"
+#include "dd_plan.h"
+
+namespace dd {
+
+static thread_local std::string g_cuda_error;
+
+static dd_status cuda_fail(cudaError_t e, const char *what)
+{
+    g_cuda_error = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+    (void)cudaGetLastError();   // clear the sticky-less error state
+    return DD_ERR_CUDA;
+}
+
+// Device staging of dd_execute_host: the whole packed input plus two output slabs.
+struct HostStage {
+    uint8_t *d_in = nullptr;
+    size_t in_bytes = 0;
+    uint8_t *d_out[2] = {nullptr, nullptr};
+    size_t out_bytes = 0;
+    cudaStream_t copy_in = nullptr, compute = nullptr, copy_out[2] = {nullptr, nullptr};
+    cudaEvent_t in_ready = nullptr, done[2] = {nullptr, nullptr}, drained[2] = {nullptr, nullptr};
+    bool streams = false;
+};
+
+static void free_stage(HostStage *s)
+{
+    if (!s)
+        return;
+    cudaFree(s->d_in);
+    cudaFree(s->d_out[0]);
+    cudaFree(s->d_out[1]);
+    if (s->streams) {
+        cudaStreamDestroy(s->copy_in);
+        cudaStreamDestroy(s->compute);
+        for (int i = 0; i < 2; ++i) {
+            cudaStreamDestroy(s->copy_out[i]);
+            cudaEventDestroy(s->done[i]);
+            cudaEventDestroy(s->drained[i]);
+        }
+        cudaEventDestroy(s->in_ready);
+    }
+    delete s;
+}
+
+static void free_device_tables(dd_plan_s *p)
+{
+    if (p->d_span)
+        cudaFree(p->d_span);
+    if (p->d_rel)
+        cudaFree(p->d_rel);
+    p->d_span = p->d_rel = nullptr;
+    p->uploaded = false;
+}
+
+// Uploads span/rel tables to the current device.  DD_ERR_CUDA when there is no usable device.
+static dd_status upload_tables(dd_plan_s *p)
+{
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess)
+        return cuda_fail(e, "cudaGetDeviceCount");
+    if (ndev <= 0)
+        return cuda_fail(cudaErrorNoDevice, "cudaGetDeviceCount");
+    free_device_tables(p);
+    if ((e = cudaGetDevice(&p->device)) != cudaSuccess)
+        return cuda_fail(e, "cudaGetDevice");
+    const size_t span_bytes = p->span.size() * sizeof(SpanMeta), rel_bytes = p->rel.size() * sizeof(uint16_t);
+    if ((e = cudaMalloc(&p->d_span, span_bytes)) != cudaSuccess)
+        return cuda_fail(e, "cudaMalloc(span)");
+    if ((e = cudaMalloc(&p->d_rel, rel_bytes)) != cudaSuccess) {
+        free_device_tables(p);
+        return cuda_fail(e, "cudaMalloc(rel)");
+    }
+    if ((e = cudaMemcpy(p->d_span, p->span.data(), span_bytes, cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemcpy(p->d_rel, p->rel.data(), rel_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
+        free_device_tables(p);
+        return cuda_fail(e, "cudaMemcpy(tables)");
+    }
+    p->uploaded = true;
+    return DD_OK;
+}
+
+static int elem_size(int out_nbits)
+{
+    switch (out_nbits) {
+    case DD_OUT_F32:
+    case DD_OUT_U32:
+        return 4;
+    case DD_OUT_U16:
+        return 2;
+    }
+    return 0;
+}
+
+// Argument checks shared by dd_execute and dd_execute_host (pointer alignment is checked by the caller).
+static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_stride, int out_nbits)
+{
+    if (p->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    const int es = elem_size(out_nbits);
+    if (nsamps <= 0 || es == 0)
+        return DD_ERR_INVALID_ARG;
+    if (in_stride <= 0 || in_stride % 16 != 0)
+        return DD_ERR_ALIGNMENT;
+    // in_stride*8 >= (nsamps + max_delay)*nbits, without overflow
+    const int64_t need_bits_hi = (nsamps + p->max_delay);
+    if (need_bits_hi > (INT64_MAX / 8) || in_stride > INT64_MAX / 8 || in_stride * 8 < need_bits_hi * p->nbits)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    const int64_t vmax = (1 << p->nbits) - 1, top = static_cast<int64_t>(p->nchans) * vmax;
+    if ((out_nbits == DD_OUT_U16 && top > 65535) || (out_nbits == DD_OUT_F32 && top >= (1 << 24)))
+        return DD_ERR_OUT_RANGE;
+    if (nsamps > (INT64_MAX / 8) / p->ndm)
+        return DD_ERR_INVALID_ARG;
+    return DD_OK;
+}
+
+static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *in, int64_t in_stride, void *out,
+                                int out_nbits, int nbeams, int64_t in_beam_stride, int64_t out_beam_stride)
+{
+    KernelParams kp{};
+    kp.in = static_cast<const uint8_t *>(in);
+    kp.in_stride = in_stride;
+    kp.in_row_bytes = in_stride;
+    kp.in_beam_stride = in_beam_stride;
+    kp.out = static_cast<uint8_t *>(out);
+    kp.out_beam_stride = out_beam_stride;
+    kp.nsamps = nsamps;
+    kp.out_code = out_nbits;
+    const int es = elem_size(out_nbits);
+    const int vec_bytes = 4 * es;
+    kp.vec_ok = (nsamps % 4 == 0) && (reinterpret_cast<uintptr_t>(out) % vec_bytes == 0) &&
+                (out_beam_stride % vec_bytes == 0);
+    kp.nchans = p->nchans;
+    kp.ndm = p->ndm;
+    kp.nblk = p->nblk;
+    kp.ntiles = static_cast<int32_t>((nsamps + p->var.TB - 1) / p->var.TB);
+    kp.nbeams = nbeams;
+    kp.cc = p->cc;
+    kp.nchunks = (p->nchans + p->cc - 1) / p->cc;
+    kp.raw_slot = p->raw_slot;
+    kp.lane_slot = p->lane_slot;
+    kp.span = static_cast<const int2 *>(p->d_span);
+    kp.rel = static_cast<const uint16_t *>(p->d_rel);
+    return kp;
+}
+
+}  // namespace dd
+
+using namespace dd;
+
+extern "C" {
+
+dd_status dd_plan_create(dd_plan *plan, int nchans, double dt, double f_top, double df, int nbits)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    *plan = nullptr;
+    if (nchans <= 0 || !(dt > 0.0) || !std::isfinite(dt) || !(f_top > 0.0) || !std::isfinite(f_top) || !(df < 0.0) ||
+        !std::isfinite(df) || (nbits != 2 && nbits != 4 && nbits != 8))
+        return DD_ERR_INVALID_ARG;
+    if (!(f_top + static_cast<double>(nchans - 1) * df > 0.0))
+        return DD_ERR_INVALID_ARG;
+    dd_plan_s *p = new (std::nothrow) dd_plan_s();
+    if (!p)
+        return DD_ERR_NOMEM;
+    p->nchans = nchans;
+    p->dt = dt;
+    p->f_top = f_top;
+    p->df = df;
+    p->nbits = nbits;
+    *plan = p;
+    return DD_OK;
+}
+
+dd_status dd_plan_destroy(dd_plan plan)
+{
+    if (!plan)
+        return DD_OK;
+    free_device_tables(plan);
+    free_stage(plan->stage);
+    delete plan;
+    return DD_OK;
+}
+
+dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
+{
+    if (!plan || !dm_list)
+        return DD_ERR_NULL;
+    if (ndm <= 0)
+        return DD_ERR_INVALID_ARG;
+    for (int d = 0; d < ndm; ++d)
+        if (!std::isfinite(dm_list[d]) || dm_list[d] < 0.0)
+            return DD_ERR_INVALID_ARG;
+    // build into a scratch copy so that a failure leaves the plan unchanged
+    dd_plan_s scratch;
+    scratch.nchans = plan->nchans;
+    scratch.dt = plan->dt;
+    scratch.f_top = plan->f_top;
+    scratch.df = plan->df;
+    scratch.nbits = plan->nbits;
+    scratch.ndm = ndm;
+    try {
+        scratch.dm.assign(dm_list, dm_list + ndm);
+        dd_status st = compute_delay_table(&scratch);
+        if (st != DD_OK)
+            return st;
+        st = build_tiles(&scratch);
+        if (st != DD_OK)
+            return st;
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+    free_device_tables(plan);
+    plan->ndm = ndm;
+    plan->dm.swap(scratch.dm);
+    plan->delay.swap(scratch.delay);
+    plan->max_delay = scratch.max_delay;
+    plan->var = scratch.var;
+    plan->nblk = scratch.nblk;
+    plan->cc = scratch.cc;
+    plan->raw_slot = scratch.raw_slot;
+    plan->lane_slot = scratch.lane_slot;
+    plan->smem_bytes = scratch.smem_bytes;
+    plan->final32 = scratch.final32;
+    plan->span.swap(scratch.span);
+    plan->rel.swap(scratch.rel);
+    plan->last_launches = 0;
+    // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
+        dd_status st = upload_tables(plan);
+        if (st != DD_OK)
+            return st;
+    } else {
+        (void)cudaGetLastError();
+    }
+    return DD_OK;
+}
+
+dd_status dd_get_delay_table(dd_plan plan, int32_t *table)
+{
+    if (!plan || !table)
+        return DD_ERR_NULL;
+    if (plan->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    std::memcpy(table, plan->delay.data(), plan->delay.size() * sizeof(int32_t));
+    return DD_OK;
+}
+
+int64_t dd_get_max_delay(dd_plan plan)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (plan->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    return plan->max_delay;
+}
+
+dd_status dd_set_batch(dd_plan plan, int nbeams, int64_t in_beam_stride, int64_t out_beam_stride)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (nbeams <= 0 || in_beam_stride < 0 || out_beam_stride < 0)
+        return DD_ERR_INVALID_ARG;
+    if (nbeams > 1 && in_beam_stride % 16 != 0)
+        return DD_ERR_ALIGNMENT;
+    plan->nbeams = nbeams;
+    plan->in_beam_stride = nbeams > 1 ? in_beam_stride : 0;
+    plan->out_beam_stride = nbeams > 1 ? out_beam_stride : 0;
+    return DD_OK;
+}
+
+dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr, int out_nbits,
+                     void *stream)
+{
+    if (!plan || !in_ptr || !out_ptr)
+        return DD_ERR_NULL;
+    dd_status st = check_execute(plan, nsamps, in_stride, out_nbits);
+    if (st != DD_OK)
+        return st;
+    const int es = elem_size(out_nbits);
+    if (reinterpret_cast<uintptr_t>(in_ptr) % 16 != 0 || reinterpret_cast<uintptr_t>(out_ptr) % es != 0)
+        return DD_ERR_ALIGNMENT;
+    if (plan->nbeams > 1) {
+        if (plan->out_beam_stride % es != 0)
+            return DD_ERR_ALIGNMENT;
+        if (plan->in_beam_stride < static_cast<int64_t>(plan->nchans) * in_stride ||
+            plan->out_beam_stride < static_cast<int64_t>(plan->ndm) * nsamps * es)
+            return DD_ERR_STRIDE_TOO_SMALL;
+    }
+    if (!plan->uploaded) {
+        st = upload_tables(plan);
+        if (st != DD_OK)
+            return st;
+    }
+    const KernelParams kp = make_params(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, plan->nbeams,
+                                        plan->in_beam_stride, plan->out_beam_stride);
+    const cudaError_t e = launch_direct(plan, kp, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess)
+        return cuda_fail(e, "dd_execute launch");
+    plan->last_launches = 1;
+    return DD_OK;
+}
+
+dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int64_t in_stride, void *out_host,
+                          int out_nbits)
+{
+    if (!plan || !in_host || !out_host)
+        return DD_ERR_NULL;
+    dd_status st = check_execute(plan, nsamps, in_stride, out_nbits);
+    if (st != DD_OK)
+        return st;
+    const int es = elem_size(out_nbits);
+    if (!plan->uploaded) {
+        st = upload_tables(plan);
+        if (st != DD_OK)
+            return st;
+    }
+    const int nbeams = plan->nbeams;
+    const int64_t in_beam = nbeams > 1 ? plan->in_beam_stride : static_cast<int64_t>(plan->nchans) * in_stride;
+    const int64_t out_beam_host = nbeams > 1 ? plan->out_beam_stride : static_cast<int64_t>(plan->ndm) * nsamps * es;
+    if (nbeams > 1 && (in_beam < static_cast<int64_t>(plan->nchans) * in_stride ||
+                       out_beam_host < static_cast<int64_t>(plan->ndm) * nsamps * es))
+        return DD_ERR_STRIDE_TOO_SMALL;
+
+    // Time slabs: the input slab of output samples [s0, s0+len) is rows [s0, s0+len+max_delay); the slab
+    // length is a multiple of the tile so that slab starts stay 16-byte aligned in the packed rows.
+    const int64_t TB = plan->var.TB;
+    int64_t slab = ((int64_t(1) << 17) + TB - 1) / TB * TB;
+    if (slab > (nsamps + TB - 1) / TB * TB)
+        slab = (nsamps + TB - 1) / TB * TB;
+    const int64_t nslabs = (nsamps + slab - 1) / slab;
+    const size_t in_bytes = static_cast<size_t>(in_beam) * nbeams;
+    const size_t out_slab_bytes = static_cast<size_t>(nbeams) * plan->ndm * slab * es;
+
+    cudaError_t e;
+    if (!plan->stage)
+        plan->stage = new (std::nothrow) HostStage();
+    HostStage *S = plan->stage;
+    if (!S)
+        return DD_ERR_NOMEM;
+    if (!S->streams) {
+        if ((e = cudaStreamCreateWithFlags(&S->copy_in, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&S->compute, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&S->copy_out[0], cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&S->copy_out[1], cudaStreamNonBlocking)) != cudaSuccess)
+            return cuda_fail(e, "cudaStreamCreate");
+        cudaEventCreateWithFlags(&S->in_ready, cudaEventDisableTiming);
+        for (int i = 0; i < 2; ++i) {
+            cudaEventCreateWithFlags(&S->done[i], cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&S->drained[i], cudaEventDisableTiming);
+        }
+        S->streams = true;
+    }
+    if (S->in_bytes < in_bytes) {
+        cudaFree(S->d_in);
+        S->d_in = nullptr;
+        S->in_bytes = 0;
+        if ((e = cudaMalloc(&S->d_in, in_bytes)) != cudaSuccess)
+            return cuda_fail(e, "cudaMalloc(stage in)");
+        S->in_bytes = in_bytes;
+    }
+    if (S->out_bytes < out_slab_bytes) {
+        for (int i = 0; i < 2; ++i) {
+            cudaFree(S->d_out[i]);
+            S->d_out[i] = nullptr;
+        }
+        S->out_bytes = 0;
+        for (int i = 0; i < 2; ++i)
+            if ((e = cudaMalloc(&S->d_out[i], out_slab_bytes)) != cudaSuccess)
+                return cuda_fail(e, "cudaMalloc(stage out)");
+        S->out_bytes = out_slab_bytes;
+    }
+
+    // input: one H2D copy of the whole packed filterbank (it is 5-30x smaller than the output)
+    if ((e = cudaMemcpyAsync(S->d_in, in_host, in_bytes, cudaMemcpyHostToDevice, S->copy_in)) != cudaSuccess)
+        return cuda_fail(e, "cudaMemcpyAsync(in)");
+    cudaEventRecord(S->in_ready, S->copy_in);
+    cudaStreamWaitEvent(S->compute, S->in_ready, 0);
+
+    int64_t launches = 0;
+    for (int64_t k = 0; k < nslabs; ++k) {
+        const int b = static_cast<int>(k & 1);
+        const int64_t s0 = k * slab, len = (s0 + slab <= nsamps) ? slab : nsamps - s0;
+        if (k >= 2)
+            cudaStreamWaitEvent(S->compute, S->drained[b], 0);   // slab buffer b has been copied out
+        const uint8_t *in_slab = S->d_in + (s0 * plan->nbits) / 8;
+        KernelParams kp = make_params(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, nbeams, in_beam,
+                                      static_cast<int64_t>(plan->ndm) * len * es);
+        kp.in_row_bytes = in_stride - (s0 * plan->nbits) / 8;
+        if ((e = launch_direct(plan, kp, S->compute)) != cudaSuccess)
+            return cuda_fail(e, "dd_execute_host launch");
+        ++launches;
+        cudaEventRecord(S->done[b], S->compute);
+        cudaStreamWaitEvent(S->copy_out[b], S->done[b], 0);
+        for (int beam = 0; beam < nbeams; ++beam) {
+            uint8_t *dst = static_cast<uint8_t *>(out_host) + static_cast<size_t>(beam) * out_beam_host + s0 * es;
+            const uint8_t *src = S->d_out[b] + static_cast<size_t>(beam) * plan->ndm * len * es;
+            if ((e = cudaMemcpy2DAsync(dst, static_cast<size_t>(nsamps) * es, src, static_cast<size_t>(len) * es,
+                                       static_cast<size_t>(len) * es, plan->ndm, cudaMemcpyDeviceToHost,
+                                       S->copy_out[b])) != cudaSuccess)
+                return cuda_fail(e, "cudaMemcpy2DAsync(out)");
+        }
+        cudaEventRecord(S->drained[b], S->copy_out[b]);
+    }
+    for (int i = 0; i < 2; ++i)
+        if ((e = cudaStreamSynchronize(S->copy_out[i])) != cudaSuccess)
+            return cuda_fail(e, "cudaStreamSynchronize(out)");
+    if ((e = cudaStreamSynchronize(S->compute)) != cudaSuccess)
+        return cuda_fail(e, "cudaStreamSynchronize(compute)");
+    plan->last_launches = launches;
+    return DD_OK;
+}
+
+dd_status dd_get_launch_info(dd_plan plan, int64_t *info)
+{
+    if (!plan || !info)
+        return DD_ERR_NULL;
+    if (plan->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    info[0] = plan->var.DB;
+    info[1] = plan->var.TB;
+    info[2] = plan->cc;
+    info[3] = plan->smem_bytes;
+    info[4] = plan->var.threads;
+    info[5] = plan->nblk;
+    info[6] = plan->last_launches;
+    info[7] = plan->var.id;
+    return DD_OK;
+}
+
+dd_status dd_int_add_peak(int mode, double *adds_per_sec, void *stream)
+{
+    if (!adds_per_sec)
+        return DD_ERR_NULL;
+    if (mode != 0 && mode != 1)
+        return DD_ERR_INVALID_ARG;
+    const cudaError_t e = int_add_peak(mode, adds_per_sec, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess)
+        return cuda_fail(e, "dd_int_add_peak");
+    return DD_OK;
+}
+
+const char *dd_strerror(dd_status s)
+{
+    switch (s) {
+    case DD_OK: return "success";
+    case DD_ERR_NULL: return "a required pointer is NULL";
+    case DD_ERR_INVALID_ARG: return "invalid argument";
+    case DD_ERR_NO_DM_LIST: return "no DM list set on this plan";
+    case DD_ERR_ALIGNMENT: return "pointer or stride not aligned as required";
+    case DD_ERR_STRIDE_TOO_SMALL: return "input rows (or a beam stride) too short for nsamps + max_delay";
+    case DD_ERR_OUT_RANGE: return "sums do not fit the requested output type exactly";
+    case DD_ERR_DELAY_OVERFLOW: return "a delay does not fit int32";
+    case DD_ERR_SMEM: return "delay spread of a DM block does not fit shared memory";
+    case DD_ERR_CUDA: return "CUDA error (see dd_last_cuda_error)";
+    case DD_ERR_NOMEM: return "host allocation failed";
+    }
+    return "unknown status";
+}
+
+const char *dd_last_cuda_error(void) { return g_cuda_error.c_str(); }
+
+}  // extern "C"

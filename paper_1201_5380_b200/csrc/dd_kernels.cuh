@@ -1,0 +1,34 @@
+// dd_kernels.cuh -- launch interface between the C ABI (dd_api.cu) and the CUDA kernels (dd_kernels.cu).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "dd_plan.h"
+
+namespace dd {
+
+// Everything one launch of the direct-dedispersion kernel needs (passed by value as a kernel parameter).
+struct KernelParams {
+    const uint8_t *in;        // device: in[beam][c][byte]
+    int64_t in_stride;        // bytes between channel rows
+    int64_t in_row_bytes;     // bytes readable from the start of a row (<= in_stride; less for a time slab)
+    int64_t in_beam_stride;   // bytes between beams
+    uint8_t *out;             // device: out[beam][d][t]
+    int64_t out_beam_stride;  // bytes between beams
+    int64_t nsamps;           // output samples per DM trial
+    int32_t out_code;         // DD_OUT_F32 / DD_OUT_U16 / DD_OUT_U32
+    int32_t vec_ok;           // rows and base pointers allow 4-sample vector stores
+    int32_t nchans, ndm, nblk, ntiles, nbeams;
+    int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
+    int32_t raw_slot, lane_slot;
+    const int2 *span;         // [nblk][nchans] {start, nbytes}
+    const uint16_t *rel;      // [nblk][nchans][DB]
+};
+
+// Enqueues the kernel variant chosen by the plan.  Returns the cudaError_t of the launch.
+cudaError_t launch_direct(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+
+// Integer-add throughput microbenchmark (roofline denominator).  Synchronises `stream`.
+cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream);
+
+}  // namespace dd

@@ -1,0 +1,127 @@
+// dd_plan.cpp -- host-side planning: the delay table (double precision) and the tile metadata.
+#include "dd_plan.h"
+
+#include <algorithm>
+#include <cmath>
+#include <limits>
+
+namespace dd {
+
+// Dispersion constant k_DM in MHz^2 pc^-1 cm^3 s.
+static const double kDispersionConstant = 4.148808e3;
+
+// eq. 4-5 in double precision on the host; "rounded to the nearest integer"
+// is taken as floor(x + 0.5) (reading R1; x >= 0 for a descending band).
+dd_status compute_delay_table(dd_plan_s *p)
+{
+    const int nchans = p->nchans, ndm = p->ndm;
+    std::vector<double> band(nchans);   // f_c^-2 - f_top^-2, shared by all DM trials
+    const double inv_top2 = 1.0 / (p->f_top * p->f_top);
+    for (int c = 0; c < nchans; ++c) {
+        const double f = p->f_top + static_cast<double>(c) * p->df;
+        band[c] = 1.0 / (f * f) - inv_top2;
+    }
+    std::vector<int32_t> table(static_cast<size_t>(ndm) * nchans);
+    int64_t maxd = 0;
+    for (int d = 0; d < ndm; ++d) {
+        const double scale = kDispersionConstant * p->dm[d];
+        int32_t *row = table.data() + static_cast<size_t>(d) * nchans;
+        for (int c = 0; c < nchans; ++c) {
+            const double x = scale * band[c] / p->dt;
+            const double r = std::floor(x + 0.5);
+            if (!(r >= 0.0) || r > static_cast<double>(std::numeric_limits<int32_t>::max() - 1))
+                return DD_ERR_DELAY_OVERFLOW;
+            row[c] = static_cast<int32_t>(r);
+            maxd = std::max<int64_t>(maxd, row[c]);
+        }
+    }
+    p->delay.swap(table);
+    p->max_delay = maxd;
+    return DD_OK;
+}
+
+static inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
+{
+    int64_t bytes = 128;                                                       // mbarriers
+    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->var.DB * 2, 128);      // rel stages (uint16)
+    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);        // packed stages
+    if (p->nbits < 8)
+        bytes += align_up(static_cast<int64_t>(cc) * p->lane_slot, 128);       // unpacked lanes
+    return bytes;
+}
+
+// The kernel variants compiled into the library (dd_kernels.cu instantiates one kernel per id).
+static const Variant kVariants[] = {
+    /* id  DB  TB   threads tail max_cc */
+    {1, 32, 640, 256, 4, 32},
+};
+
+dd_status build_tiles(dd_plan_s *p)
+{
+    const int nchans = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    const int64_t vmax = (1 << nbits) - 1;
+    p->final32 = static_cast<int64_t>(nchans) * vmax > 65535;
+    const int A = 128 / nbits;   // samples per 16 packed bytes: bulk-copy granularity
+
+    for (const Variant &v : kVariants) {
+        p->var = v;
+        const int DB = v.DB;
+        const int nblk = (ndm + DB - 1) / DB;
+        std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans);
+        std::vector<uint16_t> rel(static_cast<size_t>(nblk) * nchans * DB);
+        int64_t max_bytes = 0;
+        bool ok = true;
+        for (int b = 0; b < nblk && ok; ++b) {
+            for (int c = 0; c < nchans && ok; ++c) {
+                int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0;
+                for (int i = 0; i < DB; ++i) {
+                    const int d = std::min(b * DB + i, ndm - 1);   // pad the last block with its last DM
+                    const int32_t dl = p->delay[static_cast<size_t>(d) * nchans + c];
+                    dmin = std::min(dmin, dl);
+                    dmax = std::max(dmax, dl);
+                }
+                const int32_t start = dmin / A * A;
+                const int64_t need = static_cast<int64_t>(v.TB) + (dmax - start) + v.tail;
+                const int64_t nbytes = align_up(need, A) * nbits / 8;
+                if (dmax - start > 65535 || nbytes > (1 << 19)) {
+                    ok = false;
+                    break;
+                }
+                SpanMeta &m = span[static_cast<size_t>(b) * nchans + c];
+                m.start = start;
+                m.nbytes = static_cast<int32_t>(nbytes);
+                max_bytes = std::max(max_bytes, nbytes);
+                uint16_t *r = rel.data() + (static_cast<size_t>(b) * nchans + c) * DB;
+                for (int i = 0; i < DB; ++i) {
+                    const int d = std::min(b * DB + i, ndm - 1);
+                    r[i] = static_cast<uint16_t>(p->delay[static_cast<size_t>(d) * nchans + c] - start);
+                }
+            }
+        }
+        if (!ok)
+            continue;
+        p->raw_slot = static_cast<int>(max_bytes);
+        p->lane_slot = static_cast<int>(max_bytes * 8 / nbits);
+        int cc = v.max_cc;
+        while (cc > 1 && cc / 2 >= nchans)
+            cc /= 2;
+        for (; cc >= 1; cc /= 2) {
+            const int64_t tx = static_cast<int64_t>(cc) * p->raw_slot + static_cast<int64_t>(cc) * DB * 2;
+            if (smem_layout_bytes(p, cc) <= kMaxDynSmem && tx < (1 << 20))
+                break;
+        }
+        if (cc < 1)
+            continue;
+        p->cc = cc;
+        p->nblk = nblk;
+        p->smem_bytes = smem_layout_bytes(p, cc);
+        p->span.swap(span);
+        p->rel.swap(rel);
+        return DD_OK;
+    }
+    return DD_ERR_SMEM;
+}
+
+}  // namespace dd

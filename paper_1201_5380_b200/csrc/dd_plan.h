@@ -1,0 +1,82 @@
+// dd_plan.h -- internal plan object and host-side planning for libdd_b200 (not part of the C ABI).
+//
+// Host planning follows PAPER.md:62-67 (eq. 4-5: delay table in double precision) and PAPER.md:115
+// (the staged span of a thread block must carry "additional time samples ... to allow for
+// differences in delay across a block"): for every (DM block, channel) we record where the staged
+// span starts and how many bytes it holds, and for every (DM, channel) the offset of that DM's
+// window inside the span.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/dd.h"
+
+namespace dd {
+
+// One CUDA kernel variant: compile-time tile shape, selected at dd_set_dm_list time.
+struct Variant {
+    int id;        // reported by dd_get_launch_info[7]
+    int DB;        // DM trials per CTA
+    int TB;        // output samples per CTA
+    int threads;   // threads per CTA
+    int tail;      // extra samples a thread may read past TB + offset (over-fetch of the aligned loads)
+    int max_cc;    // most channels per pipeline stage the kernel supports
+};
+
+struct SpanMeta {   // per (DM block, channel); mirrored on the device as int2
+    int32_t start;  // first staged sample relative to the tile's first output sample; multiple of 128/nbits
+    int32_t nbytes; // packed bytes to stage (multiple of 16)
+};
+
+struct HostStage;   // device staging for dd_execute_host (dd_api.cu)
+
+}  // namespace dd
+
+struct dd_plan_s {
+    // observing parameters
+    int nchans = 0;
+    double dt = 0, f_top = 0, df = 0;
+    int nbits = 0;
+    // DM trials and the delay table (eq. 4-5)
+    int ndm = 0;
+    std::vector<double> dm;
+    std::vector<int32_t> delay;   // [ndm][nchans]
+    int64_t max_delay = -1;
+    // batching
+    int nbeams = 1;
+    int64_t in_beam_stride = 0, out_beam_stride = 0;
+    // tiling
+    dd::Variant var{};
+    int nblk = 0;          // DM blocks
+    int cc = 0;            // channels per pipeline stage
+    int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
+    int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
+    int64_t smem_bytes = 0;
+    bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
+    std::vector<dd::SpanMeta> span;   // [nblk][nchans]
+    std::vector<uint16_t> rel;        // [nblk][nchans][DB]: delay - span start, per DM slot of the block
+    // device copies
+    int device = -1;
+    bool uploaded = false;
+    void *d_span = nullptr;
+    void *d_rel = nullptr;
+    int64_t last_launches = 0;
+    dd::HostStage *stage = nullptr;
+};
+
+namespace dd {
+
+// Evaluates eq. 4-5 in double for every (d, c); fills plan->delay / max_delay.  DD_ERR_DELAY_OVERFLOW
+// if a delay does not fit int32.
+dd_status compute_delay_table(dd_plan_s *p);
+
+// Chooses the kernel variant and builds span/rel metadata.  DD_ERR_SMEM if no tiling fits.
+dd_status build_tiles(dd_plan_s *p);
+
+// Shared-memory bytes the kernel needs for `cc` channels per stage (must match the kernel's carve-up).
+int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
+
+constexpr int64_t kMaxDynSmem = 227 * 1024;   // usable shared memory per CTA on sm_100a
+
+}  // namespace dd

@@ -1,0 +1,133 @@
+"""C-ABI boundary without a GPU: the library loads, exports what include/dd.h declares, validates
+arguments, and its host-side delay table equals the oracle's on all five configs.  No compute calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import dd_workloads as W
+import oracle
+import paper_1201_5380_b200 as dd
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dd_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = dd.lib()
+    declared = _declared_symbols()
+    assert declared == sorted(dd.EXPORTED_SYMBOLS)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_strerror_and_status_codes():
+    assert dd.dd_strerror(0) == "success"
+    for s in range(-10, 0):
+        assert dd.dd_strerror(s) not in ("", "unknown status")
+    assert dd.dd_strerror(-99) == "unknown status"
+
+
+@pytest.mark.parametrize("args", [
+    (0, 64e-6, 1500.0, -1.0, 8), (64, 0.0, 1500.0, -1.0, 8), (64, 64e-6, -5.0, -1.0, 8),
+    (64, 64e-6, 1500.0, 1.0, 8), (64, 64e-6, 1500.0, 0.0, 8), (64, 64e-6, 1500.0, -1.0, 3),
+    (64, 64e-6, 1500.0, -1.0, 16), (2000, 64e-6, 1500.0, -1.0, 8), (64, float("nan"), 1500.0, -1.0, 8),
+])
+def test_plan_create_rejects_bad_arguments(args):
+    with pytest.raises(dd.DDError) as e:
+        dd.dd_plan_create(*args)
+    assert e.value.status == -2
+
+
+def test_null_pointers():
+    L = dd.lib()
+    assert L.dd_plan_create(None, 64, 64e-6, 1500.0, -1.0, 8) == -1
+    assert L.dd_plan_destroy(None) == 0
+    assert L.dd_set_dm_list(None, None, 1) == -1
+    assert L.dd_get_max_delay(None) == -1
+
+
+def test_dm_list_validation_leaves_plan_unchanged():
+    p = dd.Plan(64, 64e-6, 1500.0, -1.0, 8)
+    with pytest.raises(dd.DDError) as e:
+        p.set_dm_list([])  # ndm <= 0
+    assert e.value.status in (-2,)
+    with pytest.raises(dd.DDError) as e:
+        dd.dd_get_max_delay(p.handle)
+    assert e.value.status == -3
+    p.set_dm_list([0.0, 10.0, 20.0])
+    before = p.delay_table().copy()
+    for bad in ([1.0, -1.0], [float("inf")], [float("nan"), 1.0]):
+        with pytest.raises(dd.DDError) as e:
+            dd.dd_set_dm_list(p.handle, bad)
+        assert e.value.status == -2
+    assert np.array_equal(dd.dd_get_delay_table(p.handle, 3, 64), before)
+    # a delay that does not fit int32
+    with pytest.raises(dd.DDError) as e:
+        dd.dd_set_dm_list(p.handle, [1e12])
+    assert e.value.status == -7
+    assert np.array_equal(dd.dd_get_delay_table(p.handle, 3, 64), before)
+    p.close()
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_host_delay_table_equals_oracle(idx):
+    cfg = W.CONFIGS[idx]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(cfg.dm_list())
+        tab = p.delay_table()
+        ref = oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list())
+        assert tab.dtype == np.int32 and tab.shape == ref.shape
+        assert np.array_equal(tab.astype(np.int64), ref)
+        assert p.max_delay == int(ref.max())
+        info = p.launch_info()
+        assert info["smem_bytes"] <= 227 * 1024 and info["n_dm_blocks"] * info["dm_block"] >= cfg.ndm
+
+
+def test_unsorted_and_repeated_dm_list():
+    cfg = W.CONFIGS[2]
+    rng = np.random.default_rng(3)
+    dms = rng.permutation(np.concatenate([cfg.dm_list()[::40], [0.0, 0.0, 17.25]]))
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        assert np.array_equal(p.delay_table().astype(np.int64),
+                              oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms))
+
+
+def test_spread_too_large_for_shared_memory_is_an_error():
+    # DM trials 0 and 1e6 in one block: the staged span could never fit on chip
+    with dd.Plan(1024, 64e-6, 400.0, -0.05, 8) as p:
+        with pytest.raises(dd.DDError) as e:
+            p.set_dm_list([0.0, 1.0e6])
+        assert e.value.status == -8
+
+
+def test_execute_argument_checks_need_no_gpu():
+    cfg = W.CONFIGS[4]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        L, h = dd.lib(), p.handle
+        assert L.dd_execute(h, 100, 16, 1024, 16, 32, None) == -3          # no DM list
+        p.set_dm_list([0.0, 5.0])
+        md = p.max_delay
+        good_stride = ((100 + md) * 4 // 8 + 15) // 16 * 16
+        assert L.dd_execute(h, 100, None, good_stride, 16, 32, None) == -1
+        assert L.dd_execute(h, 0, 16, good_stride, 16, 32, None) == -2
+        assert L.dd_execute(h, 100, 16, good_stride, 16, 8, None) == -2       # unknown out_nbits
+        assert L.dd_execute(h, 100, 16, good_stride + 8, 16, 32, None) == -4  # stride not multiple of 16
+        assert L.dd_execute(h, 100, 24, good_stride, 16, 32, None) == -4      # in_ptr not 16-aligned
+        assert L.dd_execute(h, 100, 16, good_stride, 18, 32, None) == -4      # out_ptr not element aligned
+        assert L.dd_execute(h, 100, 16, 16, 16, 32, None) == -5               # rows too short
+    with dd.Plan(8192, 64e-6, 1500.0, -0.01, 4) as p:                        # 8192*15 > 65535
+        p.set_dm_list([0.0])
+        assert dd.lib().dd_execute(p.handle, 100, 16, 4096, 16, 16, None) == -6
+    with dd.Plan(4096, 64e-6, 1500.0, -0.01, 8) as p:
+        assert dd.lib().dd_set_batch(p.handle, 0, 0, 0) == -2
+        assert dd.lib().dd_set_batch(p.handle, 2, 24, 0) == -4
+        assert dd.lib().dd_set_batch(p.handle, 2, 4096 * 64, 1 << 20) == 0

@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, bit-exact.
+
+Small cases compare every output element; the full BASELINE.json sizes compare sampled outputs that the
+oracle computes one by one (plus whole DM rows for the bench config).  All inputs are seeded and
+synthetic (dd_workloads); no expected value comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+import torch
+
+import dd_workloads as W
+import oracle
+import paper_1201_5380_b200 as dd
+
+pytestmark = pytest.mark.gpu
+
+_TORCH_OUT = {"f32": torch.float32, "u32": torch.int32, "u16": torch.int16}
+_NP_VIEW = {"f32": np.float32, "u32": np.uint32, "u16": np.uint16}
+
+
+def _oracle_table(cfg, dms=None):
+    return oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list() if dms is None else dms)
+
+
+def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, beams=None):
+    """Run dd_execute on device-resident packed input [nbeams][nchans][stride]; returns a numpy array
+    [nbeams][ndm][nsamps] of the output type."""
+    out_kind = out_kind or cfg.out
+    nsamps = nsamps or cfg.nsamps
+    nbeams = packed_dev.shape[0]
+    ndm = len(dms)
+    out = torch.full((nbeams, ndm, nsamps), -1, dtype=_TORCH_OUT[out_kind], device="cuda")
+    code = {"f32": 32, "u32": -32, "u16": 16}[out_kind]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        if nbeams > 1:
+            p.set_batch(nbeams, packed_dev.stride(0), out.stride(0) * out.element_size())
+        p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert p.launch_info()["last_launches"] == 1
+    return out.cpu().numpy().view(_NP_VIEW[out_kind])
+
+
+def _full_compare(cfg, dms=None, out_kinds=None, nsamps=None):
+    dms = cfg.dm_list() if dms is None else np.asarray(dms, dtype=np.float64)
+    nsamps = nsamps or cfg.nsamps
+    tab = _oracle_table(cfg, dms)
+    # pulses follow the config's own DM list (their tracks come from the oracle's table)
+    ptab = _oracle_table(cfg)
+    pulses = W.make_pulses(cfg, lambda idx: ptab[idx])
+    max_delay = int(max(tab.max(), ptab.max() if pulses is not None else 0))
+    packed, stride = W.gen_packed(cfg, max_delay, pulses)
+    packed_dev = packed.cuda()
+    for kind in (out_kinds or [cfg.out]):
+        got = _gpu_transform(cfg, packed_dev, stride, dms, kind, nsamps)
+        for b in range(cfg.nbeams):
+            ref = oracle.cast_out(oracle.dedisperse(packed[b].numpy(), cfg.nbits, nsamps, tab), kind)
+            assert got[b].shape == ref.shape
+            bad = np.nonzero(got[b] != ref)
+            assert bad[0].size == 0, (f"{cfg.name} {kind} beam {b}: {bad[0].size} mismatches, first at "
+                                      f"d={bad[0][0]} t={bad[1][0]} got={got[b][bad[0][0], bad[1][0]]} "
+                                      f"ref={ref[bad[0][0], bad[1][0]]}")
+
+
+# ------------------------------------------------------------------ small cases, every element compared
+def test_cfg1_full_u32_and_f32():
+    _full_compare(W.CONFIGS[1], out_kinds=["u32", "f32", "u16"])
+
+
+def test_cfg2_reduced_several_tiles_ragged_tail():
+    # 1024 channels, 2-bit, 70 DMs (3 DM blocks, last ragged), 3 time tiles + ragged tail of 77 samples
+    _full_compare(W.CONFIGS[2].reduced(nsamps=3 * 640 + 77, ndm=70))
+
+
+def test_cfg2_high_dm_end():
+    # the last DMs of config 2 (largest delays and spreads), nsamps not a multiple of 4
+    cfg = W.CONFIGS[2].reduced(nsamps=1501, ndm=40)
+    _full_compare(cfg, dms=W.CONFIGS[2].dm_list()[-40:])
+
+
+def test_cfg3_reduced_8bit_4096_channels():
+    _full_compare(W.CONFIGS[3].reduced(nsamps=1300, ndm=33))
+
+
+def test_cfg3_high_dm_end_large_spread():
+    cfg = W.CONFIGS[3].reduced(nsamps=700, ndm=32)
+    _full_compare(cfg, dms=W.CONFIGS[3].dm_list()[-32:])
+
+
+def test_cfg4_reduced_4bit_u16():
+    _full_compare(W.CONFIGS[4].reduced(nsamps=2000, ndm=65), out_kinds=["u16", "u32", "f32"])
+
+
+def test_cfg5_reduced_batch_of_beams():
+    _full_compare(W.CONFIGS[5].reduced(nsamps=1000, ndm=40, nbeams=3))
+
+
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_odd_shapes(nbits):
+    # channel count not a multiple of the stage size, one DM, tiny nsamps, more channels than a flush interval
+    base = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    for nchans, ndm, nsamps in ((1, 1, 1), (37, 5, 13), (300, 33, 641), (1024, 2, 5)):
+        _full_compare(base.reduced(nsamps=nsamps, ndm=ndm, nchans=nchans), out_kinds=["u32"])
+
+
+def test_unsorted_dm_list():
+    cfg = W.CONFIGS[2].reduced(nsamps=900, ndm=48, nchans=256)
+    rng = np.random.default_rng(11)
+    dms = rng.permutation(W.CONFIGS[2].dm_list()[:200])[:48]
+    _full_compare(cfg, dms=dms, out_kinds=["f32"])
+
+
+def test_many_channels_need_32bit_accumulators():
+    # 2-bit, 24000 channels: 24000*3 > 65535 -> the 32-bit accumulator instantiation
+    cfg = W.Config(name="wide32", index=2, nchans=24000, f_top=1500.0, df=-0.01, dt=64e-6, nbits=2, nsamps=333,
+                   ndm=3, dm_max=2.0, out="u32", dist="uniform", seed=99)
+    _full_compare(cfg)
+    cfg4 = W.Config(name="wide32-4", index=4, nchans=5000, f_top=1500.0, df=-0.05, dt=64e-6, nbits=4, nsamps=200,
+                    ndm=2, dm_max=1.0, out="u32", dist="uniform", seed=98)
+    _full_compare(cfg4)
+
+
+def test_execute_host_matches_oracle():
+    cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    ref = oracle.cast_out(oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab), "u16")
+    out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.int16).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 16)
+    assert np.array_equal(out.numpy().view(np.uint16), ref)
+
+
+def test_device_generation_equals_host_generation():
+    cfg = W.CONFIGS[2].reduced(nsamps=5000, ndm=8, nchans=64)
+    a, s1 = W.gen_packed(cfg, 300)
+    b, s2 = W.gen_packed(cfg, 300, device="cuda")
+    assert s1 == s2 and torch.equal(a, b.cpu())
+    cfg = W.CONFIGS[3].reduced(nsamps=3000, ndm=8, nchans=32)
+    a, _ = W.gen_packed(cfg, 100)
+    b, _ = W.gen_packed(cfg, 100, device="cuda")
+    assert torch.equal(a, b.cpu())
+
+
+# ------------------------------------------------------- full BASELINE.json sizes, sampled by the oracle
+def _sample_points(cfg, tile, n, seed):
+    rng = np.random.default_rng(seed)
+    d = rng.integers(0, cfg.ndm, n)
+    t = rng.integers(0, cfg.nsamps, n)
+    # structured points: first/last DM, tile edges, last samples
+    edge_t = [0, 1, tile - 1, tile, tile + 1, cfg.nsamps - tile - 1, cfg.nsamps - 2, cfg.nsamps - 1]
+    edge_d = [0, 1, 31, 32, 33, cfg.ndm - 33, cfg.ndm - 2, cfg.ndm - 1]
+    dd_, tt = np.meshgrid(np.clip(edge_d, 0, cfg.ndm - 1), np.clip(edge_t, 0, cfg.nsamps - 1))
+    return np.concatenate([d, dd_.ravel()]), np.concatenate([t, tt.ravel()])
+
+
+def _full_size_sampled(cfg, npoints, whole_rows=0):
+    tab = _oracle_table(cfg)
+    pulses = W.make_pulses(cfg, lambda idx: tab[idx])
+    max_delay = int(tab.max())
+    packed_dev, stride = W.gen_packed(cfg, max_delay, pulses, device="cuda", chan_chunk=16)
+    got_dev_out = None
+    nbeams, ndm, nsamps = cfg.nbeams, cfg.ndm, cfg.nsamps
+    out = torch.full((nbeams, ndm, nsamps), -1, dtype=_TORCH_OUT[cfg.out], device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(cfg.dm_list())
+        tile = p.launch_info()["time_block"]
+        if nbeams > 1:
+            p.set_batch(nbeams, packed_dev.stride(0), out.stride(0) * out.element_size())
+        p.execute(nsamps, packed_dev, stride, out, cfg.out_nbits, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+    for b in sorted({0, nbeams - 1}):
+        d_idx, t_idx = _sample_points(cfg, tile, npoints, seed=cfg.seed + b)
+        ref = oracle.dedisperse_points(
+            lambda c, t: W.values_at(cfg, b, c, t, pulses).numpy(), tab, d_idx, t_idx)
+        got = out[b][torch.as_tensor(d_idx, device="cuda"), torch.as_tensor(t_idx, device="cuda")].cpu().numpy()
+        got = got.view(_NP_VIEW[cfg.out]).astype(np.int64)
+        bad = np.nonzero(got != ref)[0]
+        assert bad.size == 0, (f"{cfg.name} beam {b}: {bad.size}/{ref.size} sampled outputs differ; first "
+                               f"d={d_idx[bad[0]]} t={t_idx[bad[0]]} got={got[bad[0]]} ref={ref[bad[0]]}")
+    if whole_rows:
+        rows = np.unique(np.concatenate([np.linspace(0, ndm - 1, whole_rows).astype(np.int64), [ndm - 1]]))
+        packed_host = packed_dev[0].cpu().numpy()
+        ref_rows = oracle.cast_out(oracle.dedisperse(packed_host, cfg.nbits, nsamps, tab[rows]), cfg.out)
+        got_rows = out[0][torch.as_tensor(rows, device="cuda")].cpu().numpy().view(_NP_VIEW[cfg.out])
+        assert np.array_equal(got_rows, ref_rows)
+    # every element was written (the buffer was pre-filled with -1 / NaN-like patterns)
+    if cfg.out == "f32":
+        assert bool((out >= 0).all())
+    del out, packed_dev
+    torch.cuda.empty_cache()
+
+
+def test_cfg2_full_size_bench_configuration():
+    _full_size_sampled(W.CONFIGS[2], npoints=4000, whole_rows=12)
+
+
+def test_cfg3_full_size_sampled():
+    _full_size_sampled(W.CONFIGS[3], npoints=1500)
+
+
+def test_cfg4_full_size_sampled():
+    _full_size_sampled(W.CONFIGS[4], npoints=3000)
+
+
+def test_cfg5_full_size_sampled_batch():
+    _full_size_sampled(W.CONFIGS[5], npoints=2000)
