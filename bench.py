@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- dedispersion throughput (DM-trial samples/s) and fraction of the binding roofline on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path (stage -> unpack -> shifted accumulate -> convert/store,
+DESIGN.md section 2) over one synthetic batch: one dd_execute of BASELINE.json configs[1]
+(1024 channels, 2-bit, 1200 DM trials, 2^19 output samples) with the input resident in HBM.
+Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank dedisperses its own beam of the same
+shape, no data-path collective (weak scaling); value = total units / slowest rank's time.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "dedispersion throughput (DM-trial samples/s)"
+UNIT = "DM-trial samples/s"
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs (NVML)."""
+
+    REASONS = {
+        0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+        0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join(timeout=2)
+
+    def summary(self) -> dict:
+        return {"sm_mhz": (statistics.median(self.samples) if self.samples else None),
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------ helpers
+def algorithmic_counts(cfg, max_delay: int, nbeams: int) -> dict:
+    """Algorithmic work of one step: channel-adds, input bytes once + output bytes once."""
+    esize = {"f32": 4, "u32": 4, "u16": 2}[cfg.out]
+    units = nbeams * cfg.ndm * cfg.nsamps
+    in_bytes = nbeams * cfg.nchans * ((cfg.nsamps + max_delay) * cfg.nbits // 8)
+    return {"units": units, "adds": units * cfg.nchans, "bytes": in_bytes + units * esize,
+            "in_bytes": in_bytes, "out_bytes": units * esize}
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return dict(json.load(open(path)), source="measured (MEASURED_PEAKS.json)")
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def committed_traffic(workload: str, variant: int):
+    """dram bytes per launch from the committed ncu capture (profiles/dram_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    best = None
+    for line in open(path):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 3 and f[0] == workload and f[1] == str(variant):
+            best = float(f[2])
+    return best
+
+
+def cpu_sample(cfg, nsamps: int, dm_step: int):
+    """The bounded oracle sample: first `nsamps` output samples, every dm_step-th DM trial, all channels."""
+    import dd_workloads as W
+    import oracle
+    sub = W.CONFIGS[cfg.index].reduced(nsamps=nsamps)         # same band, same DM list
+    dms = sub.dm_list()[::dm_step]
+    tab = oracle.delay_table(sub.nchans, sub.dt, sub.f_top, sub.df, dms)
+    packed, stride = W.gen_packed(sub, int(tab.max()))
+    desc = (f"{cfg.name}: all {cfg.nchans} channels, first {nsamps} output samples, every {dm_step}th DM trial "
+            f"({len(dms)} of {cfg.ndm}), 1 beam")
+    return packed[0].numpy(), tab, nsamps, len(dms), desc
+
+
+def time_oracle(packed, tab, nbits, nsamps, reps: int = 1):
+    import oracle
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.dedisperse(packed, nbits, nsamps, tab, nthreads=0)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return best
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def run_reference(args) -> None:
+    import dd_workloads as W
+    import oracle
+    from paper_1201_5380_b200 import multi
+    rank, _, world = multi.env_rank()
+    if rank != 0:
+        return
+    cfg = W.CONFIGS[args.config]
+    packed, tab, nsamps, ndm, desc = cpu_sample(cfg, 1 << 15, 16)
+    cores = oracle.threads(0)
+    for _ in range(args.warmup):
+        oracle.dedisperse(packed, cfg.nbits, nsamps, tab)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.dedisperse(packed, cfg.nbits, nsamps, tab)
+    el = time.perf_counter() - t0
+    ms = el / args.steps * 1e3
+    value = ndm * nsamps / (ms * 1e-3)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg.name, "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + " per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args) -> None:
+    import torch
+
+    import dd_workloads as W
+    import paper_1201_5380_b200 as dd
+    from paper_1201_5380_b200 import multi
+
+    rank, local_rank, world = multi.env_rank()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    multi.init_process_group("nccl")
+    cfg = W.CONFIGS[args.config]
+    nbeams = cfg.nbeams
+    stream = torch.cuda.Stream()
+
+    plan = dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits).set_dm_list(cfg.dm_list())
+    max_delay = plan.max_delay
+    # synthetic input generated in HBM; rank r uses beam index r (+ the config's own beams) as generator stream
+    beams = [rank * nbeams + b for b in range(nbeams)]
+    tab = plan.delay_table() if cfg.npulses else None
+    pulses = W.make_pulses(cfg, lambda idx: tab[idx]) if cfg.npulses else None
+    packed, stride = W.gen_packed(cfg, max_delay, pulses, device="cuda", beams=beams, chan_chunk=16)
+    tdtype = {"f32": torch.float32, "u32": torch.int32, "u16": torch.int16}[cfg.out]
+    out = torch.empty((nbeams, cfg.ndm, cfg.nsamps), dtype=tdtype, device="cuda")
+    if nbeams > 1:
+        plan.set_batch(nbeams, packed.stride(0), out.stride(0) * out.element_size())
+    counts = algorithmic_counts(cfg, max_delay, nbeams)
+    info = plan.launch_info()
+
+    def step():
+        plan.execute(cfg.nsamps, packed, stride, out, cfg.out_nbits, stream)
+
+    torch.cuda.synchronize()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, barrier + sync on both sides
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    multi.barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(local_rank) as clk:
+        wall0 = time.perf_counter()
+        with torch.cuda.stream(stream):
+            ev[0].record(stream)
+            for k in range(args.steps):
+                step()
+                ev[k + 1].record(stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - wall0
+    multi.barrier()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    ms_step_rank = total_ms / args.steps
+    value, ms_step = multi.job_throughput(counts["units"], ms_step_rank)
+    kernel_ms = statistics.mean(per_launch)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region (all ranks)
+    e2e = None
+    if not args.no_e2e:
+        h_in = packed.cpu().pin_memory()
+        h_out = torch.empty((nbeams, cfg.ndm, cfg.nsamps), dtype=tdtype).pin_memory()
+        plan.execute_host(cfg.nsamps, h_in, stride, h_out, cfg.out_nbits)        # warm-up (allocates staging)
+        reps = 3
+        multi.barrier()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            plan.execute_host(cfg.nsamps, h_in, stride, h_out, cfg.out_nbits)
+        e2e_ms_rank = (time.perf_counter() - t0) / reps * 1e3
+        e2e_value, e2e_ms = multi.job_throughput(counts["units"], e2e_ms_rank)
+        ok = bool(torch.equal(h_out.cuda(), out))
+        e2e = {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms,
+               "h2d_bytes_per_step": int(h_in.numel() * h_in.element_size()),
+               "d2h_bytes_per_step": int(h_out.numel() * h_out.element_size()),
+               "kernels_per_step": plan.launch_info()["last_launches"], "matches_device_path": ok,
+               "api": "dd_execute_host, pinned host buffers, host<->device copies inside the timed region"}
+        del h_in, h_out
+
+    if rank != 0:
+        multi.barrier()
+        return
+
+    # ---- roofline of the (only) kernel: ALU-bound; HBM shown beside it
+    peak_ind = dd.dd_int_add_peak(0, stream)
+    peak_3in = dd.dd_int_add_peak(1, stream)
+    alu_peak = max(peak_ind, peak_3in)
+    peaks = measured_peaks()
+    achieved_adds = counts["adds"] / (kernel_ms * 1e-3)
+    achieved_gbs = counts["bytes"] / (kernel_ms * 1e-3) / 1e9
+    roofline = {
+        "bound": "alu", "achieved": achieved_adds / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
+        "frac": achieved_adds / alu_peak,
+        "traffic": committed_traffic(cfg.name, info["variant"]),
+        "kernel": f"dd_direct_v{info['variant']}<{cfg.nbits}>", "kernel_ms": kernel_ms,
+        "kernel_ms_p5_p50_p95": [float(np.percentile(per_launch, q)) for q in (5, 50, 95)],
+        "algorithmic_adds_per_launch": counts["adds"], "algorithmic_bytes_per_launch": counts["bytes"],
+        "peak_source": "measured in this run by dd_int_add_peak (32-bit integer additions/s, all SMs): "
+                       f"2-input chains {peak_ind / 1e12:.2f}, 3-input (IADD3) {peak_3in / 1e12:.2f} Tadd/s",
+        "hbm": {"achieved": achieved_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                "frac": achieved_gbs / peaks.get("hbm_gbs", float("nan")), "peak_source": peaks["source"]},
+    }
+
+    # ---- the oracle timed beside it on this box's host cores (bounded sample; a baseline, not the target)
+    cpu_baseline = None
+    if not args.no_cpu and world == 1:
+        import oracle
+        cpacked, ctab, cns, cndm, desc = cpu_sample(cfg, 1 << 17, 4)
+        el = time_oracle(cpacked, ctab, cfg.nbits, cns)
+        cpu_baseline = {"value": cndm * cns / el, "unit": UNIT, "cores": oracle.threads(0), "kind": "oracle",
+                        "sample": desc, "seconds": el}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg.name, "nchans": cfg.nchans, "nbits": cfg.nbits, "ndm": cfg.ndm,
+                   "nsamps": cfg.nsamps, "nbeams_per_gpu": nbeams, "out": cfg.out, "max_delay": max_delay,
+                   "tile": f"{info['dm_block']} DMs x {info['time_block']} samples, {info['threads']} threads, "
+                           f"{info['smem_bytes']} B smem",
+                   "l2": f"no flush: each step streams {counts['bytes'] / 1e9:.2f} GB (input {counts['in_bytes'] / 1e6:.0f} MB "
+                         f"+ output {counts['out_bytes'] / 1e9:.2f} GB) > 126 MB L2",
+                   "parallelism": f"beam-per-gpu x{world}" if world > 1 else "single gpu"},
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": args.steps,
+        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "wall_s_timed_region": wall,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        multi.barrier()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -132,6 +132,13 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
                           void *out_host, int out_nbits);
 
 /*
+ * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
+ *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel.
+ * Takes effect at the next dd_set_dm_list (which returns DD_ERR_SMEM if that variant cannot serve the plan).
+ */
+dd_status dd_set_kernel_variant(dd_plan plan, int variant);
+
+/*
  * dd_get_launch_info -- how the plan tiles the problem (for benchmarks and tests).  Host only.
  *   info  HOST out, 8 int64: [0] DMs per CTA (DB), [1] output samples per CTA (TB), [2] channels per
  *         pipeline stage, [3] dynamic shared memory bytes per CTA, [4] threads per CTA, [5] number of DM

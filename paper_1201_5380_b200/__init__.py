@@ -20,7 +20,7 @@ __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_strerror", "dd_last_cuda_error", "Plan",
+    "dd_set_kernel_variant", "dd_strerror", "dd_last_cuda_error", "Plan",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
 
@@ -30,7 +30,7 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_strerror", "dd_last_cuda_error",
+    "dd_set_kernel_variant", "dd_strerror", "dd_last_cuda_error",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -76,13 +76,14 @@ def lib() -> ctypes.CDLL:
         L.dd_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
         L.dd_get_launch_info.argtypes = [vp, vp]
+        L.dd_set_kernel_variant.argtypes = [vp, i32]
         L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
         L.dd_strerror.argtypes = [i32]
         L.dd_strerror.restype = ctypes.c_char_p
         L.dd_last_cuda_error.argtypes = []
         L.dd_last_cuda_error.restype = ctypes.c_char_p
         for name in ("dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_set_batch",
-                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak"):
+                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak", "dd_set_kernel_variant"):
             getattr(L, name).restype = i32
         _LIB = L
     return _LIB
@@ -167,6 +168,11 @@ def dd_execute_host(plan: int, nsamps: int, in_host, in_stride: int, out_host, o
            "dd_execute_host")
 
 
+def dd_set_kernel_variant(plan: int, variant: int) -> None:
+    """0 = automatic; takes effect at the next dd_set_dm_list."""
+    _check(lib().dd_set_kernel_variant(plan, int(variant)), "dd_set_kernel_variant")
+
+
 def dd_get_launch_info(plan: int) -> dict:
     info = np.zeros(8, dtype=np.int64)
     _check(lib().dd_get_launch_info(plan, info.ctypes.data), "dd_get_launch_info")
@@ -185,10 +191,12 @@ def dd_int_add_peak(mode: int = 0, stream=None) -> float:
 class Plan:
     """Owns one dd_plan handle (context manager); argument marshalling only."""
 
-    def __init__(self, nchans: int, dt: float, f_top: float, df: float, nbits: int):
+    def __init__(self, nchans: int, dt: float, f_top: float, df: float, nbits: int, variant: int = 0):
         self.nchans, self.nbits = int(nchans), int(nbits)
         self.ndm = 0
         self.handle = dd_plan_create(nchans, dt, f_top, df, nbits)
+        if variant:
+            dd_set_kernel_variant(self.handle, variant)
 
     def set_dm_list(self, dm_list) -> "Plan":
         dd_set_dm_list(self.handle, dm_list)

@@ -14,8 +14,8 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdd_b200.so")
-SOURCES = ["dd_api.cu", "dd_kernels.cu", "dd_plan.cpp"]
-HEADERS = ["dd_plan.h", "dd_kernels.cuh", os.path.join("..", "..", "include", "dd.h")]
+SOURCES = ["dd_api.cu", "dd_kernels.cu", "dd_kernel_v1.cu", "dd_kernel_v2.cu", "dd_plan.cpp"]
+HEADERS = ["dd_plan.h", "dd_kernels.cuh", "dd_common.cuh", os.path.join("..", "..", "include", "dd.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -73,7 +73,7 @@ static dd_status upload_tables(dd_plan_s *p)
     free_device_tables(p);
     if ((e = cudaGetDevice(&p->device)) != cudaSuccess)
         return cuda_fail(e, "cudaGetDevice");
-    const size_t span_bytes = p->span.size() * sizeof(SpanMeta), rel_bytes = p->rel.size() * sizeof(uint16_t);
+    const size_t span_bytes = p->span.size() * sizeof(SpanMeta), rel_bytes = p->rel.size();
     if ((e = cudaMalloc(&p->d_span, span_bytes)) != cudaSuccess)
         return cuda_fail(e, "cudaMalloc(span)");
     if ((e = cudaMalloc(&p->d_rel, rel_bytes)) != cudaSuccess) {
@@ -149,7 +149,7 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     kp.raw_slot = p->raw_slot;
     kp.lane_slot = p->lane_slot;
     kp.span = static_cast<const int2 *>(p->d_span);
-    kp.rel = static_cast<const uint16_t *>(p->d_rel);
+    kp.rel = p->d_rel;
     return kp;
 }
 
@@ -208,6 +208,7 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
     scratch.df = plan->df;
     scratch.nbits = plan->nbits;
     scratch.ndm = ndm;
+    scratch.force_variant = plan->force_variant;
     try {
         scratch.dm.assign(dm_list, dm_list + ndm);
         dd_status st = compute_delay_table(&scratch);
@@ -418,6 +419,16 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     if ((e = cudaStreamSynchronize(S->compute)) != cudaSuccess)
         return cuda_fail(e, "cudaStreamSynchronize(compute)");
     plan->last_launches = launches;
+    return DD_OK;
+}
+
+dd_status dd_set_kernel_variant(dd_plan plan, int variant)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (variant < 0 || variant > 2)
+        return DD_ERR_INVALID_ARG;
+    plan->force_variant = variant;
     return DD_OK;
 }
 

@@ -22,11 +22,14 @@ struct KernelParams {
     int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
     int32_t raw_slot, lane_slot;
     const int2 *span;         // [nblk][nchans] {start, nbytes}
-    const uint16_t *rel;      // [nblk][nchans][DB]
+    const void *rel;          // [nblk][nchans][DB] entries of var.rel_bytes
 };
 
 // Enqueues the kernel variant chosen by the plan.  Returns the cudaError_t of the launch.
 cudaError_t launch_direct(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+
+cudaError_t launch_variant1(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+cudaError_t launch_variant2(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 
 // Integer-add throughput microbenchmark (roofline denominator).  Synchronises `stream`.
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream);

@@ -44,18 +44,20 @@ static inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * 
 
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 {
-    int64_t bytes = 128;                                                       // mbarriers
-    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->var.DB * 2, 128);      // rel stages (uint16)
-    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);        // packed stages
-    if (p->nbits < 8)
-        bytes += align_up(static_cast<int64_t>(cc) * p->lane_slot, 128);       // unpacked lanes
+    const Variant &v = p->var;
+    int64_t bytes = 128;                                                              // mbarriers
+    bytes += 2 * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);        // offset-table stages
+    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);               // packed stages
+    if (v.lane_bits != p->nbits)                                                      // unpacked lanes
+        bytes += v.lane_stages * align_up(static_cast<int64_t>(cc) * p->lane_slot, 128);
     return bytes;
 }
 
-// The kernel variants compiled into the library (dd_kernels.cu instantiates one kernel per id).
+// The kernel variants compiled into the library (dd_kernels.cu), in order of preference.
 static const Variant kVariants[] = {
-    /* id  DB  TB   threads tail max_cc */
-    {1, 32, 640, 256, 4, 32},
+    /* id  DB   TB   thr tail rel lane stg  cc candidates      nbits     wide */
+    {2, 32, 1280, 512, 8, 4, 4, 2, {40, 20, 10, 5}, 1 << 2, false},                  // 2-bit, nibble lanes
+    {1, 32, 640, 256, 4, 2, 8, 1, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), true},
 };
 
 dd_status build_tiles(dd_plan_s *p)
@@ -66,11 +68,16 @@ dd_status build_tiles(dd_plan_s *p)
     const int A = 128 / nbits;   // samples per 16 packed bytes: bulk-copy granularity
 
     for (const Variant &v : kVariants) {
+        if (!(v.nbits_mask & (1 << nbits)) || (p->final32 && !v.wide_ok))
+            continue;
+        if (p->force_variant && v.id != p->force_variant)
+            continue;
         p->var = v;
         const int DB = v.DB;
         const int nblk = (ndm + DB - 1) / DB;
+        const int64_t rel_limit = v.rel_bytes == 2 ? 65535 : (int64_t(1) << 28);
         std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans);
-        std::vector<uint16_t> rel(static_cast<size_t>(nblk) * nchans * DB);
+        std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchans * DB * v.rel_bytes);
         int64_t max_bytes = 0;
         bool ok = true;
         for (int b = 0; b < nblk && ok; ++b) {
@@ -85,7 +92,7 @@ dd_status build_tiles(dd_plan_s *p)
                 const int32_t start = dmin / A * A;
                 const int64_t need = static_cast<int64_t>(v.TB) + (dmax - start) + v.tail;
                 const int64_t nbytes = align_up(need, A) * nbits / 8;
-                if (dmax - start > 65535 || nbytes > (1 << 19)) {
+                if (dmax - start > rel_limit || nbytes > (1 << 19)) {
                     ok = false;
                     break;
                 }
@@ -93,24 +100,31 @@ dd_status build_tiles(dd_plan_s *p)
                 m.start = start;
                 m.nbytes = static_cast<int32_t>(nbytes);
                 max_bytes = std::max(max_bytes, nbytes);
-                uint16_t *r = rel.data() + (static_cast<size_t>(b) * nchans + c) * DB;
+                const size_t base = (static_cast<size_t>(b) * nchans + c) * DB;
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);
-                    r[i] = static_cast<uint16_t>(p->delay[static_cast<size_t>(d) * nchans + c] - start);
+                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nchans + c] - start);
+                    if (v.rel_bytes == 2)
+                        reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
+                    else
+                        reinterpret_cast<uint32_t *>(rel.data())[base + i] = off * 4u;
                 }
             }
         }
         if (!ok)
             continue;
         p->raw_slot = static_cast<int>(max_bytes);
-        p->lane_slot = static_cast<int>(max_bytes * 8 / nbits);
-        int cc = v.max_cc;
-        while (cc > 1 && cc / 2 >= nchans)
-            cc /= 2;
-        for (; cc >= 1; cc /= 2) {
-            const int64_t tx = static_cast<int64_t>(cc) * p->raw_slot + static_cast<int64_t>(cc) * DB * 2;
-            if (smem_layout_bytes(p, cc) <= kMaxDynSmem && tx < (1 << 20))
+        p->lane_slot = static_cast<int>(max_bytes * v.lane_bits / nbits);
+        int cc = 0;
+        for (int k = 0; k < 4 && v.cc[k] > 0; ++k) {
+            const int cand = v.cc[k];
+            if (k + 1 < 4 && v.cc[k + 1] > 0 && v.cc[k + 1] >= nchans)
+                continue;   // a smaller stage already covers every channel
+            const int64_t tx = static_cast<int64_t>(cand) * p->raw_slot + static_cast<int64_t>(cand) * DB * v.rel_bytes;
+            if (smem_layout_bytes(p, cand) <= kMaxDynSmem && tx < (1 << 20)) {
+                cc = cand;
                 break;
+            }
         }
         if (cc < 1)
             continue;

@@ -16,12 +16,17 @@ namespace dd {
 
 // One CUDA kernel variant: compile-time tile shape, selected at dd_set_dm_list time.
 struct Variant {
-    int id;        // reported by dd_get_launch_info[7]
-    int DB;        // DM trials per CTA
-    int TB;        // output samples per CTA
-    int threads;   // threads per CTA
-    int tail;      // extra samples a thread may read past TB + offset (over-fetch of the aligned loads)
-    int max_cc;    // most channels per pipeline stage the kernel supports
+    int id;           // reported by dd_get_launch_info[7]
+    int DB;           // DM trials per CTA
+    int TB;           // output samples per CTA
+    int threads;      // threads per CTA
+    int tail;         // extra samples a thread may read past TB + offset (over-fetch of the aligned loads)
+    int rel_bytes;    // bytes per offset-table entry: 2 = sample offset (uint16), 4 = 4 * sample offset (uint32)
+    int lane_bits;    // bits per sample of the unpacked lane buffer in shared memory
+    int lane_stages;  // lane buffers (1 = single, 2 = double-buffered)
+    int cc[4];        // candidate channels-per-stage, largest first (0 = end)
+    int nbits_mask;   // input widths served (bit n set = nbits n)
+    bool wide_ok;     // can accumulate sums that need more than 16 bits
 };
 
 struct SpanMeta {   // per (DM block, channel); mirrored on the device as int2
@@ -48,6 +53,7 @@ struct dd_plan_s {
     int64_t in_beam_stride = 0, out_beam_stride = 0;
     // tiling
     dd::Variant var{};
+    int force_variant = 0; // 0 = automatic; otherwise only this variant id is considered (dd_set_kernel_variant)
     int nblk = 0;          // DM blocks
     int cc = 0;            // channels per pipeline stage
     int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
@@ -55,7 +61,7 @@ struct dd_plan_s {
     int64_t smem_bytes = 0;
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
     std::vector<dd::SpanMeta> span;   // [nblk][nchans]
-    std::vector<uint16_t> rel;        // [nblk][nchans][DB]: delay - span start, per DM slot of the block
+    std::vector<uint8_t> rel;         // [nblk][nchans][DB] entries of var.rel_bytes: delay - span start per DM slot
     // device copies
     int device = -1;
     bool uploaded = false;

@@ -22,7 +22,7 @@ def _oracle_table(cfg, dms=None):
     return oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list() if dms is None else dms)
 
 
-def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, beams=None):
+def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, variant=0):
     """Run dd_execute on device-resident packed input [nbeams][nchans][stride]; returns a numpy array
     [nbeams][ndm][nsamps] of the output type."""
     out_kind = out_kind or cfg.out
@@ -31,17 +31,18 @@ def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, bea
     ndm = len(dms)
     out = torch.full((nbeams, ndm, nsamps), -1, dtype=_TORCH_OUT[out_kind], device="cuda")
     code = {"f32": 32, "u32": -32, "u16": 16}[out_kind]
-    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=variant) as p:
         p.set_dm_list(dms)
         if nbeams > 1:
             p.set_batch(nbeams, packed_dev.stride(0), out.stride(0) * out.element_size())
         p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
         torch.cuda.synchronize()
-        assert p.launch_info()["last_launches"] == 1
+        info = p.launch_info()
+        assert info["last_launches"] == 1 and (variant == 0 or info["variant"] == variant)
     return out.cpu().numpy().view(_NP_VIEW[out_kind])
 
 
-def _full_compare(cfg, dms=None, out_kinds=None, nsamps=None):
+def _full_compare(cfg, dms=None, out_kinds=None, nsamps=None, variant=0):
     dms = cfg.dm_list() if dms is None else np.asarray(dms, dtype=np.float64)
     nsamps = nsamps or cfg.nsamps
     tab = _oracle_table(cfg, dms)
@@ -52,7 +53,7 @@ def _full_compare(cfg, dms=None, out_kinds=None, nsamps=None):
     packed, stride = W.gen_packed(cfg, max_delay, pulses)
     packed_dev = packed.cuda()
     for kind in (out_kinds or [cfg.out]):
-        got = _gpu_transform(cfg, packed_dev, stride, dms, kind, nsamps)
+        got = _gpu_transform(cfg, packed_dev, stride, dms, kind, nsamps, variant)
         for b in range(cfg.nbeams):
             ref = oracle.cast_out(oracle.dedisperse(packed[b].numpy(), cfg.nbits, nsamps, tab), kind)
             assert got[b].shape == ref.shape
@@ -67,15 +68,23 @@ def test_cfg1_full_u32_and_f32():
     _full_compare(W.CONFIGS[1], out_kinds=["u32", "f32", "u16"])
 
 
-def test_cfg2_reduced_several_tiles_ragged_tail():
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_cfg2_reduced_several_tiles_ragged_tail(variant):
     # 1024 channels, 2-bit, 70 DMs (3 DM blocks, last ragged), 3 time tiles + ragged tail of 77 samples
-    _full_compare(W.CONFIGS[2].reduced(nsamps=3 * 640 + 77, ndm=70))
+    _full_compare(W.CONFIGS[2].reduced(nsamps=3 * 1280 + 77, ndm=70), variant=variant)
 
 
-def test_cfg2_high_dm_end():
+def test_variant2_channel_counts_around_group_and_flush_boundaries():
+    # nchans not a multiple of 5 (group), of 40 (stage), beyond 85 (8-bit flush) and 17*5*k boundaries
+    for nchans in (1, 4, 5, 6, 39, 41, 84, 85, 86, 171, 1023):
+        _full_compare(W.CONFIGS[2].reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=2)
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_cfg2_high_dm_end(variant):
     # the last DMs of config 2 (largest delays and spreads), nsamps not a multiple of 4
     cfg = W.CONFIGS[2].reduced(nsamps=1501, ndm=40)
-    _full_compare(cfg, dms=W.CONFIGS[2].dm_list()[-40:])
+    _full_compare(cfg, dms=W.CONFIGS[2].dm_list()[-40:], out_kinds=["f32", "u16"], variant=variant)
 
 
 def test_cfg3_reduced_8bit_4096_channels():
