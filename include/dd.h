@@ -148,9 +148,13 @@ dd_status dd_get_launch_info(dd_plan plan, int64_t *info);
 
 /*
  * dd_int_add_peak -- measures this GPU's 32-bit integer-add throughput (the ALU roofline denominator
- * of DESIGN.md section 6) with a register-resident microbenchmark on all SMs.
- *   mode          0: independent chains of 2-input adds; 1: 3-input adds (two additions per IADD3).
- *   adds_per_sec  HOST out: additions per second (adds counted, not instructions).
+ * of DESIGN.md section 6) with a register-resident microbenchmark on all SMs.  Additions are counted, not
+ * instructions, and the chains are cross-coupled so that the compiler cannot fold two additions into one.
+ *   mode          0: 2-input adds (the compiler spreads them over both integer pipes);
+ *                 1: 3-input adds (IADD3: two additions per instruction, ALU pipe only);
+ *                 2: IADD3 interleaved 1:1 with multiply-add by a run-time 1 (IMAD on the FMA pipe): both
+ *                    pipes busy, three additions per instruction pair -- the highest rate of the three.
+ *   adds_per_sec  HOST out: additions per second.
  *   stream        cudaStream_t.  Synchronises.
  */
 dd_status dd_int_add_peak(int mode, double *adds_per_sec, void *stream);

@@ -57,7 +57,9 @@ static void free_device_tables(dd_plan_s *p)
         cudaFree(p->d_span);
     if (p->d_rel)
         cudaFree(p->d_rel);
-    p->d_span = p->d_rel = nullptr;
+    if (p->d_zero)
+        cudaFree(p->d_zero);
+    p->d_span = p->d_rel = p->d_zero = nullptr;
     p->uploaded = false;
 }
 
@@ -79,6 +81,13 @@ static dd_status upload_tables(dd_plan_s *p)
     if ((e = cudaMalloc(&p->d_rel, rel_bytes)) != cudaSuccess) {
         free_device_tables(p);
         return cuda_fail(e, "cudaMalloc(rel)");
+    }
+    if (p->var.pad_chunks) {   // the all-zero span staged for padded channels
+        if ((e = cudaMalloc(&p->d_zero, p->raw_slot)) != cudaSuccess ||
+            (e = cudaMemset(p->d_zero, 0, p->raw_slot)) != cudaSuccess) {
+            free_device_tables(p);
+            return cuda_fail(e, "cudaMalloc(zero)");
+        }
     }
     if ((e = cudaMemcpy(p->d_span, p->span.data(), span_bytes, cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(p->d_rel, p->rel.data(), rel_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
@@ -148,6 +157,9 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     kp.nchunks = (p->nchans + p->cc - 1) / p->cc;
     kp.raw_slot = p->raw_slot;
     kp.lane_slot = p->lane_slot;
+    kp.nstages = p->nstages;
+    kp.nchans_pad = p->nchans_pad;
+    kp.zero = static_cast<const uint8_t *>(p->d_zero);
     kp.span = static_cast<const int2 *>(p->d_span);
     kp.rel = p->d_rel;
     return kp;
@@ -186,6 +198,8 @@ dd_status dd_plan_destroy(dd_plan plan)
     if (!plan)
         return DD_OK;
     free_device_tables(plan);
+    if (plan->d_work)
+        cudaFree(plan->d_work);
     free_stage(plan->stage);
     delete plan;
     return DD_OK;
@@ -228,6 +242,9 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
     plan->var = scratch.var;
     plan->nblk = scratch.nblk;
     plan->cc = scratch.cc;
+    plan->nchans_pad = scratch.nchans_pad;
+    plan->nstages = scratch.nstages;
+    plan->max_span_end = scratch.max_span_end;
     plan->raw_slot = scratch.raw_slot;
     plan->lane_slot = scratch.lane_slot;
     plan->smem_bytes = scratch.smem_bytes;
@@ -308,7 +325,7 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
     const cudaError_t e = launch_direct(plan, kp, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess)
         return cuda_fail(e, "dd_execute launch");
-    plan->last_launches = 1;
+    plan->last_launches = launches_per_execute(plan);
     return DD_OK;
 }
 
@@ -400,7 +417,7 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
         kp.in_row_bytes = in_stride - (s0 * plan->nbits) / 8;
         if ((e = launch_direct(plan, kp, S->compute)) != cudaSuccess)
             return cuda_fail(e, "dd_execute_host launch");
-        ++launches;
+        launches += launches_per_execute(plan);
         cudaEventRecord(S->done[b], S->compute);
         cudaStreamWaitEvent(S->copy_out[b], S->done[b], 0);
         for (int beam = 0; beam < nbeams; ++beam) {
@@ -426,7 +443,7 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)
         return DD_ERR_NULL;
-    if (variant < 0 || variant > 2)
+    if (variant < 0 || variant > 3)
         return DD_ERR_INVALID_ARG;
     plan->force_variant = variant;
     return DD_OK;
@@ -453,7 +470,7 @@ dd_status dd_int_add_peak(int mode, double *adds_per_sec, void *stream)
 {
     if (!adds_per_sec)
         return DD_ERR_NULL;
-    if (mode != 0 && mode != 1)
+    if (mode < 0 || mode > 2)
         return DD_ERR_INVALID_ARG;
     const cudaError_t e = int_add_peak(mode, adds_per_sec, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess)

@@ -5,46 +5,64 @@ namespace dd {
 namespace {
 
 // ------------------------------------------------------------------------------------------ ALU peak probe
-// mode 0: 16 independent chains of 2-input adds; mode 1: each step adds two values (ptxas: one IADD3).
+// Register-resident chains r += q, q += r (cross-coupled, so that no two additions can be folded into one
+// multiply-add by the compiler).  Additions are counted, not instructions.
+//   mode 0: 2-input adds, ptxas picks the pipe (SASS: IADD3 on the ALU pipe and IMAD.IADD on the FMA pipe)
+//   mode 1: 3-input adds (SASS: IADD3, two additions per instruction, ALU pipe only)
+//   mode 2: 3-input adds interleaved 1:1 with multiply-adds by a run-time 1 (IADD3 + IMAD: both pipes,
+//           three additions per instruction pair) -- the highest integer-add rate the SM sustains
 template <int MODE>
-__global__ void __launch_bounds__(256) int_add_probe(uint32_t *sink, uint32_t x, uint32_t y, int iters)
+__global__ void __launch_bounds__(512) int_add_probe(uint32_t *sink, uint32_t x, uint32_t y, uint32_t one, int iters)
 {
-    uint32_t a[16];
+    constexpr int NCH = 8;
+    uint32_t r[NCH], q[NCH];
 #pragma unroll
-    for (int i = 0; i < 16; ++i)
-        a[i] = threadIdx.x + i;
+    for (int i = 0; i < NCH; ++i) {
+        r[i] = threadIdx.x * 7u + i;
+        q[i] = threadIdx.x * 3u + 5u * i;
+    }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int rep = 0; rep < 8; ++rep) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                if (MODE == 0)
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(a[i]) : "r"(x));
-                else
-                    asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(a[i]) : "r"(x), "r"(y));
+            for (int i = 0; i < NCH; ++i) {
+                if (MODE == 0) {
+                    asm volatile("add.u32 %0, %0, %1;" : "+r"(r[i]) : "r"(q[i]));
+                    asm volatile("add.u32 %0, %0, %1;" : "+r"(q[i]) : "r"(r[i]));
+                } else if (MODE == 1) {
+                    asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(r[i]) : "r"(q[i]), "r"(x));
+                    asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(q[i]) : "r"(r[i]), "r"(y));
+                } else {
+                    asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(r[i]) : "r"(q[i]), "r"(x));
+                    asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(q[i]) : "r"(r[i]), "r"(one));
+                }
             }
         }
     }
     uint32_t s = 0;
 #pragma unroll
-    for (int i = 0; i < 16; ++i)
-        s ^= a[i];
+    for (int i = 0; i < NCH; ++i)
+        s ^= r[i] ^ q[i];
     if (s == 0x12345678u)
         sink[0] = s;
 }
 
 }  // namespace
 
-cudaError_t launch_direct(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
+cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
 {
     switch (plan->var.id) {
     case 1:
         return launch_variant1(plan, kp, stream);
     case 2:
         return launch_variant2(plan, kp, stream);
+    case 3:
+        return launch_variant3(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }
+
+int launches_per_execute(const dd_plan_s *plan) { return plan->var.bitplane ? 2 : 1; }
 
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
 {
@@ -62,14 +80,16 @@ cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
     cudaEvent_t ev0, ev1;
     cudaEventCreate(&ev0);
     cudaEventCreate(&ev1);
-    const int iters = 4096, blocks = sms * 8, threads = 256;
+    const int iters = 2048, blocks = sms * 4, threads = 512;
     float best_ms = 1e30f;
     for (int rep = 0; rep < 5; ++rep) {
         cudaEventRecord(ev0, stream);
         if (mode == 0)
-            int_add_probe<0><<<blocks, threads, 0, stream>>>(sink, 3u, 5u, iters);
+            int_add_probe<0><<<blocks, threads, 0, stream>>>(sink, 3u, 5u, 1u, iters);
+        else if (mode == 1)
+            int_add_probe<1><<<blocks, threads, 0, stream>>>(sink, 3u, 5u, 1u, iters);
         else
-            int_add_probe<1><<<blocks, threads, 0, stream>>>(sink, 3u, 5u, iters);
+            int_add_probe<2><<<blocks, threads, 0, stream>>>(sink, 3u, 5u, 1u, iters);
         cudaEventRecord(ev1, stream);
         e = cudaEventSynchronize(ev1);
         if (e != cudaSuccess)
@@ -84,7 +104,8 @@ cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
     cudaFree(sink);
     if (e != cudaSuccess)
         return e;
-    const double adds = static_cast<double>(blocks) * threads * iters * 8.0 * 16.0 * (mode == 0 ? 1.0 : 2.0);
+    const double adds_per_step = (mode == 0) ? 2.0 : (mode == 1 ? 4.0 : 3.0);   // per chain per repetition
+    const double adds = static_cast<double>(blocks) * threads * iters * 8.0 * 8.0 * adds_per_step;
     *adds_per_sec = adds / (static_cast<double>(best_ms) * 1e-3);
     return cudaSuccess;
 }

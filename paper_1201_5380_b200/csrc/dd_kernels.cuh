@@ -21,15 +21,23 @@ struct KernelParams {
     int32_t nchans, ndm, nblk, ntiles, nbeams;
     int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
     int32_t raw_slot, lane_slot;
+    int32_t nstages;          // ring depth of the staged buffers (bit-plane variant)
+    int32_t nchans_pad;       // channels iterated over: nchans padded to a multiple of cc (bit-plane variant)
+    const uint8_t *zero;      // raw_slot zero bytes: the span of a padded channel
     const int2 *span;         // [nblk][nchans] {start, nbytes}
     const void *rel;          // [nblk][nchans][DB] entries of var.rel_bytes
 };
 
 // Enqueues the kernel variant chosen by the plan.  Returns the cudaError_t of the launch.
-cudaError_t launch_direct(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 
 cudaError_t launch_variant1(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 cudaError_t launch_variant2(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+// variant 3 launches two kernels (bit-plane transpose into plan->d_work, then the transform); it may grow d_work
+cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+
+// Kernels one launch_direct call enqueues for this plan.
+int launches_per_execute(const dd_plan_s *plan);
 
 // Integer-add throughput microbenchmark (roofline denominator).  Synchronises `stream`.
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream);

@@ -45,43 +45,46 @@ static inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * 
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 {
     const Variant &v = p->var;
-    int64_t bytes = 128;                                                              // mbarriers
-    bytes += 2 * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);        // offset-table stages
-    bytes += 2 * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);               // packed stages
-    if (v.lane_bits != p->nbits)                                                      // unpacked lanes
+    int64_t bytes = 128;                                                                          // mbarriers
+    bytes += p->nstages * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);           // offset-table stages
+    bytes += p->nstages * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);                  // packed / bit-plane stages
+    if (v.lane_bits != p->nbits)                                                                  // unpacked lanes
         bytes += v.lane_stages * align_up(static_cast<int64_t>(cc) * p->lane_slot, 128);
     return bytes;
 }
 
-// The kernel variants compiled into the library (dd_kernels.cu), in order of preference.
+// The kernel variants compiled into the library, in order of preference.
 static const Variant kVariants[] = {
-    /* id  DB   TB   thr tail rel lane stg  cc candidates      nbits     wide */
-    {2, 32, 1280, 512, 8, 4, 4, 2, {40, 20, 10, 5}, 1 << 2, false},                  // 2-bit, nibble lanes
-    {1, 32, 640, 256, 4, 2, 8, 1, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), true},
+    /* id  DB   TB    thr tail rel lane lst rst  cc candidates     nbits                        sum  pad    bitplane */
+    {3, 16, 5120, 512, 32, 8, 2, 0, 4, {32, 0, 0, 0}, 1 << 2, 12, true, true},                     // 2-bit, bit planes + carry-save
+    {2, 32, 1280, 512, 8, 4, 4, 2, 2, {40, 20, 10, 5}, 1 << 2, 16, false, false},                  // 2-bit, nibble lanes
+    {1, 32, 640, 256, 4, 2, 8, 1, 2, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), 32, false, false},
 };
 
 dd_status build_tiles(dd_plan_s *p)
 {
     const int nchans = p->nchans, ndm = p->ndm, nbits = p->nbits;
     const int64_t vmax = (1 << nbits) - 1;
-    p->final32 = static_cast<int64_t>(nchans) * vmax > 65535;
+    const int64_t top = static_cast<int64_t>(nchans) * vmax;   // largest possible sum
+    p->final32 = top > 65535;
     const int A = 128 / nbits;   // samples per 16 packed bytes: bulk-copy granularity
 
     for (const Variant &v : kVariants) {
-        if (!(v.nbits_mask & (1 << nbits)) || (p->final32 && !v.wide_ok))
+        if (!(v.nbits_mask & (1 << nbits)) || (v.max_sum_bits < 32 && top >= (int64_t(1) << v.max_sum_bits)))
             continue;
         if (p->force_variant && v.id != p->force_variant)
             continue;
         p->var = v;
         const int DB = v.DB;
         const int nblk = (ndm + DB - 1) / DB;
-        const int64_t rel_limit = v.rel_bytes == 2 ? 65535 : (int64_t(1) << 28);
-        std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans);
-        std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchans * DB * v.rel_bytes);
-        int64_t max_bytes = 0;
+        const int64_t rel_limit = v.rel_bytes == 2 ? 65535 : (int64_t(1) << 26);
+        // pass 1: the staged span of every (DM block, channel): [dmin rounded down to the copy granularity,
+        // dmax + time block + over-fetch)
+        std::vector<SpanMeta> span0(static_cast<size_t>(nblk) * nchans);
+        int64_t max_bytes = 0, max_end = 0;
         bool ok = true;
         for (int b = 0; b < nblk && ok; ++b) {
-            for (int c = 0; c < nchans && ok; ++c) {
+            for (int c = 0; c < nchans; ++c) {
                 int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0;
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);   // pad the last block with its last DM
@@ -96,40 +99,73 @@ dd_status build_tiles(dd_plan_s *p)
                     ok = false;
                     break;
                 }
-                SpanMeta &m = span[static_cast<size_t>(b) * nchans + c];
+                SpanMeta &m = span0[static_cast<size_t>(b) * nchans + c];
                 m.start = start;
                 m.nbytes = static_cast<int32_t>(nbytes);
                 max_bytes = std::max(max_bytes, nbytes);
-                const size_t base = (static_cast<size_t>(b) * nchans + c) * DB;
-                for (int i = 0; i < DB; ++i) {
-                    const int d = std::min(b * DB + i, ndm - 1);
-                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nchans + c] - start);
-                    if (v.rel_bytes == 2)
-                        reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
-                    else
-                        reinterpret_cast<uint32_t *>(rel.data())[base + i] = off * 4u;
-                }
+                max_end = std::max(max_end, start + nbytes * 8 / nbits);
             }
         }
         if (!ok)
             continue;
+        p->max_span_end = max_end;
         p->raw_slot = static_cast<int>(max_bytes);
         p->lane_slot = static_cast<int>(max_bytes * v.lane_bits / nbits);
         int cc = 0;
-        for (int k = 0; k < 4 && v.cc[k] > 0; ++k) {
-            const int cand = v.cc[k];
-            if (k + 1 < 4 && v.cc[k + 1] > 0 && v.cc[k + 1] >= nchans)
-                continue;   // a smaller stage already covers every channel
-            const int64_t tx = static_cast<int64_t>(cand) * p->raw_slot + static_cast<int64_t>(cand) * DB * v.rel_bytes;
-            if (smem_layout_bytes(p, cand) <= kMaxDynSmem && tx < (1 << 20)) {
-                cc = cand;
-                break;
+        for (p->nstages = v.raw_stages; p->nstages >= 2 && cc == 0; --p->nstages) {   // deepest ring that fits
+            for (int k = 0; k < 4 && v.cc[k] > 0; ++k) {
+                const int cand = v.cc[k];
+                if (!v.pad_chunks && k + 1 < 4 && v.cc[k + 1] > 0 && v.cc[k + 1] >= nchans)
+                    continue;   // a smaller stage already covers every channel
+                const int64_t tx = static_cast<int64_t>(cand) * p->raw_slot + static_cast<int64_t>(cand) * DB * v.rel_bytes;
+                if (smem_layout_bytes(p, cand) <= kMaxDynSmem && tx < (1 << 20)) {
+                    cc = cand;
+                    break;
+                }
             }
+            if (cc)
+                break;
         }
         if (cc < 1)
             continue;
+        // pass 2: per (DM, channel) the position of that DM's window inside the staged span
+        const int nchans_pad = v.pad_chunks ? static_cast<int>(align_up(nchans, cc)) : nchans;
+        std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans_pad);
+        std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchans_pad * DB * v.rel_bytes);
+        for (int b = 0; b < nblk; ++b) {
+            for (int c = 0; c < nchans_pad; ++c) {
+                SpanMeta &m = span[static_cast<size_t>(b) * nchans_pad + c];
+                const size_t base = (static_cast<size_t>(b) * nchans_pad + c) * DB;
+                const uint32_t slot_off = static_cast<uint32_t>(c % cc) * static_cast<uint32_t>(p->raw_slot);
+                if (c >= nchans) {   // padded channel: a whole slot of zeros, every window at its start
+                    m.start = 0;
+                    m.nbytes = -p->raw_slot;   // negative: stage from the zero buffer
+                    for (int i = 0; i < DB; ++i) {
+                        uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
+                        e[0] = slot_off;
+                        e[1] = 0;
+                    }
+                    continue;
+                }
+                m = span0[static_cast<size_t>(b) * nchans + c];
+                for (int i = 0; i < DB; ++i) {
+                    const int d = std::min(b * DB + i, ndm - 1);
+                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nchans + c] - m.start);
+                    if (v.rel_bytes == 2) {
+                        reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
+                    } else if (v.rel_bytes == 4) {
+                        reinterpret_cast<uint32_t *>(rel.data())[base + i] = off * 4u;
+                    } else {   // bit planes: 32 samples per group of nbits words
+                        uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
+                        e[0] = slot_off + (off >> 5) * 4u * static_cast<uint32_t>(nbits);
+                        e[1] = off & 31u;
+                    }
+                }
+            }
+        }
         p->cc = cc;
         p->nblk = nblk;
+        p->nchans_pad = nchans_pad;
         p->smem_bytes = smem_layout_bytes(p, cc);
         p->span.swap(span);
         p->rel.swap(rel);

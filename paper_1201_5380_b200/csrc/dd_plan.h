@@ -21,12 +21,17 @@ struct Variant {
     int TB;           // output samples per CTA
     int threads;      // threads per CTA
     int tail;         // extra samples a thread may read past TB + offset (over-fetch of the aligned loads)
-    int rel_bytes;    // bytes per offset-table entry: 2 = sample offset (uint16), 4 = 4 * sample offset (uint32)
-    int lane_bits;    // bits per sample of the unpacked lane buffer in shared memory
+    int rel_bytes;    // bytes per offset-table entry: 2 = sample offset (uint16), 4 = 4 * sample offset (uint32),
+                      // 8 = {byte offset of the DM's first window word inside the stage, bit shift} (2 x uint32)
+    int lane_bits;    // bits per sample of the unpacked lane buffer in shared memory (== nbits: no lane buffer)
     int lane_stages;  // lane buffers (1 = single, 2 = double-buffered)
+    int raw_stages;   // stages of the packed / bit-plane buffer and of the offset table
     int cc[4];        // candidate channels-per-stage, largest first (0 = end)
     int nbits_mask;   // input widths served (bit n set = nbits n)
-    bool wide_ok;     // can accumulate sums that need more than 16 bits
+    int max_sum_bits; // widest sum the accumulators hold: nchans*(2^nbits-1) < 2^max_sum_bits
+    bool pad_chunks;  // the kernel always processes whole stages: the channel list is padded to a multiple
+                      // of cc with all-zero channels (their spans are staged from a zeroed device buffer)
+    bool bitplane;    // stages hold bit planes produced by the transpose pre-pass (dd_kernel_bp.cu)
 };
 
 struct SpanMeta {   // per (DM block, channel); mirrored on the device as int2
@@ -56,17 +61,23 @@ struct dd_plan_s {
     int force_variant = 0; // 0 = automatic; otherwise only this variant id is considered (dd_set_kernel_variant)
     int nblk = 0;          // DM blocks
     int cc = 0;            // channels per pipeline stage
+    int nchans_pad = 0;    // channels the kernel iterates over (nchans, or padded to a multiple of cc)
+    int nstages = 2;       // ring depth of the staged buffers (<= var.raw_stages)
+    int64_t max_span_end = 0;   // max over spans of start + staged samples: how far past a tile's t0 a copy reaches
     int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
-    std::vector<dd::SpanMeta> span;   // [nblk][nchans]
-    std::vector<uint8_t> rel;         // [nblk][nchans][DB] entries of var.rel_bytes: delay - span start per DM slot
+    std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad]
+    std::vector<uint8_t> rel;         // [nblk][nchans_pad][DB] entries of var.rel_bytes: delay - span start per DM slot
     // device copies
     int device = -1;
     bool uploaded = false;
     void *d_span = nullptr;
     void *d_rel = nullptr;
+    void *d_zero = nullptr;           // raw_slot zero bytes (source of the padded channels)
+    void *d_work = nullptr;           // bit-plane copy of the input (variants with `bitplane`), grown on demand
+    size_t work_bytes = 0;
     int64_t last_launches = 0;
     dd::HostStage *stage = nullptr;
 };

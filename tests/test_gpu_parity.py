@@ -38,7 +38,7 @@ def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, var
         p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
         torch.cuda.synchronize()
         info = p.launch_info()
-        assert info["last_launches"] == 1 and (variant == 0 or info["variant"] == variant)
+        assert info["last_launches"] == (2 if info["variant"] == 3 else 1) and (variant == 0 or info["variant"] == variant)
     return out.cpu().numpy().view(_NP_VIEW[out_kind])
 
 
@@ -68,10 +68,31 @@ def test_cfg1_full_u32_and_f32():
     _full_compare(W.CONFIGS[1], out_kinds=["u32", "f32", "u16"])
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_cfg2_reduced_several_tiles_ragged_tail(variant):
-    # 1024 channels, 2-bit, 70 DMs (3 DM blocks, last ragged), 3 time tiles + ragged tail of 77 samples
+    # 1024 channels, 2-bit, 70 DMs (3 DM blocks of 32 / 5 of 16, last ragged), 3 time tiles + ragged tail of 77 samples
     _full_compare(W.CONFIGS[2].reduced(nsamps=3 * 1280 + 77, ndm=70), variant=variant)
+
+
+def test_variant3_bitplane_tiles_and_channel_padding():
+    # bit-plane kernel: 5120-sample tiles (2 tiles + ragged tail), 16-DM blocks (ragged), channel counts around
+    # the 32-channel stage (padded with zero channels) and the ring depth
+    _full_compare(W.CONFIGS[2].reduced(nsamps=2 * 5120 + 333, ndm=37), out_kinds=["f32", "u32", "u16"], variant=3)
+    for nchans in (1, 31, 32, 33, 64, 65, 95, 129, 1023, 1365):
+        _full_compare(W.CONFIGS[2].reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=3)
+
+
+def test_variant3_extreme_values_fill_all_planes():
+    # all samples 3 with 1365 channels: every sum is 4095 = 2^12 - 1 (all twelve planes set); all samples 0
+    cfg = W.CONFIGS[2].reduced(nsamps=700, ndm=5, nchans=1365)
+    tab = _oracle_table(cfg)
+    nbytes = (cfg.nsamps + int(tab.max()) + 3) // 4
+    stride = (nbytes + 15) // 16 * 16
+    for fill, want in ((0xFF, 4095), (0x00, 0)):
+        packed = torch.full((1, cfg.nchans, stride), fill, dtype=torch.uint8)
+        got = _gpu_transform(cfg, packed.cuda(), stride, cfg.dm_list(), "u32", cfg.nsamps, 3)
+        ref = oracle.dedisperse(packed[0].numpy(), 2, cfg.nsamps, tab)
+        assert np.array_equal(got[0], ref) and int(ref.max()) == want and int(ref.min()) == want
 
 
 def test_variant2_channel_counts_around_group_and_flush_boundaries():
@@ -80,7 +101,7 @@ def test_variant2_channel_counts_around_group_and_flush_boundaries():
         _full_compare(W.CONFIGS[2].reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=2)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_cfg2_high_dm_end(variant):
     # the last DMs of config 2 (largest delays and spreads), nsamps not a multiple of 4
     cfg = W.CONFIGS[2].reduced(nsamps=1501, ndm=40)
@@ -139,6 +160,20 @@ def test_execute_host_matches_oracle():
         p.set_dm_list(cfg.dm_list())
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 16)
     assert np.array_equal(out.numpy().view(np.uint16), ref)
+
+
+def test_execute_host_bitplane_variant_two_slabs():
+    # 2-bit through the host-buffer path: 140000 output samples = two time slabs (133120 + ragged rest)
+    cfg = W.CONFIGS[2].reduced(nsamps=140000, ndm=9, nchans=64)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    ref = oracle.cast_out(oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab), "f32")
+    out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
+        assert p.launch_info()["last_launches"] == 4
+    assert np.array_equal(out.numpy(), ref)
 
 
 def test_device_generation_equals_host_generation():
