@@ -147,6 +147,22 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant);
 dd_status dd_get_launch_info(dd_plan plan, int64_t *info);
 
 /*
+ * dd_profile_enable / dd_profile_read -- optional per-kernel device timing of dd_execute (benchmarks).
+ * When enabled, each dd_execute records three CUDA events on the caller's stream: before the first kernel,
+ * between the bit-plane pre-pass and the transform kernel (variants without a pre-pass record it right after
+ * the first event), and after the last kernel.  Up to `max_executes` calls are recorded; further calls run
+ * untimed.  The events cost no synchronisation.
+ *   max_executes  > 0: enable (re-arms and drops earlier records); 0: disable and free the events.
+ * dd_profile_read waits for the last recorded event, then writes, per recorded dd_execute, the pre-pass and
+ * transform-kernel durations in milliseconds and re-arms the recorder.
+ *   n_executes  HOST out: number of records written (<= max_executes).
+ *   prepass_ms  HOST out, max_executes floats (0 for variants without a pre-pass).
+ *   main_ms     HOST out, max_executes floats.
+ */
+dd_status dd_profile_enable(dd_plan plan, int max_executes);
+dd_status dd_profile_read(dd_plan plan, int *n_executes, float *prepass_ms, float *main_ms);
+
+/*
  * dd_int_add_peak -- measures this GPU's 32-bit integer-add throughput (the ALU roofline denominator
  * of DESIGN.md section 6) with a register-resident microbenchmark on all SMs.  Additions are counted, not
  * instructions, and the chains are cross-coupled so that the compiler cannot fold two additions into one.

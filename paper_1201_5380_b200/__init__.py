@@ -20,7 +20,7 @@ __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
 
@@ -30,7 +30,7 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_strerror", "dd_last_cuda_error",
+    "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -78,12 +78,15 @@ def lib() -> ctypes.CDLL:
         L.dd_get_launch_info.argtypes = [vp, vp]
         L.dd_set_kernel_variant.argtypes = [vp, i32]
         L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
+        L.dd_profile_enable.argtypes = [vp, i32]
+        L.dd_profile_read.argtypes = [vp, ctypes.POINTER(i32), vp, vp]
         L.dd_strerror.argtypes = [i32]
         L.dd_strerror.restype = ctypes.c_char_p
         L.dd_last_cuda_error.argtypes = []
         L.dd_last_cuda_error.restype = ctypes.c_char_p
         for name in ("dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_set_batch",
-                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak", "dd_set_kernel_variant"):
+                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak", "dd_set_kernel_variant",
+                     "dd_profile_enable", "dd_profile_read"):
             getattr(L, name).restype = i32
         _LIB = L
     return _LIB
@@ -181,6 +184,20 @@ def dd_get_launch_info(plan: int) -> dict:
     return {k: int(v) for k, v in zip(keys, info)}
 
 
+def dd_profile_enable(plan: int, max_executes: int) -> None:
+    """Record per-kernel CUDA-event times of the next `max_executes` dd_execute calls (0 disables)."""
+    _check(lib().dd_profile_enable(plan, int(max_executes)), "dd_profile_enable")
+
+
+def dd_profile_read(plan: int, max_executes: int):
+    """-> (prepass_ms, main_ms) float32 arrays, one entry per recorded dd_execute; synchronises; re-arms."""
+    n = ctypes.c_int(0)
+    pre = np.zeros(max_executes, dtype=np.float32)
+    main = np.zeros(max_executes, dtype=np.float32)
+    _check(lib().dd_profile_read(plan, ctypes.byref(n), pre.ctypes.data, main.ctypes.data), "dd_profile_read")
+    return pre[:n.value].copy(), main[:n.value].copy()
+
+
 def dd_int_add_peak(mode: int = 0, stream=None) -> float:
     """Measured 32-bit integer additions per second on the current device (synchronises)."""
     v = ctypes.c_double()
@@ -219,6 +236,13 @@ class Plan:
 
     def execute(self, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream=None) -> None:
         dd_execute(self.handle, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream)
+
+    def profile_enable(self, max_executes: int) -> None:
+        self._prof_cap = int(max_executes)
+        dd_profile_enable(self.handle, max_executes)
+
+    def profile_read(self):
+        return dd_profile_read(self.handle, self._prof_cap)
 
     def execute_host(self, nsamps, in_host, in_stride, out_host, out_nbits) -> None:
         dd_execute_host(self.handle, nsamps, in_host, in_stride, out_host, out_nbits)

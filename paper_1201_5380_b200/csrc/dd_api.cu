@@ -98,6 +98,15 @@ static dd_status upload_tables(dd_plan_s *p)
     return DD_OK;
 }
 
+static void free_prof_events(dd_plan_s *p)
+{
+    for (void *e : p->prof_events)
+        if (e)
+            cudaEventDestroy(static_cast<cudaEvent_t>(e));
+    p->prof_events.clear();
+    p->prof_cap = p->prof_n = 0;
+}
+
 static int elem_size(int out_nbits)
 {
     switch (out_nbits) {
@@ -201,6 +210,7 @@ dd_status dd_plan_destroy(dd_plan plan)
     if (plan->d_work)
         cudaFree(plan->d_work);
     free_stage(plan->stage);
+    free_prof_events(plan);
     delete plan;
     return DD_OK;
 }
@@ -322,9 +332,25 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
     }
     const KernelParams kp = make_params(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, plan->nbeams,
                                         plan->in_beam_stride, plan->out_beam_stride);
-    const cudaError_t e = launch_direct(plan, kp, static_cast<cudaStream_t>(stream));
+    cudaStream_t st_ = static_cast<cudaStream_t>(stream);
+    const bool prof = plan->prof_cap > 0 && plan->prof_n < plan->prof_cap;
+    cudaEvent_t *ev = prof ? reinterpret_cast<cudaEvent_t *>(plan->prof_events.data()) + 3 * plan->prof_n : nullptr;
+    plan->prof_mid = nullptr;
+    if (prof) {
+        cudaEventRecord(ev[0], st_);
+        if (plan->var.bitplane)
+            plan->prof_mid = ev[1];        // recorded by the launcher after the pre-pass
+        else
+            cudaEventRecord(ev[1], st_);
+    }
+    const cudaError_t e = launch_direct(plan, kp, st_);
+    plan->prof_mid = nullptr;
     if (e != cudaSuccess)
         return cuda_fail(e, "dd_execute launch");
+    if (prof) {
+        cudaEventRecord(ev[2], st_);
+        ++plan->prof_n;
+    }
     plan->last_launches = launches_per_execute(plan);
     return DD_OK;
 }
@@ -463,6 +489,57 @@ dd_status dd_get_launch_info(dd_plan plan, int64_t *info)
     info[5] = plan->nblk;
     info[6] = plan->last_launches;
     info[7] = plan->var.id;
+    return DD_OK;
+}
+
+dd_status dd_profile_enable(dd_plan plan, int max_executes)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (max_executes < 0 || max_executes > (1 << 20))
+        return DD_ERR_INVALID_ARG;
+    free_prof_events(plan);
+    if (max_executes == 0)
+        return DD_OK;
+    try {
+        plan->prof_events.assign(static_cast<size_t>(max_executes) * 3, nullptr);
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+    for (void *&e : plan->prof_events) {
+        cudaEvent_t ev;
+        const cudaError_t ce = cudaEventCreate(&ev);
+        if (ce != cudaSuccess) {
+            free_prof_events(plan);
+            return cuda_fail(ce, "cudaEventCreate");
+        }
+        e = ev;
+    }
+    plan->prof_cap = max_executes;
+    return DD_OK;
+}
+
+dd_status dd_profile_read(dd_plan plan, int *n_executes, float *prepass_ms, float *main_ms)
+{
+    if (!plan || !n_executes || !prepass_ms || !main_ms)
+        return DD_ERR_NULL;
+    *n_executes = 0;
+    if (plan->prof_cap <= 0)
+        return DD_ERR_INVALID_ARG;
+    cudaEvent_t *ev = reinterpret_cast<cudaEvent_t *>(plan->prof_events.data());
+    const int n = plan->prof_n;
+    if (n > 0) {
+        cudaError_t ce = cudaEventSynchronize(ev[3 * (n - 1) + 2]);
+        if (ce != cudaSuccess)
+            return cuda_fail(ce, "cudaEventSynchronize");
+        for (int i = 0; i < n; ++i) {
+            if ((ce = cudaEventElapsedTime(&prepass_ms[i], ev[3 * i], ev[3 * i + 1])) != cudaSuccess ||
+                (ce = cudaEventElapsedTime(&main_ms[i], ev[3 * i + 1], ev[3 * i + 2])) != cudaSuccess)
+                return cuda_fail(ce, "cudaEventElapsedTime");
+        }
+    }
+    *n_executes = n;
+    plan->prof_n = 0;
     return DD_OK;
 }
 

@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) {
-            mbar_init(&full[s], 32);
+            mbar_init(&full[s], BP_NWARPS);
             mbar_init(&empty[s], BP_NWARPS);
         }
         mbar_fence_init();
@@ -192,36 +192,59 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
     const int2 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans_pad;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + static_cast<int64_t>(blk) * p.nchans_pad * DB;
 
-    // producer (warp 0): lane i stages channel chunk*32 + i; lane 0 also stages the chunk's offset entries
-    auto produce = [&](int chunk) {
+    // producers: EVERY warp stages CPW = CC / NWARPS channels of each chunk (its lane 0 issues the bulk copies:
+    // a bulk copy takes its operands from uniform registers, so one warp issuing all 32 copies of a chunk
+    // serialises over its lanes and falls behind the others); warp 0 also stages the chunk's offset entries.
+    // The span metadata of the next chunk to stage is fetched one step early.
+    constexpr int CPW = CC / BP_NWARPS;
+    auto load_meta = [&](int chunk, int2 (&m)[CPW]) {
+#pragma unroll
+        for (int k = 0; k < CPW; ++k)
+            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + warp * CPW + k]) : make_int2(0, 0);
+    };
+    auto produce = [&](int chunk, const int2 (&m)[CPW]) {
         const int s = chunk % NS;
-        if (chunk >= NS)
-            mbar_wait(&empty[s], ((chunk / NS) - 1) & 1);   // every warp has finished chunk - NS
-        const int c = chunk * CC + lane;
-        const int2 m = __ldg(&span_blk[c]);
-        const uint8_t *src;
-        uint32_t bytes;
-        if (m.y < 0) {                                       // padded channel: zeros
-            src = p.zero;
-            bytes = static_cast<uint32_t>(-m.y);
-        } else {
-            const int64_t off = ((t0 + m.x) * 2) >> 3;
-            const int64_t avail = p.in_row_bytes - off;
-            bytes = static_cast<uint32_t>(m.y < avail ? m.y : (avail > 0 ? avail : 0));
-            src = in_beam + static_cast<int64_t>(c) * p.in_stride + off;
+        if (lane == 0) {
+            if (chunk >= NS)
+                mbar_wait(&empty[s], ((chunk / NS) - 1) & 1);   // every warp has finished chunk - NS
+            const uint8_t *src[CPW];
+            uint32_t bytes[CPW], tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
+#pragma unroll
+            for (int k = 0; k < CPW; ++k) {
+                const int c = chunk * CC + warp * CPW + k;
+                if (m[k].y < 0) {                                // padded channel: zeros
+                    src[k] = p.zero;
+                    bytes[k] = static_cast<uint32_t>(-m[k].y);
+                } else {
+                    const int64_t off = ((t0 + m[k].x) * 2) >> 3;
+                    const int64_t avail = p.in_row_bytes - off;
+                    bytes[k] = static_cast<uint32_t>(m[k].y < avail ? m[k].y : (avail > 0 ? avail : 0));
+                    src[k] = in_beam + static_cast<int64_t>(c) * p.in_stride + off;
+                }
+                tx += bytes[k];
+            }
+            mbar_arrive_expect_tx(&full[s], tx);
+#pragma unroll
+            for (int k = 0; k < CPW; ++k)
+                if (bytes[k])
+                    tma_bulk_g2s(raw_base + s * raw_stage + (warp * CPW + k) * p.raw_slot, src[k], bytes[k], &full[s]);
+            if (warp == 0)
+                tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(chunk) * CC * DB,
+                             static_cast<uint32_t>(CC * DB * 8), &full[s]);
         }
-        mbar_arrive_expect_tx(&full[s], bytes + (lane == 0 ? static_cast<uint32_t>(CC * DB * 8) : 0u));
-        if (bytes)
-            tma_bulk_g2s(raw_base + s * raw_stage + lane * p.raw_slot, src, bytes, &full[s]);
-        if (lane == 0)
-            tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(chunk) * CC * DB,
-                         static_cast<uint32_t>(CC * DB * 8), &full[s]);
+        __syncwarp();
     };
 
-    const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in chunks
-    if (warp == 0)
-        for (int k = 0; k < dist && k < p.nchunks; ++k)
-            produce(k);
+    const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in chunks (measured: 1 and 2 equal, 3 slower)
+    int2 meta[CPW], nxt[CPW];
+    load_meta(0, meta);
+    for (int k = 0; k < dist && k < p.nchunks; ++k) {
+        load_meta(k + 1, nxt);
+        produce(k, meta);
+#pragma unroll
+        for (int i = 0; i < CPW; ++i)
+            meta[i] = nxt[i];
+    }
 
     uint32_t P[W][NP], T[W][BP_NT];
 #pragma unroll
@@ -236,8 +259,13 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
 
     for (int chunk = 0; chunk < p.nchunks; ++chunk) {
         const int s = chunk % NS;
-        if (warp == 0 && chunk + dist < p.nchunks)
-            produce(chunk + dist);
+        if (chunk + dist < p.nchunks) {
+            load_meta(chunk + dist + 1, nxt);
+            produce(chunk + dist, meta);
+#pragma unroll
+            for (int i = 0; i < CPW; ++i)
+                meta[i] = nxt[i];
+        }
         mbar_wait(&full[s], (chunk / NS) & 1);
 
         BpShared sh;
@@ -356,6 +384,8 @@ cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp_in, cudaStre
         static_cast<int64_t>(kp.nchans) * conv, chunks);
     if ((e = cudaGetLastError()) != cudaSuccess)
         return e;
+    if (plan->prof_mid)
+        cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     kp.in = static_cast<const uint8_t *>(plan->d_work);
     kp.in_stride = conv;
     kp.in_row_bytes = conv;

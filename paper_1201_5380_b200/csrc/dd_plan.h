@@ -80,6 +80,10 @@ struct dd_plan_s {
     size_t work_bytes = 0;
     int64_t last_launches = 0;
     dd::HostStage *stage = nullptr;
+    // optional per-kernel timing of dd_execute (dd_profile_enable): 3 events per recorded call
+    std::vector<void *> prof_events;   // cudaEvent_t [3 * prof_cap]
+    int prof_cap = 0, prof_n = 0;
+    void *prof_mid = nullptr;          // event the launcher records between pre-pass and transform (or null)
 };
 
 namespace dd {
