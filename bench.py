@@ -101,7 +101,7 @@ def info_after(plan) -> int:
     return int(plan.launch_info()["last_launches"])
 
 
-KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp2"}
+KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp<{nbits}>"}
 
 
 def measured_peaks() -> dict:

@@ -166,6 +166,7 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     kp.nchunks = (p->nchans + p->cc - 1) / p->cc;
     kp.raw_slot = p->raw_slot;
     kp.lane_slot = p->lane_slot;
+    kp.sub_slot = p->sub_slot;
     kp.nstages = p->nstages;
     kp.nchans_pad = p->nchans_pad;
     kp.zero = static_cast<const uint8_t *>(p->d_zero);
@@ -256,6 +257,7 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
     plan->nstages = scratch.nstages;
     plan->max_span_end = scratch.max_span_end;
     plan->raw_slot = scratch.raw_slot;
+    plan->sub_slot = scratch.sub_slot;
     plan->lane_slot = scratch.lane_slot;
     plan->smem_bytes = scratch.smem_bytes;
     plan->final32 = scratch.final32;

@@ -1,27 +1,34 @@
-// dd_kernel_bp.cu -- variant 3: 2-bit input as BIT PLANES, summed with carry-save adders.
+// dd_kernel_bp.cu -- variant 3: the input as BIT PLANES, summed with carry-save adders.
 //
 //     D[d][t] = sum_c A[c][t + delay[d][c]]                       (eq. 3)
 //
 // The paper's bit-level parallelism (several samples per machine word, one word operation
 // acting on all of them) taken to its end: ONE BIT per lane.  A pre-pass transposes every 32 consecutive
-// 2-bit samples of a channel into two 32-bit words, plane 0 (the low bits) and plane 1 (the high bits), in
-// time order (sub-word samples handled by shift and mask).  The sum over channels is then a
-// population count per lane, kept as NP bit planes P[0..NP) (P[k] holds bit k of 32 sums) and updated with
-// 3:2 carry-save adders: sum = a ^ b ^ c, carry = maj(a, b, c), two LOP3 instructions that add one more
-// 32-sample word into the counter.  Per channel and 32 outputs that is 2 funnel shifts (the delay is an
-// arbitrary bit offset into the plane words) + ~4.3 LOP3 for 32 channel-adds, against 4 shifts + 2 adds +
-// 4 flush operations for the nibble lanes of variant 2, and half the shared-memory traffic.
+// n-bit samples of a channel into n 32-bit words, plane k holding bit k of the 32 samples in time order
+// (sub-word samples handled by shift and mask).  The sum over channels is then a population
+// count per lane, kept as NP bit planes P[0..NP) (P[k] holds bit k of 32 sums) and updated with 3:2
+// carry-save adders: sum = a ^ b ^ c, carry = maj(a, b, c), two LOP3 instructions that add one more
+// 32-sample word into the counter.  Per channel and 32 outputs that is n funnel shifts (the delay is an
+// arbitrary bit offset into the plane words) + ~2.1 n LOP3 for 32 channel-adds, i.e. ~3.1 ALU instructions
+// per 32 input bits whatever the sample width.
 //
-// One CTA = 16 DM trials x 5120 output samples, 16 warps; warp w owns DM slot w, lane l owns the five
-// 32-sample units 5l .. 5l+4 of the time block (W = 5: six 8-byte loads serve five units).
+// Layout.  A "unit" is 32 consecutive samples.  Planes are stored in SUB-ROWS of NB planes: unit u of a
+// sub-row is NB consecutive words {plane 0 .. plane NB-1} (8 bytes for NB = 2, 16 bytes for NB = 4) so that
+// one LDS.64 / LDS.128 fetches all of them.  2- and 4-bit input has one sub-row per channel; 8-bit input
+// has two (planes 0-3 and planes 4-7), handled as two 4-plane channels of the same delay whose words carry
+// weights 1..8 and 16..128.  With W odd, the lanes of a warp (W units = W * 4 NB bytes apart) fall into
+// distinct shared-memory banks.
+//
+// One CTA = 16 DM trials x (32 * 32 * W) output samples, 16 warps; warp w owns DM slot w, lane l owns the W
+// units W l .. W l + W - 1 of the time block (W + 1 loads serve W units).
 //   stage  : per channel, the bit-plane span [t0 + start, ...) of the DM block (time block + delay range,
-//            PAPER.md:115) arrives by TMA bulk copy; ring of `nstages` stages of 32 channels, full/empty
+//            PAPER.md:115) arrives by TMA bulk copy; ring of `nstages` stages of CC channels, full/empty
 //            mbarriers, no CTA-wide barrier in the channel loop;
 //   add    : carry-save counter per unit; words of equal weight are paired as they appear (a binary counter
-//            of pending words, resolved at compile time), the pending words left after 32 channels are
-//            rippled into the upper planes;
-//   store  : 16x16 bit-matrix transposes turn 12 planes x 32 lanes into 32 integers; float32 / uint32 /
-//            uint16, 128-bit stores, time contiguous.
+//            of pending words, resolved at compile time), the pending words left after a stage are rippled
+//            into the upper planes;
+//   store  : bit-matrix transposes turn NP planes x 32 lanes into 32 integers; float32 / uint32 / uint16,
+//            128-bit stores, time contiguous.
 #include <utility>
 
 #include "dd_common.cuh"
@@ -30,10 +37,25 @@
 namespace dd {
 namespace {
 
-constexpr int BP_DB = 16, BP_W = 5, BP_NWARPS = 16, BP_TB = 32 * 32 * BP_W, BP_CC = 32;
-constexpr int BP_NP = 12;                 // planes: sums < 2^12 (plan: nchans * 3 < 4096)
-constexpr int BP_NT = 8;                  // pending slots (weights 1 .. 128; 32 channels * 3 = 96 < 256)
-constexpr uint32_t BP_WSUM = 3;           // weight added per channel: 2^nbits - 1
+constexpr int BP_DB = 16, BP_NWARPS = 16;
+
+// Tile shape per input width.  NP planes hold sums < 2^NP (the plan checks nchans * (2^nbits - 1) < 2^NP).
+template <int NBITS>
+struct Bp;
+template <>
+struct Bp<2> {
+    static constexpr int NB = 2, NSUB = 1, NP = 12, W = 5, CC = 32;
+};
+template <>
+struct Bp<4> {
+    static constexpr int NB = 4, NSUB = 1, NP = 16, W = 3, CC = 16;
+};
+template <>
+struct Bp<8> {
+    static constexpr int NB = 4, NSUB = 2, NP = 20, W = 3, CC = 8;
+};
+
+__host__ __device__ constexpr int bit_length(uint32_t v) { return v == 0 ? 0 : 1 + bit_length(v >> 1); }
 
 // ------------------------------------------------------------------------------------------ pre-pass
 // bits at even positions of y (y & 0x55555555 == y) -> the low 16 bits, order kept
@@ -45,6 +67,16 @@ __device__ __forceinline__ uint32_t compress_even(uint32_t y)
     y = (y | (y >> 8)) & 0x0000FFFFu;
     return y;
 }
+// bits at positions 0, 4, .., 28 of y -> the low 8 bits, order kept
+__device__ __forceinline__ uint32_t compress_4th(uint32_t y)
+{
+    y = (y | (y >> 3)) & 0x03030303u;
+    y = (y | (y >> 6)) & 0x000F000Fu;
+    y = (y | (y >> 12)) & 0x000000FFu;
+    return y;
+}
+// bits at positions 0, 8, 16, 24 of y -> the low 4 bits, order kept
+__device__ __forceinline__ uint32_t compress_8th(uint32_t y) { return (y | (y >> 7) | (y >> 14) | (y >> 21)) & 0xFu; }
 
 // 32 two-bit samples (two packed words, LSB first) -> {plane 0, plane 1}; bit k of a plane = sample k
 __device__ __forceinline__ uint2 planes_of(uint32_t x0, uint32_t x1)
@@ -54,19 +86,53 @@ __device__ __forceinline__ uint2 planes_of(uint32_t x0, uint32_t x1)
                       compress_even((x0 >> 1) & m) | (compress_even((x1 >> 1) & m) << 16));
 }
 
-// in: packed rows [beam][c][in_stride]; work: bit-plane rows [beam][c][w_stride], unit u of a row is the
-// uint2 {plane 0, plane 1} of samples 32u .. 32u+31.  One thread converts 16 bytes (64 samples, 2 units).
-__global__ void __launch_bounds__(256) dd_to_bitplanes2(const uint8_t *__restrict__ in, int64_t in_stride,
-                                                        int64_t in_beam_stride, uint8_t *__restrict__ work,
-                                                        int64_t w_stride, int64_t w_beam_stride, int32_t chunks)
+// in: packed rows [beam][c][in_stride]; work: bit-plane rows [beam][c][sub][w_sub bytes].  One thread writes
+// 16 bytes of every sub-row of a channel: 64 samples (2 units) of 2-bit input, 32 samples (1 unit) of 4- and
+// 8-bit input.  Input bytes at or beyond in_row_bytes read as zero (only the last, partial unit of an 8-bit row).
+template <int NBITS>
+__global__ void __launch_bounds__(256) dd_to_bitplanes(const uint8_t *__restrict__ in, int64_t in_stride, int64_t in_row_bytes,
+                                                       int64_t in_beam_stride, uint8_t *__restrict__ work, int64_t w_sub,
+                                                       int64_t w_beam_stride, int32_t groups)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= chunks)
+    if (i >= groups)
         return;
     const int64_t c = blockIdx.y, beam = blockIdx.z;
-    const uint4 x = __ldg(reinterpret_cast<const uint4 *>(in + beam * in_beam_stride + c * in_stride) + i);
-    const uint2 a = planes_of(x.x, x.y), b = planes_of(x.z, x.w);
-    reinterpret_cast<uint4 *>(work + beam * w_beam_stride + c * w_stride)[i] = make_uint4(a.x, a.y, b.x, b.y);
+    const uint8_t *row = in + beam * in_beam_stride + c * in_stride;
+    uint8_t *wrow = work + beam * w_beam_stride + c * (Bp<NBITS>::NSUB * w_sub);
+    if constexpr (NBITS == 2) {
+        const uint4 x = __ldg(reinterpret_cast<const uint4 *>(row) + i);
+        const uint2 a = planes_of(x.x, x.y), b = planes_of(x.z, x.w);
+        reinterpret_cast<uint4 *>(wrow)[i] = make_uint4(a.x, a.y, b.x, b.y);
+    } else if constexpr (NBITS == 4) {
+        const uint4 x = __ldg(reinterpret_cast<const uint4 *>(row) + i);
+        const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+        uint32_t pl[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            pl[k] = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q)   // word q = samples 8q .. 8q+7
+                pl[k] |= compress_4th((w[q] >> k) & 0x11111111u) << (8 * q);
+        }
+        reinterpret_cast<uint4 *>(wrow)[i] = make_uint4(pl[0], pl[1], pl[2], pl[3]);
+    } else {
+        const int64_t b0 = static_cast<int64_t>(i) * 32;
+        const uint4 z = make_uint4(0, 0, 0, 0);
+        const uint4 xa = (b0 + 16 <= in_row_bytes) ? __ldg(reinterpret_cast<const uint4 *>(row + b0)) : z;
+        const uint4 xb = (b0 + 32 <= in_row_bytes) ? __ldg(reinterpret_cast<const uint4 *>(row + b0 + 16)) : z;
+        const uint32_t w[8] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
+        uint32_t pl[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            pl[k] = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q)   // word q = samples 4q .. 4q+3
+                pl[k] |= compress_8th((w[q] >> k) & 0x01010101u) << (4 * q);
+        }
+        reinterpret_cast<uint4 *>(wrow)[i] = make_uint4(pl[0], pl[1], pl[2], pl[3]);
+        reinterpret_cast<uint4 *>(wrow + w_sub)[i] = make_uint4(pl[4], pl[5], pl[6], pl[7]);
+    }
 }
 
 // ------------------------------------------------------------------------------------------ carry-save counter
@@ -85,9 +151,10 @@ __device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c)
 
 // Adds the word x of weight 2^L to the counter.  S is the compile-time occupancy of the pending slots
 // (bit k set: T[k] holds a word of weight 2^k waiting for a partner) -- a binary counter of the words seen.
-template <uint32_t S, int L>
-__device__ __forceinline__ void csa_add(uint32_t (&P)[BP_NP], uint32_t (&T)[BP_NT], uint32_t x)
+template <uint32_t S, int L, int NP, int NT>
+__device__ __forceinline__ void csa_add(uint32_t (&P)[NP], uint32_t (&T)[NT], uint32_t x)
 {
+    static_assert(L < NT && L < NP, "carry-save counter overflow");
     if constexpr (((S >> L) & 1u) == 0u) {
         T[L] = x;
     } else {
@@ -99,17 +166,17 @@ __device__ __forceinline__ void csa_add(uint32_t (&P)[BP_NP], uint32_t (&T)[BP_N
 
 // Empties the pending slots into the planes: ripple-carry addition of the pending number (occupancy S) from
 // level L upwards.  CARRY: a carry word `cy` of weight 2^L comes in from below.
-template <uint32_t S, int L, bool CARRY>
-__device__ __forceinline__ void csa_flush(uint32_t (&P)[BP_NP], const uint32_t (&T)[BP_NT], uint32_t cy)
+template <uint32_t S, int L, bool CARRY, int NP, int NT>
+__device__ __forceinline__ void csa_flush(uint32_t (&P)[NP], const uint32_t (&T)[NT], uint32_t cy)
 {
-    if constexpr (L < BP_NP) {
-        constexpr bool pend = L < BP_NT && ((S >> L) & 1u) != 0u;
+    if constexpr (L < NP) {
+        constexpr bool pend = L < NT && ((S >> L) & 1u) != 0u;
         if constexpr (pend && CARRY) {
             const uint32_t a = P[L];
             P[L] = xor3(a, T[L], cy);
             csa_flush<S, L + 1, true>(P, T, maj3(a, T[L], cy));
         } else if constexpr (pend || CARRY) {
-            const uint32_t a = P[L], b = pend ? T[L < BP_NT ? L : 0] : cy;
+            const uint32_t a = P[L], b = pend ? T[L < NT ? L : 0] : cy;
             P[L] = a ^ b;
             csa_flush<S, L + 1, true>(P, T, a & b);
         } else {
@@ -119,35 +186,73 @@ __device__ __forceinline__ void csa_flush(uint32_t (&P)[BP_NP], const uint32_t (
 }
 
 // ------------------------------------------------------------------------------------------ the kernel
-struct BpShared {
-    const uint8_t *lane_base;   // stage base + this lane's byte offset (5 units = 40 bytes per lane)
-    const uint2 *rel;           // this warp's offset entries of the stage: [cl * BP_DB]
+template <int NB>
+struct PlaneVec;
+template <>
+struct PlaneVec<2> {
+    uint32_t w[2];
+    __device__ __forceinline__ void load(const uint8_t *p)
+    {
+        const uint2 v = *reinterpret_cast<const uint2 *>(p);
+        w[0] = v.x, w[1] = v.y;
+    }
+};
+template <>
+struct PlaneVec<4> {
+    uint32_t w[4];
+    __device__ __forceinline__ void load(const uint8_t *p)
+    {
+        const uint4 v = *reinterpret_cast<const uint4 *>(p);
+        w[0] = v.x, w[1] = v.y, w[2] = v.z, w[3] = v.w;
+    }
 };
 
-// channel K of the stage: one window of W+1 units serves W units; 2 funnel shifts + carry-save adds per unit
-template <int K>
-__device__ __forceinline__ void channel_step(const BpShared &sh, uint32_t (&P)[BP_W][BP_NP], uint32_t (&T)[BP_W][BP_NT])
+struct BpShared {
+    const uint8_t *lane_base;   // stage base + this lane's byte offset (W units per lane)
+    const uint2 *rel;           // this warp's offset entries of the stage: [cl * BP_DB]
+    int sub_slot;               // bytes between the sub-rows of a channel slot
+};
+
+// plane k of sub-row SUB of channel CL of the stage, for every unit of the lane
+template <int NBITS, int CL, int SUB, int K, int NP, int NT>
+__device__ __forceinline__ void plane_step(const PlaneVec<Bp<NBITS>::NB> (&x)[Bp<NBITS>::W + 1], uint32_t shift,
+                                           uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
-    const uint2 e = sh.rel[K * BP_DB];                                        // {byte offset in the stage, bit shift}
-    const uint2 *wp = reinterpret_cast<const uint2 *>(sh.lane_base + e.x);
-    uint2 x[BP_W + 1];
+    using C = Bp<NBITS>;
+    if constexpr (K < C::NB) {
+        constexpr int L = SUB * C::NB + K;                                   // weight 2^L
+        constexpr uint32_t VMAX = (1u << NBITS) - 1u;
+        constexpr uint32_t S = VMAX * CL + ((1u << L) - 1u);                 // weight added to the counter so far
 #pragma unroll
-    for (int j = 0; j <= BP_W; ++j)
-        x[j] = wp[j];
-#pragma unroll
-    for (int j = 0; j < BP_W; ++j) {
-        const uint32_t b0 = __funnelshift_r(x[j].x, x[j + 1].x, e.y);
-        const uint32_t b1 = __funnelshift_r(x[j].y, x[j + 1].y, e.y);
-        csa_add<BP_WSUM * K, 0>(P[j], T[j], b0);
-        csa_add<BP_WSUM * K + 1u, 1>(P[j], T[j], b1);
+        for (int j = 0; j < C::W; ++j)
+            csa_add<S, L>(P[j], T[j], __funnelshift_r(x[j].w[K], x[j + 1].w[K], shift));
+        plane_step<NBITS, CL, SUB, K + 1>(x, shift, P, T);
     }
 }
 
-template <int... Ks>
-__device__ __forceinline__ void stage_steps(std::integer_sequence<int, Ks...>, const BpShared &sh,
-                                            uint32_t (&P)[BP_W][BP_NP], uint32_t (&T)[BP_W][BP_NT])
+// channel CL of the stage: per sub-row one window of W+1 units serves W units; per unit and plane one funnel
+// shift + carry-save adds
+template <int NBITS, int CL, int SUB, int NP, int NT>
+__device__ __forceinline__ void subrow_step(const BpShared &sh, const uint2 e, uint32_t (&P)[Bp<NBITS>::W][NP],
+                                            uint32_t (&T)[Bp<NBITS>::W][NT])
 {
-    (channel_step<Ks>(sh, P, T), ...);
+    using C = Bp<NBITS>;
+    if constexpr (SUB < C::NSUB) {
+        const uint8_t *wp = sh.lane_base + e.x + SUB * sh.sub_slot;
+        PlaneVec<C::NB> x[C::W + 1];
+#pragma unroll
+        for (int j = 0; j <= C::W; ++j)
+            x[j].load(wp + j * (C::NB * 4));
+        plane_step<NBITS, CL, SUB, 0>(x, e.y, P, T);
+        subrow_step<NBITS, CL, SUB + 1>(sh, e, P, T);
+    }
+}
+
+template <int NBITS, int NP, int NT, int... CLs>
+__device__ __forceinline__ void stage_steps(std::integer_sequence<int, CLs...>, const BpShared &sh,
+                                            uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
+{
+    (subrow_step<NBITS, CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);   // rel entry: {byte offset in the stage, bit shift}
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -155,9 +260,90 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
 }
 
-__global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelParams p)
+// 32 x 32 bit-matrix transpose: R[i] bit k  <-  R[k] bit i
+__device__ __forceinline__ void transpose32(uint32_t (&R)[32])
 {
-    constexpr int DB = BP_DB, W = BP_W, TB = BP_TB, CC = BP_CC, NP = BP_NP;
+#pragma unroll
+    for (int st = 0; st < 5; ++st) {
+        const int sh = 16 >> st;
+        const uint32_t m = st == 0 ? 0x0000FFFFu : st == 1 ? 0x00FF00FFu : st == 2 ? 0x0F0F0F0Fu : st == 3 ? 0x33333333u : 0x55555555u;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if (k & sh)
+                continue;
+            const uint32_t t = ((R[k] >> sh) ^ R[k + sh]) & m;
+            R[k + sh] ^= t;
+            R[k] ^= t << sh;
+        }
+    }
+}
+// 16 x 16 bit-matrix transpose of both half-words at once: afterwards R[k] = {sum of sample 16+k, sum of sample k}
+__device__ __forceinline__ void transpose16x2(uint32_t (&R)[16])
+{
+#pragma unroll
+    for (int st = 0; st < 4; ++st) {
+        const int sh = 8 >> st;
+        const uint32_t m = st == 0 ? 0x00FF00FFu : st == 1 ? 0x0F0F0F0Fu : st == 2 ? 0x33333333u : 0x55555555u;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            if (k & sh)
+                continue;
+            const uint32_t t = ((R[k] >> sh) ^ R[k + sh]) & m;
+            R[k + sh] ^= t;
+            R[k] ^= t << sh;
+        }
+    }
+}
+
+// four consecutive sums q[0..3] of DM row `orow` at sample t (a multiple of 4)
+__device__ __forceinline__ void store4(const KernelParams &p, uint8_t *orow, int64_t t, const uint32_t (&q)[4])
+{
+    if (t >= p.nsamps)
+        return;
+    const bool whole = p.vec_ok && (t + 4 <= p.nsamps);
+    if (p.out_code == DD_OUT_F32) {
+        float *o = reinterpret_cast<float *>(orow) + t;
+        if (whole) {
+            *reinterpret_cast<float4 *>(o) =
+                make_float4(__uint2float_rn(q[0]), __uint2float_rn(q[1]), __uint2float_rn(q[2]), __uint2float_rn(q[3]));
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k < p.nsamps)
+                    o[k] = __uint2float_rn(q[k]);
+        }
+    } else if (p.out_code == DD_OUT_U32) {
+        uint32_t *o = reinterpret_cast<uint32_t *>(orow) + t;
+        if (whole) {
+            *reinterpret_cast<uint4 *>(o) = make_uint4(q[0], q[1], q[2], q[3]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k < p.nsamps)
+                    o[k] = q[k];
+        }
+    } else {
+        uint16_t *o = reinterpret_cast<uint16_t *>(orow) + t;
+        if (whole) {
+            *reinterpret_cast<uint2 *>(o) = make_uint2(q[0] | (q[1] << 16), q[2] | (q[3] << 16));
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k < p.nsamps)
+                    o[k] = static_cast<uint16_t>(q[k]);
+        }
+    }
+}
+
+template <int NBITS>
+__global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
+{
+    using C = Bp<NBITS>;
+    constexpr int DB = BP_DB, W = C::W, TB = 32 * 32 * W, CC = C::CC, NP = C::NP, NSUB = C::NSUB;
+    constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
+    constexpr uint32_t STAGE_SUM = ((1u << NBITS) - 1u) * CC;        // largest value one stage adds to a counter
+    constexpr int NT = bit_length(STAGE_SUM);                        // pending slots
+    static_assert((CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
 
     extern __shared__ __align__(128) uint8_t smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -192,15 +378,15 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
     const int2 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans_pad;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + static_cast<int64_t>(blk) * p.nchans_pad * DB;
 
-    // producers: EVERY warp stages CPW = CC / NWARPS channels of each chunk (its lane 0 issues the bulk copies:
-    // a bulk copy takes its operands from uniform registers, so one warp issuing all 32 copies of a chunk
+    // producers: EVERY warp stages CPW = CC * NSUB / NWARPS sub-rows of each chunk (its lane 0 issues the bulk
+    // copies: a bulk copy takes its operands from uniform registers, so one warp issuing all copies of a chunk
     // serialises over its lanes and falls behind the others); warp 0 also stages the chunk's offset entries.
     // The span metadata of the next chunk to stage is fetched one step early.
-    constexpr int CPW = CC / BP_NWARPS;
+    constexpr int CPW = CC * NSUB / BP_NWARPS;
     auto load_meta = [&](int chunk, int2 (&m)[CPW]) {
 #pragma unroll
         for (int k = 0; k < CPW; ++k)
-            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + warp * CPW + k]) : make_int2(0, 0);
+            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int2(0, 0);
     };
     auto produce = [&](int chunk, const int2 (&m)[CPW]) {
         const int s = chunk % NS;
@@ -211,23 +397,26 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
             uint32_t bytes[CPW], tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
 #pragma unroll
             for (int k = 0; k < CPW; ++k) {
-                const int c = chunk * CC + warp * CPW + k;
+                const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
+                const int c = chunk * CC + cl;
                 if (m[k].y < 0) {                                // padded channel: zeros
                     src[k] = p.zero;
                     bytes[k] = static_cast<uint32_t>(-m[k].y);
                 } else {
-                    const int64_t off = ((t0 + m[k].x) * 2) >> 3;
+                    const int64_t off = ((t0 + m[k].x) >> 5) * UB;
                     const int64_t avail = p.in_row_bytes - off;
                     bytes[k] = static_cast<uint32_t>(m[k].y < avail ? m[k].y : (avail > 0 ? avail : 0));
-                    src[k] = in_beam + static_cast<int64_t>(c) * p.in_stride + off;
+                    src[k] = in_beam + static_cast<int64_t>(c) * p.in_stride + sub * p.in_row_bytes + off;
                 }
                 tx += bytes[k];
             }
             mbar_arrive_expect_tx(&full[s], tx);
 #pragma unroll
-            for (int k = 0; k < CPW; ++k)
+            for (int k = 0; k < CPW; ++k) {
+                const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
                 if (bytes[k])
-                    tma_bulk_g2s(raw_base + s * raw_stage + (warp * CPW + k) * p.raw_slot, src[k], bytes[k], &full[s]);
+                    tma_bulk_g2s(raw_base + s * raw_stage + cl * p.raw_slot + sub * p.sub_slot, src[k], bytes[k], &full[s]);
+            }
             if (warp == 0)
                 tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(chunk) * CC * DB,
                              static_cast<uint32_t>(CC * DB * 8), &full[s]);
@@ -246,14 +435,14 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
             meta[i] = nxt[i];
     }
 
-    uint32_t P[W][NP], T[W][BP_NT];
+    uint32_t P[W][NP], T[W][NT];
 #pragma unroll
     for (int j = 0; j < W; ++j) {
 #pragma unroll
         for (int k = 0; k < NP; ++k)
             P[j][k] = 0;
 #pragma unroll
-        for (int k = 0; k < BP_NT; ++k)
+        for (int k = 0; k < NT; ++k)
             T[j][k] = 0;
     }
 
@@ -269,19 +458,20 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
         mbar_wait(&full[s], (chunk / NS) & 1);
 
         BpShared sh;
-        sh.lane_base = raw_base + s * raw_stage + lane * (W * 8);
+        sh.lane_base = raw_base + s * raw_stage + lane * (W * UB);
         sh.rel = reinterpret_cast<const uint2 *>(rel_base + s * rel_stage) + warp;
-        stage_steps(std::make_integer_sequence<int, CC>{}, sh, P, T);
+        sh.sub_slot = p.sub_slot;
+        stage_steps<NBITS>(std::make_integer_sequence<int, CC>{}, sh, P, T);
 #pragma unroll
         for (int j = 0; j < W; ++j)
-            csa_flush<BP_WSUM * CC, 0, false>(P[j], T[j], 0u);
+            csa_flush<STAGE_SUM, 0, false>(P[j], T[j], 0u);
 
         __syncwarp();
         if (lane == 0)
             mbar_arrive(&empty[s]);
     }
 
-    // ---- epilogue: thread owns samples t0 + 32*(5*lane + j) + [0, 32) of DM slot `warp`
+    // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp`
     const int d = blk * DB + warp;
     if (d >= p.ndm)
         return;
@@ -289,85 +479,53 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp2(const KernelP
     uint8_t *orow = p.out + static_cast<int64_t>(beam) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
 #pragma unroll
     for (int j = 0; j < W; ++j) {
-        // 16x16 bit-matrix transpose of both half-words at once: R[k] = {sum of sample 16+k, sum of sample k}
-        uint32_t R[16];
-#pragma unroll
-        for (int k = 0; k < 16; ++k)
-            R[k] = k < NP ? P[j][k] : 0u;
-#pragma unroll
-        for (int st = 0; st < 4; ++st) {
-            const int sh = 8 >> st;
-            const uint32_t m = st == 0 ? 0x00FF00FFu : st == 1 ? 0x0F0F0F0Fu : st == 2 ? 0x33333333u : 0x55555555u;
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                if (k & sh)
-                    continue;
-                const uint32_t t = ((R[k] >> sh) ^ R[k + sh]) & m;
-                R[k + sh] ^= t;
-                R[k] ^= t << sh;
-            }
-        }
         const int64_t tunit = t0 + 32 * (W * lane + j);
+        if constexpr (NP <= 16) {
+            uint32_t R[16];
 #pragma unroll
-        for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
-            const int64_t t = tunit + 4 * h;
-            if (t >= p.nsamps)
-                continue;
-            uint32_t q[4];
+            for (int k = 0; k < 16; ++k)
+                R[k] = k < NP ? P[j][k] : 0u;
+            transpose16x2(R);
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                q[k] = h < 4 ? (R[4 * h + k] & 0xFFFFu) : (R[4 * (h - 4) + k] >> 16);
-            const bool whole = p.vec_ok && (t + 4 <= p.nsamps);
-            if (p.out_code == DD_OUT_F32) {
-                float *o = reinterpret_cast<float *>(orow) + t;
-                if (whole) {
-                    *reinterpret_cast<float4 *>(o) = make_float4(__uint2float_rn(q[0]), __uint2float_rn(q[1]),
-                                                                 __uint2float_rn(q[2]), __uint2float_rn(q[3]));
-                } else {
+            for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
+                uint32_t q[4];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (t + k < p.nsamps)
-                            o[k] = __uint2float_rn(q[k]);
-                }
-            } else if (p.out_code == DD_OUT_U32) {
-                uint32_t *o = reinterpret_cast<uint32_t *>(orow) + t;
-                if (whole) {
-                    *reinterpret_cast<uint4 *>(o) = make_uint4(q[0], q[1], q[2], q[3]);
-                } else {
+                for (int k = 0; k < 4; ++k)
+                    q[k] = h < 4 ? (R[4 * h + k] & 0xFFFFu) : (R[4 * (h - 4) + k] >> 16);
+                store4(p, orow, tunit + 4 * h, q);
+            }
+        } else {
+            uint32_t R[32];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (t + k < p.nsamps)
-                            o[k] = q[k];
-                }
-            } else {
-                uint16_t *o = reinterpret_cast<uint16_t *>(orow) + t;
-                if (whole) {
-                    *reinterpret_cast<uint2 *>(o) = make_uint2(q[0] | (q[1] << 16), q[2] | (q[3] << 16));
-                } else {
+            for (int k = 0; k < 32; ++k)
+                R[k] = k < NP ? P[j][k] : 0u;
+            transpose32(R);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (t + k < p.nsamps)
-                            o[k] = static_cast<uint16_t>(q[k]);
-                }
+            for (int h = 0; h < 8; ++h) {
+                const uint32_t q[4] = {R[4 * h], R[4 * h + 1], R[4 * h + 2], R[4 * h + 3]};
+                store4(p, orow, tunit + 4 * h, q);
             }
         }
     }
 }
 
-}  // namespace
-
-// Two launches: the bit-plane transpose of the rows the tiles will read, then the dedispersion kernel.
-cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
+template <int NBITS>
+cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
 {
-    if (plan->nbits != 2 || !plan->var.bitplane || plan->cc != BP_CC)
+    using C = Bp<NBITS>;
+    constexpr int TB = 32 * 32 * C::W;
+    if (plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB)
         return cudaErrorInvalidValue;
     KernelParams kp = kp_in;
-    // bytes of every row the tiles can touch, rounded to the 16-byte conversion unit
-    int64_t conv = ((static_cast<int64_t>(kp.ntiles - 1) * BP_TB + plan->max_span_end) * 2 + 7) / 8;
-    conv = (conv + 15) / 16 * 16;
-    if (conv > kp.in_row_bytes)
-        conv = kp.in_row_bytes / 16 * 16;
-    const size_t need = static_cast<size_t>(kp.nbeams) * kp.nchans * static_cast<size_t>(conv);
+    // 16-byte groups of every sub-row the tiles can touch (2 units of 2-bit input, 1 unit otherwise)
+    const int64_t spg = (16 / (C::NB * 4)) * 32;   // samples per group
+    int64_t groups = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
+    const int64_t in_bytes_per_group = spg * NBITS / 8;
+    const int64_t have = (kp.in_row_bytes + in_bytes_per_group - 1) / in_bytes_per_group;
+    if (groups > have)
+        groups = have;
+    const int64_t conv = groups * 16;   // bytes per sub-row
+    const size_t need = static_cast<size_t>(kp.nbeams) * kp.nchans * C::NSUB * static_cast<size_t>(conv);
     cudaError_t e;
     if (plan->work_bytes < need) {
         if (plan->d_work)
@@ -378,27 +536,45 @@ cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp_in, cudaStre
             return e;
         plan->work_bytes = need;
     }
-    const int chunks = static_cast<int>(conv / 16);
-    dd_to_bitplanes2<<<dim3((chunks + 255) / 256, kp.nchans, kp.nbeams), 256, 0, stream>>>(
-        kp.in, kp.in_stride, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv,
-        static_cast<int64_t>(kp.nchans) * conv, chunks);
+    const int64_t w_beam = static_cast<int64_t>(kp.nchans) * C::NSUB * conv;
+    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups + 255) / 256), kp.nchans, kp.nbeams), 256, 0, stream>>>(
+        kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv, w_beam,
+        static_cast<int32_t>(groups));
     if ((e = cudaGetLastError()) != cudaSuccess)
         return e;
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     kp.in = static_cast<const uint8_t *>(plan->d_work);
-    kp.in_stride = conv;
+    kp.in_stride = C::NSUB * conv;   // between channels; sub-rows are in_row_bytes apart
     kp.in_row_bytes = conv;
-    kp.in_beam_stride = static_cast<int64_t>(kp.nchans) * conv;
+    kp.in_beam_stride = w_beam;
 
-    e = cudaFuncSetAttribute(dd_direct_bp2, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
+    e = cudaFuncSetAttribute(dd_direct_bp<NBITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)
         return e;
     const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
-    dd_direct_bp2<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
+    dd_direct_bp<NBITS><<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
     return cudaGetLastError();
+}
+
+}  // namespace
+
+// Two launches: the bit-plane transpose of the rows the tiles will read, then the dedispersion kernel.
+cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
+{
+    if (!plan->var.bitplane)
+        return cudaErrorInvalidValue;
+    switch (plan->nbits) {
+    case 2:
+        return launch_bp<2>(plan, kp, stream);
+    case 4:
+        return launch_bp<4>(plan, kp, stream);
+    case 8:
+        return launch_bp<8>(plan, kp, stream);
+    }
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace dd

@@ -21,6 +21,7 @@ struct KernelParams {
     int32_t nchans, ndm, nblk, ntiles, nbeams;
     int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
     int32_t raw_slot, lane_slot;
+    int32_t sub_slot;         // bit planes: bytes per sub-row inside a channel slot
     int32_t nstages;          // ring depth of the staged buffers (bit-plane variant)
     int32_t nchans_pad;       // channels iterated over: nchans padded to a multiple of cc (bit-plane variant)
     const uint8_t *zero;      // raw_slot zero bytes: the span of a padded channel

@@ -56,9 +56,12 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 // The kernel variants compiled into the library, in order of preference.
 static const Variant kVariants[] = {
     /* id  DB   TB    thr tail rel lane lst rst  cc candidates     nbits                        sum  pad    bitplane */
-    {3, 16, 5120, 512, 32, 8, 2, 0, 4, {32, 0, 0, 0}, 1 << 2, 12, true, true},                     // 2-bit, bit planes + carry-save
-    {2, 32, 1280, 512, 8, 4, 4, 2, 2, {40, 20, 10, 5}, 1 << 2, 16, false, false},                  // 2-bit, nibble lanes
-    {1, 32, 640, 256, 4, 2, 8, 1, 2, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), 32, false, false},
+    // bit planes + carry-save counters (dd_kernel_bp.cu): tile shapes must match Bp<nbits> there
+    {3, 16, 5120, 512, 32, 8, 2, 0, 4, {32, 0, 0, 0}, 1 << 2, 12, true, true, 8, 1},               // 2-bit: 2 planes, W = 5
+    {3, 16, 3072, 512, 32, 8, 4, 0, 4, {16, 0, 0, 0}, 1 << 4, 16, true, true, 16, 1},              // 4-bit: 4 planes, W = 3
+    {3, 16, 3072, 512, 32, 8, 8, 0, 4, {8, 0, 0, 0}, 1 << 8, 20, true, true, 16, 2},               // 8-bit: 2 x 4 planes, W = 3
+    {2, 32, 1280, 512, 8, 4, 4, 2, 2, {40, 20, 10, 5}, 1 << 2, 16, false, false, 0, 1},            // 2-bit, nibble lanes
+    {1, 32, 640, 256, 4, 2, 8, 1, 2, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), 32, false, false, 0, 1},
 };
 
 dd_status build_tiles(dd_plan_s *p)
@@ -67,9 +70,10 @@ dd_status build_tiles(dd_plan_s *p)
     const int64_t vmax = (1 << nbits) - 1;
     const int64_t top = static_cast<int64_t>(nchans) * vmax;   // largest possible sum
     p->final32 = top > 65535;
-    const int A = 128 / nbits;   // samples per 16 packed bytes: bulk-copy granularity
 
     for (const Variant &v : kVariants) {
+        // samples per 16 staged bytes (the bulk-copy granularity): of the packed row, or of a bit-plane sub-row
+        const int A = v.bitplane ? (16 / v.unit_bytes) * 32 : 128 / nbits;
         if (!(v.nbits_mask & (1 << nbits)) || (v.max_sum_bits < 32 && top >= (int64_t(1) << v.max_sum_bits)))
             continue;
         if (p->force_variant && v.id != p->force_variant)
@@ -94,7 +98,8 @@ dd_status build_tiles(dd_plan_s *p)
                 }
                 const int32_t start = dmin / A * A;
                 const int64_t need = static_cast<int64_t>(v.TB) + (dmax - start) + v.tail;
-                const int64_t nbytes = align_up(need, A) * nbits / 8;
+                const int64_t nbytes = v.bitplane ? align_up(need, A) / 32 * v.unit_bytes   // per sub-row
+                                                  : align_up(need, A) * nbits / 8;
                 if (dmax - start > rel_limit || nbytes > (1 << 19)) {
                     ok = false;
                     break;
@@ -103,13 +108,14 @@ dd_status build_tiles(dd_plan_s *p)
                 m.start = start;
                 m.nbytes = static_cast<int32_t>(nbytes);
                 max_bytes = std::max(max_bytes, nbytes);
-                max_end = std::max(max_end, start + nbytes * 8 / nbits);
+                max_end = std::max(max_end, start + (v.bitplane ? nbytes / v.unit_bytes * 32 : nbytes * 8 / nbits));
             }
         }
         if (!ok)
             continue;
         p->max_span_end = max_end;
-        p->raw_slot = static_cast<int>(max_bytes);
+        p->sub_slot = static_cast<int>(max_bytes);
+        p->raw_slot = static_cast<int>(max_bytes) * v.nsub;
         p->lane_slot = static_cast<int>(max_bytes * v.lane_bits / nbits);
         int cc = 0;
         for (p->nstages = v.raw_stages; p->nstages >= 2 && cc == 0; --p->nstages) {   // deepest ring that fits
@@ -139,7 +145,7 @@ dd_status build_tiles(dd_plan_s *p)
                 const uint32_t slot_off = static_cast<uint32_t>(c % cc) * static_cast<uint32_t>(p->raw_slot);
                 if (c >= nchans) {   // padded channel: a whole slot of zeros, every window at its start
                     m.start = 0;
-                    m.nbytes = -p->raw_slot;   // negative: stage from the zero buffer
+                    m.nbytes = -(v.bitplane ? p->sub_slot : p->raw_slot);   // negative: stage from the zero buffer
                     for (int i = 0; i < DB; ++i) {
                         uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
                         e[0] = slot_off;
@@ -157,7 +163,7 @@ dd_status build_tiles(dd_plan_s *p)
                         reinterpret_cast<uint32_t *>(rel.data())[base + i] = off * 4u;
                     } else {   // bit planes: 32 samples per group of nbits words
                         uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
-                        e[0] = slot_off + (off >> 5) * 4u * static_cast<uint32_t>(nbits);
+                        e[0] = slot_off + (off >> 5) * static_cast<uint32_t>(v.unit_bytes);
                         e[1] = off & 31u;
                     }
                 }

@@ -32,6 +32,8 @@ struct Variant {
     bool pad_chunks;  // the kernel always processes whole stages: the channel list is padded to a multiple
                       // of cc with all-zero channels (their spans are staged from a zeroed device buffer)
     bool bitplane;    // stages hold bit planes produced by the transpose pre-pass (dd_kernel_bp.cu)
+    int unit_bytes;   // bit planes: bytes per 32-sample unit of a sub-row (4 * planes per sub-row); else 0
+    int nsub;         // bit planes: sub-rows per channel (nbits / planes per sub-row); else 1
 };
 
 struct SpanMeta {   // per (DM block, channel); mirrored on the device as int2
@@ -65,6 +67,7 @@ struct dd_plan_s {
     int nstages = 2;       // ring depth of the staged buffers (<= var.raw_stages)
     int64_t max_span_end = 0;   // max over spans of start + staged samples: how far past a tile's t0 a copy reaches
     int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
+    int sub_slot = 0;      // bit planes: bytes per sub-row inside a channel slot (raw_slot / nsub)
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)

@@ -108,29 +108,64 @@ def test_cfg2_high_dm_end(variant):
     _full_compare(cfg, dms=W.CONFIGS[2].dm_list()[-40:], out_kinds=["f32", "u16"], variant=variant)
 
 
-def test_cfg3_reduced_8bit_4096_channels():
-    _full_compare(W.CONFIGS[3].reduced(nsamps=1300, ndm=33))
+@pytest.mark.parametrize("variant", [1, 3])
+def test_cfg3_reduced_8bit_4096_channels(variant):
+    _full_compare(W.CONFIGS[3].reduced(nsamps=1300, ndm=33), variant=variant)
 
 
-def test_cfg3_high_dm_end_large_spread():
+@pytest.mark.parametrize("variant", [1, 3])
+def test_cfg3_high_dm_end_large_spread(variant):
     cfg = W.CONFIGS[3].reduced(nsamps=700, ndm=32)
-    _full_compare(cfg, dms=W.CONFIGS[3].dm_list()[-32:])
+    _full_compare(cfg, dms=W.CONFIGS[3].dm_list()[-32:], variant=variant)
 
 
-def test_cfg4_reduced_4bit_u16():
-    _full_compare(W.CONFIGS[4].reduced(nsamps=2000, ndm=65), out_kinds=["u16", "u32", "f32"])
+@pytest.mark.parametrize("variant", [1, 3])
+def test_cfg4_reduced_4bit_u16(variant):
+    _full_compare(W.CONFIGS[4].reduced(nsamps=2000, ndm=65), out_kinds=["u16", "u32", "f32"], variant=variant)
 
 
-def test_cfg5_reduced_batch_of_beams():
-    _full_compare(W.CONFIGS[5].reduced(nsamps=1000, ndm=40, nbeams=3))
+@pytest.mark.parametrize("variant", [1, 3])
+def test_cfg5_reduced_batch_of_beams(variant):
+    _full_compare(W.CONFIGS[5].reduced(nsamps=1000, ndm=40, nbeams=3), variant=variant)
 
 
+@pytest.mark.parametrize("nbits", [4, 8])
+def test_variant3_bitplane_4_and_8_bit_tiles_and_channel_padding(nbits):
+    # bit-plane kernel, 4 planes per sub-row: 3072-sample tiles (2 tiles + ragged tail), 16-DM blocks (ragged),
+    # all output types; channel counts around the stage size (16 / 8 channels, padded with zero channels) and the
+    # ring depth; nsamps chosen so that 8-bit rows end in a half unit (16 bytes)
+    base = W.CONFIGS[{4: 4, 8: 5}[nbits]]
+    _full_compare(base.reduced(nsamps=2 * 3072 + 333, ndm=37, nchans=96), out_kinds=["f32", "u32", "u16"], variant=3)
+    for nchans in (1, 7, 8, 9, 15, 16, 17, 33, 63, 65, 257):
+        _full_compare(base.reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=3)
+    _full_compare(base.reduced(nsamps=3072 + 8, ndm=2, nchans=5), out_kinds=["u32"], variant=3)
+
+
+@pytest.mark.parametrize("nbits", [4, 8])
+def test_variant3_bitplane_4_and_8_bit_extreme_values(nbits):
+    # every sample at its maximum with the largest channel count the planes hold: 4369 * 15 = 65535 (all 16
+    # planes set); 4112 * 255 = 1048560 (the top of the 20-plane range); and all zero
+    nchans = {4: 4369, 8: 4112}[nbits]
+    base = W.CONFIGS[{4: 4, 8: 3}[nbits]]
+    cfg = W.Config(name="extreme", index=base.index, nchans=nchans, f_top=base.f_top, df=-100.0 / nchans, dt=base.dt,
+                   nbits=nbits, nsamps=700, ndm=5, dm_max=20.0, out="u32", dist="uniform", seed=7)
+    tab = _oracle_table(cfg)
+    nbytes = ((cfg.nsamps + int(tab.max())) * nbits + 7) // 8
+    stride = (nbytes + 15) // 16 * 16
+    for fill, want in ((0xFF, nchans * ((1 << nbits) - 1)), (0x00, 0)):
+        packed = torch.full((1, cfg.nchans, stride), fill, dtype=torch.uint8)
+        got = _gpu_transform(cfg, packed.cuda(), stride, cfg.dm_list(), "u32", cfg.nsamps, 3)
+        ref = oracle.dedisperse(packed[0].numpy(), nbits, cfg.nsamps, tab)
+        assert np.array_equal(got[0], ref) and int(ref.max()) == want and int(ref.min()) == want
+
+
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("nbits", [2, 4, 8])
-def test_odd_shapes(nbits):
+def test_odd_shapes(nbits, variant):
     # channel count not a multiple of the stage size, one DM, tiny nsamps, more channels than a flush interval
     base = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
     for nchans, ndm, nsamps in ((1, 1, 1), (37, 5, 13), (300, 33, 641), (1024, 2, 5)):
-        _full_compare(base.reduced(nsamps=nsamps, ndm=ndm, nchans=nchans), out_kinds=["u32"])
+        _full_compare(base.reduced(nsamps=nsamps, ndm=ndm, nchans=nchans), out_kinds=["u32"], variant=variant)
 
 
 def test_unsorted_dm_list():
@@ -165,6 +200,20 @@ def test_execute_host_matches_oracle():
 def test_execute_host_bitplane_variant_two_slabs():
     # 2-bit through the host-buffer path: 140000 output samples = two time slabs (133120 + ragged rest)
     cfg = W.CONFIGS[2].reduced(nsamps=140000, ndm=9, nchans=64)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    ref = oracle.cast_out(oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab), "f32")
+    out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
+        assert p.launch_info()["last_launches"] == 4
+    assert np.array_equal(out.numpy(), ref)
+
+
+def test_execute_host_bitplane_8bit_two_slabs():
+    # 8-bit through the host-buffer path: two time slabs, rows ending in a half unit
+    cfg = W.CONFIGS[5].reduced(nsamps=140008, ndm=5, nchans=24)
     tab = _oracle_table(cfg)
     packed, stride = W.gen_packed(cfg, int(tab.max()))
     ref = oracle.cast_out(oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab), "f32")
