@@ -86,6 +86,19 @@ dd_status dd_plan_destroy(dd_plan plan);
  */
 dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm);
 
+/*
+ * dd_set_killmask -- the channel "kill mask" of PAPER.md:113: which frequency channels are included in the sum
+ * and which are skipped (e.g. channels with radio-frequency interference).  With a mask,
+ *     D[d][t] = sum over channels c with mask[c] != 0 of A[c][t + delay[d][c]]
+ * i.e. the paper's arithmetic form `sum += data * kill_mask[channel]` with a 0/1 mask.
+ *   mask  HOST, nchans int32 (copied): nonzero = summed, 0 = skipped.  NULL removes the mask (all channels summed).
+ * May be called before or after dd_set_dm_list; with a DM list present the tile metadata is rebuilt over the
+ * surviving channels at once (they are skipped entirely: no copy, no add), and on error the plan is unchanged.
+ * The delay table and dd_get_max_delay still cover all channels, and so does the input-row length check of
+ * dd_execute; the output-range check counts only the summed channels.  With every channel masked the output is zero.
+ */
+dd_status dd_set_killmask(dd_plan plan, const int32_t *mask);
+
 /* Copies the delay table to `table` (HOST, ndm*nchans int32, row-major [d][c]).  Host only. */
 dd_status dd_get_delay_table(dd_plan plan, int32_t *table);
 
@@ -133,7 +146,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
 
 /*
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
- *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel.
+ *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
+ *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20).
  * Takes effect at the next dd_set_dm_list (which returns DD_ERR_SMEM if that variant cannot serve the plan).
  */
 dd_status dd_set_kernel_variant(dd_plan plan, int variant);

@@ -11,7 +11,7 @@ Contents
   oracle_np.py         a second, independent numpy formulation + per-point evaluation
   this file            ctypes wrapper around the C library + the O6 cast
 
-Parity status: all functions pinned (tests/test_oracle_pins.py, pins P1..P11 in DESIGN.md §3).
+Parity status: all functions pinned (tests/test_oracle_pins.py, pins P1..P12 in DESIGN.md §3).
 """
 from __future__ import annotations
 
@@ -41,9 +41,9 @@ def lib() -> ctypes.CDLL:
         L.oracle_unpack_row.restype = None
         L.oracle_threads.argtypes = [i32]
         L.oracle_threads.restype = i32
-        L.oracle_dedisperse_unpacked.argtypes = [i32, i64, vp, i64, i32, vp, vp, i32]
+        L.oracle_dedisperse_unpacked.argtypes = [i32, i64, vp, i64, i32, vp, vp, vp, i32]
         L.oracle_dedisperse_unpacked.restype = i32
-        L.oracle_dedisperse.argtypes = [i32, i64, i32, vp, i64, i32, vp, vp, i32]
+        L.oracle_dedisperse.argtypes = [i32, i64, i32, vp, i64, i32, vp, vp, vp, i32]
         L.oracle_dedisperse.restype = i32
         _LIB = L
     return _LIB
@@ -80,28 +80,41 @@ def unpack(packed_rows: np.ndarray, nbits: int, nsamp: int) -> np.ndarray:
     return out
 
 
-def dedisperse(packed: np.ndarray, nbits: int, nsamps: int, delays: np.ndarray, nthreads: int = 0) -> np.ndarray:
-    """O4+O5 (eq. 3) for one beam: packed uint8 [nchans][stride] -> uint32 [ndm][nsamps]."""
+def _mask_arg(mask, nchans: int):
+    """O7: None, or nchans values, nonzero = channel kept."""
+    if mask is None:
+        return None, None
+    m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.int32)
+    assert m.shape == (nchans,)
+    return m, _ptr(m)
+
+
+def dedisperse(packed: np.ndarray, nbits: int, nsamps: int, delays: np.ndarray, nthreads: int = 0,
+               mask=None) -> np.ndarray:
+    """O4+O5 (eq. 3) for one beam: packed uint8 [nchans][stride] -> uint32 [ndm][nsamps].
+    `mask` (optional): the channel kill mask of PAPER.md:113, nonzero = channel summed (O7)."""
     p = np.ascontiguousarray(packed, dtype=np.uint8)
     dl = np.ascontiguousarray(delays, dtype=np.int64)
     nchans, stride = p.shape
     assert dl.ndim == 2 and dl.shape[1] == nchans
     out = np.empty((dl.shape[0], nsamps), dtype=np.uint32)
-    rc = lib().oracle_dedisperse(nchans, nsamps, nbits, _ptr(p), stride, dl.shape[0], _ptr(dl), _ptr(out),
+    m, mp = _mask_arg(mask, nchans)
+    rc = lib().oracle_dedisperse(nchans, nsamps, nbits, _ptr(p), stride, dl.shape[0], _ptr(dl), mp, _ptr(out),
                                  int(nthreads))
     if rc != 0:
         raise ValueError(f"oracle_dedisperse rc={rc}")
     return out
 
 
-def dedisperse_unpacked(a: np.ndarray, nsamps: int, delays: np.ndarray, nthreads: int = 0) -> np.ndarray:
+def dedisperse_unpacked(a: np.ndarray, nsamps: int, delays: np.ndarray, nthreads: int = 0, mask=None) -> np.ndarray:
     """O5 on already unpacked samples a uint8 [nchans][a_len] -> uint32 [ndm][nsamps]."""
     a = np.ascontiguousarray(a, dtype=np.uint8)
     dl = np.ascontiguousarray(delays, dtype=np.int64)
     nchans, a_len = a.shape
     assert dl.ndim == 2 and dl.shape[1] == nchans
     out = np.empty((dl.shape[0], nsamps), dtype=np.uint32)
-    rc = lib().oracle_dedisperse_unpacked(nchans, nsamps, _ptr(a), a_len, dl.shape[0], _ptr(dl), _ptr(out),
+    m, mp = _mask_arg(mask, nchans)
+    rc = lib().oracle_dedisperse_unpacked(nchans, nsamps, _ptr(a), a_len, dl.shape[0], _ptr(dl), mp, _ptr(out),
                                           int(nthreads))
     if rc != 0:
         raise ValueError(f"oracle_dedisperse_unpacked rc={rc}")

@@ -15,6 +15,8 @@
  *   O4  a[c][t]     = sample t of packed row c                      PAPER.md:101 (sub-word samples, shift and mask)
  *   O5  out[d][t]   = sum_{c=0}^{nchans-1} a[c][t + delay[d][c]]    PAPER.md:57-60 (eq. 3; sum_i^N means i=0..N-1)
  *   O6  cast to the requested output type (value preserving)        done by the Python wrapper, which asserts it fits
+ *   O7  channel kill mask, applied arithmetically:                  PAPER.md:113 ("sum += data * kill_mask[channel]")
+ *       out[d][t] = sum_c a[c][t + delay[d][c]] * mask[c],  mask[c] in {0, 1};  no mask = all ones
  *
  * K = k_DM = 4.148808e3 MHz^2 pc^-1 cm^3 s, frequencies in MHz, dt in seconds,
  * DM in pc cm^-3, all floating point in double (fp64).
@@ -85,9 +87,10 @@ int oracle_threads(int nthreads)
 
 /* O5 on unpacked samples a[c][t] (row length a_len >= nsamps + max delay), for the ndm rows of
  * `delay` ([ndm][nchans], int64).  out is [ndm][nsamps] uint32, overwritten.
+ * mask: NULL, or nchans ints, nonzero = channel kept (O7).
  * Returns 0; -1 bad argument; -2 a delay is negative or reaches past a_len. */
 int oracle_dedisperse_unpacked(int nchans, int64_t nsamps, const uint8_t *a, int64_t a_len, int ndm,
-                               const int64_t *delay, uint32_t *out, int nthreads)
+                               const int64_t *delay, const int32_t *mask, uint32_t *out, int nthreads)
 {
     if (nchans <= 0 || nsamps <= 0 || ndm <= 0 || !a || !delay || !out)
         return -1;
@@ -102,8 +105,9 @@ int oracle_dedisperse_unpacked(int nchans, int64_t nsamps, const uint8_t *a, int
         memset(row, 0, (size_t)nsamps * sizeof(uint32_t));
         for (int c = 0; c < nchans; ++c) {
             const uint8_t *src = a + (size_t)c * (size_t)a_len + delay[(size_t)d * nchans + c];
+            const uint32_t keep = (mask == NULL || mask[c] != 0) ? 1u : 0u;
             for (int64_t t = 0; t < nsamps; ++t)
-                row[t] += src[t];                                                    /* O5 */
+                row[t] += src[t] * keep;                                             /* O5, O7 */
         }
     }
     return 0;
@@ -112,7 +116,7 @@ int oracle_dedisperse_unpacked(int nchans, int64_t nsamps, const uint8_t *a, int
 /* O4 + O5 from the packed input in[c] (rows in_stride bytes apart, each holding at least
  * nsamps + max delay samples).  out as above.  -3 = out of memory, -4 = row too short. */
 int oracle_dedisperse(int nchans, int64_t nsamps, int nbits, const uint8_t *in, int64_t in_stride,
-                      int ndm, const int64_t *delay, uint32_t *out, int nthreads)
+                      int ndm, const int64_t *delay, const int32_t *mask, uint32_t *out, int nthreads)
 {
     if (nchans <= 0 || nsamps <= 0 || ndm <= 0 || !in || !delay || !out)
         return -1;
@@ -133,7 +137,7 @@ int oracle_dedisperse(int nchans, int64_t nsamps, int nbits, const uint8_t *in, 
         return -3;
     for (int c = 0; c < nchans; ++c)                                                  /* O4 */
         oracle_unpack_row(in + (size_t)c * (size_t)in_stride, nbits, a_len, a + (size_t)c * (size_t)a_len);
-    int rc = oracle_dedisperse_unpacked(nchans, nsamps, a, a_len, ndm, delay, out, nthreads);
+    int rc = oracle_dedisperse_unpacked(nchans, nsamps, a, a_len, ndm, delay, mask, out, nthreads);
     free(a);
     return rc;
 }

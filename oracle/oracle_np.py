@@ -58,11 +58,12 @@ def dedisperse_loops_py(a, delays, nsamps: int):
 
 
 def dedisperse_points(sample_fn: Callable[[np.ndarray, np.ndarray], np.ndarray], delays: np.ndarray,
-                      d_idx, t_idx) -> np.ndarray:
+                      d_idx, t_idx, mask=None) -> np.ndarray:
     """out[d_i][t_i] = sum_c sample_fn(c, t_i + delay[d_i][c]) for a list of (d_i, t_i) (eq. 3, one output at a time).
 
     `delays` is the full table [ndm][nchans]; `sample_fn(c, t)` returns the unpacked input values
-    at integer arrays (c, t) of equal shape.
+    at integer arrays (c, t) of equal shape.  `mask` (optional, nchans values): the kill mask of PAPER.md:113,
+    applied as the paper states it, by multiplication with 0 or 1.
     """
     d_idx = np.asarray(d_idx, dtype=np.int64)
     t_idx = np.asarray(t_idx, dtype=np.int64)
@@ -71,4 +72,6 @@ def dedisperse_points(sample_fn: Callable[[np.ndarray, np.ndarray], np.ndarray],
     c = np.broadcast_to(np.arange(nchans, dtype=np.int64)[None, :], rows.shape)
     t = t_idx[:, None] + rows
     v = np.asarray(sample_fn(c, t)).astype(np.int64)
+    if mask is not None:
+        v = v * (np.asarray(mask) != 0).astype(np.int64)[None, :]
     return v.sum(axis=1)

@@ -19,7 +19,7 @@ import numpy as np
 __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_set_batch", "dd_set_killmask", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
@@ -29,7 +29,7 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 # every symbol include/dd.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_set_batch", "dd_set_killmask", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
 )
 
@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.dd_get_max_delay.argtypes = [vp]
         L.dd_get_max_delay.restype = i64
         L.dd_set_batch.argtypes = [vp, i32, i64, i64]
+        L.dd_set_killmask.argtypes = [vp, vp]
         L.dd_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
         L.dd_get_launch_info.argtypes = [vp, vp]
@@ -85,7 +86,7 @@ def lib() -> ctypes.CDLL:
         L.dd_last_cuda_error.argtypes = []
         L.dd_last_cuda_error.restype = ctypes.c_char_p
         for name in ("dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_set_batch",
-                     "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak", "dd_set_kernel_variant",
+                     "dd_set_killmask", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak", "dd_set_kernel_variant",
                      "dd_profile_enable", "dd_profile_read"):
             getattr(L, name).restype = i32
         _LIB = L
@@ -159,6 +160,15 @@ def dd_set_batch(plan: int, nbeams: int, in_beam_stride: int, out_beam_stride: i
     _check(lib().dd_set_batch(plan, int(nbeams), int(in_beam_stride), int(out_beam_stride)), "dd_set_batch")
 
 
+def dd_set_killmask(plan: int, mask) -> None:
+    """mask: nchans values, nonzero = channel summed, 0 = skipped; None removes the mask."""
+    if mask is None:
+        _check(lib().dd_set_killmask(plan, None), "dd_set_killmask")
+        return
+    m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.int32)
+    _check(lib().dd_set_killmask(plan, ctypes.c_void_p(m.ctypes.data)), "dd_set_killmask")
+
+
 def dd_execute(plan: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbits: int, stream=None) -> None:
     """Asynchronous; in_ptr/out_ptr are DEVICE buffers (tensors or addresses)."""
     _check(lib().dd_execute(plan, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits),
@@ -222,6 +232,12 @@ class Plan:
 
     def set_batch(self, nbeams: int, in_beam_stride: int, out_beam_stride: int) -> "Plan":
         dd_set_batch(self.handle, nbeams, in_beam_stride, out_beam_stride)
+        return self
+
+    def set_killmask(self, mask) -> "Plan":
+        if mask is not None and len(mask) != self.nchans:
+            raise ValueError("kill mask must have nchans entries")
+        dd_set_killmask(self.handle, mask)
         return self
 
     @property

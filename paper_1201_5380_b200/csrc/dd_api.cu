@@ -3,6 +3,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include <cuda_runtime.h>
 
@@ -133,7 +134,7 @@ static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_st
     const int64_t need_bits_hi = (nsamps + p->max_delay);
     if (need_bits_hi > (INT64_MAX / 8) || in_stride > INT64_MAX / 8 || in_stride * 8 < need_bits_hi * p->nbits)
         return DD_ERR_STRIDE_TOO_SMALL;
-    const int64_t vmax = (1 << p->nbits) - 1, top = static_cast<int64_t>(p->nchans) * vmax;
+    const int64_t vmax = (1 << p->nbits) - 1, top = static_cast<int64_t>(p->nlive) * vmax;   // over the summed channels
     if ((out_nbits == DD_OUT_U16 && top > 65535) || (out_nbits == DD_OUT_F32 && top >= (1 << 24)))
         return DD_ERR_OUT_RANGE;
     if (nsamps > (INT64_MAX / 8) / p->ndm)
@@ -157,22 +158,77 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     const int vec_bytes = 4 * es;
     kp.vec_ok = (nsamps % 4 == 0) && (reinterpret_cast<uintptr_t>(out) % vec_bytes == 0) &&
                 (out_beam_stride % vec_bytes == 0);
-    kp.nchans = p->nchans;
+    kp.nchans = p->nlive;
+    kp.nrows = p->nchans;
     kp.ndm = p->ndm;
     kp.nblk = p->nblk;
     kp.ntiles = static_cast<int32_t>((nsamps + p->var.TB - 1) / p->var.TB);
     kp.nbeams = nbeams;
     kp.cc = p->cc;
-    kp.nchunks = (p->nchans + p->cc - 1) / p->cc;
+    kp.nchunks = (p->nlive + p->cc - 1) / p->cc;
     kp.raw_slot = p->raw_slot;
     kp.lane_slot = p->lane_slot;
     kp.sub_slot = p->sub_slot;
     kp.nstages = p->nstages;
     kp.nchans_pad = p->nchans_pad;
     kp.zero = static_cast<const uint8_t *>(p->d_zero);
-    kp.span = static_cast<const int2 *>(p->d_span);
+    kp.span = static_cast<const int4 *>(p->d_span);
     kp.rel = p->d_rel;
     return kp;
+}
+
+// Rebuilds delay table and tile metadata for (DM list, kill mask) into a scratch plan, then commits: a failure
+// leaves the plan unchanged.  Uploads the tables when a device exists.
+static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uint8_t> keep)
+{
+    dd_plan_s scratch;
+    scratch.nchans = plan->nchans;
+    scratch.dt = plan->dt;
+    scratch.f_top = plan->f_top;
+    scratch.df = plan->df;
+    scratch.nbits = plan->nbits;
+    scratch.ndm = static_cast<int>(dm.size());
+    scratch.force_variant = plan->force_variant;
+    scratch.dm.swap(dm);
+    scratch.keep.swap(keep);
+    dd_status st = compute_delay_table(&scratch);
+    if (st != DD_OK)
+        return st;
+    st = build_tiles(&scratch);
+    if (st != DD_OK)
+        return st;
+    free_device_tables(plan);
+    plan->ndm = scratch.ndm;
+    plan->dm.swap(scratch.dm);
+    plan->keep.swap(scratch.keep);
+    plan->live.swap(scratch.live);
+    plan->nlive = scratch.nlive;
+    plan->delay.swap(scratch.delay);
+    plan->max_delay = scratch.max_delay;
+    plan->var = scratch.var;
+    plan->nblk = scratch.nblk;
+    plan->cc = scratch.cc;
+    plan->nchans_pad = scratch.nchans_pad;
+    plan->nstages = scratch.nstages;
+    plan->max_span_end = scratch.max_span_end;
+    plan->raw_slot = scratch.raw_slot;
+    plan->sub_slot = scratch.sub_slot;
+    plan->lane_slot = scratch.lane_slot;
+    plan->smem_bytes = scratch.smem_bytes;
+    plan->final32 = scratch.final32;
+    plan->span.swap(scratch.span);
+    plan->rel.swap(scratch.rel);
+    plan->last_launches = 0;
+    // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
+        st = upload_tables(plan);
+        if (st != DD_OK)
+            return st;
+    } else {
+        (void)cudaGetLastError();
+    }
+    return DD_OK;
 }
 
 }  // namespace dd
@@ -225,55 +281,32 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
     for (int d = 0; d < ndm; ++d)
         if (!std::isfinite(dm_list[d]) || dm_list[d] < 0.0)
             return DD_ERR_INVALID_ARG;
-    // build into a scratch copy so that a failure leaves the plan unchanged
-    dd_plan_s scratch;
-    scratch.nchans = plan->nchans;
-    scratch.dt = plan->dt;
-    scratch.f_top = plan->f_top;
-    scratch.df = plan->df;
-    scratch.nbits = plan->nbits;
-    scratch.ndm = ndm;
-    scratch.force_variant = plan->force_variant;
     try {
-        scratch.dm.assign(dm_list, dm_list + ndm);
-        dd_status st = compute_delay_table(&scratch);
-        if (st != DD_OK)
-            return st;
-        st = build_tiles(&scratch);
-        if (st != DD_OK)
-            return st;
+        return replan(plan, std::vector<double>(dm_list, dm_list + ndm), plan->keep);
     } catch (const std::bad_alloc &) {
         return DD_ERR_NOMEM;
     }
-    free_device_tables(plan);
-    plan->ndm = ndm;
-    plan->dm.swap(scratch.dm);
-    plan->delay.swap(scratch.delay);
-    plan->max_delay = scratch.max_delay;
-    plan->var = scratch.var;
-    plan->nblk = scratch.nblk;
-    plan->cc = scratch.cc;
-    plan->nchans_pad = scratch.nchans_pad;
-    plan->nstages = scratch.nstages;
-    plan->max_span_end = scratch.max_span_end;
-    plan->raw_slot = scratch.raw_slot;
-    plan->sub_slot = scratch.sub_slot;
-    plan->lane_slot = scratch.lane_slot;
-    plan->smem_bytes = scratch.smem_bytes;
-    plan->final32 = scratch.final32;
-    plan->span.swap(scratch.span);
-    plan->rel.swap(scratch.rel);
-    plan->last_launches = 0;
-    // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
-        dd_status st = upload_tables(plan);
-        if (st != DD_OK)
-            return st;
-    } else {
-        (void)cudaGetLastError();
+}
+
+dd_status dd_set_killmask(dd_plan plan, const int32_t *mask)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    try {
+        std::vector<uint8_t> keep;
+        if (mask) {
+            keep.resize(plan->nchans);
+            for (int c = 0; c < plan->nchans; ++c)
+                keep[c] = mask[c] != 0;
+        }
+        if (plan->ndm <= 0) {   // no DM list yet: remembered, applied by dd_set_dm_list
+            plan->keep.swap(keep);
+            return DD_OK;
+        }
+        return replan(plan, plan->dm, keep);
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
     }
-    return DD_OK;
 }
 
 dd_status dd_get_delay_table(dd_plan plan, int32_t *table)
@@ -327,6 +360,17 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
             plan->out_beam_stride < static_cast<int64_t>(plan->ndm) * nsamps * es)
             return DD_ERR_STRIDE_TOO_SMALL;
     }
+    cudaStream_t st_ = static_cast<cudaStream_t>(stream);
+    if (plan->nlive == 0) {   // every channel killed: the sums are zero (float32 zero is all-zero bits too)
+        const size_t beam_bytes = static_cast<size_t>(plan->ndm) * nsamps * es;
+        const cudaError_t me = plan->nbeams > 1
+                                   ? cudaMemset2DAsync(out_ptr, plan->out_beam_stride, 0, beam_bytes, plan->nbeams, st_)
+                                   : cudaMemsetAsync(out_ptr, 0, beam_bytes, st_);
+        if (me != cudaSuccess)
+            return cuda_fail(me, "dd_execute memset");
+        plan->last_launches = 0;
+        return DD_OK;
+    }
     if (!plan->uploaded) {
         st = upload_tables(plan);
         if (st != DD_OK)
@@ -334,7 +378,6 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
     }
     const KernelParams kp = make_params(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, plan->nbeams,
                                         plan->in_beam_stride, plan->out_beam_stride);
-    cudaStream_t st_ = static_cast<cudaStream_t>(stream);
     const bool prof = plan->prof_cap > 0 && plan->prof_n < plan->prof_cap;
     cudaEvent_t *ev = prof ? reinterpret_cast<cudaEvent_t *>(plan->prof_events.data()) + 3 * plan->prof_n : nullptr;
     plan->prof_mid = nullptr;
@@ -366,6 +409,16 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     if (st != DD_OK)
         return st;
     const int es = elem_size(out_nbits);
+    if (plan->nlive == 0) {   // every channel killed
+        const size_t beam_bytes = static_cast<size_t>(plan->ndm) * nsamps * es;
+        const size_t pitch = plan->nbeams > 1 ? static_cast<size_t>(plan->out_beam_stride) : beam_bytes;
+        if (plan->nbeams > 1 && pitch < beam_bytes)
+            return DD_ERR_STRIDE_TOO_SMALL;
+        for (int b = 0; b < plan->nbeams; ++b)
+            std::memset(static_cast<uint8_t *>(out_host) + b * pitch, 0, beam_bytes);
+        plan->last_launches = 0;
+        return DD_OK;
+    }
     if (!plan->uploaded) {
         st = upload_tables(plan);
         if (st != DD_OK)

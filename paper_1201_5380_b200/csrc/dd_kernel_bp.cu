@@ -375,7 +375,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     __syncthreads();
 
     const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
-    const int2 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans_pad;
+    const int4 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans_pad;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + static_cast<int64_t>(blk) * p.nchans_pad * DB;
 
     // producers: EVERY warp stages CPW = CC * NSUB / NWARPS sub-rows of each chunk (its lane 0 issues the bulk
@@ -383,12 +383,12 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     // serialises over its lanes and falls behind the others); warp 0 also stages the chunk's offset entries.
     // The span metadata of the next chunk to stage is fetched one step early.
     constexpr int CPW = CC * NSUB / BP_NWARPS;
-    auto load_meta = [&](int chunk, int2 (&m)[CPW]) {
+    auto load_meta = [&](int chunk, int4 (&m)[CPW]) {
 #pragma unroll
         for (int k = 0; k < CPW; ++k)
-            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int2(0, 0);
+            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
     };
-    auto produce = [&](int chunk, const int2 (&m)[CPW]) {
+    auto produce = [&](int chunk, const int4 (&m)[CPW]) {
         const int s = chunk % NS;
         if (lane == 0) {
             if (chunk >= NS)
@@ -397,8 +397,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             uint32_t bytes[CPW], tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
 #pragma unroll
             for (int k = 0; k < CPW; ++k) {
-                const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
-                const int c = chunk * CC + cl;
+                const int sub = (warp * CPW + k) % NSUB;
                 if (m[k].y < 0) {                                // padded channel: zeros
                     src[k] = p.zero;
                     bytes[k] = static_cast<uint32_t>(-m[k].y);
@@ -406,7 +405,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                     const int64_t off = ((t0 + m[k].x) >> 5) * UB;
                     const int64_t avail = p.in_row_bytes - off;
                     bytes[k] = static_cast<uint32_t>(m[k].y < avail ? m[k].y : (avail > 0 ? avail : 0));
-                    src[k] = in_beam + static_cast<int64_t>(c) * p.in_stride + sub * p.in_row_bytes + off;
+                    src[k] = in_beam + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + off;
                 }
                 tx += bytes[k];
             }
@@ -425,7 +424,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     };
 
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in chunks (measured: 1 and 2 equal, 3 slower)
-    int2 meta[CPW], nxt[CPW];
+    int4 meta[CPW], nxt[CPW];
     load_meta(0, meta);
     for (int k = 0; k < dist && k < p.nchunks; ++k) {
         load_meta(k + 1, nxt);
@@ -525,7 +524,7 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     if (groups > have)
         groups = have;
     const int64_t conv = groups * 16;   // bytes per sub-row
-    const size_t need = static_cast<size_t>(kp.nbeams) * kp.nchans * C::NSUB * static_cast<size_t>(conv);
+    const size_t need = static_cast<size_t>(kp.nbeams) * kp.nrows * C::NSUB * static_cast<size_t>(conv);
     cudaError_t e;
     if (plan->work_bytes < need) {
         if (plan->d_work)
@@ -536,8 +535,8 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
             return e;
         plan->work_bytes = need;
     }
-    const int64_t w_beam = static_cast<int64_t>(kp.nchans) * C::NSUB * conv;
-    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups + 255) / 256), kp.nchans, kp.nbeams), 256, 0, stream>>>(
+    const int64_t w_beam = static_cast<int64_t>(kp.nrows) * C::NSUB * conv;
+    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
         kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv, w_beam,
         static_cast<int32_t>(groups));
     if ((e = cudaGetLastError()) != cudaSuccess)

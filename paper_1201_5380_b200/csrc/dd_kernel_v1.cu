@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(V1_NWARPS * 32, 1) dd_direct_v1(const KernelPa
     __syncthreads();
 
     const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
-    const int2 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans;
+    const int4 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans;
     const uint16_t *rel_blk = static_cast<const uint16_t *>(p.rel) + static_cast<int64_t>(blk) * p.nchans * DB;
 
     // producer: warp 0, lane i stages channel (chunk*cc + i); lane 0 also stages the chunk's offsets
@@ -88,11 +88,11 @@ __global__ void __launch_bounds__(V1_NWARPS * 32, 1) dd_direct_v1(const KernelPa
         uint32_t bytes = 0;
         const uint8_t *src = nullptr;
         if (lane < p.cc && c < p.nchans) {
-            const int2 m = __ldg(&span_blk[c]);
+            const int4 m = __ldg(&span_blk[c]);
             const int64_t off = ((t0 + m.x) * NBITS) >> 3;
             const int64_t avail = p.in_row_bytes - off;
             bytes = static_cast<uint32_t>(m.y < avail ? m.y : avail);
-            src = in_beam + static_cast<int64_t>(c) * p.in_stride + off;
+            src = in_beam + static_cast<int64_t>(m.z) * p.in_stride + off;
         }
         const int nch = min(p.cc, p.nchans - chunk * p.cc);
         const uint32_t rel_bytes = static_cast<uint32_t>(nch) * DB * 2;

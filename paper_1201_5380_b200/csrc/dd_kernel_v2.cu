@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(V2_NWARPS * 32, 1) dd_direct_v2(const KernelPa
     __syncthreads();
 
     const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
-    const int2 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans;
+    const int4 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans;
     const uint32_t *rel_blk = static_cast<const uint32_t *>(p.rel) + static_cast<int64_t>(blk) * p.nchans * DB;
 
     // producer (warp 0): lane i stages channels chunk*cc + i, + i + 32; lane 0 also stages the offsets
@@ -80,11 +80,11 @@ __global__ void __launch_bounds__(V2_NWARPS * 32, 1) dd_direct_v2(const KernelPa
             const int cl = lane + 32 * k;
             if (cl < nch) {
                 const int c = chunk * p.cc + cl;
-                const int2 m = __ldg(&span_blk[c]);
+                const int4 m = __ldg(&span_blk[c]);
                 const int64_t off = ((t0 + m.x) * 2) >> 3;
                 const int64_t avail = p.in_row_bytes - off;
                 bytes[k] = static_cast<uint32_t>(m.y < avail ? m.y : avail);
-                src[k] = in_beam + static_cast<int64_t>(c) * p.in_stride + off;
+                src[k] = in_beam + static_cast<int64_t>(m.z) * p.in_stride + off;
                 tx += bytes[k];
             }
         }

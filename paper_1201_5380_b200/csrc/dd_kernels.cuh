@@ -18,14 +18,16 @@ struct KernelParams {
     int64_t nsamps;           // output samples per DM trial
     int32_t out_code;         // DD_OUT_F32 / DD_OUT_U16 / DD_OUT_U32
     int32_t vec_ok;           // rows and base pointers allow 4-sample vector stores
-    int32_t nchans, ndm, nblk, ntiles, nbeams;
+    int32_t nchans;           // channels summed (the live list under a kill mask); span/rel are indexed by list position
+    int32_t nrows;            // channel rows of the input
+    int32_t ndm, nblk, ntiles, nbeams;
     int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
     int32_t raw_slot, lane_slot;
     int32_t sub_slot;         // bit planes: bytes per sub-row inside a channel slot
     int32_t nstages;          // ring depth of the staged buffers (bit-plane variant)
     int32_t nchans_pad;       // channels iterated over: nchans padded to a multiple of cc (bit-plane variant)
     const uint8_t *zero;      // raw_slot zero bytes: the span of a padded channel
-    const int2 *span;         // [nblk][nchans] {start, nbytes}
+    const int4 *span;         // [nblk][nchans_pad] {start, nbytes, input row, 0}
     const void *rel;          // [nblk][nchans][DB] entries of var.rel_bytes
 };
 

@@ -66,7 +66,13 @@ static const Variant kVariants[] = {
 
 dd_status build_tiles(dd_plan_s *p)
 {
-    const int nchans = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    // the channels that are summed (PAPER.md:113 kill mask): the kernels iterate over this list only
+    std::vector<int32_t> live;
+    for (int c = 0; c < nrows; ++c)
+        if (p->keep.empty() || p->keep[c])
+            live.push_back(c);
+    const int nchans = static_cast<int>(live.size());
     const int64_t vmax = (1 << nbits) - 1;
     const int64_t top = static_cast<int64_t>(nchans) * vmax;   // largest possible sum
     p->final32 = top > 65535;
@@ -92,7 +98,7 @@ dd_status build_tiles(dd_plan_s *p)
                 int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0;
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);   // pad the last block with its last DM
-                    const int32_t dl = p->delay[static_cast<size_t>(d) * nchans + c];
+                    const int32_t dl = p->delay[static_cast<size_t>(d) * nrows + live[c]];
                     dmin = std::min(dmin, dl);
                     dmax = std::max(dmax, dl);
                 }
@@ -107,6 +113,8 @@ dd_status build_tiles(dd_plan_s *p)
                 SpanMeta &m = span0[static_cast<size_t>(b) * nchans + c];
                 m.start = start;
                 m.nbytes = static_cast<int32_t>(nbytes);
+                m.row = live[c];
+                m.pad = 0;
                 max_bytes = std::max(max_bytes, nbytes);
                 max_end = std::max(max_end, start + (v.bitplane ? nbytes / v.unit_bytes * 32 : nbytes * 8 / nbits));
             }
@@ -145,6 +153,8 @@ dd_status build_tiles(dd_plan_s *p)
                 const uint32_t slot_off = static_cast<uint32_t>(c % cc) * static_cast<uint32_t>(p->raw_slot);
                 if (c >= nchans) {   // padded channel: a whole slot of zeros, every window at its start
                     m.start = 0;
+                    m.row = 0;
+                    m.pad = 0;
                     m.nbytes = -(v.bitplane ? p->sub_slot : p->raw_slot);   // negative: stage from the zero buffer
                     for (int i = 0; i < DB; ++i) {
                         uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
@@ -156,7 +166,7 @@ dd_status build_tiles(dd_plan_s *p)
                 m = span0[static_cast<size_t>(b) * nchans + c];
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);
-                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nchans + c] - m.start);
+                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nrows + live[c]] - m.start);
                     if (v.rel_bytes == 2) {
                         reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
                     } else if (v.rel_bytes == 4) {
@@ -175,6 +185,8 @@ dd_status build_tiles(dd_plan_s *p)
         p->smem_bytes = smem_layout_bytes(p, cc);
         p->span.swap(span);
         p->rel.swap(rel);
+        p->live.swap(live);
+        p->nlive = nchans;
         return DD_OK;
     }
     return DD_ERR_SMEM;

@@ -36,9 +36,11 @@ struct Variant {
     int nsub;         // bit planes: sub-rows per channel (nbits / planes per sub-row); else 1
 };
 
-struct SpanMeta {   // per (DM block, channel); mirrored on the device as int2
+struct SpanMeta {   // per (DM block, live channel); mirrored on the device as int4
     int32_t start;  // first staged sample relative to the tile's first output sample; multiple of 128/nbits
-    int32_t nbytes; // packed bytes to stage (multiple of 16)
+    int32_t nbytes; // packed bytes to stage (multiple of 16); negative: a padded channel staged from the zero buffer
+    int32_t row;    // the channel's row in the input (differs from its position in the list under a kill mask)
+    int32_t pad;
 };
 
 struct HostStage;   // device staging for dd_execute_host (dd_api.cu)
@@ -55,6 +57,10 @@ struct dd_plan_s {
     std::vector<double> dm;
     std::vector<int32_t> delay;   // [ndm][nchans]
     int64_t max_delay = -1;
+    // channel kill mask: the channels that are summed, in ascending order; all of them by default
+    std::vector<uint8_t> keep;    // [nchans] 1 = summed, 0 = skipped; empty = no mask
+    std::vector<int32_t> live;    // rows of the summed channels (built by build_tiles)
+    int nlive = 0;
     // batching
     int nbeams = 1;
     int64_t in_beam_stride = 0, out_beam_stride = 0;
@@ -63,7 +69,7 @@ struct dd_plan_s {
     int force_variant = 0; // 0 = automatic; otherwise only this variant id is considered (dd_set_kernel_variant)
     int nblk = 0;          // DM blocks
     int cc = 0;            // channels per pipeline stage
-    int nchans_pad = 0;    // channels the kernel iterates over (nchans, or padded to a multiple of cc)
+    int nchans_pad = 0;    // channels the kernel iterates over (nlive, or padded to a multiple of cc)
     int nstages = 2;       // ring depth of the staged buffers (<= var.raw_stages)
     int64_t max_span_end = 0;   // max over spans of start + staged samples: how far past a tile's t0 a copy reaches
     int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
@@ -71,7 +77,7 @@ struct dd_plan_s {
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
-    std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad]
+    std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels
     std::vector<uint8_t> rel;         // [nblk][nchans_pad][DB] entries of var.rel_bytes: delay - span start per DM slot
     // device copies
     int device = -1;

@@ -131,3 +131,34 @@ def test_execute_argument_checks_need_no_gpu():
         assert dd.lib().dd_set_batch(p.handle, 0, 0, 0) == -2
         assert dd.lib().dd_set_batch(p.handle, 2, 24, 0) == -4
         assert dd.lib().dd_set_batch(p.handle, 2, 4096 * 64, 1 << 20) == 0
+
+
+def test_killmask_host_side():
+    # the mask changes which channels are summed, not the delay table; NULL removes it
+    cfg = W.CONFIGS[2]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        assert dd.lib().dd_set_killmask(None, None) == -1
+        mask = np.ones(cfg.nchans, dtype=np.int32)
+        mask[100:300] = 0
+        p.set_killmask(mask)                       # before the DM list: remembered
+        p.set_dm_list(cfg.dm_list()[:40])
+        full = oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.dm_list()[:40])
+        assert np.array_equal(p.delay_table().astype(np.int64), full)
+        assert p.max_delay == int(full.max())
+        p.set_killmask(None)
+        p.set_killmask(np.zeros(cfg.nchans, dtype=np.int32))   # every channel killed is legal
+        p.set_killmask(mask * 5)
+        assert np.array_equal(p.delay_table().astype(np.int64), full)
+        with pytest.raises(ValueError):
+            p.set_killmask(mask[:10])
+    # a mask can bring a plan into the output range: 8192 4-bit channels do not fit uint16, 4000 of them do
+    with dd.Plan(8192, 64e-6, 1500.0, -0.01, 4) as p:
+        p.set_dm_list([0.0])
+        assert dd.lib().dd_execute(p.handle, 100, 16, 4096, 16, 16, None) == -6
+        m = np.zeros(8192, dtype=np.int32)
+        m[:4000] = 1
+        p.set_killmask(m)
+        assert p.launch_info()["variant"] == 3      # 4000 * 15 < 2^16: the bit-plane kernel serves it now
+        m[:5000] = 1
+        p.set_killmask(m)                           # 5000 * 15 > 65535: still out of range
+        assert dd.lib().dd_execute(p.handle, 100, 16, 4096, 16, 16, None) == -6

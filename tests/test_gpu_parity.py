@@ -185,6 +185,51 @@ def test_many_channels_need_32bit_accumulators():
     _full_compare(cfg4)
 
 
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+def test_killmask_every_variant(variant):
+    # PAPER.md:113 kill mask against the oracle's arithmetic form (sum += data * mask[c]); masks that kill
+    # runs, single channels, the first and the last channel, so that the live list is ragged against the stage size
+    cfg = W.CONFIGS[2].reduced(nsamps=5120 + 700, ndm=21, nchans=200)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    rng = np.random.default_rng(113)
+    masks = [(rng.random(cfg.nchans) < 0.7).astype(np.int32), np.zeros(cfg.nchans, np.int32), None]
+    masks[0][[0, cfg.nchans - 1]] = 0
+    masks[0][50:90] = 0
+    for mask in masks:
+        out = torch.full((cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=variant) as p:
+            p.set_dm_list(cfg.dm_list())
+            p.set_killmask(mask)                   # after the DM list: tiles rebuilt at once
+            p.execute(cfg.nsamps, dev[0], stride, out, -32, torch.cuda.current_stream())
+            torch.cuda.synchronize()
+        ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask)
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+
+
+@pytest.mark.parametrize("nbits", [4, 8])
+def test_killmask_4_and_8_bit_batch_and_host_path(nbits):
+    cfg = W.CONFIGS[{4: 4, 8: 5}[nbits]].reduced(nsamps=3072 + 100, ndm=18, nchans=77, nbeams=2)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    mask = (np.arange(cfg.nchans) % 3 != 1).astype(np.int32)
+    out = torch.full((2, cfg.ndm, cfg.nsamps), -1, dtype=torch.float32, device="cuda")
+    h_out = torch.zeros((2, cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_killmask(mask)                       # before the DM list
+        p.set_dm_list(cfg.dm_list())
+        p.set_batch(2, dev.stride(0), out.stride(0) * 4)
+        p.execute(cfg.nsamps, dev, stride, out, 32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, 32)
+    for b in range(2):
+        ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask).astype(np.float32)
+        assert np.array_equal(out[b].cpu().numpy(), ref)
+        assert np.array_equal(h_out[b].numpy(), ref)
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)

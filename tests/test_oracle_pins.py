@@ -1,6 +1,6 @@
 """Pins for the CPU oracle (oracle/) -- what the paper and the mathematics fix, NOT the oracle re-typed.
 
-Pin numbering follows DESIGN.md section 3 (P1..P11).  None of these tests touches the CUDA path.
+Pin numbering follows DESIGN.md section 3 (P1..P12).  None of these tests touches the CUDA path.
 
   P1  hand-evaluated eq. 1 delays (tests/golden/delays_eq1_hand.txt)
   P2  closed-form properties + exact rational arithmetic (fractions.Fraction)
@@ -13,6 +13,7 @@ Pin numbering follows DESIGN.md section 3 (P1..P11).  None of these tests touche
   P9  C loop == numpy gather == pure-Python triple loop on tiny inputs           eq. 3
   P10 output statistics of uniform 2-bit noise                                   eq. 3 + CLT
   P11 packing convention: bytes 0xE4 / 0x21                                      reading R9
+  P12 kill mask: equals the unmasked sum over zeroed rows; complements add up
 """
 import math
 import os
@@ -301,6 +302,41 @@ def test_p11_packing_convention():
         p = W.pack_rows(torch.from_numpy(a), nbits).numpy()
         assert p.shape == (3, 64 * nbits // 8)
         assert np.array_equal(oracle.unpack(p, nbits, 64), a)
+
+
+# ----------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_p12_kill_mask(nbits):
+    """`sum += data * kill_mask[channel]`.  Pinned by what the mask must mean, through paths that
+    never touch the mask argument: (i) zeroing the killed rows of the INPUT and summing everything; (ii) the sum
+    over the kept channels only, as a smaller problem; (iii) complementary masks add up to the unmasked sum."""
+    nchans, nsamps, ndm, maxdelay = 23, 300, 6, 40
+    a, packed, delays = _random_case(nbits, nchans, nsamps, ndm, maxdelay, seed=1200 + nbits)
+    rng = np.random.default_rng(12)
+    mask = (rng.random(nchans) < 0.6).astype(np.int32)
+    mask[0], mask[1] = 0, 1                       # both values certainly present
+    masked = oracle.dedisperse(packed, nbits, nsamps, delays, mask=mask)
+    # (i) zero the killed rows, no mask
+    a0 = a.copy()
+    a0[mask == 0] = 0
+    p0 = W.pack_rows(torch.from_numpy(a0), nbits).numpy()
+    assert np.array_equal(masked, oracle.dedisperse(p0, nbits, nsamps, delays))
+    # (ii) the kept channels alone
+    keep = np.nonzero(mask)[0]
+    assert np.array_equal(masked, oracle.dedisperse(packed[keep], nbits, nsamps, delays[:, keep]))
+    # (iii) complements
+    comp = oracle.dedisperse(packed, nbits, nsamps, delays, mask=1 - mask)
+    full = oracle.dedisperse(packed, nbits, nsamps, delays)
+    assert np.array_equal(masked.astype(np.int64) + comp, full)
+    # any nonzero mask value keeps the channel; all ones == no mask; all zeros == 0
+    assert np.array_equal(oracle.dedisperse(packed, nbits, nsamps, delays, mask=mask * 7), masked)
+    assert np.array_equal(oracle.dedisperse(packed, nbits, nsamps, delays, mask=np.ones(nchans)), full)
+    assert not oracle.dedisperse(packed, nbits, nsamps, delays, mask=np.zeros(nchans)).any()
+    # the unpacked entry point and the per-point form take the same mask
+    assert np.array_equal(oracle.dedisperse_unpacked(a, nsamps, delays, mask=mask), masked)
+    d_idx, t_idx = rng.integers(0, ndm, 40), rng.integers(0, nsamps, 40)
+    pts = oracle.dedisperse_points(lambda c, t: a[c, t], delays, d_idx, t_idx, mask=mask)
+    assert np.array_equal(pts, masked[d_idx, t_idx])
 
 
 # --------------------------------------------------------------- oracle regression
