@@ -23,7 +23,8 @@ import numpy as np
 
 from . import build as _build
 from .oracle_np import (delay_table_np, dedisperse_gather_np, dedisperse_points,  # noqa: F401
-                        unpack_np, dedisperse_loops_py)
+                        unpack_np, dedisperse_loops_py, subband_tables, subband_required_samples,
+                        subband_dedisperse_np)
 
 _LIB: Optional[ctypes.CDLL] = None
 
@@ -119,6 +120,16 @@ def dedisperse_unpacked(a: np.ndarray, nsamps: int, delays: np.ndarray, nthreads
     if rc != 0:
         raise ValueError(f"oracle_dedisperse_unpacked rc={rc}")
     return out
+
+
+def subband_dedisperse(packed: np.ndarray, nbits: int, nsamps: int, nchans: int, dt: float, f_top: float, df: float,
+                       dm_list, sb_nchans: int, dm_group: int, mask=None) -> np.ndarray:
+    """Sub-band dedispersion (readings S1..S4 in oracle_np.py) of one packed beam:
+    uint8 [nchans][stride] -> int64 [ndm][nsamps]."""
+    nominal, delta1, delta2 = subband_tables(nchans, dt, f_top, df, dm_list, sb_nchans, dm_group)
+    need = subband_required_samples(nsamps, delta1, delta2, sb_nchans)
+    a = unpack(packed, nbits, need)
+    return subband_dedisperse_np(a, nsamps, nominal, delta1, delta2, sb_nchans, dm_group, mask=mask)
 
 
 def cast_out(sums: np.ndarray, kind: str) -> np.ndarray:

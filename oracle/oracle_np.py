@@ -75,3 +75,70 @@ def dedisperse_points(sample_fn: Callable[[np.ndarray, np.ndarray], np.ndarray],
     if mask is not None:
         v = v * (np.asarray(mask) != 0).astype(np.int64)[None, :]
     return v.sum(axis=1)
+
+
+# ------------------------------------------------------------------------------------------ sub-band dedispersion
+# PAPER.md:317-321 (section 4.1) and 358-360 (section 4.3): "two consecutive calls to the direct dedispersion
+# routine and the addition of a temporary data buffer".  The paper gives the procedure in words only; the
+# readings below (S1..S4) are listed in DESIGN.md section 10.
+#
+#   S1  trial DMs are grouped in runs of N'DM consecutive entries of the DM list; group g covers trials
+#       [g N'DM, min((g+1) N'DM, N_DM)); its nominal DM is the DM of its middle trial, index g N'DM + N'DM // 2
+#       (clipped to the last trial)                          "nominal DMs, each separated by N'DM trial DMs"
+#   S2  step 1 -- the direct algorithm (eq. 3) on every sub-band b of N'nu channels at every nominal DM, delays
+#       by eq. 4-5 with the sub-band's first channel as the start of the band:
+#           delta1[g][c] = floor(K DMnom_g (f_c^-2 - f_{b N'nu}^-2) / dt + 0.5),  b = c // N'nu
+#           S[b][g][t]   = sum_{c in sub-band b} A[c][t + delta1[g][c]]
+#   S3  step 2 -- the direct algorithm on the "miniature filterbank" S[.][g][.] of N_SB channels (channel b at
+#       the frequency of the sub-band's first channel) for the trials of group g, delays by eq. 4-5 on the full band:
+#           delta2[d][b] = floor(K DM_d (f_{b N'nu}^-2 - f_top^-2) / dt + 0.5)
+#           D[d][t]      = sum_b S[b][g(d)][t + delta2[d][b]]
+#   S4  step 1 is evaluated for 0 <= t < nsamps + max delta2, so the input rows must hold
+#       nsamps + max_b (max delta2[.][b] + max delta1[.][sub-band b]) samples.
+def subband_tables(nchans: int, dt: float, f_top: float, df: float, dm_list, sb_nchans: int, dm_group: int):
+    """(nominal trial index per group [ngroups], delta1 [ngroups][nchans], delta2 [ndm][nsb]) -- S1..S3, float64."""
+    dm = np.asarray(dm_list, dtype=np.float64)
+    ndm = dm.shape[0]
+    assert nchans % sb_nchans == 0 and dm_group >= 1
+    nsb = nchans // sb_nchans
+    ngroups = -(-ndm // dm_group)
+    nominal = np.minimum(np.arange(ngroups) * dm_group + dm_group // 2, ndm - 1)                 # S1
+    c = np.arange(nchans, dtype=np.float64)
+    f = f_top + c * df
+    f_sb = f_top + (np.arange(nchans) // sb_nchans * sb_nchans).astype(np.float64) * df         # first channel of c's sub-band
+    delta1 = np.floor(K_DM * dm[nominal][:, None] * (1.0 / f ** 2 - 1.0 / f_sb ** 2)[None, :] / dt + 0.5).astype(np.int64)   # S2
+    f_b = f_top + (np.arange(nsb) * sb_nchans).astype(np.float64) * df
+    delta2 = np.floor(K_DM * dm[:, None] * (1.0 / f_b ** 2 - 1.0 / f_top ** 2)[None, :] / dt + 0.5).astype(np.int64)         # S3
+    return nominal, delta1, delta2
+
+
+def subband_required_samples(nsamps: int, delta1: np.ndarray, delta2: np.ndarray, sb_nchans: int) -> int:
+    """S4: input samples per row the two steps read."""
+    nsb = delta2.shape[1]
+    d1 = delta1.reshape(delta1.shape[0], nsb, sb_nchans).max(axis=(0, 2))       # per sub-band
+    return int(nsamps + (delta2.max(axis=0) + d1).max())
+
+
+def subband_dedisperse_np(a: np.ndarray, nsamps: int, nominal, delta1, delta2, sb_nchans: int, dm_group: int,
+                          mask=None) -> np.ndarray:
+    """S2 then S3 on unpacked samples a [nchans][len]; returns int64 [ndm][nsamps].  Step by step, with the
+    intermediate buffer S [nsb][ngroups][nsamps + max delta2] written out in full as the paper describes."""
+    a = np.asarray(a).astype(np.int64)
+    nchans = a.shape[0]
+    ndm, nsb = delta2.shape
+    ngroups = delta1.shape[0]
+    keep = np.ones(nchans, dtype=np.int64) if mask is None else (np.asarray(mask) != 0).astype(np.int64)
+    t1 = nsamps + int(delta2.max())
+    S = np.zeros((nsb, ngroups, t1), dtype=np.int64)
+    for b in range(nsb):                                                         # step 1 (S2)
+        for g in range(ngroups):
+            for c in range(b * sb_nchans, (b + 1) * sb_nchans):
+                o = int(delta1[g][c])
+                S[b, g] += a[c, o:o + t1] * keep[c]
+    out = np.zeros((ndm, nsamps), dtype=np.int64)
+    for d in range(ndm):                                                         # step 2 (S3)
+        g = d // dm_group
+        for b in range(nsb):
+            o = int(delta2[d][b])
+            out[d] += S[b, g, o:o + nsamps]
+    return out

@@ -14,6 +14,8 @@ Pin numbering follows DESIGN.md section 3 (P1..P12).  None of these tests touche
   P10 output statistics of uniform 2-bit noise                                   eq. 3 + CLT
   P11 packing convention: bytes 0xE4 / 0x21                                      reading R9
   P12 kill mask: equals the unmasked sum over zeroed rows; complements add up
+  P13 sub-band method: reduces to the direct transform for 1-channel sub-bands; equals a direct transform with
+      the summed delays; error of the summed delays within the analytic bound; impulse response
 """
 import math
 import os
@@ -337,6 +339,81 @@ def test_p12_kill_mask(nbits):
     d_idx, t_idx = rng.integers(0, ndm, 40), rng.integers(0, nsamps, 40)
     pts = oracle.dedisperse_points(lambda c, t: a[c, t], delays, d_idx, t_idx, mask=mask)
     assert np.array_equal(pts, masked[d_idx, t_idx])
+
+
+# ----------------------------------------------------------------------------- P13
+def _subband_case(nbits, sb, grp, seed, nchans=24, ndm=11, nsamps=200):
+    cfg = W.CONFIGS[1]
+    dms = np.arange(ndm, dtype=np.float64) * 7.5
+    nominal, d1, d2 = oracle.subband_tables(nchans, cfg.dt, cfg.f_top, -2.0, dms, sb, grp)
+    need = oracle.subband_required_samples(nsamps, d1, d2, sb)
+    rng = np.random.default_rng(seed)
+    per = 8 // nbits
+    a_len = -(-need // (16 * per)) * (16 * per)
+    a = rng.integers(0, 1 << nbits, size=(nchans, a_len)).astype(np.uint8)
+    packed = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+    return cfg, dms, nominal, d1, d2, a, packed
+
+
+@pytest.mark.parametrize("nbits", [2, 8])
+def test_p13_subband_one_channel_subbands_is_the_direct_transform(nbits):
+    """N'nu = 1: step 1 copies the channels (delta1 = 0) and step 2 is eq. 3, whatever N'DM is."""
+    nchans, nsamps = 24, 200
+    for grp in (1, 4):
+        cfg, dms, nominal, d1, d2, a, packed = _subband_case(nbits, 1, grp, seed=13)
+        assert not d1.any()
+        exact = oracle.delay_table(nchans, cfg.dt, cfg.f_top, -2.0, dms)
+        assert np.array_equal(d2, exact)
+        got = oracle.subband_dedisperse(packed, nbits, nsamps, nchans, cfg.dt, cfg.f_top, -2.0, dms, 1, grp)
+        assert np.array_equal(got, oracle.dedisperse(packed, nbits, nsamps, exact))
+
+
+@pytest.mark.parametrize("sb,grp", [(4, 1), (4, 3), (8, 4), (24, 11)])
+def test_p13_subband_equals_direct_with_summed_delays_and_error_bound(sb, grp):
+    """The two steps are linear, so the result is eq. 3 with delay delta1[g(d)][c] + delta2[d][c // N'nu] (run through
+    the pinned C loop); that delay differs from eq. 5 by at most 1 + |DMnom - DM| (DeltaT(c) - DeltaT(first channel of
+    the sub-band)) samples -- two roundings plus the nominal-DM approximation inside the sub-band."""
+    nbits, nchans, nsamps = 4, 24, 200
+    cfg, dms, nominal, d1, d2, a, packed = _subband_case(nbits, sb, grp, seed=131)
+    got = oracle.subband_dedisperse(packed, nbits, nsamps, nchans, cfg.dt, cfg.f_top, -2.0, dms, sb, grp)
+    g_of_d = np.arange(len(dms)) // grp
+    eff = d1[g_of_d] + d2[:, np.arange(nchans) // sb]
+    assert np.array_equal(got, oracle.dedisperse(packed, nbits, nsamps, eff))
+    # DM 0 is its own nominal DM only when it sits in the middle of its group; its row is the channel sum when grp == 1
+    if grp == 1:
+        assert np.array_equal(got[0], a[:, :nsamps].astype(np.int64).sum(axis=0))
+    f = cfg.f_top + np.arange(nchans) * -2.0
+    T = 4.148808e3 / cfg.dt * (1.0 / f ** 2 - 1.0 / cfg.f_top ** 2)
+    Tsb = T[np.arange(nchans) // sb * sb]
+    bound = 1.0 + np.abs(dms[nominal][g_of_d] - dms)[:, None] * (T - Tsb)[None, :]
+    exact_x = dms[:, None] * T[None, :]
+    assert np.all(np.abs(eff - exact_x) <= bound + 1e-9)
+    assert np.abs(eff - np.floor(exact_x + 0.5)).max() >= (1 if grp > 1 else 0)    # and the approximation is real
+    # masks pass through step 1
+    mask = (np.arange(nchans) % 5 != 2).astype(np.int32)
+    gm = oracle.subband_dedisperse(packed, nbits, nsamps, nchans, cfg.dt, cfg.f_top, -2.0, dms, sb, grp, mask=mask)
+    assert np.array_equal(gm, oracle.dedisperse(packed, nbits, nsamps, eff, mask=mask))
+
+
+def test_p13_subband_impulse_response():
+    """One non-zero input sample a[c*][tau] shows up in trial d at t = tau - delta1 - delta2 and nowhere else."""
+    nchans, nsamps, sb, grp = 12, 64, 4, 2
+    cfg = W.CONFIGS[1]
+    dms = np.array([0.0, 30.0, 60.0, 90.0, 120.0])
+    nominal, d1, d2 = oracle.subband_tables(nchans, cfg.dt, cfg.f_top, -5.0, dms, sb, grp)
+    assert nominal.tolist() == [1, 3, 4]
+    need = oracle.subband_required_samples(nsamps, d1, d2, sb)
+    for cstar in (0, 5, 11):
+        for tau in (0, 17, need - 1):
+            a = np.zeros((nchans, need), dtype=np.uint8)
+            a[cstar, tau] = 3
+            out = oracle.subband_dedisperse_np(a, nsamps, nominal, d1, d2, sb, grp)
+            for d in range(len(dms)):
+                t = tau - int(d1[d // grp][cstar]) - int(d2[d][cstar // sb])
+                want = np.zeros(nsamps, dtype=np.int64)
+                if 0 <= t < nsamps:
+                    want[t] = 3
+                assert np.array_equal(out[d], want)
 
 
 # --------------------------------------------------------------- oracle regression
