@@ -99,6 +99,36 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm);
  */
 dd_status dd_set_killmask(dd_plan plan, const int32_t *mask);
 
+/*
+ * dd_set_subband -- switches the plan to the SUB-BAND method of PAPER.md:317-321, an approximation of the
+ * transform that costs about (1/dm_group + 1/sb_nchans) of the direct one (eq. 30), done as the paper's own
+ * implementation did it: "two consecutive calls to the direct dedispersion routine and the addition of a
+ * temporary data buffer".  With b = c / sb_nchans the sub-band of channel c and g = d / dm_group
+ * the group of trial d, whose nominal DM is the DM of trial min(g*dm_group + dm_group/2, ndm-1):
+ *     step 1   S[b][g][t] = sum_{c in sub-band b} A[c][t + delta1[g][c]],
+ *              delta1[g][c] = floor(k_DM * DMnom_g * (f_c^-2 - f_{b*sb_nchans}^-2) / dt + 0.5)
+ *     step 2   D[d][t]    = sum_b S[b][g][t + delta2[d][b]],   delta2[d][b] = delay[d][b*sb_nchans]   (eq. 4-5)
+ * (readings S1-S4 of DESIGN.md section 10).  The result equals the direct transform with the delay
+ * delta1 + delta2, which differs from eq. 5 by at most 1 + |DMnom - DM| * (DeltaT(c) - DeltaT(first channel of b)).
+ *   sb_nchans  channels per sub-band N'nu: divides nchans; sb_nchans * (2^nbits - 1) <= 255 because the
+ *              intermediate series are kept in 8 bits (else DD_ERR_OUT_RANGE).
+ *   dm_group   trials per nominal DM N'DM: a multiple of 16.  The DM list is taken in the order given.
+ *   (0, 0) returns to the direct transform.
+ * Takes effect at once when a DM list is present (else at dd_set_dm_list); on error the plan is unchanged.  Honours
+ * the kill mask and dd_set_batch.  dd_execute then needs input rows of nsamps + dd_get_subband_extent() samples,
+ * allocates its temporary buffers on first use, and launches four kernels.  dd_execute_host returns
+ * DD_ERR_INVALID_ARG while the sub-band method is selected.
+ */
+dd_status dd_set_subband(dd_plan plan, int sb_nchans, int dm_group);
+
+/* Input samples per row beyond nsamps that the two steps read: max_b (max delta2[.][b] + max delta1[.][sub-band b])
+ * (>= 0), or a negative status (DD_ERR_INVALID_ARG when the sub-band method is not selected).  Host only. */
+int64_t dd_get_subband_extent(dd_plan plan);
+
+/* Copies the sub-band tables (HOST; any pointer may be NULL): nominal[ngroups] trial index of every group's nominal
+ * DM, delta1[ngroups][nchans], delta2[ndm][nchans/sb_nchans]; ngroups = ceil(ndm / dm_group).  Host only. */
+dd_status dd_get_subband_tables(dd_plan plan, int32_t *nominal, int32_t *delta1, int32_t *delta2);
+
 /* Copies the delay table to `table` (HOST, ndm*nchans int32, row-major [d][c]).  Host only. */
 dd_status dd_get_delay_table(dd_plan plan, int32_t *table);
 

@@ -19,7 +19,8 @@ import numpy as np
 __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_set_killmask", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
+    "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
@@ -29,7 +30,8 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 # every symbol include/dd.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_set_killmask", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
+    "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
 )
 
@@ -74,6 +76,12 @@ def lib() -> ctypes.CDLL:
         L.dd_get_max_delay.restype = i64
         L.dd_set_batch.argtypes = [vp, i32, i64, i64]
         L.dd_set_killmask.argtypes = [vp, vp]
+        L.dd_set_subband.argtypes = [vp, i32, i32]
+        L.dd_set_subband.restype = i32
+        L.dd_get_subband_extent.argtypes = [vp]
+        L.dd_get_subband_extent.restype = i64
+        L.dd_get_subband_tables.argtypes = [vp, vp, vp, vp]
+        L.dd_get_subband_tables.restype = i32
         L.dd_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
         L.dd_get_launch_info.argtypes = [vp, vp]
@@ -169,6 +177,30 @@ def dd_set_killmask(plan: int, mask) -> None:
     _check(lib().dd_set_killmask(plan, ctypes.c_void_p(m.ctypes.data)), "dd_set_killmask")
 
 
+def dd_set_subband(plan: int, sb_nchans: int, dm_group: int) -> None:
+    """Sub-band method (PAPER.md:317-321) with sb_nchans channels per sub-band and dm_group trials per nominal DM;
+    (0, 0) returns to the direct transform."""
+    _check(lib().dd_set_subband(plan, int(sb_nchans), int(dm_group)), "dd_set_subband")
+
+
+def dd_get_subband_extent(plan: int) -> int:
+    r = int(lib().dd_get_subband_extent(plan))
+    if r < 0:
+        raise DDError(r, "dd_get_subband_extent")
+    return r
+
+
+def dd_get_subband_tables(plan: int, ndm: int, nchans: int, sb_nchans: int, dm_group: int):
+    """(nominal [ngroups], delta1 [ngroups][nchans], delta2 [ndm][nchans // sb_nchans]) as int32 arrays."""
+    ngroups = -(-ndm // dm_group)
+    nominal = np.empty(ngroups, dtype=np.int32)
+    d1 = np.empty((ngroups, nchans), dtype=np.int32)
+    d2 = np.empty((ndm, nchans // sb_nchans), dtype=np.int32)
+    _check(lib().dd_get_subband_tables(plan, ctypes.c_void_p(nominal.ctypes.data), ctypes.c_void_p(d1.ctypes.data),
+                                       ctypes.c_void_p(d2.ctypes.data)), "dd_get_subband_tables")
+    return nominal, d1, d2
+
+
 def dd_execute(plan: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbits: int, stream=None) -> None:
     """Asynchronous; in_ptr/out_ptr are DEVICE buffers (tensors or addresses)."""
     _check(lib().dd_execute(plan, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits),
@@ -233,6 +265,19 @@ class Plan:
     def set_batch(self, nbeams: int, in_beam_stride: int, out_beam_stride: int) -> "Plan":
         dd_set_batch(self.handle, nbeams, in_beam_stride, out_beam_stride)
         return self
+
+    def set_subband(self, sb_nchans: int, dm_group: int) -> "Plan":
+        dd_set_subband(self.handle, sb_nchans, dm_group)
+        self._subband = (int(sb_nchans), int(dm_group))
+        return self
+
+    @property
+    def subband_extent(self) -> int:
+        return dd_get_subband_extent(self.handle)
+
+    def subband_tables(self):
+        sb, grp = self._subband
+        return dd_get_subband_tables(self.handle, self.ndm, self.nchans, sb, grp)
 
     def set_killmask(self, mask) -> "Plan":
         if mask is not None and len(mask) != self.nchans:

@@ -116,6 +116,8 @@ static int elem_size(int out_nbits)
         return 4;
     case DD_OUT_U16:
         return 2;
+    case kOutU8:   // internal (sub-band intermediate); check_execute rejects it at the C ABI
+        return 1;
     }
     return 0;
 }
@@ -126,7 +128,7 @@ static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_st
     if (p->ndm <= 0)
         return DD_ERR_NO_DM_LIST;
     const int es = elem_size(out_nbits);
-    if (nsamps <= 0 || es == 0)
+    if (nsamps <= 0 || es == 0 || out_nbits == kOutU8)
         return DD_ERR_INVALID_ARG;
     if (in_stride <= 0 || in_stride % 16 != 0)
         return DD_ERR_ALIGNMENT;
@@ -165,7 +167,13 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     kp.ntiles = static_cast<int32_t>((nsamps + p->var.TB - 1) / p->var.TB);
     kp.nbeams = nbeams;
     kp.cc = p->cc;
-    kp.nchunks = (p->nlive + p->cc - 1) / p->cc;
+    kp.ngroups = p->ngroups;
+    kp.group_cols = p->group_cols;
+    kp.row_mul = 1;
+    kp.in_blk_div = 0;
+    kp.in_blk_stride = 0;
+    // channels a CTA iterates over: the columns of one group (padded for the bit-plane kernel)
+    kp.nchunks = ((p->var.pad_chunks ? p->group_cols : p->nlive) + p->cc - 1) / p->cc;
     kp.raw_slot = p->raw_slot;
     kp.lane_slot = p->lane_slot;
     kp.sub_slot = p->sub_slot;
@@ -179,9 +187,82 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
 
 // Rebuilds delay table and tile metadata for (DM list, kill mask) into a scratch plan, then commits: a failure
 // leaves the plan unchanged.  Uploads the tables when a device exists.
-static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uint8_t> keep)
+// The sub-band method on device-resident data ("two consecutive calls to the direct dedispersion
+// routine and the addition of a temporary data buffer"): step 1 writes uint8 series S[beam][sub-band][nominal DM][t]
+// for t < nsamps + largest step-2 delay (rounded up to 32 so that the rows can be staged by bulk copies), step 2
+// dedisperses, for every group of trials, the miniature filterbank of its nominal DM.
+static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
+                                 int out_nbits, cudaStream_t st_)
+{
+    dd_plan_s *s1 = plan->s1, *s2 = plan->s2;
+    if (!s1 || !s2)
+        return DD_ERR_INVALID_ARG;
+    if (in_stride * 8 < (nsamps + plan->sb_extent) * plan->nbits)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    dd_status st;
+    for (dd_plan_s *q : {plan, s1, s2})
+        if (!q->uploaded && (st = upload_tables(q)) != DD_OK)
+            return st;
+    const int nbeams = plan->nbeams, nsb = s2->nchans, ngrp = s1->ndm;
+    const int64_t t1 = (nsamps + plan->sb_max_d2 + 31) / 32 * 32;
+    const size_t need = static_cast<size_t>(nbeams) * nsb * ngrp * static_cast<size_t>(t1);
+    cudaError_t e;
+    if (plan->tmp_bytes < need) {
+        if (plan->d_tmp)
+            cudaFree(plan->d_tmp);
+        plan->d_tmp = nullptr;
+        plan->tmp_bytes = 0;
+        if ((e = cudaMalloc(&plan->d_tmp, need)) != cudaSuccess)
+            return cuda_fail(e, "cudaMalloc(sub-band intermediate)");
+        plan->tmp_bytes = need;
+    }
+    const bool prof = plan->prof_cap > 0 && plan->prof_n < plan->prof_cap;
+    cudaEvent_t *ev = prof ? reinterpret_cast<cudaEvent_t *>(plan->prof_events.data()) + 3 * plan->prof_n : nullptr;
+    if (prof)
+        cudaEventRecord(ev[0], st_);
+    // step 1: batch index = (beam, sub-band); "DM trials" = the nominal DMs
+    const int64_t in_beam = nbeams > 1 ? plan->in_beam_stride : 0;
+    KernelParams k1 = make_params(s1, t1, in_ptr, in_stride, plan->d_tmp, kOutU8, nbeams, in_beam,
+                                  static_cast<int64_t>(ngrp) * t1);
+    k1.vec_ok = 1;
+    s1->prof_mid = nullptr;
+    if ((e = launch_direct(s1, k1, st_)) != cudaSuccess)
+        return cuda_fail(e, "dd_execute sub-band step 1");
+    // step 2: N_SB channels; DM block blk reads the rows of nominal DM blk / (dm_group / 16)
+    const int64_t out_beam = nbeams > 1 ? plan->out_beam_stride : 0;
+    KernelParams k2 = make_params(s2, nsamps, plan->d_tmp, t1, out_ptr, out_nbits, nbeams,
+                                  static_cast<int64_t>(nsb) * ngrp * t1, out_beam);
+    k2.nrows = nsb * ngrp;
+    k2.row_mul = ngrp;
+    k2.in_blk_div = plan->dm_group / s2->var.DB;
+    s2->prof_mid = prof ? ev[1] : nullptr;
+    e = launch_direct(s2, k2, st_);
+    s2->prof_mid = nullptr;
+    if (e != cudaSuccess)
+        return cuda_fail(e, "dd_execute sub-band step 2");
+    if (prof) {
+        cudaEventRecord(ev[2], st_);
+        ++plan->prof_n;
+    }
+    plan->last_launches = launches_per_execute(s1) + launches_per_execute(s2);
+    return DD_OK;
+}
+
+static void destroy_subplan(dd_plan_s *q)
+{
+    if (!q)
+        return;
+    free_device_tables(q);
+    if (q->d_work)
+        cudaFree(q->d_work);
+    delete q;
+}
+
+static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uint8_t> keep, int sb_nchans, int dm_group)
 {
     dd_plan_s scratch;
+    scratch.sb_nchans = sb_nchans;
+    scratch.dm_group = dm_group;
     scratch.nchans = plan->nchans;
     scratch.dt = plan->dt;
     scratch.f_top = plan->f_top;
@@ -197,7 +278,29 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     st = build_tiles(&scratch);
     if (st != DD_OK)
         return st;
+    dd_plan_s *s1 = nullptr, *s2 = nullptr;
+    if (sb_nchans > 0) {   // the two direct steps of the sub-band method
+        s1 = new dd_plan_s();
+        s2 = new dd_plan_s();
+        st = build_subband(&scratch, s1, s2, &scratch.sb_nominal, &scratch.sb_max_d2, &scratch.sb_extent);
+        if (st == DD_OK && (!s1->var.bitplane || !s2->var.bitplane))
+            st = DD_ERR_SMEM;
+        if (st != DD_OK) {
+            delete s1;
+            delete s2;
+            return st;
+        }
+    }
     free_device_tables(plan);
+    destroy_subplan(plan->s1);
+    destroy_subplan(plan->s2);
+    plan->s1 = s1;
+    plan->s2 = s2;
+    plan->sb_nchans = sb_nchans;
+    plan->dm_group = dm_group;
+    plan->sb_nominal.swap(scratch.sb_nominal);
+    plan->sb_max_d2 = scratch.sb_max_d2;
+    plan->sb_extent = sb_nchans > 0 ? scratch.sb_extent : -1;
     plan->ndm = scratch.ndm;
     plan->dm.swap(scratch.dm);
     plan->keep.swap(scratch.keep);
@@ -209,6 +312,8 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->nblk = scratch.nblk;
     plan->cc = scratch.cc;
     plan->nchans_pad = scratch.nchans_pad;
+    plan->ngroups = scratch.ngroups;
+    plan->group_cols = scratch.group_cols;
     plan->nstages = scratch.nstages;
     plan->max_span_end = scratch.max_span_end;
     plan->raw_slot = scratch.raw_slot;
@@ -223,6 +328,10 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
         st = upload_tables(plan);
+        if (st == DD_OK && plan->s1)
+            st = upload_tables(plan->s1);
+        if (st == DD_OK && plan->s2)
+            st = upload_tables(plan->s2);
         if (st != DD_OK)
             return st;
     } else {
@@ -266,6 +375,10 @@ dd_status dd_plan_destroy(dd_plan plan)
     free_device_tables(plan);
     if (plan->d_work)
         cudaFree(plan->d_work);
+    if (plan->d_tmp)
+        cudaFree(plan->d_tmp);
+    destroy_subplan(plan->s1);
+    destroy_subplan(plan->s2);
     free_stage(plan->stage);
     free_prof_events(plan);
     delete plan;
@@ -282,7 +395,7 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm)
         if (!std::isfinite(dm_list[d]) || dm_list[d] < 0.0)
             return DD_ERR_INVALID_ARG;
     try {
-        return replan(plan, std::vector<double>(dm_list, dm_list + ndm), plan->keep);
+        return replan(plan, std::vector<double>(dm_list, dm_list + ndm), plan->keep, plan->sb_nchans, plan->dm_group);
     } catch (const std::bad_alloc &) {
         return DD_ERR_NOMEM;
     }
@@ -303,10 +416,65 @@ dd_status dd_set_killmask(dd_plan plan, const int32_t *mask)
             plan->keep.swap(keep);
             return DD_OK;
         }
-        return replan(plan, plan->dm, keep);
+        return replan(plan, plan->dm, keep, plan->sb_nchans, plan->dm_group);
     } catch (const std::bad_alloc &) {
         return DD_ERR_NOMEM;
     }
+}
+
+dd_status dd_set_subband(dd_plan plan, int sb_nchans, int dm_group)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (sb_nchans == 0 && dm_group == 0) {   // back to the direct transform
+        if (plan->ndm <= 0) {
+            plan->sb_nchans = plan->dm_group = 0;
+            return DD_OK;
+        }
+    } else {
+        if (sb_nchans < 1 || dm_group < 1 || plan->nchans % sb_nchans != 0 || dm_group % 16 != 0)
+            return DD_ERR_INVALID_ARG;
+        if (static_cast<int64_t>(sb_nchans) * ((1 << plan->nbits) - 1) > 255)
+            return DD_ERR_OUT_RANGE;   // the intermediate series are kept in 8 bits
+        if (plan->ndm <= 0) {
+            plan->sb_nchans = sb_nchans;
+            plan->dm_group = dm_group;
+            return DD_OK;
+        }
+    }
+    try {
+        return replan(plan, plan->dm, plan->keep, sb_nchans, dm_group);
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+}
+
+int64_t dd_get_subband_extent(dd_plan plan)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (plan->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    if (plan->sb_nchans <= 0)
+        return DD_ERR_INVALID_ARG;
+    return plan->sb_extent;
+}
+
+dd_status dd_get_subband_tables(dd_plan plan, int32_t *nominal, int32_t *delta1, int32_t *delta2)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (plan->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    if (plan->sb_nchans <= 0 || !plan->s1 || !plan->s2)
+        return DD_ERR_INVALID_ARG;
+    if (nominal)
+        std::memcpy(nominal, plan->sb_nominal.data(), plan->sb_nominal.size() * sizeof(int32_t));
+    if (delta1)
+        std::memcpy(delta1, plan->s1->delay.data(), plan->s1->delay.size() * sizeof(int32_t));
+    if (delta2)
+        std::memcpy(delta2, plan->s2->delay.data(), plan->s2->delay.size() * sizeof(int32_t));
+    return DD_OK;
 }
 
 dd_status dd_get_delay_table(dd_plan plan, int32_t *table)
@@ -371,6 +539,8 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
         plan->last_launches = 0;
         return DD_OK;
     }
+    if (plan->sb_nchans > 0)
+        return execute_subband(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, st_);
     if (!plan->uploaded) {
         st = upload_tables(plan);
         if (st != DD_OK)
@@ -409,6 +579,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     if (st != DD_OK)
         return st;
     const int es = elem_size(out_nbits);
+    if (plan->sb_nchans > 0)
+        return DD_ERR_INVALID_ARG;   // the sub-band method is offered on device buffers only (dd.h)
     if (plan->nlive == 0) {   // every channel killed
         const size_t beam_bytes = static_cast<size_t>(plan->ndm) * nsamps * es;
         const size_t pitch = plan->nbeams > 1 ? static_cast<size_t>(plan->out_beam_stride) : beam_bytes;

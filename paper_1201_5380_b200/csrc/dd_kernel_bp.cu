@@ -322,6 +322,16 @@ __device__ __forceinline__ void store4(const KernelParams &p, uint8_t *orow, int
                 if (t + k < p.nsamps)
                     o[k] = q[k];
         }
+    } else if (p.out_code == kOutU8) {   // internal: the intermediate series of the sub-band method
+        uint8_t *o = orow + t;
+        if (whole) {
+            *reinterpret_cast<uint32_t *>(o) = q[0] | (q[1] << 8) | (q[2] << 16) | (q[3] << 24);
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k < p.nsamps)
+                    o[k] = static_cast<uint8_t>(q[k]);
+        }
     } else {
         uint16_t *o = reinterpret_cast<uint16_t *>(orow) + t;
         if (whole) {
@@ -353,7 +363,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int blk = static_cast<int>(cta % p.nblk);
     const int64_t rest = cta / p.nblk;
     const int tile = static_cast<int>(rest % p.ntiles);
-    const int beam = static_cast<int>(rest / p.ntiles);
+    const int batch = static_cast<int>(rest / p.ntiles);          // (beam, channel group)
+    const int beam = batch / p.ngroups, group = batch - beam * p.ngroups;
     const int64_t t0 = static_cast<int64_t>(tile) * TB;
 
     // shared memory carve-up (must match dd::smem_layout_bytes)
@@ -374,9 +385,11 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     }
     __syncthreads();
 
-    const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
-    const int4 *span_blk = p.span + static_cast<int64_t>(blk) * p.nchans_pad;
-    const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + static_cast<int64_t>(blk) * p.nchans_pad * DB;
+    const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride +
+                             (p.in_blk_div > 0 ? static_cast<int64_t>(blk / p.in_blk_div) * p.in_blk_stride : 0);
+    const int64_t col0 = static_cast<int64_t>(blk) * p.nchans_pad + static_cast<int64_t>(group) * p.group_cols;
+    const int4 *span_blk = p.span + col0;
+    const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + col0 * DB;
 
     // producers: EVERY warp stages CPW = CC * NSUB / NWARPS sub-rows of each chunk (its lane 0 issues the bulk
     // copies: a bulk copy takes its operands from uniform registers, so one warp issuing all copies of a chunk
@@ -474,8 +487,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int d = blk * DB + warp;
     if (d >= p.ndm)
         return;
-    const int esize = (p.out_code == DD_OUT_U16) ? 2 : 4;
-    uint8_t *orow = p.out + static_cast<int64_t>(beam) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
+    const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
+    uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
 #pragma unroll
     for (int j = 0; j < W; ++j) {
         const int64_t tunit = t0 + 32 * (W * lane + j);
@@ -544,14 +557,15 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     kp.in = static_cast<const uint8_t *>(plan->d_work);
-    kp.in_stride = C::NSUB * conv;   // between channels; sub-rows are in_row_bytes apart
+    kp.in_stride = C::NSUB * conv * kp.row_mul;   // between channel indices; sub-rows are in_row_bytes apart
+    kp.in_blk_stride = C::NSUB * conv;            // between the rows of one channel index (sub-band step 2)
     kp.in_row_bytes = conv;
     kp.in_beam_stride = w_beam;
 
     e = cudaFuncSetAttribute(dd_direct_bp<NBITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)
         return e;
-    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams;
+    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * kp.ngroups;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
     dd_direct_bp<NBITS><<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);

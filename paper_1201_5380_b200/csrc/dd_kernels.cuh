@@ -24,6 +24,11 @@ struct KernelParams {
     int32_t cc, nchunks;      // channels per stage, number of stages' worth of channels
     int32_t raw_slot, lane_slot;
     int32_t sub_slot;         // bit planes: bytes per sub-row inside a channel slot
+    int32_t ngroups;          // channel groups per beam (sub-bands); the batch index is (beam, group)
+    int32_t group_cols;       // span/rel columns per group
+    int32_t row_mul;          // input rows per channel index (sub-band step 2: one row per nominal DM), else 1
+    int32_t in_blk_div;       // > 0: DM block blk reads the input row  row * row_mul + blk / in_blk_div
+    int64_t in_blk_stride;    // bytes between those rows (set by the launcher)
     int32_t nstages;          // ring depth of the staged buffers (bit-plane variant)
     int32_t nchans_pad;       // channels iterated over: nchans padded to a multiple of cc (bit-plane variant)
     const uint8_t *zero;      // raw_slot zero bytes: the span of a padded channel

@@ -42,6 +42,84 @@ dd_status compute_delay_table(dd_plan_s *p)
 
 static inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
+// Sub-band method: "the direct dedispersion algorithm is applied to sub-bands of N'nu channels
+// to compute a dedispersed time series for each nominal DM and sub-band.  In the second step, the DM trials near
+// each nominal value are computed by applying the direct algorithm to the miniature filterbanks".  Readings
+// S1-S4 of DESIGN.md section 10: groups of dm_group consecutive trials, nominal = the group's middle trial;
+// step-1 delays by eq. 4-5 relative to the sub-band's first channel; step-2 delays = the full-band delays of
+// the sub-bands' first channels.
+dd_status build_subband(const dd_plan_s *p, dd_plan_s *s1, dd_plan_s *s2, std::vector<int32_t> *nominal,
+                        int64_t *max_d2, int64_t *extent)
+{
+    const int nchans = p->nchans, ndm = p->ndm, sb = p->sb_nchans, grp = p->dm_group;
+    const int nsb = nchans / sb, ngrp = (ndm + grp - 1) / grp;
+    nominal->resize(ngrp);
+    for (int g = 0; g < ngrp; ++g)
+        (*nominal)[g] = std::min(g * grp + grp / 2, ndm - 1);
+    // step 1: nominal DMs, every channel delayed relative to the first channel of its sub-band
+    s1->nchans = nchans;
+    s1->dt = p->dt;
+    s1->f_top = p->f_top;
+    s1->df = p->df;
+    s1->nbits = p->nbits;
+    s1->ndm = ngrp;
+    s1->dm.resize(ngrp);
+    s1->keep = p->keep;
+    s1->group_size = sb;
+    s1->force_variant = 3;
+    s1->delay.resize(static_cast<size_t>(ngrp) * nchans);
+    std::vector<double> band(nchans);
+    for (int c = 0; c < nchans; ++c) {
+        const double f = p->f_top + static_cast<double>(c) * p->df;
+        const double f_sb = p->f_top + static_cast<double>(c / sb * sb) * p->df;
+        band[c] = 1.0 / (f * f) - 1.0 / (f_sb * f_sb);
+    }
+    std::vector<int64_t> d1max(nsb, 0);
+    int64_t maxd = 0;
+    for (int g = 0; g < ngrp; ++g) {
+        s1->dm[g] = p->dm[(*nominal)[g]];
+        const double scale = kDispersionConstant * s1->dm[g];
+        for (int c = 0; c < nchans; ++c) {
+            const double r = std::floor(scale * band[c] / p->dt + 0.5);
+            if (!(r >= 0.0) || r > static_cast<double>(std::numeric_limits<int32_t>::max() - 1))
+                return DD_ERR_DELAY_OVERFLOW;
+            const int32_t v = static_cast<int32_t>(r);
+            s1->delay[static_cast<size_t>(g) * nchans + c] = v;
+            d1max[c / sb] = std::max<int64_t>(d1max[c / sb], v);
+            maxd = std::max<int64_t>(maxd, v);
+        }
+    }
+    s1->max_delay = maxd;
+    // step 2: N_SB channels at the sub-bands' first frequencies, all trials, delays taken from the full table
+    s2->nchans = nsb;
+    s2->dt = p->dt;
+    s2->f_top = p->f_top;
+    s2->df = p->df * sb;
+    s2->nbits = 8;
+    s2->ndm = ndm;
+    s2->dm = p->dm;
+    s2->force_variant = 3;
+    s2->delay.resize(static_cast<size_t>(ndm) * nsb);
+    int64_t m2 = 0, ext = 0;
+    for (int b = 0; b < nsb; ++b) {
+        int64_t colmax = 0;
+        for (int d = 0; d < ndm; ++d) {
+            const int32_t v = p->delay[static_cast<size_t>(d) * nchans + static_cast<size_t>(b) * sb];
+            s2->delay[static_cast<size_t>(d) * nsb + b] = v;
+            colmax = std::max<int64_t>(colmax, v);
+        }
+        m2 = std::max(m2, colmax);
+        ext = std::max(ext, colmax + d1max[b]);
+    }
+    s2->max_delay = m2;
+    *max_d2 = m2;
+    *extent = ext;
+    dd_status st = build_tiles(s1);
+    if (st != DD_OK)
+        return st;
+    return build_tiles(s2);
+}
+
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 {
     const Variant &v = p->var;
@@ -73,8 +151,19 @@ dd_status build_tiles(dd_plan_s *p)
         if (p->keep.empty() || p->keep[c])
             live.push_back(c);
     const int nchans = static_cast<int>(live.size());
+    // channel groups (sub-bands): position range [gbeg[g], gbeg[g+1]) of the live list
+    const int gsize = p->group_size > 0 ? p->group_size : std::max(nrows, 1);
+    const int ngroups = (nrows + gsize - 1) / gsize;
+    std::vector<int> gbeg(ngroups + 1, 0);
+    for (int c : live)
+        ++gbeg[c / gsize + 1];
+    int gmax = 0;
+    for (int g = 0; g < ngroups; ++g) {
+        gmax = std::max(gmax, gbeg[g + 1]);
+        gbeg[g + 1] += gbeg[g];
+    }
     const int64_t vmax = (1 << nbits) - 1;
-    const int64_t top = static_cast<int64_t>(nchans) * vmax;   // largest possible sum
+    const int64_t top = static_cast<int64_t>(gmax) * vmax;   // largest possible sum
     p->final32 = top > 65535;
 
     for (const Variant &v : kVariants) {
@@ -84,6 +173,8 @@ dd_status build_tiles(dd_plan_s *p)
             continue;
         if (p->force_variant && v.id != p->force_variant)
             continue;
+        if (ngroups > 1 && !v.bitplane)
+            continue;   // channel groups are served by the bit-plane kernel only
         p->var = v;
         const int DB = v.DB;
         const int nblk = (ndm + DB - 1) / DB;
@@ -142,16 +233,19 @@ dd_status build_tiles(dd_plan_s *p)
         }
         if (cc < 1)
             continue;
-        // pass 2: per (DM, channel) the position of that DM's window inside the staged span
-        const int nchans_pad = v.pad_chunks ? static_cast<int>(align_up(nchans, cc)) : nchans;
+        // pass 2: per (DM, column) the position of that DM's window inside the staged span.  Column k of group g
+        // is the k-th live channel of the group; columns past the group's live count are padded (zero) channels.
+        const int group_cols = v.pad_chunks ? static_cast<int>(align_up(gmax, cc)) : gmax;
+        const int nchans_pad = ngroups * group_cols;
         std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans_pad);
         std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchans_pad * DB * v.rel_bytes);
         for (int b = 0; b < nblk; ++b) {
-            for (int c = 0; c < nchans_pad; ++c) {
-                SpanMeta &m = span[static_cast<size_t>(b) * nchans_pad + c];
-                const size_t base = (static_cast<size_t>(b) * nchans_pad + c) * DB;
-                const uint32_t slot_off = static_cast<uint32_t>(c % cc) * static_cast<uint32_t>(p->raw_slot);
-                if (c >= nchans) {   // padded channel: a whole slot of zeros, every window at its start
+            for (int col = 0; col < nchans_pad; ++col) {
+                SpanMeta &m = span[static_cast<size_t>(b) * nchans_pad + col];
+                const size_t base = (static_cast<size_t>(b) * nchans_pad + col) * DB;
+                const int g = col / std::max(group_cols, 1), k = col - g * group_cols;
+                const uint32_t slot_off = static_cast<uint32_t>(k % cc) * static_cast<uint32_t>(p->raw_slot);
+                if (k >= gbeg[g + 1] - gbeg[g]) {   // padded channel: a whole slot of zeros, every window at its start
                     m.start = 0;
                     m.row = 0;
                     m.pad = 0;
@@ -163,6 +257,7 @@ dd_status build_tiles(dd_plan_s *p)
                     }
                     continue;
                 }
+                const int c = gbeg[g] + k;   // position in the live list
                 m = span0[static_cast<size_t>(b) * nchans + c];
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);
@@ -171,7 +266,7 @@ dd_status build_tiles(dd_plan_s *p)
                         reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
                     } else if (v.rel_bytes == 4) {
                         reinterpret_cast<uint32_t *>(rel.data())[base + i] = off * 4u;
-                    } else {   // bit planes: 32 samples per group of nbits words
+                    } else {   // bit planes: 32 samples per unit of unit_bytes
                         uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
                         e[0] = slot_off + (off >> 5) * static_cast<uint32_t>(v.unit_bytes);
                         e[1] = off & 31u;
@@ -180,6 +275,8 @@ dd_status build_tiles(dd_plan_s *p)
             }
         }
         p->cc = cc;
+        p->ngroups = ngroups;
+        p->group_cols = group_cols;
         p->nblk = nblk;
         p->nchans_pad = nchans_pad;
         p->smem_bytes = smem_layout_bytes(p, cc);

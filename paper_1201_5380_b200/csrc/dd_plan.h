@@ -61,6 +61,20 @@ struct dd_plan_s {
     std::vector<uint8_t> keep;    // [nchans] 1 = summed, 0 = skipped; empty = no mask
     std::vector<int32_t> live;    // rows of the summed channels (built by build_tiles)
     int nlive = 0;
+    // channel groups: with group_size > 0 every run of group_size consecutive channels is summed on its own (the
+    // sub-bands of PAPER.md:317); the launch then treats (beam, group) as the batch index.  0 = one group.
+    int group_size = 0;
+    int ngroups = 1;       // built by build_tiles
+    int group_cols = 0;    // columns of span/rel per group: the largest live count of a group, padded to a multiple of cc
+    // sub-band method: two direct steps through sub-plans and a temporary buffer
+    int sb_nchans = 0, dm_group = 0;      // channels per sub-band N'nu, trials per nominal DM N'DM; 0 = direct
+    dd_plan_s *s1 = nullptr;              // step 1: sub-bands x nominal DMs, uint8 sums (owned)
+    dd_plan_s *s2 = nullptr;              // step 2: the miniature filterbanks, 8-bit input (owned)
+    std::vector<int32_t> sb_nominal;      // [ngroups of trials] index of the nominal trial
+    int64_t sb_max_d2 = 0;                // largest step-2 delay: step 1 computes nsamps + sb_max_d2 samples
+    int64_t sb_extent = -1;               // input samples per row beyond nsamps that the two steps read
+    void *d_tmp = nullptr;                // intermediate series [beam][sub-band][nominal DM][t], uint8
+    size_t tmp_bytes = 0;
     // batching
     int nbeams = 1;
     int64_t in_beam_stride = 0, out_beam_stride = 0;
@@ -77,7 +91,7 @@ struct dd_plan_s {
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
-    std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels
+    std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels (nchans_pad = ngroups * group_cols)
     std::vector<uint8_t> rel;         // [nblk][nchans_pad][DB] entries of var.rel_bytes: delay - span start per DM slot
     // device copies
     int device = -1;
@@ -101,6 +115,11 @@ namespace dd {
 // if a delay does not fit int32.
 dd_status compute_delay_table(dd_plan_s *p);
 
+// The two sub-plans of the sub-band method for p's DM list, kill mask and (sb_nchans, dm_group): fills s1/s2
+// (delay tables + tiles), sb_nominal, sb_max_d2, sb_extent.  s1/s2 must be fresh plans.
+dd_status build_subband(const dd_plan_s *p, dd_plan_s *s1, dd_plan_s *s2, std::vector<int32_t> *nominal,
+                        int64_t *max_d2, int64_t *extent);
+
 // Chooses the kernel variant and builds span/rel metadata.  DD_ERR_SMEM if no tiling fits.
 dd_status build_tiles(dd_plan_s *p);
 
@@ -108,5 +127,6 @@ dd_status build_tiles(dd_plan_s *p);
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
 
 constexpr int64_t kMaxDynSmem = 227 * 1024;   // usable shared memory per CTA on sm_100a
+constexpr int kOutU8 = 8;                     // internal output code: uint8 sums (sub-band intermediate), not in the C ABI
 
 }  // namespace dd

@@ -162,3 +162,28 @@ def test_killmask_host_side():
         m[:5000] = 1
         p.set_killmask(m)                           # 5000 * 15 > 65535: still out of range
         assert dd.lib().dd_execute(p.handle, 100, 16, 4096, 16, 16, None) == -6
+
+
+def test_subband_host_side():
+    # argument checks and tables of the sub-band method, no device needed
+    cfg = W.CONFIGS[2]
+    dms = cfg.dm_list()[:100]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        L, h = dd.lib(), p.handle
+        assert L.dd_set_subband(None, 32, 32) == -1
+        assert L.dd_set_subband(h, 33, 32) == -2           # does not divide nchans
+        assert L.dd_set_subband(h, 32, 20) == -2           # not a multiple of 16
+        assert L.dd_set_subband(h, 128, 32) == -6          # 128 * 3 > 255: intermediate series do not fit 8 bits
+        assert L.dd_get_subband_extent(h) == -3            # no DM list
+        p.set_subband(32, 32)                              # before the DM list: remembered
+        p.set_dm_list(dms)
+        nominal, d1, d2 = p.subband_tables()
+        rn, r1, r2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, 32, 32)
+        assert np.array_equal(nominal, rn) and np.array_equal(d1, r1) and np.array_equal(d2, r2)
+        assert p.subband_extent == oracle.subband_required_samples(1000, r1, r2, 32) - 1000
+        # the direct delay table is untouched, and rows shorter than nsamps + extent are refused
+        assert np.array_equal(p.delay_table().astype(np.int64),
+                              oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms))
+        assert L.dd_execute_host(h, 100, 16, 4096, 16, 32) == -2
+        p.set_subband(0, 0)
+        assert L.dd_get_subband_extent(h) == -2

@@ -230,6 +230,52 @@ def test_killmask_4_and_8_bit_batch_and_host_path(nbits):
         assert np.array_equal(h_out[b].numpy(), ref)
 
 
+@pytest.mark.parametrize("case", [
+    # (config, nchans, ndm, nsamps, sb_nchans, dm_group, nbeams, masked)
+    (2, 256, 50, 5120 + 333, 32, 16, 1, False),     # 2-bit, ragged last group of trials, two time tiles
+    (2, 256, 70, 1500, 64, 32, 2, True),            # two beams, kill mask, ragged last group
+    (2, 96, 33, 700, 8, 16, 1, False),              # sub-bands smaller than a stage (padded groups)
+    (2, 1024, 48, 2000, 1, 16, 1, False),           # 1-channel sub-bands: the direct transform through 2 steps
+    (4, 64, 40, 3072 + 50, 16, 16, 1, True),        # 4-bit: 16 * 15 = 240 <= 255
+    (5, 48, 35, 900, 1, 32, 1, False),              # 8-bit input: only 1-channel sub-bands fit 8-bit intermediates
+])
+def test_subband_method_matches_the_two_step_oracle(case):
+    idx, nchans, ndm, nsamps, sb, grp, nbeams, masked = case
+    cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=nbeams)
+    dms = cfg.dm_list()
+    nominal, d1, d2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb, grp)
+    extent = oracle.subband_required_samples(nsamps, d1, d2, sb) - nsamps
+    packed, stride = W.gen_packed(cfg, max(extent, int(_oracle_table(cfg).max())))
+    dev = packed.cuda()
+    mask = (np.arange(nchans) % 7 != 3).astype(np.int32) if masked else None
+    out = torch.full((nbeams, ndm, nsamps), -1, dtype=torch.int32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        p.set_killmask(mask)
+        p.set_subband(sb, grp)
+        assert p.subband_extent == extent
+        g_nom, g_d1, g_d2 = p.subband_tables()
+        assert np.array_equal(g_nom, nominal) and np.array_equal(g_d1, d1) and np.array_equal(g_d2, d2)
+        if nbeams > 1:
+            p.set_batch(nbeams, dev.stride(0), out.stride(0) * 4)
+        p.execute(nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert p.launch_info()["last_launches"] == 4
+        got = out.cpu().numpy().view(np.uint32)
+        for b in range(nbeams):
+            ref = oracle.subband_dedisperse(packed[b].numpy(), cfg.nbits, nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df,
+                                            dms, sb, grp, mask=mask)
+            assert np.array_equal(got[b], ref), f"beam {b}"
+        if sb == 1:       # and that IS the direct transform
+            assert np.array_equal(got[0], oracle.dedisperse(packed[0].numpy(), cfg.nbits, nsamps, _oracle_table(cfg)))
+        # back to the direct transform on the same plan
+        p.set_subband(0, 0)
+        p.execute(nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, nsamps, _oracle_table(cfg), mask=mask)
+        assert np.array_equal(out[0].cpu().numpy().view(np.uint32), ref)
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)
