@@ -24,7 +24,7 @@ import numpy as np
 from . import build as _build
 from .oracle_np import (delay_table_np, dedisperse_gather_np, dedisperse_points,  # noqa: F401
                         unpack_np, dedisperse_loops_py, subband_tables, subband_required_samples,
-                        subband_dedisperse_np)
+                        subband_dedisperse_np, time_scrunch_np)
 
 _LIB: Optional[ctypes.CDLL] = None
 
@@ -130,6 +130,11 @@ def subband_dedisperse(packed: np.ndarray, nbits: int, nsamps: int, nchans: int,
     need = subband_required_samples(nsamps, delta1, delta2, sb_nchans)
     a = unpack(packed, nbits, need)
     return subband_dedisperse_np(a, nsamps, nominal, delta1, delta2, sb_nchans, dm_group, mask=mask)
+
+
+def time_scrunch(packed: np.ndarray, nbits_in: int, nsamps_out: int) -> np.ndarray:
+    """Time-scrunching of packed rows uint8 [nrows][stride]: unpacked int64 sums [nrows][nsamps_out]."""
+    return time_scrunch_np(unpack(packed, nbits_in, 2 * nsamps_out), nsamps_out)
 
 
 def cast_out(sums: np.ndarray, kind: str) -> np.ndarray:

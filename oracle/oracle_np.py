@@ -142,3 +142,14 @@ def subband_dedisperse_np(a: np.ndarray, nsamps: int, nominal, delta1, delta2, s
             o = int(delta2[d][b])
             out[d] += S[b, g, o:o + nsamps]
     return out
+
+
+# ------------------------------------------------------------------------------------------ time-scrunching
+def time_scrunch_np(a: np.ndarray, nsamps_out: int) -> np.ndarray:
+    """"reduce the time resolution by a factor of two ... by adding adjacent pairs of time
+    samples": out[c][t] = a[c][2t] + a[c][2t+1], 0 <= t < nsamps_out, on unpacked samples (int64 out)."""
+    a = np.asarray(a).astype(np.int64)
+    out = np.zeros((a.shape[0], nsamps_out), dtype=np.int64)
+    for t in range(nsamps_out):
+        out[:, t] = a[:, 2 * t] + a[:, 2 * t + 1]
+    return out

@@ -16,6 +16,7 @@ Pin numbering follows DESIGN.md section 3 (P1..P12).  None of these tests touche
   P12 kill mask: equals the unmasked sum over zeroed rows; complements add up
   P13 sub-band method: reduces to the direct transform for 1-channel sub-bands; equals a direct transform with
       the summed delays; error of the summed delays within the analytic bound; impulse response
+  P14 time-scrunching: hand example, conservation of the total, equals a reshape-sum
 """
 import math
 import os
@@ -414,6 +415,27 @@ def test_p13_subband_impulse_response():
                 if 0 <= t < nsamps:
                     want[t] = 3
                 assert np.array_equal(out[d], want)
+
+
+# ----------------------------------------------------------------------------- P14
+def test_p14_time_scrunch():
+    """adjacent pairs added.  Hand example: byte 0xE4 = 2-bit samples 0,1,2,3 -> sums 1, 5; totals are
+    conserved; scrunching commutes with the DM = 0 channel sum; a pulse of width 2 aligned on a pair keeps its area
+    in one sample."""
+    assert oracle.time_scrunch(np.array([[0xE4]], np.uint8), 2, 2).tolist() == [[1, 5]]
+    assert oracle.time_scrunch(np.array([[0x21, 0xFF]], np.uint8), 4, 2).tolist() == [[3, 30]]
+    rng = np.random.default_rng(14)
+    for nbits in (2, 4, 8):
+        a = rng.integers(0, 1 << nbits, size=(5, 128)).astype(np.uint8)
+        p = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+        s = oracle.time_scrunch(p, nbits, 64)
+        assert s.shape == (5, 64) and np.array_equal(s.sum(axis=1), a.astype(np.int64).sum(axis=1))
+        assert np.array_equal(s, a.reshape(5, 64, 2).astype(np.int64).sum(axis=2))
+        assert np.array_equal(s.sum(axis=0), oracle.time_scrunch_np(a.astype(np.int64).sum(axis=0)[None, :], 64)[0])
+        assert np.array_equal(oracle.time_scrunch(p, nbits, 10), s[:, :10])
+    z = np.zeros((1, 32), np.uint8)
+    z[0, 10:12] = 3
+    assert oracle.time_scrunch_np(z, 16)[0].tolist() == [0] * 5 + [6] + [0] * 10
 
 
 # --------------------------------------------------------------- oracle regression
