@@ -175,6 +175,23 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
                           void *out_host, int out_nbits);
 
 /*
+ * dd_time_scrunch -- "time-scrunching": halves the time resolution of packed rows by adding
+ * adjacent pairs of samples, out[r][t] = in[r][2t] + in[r][2t+1], 0 <= t < nsamps_out.  The scrunched rows are
+ * packed like the input (LSB first, reading R9) at a width that holds the sums, so that they can be dedispersed by
+ * a plan created with 2*dt and nbits_out (the paper applies this beyond the "diagonal" DM, then again at 2x, 4x...).
+ *   nrows       rows (channels, or beams * channels when the beams are adjacent) (> 0).
+ *   nsamps_out  output samples per row (> 0).
+ *   in_ptr      DEVICE, 16-byte aligned; rows in_stride bytes apart (multiple of 16), readable for
+ *               ceil16(nsamps_out * nbits_out / 8) * 2 * nbits_in / nbits_out bytes (whole 16-byte groups are read).
+ *   out_ptr     DEVICE, 16-byte aligned; rows out_stride bytes apart (multiple of 16, >= ceil16(nsamps_out*nbits_out/8));
+ *               the row is written up to that 16-byte boundary.
+ *   nbits_in / nbits_out   (2, 4), (2, 8) or (4, 8); DD_ERR_OUT_RANGE when 2*(2^nbits_in - 1) > 2^nbits_out - 1.
+ * Asynchronous on `stream`; no plan is involved.
+ */
+dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int64_t in_stride, int nbits_in, void *out_ptr,
+                          int64_t out_stride, int nbits_out, void *stream);
+
+/*
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
  *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20).

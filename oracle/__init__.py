@@ -11,7 +11,7 @@ Contents
   oracle_np.py         a second, independent numpy formulation + per-point evaluation
   this file            ctypes wrapper around the C library + the O6 cast
 
-Parity status: all functions pinned (tests/test_oracle_pins.py, pins P1..P12 in DESIGN.md §3).
+Parity status: all functions pinned (tests/test_oracle_pins.py, pins P1..P14 in DESIGN.md §3 and §10).
 """
 from __future__ import annotations
 

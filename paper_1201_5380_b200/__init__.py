@@ -20,7 +20,7 @@ __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
-    "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
@@ -31,7 +31,7 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
-    "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
 )
 
@@ -75,6 +75,8 @@ def lib() -> ctypes.CDLL:
         L.dd_get_max_delay.argtypes = [vp]
         L.dd_get_max_delay.restype = i64
         L.dd_set_batch.argtypes = [vp, i32, i64, i64]
+        L.dd_time_scrunch.argtypes = [i32, i64, vp, i64, i32, vp, i64, i32, vp]
+        L.dd_time_scrunch.restype = i32
         L.dd_set_killmask.argtypes = [vp, vp]
         L.dd_set_subband.argtypes = [vp, i32, i32]
         L.dd_set_subband.restype = i32
@@ -175,6 +177,13 @@ def dd_set_killmask(plan: int, mask) -> None:
         return
     m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.int32)
     _check(lib().dd_set_killmask(plan, ctypes.c_void_p(m.ctypes.data)), "dd_set_killmask")
+
+
+def dd_time_scrunch(nrows: int, nsamps_out: int, in_ptr, in_stride: int, nbits_in: int, out_ptr, out_stride: int,
+                    nbits_out: int, stream=None) -> None:
+    """out[r][t] = in[r][2t] + in[r][2t+1] on packed DEVICE rows; asynchronous."""
+    _check(lib().dd_time_scrunch(int(nrows), int(nsamps_out), _addr(in_ptr), int(in_stride), int(nbits_in), _addr(out_ptr),
+                                 int(out_stride), int(nbits_out), _stream(stream)), "dd_time_scrunch")
 
 
 def dd_set_subband(plan: int, sb_nchans: int, dm_group: int) -> None:

@@ -692,6 +692,32 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     return DD_OK;
 }
 
+dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int64_t in_stride, int nbits_in, void *out_ptr,
+                          int64_t out_stride, int nbits_out, void *stream)
+{
+    if (!in_ptr || !out_ptr)
+        return DD_ERR_NULL;
+    if (nrows <= 0 || nsamps_out <= 0 || (nbits_in != 2 && nbits_in != 4 && nbits_in != 8) ||
+        (nbits_out != 2 && nbits_out != 4 && nbits_out != 8))
+        return DD_ERR_INVALID_ARG;
+    if (2 * ((1 << nbits_in) - 1) > (1 << nbits_out) - 1)
+        return DD_ERR_OUT_RANGE;   // the pair sums do not fit the output width (8-bit input has no wider packed width)
+    if (reinterpret_cast<uintptr_t>(in_ptr) % 16 != 0 || reinterpret_cast<uintptr_t>(out_ptr) % 16 != 0 || in_stride % 16 != 0 ||
+        out_stride % 16 != 0)
+        return DD_ERR_ALIGNMENT;
+    if (nsamps_out > (INT64_MAX / 64))
+        return DD_ERR_INVALID_ARG;
+    const int64_t out_bytes = ((nsamps_out * nbits_out + 7) / 8 + 15) / 16 * 16;
+    const int64_t in_bytes = out_bytes * 2 * nbits_in / nbits_out;   // whole 16-byte groups of the input are read
+    if (out_stride < out_bytes || in_stride < in_bytes)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    const cudaError_t e = launch_scrunch(nbits_in, nbits_out, nrows, static_cast<const uint8_t *>(in_ptr), in_stride,
+                                         static_cast<uint8_t *>(out_ptr), out_stride, out_bytes, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess)
+        return cuda_fail(e, "dd_time_scrunch launch");
+    return DD_OK;
+}
+
 dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)

@@ -44,6 +44,10 @@ cudaError_t launch_variant2(const dd_plan_s *plan, const KernelParams &kp, cudaS
 // variant 3 launches two kernels (bit-plane transpose into plan->d_work, then the transform); it may grow d_work
 cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 
+// Time-scrunching of packed rows (dd_scrunch.cu).  out_bytes = bytes of every output row to produce (multiple of 16).
+cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t *in, int64_t in_stride, uint8_t *out,
+                           int64_t out_stride, int64_t out_bytes, cudaStream_t stream);
+
 // Kernels one launch_direct call enqueues for this plan.
 int launches_per_execute(const dd_plan_s *plan);
 

@@ -187,3 +187,19 @@ def test_subband_host_side():
         assert L.dd_execute_host(h, 100, 16, 4096, 16, 32) == -2
         p.set_subband(0, 0)
         assert L.dd_get_subband_extent(h) == -2
+
+
+def test_time_scrunch_argument_checks_need_no_gpu():
+    L = dd.lib()
+    ok = (4, 1000, 16, 512, 2, 32, 512, 4, None)
+    def call(**kw):
+        names = ("nrows", "nsamps_out", "in_ptr", "in_stride", "nbits_in", "out_ptr", "out_stride", "nbits_out", "stream")
+        a = dict(zip(names, ok))
+        a.update(kw)
+        return L.dd_time_scrunch(*[a[n] for n in names])
+    assert call(in_ptr=None) == -1 and call(out_ptr=None) == -1
+    assert call(nrows=0) == -2 and call(nsamps_out=0) == -2 and call(nbits_in=3) == -2 and call(nbits_out=16) == -2
+    assert call(nbits_in=2, nbits_out=2) == -6 and call(nbits_in=4, nbits_out=4) == -6 and call(nbits_in=8, nbits_out=8) == -6
+    assert call(in_ptr=24) == -4 and call(out_ptr=8) == -4 and call(in_stride=520) == -4 and call(out_stride=500) == -4
+    assert call(out_stride=496) == -5          # 1000 4-bit samples = 500 bytes -> 512
+    assert call(in_stride=496) == -5           # 512 output bytes of 4-bit sums need 512 input bytes of 2-bit samples

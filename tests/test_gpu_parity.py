@@ -276,6 +276,36 @@ def test_subband_method_matches_the_two_step_oracle(case):
         assert np.array_equal(out[0].cpu().numpy().view(np.uint32), ref)
 
 
+@pytest.mark.parametrize("widths", [(2, 4), (2, 8), (4, 8)])
+def test_time_scrunch_and_dedispersion_of_the_scrunched_series(widths):
+    # pairs of samples added; then the scrunched rows go through a plan made with 2*dt
+    nin, nout = widths
+    base = W.CONFIGS[2 if nin == 2 else 4]
+    nchans, ndm, ns2 = 64, 20, 2000 + 37                       # scrunched output samples per DM trial
+    cfg2x = W.Config(name="scrunched", index=base.index, nchans=nchans, f_top=base.f_top, df=base.df, dt=2 * base.dt,
+                     nbits=nout, nsamps=ns2, ndm=ndm, dm_max=400.0, out="u32", dist="uniform", seed=71)
+    tab2 = _oracle_table(cfg2x)                                # delays in units of 2*dt
+    n2 = ns2 + int(tab2.max())                                 # scrunched samples per row
+    src = base.reduced(nsamps=2 * n2, ndm=1, nchans=nchans)    # 2*n2 raw samples per row, no extra delay
+    packed, stride = W.gen_packed(src, 64)
+    out_stride = ((n2 * nout + 7) // 8 + 15) // 16 * 16
+    dev_in = packed[0].cuda()
+    dev_s = torch.zeros((nchans, out_stride), dtype=torch.uint8, device="cuda")
+    dd.dd_time_scrunch(nchans, n2, dev_in, stride, nin, dev_s, out_stride, nout, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    want = oracle.time_scrunch(packed[0].numpy(), nin, n2)      # unpacked int64 sums
+    got = oracle.unpack(dev_s.cpu().numpy(), nout, n2).astype(np.int64)
+    assert np.array_equal(got, want) and int(want.max()) == 2 * ((1 << nin) - 1)
+    # the scrunched rows through the transform at half the time resolution
+    out = torch.full((ndm, ns2), -1, dtype=torch.int32, device="cuda")
+    with dd.Plan(nchans, cfg2x.dt, cfg2x.f_top, cfg2x.df, nout) as p:
+        p.set_dm_list(cfg2x.dm_list())
+        p.execute(ns2, dev_s, out_stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+    ref = oracle.dedisperse_unpacked(want.astype(np.uint8), ns2, tab2)
+    assert np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)

@@ -1,6 +1,6 @@
 """Pins for the CPU oracle (oracle/) -- what the paper and the mathematics fix, NOT the oracle re-typed.
 
-Pin numbering follows DESIGN.md section 3 (P1..P12).  None of these tests touches the CUDA path.
+Pin numbering follows DESIGN.md section 3 (P1..P14).  None of these tests touches the CUDA path.
 
   P1  hand-evaluated eq. 1 delays (tests/golden/delays_eq1_hand.txt)
   P2  closed-form properties + exact rational arithmetic (fractions.Fraction)
