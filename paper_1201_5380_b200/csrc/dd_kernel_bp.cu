@@ -345,6 +345,51 @@ __device__ __forceinline__ void store4(const KernelParams &p, uint8_t *orow, int
     }
 }
 
+// One unit (32 consecutive sums per lane) of a warp to global memory through the warp's shared-memory patch.
+// Each lane packs its 32 sums into CH = 2 ES chunks of 16 bytes and writes them to its row of the patch; then
+// the warp reads the patch back so that consecutive lanes hold consecutive chunks of the SAME unit and stores:
+// every STG.128 covers whole 128-byte lines (4 units of float32) instead of 32 scattered 16-byte pieces.
+// The chunk index is XOR-swizzled so that both the write and the read phase are free of bank conflicts.
+//   ES     bytes per output element (4, 2, 1);  F32: convert to float32
+//   gunit  address of this unit of lane 0;  lane s's unit is s * lane_pitch bytes further
+template <int ES, bool F32>
+__device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], uint8_t *patch, int lane, uint8_t *gunit,
+                                                     int lane_pitch)
+{
+    constexpr int CH = 2 * ES;            // 16-byte chunks per unit
+    constexpr int LPL = 8 / CH;           // lanes per 128 bytes of the patch
+    const int swz = (lane / LPL) % CH;
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+        uint4 v;
+        if constexpr (ES == 4) {
+            if constexpr (F32)
+                v = make_uint4(__float_as_uint(__uint2float_rn(q[4 * c])), __float_as_uint(__uint2float_rn(q[4 * c + 1])),
+                               __float_as_uint(__uint2float_rn(q[4 * c + 2])), __float_as_uint(__uint2float_rn(q[4 * c + 3])));
+            else
+                v = make_uint4(q[4 * c], q[4 * c + 1], q[4 * c + 2], q[4 * c + 3]);
+        } else if constexpr (ES == 2) {
+            v = make_uint4(q[8 * c] | (q[8 * c + 1] << 16), q[8 * c + 2] | (q[8 * c + 3] << 16),
+                           q[8 * c + 4] | (q[8 * c + 5] << 16), q[8 * c + 6] | (q[8 * c + 7] << 16));
+        } else {
+            uint32_t w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                w[k] = q[16 * c + 4 * k] | (q[16 * c + 4 * k + 1] << 8) | (q[16 * c + 4 * k + 2] << 16) | (q[16 * c + 4 * k + 3] << 24);
+            v = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        *reinterpret_cast<uint4 *>(patch + lane * (CH * 16) + ((c ^ swz) * 16)) = v;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < CH; ++i) {
+        const int idx = i * 32 + lane, src = idx / CH, c = idx % CH;
+        const uint4 v = *reinterpret_cast<const uint4 *>(patch + src * (CH * 16) + ((c ^ ((src / LPL) % CH)) * 16));
+        *reinterpret_cast<uint4 *>(gunit + static_cast<int64_t>(src) * lane_pitch + c * 16) = v;
+    }
+    __syncwarp();
+}
+
 template <int NBITS>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
@@ -373,7 +418,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     uint64_t *empty = full + 8;                                 // [NS]
     const int rel_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * DB * 8));
     const int raw_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * p.raw_slot));
-    uint8_t *rel_base = smem + 128;
+    uint8_t *rel_base = smem + 128 + BP_NWARPS * kBpPatchBytes;   // after the warps' output patches
     uint8_t *raw_base = rel_base + NS * rel_stage;
 
     if (tid == 0) {
@@ -484,14 +529,19 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     }
 
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp`
+    // Interior tiles (the whole time block inside the row, vector stores allowed) go through a per-warp patch of
+    // shared memory so that every store instruction writes whole 128-byte lines.  The patches lie outside the
+    // stage ring: a warp that is done stores while the others are still adding.
     const int d = blk * DB + warp;
     if (d >= p.ndm)
         return;
     const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
     uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
+    const bool interior = p.vec_ok && (t0 + TB <= p.nsamps);
+    uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
 #pragma unroll
     for (int j = 0; j < W; ++j) {
-        const int64_t tunit = t0 + 32 * (W * lane + j);
+        uint32_t q[32];   // the 32 sums of the unit, in time order
         if constexpr (NP <= 16) {
             uint32_t R[16];
 #pragma unroll
@@ -499,23 +549,32 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                 R[k] = k < NP ? P[j][k] : 0u;
             transpose16x2(R);
 #pragma unroll
-            for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
-                uint32_t q[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    q[k] = h < 4 ? (R[4 * h + k] & 0xFFFFu) : (R[4 * (h - 4) + k] >> 16);
-                store4(p, orow, tunit + 4 * h, q);
+            for (int k = 0; k < 16; ++k) {
+                q[k] = R[k] & 0xFFFFu;
+                q[16 + k] = R[k] >> 16;
             }
         } else {
-            uint32_t R[32];
 #pragma unroll
             for (int k = 0; k < 32; ++k)
-                R[k] = k < NP ? P[j][k] : 0u;
-            transpose32(R);
+                q[k] = k < NP ? P[j][k] : 0u;
+            transpose32(q);
+        }
+        if (interior) {
+            uint8_t *gunit = orow + (t0 + 32 * j) * esize;   // unit j of lane 0; lane s is W * 32 samples further
+            if (p.out_code == DD_OUT_F32)
+                store_unit_coalesced<4, true>(q, patch, lane, gunit, W * 32 * 4);
+            else if (p.out_code == DD_OUT_U32)
+                store_unit_coalesced<4, false>(q, patch, lane, gunit, W * 32 * 4);
+            else if (p.out_code == DD_OUT_U16)
+                store_unit_coalesced<2, false>(q, patch, lane, gunit, W * 32 * 2);
+            else
+                store_unit_coalesced<1, false>(q, patch, lane, gunit, W * 32);
+        } else {
+            const int64_t tunit = t0 + 32 * (W * lane + j);
 #pragma unroll
-            for (int h = 0; h < 8; ++h) {
-                const uint32_t q[4] = {R[4 * h], R[4 * h + 1], R[4 * h + 2], R[4 * h + 3]};
-                store4(p, orow, tunit + 4 * h, q);
+            for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
+                const uint32_t q4[4] = {q[4 * h], q[4 * h + 1], q[4 * h + 2], q[4 * h + 3]};
+                store4(p, orow, tunit + 4 * h, q4);
             }
         }
     }

@@ -124,6 +124,8 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 {
     const Variant &v = p->var;
     int64_t bytes = 128;                                                                          // mbarriers
+    if (v.bitplane)   // one output patch per warp for the coalescing epilogue (kept apart from the stages, so that a
+        bytes += static_cast<int64_t>(v.threads / 32) * kBpPatchBytes;   // warp can store while others still add)
     bytes += p->nstages * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);           // offset-table stages
     bytes += p->nstages * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);                  // packed / bit-plane stages
     if (v.lane_bits != p->nbits)                                                                  // unpacked lanes

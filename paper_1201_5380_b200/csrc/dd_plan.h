@@ -127,6 +127,7 @@ dd_status build_tiles(dd_plan_s *p);
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
 
 constexpr int64_t kMaxDynSmem = 227 * 1024;   // usable shared memory per CTA on sm_100a
+constexpr int kBpPatchBytes = 4096;             // bit-plane kernel epilogue: shared memory per warp (32 lanes x 128 B)
 constexpr int kOutU8 = 8;                     // internal output code: uint8 sums (sub-band intermediate), not in the C ABI
 
 }  // namespace dd
