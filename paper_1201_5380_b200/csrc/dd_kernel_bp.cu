@@ -390,7 +390,9 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
     __syncwarp();
 }
 
-template <int NBITS>
+// PATCH: the epilogue goes through per-warp shared-memory patches (coalesced stores); the plan turns it off where
+// the channel loop is so long that a deeper stage ring is worth more than the epilogue (8-bit input, many channels).
+template <int NBITS, bool PATCH>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
     using C = Bp<NBITS>;
@@ -418,7 +420,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     uint64_t *empty = full + 8;                                 // [NS]
     const int rel_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * DB * 8));
     const int raw_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * p.raw_slot));
-    uint8_t *rel_base = smem + 128 + BP_NWARPS * kBpPatchBytes;   // after the warps' output patches
+    uint8_t *rel_base = smem + 128 + (PATCH ? BP_NWARPS * kBpPatchBytes : 0);   // after the warps' output patches
     uint8_t *raw_base = rel_base + NS * rel_stage;
 
     if (tid == 0) {
@@ -537,7 +539,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         return;
     const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
     uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
-    const bool interior = p.vec_ok && (t0 + TB <= p.nsamps);
+    const bool interior = PATCH && p.vec_ok && (t0 + TB <= p.nsamps);
     uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
 #pragma unroll
     for (int j = 0; j < W; ++j) {
@@ -621,13 +623,14 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     kp.in_row_bytes = conv;
     kp.in_beam_stride = w_beam;
 
-    e = cudaFuncSetAttribute(dd_direct_bp<NBITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
-    if (e != cudaSuccess)
-        return e;
     const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * kp.ngroups;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
-    dd_direct_bp<NBITS><<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
+    auto kernel = plan->patch ? dd_direct_bp<NBITS, true> : dd_direct_bp<NBITS, false>;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
+    if (e != cudaSuccess)
+        return e;
+    kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
     return cudaGetLastError();
 }
 

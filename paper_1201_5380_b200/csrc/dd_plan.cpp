@@ -124,8 +124,8 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 {
     const Variant &v = p->var;
     int64_t bytes = 128;                                                                          // mbarriers
-    if (v.bitplane)   // one output patch per warp for the coalescing epilogue (kept apart from the stages, so that a
-        bytes += static_cast<int64_t>(v.threads / 32) * kBpPatchBytes;   // warp can store while others still add)
+    if (p->patch)   // one output patch per warp for the coalescing epilogue (kept apart from the stages,
+        bytes += static_cast<int64_t>(v.threads / 32) * kBpPatchBytes;   // so that a warp can store while others still add); Bp<nbits>::PATCH
     bytes += p->nstages * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);           // offset-table stages
     bytes += p->nstages * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);                  // packed / bit-plane stages
     if (v.lane_bits != p->nbits)                                                                  // unpacked lanes
@@ -178,6 +178,9 @@ dd_status build_tiles(dd_plan_s *p)
         if (ngroups > 1 && !v.bitplane)
             continue;   // channel groups are served by the bit-plane kernel only
         p->var = v;
+        // 8-bit input costs four times the work of 2-bit input per channel: with many channels the epilogue is
+        // a per-mille effect and a deeper ring matters more; with few (sub-band step 2) the epilogue dominates
+        p->patch = v.bitplane && (nbits < 8 || gmax <= 256);
         const int DB = v.DB;
         const int nblk = (ndm + DB - 1) / DB;
         const int64_t rel_limit = v.rel_bytes == 2 ? 65535 : (int64_t(1) << 26);
