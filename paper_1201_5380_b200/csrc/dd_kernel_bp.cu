@@ -88,7 +88,8 @@ __device__ __forceinline__ uint2 planes_of(uint32_t x0, uint32_t x1)
 
 // in: packed rows [beam][c][in_stride]; work: bit-plane rows [beam][c][sub][w_sub bytes].  One thread writes
 // 16 bytes of every sub-row of a channel: 64 samples (2 units) of 2-bit input, 32 samples (1 unit) of 4- and
-// 8-bit input.  Input bytes at or beyond in_row_bytes read as zero (only the last, partial unit of an 8-bit row).
+// 8-bit input.  Input bytes at or beyond in_row_bytes read as zero: the bit-plane rows are longer than the input
+// (whole tiles plus the longest span), so that the transform kernel never has to clamp a copy.
 template <int NBITS>
 __global__ void __launch_bounds__(256) dd_to_bitplanes(const uint8_t *__restrict__ in, int64_t in_stride, int64_t in_row_bytes,
                                                        int64_t in_beam_stride, uint8_t *__restrict__ work, int64_t w_sub,
@@ -101,11 +102,13 @@ __global__ void __launch_bounds__(256) dd_to_bitplanes(const uint8_t *__restrict
     const uint8_t *row = in + beam * in_beam_stride + c * in_stride;
     uint8_t *wrow = work + beam * w_beam_stride + c * (Bp<NBITS>::NSUB * w_sub);
     if constexpr (NBITS == 2) {
-        const uint4 x = __ldg(reinterpret_cast<const uint4 *>(row) + i);
+        const uint4 x = (static_cast<int64_t>(i) * 16 + 16 <= in_row_bytes) ? __ldg(reinterpret_cast<const uint4 *>(row) + i)
+                                                                          : make_uint4(0, 0, 0, 0);
         const uint2 a = planes_of(x.x, x.y), b = planes_of(x.z, x.w);
         reinterpret_cast<uint4 *>(wrow)[i] = make_uint4(a.x, a.y, b.x, b.y);
     } else if constexpr (NBITS == 4) {
-        const uint4 x = __ldg(reinterpret_cast<const uint4 *>(row) + i);
+        const uint4 x = (static_cast<int64_t>(i) * 16 + 16 <= in_row_bytes) ? __ldg(reinterpret_cast<const uint4 *>(row) + i)
+                                                                          : make_uint4(0, 0, 0, 0);
         const uint32_t w[4] = {x.x, x.y, x.z, x.w};
         uint32_t pl[4];
 #pragma unroll
@@ -434,6 +437,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
 
     const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride +
                              (p.in_blk_div > 0 ? static_cast<int64_t>(blk / p.in_blk_div) * p.in_blk_stride : 0);
+    const uint8_t *in_tile = in_beam + (t0 >> 5) * UB;   // this tile's first unit in every sub-row
     const int64_t col0 = static_cast<int64_t>(blk) * p.nchans_pad + static_cast<int64_t>(group) * p.group_cols;
     const int4 *span_blk = p.span + col0;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + col0 * DB;
@@ -453,28 +457,19 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         if (lane == 0) {
             if (chunk >= NS)
                 mbar_wait(&empty[s], ((chunk / NS) - 1) & 1);   // every warp has finished chunk - NS
-            const uint8_t *src[CPW];
-            uint32_t bytes[CPW], tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
+            // span entry: {byte offset inside the sub-row for tile 0, bytes, row, -}; rows are padded by the launcher
+            // so that no copy needs clamping, and padded channels point at an all-zero row
+            uint32_t tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
 #pragma unroll
-            for (int k = 0; k < CPW; ++k) {
-                const int sub = (warp * CPW + k) % NSUB;
-                if (m[k].y < 0) {                                // padded channel: zeros
-                    src[k] = p.zero;
-                    bytes[k] = static_cast<uint32_t>(-m[k].y);
-                } else {
-                    const int64_t off = ((t0 + m[k].x) >> 5) * UB;
-                    const int64_t avail = p.in_row_bytes - off;
-                    bytes[k] = static_cast<uint32_t>(m[k].y < avail ? m[k].y : (avail > 0 ? avail : 0));
-                    src[k] = in_beam + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + off;
-                }
-                tx += bytes[k];
-            }
+            for (int k = 0; k < CPW; ++k)
+                tx += static_cast<uint32_t>(m[k].y);
             mbar_arrive_expect_tx(&full[s], tx);
 #pragma unroll
             for (int k = 0; k < CPW; ++k) {
                 const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
-                if (bytes[k])
-                    tma_bulk_g2s(raw_base + s * raw_stage + cl * p.raw_slot + sub * p.sub_slot, src[k], bytes[k], &full[s]);
+                const uint8_t *src = in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x;
+                tma_bulk_g2s(raw_base + s * raw_stage + cl * p.raw_slot + sub * p.sub_slot, src, static_cast<uint32_t>(m[k].y),
+                             &full[s]);
             }
             if (warp == 0)
                 tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(chunk) * CC * DB,
@@ -590,26 +585,35 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     if (plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB)
         return cudaErrorInvalidValue;
     KernelParams kp = kp_in;
-    // 16-byte groups of every sub-row the tiles can touch (2 units of 2-bit input, 1 unit otherwise)
+    // 16-byte groups of every sub-row the tiles can touch (2 units of 2-bit input, 1 unit otherwise).  The bit-plane
+    // rows are as long as the longest span needs, zero beyond the input, so that the kernel's copies need no
+    // clamping; behind the nrows input rows of a beam lie row_mul all-zero rows, the source of padded channels.
     const int64_t spg = (16 / (C::NB * 4)) * 32;   // samples per group
-    int64_t groups = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
-    const int64_t in_bytes_per_group = spg * NBITS / 8;
-    const int64_t have = (kp.in_row_bytes + in_bytes_per_group - 1) / in_bytes_per_group;
-    if (groups > have)
-        groups = have;
+    const int64_t groups = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
     const int64_t conv = groups * 16;   // bytes per sub-row
-    const size_t need = static_cast<size_t>(kp.nbeams) * kp.nrows * C::NSUB * static_cast<size_t>(conv);
+    const int64_t rows = static_cast<int64_t>(kp.nrows) + kp.row_mul;
+    const int64_t w_beam = rows * C::NSUB * conv;
+    const size_t need = static_cast<size_t>(kp.nbeams) * static_cast<size_t>(w_beam);
     cudaError_t e;
     if (plan->work_bytes < need) {
         if (plan->d_work)
             cudaFree(plan->d_work);   // synchronises with any kernel still reading the old buffer
         plan->d_work = nullptr;
         plan->work_bytes = 0;
+        plan->work_layout[0] = 0;
         if ((e = cudaMalloc(&plan->d_work, need)) != cudaSuccess)
             return e;
         plan->work_bytes = need;
     }
-    const int64_t w_beam = static_cast<int64_t>(kp.nrows) * C::NSUB * conv;
+    if (plan->work_layout[0] != conv || plan->work_layout[1] != rows || plan->work_layout[2] != kp.nbeams) {
+        e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_work) + static_cast<int64_t>(kp.nrows) * C::NSUB * conv,
+                              static_cast<size_t>(w_beam), 0, static_cast<size_t>(kp.row_mul) * C::NSUB * conv, kp.nbeams, stream);
+        if (e != cudaSuccess)
+            return e;
+        plan->work_layout[0] = conv;
+        plan->work_layout[1] = rows;
+        plan->work_layout[2] = kp.nbeams;
+    }
     dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
         kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv, w_beam,
         static_cast<int32_t>(groups));

@@ -252,9 +252,14 @@ dd_status build_tiles(dd_plan_s *p)
                 const uint32_t slot_off = static_cast<uint32_t>(k % cc) * static_cast<uint32_t>(p->raw_slot);
                 if (k >= gbeg[g + 1] - gbeg[g]) {   // padded channel: a whole slot of zeros, every window at its start
                     m.start = 0;
-                    m.row = 0;
                     m.pad = 0;
-                    m.nbytes = -(v.bitplane ? p->sub_slot : p->raw_slot);   // negative: stage from the zero buffer
+                    if (v.bitplane) {   // staged from the all-zero row the launcher keeps behind the input rows
+                        m.row = nrows;
+                        m.nbytes = p->sub_slot;
+                    } else {
+                        m.row = 0;
+                        m.nbytes = -p->raw_slot;   // negative: stage from the zero buffer
+                    }
                     for (int i = 0; i < DB; ++i) {
                         uint32_t *e = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
                         e[0] = slot_off;
@@ -264,9 +269,14 @@ dd_status build_tiles(dd_plan_s *p)
                 }
                 const int c = gbeg[g] + k;   // position in the live list
                 m = span0[static_cast<size_t>(b) * nchans + c];
+                const int32_t start = m.start;
+                if (v.bitplane) {   // the kernel wants the byte offset of the span inside a bit-plane sub-row (tile 0)
+                    m.pad = start;
+                    m.start = start / 32 * v.unit_bytes;
+                }
                 for (int i = 0; i < DB; ++i) {
                     const int d = std::min(b * DB + i, ndm - 1);
-                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nrows + live[c]] - m.start);
+                    const uint32_t off = static_cast<uint32_t>(p->delay[static_cast<size_t>(d) * nrows + live[c]] - start);
                     if (v.rel_bytes == 2) {
                         reinterpret_cast<uint16_t *>(rel.data())[base + i] = static_cast<uint16_t>(off);
                     } else if (v.rel_bytes == 4) {

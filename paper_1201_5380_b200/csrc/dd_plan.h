@@ -37,8 +37,10 @@ struct Variant {
 };
 
 struct SpanMeta {   // per (DM block, live channel); mirrored on the device as int4
-    int32_t start;  // first staged sample relative to the tile's first output sample; multiple of 128/nbits
-    int32_t nbytes; // packed bytes to stage (multiple of 16); negative: a padded channel staged from the zero buffer
+    int32_t start;  // first staged sample relative to the tile's first output sample; multiple of 128/nbits.
+                    // Bit-plane variants: the same as a byte offset inside a bit-plane sub-row (sample offset in `pad`)
+    int32_t nbytes; // packed bytes to stage (multiple of 16); negative (variants 1, 2): a padded channel staged from the
+                    // zero buffer; bit-plane variants stage padded channels from the zero row `row` = nchans
     int32_t row;    // the channel's row in the input (differs from its position in the list under a kill mask)
     int32_t pad;
 };
@@ -102,6 +104,7 @@ struct dd_plan_s {
     void *d_zero = nullptr;           // raw_slot zero bytes (source of the padded channels)
     void *d_work = nullptr;           // bit-plane copy of the input (variants with `bitplane`), grown on demand
     size_t work_bytes = 0;
+    int64_t work_layout[3] = {0, 0, 0};   // {bytes per sub-row, rows, beams} the zero rows of d_work were written for
     int64_t last_launches = 0;
     dd::HostStage *stage = nullptr;
     // optional per-kernel timing of dd_execute (dd_profile_enable): 3 events per recorded call
