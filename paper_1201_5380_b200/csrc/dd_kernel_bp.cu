@@ -452,11 +452,13 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         for (int k = 0; k < CPW; ++k)
             m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
     };
+    // chunk = round * NS + s: the ring position is carried along instead of divided out (NS is a run-time value)
+    int prod_s = 0, prod_round = 0;
     auto produce = [&](int chunk, const int4 (&m)[CPW]) {
-        const int s = chunk % NS;
+        const int s = prod_s;
         if (lane == 0) {
-            if (chunk >= NS)
-                mbar_wait(&empty[s], ((chunk / NS) - 1) & 1);   // every warp has finished chunk - NS
+            if (prod_round > 0)
+                mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has finished chunk - NS
             // span entry: {byte offset inside the sub-row for tile 0, bytes, row, -}; rows are padded by the launcher
             // so that no copy needs clamping, and padded channels point at an all-zero row
             uint32_t tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
@@ -476,6 +478,10 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                              static_cast<uint32_t>(CC * DB * 8), &full[s]);
         }
         __syncwarp();
+        if (++prod_s == NS) {
+            prod_s = 0;
+            ++prod_round;
+        }
     };
 
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in chunks (measured: 1 and 2 equal, 3 slower)
@@ -500,8 +506,9 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             T[j][k] = 0;
     }
 
+    int s = 0;
+    uint32_t full_parity = 0;
     for (int chunk = 0; chunk < p.nchunks; ++chunk) {
-        const int s = chunk % NS;
         if (chunk + dist < p.nchunks) {
             load_meta(chunk + dist + 1, nxt);
             produce(chunk + dist, meta);
@@ -509,7 +516,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             for (int i = 0; i < CPW; ++i)
                 meta[i] = nxt[i];
         }
-        mbar_wait(&full[s], (chunk / NS) & 1);
+        mbar_wait(&full[s], full_parity);
 
         BpShared sh;
         sh.lane_base = raw_base + s * raw_stage + lane * (W * UB);
@@ -523,6 +530,10 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         __syncwarp();
         if (lane == 0)
             mbar_arrive(&empty[s]);
+        if (++s == NS) {
+            s = 0;
+            full_parity ^= 1u;
+        }
     }
 
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp`
