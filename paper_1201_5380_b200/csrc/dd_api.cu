@@ -316,6 +316,7 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->group_cols = scratch.group_cols;
     plan->nstages = scratch.nstages;
     plan->patch = scratch.patch;
+    plan->long_mode = scratch.long_mode;
     plan->max_span_end = scratch.max_span_end;
     plan->raw_slot = scratch.raw_slot;
     plan->sub_slot = scratch.sub_slot;

@@ -39,20 +39,27 @@ namespace {
 
 constexpr int BP_DB = 16, BP_NWARPS = 16;
 
+// Tile shape per input width.  FL = stages between flushes of the pending words in the LONG instantiation
+// (dd_plan.cpp pads the channel list accordingly: kBpFlushStages there must agree).
+#ifndef DD_BP_FL2
+#define DD_BP_FL2 2   // measured on B200: cfg2 8.95 / 8.78 / 9.09 ms for 1 / 2 / 4 stages between flushes
+#define DD_BP_FL4 4   //                  cfg4 116.7 / 114.5 / 112.6 ms
+#define DD_BP_FL8 2   //                  cfg5 246.4 / 223.7 / 224.8 ms
+#endif
 // Tile shape per input width.  NP planes hold sums < 2^NP (the plan checks nchans * (2^nbits - 1) < 2^NP).
 template <int NBITS>
 struct Bp;
 template <>
 struct Bp<2> {
-    static constexpr int NB = 2, NSUB = 1, NP = 12, W = 5, CC = 32;
+    static constexpr int NB = 2, NSUB = 1, NP = 12, W = 5, CC = 32, FL = DD_BP_FL2;
 };
 template <>
 struct Bp<4> {
-    static constexpr int NB = 4, NSUB = 1, NP = 16, W = 3, CC = 16;
+    static constexpr int NB = 4, NSUB = 1, NP = 16, W = 3, CC = 16, FL = DD_BP_FL4;
 };
 template <>
 struct Bp<8> {
-    static constexpr int NB = 4, NSUB = 2, NP = 20, W = 3, CC = 8;
+    static constexpr int NB = 4, NSUB = 2, NP = 20, W = 3, CC = 8, FL = DD_BP_FL8;
 };
 
 __host__ __device__ constexpr int bit_length(uint32_t v) { return v == 0 ? 0 : 1 + bit_length(v >> 1); }
@@ -216,8 +223,8 @@ struct BpShared {
     int sub_slot;               // bytes between the sub-rows of a channel slot
 };
 
-// plane k of sub-row SUB of channel CL of the stage, for every unit of the lane
-template <int NBITS, int CL, int SUB, int K, int NP, int NT>
+// plane k of sub-row SUB of a channel, for every unit of the lane; CLS = channels added since the last flush
+template <int NBITS, int CLS, int SUB, int K, int NP, int NT>
 __device__ __forceinline__ void plane_step(const PlaneVec<Bp<NBITS>::NB> (&x)[Bp<NBITS>::W + 1], uint32_t shift,
                                            uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
@@ -225,17 +232,17 @@ __device__ __forceinline__ void plane_step(const PlaneVec<Bp<NBITS>::NB> (&x)[Bp
     if constexpr (K < C::NB) {
         constexpr int L = SUB * C::NB + K;                                   // weight 2^L
         constexpr uint32_t VMAX = (1u << NBITS) - 1u;
-        constexpr uint32_t S = VMAX * CL + ((1u << L) - 1u);                 // weight added to the counter so far
+        constexpr uint32_t S = VMAX * CLS + ((1u << L) - 1u);                // weight added to the counter so far
 #pragma unroll
         for (int j = 0; j < C::W; ++j)
             csa_add<S, L>(P[j], T[j], __funnelshift_r(x[j].w[K], x[j + 1].w[K], shift));
-        plane_step<NBITS, CL, SUB, K + 1>(x, shift, P, T);
+        plane_step<NBITS, CLS, SUB, K + 1>(x, shift, P, T);
     }
 }
 
 // channel CL of the stage: per sub-row one window of W+1 units serves W units; per unit and plane one funnel
 // shift + carry-save adds
-template <int NBITS, int CL, int SUB, int NP, int NT>
+template <int NBITS, int CLS, int SUB, int NP, int NT>
 __device__ __forceinline__ void subrow_step(const BpShared &sh, const uint2 e, uint32_t (&P)[Bp<NBITS>::W][NP],
                                             uint32_t (&T)[Bp<NBITS>::W][NT])
 {
@@ -246,16 +253,18 @@ __device__ __forceinline__ void subrow_step(const BpShared &sh, const uint2 e, u
 #pragma unroll
         for (int j = 0; j <= C::W; ++j)
             x[j].load(wp + j * (C::NB * 4));
-        plane_step<NBITS, CL, SUB, 0>(x, e.y, P, T);
-        subrow_step<NBITS, CL, SUB + 1>(sh, e, P, T);
+        plane_step<NBITS, CLS, SUB, 0>(x, e.y, P, T);
+        subrow_step<NBITS, CLS, SUB + 1>(sh, e, P, T);
     }
 }
 
-template <int NBITS, int NP, int NT, int... CLs>
+// PHASE: stages added since the last flush (the pending words are rippled into the planes every FL stages)
+template <int NBITS, int PHASE, int NP, int NT, int... CLs>
 __device__ __forceinline__ void stage_steps(std::integer_sequence<int, CLs...>, const BpShared &sh,
                                             uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
-    (subrow_step<NBITS, CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);   // rel entry: {byte offset in the stage, bit shift}
+    // rel entry: {byte offset in the stage, bit shift}
+    (subrow_step<NBITS, PHASE * Bp<NBITS>::CC + CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -393,16 +402,20 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
     __syncwarp();
 }
 
-// PATCH: the epilogue goes through per-warp shared-memory patches (coalesced stores); the plan turns it off where
-// the channel loop is so long that a deeper stage ring is worth more than the epilogue (8-bit input, many channels).
-template <int NBITS, bool PATCH>
+// LONG: the plan found many channels per group.  The pending words are then rippled into the planes only every
+// Bp<NBITS>::FL stages (the plan pads the channel list to whole groups of FL stages), and for 8-bit input the
+// epilogue stores straight from registers (a deeper stage ring is worth more than coalesced stores there).
+// Otherwise: a flush after every stage, and the epilogue goes through per-warp shared-memory patches.
+template <int NBITS, bool LONG>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
     using C = Bp<NBITS>;
     constexpr int DB = BP_DB, W = C::W, TB = 32 * 32 * W, CC = C::CC, NP = C::NP, NSUB = C::NSUB;
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
+    constexpr int FL = LONG ? C::FL : 1;
+    constexpr bool PATCH = !LONG || NBITS < 8;
     constexpr uint32_t STAGE_SUM = ((1u << NBITS) - 1u) * CC;        // largest value one stage adds to a counter
-    constexpr int NT = bit_length(STAGE_SUM);                        // pending slots
+    constexpr int NT = bit_length(FL * STAGE_SUM);                   // pending slots
     static_assert((CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
 
     extern __shared__ __align__(128) uint8_t smem[];
@@ -508,7 +521,11 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
 
     int s = 0;
     uint32_t full_parity = 0;
-    for (int chunk = 0; chunk < p.nchunks; ++chunk) {
+    // one stage: keep the ring fed, wait for the stage, add its CC channels (PHASE = stages since the last flush)
+    // FLUSH = weight the counter has taken since the last flush if the pending words are to be rippled in now, else 0
+    auto stage = [&](int chunk, auto phase, auto flush) {
+        constexpr int PHASE = decltype(phase)::value;
+        constexpr uint32_t FLUSH = decltype(flush)::value;
         if (chunk + dist < p.nchunks) {
             load_meta(chunk + dist + 1, nxt);
             produce(chunk + dist, meta);
@@ -522,17 +539,35 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         sh.lane_base = raw_base + s * raw_stage + lane * (W * UB);
         sh.rel = reinterpret_cast<const uint2 *>(rel_base + s * rel_stage) + warp;
         sh.sub_slot = p.sub_slot;
-        stage_steps<NBITS>(std::make_integer_sequence<int, CC>{}, sh, P, T);
+        stage_steps<NBITS, PHASE>(std::make_integer_sequence<int, CC>{}, sh, P, T);
+        if constexpr (FLUSH != 0u) {
 #pragma unroll
-        for (int j = 0; j < W; ++j)
-            csa_flush<STAGE_SUM, 0, false>(P[j], T[j], 0u);
-
+            for (int j = 0; j < W; ++j)
+                csa_flush<FLUSH, 0, false>(P[j], T[j], 0u);
+        }
         __syncwarp();
         if (lane == 0)
             mbar_arrive(&empty[s]);
         if (++s == NS) {
             s = 0;
             full_parity ^= 1u;
+        }
+    };
+    // groups of FL stages with one flush at the end (nchunks is a multiple of FL by plan construction)
+    using NoFlush = std::integral_constant<uint32_t, 0u>;
+    using FlushAll = std::integral_constant<uint32_t, FL * STAGE_SUM>;
+    for (int chunk = 0; chunk < p.nchunks; chunk += FL) {
+        if constexpr (FL == 1) {
+            stage(chunk, std::integral_constant<int, 0>{}, FlushAll{});
+        } else if constexpr (FL == 2) {
+            stage(chunk, std::integral_constant<int, 0>{}, NoFlush{});
+            stage(chunk + 1, std::integral_constant<int, 1>{}, FlushAll{});
+        } else {
+            static_assert(FL == 1 || FL == 2 || FL == 4, "unroll more phases here");
+            stage(chunk, std::integral_constant<int, 0>{}, NoFlush{});
+            stage(chunk + 1, std::integral_constant<int, 1>{}, NoFlush{});
+            stage(chunk + 2, std::integral_constant<int, 2>{}, NoFlush{});
+            stage(chunk + 3, std::integral_constant<int, 3>{}, FlushAll{});
         }
     }
 
@@ -641,7 +676,9 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * kp.ngroups;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
-    auto kernel = plan->patch ? dd_direct_bp<NBITS, true> : dd_direct_bp<NBITS, false>;
+    if (plan->long_mode && kp.nchunks % C::FL != 0)
+        return cudaErrorInvalidValue;
+    auto kernel = plan->long_mode ? dd_direct_bp<NBITS, true> : dd_direct_bp<NBITS, false>;
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)
         return e;

@@ -133,6 +133,14 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
     return bytes;
 }
 
+// Stages between flushes in the LONG bit-plane kernel: must agree with Bp<nbits>::FL (DD_BP_FL*) in dd_kernel_bp.cu.
+#ifndef DD_BP_FL2
+#define DD_BP_FL2 2
+#define DD_BP_FL4 4
+#define DD_BP_FL8 2
+#endif
+static int kBpFlushStages(int nbits) { return nbits == 2 ? DD_BP_FL2 : (nbits == 4 ? DD_BP_FL4 : DD_BP_FL8); }
+
 // The kernel variants compiled into the library, in order of preference.
 static const Variant kVariants[] = {
     /* id  DB   TB    thr tail rel lane lst rst  cc candidates     nbits                        sum  pad    bitplane */
@@ -178,9 +186,13 @@ dd_status build_tiles(dd_plan_s *p)
         if (ngroups > 1 && !v.bitplane)
             continue;   // channel groups are served by the bit-plane kernel only
         p->var = v;
-        // 8-bit input costs four times the work of 2-bit input per channel: with many channels the epilogue is
-        // a per-mille effect and a deeper ring matters more; with few (sub-band step 2) the epilogue dominates
-        p->patch = v.bitplane && (nbits < 8 || gmax <= 256);
+        // Bit planes: with many channels per group the LONG instantiation flushes the pending words only every
+        // kBpFlushStages stages (channel list padded to whole flush groups) and, for 8-bit input -- four times the
+        // work of 2-bit input per channel, the epilogue a per-mille effect -- spends the shared memory of the
+        // output patches on a deeper ring.  With few channels (sub-band steps) the epilogue dominates.
+        const int fl = v.bitplane ? kBpFlushStages(nbits) : 1;
+        p->long_mode = v.bitplane && gmax >= 8 * v.cc[0] * fl;
+        p->patch = v.bitplane && (!p->long_mode || nbits < 8);
         const int DB = v.DB;
         const int nblk = (ndm + DB - 1) / DB;
         const int64_t rel_limit = v.rel_bytes == 2 ? 65535 : (int64_t(1) << 26);
@@ -240,7 +252,7 @@ dd_status build_tiles(dd_plan_s *p)
             continue;
         // pass 2: per (DM, column) the position of that DM's window inside the staged span.  Column k of group g
         // is the k-th live channel of the group; columns past the group's live count are padded (zero) channels.
-        const int group_cols = v.pad_chunks ? static_cast<int>(align_up(gmax, cc)) : gmax;
+        const int group_cols = v.pad_chunks ? static_cast<int>(align_up(gmax, cc * (p->long_mode ? fl : 1))) : gmax;
         const int nchans_pad = ngroups * group_cols;
         std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchans_pad);
         std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchans_pad * DB * v.rel_bytes);

@@ -87,7 +87,8 @@ struct dd_plan_s {
     int cc = 0;            // channels per pipeline stage
     int nchans_pad = 0;    // channels the kernel iterates over (nlive, or padded to a multiple of cc)
     int nstages = 2;       // ring depth of the staged buffers (<= var.raw_stages)
-    bool patch = false;    // bit planes: epilogue through per-warp shared-memory patches (chosen by build_tiles)
+    bool long_mode = false; // bit planes: many channels per group -> the LONG kernel instantiation (flush every FL stages)
+    bool patch = false;    // bit planes: epilogue through per-warp shared-memory patches (!long_mode || nbits < 8)
     int64_t max_span_end = 0;   // max over spans of start + staged samples: how far past a tile's t0 a copy reaches
     int raw_slot = 0;      // bytes per channel slot of the packed stage buffer (multiple of 16)
     int sub_slot = 0;      // bit planes: bytes per sub-row inside a channel slot (raw_slot / nsub)
