@@ -1,5 +1,7 @@
 // dd_api.cu -- the C ABI of include/dd.h: argument checking, table upload, kernel launch.
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -116,7 +118,8 @@ static int elem_size(int out_nbits)
         return 4;
     case DD_OUT_U16:
         return 2;
-    case kOutU8:   // internal (sub-band intermediate); check_execute rejects it at the C ABI
+    case kOutU8:       // internal; check_execute rejects both at the C ABI
+    case kOutPlanes:   // (sub-band intermediate: bit planes, one byte per sample)
         return 1;
     }
     return 0;
@@ -128,7 +131,7 @@ static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_st
     if (p->ndm <= 0)
         return DD_ERR_NO_DM_LIST;
     const int es = elem_size(out_nbits);
-    if (nsamps <= 0 || es == 0 || out_nbits == kOutU8)
+    if (nsamps <= 0 || es == 0 || out_nbits == kOutU8 || out_nbits == kOutPlanes)
         return DD_ERR_INVALID_ARG;
     if (in_stride <= 0 || in_stride % 16 != 0)
         return DD_ERR_ALIGNMENT;
@@ -188,9 +191,11 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
 // Rebuilds delay table and tile metadata for (DM list, kill mask) into a scratch plan, then commits: a failure
 // leaves the plan unchanged.  Uploads the tables when a device exists.
 // The sub-band method on device-resident data ("two consecutive calls to the direct dedispersion
-// routine and the addition of a temporary data buffer"): step 1 writes uint8 series S[beam][sub-band][nominal DM][t]
-// for t < nsamps + largest step-2 delay (rounded up to 32 so that the rows can be staged by bulk copies), step 2
-// dedisperses, for every group of trials, the miniature filterbank of its nominal DM.
+// routine and the addition of a temporary data buffer").  The temporary buffer is step 2's bit-plane work buffer:
+// step 1 sums every sub-band for every nominal DM and stores the low 8 planes of its carry-save counters -- which
+// ARE the 8-bit series S[beam][sub-band][nominal DM][t], t < nsamps + largest step-2 delay, in the layout step 2
+// stages -- so that neither an output transpose, nor a byte buffer, nor a second pre-pass is needed; step 2
+// dedisperses, for every group of trials, the miniature filterbank of its nominal DM.  Three kernels.
 static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
                                  int out_nbits, cudaStream_t st_)
 {
@@ -205,38 +210,39 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
             return st;
     const int nbeams = plan->nbeams, nsb = s2->nchans, ngrp = s1->ndm;
     const int64_t t1 = (nsamps + plan->sb_max_d2 + 31) / 32 * 32;
-    const size_t need = static_cast<size_t>(nbeams) * nsb * ngrp * static_cast<size_t>(t1);
     cudaError_t e;
-    if (plan->tmp_bytes < need) {
-        if (plan->d_tmp)
-            cudaFree(plan->d_tmp);
-        plan->d_tmp = nullptr;
-        plan->tmp_bytes = 0;
-        if ((e = cudaMalloc(&plan->d_tmp, need)) != cudaSuccess)
-            return cuda_fail(e, "cudaMalloc(sub-band intermediate)");
-        plan->tmp_bytes = need;
-    }
+    // step 2's launch geometry first: N_SB channels; DM block blk reads the rows of nominal DM blk / (dm_group / 16)
+    const int64_t out_beam = nbeams > 1 ? plan->out_beam_stride : 0;
+    KernelParams k2 = make_params(s2, nsamps, nullptr, 16, out_ptr, out_nbits, nbeams, 0, out_beam);
+    k2.nrows = nsb * ngrp;
+    k2.row_mul = ngrp;
+    k2.in_blk_div = plan->dm_group / s2->var.DB;
+    BpWork w2;
+    if ((e = bp_prepare_work(s2, k2, st_, true, &w2)) != cudaSuccess)
+        return cuda_fail(e, "dd_execute sub-band work buffer");
     const bool prof = plan->prof_cap > 0 && plan->prof_n < plan->prof_cap;
     cudaEvent_t *ev = prof ? reinterpret_cast<cudaEvent_t *>(plan->prof_events.data()) + 3 * plan->prof_n : nullptr;
     if (prof)
         cudaEventRecord(ev[0], st_);
-    // step 1: batch index = (beam, sub-band); "DM trials" = the nominal DMs
+    // step 1: "DM trials" = the nominal DMs; a CTA sums gpc sub-bands one after the other (enough CTAs left to
+    // fill the SMs a few times over), so that the copies of the next sub-band fly while this one is added
     const int64_t in_beam = nbeams > 1 ? plan->in_beam_stride : 0;
-    KernelParams k1 = make_params(s1, t1, in_ptr, in_stride, plan->d_tmp, kOutU8, nbeams, in_beam,
-                                  static_cast<int64_t>(ngrp) * t1);
-    k1.vec_ok = 1;
+    KernelParams k1 = make_params(s1, t1, in_ptr, in_stride, s2->d_work, kOutPlanes, nbeams, in_beam, 0);
+    k1.pl_conv = w2.conv;
+    k1.pl_beam = w2.w_beam;
+    k1.pl_units = static_cast<int32_t>(w2.units);
+    int sms = 148;
+    (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device >= 0 ? plan->device : 0);
+    const int64_t ctas1 = static_cast<int64_t>(k1.nblk) * k1.ntiles * nbeams * k1.ngroups;
+    int64_t gpc = ctas1 / (4 * static_cast<int64_t>(sms));
+    if (const char *envv = std::getenv("DD_SB_GPC"))   // test hook: groups per CTA
+        gpc = std::atoi(envv);
+    k1.gpc = static_cast<int32_t>(std::max<int64_t>(1, std::min<int64_t>(gpc, k1.ngroups)));
     s1->prof_mid = nullptr;
     if ((e = launch_direct(s1, k1, st_)) != cudaSuccess)
         return cuda_fail(e, "dd_execute sub-band step 1");
-    // step 2: N_SB channels; DM block blk reads the rows of nominal DM blk / (dm_group / 16)
-    const int64_t out_beam = nbeams > 1 ? plan->out_beam_stride : 0;
-    KernelParams k2 = make_params(s2, nsamps, plan->d_tmp, t1, out_ptr, out_nbits, nbeams,
-                                  static_cast<int64_t>(nsb) * ngrp * t1, out_beam);
-    k2.nrows = nsb * ngrp;
-    k2.row_mul = ngrp;
-    k2.in_blk_div = plan->dm_group / s2->var.DB;
     s2->prof_mid = prof ? ev[1] : nullptr;
-    e = launch_direct(s2, k2, st_);
+    e = launch_variant3(s2, k2, st_, true);
     s2->prof_mid = nullptr;
     if (e != cudaSuccess)
         return cuda_fail(e, "dd_execute sub-band step 2");
@@ -244,7 +250,7 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
         cudaEventRecord(ev[2], st_);
         ++plan->prof_n;
     }
-    plan->last_launches = launches_per_execute(s1) + launches_per_execute(s2);
+    plan->last_launches = launches_per_execute(s1) + 1;
     return DD_OK;
 }
 

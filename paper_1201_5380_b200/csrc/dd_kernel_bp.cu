@@ -426,8 +426,21 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int blk = static_cast<int>(cta % p.nblk);
     const int64_t rest = cta / p.nblk;
     const int tile = static_cast<int>(rest % p.ntiles);
-    const int batch = static_cast<int>(rest / p.ntiles);          // (beam, channel group)
-    const int beam = batch / p.ngroups, group = batch - beam * p.ngroups;
+    const int batch = static_cast<int>(rest / p.ntiles);          // (beam, set of gpc channel groups); gpc = 1: (beam, group)
+    int beam, group, nch_set = 0;   // group: the first one of the set; nch_set: stages this CTA works through
+    if constexpr (LONG) {           // always one group per CTA
+        beam = batch / p.ngroups, group = batch - beam * p.ngroups;
+    } else {
+        const int nsets = (p.ngroups + p.gpc - 1) / p.gpc;
+        beam = batch / nsets, group = (batch - beam * nsets) * p.gpc;
+        nch_set = min(p.gpc, p.ngroups - group) * p.nchunks;
+    }
+    auto nchunks_cta = [&]() -> int {   // LONG: straight from the parameter bank, no register held across the loop
+        if constexpr (LONG)
+            return p.nchunks;
+        else
+            return nch_set;
+    };
     const int64_t t0 = static_cast<int64_t>(tile) * TB;
 
     // shared memory carve-up (must match dd::smem_layout_bytes)
@@ -463,7 +476,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     auto load_meta = [&](int chunk, int4 (&m)[CPW]) {
 #pragma unroll
         for (int k = 0; k < CPW; ++k)
-            m[k] = (lane == 0 && chunk < p.nchunks) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
+            m[k] = (lane == 0 && chunk < nchunks_cta()) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
     };
     // chunk = round * NS + s: the ring position is carried along instead of divided out (NS is a run-time value)
     int prod_s = 0, prod_round = 0;
@@ -500,7 +513,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in chunks (measured: 1 and 2 equal, 3 slower)
     int4 meta[CPW], nxt[CPW];
     load_meta(0, meta);
-    for (int k = 0; k < dist && k < p.nchunks; ++k) {
+    for (int k = 0; k < dist && k < nchunks_cta(); ++k) {
         load_meta(k + 1, nxt);
         produce(k, meta);
 #pragma unroll
@@ -526,7 +539,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     auto stage = [&](int chunk, auto phase, auto flush) {
         constexpr int PHASE = decltype(phase)::value;
         constexpr uint32_t FLUSH = decltype(flush)::value;
-        if (chunk + dist < p.nchunks) {
+        if (chunk + dist < nchunks_cta()) {
             load_meta(chunk + dist + 1, nxt);
             produce(chunk + dist, meta);
 #pragma unroll
@@ -556,9 +569,41 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     // groups of FL stages with one flush at the end (nchunks is a multiple of FL by plan construction)
     using NoFlush = std::integral_constant<uint32_t, 0u>;
     using FlushAll = std::integral_constant<uint32_t, FL * STAGE_SUM>;
-    for (int chunk = 0; chunk < p.nchunks; chunk += FL) {
+    // Bit-plane output (kOutPlanes, the intermediate series of the sub-band method): the counter's low 8 planes ARE
+    // the 8-bit samples of the next step in the layout its stages want, so they are stored as they stand -- no
+    // transposes, no pre-pass afterwards -- and the CTA carries on with its next channel group while the ring keeps
+    // the copies of that group in flight.
+    [[maybe_unused]] auto store_planes = [&](int g) {
+        const int dpl = blk * DB + warp;
+        if (dpl < p.ndm) {
+            uint8_t *row = p.out + static_cast<int64_t>(beam) * p.pl_beam +
+                           (static_cast<int64_t>(g) * p.ndm + dpl) * (2 * p.pl_conv);
+            const int64_t u0 = (t0 >> 5) + W * lane;
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                if (u0 + j < p.pl_units) {
+                    uint8_t *dst = row + (u0 + j) * 16;
+                    *reinterpret_cast<uint4 *>(dst) = make_uint4(P[j][0], P[j][1], P[j][2], P[j][3]);
+                    *reinterpret_cast<uint4 *>(dst + p.pl_conv) = make_uint4(P[j][4], P[j][5], P[j][6], P[j][7]);
+                }
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+#pragma unroll
+            for (int k = 0; k < NP; ++k)
+                P[j][k] = 0;
+        }
+    };
+    int cig = 0, gi = 0;   // stages done of the current group, groups done
+    for (int chunk = 0; chunk < nchunks_cta(); chunk += FL) {
         if constexpr (FL == 1) {
             stage(chunk, std::integral_constant<int, 0>{}, FlushAll{});
+            if (p.out_code == kOutPlanes && ++cig == p.nchunks) {
+                cig = 0;
+                store_planes(group + gi);
+                ++gi;
+            }
         } else if constexpr (FL == 2) {
             stage(chunk, std::integral_constant<int, 0>{}, NoFlush{});
             stage(chunk + 1, std::integral_constant<int, 1>{}, FlushAll{});
@@ -575,6 +620,10 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     // Interior tiles (the whole time block inside the row, vector stores allowed) go through a per-warp patch of
     // shared memory so that every store instruction writes whole 128-byte lines.  The patches lie outside the
     // stage ring: a warp that is done stores while the others are still adding.
+    if constexpr (!LONG) {
+        if (p.out_code == kOutPlanes)
+            return;
+    }
     const int d = blk * DB + warp;
     if (d >= p.ndm)
         return;
@@ -624,22 +673,19 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
 }
 
 template <int NBITS>
-cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
+cudaError_t prepare_bp(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w)
 {
     using C = Bp<NBITS>;
     constexpr int TB = 32 * 32 * C::W;
-    if (plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB)
-        return cudaErrorInvalidValue;
-    KernelParams kp = kp_in;
     // 16-byte groups of every sub-row the tiles can touch (2 units of 2-bit input, 1 unit otherwise).  The bit-plane
     // rows are as long as the longest span needs, zero beyond the input, so that the kernel's copies need no
     // clamping; behind the nrows input rows of a beam lie row_mul all-zero rows, the source of padded channels.
     const int64_t spg = (16 / (C::NB * 4)) * 32;   // samples per group
-    const int64_t groups = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
-    const int64_t conv = groups * 16;   // bytes per sub-row
-    const int64_t rows = static_cast<int64_t>(kp.nrows) + kp.row_mul;
-    const int64_t w_beam = rows * C::NSUB * conv;
-    const size_t need = static_cast<size_t>(kp.nbeams) * static_cast<size_t>(w_beam);
+    w->units = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
+    w->conv = w->units * 16;   // bytes per sub-row
+    w->rows = static_cast<int64_t>(kp.nrows) + kp.row_mul;
+    w->w_beam = w->rows * C::NSUB * w->conv;
+    const size_t need = static_cast<size_t>(kp.nbeams) * static_cast<size_t>(w->w_beam);
     cudaError_t e;
     if (plan->work_bytes < need) {
         if (plan->d_work)
@@ -651,29 +697,57 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
             return e;
         plan->work_bytes = need;
     }
-    if (plan->work_layout[0] != conv || plan->work_layout[1] != rows || plan->work_layout[2] != kp.nbeams) {
-        e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_work) + static_cast<int64_t>(kp.nrows) * C::NSUB * conv,
-                              static_cast<size_t>(w_beam), 0, static_cast<size_t>(kp.row_mul) * C::NSUB * conv, kp.nbeams, stream);
+    if (plan->work_layout[0] != w->conv || plan->work_layout[1] != w->rows || plan->work_layout[2] != kp.nbeams ||
+        plan->work_layout[3] != (zero_all ? 1 : 0)) {
+        if (zero_all)
+            e = cudaMemsetAsync(plan->d_work, 0, need, stream);
+        else
+            e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_work) + static_cast<int64_t>(kp.nrows) * C::NSUB * w->conv,
+                                  static_cast<size_t>(w->w_beam), 0, static_cast<size_t>(kp.row_mul) * C::NSUB * w->conv,
+                                  kp.nbeams, stream);
         if (e != cudaSuccess)
             return e;
-        plan->work_layout[0] = conv;
-        plan->work_layout[1] = rows;
+        plan->work_layout[0] = w->conv;
+        plan->work_layout[1] = w->rows;
         plan->work_layout[2] = kp.nbeams;
+        plan->work_layout[3] = zero_all ? 1 : 0;
     }
-    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
-        kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv, w_beam,
-        static_cast<int32_t>(groups));
-    if ((e = cudaGetLastError()) != cudaSuccess)
+    return cudaSuccess;
+}
+
+template <int NBITS>
+cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream, bool planes_ready)
+{
+    using C = Bp<NBITS>;
+    constexpr int TB = 32 * 32 * C::W;
+    if (plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB)
+        return cudaErrorInvalidValue;
+    KernelParams kp = kp_in;
+    BpWork w;
+    cudaError_t e = prepare_bp<NBITS>(plan, kp, stream, planes_ready, &w);
+    if (e != cudaSuccess)
         return e;
+    if (!planes_ready) {
+        dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((w.units + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
+            kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), w.conv, w.w_beam,
+            static_cast<int32_t>(w.units));
+        if ((e = cudaGetLastError()) != cudaSuccess)
+            return e;
+    }
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     kp.in = static_cast<const uint8_t *>(plan->d_work);
-    kp.in_stride = C::NSUB * conv * kp.row_mul;   // between channel indices; sub-rows are in_row_bytes apart
-    kp.in_blk_stride = C::NSUB * conv;            // between the rows of one channel index (sub-band step 2)
-    kp.in_row_bytes = conv;
-    kp.in_beam_stride = w_beam;
+    kp.in_stride = C::NSUB * w.conv * kp.row_mul;   // between channel indices; sub-rows are in_row_bytes apart
+    kp.in_blk_stride = C::NSUB * w.conv;            // between the rows of one channel index (sub-band step 2)
+    kp.in_row_bytes = w.conv;
+    kp.in_beam_stride = w.w_beam;
+    if (kp.out_code == kOutPlanes && plan->long_mode)
+        return cudaErrorInvalidValue;   // bit-plane output is compiled into the short instantiation only
+    if (kp.gpc < 1 || kp.out_code != kOutPlanes)
+        kp.gpc = 1;
 
-    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * kp.ngroups;
+    const int64_t nsets = (kp.ngroups + kp.gpc - 1) / kp.gpc;
+    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * nsets;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
     if (plan->long_mode && kp.nchunks % C::FL != 0)
@@ -689,17 +763,32 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
 }  // namespace
 
 // Two launches: the bit-plane transpose of the rows the tiles will read, then the dedispersion kernel.
-cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
+cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool planes_ready)
 {
     if (!plan->var.bitplane)
         return cudaErrorInvalidValue;
     switch (plan->nbits) {
     case 2:
-        return launch_bp<2>(plan, kp, stream);
+        return launch_bp<2>(plan, kp, stream, planes_ready);
     case 4:
-        return launch_bp<4>(plan, kp, stream);
+        return launch_bp<4>(plan, kp, stream, planes_ready);
     case 8:
-        return launch_bp<8>(plan, kp, stream);
+        return launch_bp<8>(plan, kp, stream, planes_ready);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w)
+{
+    if (!plan->var.bitplane)
+        return cudaErrorInvalidValue;
+    switch (plan->nbits) {
+    case 2:
+        return prepare_bp<2>(plan, kp, stream, zero_all, w);
+    case 4:
+        return prepare_bp<4>(plan, kp, stream, zero_all, w);
+    case 8:
+        return prepare_bp<8>(plan, kp, stream, zero_all, w);
     }
     return cudaErrorInvalidValue;
 }

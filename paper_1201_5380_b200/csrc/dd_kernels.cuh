@@ -34,6 +34,20 @@ struct KernelParams {
     const uint8_t *zero;      // raw_slot zero bytes: the span of a padded channel
     const int4 *span;         // [nblk][nchans_pad] {start, nbytes, input row, 0}
     const void *rel;          // [nblk][nchans][DB] entries of var.rel_bytes
+    // out_code == kOutPlanes (bit-plane kernel only): `out` is the bit-plane work buffer of an 8-bit plan, rows
+    // [beam][group * ndm + d][sub-row 0..1][unit][4 planes]
+    int64_t pl_conv;          // bytes per sub-row
+    int64_t pl_beam;          // bytes between beams
+    int32_t pl_units;         // units (32 samples) per sub-row
+    int32_t gpc;              // channel groups summed one after the other by a CTA (>= 1; > 1 only with kOutPlanes)
+};
+
+// Geometry of the bit-plane work buffer of a plan for one launch (dd_kernel_bp.cu).
+struct BpWork {
+    int64_t units;    // 16-byte groups per sub-row
+    int64_t conv;     // bytes per sub-row
+    int64_t rows;     // rows per beam, the all-zero rows of the padded channels included
+    int64_t w_beam;   // bytes per beam
 };
 
 // Enqueues the kernel variant chosen by the plan.  Returns the cudaError_t of the launch.
@@ -41,8 +55,13 @@ cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t 
 
 cudaError_t launch_variant1(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 cudaError_t launch_variant2(const dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
-// variant 3 launches two kernels (bit-plane transpose into plan->d_work, then the transform); it may grow d_work
-cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+// variant 3 launches two kernels (bit-plane transpose into plan->d_work, then the transform); it may grow d_work.
+// planes_ready: plan->d_work already holds the bit planes (written by another launch with kOutPlanes after
+// bp_prepare_work): the transpose is skipped.
+cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool planes_ready = false);
+// Sizes (and grows) plan->d_work for the launch described by kp and keeps its all-zero rows; zero_all: the whole
+// buffer is cleared whenever it is new or its layout changed (for a producer that does not write every unit).
+cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w);
 
 // Time-scrunching of packed rows (dd_scrunch.cu).  out_bytes = bytes of every output row to produce (multiple of 16).
 cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t *in, int64_t in_stride, uint8_t *out,

@@ -105,7 +105,7 @@ struct dd_plan_s {
     void *d_zero = nullptr;           // raw_slot zero bytes (source of the padded channels)
     void *d_work = nullptr;           // bit-plane copy of the input (variants with `bitplane`), grown on demand
     size_t work_bytes = 0;
-    int64_t work_layout[3] = {0, 0, 0};   // {bytes per sub-row, rows, beams} the zero rows of d_work were written for
+    int64_t work_layout[4] = {0, 0, 0, 0};   // {bytes per sub-row, rows, beams, cleared as a whole} d_work's zeros were written for
     int64_t last_launches = 0;
     dd::HostStage *stage = nullptr;
     // optional per-kernel timing of dd_execute (dd_profile_enable): 3 events per recorded call
@@ -133,6 +133,8 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
 
 constexpr int64_t kMaxDynSmem = 227 * 1024;   // usable shared memory per CTA on sm_100a
 constexpr int kBpPatchBytes = 4096;             // bit-plane kernel epilogue: shared memory per warp (32 lanes x 128 B)
-constexpr int kOutU8 = 8;                     // internal output code: uint8 sums (sub-band intermediate), not in the C ABI
+constexpr int kOutU8 = 8;                     // internal output code: uint8 sums, not in the C ABI
+constexpr int kOutPlanes = 9;                 // internal output code: the low 8 bit planes of the sums, written in the layout the
+                                              // 8-bit bit-plane kernel stages (sub-band intermediate: step 2 needs no pre-pass)
 
 }  // namespace dd

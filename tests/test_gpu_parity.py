@@ -239,8 +239,13 @@ def test_killmask_4_and_8_bit_batch_and_host_path(nbits):
     (4, 64, 40, 3072 + 50, 16, 16, 1, True),        # 4-bit: 16 * 15 = 240 <= 255
     (5, 48, 35, 900, 1, 32, 1, False),              # 8-bit input: only 1-channel sub-bands fit 8-bit intermediates
 ])
-def test_subband_method_matches_the_two_step_oracle(case):
+@pytest.mark.parametrize("gpc", [0, 3])   # sub-bands summed per CTA in step 1: the library's choice / forced to 3
+def test_subband_method_matches_the_two_step_oracle(case, gpc, monkeypatch):
     idx, nchans, ndm, nsamps, sb, grp, nbeams, masked = case
+    if gpc:
+        monkeypatch.setenv("DD_SB_GPC", str(gpc))
+    else:
+        monkeypatch.delenv("DD_SB_GPC", raising=False)
     cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=nbeams)
     dms = cfg.dm_list()
     nominal, d1, d2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb, grp)
@@ -260,7 +265,7 @@ def test_subband_method_matches_the_two_step_oracle(case):
             p.set_batch(nbeams, dev.stride(0), out.stride(0) * 4)
         p.execute(nsamps, dev, stride, out, -32, torch.cuda.current_stream())
         torch.cuda.synchronize()
-        assert p.launch_info()["last_launches"] == 4
+        assert p.launch_info()["last_launches"] == 3    # pre-pass, step 1 (writes bit planes), step 2
         got = out.cpu().numpy().view(np.uint32)
         for b in range(nbeams):
             ref = oracle.subband_dedisperse(packed[b].numpy(), cfg.nbits, nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df,
@@ -328,7 +333,7 @@ def test_execute_host_bitplane_variant_two_slabs():
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
-        assert p.launch_info()["last_launches"] == 4
+        assert p.launch_info()["last_launches"] == 3    # pre-pass, step 1 (writes bit planes), step 2
     assert np.array_equal(out.numpy(), ref)
 
 
@@ -342,7 +347,7 @@ def test_execute_host_bitplane_8bit_two_slabs():
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
-        assert p.launch_info()["last_launches"] == 4
+        assert p.launch_info()["last_launches"] == 3    # pre-pass, step 1 (writes bit planes), step 2
     assert np.array_equal(out.numpy(), ref)
 
 
