@@ -224,47 +224,48 @@ struct BpShared {
 };
 
 // plane k of sub-row SUB of a channel, for every unit of the lane; CLS = channels added since the last flush
-template <int NBITS, int CLS, int SUB, int K, int NP, int NT>
+// PIN: planes of a sample that can be non-zero (NBITS, or fewer for the sub-band intermediate: the rest is skipped)
+template <int NBITS, int PIN, int CLS, int SUB, int K, int NP, int NT>
 __device__ __forceinline__ void plane_step(const PlaneVec<Bp<NBITS>::NB> (&x)[Bp<NBITS>::W + 1], uint32_t shift,
                                            uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
     using C = Bp<NBITS>;
-    if constexpr (K < C::NB) {
+    if constexpr (K < C::NB && SUB * C::NB + K < PIN) {
         constexpr int L = SUB * C::NB + K;                                   // weight 2^L
-        constexpr uint32_t VMAX = (1u << NBITS) - 1u;
+        constexpr uint32_t VMAX = (1u << PIN) - 1u;
         constexpr uint32_t S = VMAX * CLS + ((1u << L) - 1u);                // weight added to the counter so far
 #pragma unroll
         for (int j = 0; j < C::W; ++j)
             csa_add<S, L>(P[j], T[j], __funnelshift_r(x[j].w[K], x[j + 1].w[K], shift));
-        plane_step<NBITS, CLS, SUB, K + 1>(x, shift, P, T);
+        plane_step<NBITS, PIN, CLS, SUB, K + 1>(x, shift, P, T);
     }
 }
 
 // channel CL of the stage: per sub-row one window of W+1 units serves W units; per unit and plane one funnel
 // shift + carry-save adds
-template <int NBITS, int CLS, int SUB, int NP, int NT>
+template <int NBITS, int PIN, int CLS, int SUB, int NP, int NT>
 __device__ __forceinline__ void subrow_step(const BpShared &sh, const uint2 e, uint32_t (&P)[Bp<NBITS>::W][NP],
                                             uint32_t (&T)[Bp<NBITS>::W][NT])
 {
     using C = Bp<NBITS>;
-    if constexpr (SUB < C::NSUB) {
+    if constexpr (SUB < C::NSUB && SUB * C::NB < PIN) {
         const uint8_t *wp = sh.lane_base + e.x + SUB * sh.sub_slot;
         PlaneVec<C::NB> x[C::W + 1];
 #pragma unroll
         for (int j = 0; j <= C::W; ++j)
             x[j].load(wp + j * (C::NB * 4));
-        plane_step<NBITS, CLS, SUB, 0>(x, e.y, P, T);
-        subrow_step<NBITS, CLS, SUB + 1>(sh, e, P, T);
+        plane_step<NBITS, PIN, CLS, SUB, 0>(x, e.y, P, T);
+        subrow_step<NBITS, PIN, CLS, SUB + 1>(sh, e, P, T);
     }
 }
 
 // PHASE: stages added since the last flush (the pending words are rippled into the planes every FL stages)
-template <int NBITS, int PHASE, int NP, int NT, int... CLs>
+template <int NBITS, int PIN, int PHASE, int NP, int NT, int... CLs>
 __device__ __forceinline__ void stage_steps(std::integer_sequence<int, CLs...>, const BpShared &sh,
                                             uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
     // rel entry: {byte offset in the stage, bit shift}
-    (subrow_step<NBITS, PHASE * Bp<NBITS>::CC + CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);
+    (subrow_step<NBITS, PIN, PHASE * Bp<NBITS>::CC + CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -406,15 +407,22 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
 // Bp<NBITS>::FL stages (the plan pads the channel list to whole groups of FL stages), and for 8-bit input the
 // epilogue stores straight from registers (a deeper stage ring is worth more than coalesced stores there).
 // Otherwise: a flush after every stage, and the epilogue goes through per-warp shared-memory patches.
-template <int NBITS, bool LONG>
+// PIN < NBITS (short instantiation, 8-bit input): only the low PIN planes of a sample can be set (the plan knows the
+// largest sample of the sub-band intermediate), the others are neither shifted nor added.
+template <int NBITS, bool LONG, int PIN = NBITS>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
     using C = Bp<NBITS>;
-    constexpr int DB = BP_DB, W = C::W, TB = 32 * 32 * W, CC = C::CC, NP = C::NP, NSUB = C::NSUB;
+    constexpr int DB = BP_DB, W = C::W, TB = 32 * 32 * W, CC = C::CC, NSUB = C::NSUB;
+    // the short instantiation serves fewer than 8 * CC * FL channels per group: 8-bit sums then fit 16 planes and the
+    // epilogue transposes 16 x 16 bit matrices instead of 32 x 32
+    constexpr int NP = (NBITS == 8 && !LONG) ? 16 : C::NP;
+    static_assert(LONG || static_cast<int64_t>(8 * CC * C::FL) * ((1 << NBITS) - 1) <= (int64_t(1) << NP), "short-mode sums must fit NP planes");
+    static_assert(PIN >= 1 && PIN <= NBITS && (PIN == NBITS || !LONG), "fewer planes: short instantiation only");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
     constexpr int FL = LONG ? C::FL : 1;
     constexpr bool PATCH = !LONG || NBITS < 8;
-    constexpr uint32_t STAGE_SUM = ((1u << NBITS) - 1u) * CC;        // largest value one stage adds to a counter
+    constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;        // largest value one stage adds to a counter
     constexpr int NT = bit_length(FL * STAGE_SUM);                   // pending slots
     static_assert((CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
 
@@ -552,7 +560,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         sh.lane_base = raw_base + s * raw_stage + lane * (W * UB);
         sh.rel = reinterpret_cast<const uint2 *>(rel_base + s * rel_stage) + warp;
         sh.sub_slot = p.sub_slot;
-        stage_steps<NBITS, PHASE>(std::make_integer_sequence<int, CC>{}, sh, P, T);
+        stage_steps<NBITS, PIN, PHASE>(std::make_integer_sequence<int, CC>{}, sh, P, T);
         if constexpr (FLUSH != 0u) {
 #pragma unroll
             for (int j = 0; j < W; ++j)
@@ -753,6 +761,12 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     if (plan->long_mode && kp.nchunks % C::FL != 0)
         return cudaErrorInvalidValue;
     auto kernel = plan->long_mode ? dd_direct_bp<NBITS, true> : dd_direct_bp<NBITS, false>;
+    if constexpr (NBITS == 8) {   // sub-band step 2: samples known to stay below 2^in_planes
+        if (!plan->long_mode && plan->in_planes > 0 && plan->in_planes <= 6)
+            kernel = dd_direct_bp<8, false, 6>;
+        else if (!plan->long_mode && plan->in_planes == 7)
+            kernel = dd_direct_bp<8, false, 7>;
+    }
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)
         return e;

@@ -99,6 +99,19 @@ dd_status build_subband(const dd_plan_s *p, dd_plan_s *s1, dd_plan_s *s2, std::v
     s2->ndm = ndm;
     s2->dm = p->dm;
     s2->force_variant = 3;
+    {   // the largest sample of the miniature filterbanks: live channels of the fullest sub-band times the largest input
+        int most = 0;
+        for (int b = 0; b < nsb; ++b) {
+            int n = 0;
+            for (int c = b * sb; c < (b + 1) * sb; ++c)
+                n += (p->keep.empty() || p->keep[c]) ? 1 : 0;
+            most = std::max(most, n);
+        }
+        int64_t vtop = static_cast<int64_t>(most) * ((1 << p->nbits) - 1);
+        s2->in_planes = 1;
+        while ((int64_t(1) << s2->in_planes) <= vtop)
+            ++s2->in_planes;
+    }
     s2->delay.resize(static_cast<size_t>(ndm) * nsb);
     int64_t m2 = 0, ext = 0;
     for (int b = 0; b < nsb; ++b) {

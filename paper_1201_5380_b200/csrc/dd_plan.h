@@ -94,6 +94,7 @@ struct dd_plan_s {
     int sub_slot = 0;      // bit planes: bytes per sub-row inside a channel slot (raw_slot / nsub)
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
+    int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
     std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels (nchans_pad = ngroups * group_cols)
     std::vector<uint8_t> rel;         // [nblk][nchans_pad][DB] entries of var.rel_bytes: delay - span start per DM slot

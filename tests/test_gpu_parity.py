@@ -333,7 +333,7 @@ def test_execute_host_bitplane_variant_two_slabs():
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
-        assert p.launch_info()["last_launches"] == 3    # pre-pass, step 1 (writes bit planes), step 2
+        assert p.launch_info()["last_launches"] == 4
     assert np.array_equal(out.numpy(), ref)
 
 
@@ -347,7 +347,7 @@ def test_execute_host_bitplane_8bit_two_slabs():
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
-        assert p.launch_info()["last_launches"] == 3    # pre-pass, step 1 (writes bit planes), step 2
+        assert p.launch_info()["last_launches"] == 4
     assert np.array_equal(out.numpy(), ref)
 
 
