@@ -253,7 +253,7 @@ def run_ours(args) -> None:
     ms_step_rank = total_ms / args.steps
     value, ms_step = multi.job_throughput(counts["units"], ms_step_rank)
     kernel_ms = float(np.mean(main_ms))
-    if subband:     # four kernels share the work: report the whole step, and step 2's transform kernel beside it
+    if subband:     # three kernels share the work: report the whole step, and step 2's transform kernel beside it
         subband["step2_kernel_ms"] = kernel_ms
         kernel_ms = float(np.mean(np.asarray(main_ms) + np.asarray(prepass_ms)))
 

@@ -116,7 +116,8 @@ dd_status dd_set_killmask(dd_plan plan, const int32_t *mask);
  *   (0, 0) returns to the direct transform.
  * Takes effect at once when a DM list is present (else at dd_set_dm_list); on error the plan is unchanged.  Honours
  * the kill mask and dd_set_batch.  dd_execute then needs input rows of nsamps + dd_get_subband_extent() samples,
- * allocates its temporary buffers on first use, and launches four kernels.  dd_execute_host returns
+ * allocates its temporary buffers on first use, and launches three kernels (bit-plane transpose of the input,
+ * step 1 writing S as bit planes, step 2).  dd_execute_host returns
  * DD_ERR_INVALID_ARG while the sub-band method is selected.
  */
 dd_status dd_set_subband(dd_plan plan, int sb_nchans, int dm_group);
