@@ -77,3 +77,49 @@ def job_throughput(units_this_rank: float, ms_this_rank: float) -> Tuple[float, 
     total = sum_over_ranks(units_this_rank)
     ms = max_over_ranks(ms_this_rank)
     return (total / (ms * 1e-3) if ms > 0 else 0.0), ms
+
+
+# ---- the other two exchange-free splits ----------------------------
+
+def shard_dm_slabs(ndm: int, world_size: int, rank: int, align: int = 16) -> Tuple[int, int]:
+    """DM slab [lo, hi) of rank `rank`: contiguous (a rank's delay spread stays compact), balanced in units of
+    `align` trials (the kernel's DM block), the last slab taking the ragged rest.  The input is replicated, the
+    outputs are disjoint rows: no exchange.  Ranks beyond the number of blocks get an empty slab."""
+    if ndm < 0 or world_size <= 0 or align <= 0 or not (0 <= rank < world_size):
+        raise ValueError("bad shard request")
+    nblk = -(-ndm // align)
+    base, extra = divmod(nblk, world_size)
+    lo = rank * base + min(rank, extra)
+    hi = lo + base + (1 if rank < extra else 0)
+    return min(lo * align, ndm), min(hi * align, ndm)
+
+
+def shard_time_slabs(nsamps: int, world_size: int, rank: int, max_delay: int, align: int = 128) -> Tuple[int, int, int, int]:
+    """Time slab of rank `rank` ("time-division multiplexing"): output samples [t_lo, t_hi) and the
+    input samples [t_lo, in_hi) it reads, in_hi = t_hi + max_delay -- a halo of max_delay samples that the next
+    rank reads too, so nothing is exchanged.  Slab starts are multiples of `align` samples (128 keeps the start of a
+    2-bit row slab 16-byte aligned for the bulk copies).  -> (t_lo, t_hi, t_lo, in_hi)."""
+    if nsamps < 0 or world_size <= 0 or align <= 0 or max_delay < 0 or not (0 <= rank < world_size):
+        raise ValueError("bad shard request")
+    nunits = -(-nsamps // align)
+    base, extra = divmod(nunits, world_size)
+    lo = rank * base + min(rank, extra)
+    hi = lo + base + (1 if rank < extra else 0)
+    t_lo, t_hi = min(lo * align, nsamps), min(hi * align, nsamps)
+    return t_lo, t_hi, t_lo, (t_hi + max_delay if t_hi > t_lo else t_lo)
+
+
+def gather_dm_rows(local_rows: torch.Tensor, ndm: int, world_size: int, align: int = 16) -> torch.Tensor:
+    """Optional assembly of the whole transform on every rank from DM slabs (only when one consumer wants all of
+    it; the transform itself needs no collective): all_gather of the slabs, padded to the largest one.
+    local_rows: [hi - lo, nsamps] of this rank's slab (shard_dm_slabs).  -> [ndm, nsamps]."""
+    if not (dist.is_available() and dist.is_initialized()):
+        return local_rows
+    bounds = [shard_dm_slabs(ndm, world_size, r, align) for r in range(world_size)]
+    most = max(hi - lo for lo, hi in bounds)
+    nsamps = local_rows.shape[1]
+    pad = torch.zeros((most, nsamps), dtype=local_rows.dtype, device=local_rows.device)
+    pad[: local_rows.shape[0]] = local_rows
+    parts = [torch.empty_like(pad) for _ in range(world_size)]
+    dist.all_gather(parts, pad)
+    return torch.cat([parts[r][: hi - lo] for r, (lo, hi) in enumerate(bounds)], dim=0)

@@ -43,8 +43,25 @@ def _worker(rank: int, world: int, port: int, nbeams: int, ret):
     ms = 10.0 * (rank + 1)                         # rank 1 is the slow one
     value, max_ms = multi.job_throughput(units, ms)
     total = multi.sum_over_ranks(units)
+    # DM slabs (input replicated, rows disjoint) and time slabs (halo of max_delay samples): each rank runs the
+    # transform of its slab only; the slabs are then assembled with the optional all_gather and compared
+    # with the single-process transform by the parent
+    one = W.CONFIGS[2].reduced(nsamps=700, ndm=40, nchans=24)
+    tab1 = oracle.delay_table(one.nchans, one.dt, one.f_top, one.df, one.dm_list())
+    maxd = int(tab1.max())
+    packed1, _ = W.gen_packed(one, maxd)
+    rows = packed1[0].numpy()
+    lo, hi = multi.shard_dm_slabs(one.ndm, world, rank)
+    slab = oracle.dedisperse(rows, one.nbits, one.nsamps, tab1[lo:hi]) if hi > lo else np.zeros((0, one.nsamps), np.int64)
+    whole = multi.gather_dm_rows(torch.from_numpy(slab.astype(np.int64)), one.ndm, world)
+    t_lo, t_hi, i_lo, i_hi = multi.shard_time_slabs(one.nsamps, world, rank, maxd)
+    unp = oracle.unpack(rows, one.nbits, one.nsamps + maxd)[:, i_lo:i_hi]          # this rank's input slab only
+    unp = np.pad(unp, ((0, 0), (0, -unp.shape[1] % 4)))                             # whole bytes of 2-bit samples
+    tslab = oracle.dedisperse(W.pack_rows(torch.from_numpy(unp.astype(np.uint8)), one.nbits).numpy(), one.nbits,
+                              t_hi - t_lo, tab1)
     ret[rank] = dict(mine=mine, sums=sums, value=value, max_ms=max_ms, total=total,
-                     mx=multi.max_over_ranks(float(rank)))
+                     mx=multi.max_over_ranks(float(rank)), dm_bounds=(lo, hi), whole=whole.numpy(),
+                     t_bounds=(t_lo, t_hi), tslab=np.asarray(tslab))
     multi.barrier()
     torch.distributed.destroy_process_group()
 
@@ -74,6 +91,37 @@ def test_world2_gloo_beam_sharding_and_timing_reduction():
         got = (r0["sums"] if b in r0["sums"] else r1["sums"])[b]
         assert got == want
     assert len({r0["sums"][b] for b in r0["sums"]} | {r1["sums"][b] for b in r1["sums"]}) == nbeams
+
+
+    # DM slabs and time slabs: assembled shards == the single-process transform
+    one = W.CONFIGS[2].reduced(nsamps=700, ndm=40, nchans=24)
+    tab1 = oracle.delay_table(one.nchans, one.dt, one.f_top, one.df, one.dm_list())
+    packed1, _ = W.gen_packed(one, int(tab1.max()))
+    ref = oracle.dedisperse(packed1[0].numpy(), one.nbits, one.nsamps, tab1)
+    assert r0["dm_bounds"] == (0, 32) and r1["dm_bounds"] == (32, 40)              # 3 DM blocks of 16: 2 + 1 (ragged)
+    assert np.array_equal(r0["whole"], ref) and np.array_equal(r1["whole"], ref)
+    assert r0["t_bounds"] == (0, 384) and r1["t_bounds"] == (384, 700)
+    assert np.array_equal(np.concatenate([r0["tslab"], r1["tslab"]], axis=1), ref)
+
+
+def test_dm_and_time_slab_properties():
+    for n in (0, 1, 15, 16, 17, 1200, 4096):
+        for world in (1, 2, 3, 8):
+            b = [multi.shard_dm_slabs(n, world, r) for r in range(world)]
+            assert b[0][0] == 0 and b[-1][1] == n and all(b[i][1] == b[i + 1][0] for i in range(world - 1))
+            assert all((lo % 16 == 0 or lo == hi == n) and lo <= hi for lo, hi in b)   # empty slabs sit at the end
+            sizes = [-(-(hi - lo) // 16) for lo, hi in b]
+            assert max(sizes) - min(sizes) <= 1
+    for n in (0, 100, 128, 1 << 19, (1 << 19) + 77):
+        for world in (1, 2, 4, 8):
+            s = [multi.shard_time_slabs(n, world, r, 20476) for r in range(world)]
+            assert s[0][0] == 0 and s[-1][1] == n and all(s[i][1] == s[i + 1][0] for i in range(world - 1))
+            assert all(t_lo % 128 == 0 or t_lo == t_hi == n for t_lo, t_hi, _, _ in s)
+            assert all(i_hi == t_hi + 20476 for t_lo, t_hi, _, i_hi in s if t_hi > t_lo)
+    with pytest.raises(ValueError):
+        multi.shard_dm_slabs(10, 2, 2)
+    with pytest.raises(ValueError):
+        multi.shard_time_slabs(10, 2, 0, -1)
 
 
 def test_shard_beams_properties():
