@@ -41,6 +41,9 @@ constexpr int BP_DB = 16, BP_NWARPS = 16;
 
 // Tile shape per input width.  FL = stages between flushes of the pending words in the LONG instantiation
 // (dd_plan.cpp pads the channel list accordingly: kBpFlushStages there must agree).
+#ifndef DD_BP_W2
+#define DD_BP_W2 5     // units per lane of the 2-bit kernel (dd_plan.cpp: the tile is 1024 * DD_BP_W2 samples)
+#endif
 #ifndef DD_BP_FL2
 #define DD_BP_FL2 2   // measured on B200: cfg2 8.95 / 8.78 / 9.09 ms for 1 / 2 / 4 stages between flushes
 #define DD_BP_FL4 4   //                  cfg4 116.7 / 114.5 / 112.6 ms
@@ -51,7 +54,7 @@ template <int NBITS>
 struct Bp;
 template <>
 struct Bp<2> {
-    static constexpr int NB = 2, NSUB = 1, NP = 12, W = 5, CC = 32, FL = DD_BP_FL2;
+    static constexpr int NB = 2, NSUB = 1, NP = 12, W = DD_BP_W2, CC = 32, FL = DD_BP_FL2;
 };
 template <>
 struct Bp<4> {

@@ -147,6 +147,9 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 }
 
 // Stages between flushes in the LONG bit-plane kernel: must agree with Bp<nbits>::FL (DD_BP_FL*) in dd_kernel_bp.cu.
+#ifndef DD_BP_W2
+#define DD_BP_W2 5
+#endif
 #ifndef DD_BP_FL2
 #define DD_BP_FL2 2
 #define DD_BP_FL4 4
@@ -158,7 +161,7 @@ static int kBpFlushStages(int nbits) { return nbits == 2 ? DD_BP_FL2 : (nbits ==
 static const Variant kVariants[] = {
     /* id  DB   TB    thr tail rel lane lst rst  cc candidates     nbits                        sum  pad    bitplane */
     // bit planes + carry-save counters (dd_kernel_bp.cu): tile shapes must match Bp<nbits> there
-    {3, 16, 5120, 512, 32, 8, 2, 0, 4, {32, 0, 0, 0}, 1 << 2, 12, true, true, 8, 1},               // 2-bit: 2 planes, W = 5
+    {3, 16, 1024 * DD_BP_W2, 512, 32, 8, 2, 0, 4, {32, 0, 0, 0}, 1 << 2, 12, true, true, 8, 1},      // 2-bit: 2 planes, W = 5
     {3, 16, 3072, 512, 32, 8, 4, 0, 4, {16, 0, 0, 0}, 1 << 4, 16, true, true, 16, 1},              // 4-bit: 4 planes, W = 3
     {3, 16, 3072, 512, 32, 8, 8, 0, 4, {8, 0, 0, 0}, 1 << 8, 20, true, true, 16, 2},               // 8-bit: 2 x 4 planes, W = 3
     {2, 32, 1280, 512, 8, 4, 4, 2, 2, {40, 20, 10, 5}, 1 << 2, 16, false, false, 0, 1},            // 2-bit, nibble lanes
