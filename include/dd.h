@@ -193,6 +193,45 @@ dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int
                           int64_t out_stride, int nbits_out, void *stream);
 
 /*
+ * dd_scrunch_* -- the direct transform WITH time-scrunching: "reduce the time
+ * resolution by a factor of two when the DM exceeds the diagonal by adding adjacent pairs of time samples ...
+ * repeated at 2x the diagonal, 4x etc."  The diagonal DM is the one whose dispersion curve has unit gradient at the
+ * end of the band, where the delay is greatest:
+ *     DM_diag = 1 / (DeltaT(nchans-1) - DeltaT(nchans-2)),   DeltaT(c) = k_DM (f_c^-2 - f_top^-2) / dt   (samples per unit DM)
+ * and, following the order of the paper's procedure (0..DM_diag and DM_diag..2 DM_diag at full
+ * resolution, scrunch, 2..4 DM_diag, scrunch, ...) and of its benchmark projection, trial d runs at
+ *     factor F_d = 1 for DM_d <= 2 DM_diag,   2^k for 2^k DM_diag < DM_d <= 2^(k+1) DM_diag  (k >= 1)
+ * (reading T1 of DESIGN.md section 11), capped at max_factor and at the largest factor whose samples still fit 8
+ * bits, F (2^nbits - 1) <= 255.  Level l = the run of trials with the l-th smallest factor F:
+ *     A_F[c][t] = sum_{i<F} A[c][F t + i]                         (pairs added log2 F times, packed at 2/4/8 bits)
+ *     D_l[d][t] = sum_c A_F[c][t + delay_F[d][c]],  0 <= t < nsamps / F,   delay_F = eq. 4-5 with dt * F
+ * An approximation of the transform by design (lower time resolution at high DM); each level is bit-exact against
+ * the oracle's scrunched transform.
+ *
+ * dd_scrunch_create: dm_list HOST, non-decreasing (DD_ERR_INVALID_ARG otherwise), ndm > 0; max_factor a power of two
+ *   >= 1 (1 = no scrunching: one level, the plain transform).  The set owns one plan per level.
+ * dd_scrunch_levels: number of levels (>= 1), or a negative status.
+ * dd_scrunch_level_info: HOST out, 6 int64: [0] factor F, [1] index of the level's first trial in dm_list,
+ *   [2] trials in the level, [3] largest delay in samples of dt*F, [4] bits per sample of A_F, [5] DM_diag * 1e6 rounded.
+ * dd_scrunch_required_bytes: bytes per input row that dd_scrunch_execute reads for `nsamps` (a multiple of 16;
+ *   in_stride must be at least this; it covers nsamps + the largest F * max delay, rounded up to the 16-byte
+ *   groups the pair-adding kernels read), or a negative status.
+ * dd_scrunch_execute: in_ptr DEVICE packed rows as for dd_execute (one beam); out_ptrs HOST array of
+ *   dd_scrunch_levels() DEVICE pointers, level l receiving dense rows out[d][t] of nsamps / F_l elements for its
+ *   trials; out_nbits as for dd_execute.  nsamps >= the largest factor.  Asynchronous on `stream`; the scrunched
+ *   rows live in device buffers owned by the set, (re)allocated when nsamps grows.
+ */
+typedef struct dd_scrunch_s *dd_scrunch;
+dd_status dd_scrunch_create(dd_scrunch *set, int nchans, double dt, double f_top, double df, int nbits,
+                            const double *dm_list, int ndm, int max_factor);
+int dd_scrunch_levels(dd_scrunch set);
+dd_status dd_scrunch_level_info(dd_scrunch set, int level, int64_t *info);
+int64_t dd_scrunch_required_bytes(dd_scrunch set, int64_t nsamps);
+dd_status dd_scrunch_execute(dd_scrunch set, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *const *out_ptrs,
+                             int out_nbits, void *stream);
+dd_status dd_scrunch_destroy(dd_scrunch set);
+
+/*
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
  *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20).

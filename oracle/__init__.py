@@ -24,7 +24,8 @@ import numpy as np
 from . import build as _build
 from .oracle_np import (delay_table_np, dedisperse_gather_np, dedisperse_points,  # noqa: F401
                         unpack_np, dedisperse_loops_py, subband_tables, subband_required_samples,
-                        subband_dedisperse_np, time_scrunch_np)
+                        subband_dedisperse_np, time_scrunch_np, diagonal_dm_np, scrunch_factors_np,
+                        scrunched_dedisperse_np)
 
 _LIB: Optional[ctypes.CDLL] = None
 
@@ -135,6 +136,14 @@ def subband_dedisperse(packed: np.ndarray, nbits: int, nsamps: int, nchans: int,
 def time_scrunch(packed: np.ndarray, nbits_in: int, nsamps_out: int) -> np.ndarray:
     """Time-scrunching of packed rows uint8 [nrows][stride]: unpacked int64 sums [nrows][nsamps_out]."""
     return time_scrunch_np(unpack(packed, nbits_in, 2 * nsamps_out), nsamps_out)
+
+
+def scrunched_dedisperse(packed: np.ndarray, nbits: int, nsamps: int, nchans: int, dt: float, f_top: float, df: float,
+                         dm_list, max_factor: int, nsamp_in: int):
+    """Direct transform with time-scrunching of packed rows holding nsamp_in samples:
+    list of (factor, first trial, int64 sums [ndm_F][nsamps // factor]).  Readings T1-T4 (DESIGN.md section 11)."""
+    return scrunched_dedisperse_np(unpack(packed, nbits, nsamp_in), nsamps, nchans, dt, f_top, df, dm_list, max_factor,
+                                   (1 << nbits) - 1)
 
 
 def cast_out(sums: np.ndarray, kind: str) -> np.ndarray:

@@ -153,3 +153,61 @@ def time_scrunch_np(a: np.ndarray, nsamps_out: int) -> np.ndarray:
     for t in range(nsamps_out):
         out[:, t] = a[:, 2 * t] + a[:, 2 * t + 1]
     return out
+
+
+# ------------------------------------------------------------------------------------------ scrunched transform
+K_DM_SCRUNCH = 4.148808e3
+
+
+def diagonal_dm_np(nchans: int, dt: float, f_top: float, df: float) -> float:
+    """smearing within a channel is significant "when the gradient of a dispersion curve on the
+    time-frequency grid is less than unity (i.e., beyond the 'diagonal')"; "the greatest dispersion
+    delay occurs at the end of the band".  Reading T2: DM_diag = 1 / (DeltaT(nchans-1) - DeltaT(nchans-2)) with
+    DeltaT(c) = k_DM (f_c^-2 - f_top^-2) / dt in samples per unit DM (eq. 4), i.e. the DM at which the last two
+    channels are exactly one sample apart."""
+    if nchans < 2:
+        return float("inf")
+    fa = f_top + (nchans - 2) * df
+    fb = f_top + (nchans - 1) * df
+    return 1.0 / (K_DM_SCRUNCH * (1.0 / (fb * fb) - 1.0 / (fa * fa)) / dt)
+
+
+def scrunch_factors_np(dm_list, dm_diag: float, max_factor: int, vmax: int) -> np.ndarray:
+    """Reading T1 (0..DM_diag and DM_diag..2 DM_diag at full resolution, then "compress time by a
+    factor of 2", 2..4 DM_diag, repeat; "DMs between 2x and 4x the diagonal would proceed twice as
+    fast as the computation up to 2x the diagonal"): factor 1 up to 2 DM_diag, 2^k for 2^k DM_diag < DM <= 2^(k+1)
+    DM_diag.  Capped at max_factor and (reading T3) at the largest factor with factor * vmax <= 255."""
+    out = []
+    for dm in np.asarray(dm_list, dtype=np.float64):
+        f = 1
+        while f < max_factor and 2 * f * vmax <= 255 and dm > dm_diag * (2.0 * f):
+            f *= 2
+        out.append(f)
+    return np.asarray(out, dtype=np.int64)
+
+
+def scrunched_dedisperse_np(a: np.ndarray, nsamps: int, nchans: int, dt: float, f_top: float, df: float, dm_list,
+                            max_factor: int, vmax: int):
+    """The direct transform with time-scrunching, step by step in the paper's order: for every
+    factor F in use, the series at resolution F dt is made by adding adjacent pairs log2 F times; the trials of
+    that factor are dedispersed with eq. 3-5 evaluated for the sampling interval F dt (reading T4), nsamps // F
+    output samples each.  a: unpacked samples [nchans][>= needed].  -> list of (F, first trial, int64 [ndm_F][nsamps//F])."""
+    dms = np.asarray(dm_list, dtype=np.float64)
+    fac = scrunch_factors_np(dms, diagonal_dm_np(nchans, dt, f_top, df), max_factor, vmax)
+    series = np.asarray(a).astype(np.int64)
+    cur = 1
+    out = []
+    for F in sorted(set(int(f) for f in fac)):
+        while cur < F:                                    # pairs added (PAPER.md:73)
+            series = time_scrunch_np(series, series.shape[1] // 2)
+            cur *= 2
+        idx = np.nonzero(fac == F)[0]
+        delays = delay_table_np(nchans, dt * F, f_top, df, dms[idx])
+        ns = nsamps // F
+        res = np.zeros((len(idx), ns), dtype=np.int64)
+        for i in range(len(idx)):
+            for c in range(nchans):
+                d = int(delays[i, c])
+                res[i] += series[c, d:d + ns]
+        out.append((F, int(idx[0]), res))
+    return out

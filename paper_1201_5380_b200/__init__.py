@@ -22,6 +22,8 @@ __all__ = [
     "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
+    "dd_scrunch_destroy", "ScrunchSet",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
 
@@ -33,6 +35,8 @@ EXPORTED_SYMBOLS = (
     "dd_set_batch", "dd_set_killmask", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
+    "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
+    "dd_scrunch_destroy",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -91,6 +95,15 @@ def lib() -> ctypes.CDLL:
         L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
         L.dd_profile_enable.argtypes = [vp, i32]
         L.dd_profile_read.argtypes = [vp, ctypes.POINTER(i32), vp, vp]
+        L.dd_scrunch_create.argtypes = [ctypes.POINTER(vp), i32, dbl, dbl, dbl, i32, vp, i32, i32]
+        L.dd_scrunch_levels.argtypes = [vp]
+        L.dd_scrunch_level_info.argtypes = [vp, i32, vp]
+        L.dd_scrunch_required_bytes.argtypes = [vp, i64]
+        L.dd_scrunch_required_bytes.restype = i64
+        L.dd_scrunch_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
+        L.dd_scrunch_destroy.argtypes = [vp]
+        for name in ("dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_execute", "dd_scrunch_destroy"):
+            getattr(L, name).restype = i32
         L.dd_strerror.argtypes = [i32]
         L.dd_strerror.restype = ctypes.c_char_p
         L.dd_last_cuda_error.argtypes = []
@@ -254,6 +267,72 @@ def dd_int_add_peak(mode: int = 0, stream=None) -> float:
     v = ctypes.c_double()
     _check(lib().dd_int_add_peak(int(mode), ctypes.byref(v), _stream(stream)), "dd_int_add_peak")
     return float(v.value)
+
+
+def dd_scrunch_create(nchans: int, dt: float, f_top: float, df: float, nbits: int, dm_list: Sequence[float],
+                      max_factor: int) -> int:
+    """Direct transform with time-scrunching: -> opaque set handle.  See include/dd.h."""
+    dm = np.ascontiguousarray(dm_list, dtype=np.float64)
+    h = ctypes.c_void_p()
+    _check(lib().dd_scrunch_create(ctypes.byref(h), int(nchans), float(dt), float(f_top), float(df), int(nbits),
+                                   dm.ctypes.data, int(dm.shape[0]), int(max_factor)), "dd_scrunch_create")
+    return int(h.value)
+
+
+def dd_scrunch_levels(sset: int) -> int:
+    return _check(int(lib().dd_scrunch_levels(sset)), "dd_scrunch_levels")
+
+
+def dd_scrunch_level_info(sset: int, level: int) -> dict:
+    a = np.zeros(6, dtype=np.int64)
+    _check(lib().dd_scrunch_level_info(sset, int(level), a.ctypes.data), "dd_scrunch_level_info")
+    return dict(zip(("factor", "first_dm", "ndm", "max_delay", "nbits", "dm_diag_micro"), (int(v) for v in a)))
+
+
+def dd_scrunch_required_bytes(sset: int, nsamps: int) -> int:
+    r = int(lib().dd_scrunch_required_bytes(sset, int(nsamps)))
+    if r < 0:
+        raise DDError(r, "dd_scrunch_required_bytes")
+    return r
+
+
+def dd_scrunch_execute(sset: int, nsamps: int, in_ptr, in_stride: int, out_ptrs, out_nbits: int, stream=None) -> None:
+    """out_ptrs: one DEVICE buffer per level ([ndm_l][nsamps // F_l]).  Asynchronous."""
+    arr = (ctypes.c_void_p * len(out_ptrs))(*[_addr(o) for o in out_ptrs])
+    _check(lib().dd_scrunch_execute(sset, int(nsamps), _addr(in_ptr), int(in_stride), arr, int(out_nbits),
+                                    _stream(stream)), "dd_scrunch_execute")
+
+
+def dd_scrunch_destroy(sset: int) -> None:
+    _check(lib().dd_scrunch_destroy(sset), "dd_scrunch_destroy")
+
+
+class ScrunchSet:
+    """Context-managed handle of dd_scrunch_* (argument marshalling only)."""
+
+    def __init__(self, nchans, dt, f_top, df, nbits, dm_list, max_factor):
+        self.handle = dd_scrunch_create(nchans, dt, f_top, df, nbits, dm_list, max_factor)
+
+    @property
+    def levels(self):
+        return [dd_scrunch_level_info(self.handle, l) for l in range(dd_scrunch_levels(self.handle))]
+
+    def required_bytes(self, nsamps: int) -> int:
+        return dd_scrunch_required_bytes(self.handle, nsamps)
+
+    def execute(self, nsamps, in_ptr, in_stride, out_ptrs, out_nbits, stream=None) -> None:
+        dd_scrunch_execute(self.handle, nsamps, in_ptr, in_stride, out_ptrs, out_nbits, stream)
+
+    def close(self) -> None:
+        if self.handle:
+            dd_scrunch_destroy(self.handle)
+            self.handle = 0
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
 
 
 class Plan:

@@ -20,6 +20,36 @@ __device__ __forceinline__ uint32_t nib_lo(uint32_t y)
     return (y & 0xFu) | ((y & 0xF0u) << 4) | ((y & 0xF00u) << 8) | ((y & 0xF000u) << 12);
 }
 
+// pair sums of the bytes of x in 16-bit fields
+__device__ __forceinline__ uint32_t pairs8(uint32_t x) { return (x & 0x00FF00FFu) + ((x >> 8) & 0x00FF00FFu); }
+
+// Same-width scrunch (4 -> 4, 8 -> 8 bits) for rows whose pair sums are KNOWN to fit the width: the later stages of
+// the scrunch cascade (dd_scrunch_set.cu), where a sample of the series at 2^k dt is at most 2^k (2^nbits - 1).
+// 16 input bytes -> 8 output bytes.
+template <int NB>
+__global__ void __launch_bounds__(256) dd_scrunch_same_kernel(const uint8_t *__restrict__ in, int64_t in_stride,
+                                                              uint8_t *__restrict__ out, int64_t out_stride, int64_t out_bytes)
+{
+    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i * 8 >= out_bytes)
+        return;
+    const uint4 x = __ldg(reinterpret_cast<const uint4 *>(in + static_cast<int64_t>(blockIdx.y) * in_stride) + i);
+    const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+    uint32_t h[4];   // 16 output bits per input word
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if constexpr (NB == 4) {
+            const uint32_t y = pairs4(xs[k]);   // four sums, one per byte
+            h[k] = (y & 0xFu) | ((y >> 4) & 0xF0u) | ((y >> 8) & 0xF00u) | ((y >> 12) & 0xF000u);
+        } else {
+            const uint32_t y = pairs8(xs[k]);   // two sums, one per half word
+            h[k] = (y & 0xFFu) | ((y >> 8) & 0xFF00u);
+        }
+    }
+    *reinterpret_cast<uint2 *>(out + static_cast<int64_t>(blockIdx.y) * out_stride + i * 8) =
+        make_uint2(h[0] | (h[1] << 16), h[2] | (h[3] << 16));
+}
+
 template <int NIN, int NOUT>
 __global__ void __launch_bounds__(256) dd_scrunch_kernel(const uint8_t *__restrict__ in, int64_t in_stride,
                                                          uint8_t *__restrict__ out, int64_t out_stride, int64_t out_bytes)
@@ -57,7 +87,7 @@ __global__ void __launch_bounds__(256) dd_scrunch_kernel(const uint8_t *__restri
 cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t *in, int64_t in_stride, uint8_t *out,
                            int64_t out_stride, int64_t out_bytes, cudaStream_t stream)
 {
-    const int ob = 16 * nbits_out / (2 * nbits_in);
+    const int ob = 16 * nbits_out / (2 * nbits_in);   // output bytes per thread (16 input bytes)
     const int64_t threads = (out_bytes + ob - 1) / ob;
     const dim3 grid(static_cast<unsigned>((threads + 255) / 256), static_cast<unsigned>(nrows));
     if (nbits_in == 2 && nbits_out == 4)
@@ -66,7 +96,13 @@ cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t
         dd_scrunch_kernel<4, 8><<<grid, 256, 0, stream>>>(in, in_stride, out, out_stride, out_bytes);
     else if (nbits_in == 2 && nbits_out == 8)
         dd_scrunch_kernel<2, 8><<<grid, 256, 0, stream>>>(in, in_stride, out, out_stride, out_bytes);
-    else
+    else if (nbits_in == nbits_out && (nbits_in == 4 || nbits_in == 8)) {   // sums known to fit (scrunch cascade)
+        const dim3 g8(static_cast<unsigned>(((out_bytes + 7) / 8 + 255) / 256), static_cast<unsigned>(nrows));
+        if (nbits_in == 4)
+            dd_scrunch_same_kernel<4><<<g8, 256, 0, stream>>>(in, in_stride, out, out_stride, out_bytes);
+        else
+            dd_scrunch_same_kernel<8><<<g8, 256, 0, stream>>>(in, in_stride, out, out_stride, out_bytes);
+    } else
         return cudaErrorInvalidValue;
     return cudaGetLastError();
 }

@@ -203,3 +203,38 @@ def test_time_scrunch_argument_checks_need_no_gpu():
     assert call(in_ptr=24) == -4 and call(out_ptr=8) == -4 and call(in_stride=520) == -4 and call(out_stride=500) == -4
     assert call(out_stride=496) == -5          # 1000 4-bit samples = 500 bytes -> 512
     assert call(in_stride=496) == -5           # 512 output bytes of 4-bit sums need 512 input bytes of 2-bit samples
+
+
+def test_scrunch_set_host_side():
+    # dd_scrunch_*: levels, factors and delays equal the oracle's readings T1-T4; argument errors; no GPU needed
+    cfg = W.CONFIGS[2]
+    dms = cfg.dm_list()
+    with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, 64) as s:
+        lv = s.levels
+        diag = oracle.diagonal_dm_np(cfg.nchans, cfg.dt, cfg.f_top, cfg.df)
+        fac = oracle.scrunch_factors_np(dms, diag, 64, 3)
+        assert [l["factor"] for l in lv] == sorted(set(int(f) for f in fac)) == [1, 2, 4, 8, 16]
+        assert lv[0]["dm_diag_micro"] == round(diag * 1e6)
+        for l in lv:
+            idx = np.nonzero(fac == l["factor"])[0]
+            assert (l["first_dm"], l["ndm"]) == (int(idx[0]), len(idx))
+            tab = oracle.delay_table(cfg.nchans, cfg.dt * l["factor"], cfg.f_top, cfg.df, np.asarray(dms)[idx])
+            assert l["max_delay"] == int(tab.max())
+            assert l["nbits"] == {1: 2, 2: 4, 4: 4, 8: 8, 16: 8}[l["factor"]]
+        need = s.required_bytes(1 << 16)
+        assert need % 16 == 0
+        for l in lv:   # every level's own rows fit into what the input must provide
+            assert need * 8 // cfg.nbits >= l["factor"] * ((1 << 16) // l["factor"] + l["max_delay"])
+        assert need * 8 // cfg.nbits <= (1 << 16) + 16 * lv[-1]["max_delay"] + 16 * 128 * 4
+        with pytest.raises(dd.DDError):
+            s.required_bytes(8)                      # fewer samples than the largest factor
+    with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, 1) as s:
+        assert [l["factor"] for l in s.levels] == [1] and s.levels[0]["ndm"] == cfg.ndm
+    with dd.ScrunchSet(64, 64e-6, 1500.0, -1.0, 8, [0.0, 500.0, 5000.0], 64) as s:
+        assert [l["factor"] for l in s.levels] == [1]                       # 8-bit pair sums do not fit 8 bits
+    for bad in (dict(dm=[10.0, 5.0], mf=4), dict(dm=[0.0, 1.0], mf=3), dict(dm=[0.0, 1.0], mf=0), dict(dm=[], mf=2),
+                dict(dm=[-1.0], mf=2)):
+        with pytest.raises(dd.DDError):
+            dd.ScrunchSet(64, 64e-6, 1500.0, -1.0, 2, bad["dm"], bad["mf"])
+    with pytest.raises(dd.DDError):
+        dd.ScrunchSet(64, 64e-6, 1500.0, +1.0, 2, [0.0], 2)                 # observing parameters are validated too

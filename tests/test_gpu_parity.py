@@ -311,6 +311,47 @@ def test_time_scrunch_and_dedispersion_of_the_scrunched_series(widths):
     assert np.array_equal(out.cpu().numpy().view(np.uint32), ref)
 
 
+@pytest.mark.parametrize("case", [
+    # (config, nchans, nsamps, max_factor, DM list)
+    (2, 96, 4000 + 37, 64, [0.0, 30.0, 90.0, 150.0, 155.0, 290.0, 400.0, 640.0, 990.0, 1000.0]),   # 2-bit: factors 1..8
+    (2, 1024, 2048, 4, [0.0, 60.0, 70.0, 200.0, 999.0]),                                          # capped at 4
+    (4, 64, 3100, 64, [0.0, 100.0, 300.0, 700.0, 1500.0, 1999.0, 2000.0]),                        # 4-bit: up to 16
+    (5, 32, 900, 64, [0.0, 500.0, 1000.0]),                                                       # 8-bit: one level
+])
+def test_scrunched_transform_matches_the_oracle_level_by_level(case):
+    # pairs of samples added beyond 2x, 4x, ... the diagonal DM; every level bit-exact
+    idx, nchans, nsamps, max_factor, dms = case
+    base = W.CONFIGS[idx]
+    cfg = base.reduced(nsamps=nsamps, ndm=len(dms), nchans=nchans)
+    dms = np.asarray(dms, dtype=np.float64)
+    with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, max_factor) as s:
+        lv = s.levels
+        need_bytes = s.required_bytes(nsamps)
+        nsamp_in = need_bytes * 8 // cfg.nbits
+        packed, stride = W.gen_packed(cfg, nsamp_in - nsamps)
+        assert stride >= need_bytes
+        ref = oracle.scrunched_dedisperse(packed[0].numpy(), cfg.nbits, nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df,
+                                          dms, max_factor, nsamp_in)
+        assert [l["factor"] for l in lv] == [F for F, _, _ in ref]
+        if idx == 2 and nchans == 96:
+            assert [l["factor"] for l in lv] == [1, 2, 4, 8]
+        dev = packed[0].cuda()
+        outs = [torch.full((l["ndm"], nsamps // l["factor"]), -1, dtype=torch.int32, device="cuda") for l in lv]
+        for rep in range(2):                               # the second call reuses the set's buffers
+            s.execute(nsamps, dev, stride, outs, -32, torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            for l, o, (F, first, want) in zip(lv, outs, ref):
+                assert l["first_dm"] == first
+                assert np.array_equal(o.cpu().numpy().view(np.uint32), want.astype(np.uint32)), f"factor {F}"
+        f_outs = [torch.zeros((l["ndm"], nsamps // l["factor"]), dtype=torch.float32, device="cuda") for l in lv]
+        s.execute(nsamps, dev, stride, f_outs, 32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        for o, (F, first, want) in zip(f_outs, ref):
+            assert np.array_equal(o.cpu().numpy(), want.astype(np.float32))
+        with pytest.raises(dd.DDError):                    # rows shorter than the set needs
+            s.execute(nsamps, dev, 16, outs, -32, None)
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)

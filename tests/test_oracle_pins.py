@@ -1,6 +1,6 @@
 """Pins for the CPU oracle (oracle/) -- what the paper and the mathematics fix, NOT the oracle re-typed.
 
-Pin numbering follows DESIGN.md section 3 (P1..P14).  None of these tests touches the CUDA path.
+Pin numbering follows DESIGN.md section 3 (P1..P15).  None of these tests touches the CUDA path.
 
   P1  hand-evaluated eq. 1 delays (tests/golden/delays_eq1_hand.txt)
   P2  closed-form properties + exact rational arithmetic (fractions.Fraction)
@@ -17,6 +17,9 @@ Pin numbering follows DESIGN.md section 3 (P1..P14).  None of these tests touche
   P13 sub-band method: reduces to the direct transform for 1-channel sub-bands; equals a direct transform with
       the summed delays; error of the summed delays within the analytic bound; impulse response
   P14 time-scrunching: hand example, conservation of the total, equals a reshape-sum
+  P15 transform with time-scrunching: the diagonal DM in exact rational arithmetic (unit gradient at the end of the
+      band); factor ranges by their definition; every level equals the pinned C loop at full resolution with the
+      delays F * delay_F, summed over F consecutive outputs; max_factor 1 is the plain transform
 """
 import math
 import os
@@ -447,3 +450,60 @@ def test_oracle_regression_file(golden_dir):
     stored = {r[0]: tuple(int(x) for x in r[1:]) for r in _read_rows(os.path.join(golden_dir, "oracle_regression.txt"))}
     for name, cfg in mg.cases():
         assert mg.checksum(mg.run_case(cfg)) == stored[name], name
+
+
+# ----------------------------------------------------------------------------- P15
+def test_p15_diagonal_dm_is_the_unit_gradient_at_the_end_of_the_band():
+    # exact rational arithmetic: at DM_diag the (unrounded) eq. 4 delays of the last two channels differ by 1 sample
+    K = Fraction(4148808, 1000)
+    for idx in (1, 2, 3, 4):
+        cfg = W.CONFIGS[idx]
+        dt, f_top, df = Fraction(cfg.dt).limit_denominator(10 ** 12), Fraction(cfg.f_top).limit_denominator(10 ** 9), \
+            Fraction(cfg.df).limit_denominator(10 ** 12)
+        fa, fb = f_top + (cfg.nchans - 2) * df, f_top + (cfg.nchans - 1) * df
+        grad = K * (1 / (fb * fb) - 1 / (fa * fa)) / dt                      # samples per unit DM between the two
+        got = oracle.diagonal_dm_np(cfg.nchans, cfg.dt, cfg.f_top, cfg.df)
+        assert abs(Fraction(got) * grad - 1) < Fraction(1, 10 ** 9)
+    # cfg1 by hand: 4148.808 * (1437^-2 - 1438^-2) / 64e-6 = 0.0436465...  ->  DM_diag = 22.9113
+    assert oracle.diagonal_dm_np(64, 64e-6, 1500.0, -1.0) == pytest.approx(22.9113, abs=5e-5)
+    assert oracle.diagonal_dm_np(1, 64e-6, 1500.0, -1.0) == float("inf")
+
+
+def test_p15_factor_ranges_by_definition():
+    diag = 32.5
+    dms = np.array([0.0, 32.5, 65.0, 65.0001, 130.0, 130.0001, 260.0, 260.1, 520.0, 520.1, 1000.0, 5000.0])
+    got = oracle.scrunch_factors_np(dms, diag, 64, 3)
+    assert list(got) == [1, 1, 1, 2, 2, 4, 4, 8, 8, 16, 16, 64]            # 5000 > 64 * 32.5: capped at max_factor
+    for dm, f in zip(dms, got):                                           # the definition: F diag < DM <= 2 F diag
+        assert (f == 1 and dm <= 2 * diag) or (f * diag < dm and (dm <= 2 * f * diag or f == 64))
+    assert list(oracle.scrunch_factors_np(dms, diag, 4, 3)) == [1, 1, 1, 2, 2, 4, 4, 4, 4, 4, 4, 4]
+    assert list(oracle.scrunch_factors_np(dms, diag, 64, 15)) == [1, 1, 1, 2, 2, 4, 4, 8, 8, 16, 16, 16]   # 32 * 15 > 255
+    assert set(oracle.scrunch_factors_np(dms, diag, 64, 255)) == {1}                                       # 8-bit input
+
+
+@pytest.mark.parametrize("nbits", [2, 4])
+def test_p15_levels_equal_the_full_resolution_loop_summed_over_f_outputs(nbits):
+    # A_F[c][t + d] = sum_{i<F} A[c][F (t + d) + i]  =>  D_F[d][t] = sum_{i<F} D'[d][F t + i], D' = eq. 3 at full
+    # resolution with the delays F * delay_F -- evaluated by the pinned C loop
+    base = W.CONFIGS[2 if nbits == 2 else 4]
+    nchans, nsamps = 48, 640
+    dms = np.array([0.0, 40.0, 100.0, 170.0, 200.0, 390.0, 500.0, 800.0, 1500.0, 1999.0])
+    diag = oracle.diagonal_dm_np(nchans, base.dt, base.f_top, base.df)
+    fac = oracle.scrunch_factors_np(dms, diag, 64, (1 << nbits) - 1)
+    assert len(set(fac)) >= 4 and fac[0] == 1
+    need = max(int(F) * (nsamps // int(F) + int(oracle.delay_table(nchans, base.dt * int(F), base.f_top, base.df, dms[fac == F]).max()))
+               for F in set(fac)) + 64
+    rng = np.random.default_rng(150 + nbits)
+    a = rng.integers(0, 1 << nbits, size=(nchans, need), dtype=np.int64)
+    levels = oracle.scrunched_dedisperse_np(a, nsamps, nchans, base.dt, base.f_top, base.df, dms, 64, (1 << nbits) - 1)
+    assert [F for F, _, _ in levels] == sorted(set(int(f) for f in fac))
+    for F, first, res in levels:
+        idx = np.nonzero(fac == F)[0]
+        assert first == idx[0] and res.shape == (len(idx), nsamps // F)
+        dF = oracle.delay_table(nchans, base.dt * F, base.f_top, base.df, dms[idx])
+        full = oracle.dedisperse_unpacked(a, (nsamps // F) * F, dF * F)
+        assert np.array_equal(res, full.reshape(len(idx), nsamps // F, F).sum(axis=2))
+    # max_factor = 1: one level, the plain transform
+    one = oracle.scrunched_dedisperse_np(a, nsamps, nchans, base.dt, base.f_top, base.df, dms[:5], 1, (1 << nbits) - 1)
+    assert len(one) == 1 and one[0][0] == 1
+    assert np.array_equal(one[0][2], oracle.dedisperse_unpacked(a, nsamps, oracle.delay_table(nchans, base.dt, base.f_top, base.df, dms[:5])))
