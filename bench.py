@@ -182,6 +182,47 @@ def run_reference(args) -> None:
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------ time-scrunching (side measurement)
+def run_scrunch(args) -> None:
+    """`--scrunch MAXF`: the transform with time-scrunching (dd_scrunch_*) on the config's DM list,
+    timed like the main arm (CUDA events on the launching stream).  A side measurement, not the headline line."""
+    import torch
+
+    import dd_workloads as W
+    import paper_1201_5380_b200 as dd
+
+    torch.cuda.set_device(0)
+    cfg = W.CONFIGS[args.config]
+    stream = torch.cuda.Stream()
+    sset = dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, cfg.dm_list(), args.scrunch)
+    lv = sset.levels
+    need = sset.required_bytes(cfg.nsamps)
+    packed, stride = W.gen_packed(cfg, need * 8 // cfg.nbits - cfg.nsamps, None, device="cuda", beams=[0], chan_chunk=16)
+    outs = [torch.empty((l["ndm"], cfg.nsamps // l["factor"]), dtype=torch.float32, device="cuda") for l in lv]
+    for _ in range(max(args.warmup, 3)):
+        sset.execute(cfg.nsamps, packed[0], stride, outs, 32, stream)
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    with ClockSampler(0) as clk:
+        with torch.cuda.stream(stream):
+            ev[0].record(stream)
+            for _ in range(args.steps):
+                sset.execute(cfg.nsamps, packed[0], stride, outs, 32, stream)
+            ev[1].record(stream)
+        torch.cuda.synchronize()
+    ms = ev[0].elapsed_time(ev[1]) / args.steps
+    units = sum(l["ndm"] * (cfg.nsamps // l["factor"]) for l in lv)
+    print(json.dumps({
+        "metric": METRIC + " -- with time-scrunching (side measurement)", "value": units / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg.name, "method": "direct with time-scrunching (lower time resolution at high DM)",
+                   "max_factor": args.scrunch, "dm_diag": lv[0]["dm_diag_micro"] / 1e6, "levels": lv,
+                   "outputs_per_step": units, "full_resolution_outputs": cfg.ndm * cfg.nsamps},
+        "full_resolution_equivalent_per_s": cfg.ndm * cfg.nsamps / (ms * 1e-3), "clocks": clk.summary()}))
+    sset.close()
+
+
 # ------------------------------------------------------------------------------------------ our arm
 def run_ours(args) -> None:
     import torch
@@ -347,6 +388,8 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--subband", default="", help="SB,GRP: time the sub-band method (channels per sub-band, trials per "
                     "nominal DM) instead of the direct transform; implies --no-e2e")
+    ap.add_argument("--scrunch", type=int, default=0, help="MAXF: time the transform with time-scrunching up to this "
+                    "factor (a power of two) instead -- a side measurement")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")
     ap.add_argument("--cpu-nsamps", type=int, default=1 << 18, help="output samples of the bounded oracle sample")
@@ -356,6 +399,8 @@ def main() -> None:
         args.no_e2e = True
     if args.impl == "reference":
         run_reference(args)
+    elif args.scrunch:
+        run_scrunch(args)
     else:
         run_ours(args)
 

@@ -100,6 +100,15 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm);
 dd_status dd_set_killmask(dd_plan plan, const int32_t *mask);
 
 /*
+ * dd_set_input_max -- the caller's promise that no input sample exceeds vmax (e.g. a series made by adding 2^k
+ * 2-bit samples: vmax = 3 * 2^k).  The bit-plane kernel then neither shifts nor adds the planes that
+ * cannot be set (bit_length(vmax) of the nbits planes are used).  Results are undefined if the promise is broken.
+ *   vmax  1 .. 2^nbits - 1, or 0 to withdraw the promise (DD_ERR_INVALID_ARG otherwise).  Takes effect at the
+ *         next dd_execute; independent of the DM list, kill mask and batch.
+ */
+dd_status dd_set_input_max(dd_plan plan, int vmax);
+
+/*
  * dd_set_subband -- switches the plan to the SUB-BAND method of PAPER.md:317-321, an approximation of the
  * transform that costs about (1/dm_group + 1/sb_nchans) of the direct one (eq. 30), done as the paper's own
  * implementation did it: "two consecutive calls to the direct dedispersion routine and the addition of a

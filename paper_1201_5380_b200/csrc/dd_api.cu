@@ -726,6 +726,19 @@ dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int
     return DD_OK;
 }
 
+dd_status dd_set_input_max(dd_plan plan, int vmax)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (vmax < 0 || vmax > (1 << plan->nbits) - 1)
+        return DD_ERR_INVALID_ARG;
+    int planes = 0;
+    while (vmax >> planes)
+        ++planes;
+    plan->in_planes = planes;   // 0 = all nbits planes
+    return DD_OK;
+}
+
 dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)

@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     // epilogue transposes 16 x 16 bit matrices instead of 32 x 32
     constexpr int NP = (NBITS == 8 && !LONG) ? 16 : C::NP;
     static_assert(LONG || static_cast<int64_t>(8 * CC * C::FL) * ((1 << NBITS) - 1) <= (int64_t(1) << NP), "short-mode sums must fit NP planes");
-    static_assert(PIN >= 1 && PIN <= NBITS && (PIN == NBITS || !LONG), "fewer planes: short instantiation only");
+    static_assert(PIN >= 1 && PIN <= NBITS, "planes in use");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
     constexpr int FL = LONG ? C::FL : 1;
     constexpr bool PATCH = !LONG || NBITS < 8;
@@ -764,11 +764,17 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     if (plan->long_mode && kp.nchunks % C::FL != 0)
         return cudaErrorInvalidValue;
     auto kernel = plan->long_mode ? dd_direct_bp<NBITS, true> : dd_direct_bp<NBITS, false>;
-    if constexpr (NBITS == 8) {   // sub-band step 2: samples known to stay below 2^in_planes
-        if (!plan->long_mode && plan->in_planes > 0 && plan->in_planes <= 6)
-            kernel = dd_direct_bp<8, false, 6>;
-        else if (!plan->long_mode && plan->in_planes == 7)
-            kernel = dd_direct_bp<8, false, 7>;
+    // samples known to stay below 2^in_planes (sub-band step 2; scrunched series via dd_set_input_max): the
+    // instantiation that skips the planes which cannot be set
+    const int pin = plan->in_planes > 0 ? plan->in_planes : NBITS;
+    if constexpr (NBITS == 8) {
+        if (plan->long_mode)
+            kernel = pin <= 5 ? dd_direct_bp<8, true, 5> : pin == 6 ? dd_direct_bp<8, true, 6> : pin == 7 ? dd_direct_bp<8, true, 7> : kernel;
+        else
+            kernel = pin <= 6 ? dd_direct_bp<8, false, 6> : pin == 7 ? dd_direct_bp<8, false, 7> : kernel;
+    } else if constexpr (NBITS == 4) {
+        if (plan->long_mode && pin <= 3)
+            kernel = dd_direct_bp<4, true, 3>;
     }
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)

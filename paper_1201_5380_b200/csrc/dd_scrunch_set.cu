@@ -143,6 +143,8 @@ dd_status dd_scrunch_create(dd_scrunch *set, int nchans, double dt, double f_top
             if (s->stages[k].factor == l.factor)
                 l.stage = static_cast<int>(k);
         st = dd_plan_create(&l.plan, nchans, dt * l.factor, f_top, df, l.nbits);
+        if (st == DD_OK && l.factor > 1)   // a sample of the series at F dt is at most F (2^nbits - 1)
+            st = dd_set_input_max(l.plan, l.factor * ((1 << nbits) - 1));
         if (st == DD_OK)
             st = dd_set_dm_list(l.plan, dm_list + d, l.ndm);
         if (st == DD_OK) {

@@ -352,6 +352,36 @@ def test_scrunched_transform_matches_the_oracle_level_by_level(case):
             s.execute(nsamps, dev, 16, outs, -32, None)
 
 
+@pytest.mark.parametrize("case", [(8, 160, 24), (8, 160, 48), (8, 136, 100), (8, 40, 30), (8, 40, 200), (4, 528, 6), (4, 48, 5)])
+def test_input_max_promise_skips_planes_but_not_results(case):
+    # dd_set_input_max: samples <= vmax -> the instantiation that leaves out the planes that cannot be set
+    # (long instantiations: 8-bit with >= 128 channels, 4-bit with >= 512; short ones below that)
+    nbits, nchans, vmax = case
+    base = W.CONFIGS[5 if nbits == 8 else 4]
+    cfg = base.reduced(nsamps=3072 + 100, ndm=19, nchans=nchans)
+    tab = _oracle_table(cfg)
+    nsamp_in = (cfg.nsamps + int(tab.max()) + 127) // 128 * 128
+    rng = np.random.default_rng(1000 * nbits + vmax)
+    vals = rng.integers(0, vmax + 1, size=(nchans, nsamp_in), dtype=np.int64)
+    vals[:, ::97] = vmax                                                      # the largest value does occur
+    packed = W.pack_rows(torch.from_numpy(vals.astype(np.uint8)), nbits).contiguous()
+    stride = packed.shape[1]
+    ref = oracle.dedisperse(packed.numpy(), nbits, cfg.nsamps, tab)
+    out = torch.full((cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, nbits) as p:
+        p.set_dm_list(cfg.dm_list()).set_input_max(vmax)
+        p.execute(cfg.nsamps, packed.cuda(), stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref.astype(np.uint32))
+        p.set_input_max(0)                                                    # promise withdrawn: same result
+        out.fill_(-1)
+        p.execute(cfg.nsamps, packed.cuda(), stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref.astype(np.uint32))
+        with pytest.raises(dd.DDError):
+            p.set_input_max(1 << nbits)
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)
