@@ -234,7 +234,7 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
     int sms = 148;
     (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device >= 0 ? plan->device : 0);
     const int64_t ctas1 = static_cast<int64_t>(k1.nblk) * k1.ntiles * nbeams * k1.ngroups;
-    int64_t gpc = ctas1 / (4 * static_cast<int64_t>(sms));
+    int64_t gpc = ctas1 / (8 * static_cast<int64_t>(sms));   // measured on the cfg2 shape: flat from 4 to 16 sub-bands per CTA
     if (const char *envv = std::getenv("DD_SB_GPC"))   // test hook: groups per CTA
         gpc = std::atoi(envv);
     k1.gpc = static_cast<int32_t>(std::max<int64_t>(1, std::min<int64_t>(gpc, k1.ngroups)));
