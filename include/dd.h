@@ -100,6 +100,18 @@ dd_status dd_set_dm_list(dd_plan plan, const double *dm_list, int ndm);
 dd_status dd_set_killmask(dd_plan plan, const int32_t *mask);
 
 /*
+ * dd_set_output_stride -- "arbitrary strides through the ... output arrays" (footnote 5): the rows of
+ * consecutive DM trials of the output lie out_dm_stride BYTES apart instead of densely, out[beam][d] starting at
+ * out_ptr + beam * out_beam_stride + d * out_dm_stride (e.g. rows padded to a power of two for a later FFT, or a
+ * window of a larger array).  Applies to dd_execute (device rows) and dd_execute_host (host rows).
+ *   out_dm_stride  0 = dense rows of nsamps elements (default); otherwise a multiple of the element size
+ *                  (DD_ERR_ALIGNMENT at execute) and >= nsamps * element size (DD_ERR_STRIDE_TOO_SMALL at execute);
+ *                  with a batch, out_beam_stride must cover (ndm - 1) * out_dm_stride + nsamps elements.
+ *                  Rows that are 16-byte aligned take the fastest store path.  Negative: DD_ERR_INVALID_ARG.
+ */
+dd_status dd_set_output_stride(dd_plan plan, int64_t out_dm_stride);
+
+/*
  * dd_set_input_max -- the caller's promise that no input sample exceeds vmax (e.g. a series made by adding 2^k
  * 2-bit samples: vmax = 3 * 2^k).  The bit-plane kernel then neither shifts nor adds the planes that
  * cannot be set (bit_length(vmax) of the nbits planes are used).  Results are undefined if the promise is broken.

@@ -19,7 +19,7 @@ import numpy as np
 __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_set_killmask", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
+    "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
@@ -32,7 +32,7 @@ DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
 # every symbol include/dd.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
-    "dd_set_batch", "dd_set_killmask", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
+    "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
@@ -84,6 +84,8 @@ def lib() -> ctypes.CDLL:
         L.dd_set_killmask.argtypes = [vp, vp]
         L.dd_set_subband.argtypes = [vp, i32, i32]
         L.dd_set_input_max.argtypes = [vp, i32]
+        L.dd_set_output_stride.argtypes = [vp, i64]
+        L.dd_set_output_stride.restype = i32
         L.dd_set_input_max.restype = i32
         L.dd_set_subband.restype = i32
         L.dd_get_subband_extent.argtypes = [vp]
@@ -199,6 +201,11 @@ def dd_time_scrunch(nrows: int, nsamps_out: int, in_ptr, in_stride: int, nbits_i
     """out[r][t] = in[r][2t] + in[r][2t+1] on packed DEVICE rows; asynchronous."""
     _check(lib().dd_time_scrunch(int(nrows), int(nsamps_out), _addr(in_ptr), int(in_stride), int(nbits_in), _addr(out_ptr),
                                  int(out_stride), int(nbits_out), _stream(stream)), "dd_time_scrunch")
+
+
+def dd_set_output_stride(plan: int, out_dm_stride: int) -> None:
+    """Bytes between the output rows of consecutive DM trials (0 = dense)."""
+    _check(lib().dd_set_output_stride(plan, int(out_dm_stride)), "dd_set_output_stride")
 
 
 def dd_set_input_max(plan: int, vmax: int) -> None:
@@ -373,6 +380,10 @@ class Plan:
     def subband_tables(self):
         sb, grp = self._subband
         return dd_get_subband_tables(self.handle, self.ndm, self.nchans, sb, grp)
+
+    def set_output_stride(self, out_dm_stride: int) -> "Plan":
+        dd_set_output_stride(self.handle, out_dm_stride)
+        return self
 
     def set_input_max(self, vmax: int) -> "Plan":
         dd_set_input_max(self.handle, vmax)

@@ -147,8 +147,10 @@ static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_st
     return DD_OK;
 }
 
+// out_dm_stride: bytes between output rows, 0 = dense
 static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *in, int64_t in_stride, void *out,
-                                int out_nbits, int nbeams, int64_t in_beam_stride, int64_t out_beam_stride)
+                                int out_nbits, int nbeams, int64_t in_beam_stride, int64_t out_beam_stride,
+                                int64_t out_dm_stride = 0)
 {
     KernelParams kp{};
     kp.in = static_cast<const uint8_t *>(in);
@@ -161,8 +163,12 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
     kp.out_code = out_nbits;
     const int es = elem_size(out_nbits);
     const int vec_bytes = 4 * es;
-    kp.vec_ok = (nsamps % 4 == 0) && (reinterpret_cast<uintptr_t>(out) % vec_bytes == 0) &&
-                (out_beam_stride % vec_bytes == 0);
+    kp.out_dm_stride = out_dm_stride > 0 ? out_dm_stride : nsamps * es;
+    auto aligned = [&](int64_t a) {   // every row starts on a multiple of a bytes
+        return kp.out_dm_stride % a == 0 && reinterpret_cast<uintptr_t>(out) % a == 0 && out_beam_stride % a == 0;
+    };
+    kp.vec_ok = aligned(vec_bytes);
+    kp.vec16_ok = aligned(16);
     kp.nchans = p->nlive;
     kp.nrows = p->nchans;
     kp.ndm = p->ndm;
@@ -213,7 +219,7 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
     cudaError_t e;
     // step 2's launch geometry first: N_SB channels; DM block blk reads the rows of nominal DM blk / (dm_group / 16)
     const int64_t out_beam = nbeams > 1 ? plan->out_beam_stride : 0;
-    KernelParams k2 = make_params(s2, nsamps, nullptr, 16, out_ptr, out_nbits, nbeams, 0, out_beam);
+    KernelParams k2 = make_params(s2, nsamps, nullptr, 16, out_ptr, out_nbits, nbeams, 0, out_beam, plan->out_dm_stride);
     k2.nrows = nsb * ngrp;
     k2.row_mul = ngrp;
     k2.in_blk_div = plan->dm_group / s2->var.DB;
@@ -529,21 +535,27 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
     const int es = elem_size(out_nbits);
     if (reinterpret_cast<uintptr_t>(in_ptr) % 16 != 0 || reinterpret_cast<uintptr_t>(out_ptr) % es != 0)
         return DD_ERR_ALIGNMENT;
+    const int64_t pitch = plan->out_dm_stride > 0 ? plan->out_dm_stride : nsamps * es;   // bytes between output rows
+    if (pitch % es != 0)
+        return DD_ERR_ALIGNMENT;
+    if (pitch < nsamps * es)
+        return DD_ERR_STRIDE_TOO_SMALL;
     if (plan->nbeams > 1) {
         if (plan->out_beam_stride % es != 0)
             return DD_ERR_ALIGNMENT;
         if (plan->in_beam_stride < static_cast<int64_t>(plan->nchans) * in_stride ||
-            plan->out_beam_stride < static_cast<int64_t>(plan->ndm) * nsamps * es)
+            plan->out_beam_stride < static_cast<int64_t>(plan->ndm - 1) * pitch + nsamps * es)
             return DD_ERR_STRIDE_TOO_SMALL;
     }
     cudaStream_t st_ = static_cast<cudaStream_t>(stream);
     if (plan->nlive == 0) {   // every channel killed: the sums are zero (float32 zero is all-zero bits too)
-        const size_t beam_bytes = static_cast<size_t>(plan->ndm) * nsamps * es;
-        const cudaError_t me = plan->nbeams > 1
-                                   ? cudaMemset2DAsync(out_ptr, plan->out_beam_stride, 0, beam_bytes, plan->nbeams, st_)
-                                   : cudaMemsetAsync(out_ptr, 0, beam_bytes, st_);
-        if (me != cudaSuccess)
-            return cuda_fail(me, "dd_execute memset");
+        for (int b = 0; b < plan->nbeams; ++b) {
+            uint8_t *o = static_cast<uint8_t *>(out_ptr) + static_cast<int64_t>(b) * (plan->nbeams > 1 ? plan->out_beam_stride : 0);
+            const cudaError_t me = cudaMemset2DAsync(o, static_cast<size_t>(pitch), 0, static_cast<size_t>(nsamps) * es,
+                                                     static_cast<size_t>(plan->ndm), st_);
+            if (me != cudaSuccess)
+                return cuda_fail(me, "dd_execute memset");
+        }
         plan->last_launches = 0;
         return DD_OK;
     }
@@ -555,7 +567,7 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
             return st;
     }
     const KernelParams kp = make_params(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, plan->nbeams,
-                                        plan->in_beam_stride, plan->out_beam_stride);
+                                        plan->in_beam_stride, plan->out_beam_stride, plan->out_dm_stride);
     const bool prof = plan->prof_cap > 0 && plan->prof_n < plan->prof_cap;
     cudaEvent_t *ev = prof ? reinterpret_cast<cudaEvent_t *>(plan->prof_events.data()) + 3 * plan->prof_n : nullptr;
     plan->prof_mid = nullptr;
@@ -589,13 +601,19 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     const int es = elem_size(out_nbits);
     if (plan->sb_nchans > 0)
         return DD_ERR_INVALID_ARG;   // the sub-band method is offered on device buffers only (dd.h)
+    const int64_t row_pitch = plan->out_dm_stride > 0 ? plan->out_dm_stride : nsamps * es;   // host rows (dd_set_output_stride)
+    if (row_pitch % es != 0)
+        return DD_ERR_ALIGNMENT;
+    if (row_pitch < nsamps * es)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    const int64_t beam_span = static_cast<int64_t>(plan->ndm - 1) * row_pitch + nsamps * es;   // bytes a beam's rows cover
     if (plan->nlive == 0) {   // every channel killed
-        const size_t beam_bytes = static_cast<size_t>(plan->ndm) * nsamps * es;
-        const size_t pitch = plan->nbeams > 1 ? static_cast<size_t>(plan->out_beam_stride) : beam_bytes;
-        if (plan->nbeams > 1 && pitch < beam_bytes)
+        const int64_t pitch = plan->nbeams > 1 ? plan->out_beam_stride : 0;
+        if (plan->nbeams > 1 && pitch < beam_span)
             return DD_ERR_STRIDE_TOO_SMALL;
         for (int b = 0; b < plan->nbeams; ++b)
-            std::memset(static_cast<uint8_t *>(out_host) + b * pitch, 0, beam_bytes);
+            for (int d = 0; d < plan->ndm; ++d)
+                std::memset(static_cast<uint8_t *>(out_host) + b * pitch + d * row_pitch, 0, static_cast<size_t>(nsamps) * es);
         plan->last_launches = 0;
         return DD_OK;
     }
@@ -606,9 +624,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     }
     const int nbeams = plan->nbeams;
     const int64_t in_beam = nbeams > 1 ? plan->in_beam_stride : static_cast<int64_t>(plan->nchans) * in_stride;
-    const int64_t out_beam_host = nbeams > 1 ? plan->out_beam_stride : static_cast<int64_t>(plan->ndm) * nsamps * es;
-    if (nbeams > 1 && (in_beam < static_cast<int64_t>(plan->nchans) * in_stride ||
-                       out_beam_host < static_cast<int64_t>(plan->ndm) * nsamps * es))
+    const int64_t out_beam_host = nbeams > 1 ? plan->out_beam_stride : static_cast<int64_t>(plan->ndm) * row_pitch;
+    if (nbeams > 1 && (in_beam < static_cast<int64_t>(plan->nchans) * in_stride || out_beam_host < beam_span))
         return DD_ERR_STRIDE_TOO_SMALL;
 
     // Time slabs: the input slab of output samples [s0, s0+len) is rows [s0, s0+len+max_delay); the slab
@@ -684,7 +701,7 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
         for (int beam = 0; beam < nbeams; ++beam) {
             uint8_t *dst = static_cast<uint8_t *>(out_host) + static_cast<size_t>(beam) * out_beam_host + s0 * es;
             const uint8_t *src = S->d_out[b] + static_cast<size_t>(beam) * plan->ndm * len * es;
-            if ((e = cudaMemcpy2DAsync(dst, static_cast<size_t>(nsamps) * es, src, static_cast<size_t>(len) * es,
+            if ((e = cudaMemcpy2DAsync(dst, static_cast<size_t>(row_pitch), src, static_cast<size_t>(len) * es,
                                        static_cast<size_t>(len) * es, plan->ndm, cudaMemcpyDeviceToHost,
                                        S->copy_out[b])) != cudaSuccess)
                 return cuda_fail(e, "cudaMemcpy2DAsync(out)");
@@ -723,6 +740,16 @@ dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int
                                          static_cast<uint8_t *>(out_ptr), out_stride, out_bytes, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess)
         return cuda_fail(e, "dd_time_scrunch launch");
+    return DD_OK;
+}
+
+dd_status dd_set_output_stride(dd_plan plan, int64_t out_dm_stride)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (out_dm_stride < 0)
+        return DD_ERR_INVALID_ARG;
+    plan->out_dm_stride = out_dm_stride;
     return DD_OK;
 }
 

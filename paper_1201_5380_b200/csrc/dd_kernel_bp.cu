@@ -639,8 +639,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     if (d >= p.ndm)
         return;
     const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
-    uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.nsamps * esize;
-    const bool interior = PATCH && p.vec_ok && (t0 + TB <= p.nsamps);
+    uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.out_dm_stride;
+    const bool interior = PATCH && p.vec16_ok && (t0 + TB <= p.nsamps);   // 16-byte stores: rows must be 16-byte aligned
     uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
 #pragma unroll
     for (int j = 0; j < W; ++j) {

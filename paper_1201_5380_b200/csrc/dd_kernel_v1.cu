@@ -211,14 +211,13 @@ __global__ void __launch_bounds__(V1_NWARPS * 32, 1) dd_direct_v1(const KernelPa
 
     // ---- epilogue: convert and store.  Thread owns samples t0 + lane*4W + [0, 4W) of DPW DM rows.
     const int64_t tbase = t0 + lane * (4 * W);
-    const int esize = (p.out_code == DD_OUT_U16) ? 2 : 4;
     uint8_t *out_beam = p.out + static_cast<int64_t>(beam) * p.out_beam_stride;
 #pragma unroll
     for (int i = 0; i < DPW; ++i) {
         const int d = blk * DB + warp * DPW + i;
         if (d >= p.ndm)
             continue;
-        uint8_t *orow = out_beam + static_cast<int64_t>(d) * p.nsamps * esize;
+        uint8_t *orow = out_beam + static_cast<int64_t>(d) * p.out_dm_stride;
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             const int64_t t = tbase + 4 * j;

@@ -206,14 +206,13 @@ __global__ void __launch_bounds__(V2_NWARPS * 32, 1) dd_direct_v2(const KernelPa
 
     // ---- epilogue: thread owns samples t0 + lane*8W + [0, 8W) of DM slots 2*warp, 2*warp+1
     const int64_t tbase = t0 + lane * (8 * W);
-    const int esize = (p.out_code == DD_OUT_U16) ? 2 : 4;
     uint8_t *out_beam = p.out + static_cast<int64_t>(beam) * p.out_beam_stride;
 #pragma unroll
     for (int i = 0; i < DPT; ++i) {
         const int d = blk * DB + warp * DPT + i;
         if (d >= p.ndm)
             continue;
-        uint8_t *orow = out_beam + static_cast<int64_t>(d) * p.nsamps * esize;
+        uint8_t *orow = out_beam + static_cast<int64_t>(d) * p.out_dm_stride;
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             const uint32_t a = acc16[i][4 * j], b = acc16[i][4 * j + 1], c = acc16[i][4 * j + 2], dd_ = acc16[i][4 * j + 3];

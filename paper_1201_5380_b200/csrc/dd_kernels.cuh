@@ -15,9 +15,11 @@ struct KernelParams {
     int64_t in_beam_stride;   // bytes between beams
     uint8_t *out;             // device: out[beam][d][t]
     int64_t out_beam_stride;  // bytes between beams
+    int64_t out_dm_stride;    // bytes between the rows of consecutive DM trials (dense: nsamps * element size)
     int64_t nsamps;           // output samples per DM trial
     int32_t out_code;         // DD_OUT_F32 / DD_OUT_U16 / DD_OUT_U32
     int32_t vec_ok;           // rows and base pointers allow 4-sample vector stores
+    int32_t vec16_ok;         // ... and 16-byte stores at every multiple of 16 bytes inside a row (coalescing epilogue)
     int32_t nchans;           // channels summed (the live list under a kill mask); span/rel are indexed by list position
     int32_t nrows;            // channel rows of the input
     int32_t ndm, nblk, ntiles, nbeams;

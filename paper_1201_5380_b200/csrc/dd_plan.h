@@ -80,6 +80,7 @@ struct dd_plan_s {
     // batching
     int nbeams = 1;
     int64_t in_beam_stride = 0, out_beam_stride = 0;
+    int64_t out_dm_stride = 0;   // bytes between output rows (dd_set_output_stride); 0 = dense rows of nsamps elements
     // tiling
     dd::Variant var{};
     int force_variant = 0; // 0 = automatic; otherwise only this variant id is considered (dd_set_kernel_variant)

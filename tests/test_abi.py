@@ -124,6 +124,13 @@ def test_execute_argument_checks_need_no_gpu():
         assert L.dd_execute(h, 100, 24, good_stride, 16, 32, None) == -4      # in_ptr not 16-aligned
         assert L.dd_execute(h, 100, 16, good_stride, 18, 32, None) == -4      # out_ptr not element aligned
         assert L.dd_execute(h, 100, 16, 16, 16, 32, None) == -5               # rows too short
+        # dd_set_output_stride: bytes between output rows, checked at execute
+        assert L.dd_set_output_stride(h, -1) == -2
+        assert L.dd_set_output_stride(h, 398) == 0
+        assert L.dd_execute(h, 100, 16, good_stride, 16, 32, None) == -4      # not a multiple of the element size
+        assert L.dd_set_output_stride(h, 396) == 0
+        assert L.dd_execute(h, 100, 16, good_stride, 16, 32, None) == -5      # shorter than a row of 100 float32
+        assert L.dd_set_output_stride(h, 0) == 0
     with dd.Plan(8192, 64e-6, 1500.0, -0.01, 4) as p:                        # 8192*15 > 65535
         p.set_dm_list([0.0])
         assert dd.lib().dd_execute(p.handle, 100, 16, 4096, 16, 16, None) == -6

@@ -382,6 +382,76 @@ def test_input_max_promise_skips_planes_but_not_results(case):
             p.set_input_max(1 << nbits)
 
 
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_u16_rows_that_are_not_16_byte_aligned(nbits):
+    # regression: uint16 rows of nsamps % 8 == 4 samples start on 8-byte, not 16-byte boundaries; the coalescing
+    # epilogue of the bit-plane kernel stores 16 bytes at a time and must leave such rows to the plain path
+    idx = {2: 2, 4: 4, 8: 5}[nbits]
+    tb = 5120 if nbits == 2 else 3072
+    cfg = W.CONFIGS[idx].reduced(nsamps=tb + 4, ndm=5, nchans=32)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab)
+    out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.int16, device="cuda")
+    h_out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.int16).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.execute(cfg.nsamps, packed[0].cuda(), stride, out, 16, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, h_out, 16)
+    assert np.array_equal(out.cpu().numpy().view(np.uint16), ref.astype(np.uint16))
+    assert np.array_equal(h_out.numpy().view(np.uint16), ref.astype(np.uint16))
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("pad", [16, 1])   # rows padded by 16 elements (16-byte aligned rows) / by one element
+def test_output_row_stride(variant, pad):
+    # PAPER.md:388 "arbitrary strides through the ... output arrays": rows out_dm_stride bytes apart, padding untouched
+    cfg = W.CONFIGS[2].reduced(nsamps=5120 + 40, ndm=19, nchans=40, nbeams=2)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    pitch = cfg.nsamps + pad
+    for tdtype, code, es in ((torch.float32, 32, 4), (torch.int16, 16, 2)):
+        out = torch.full((2, cfg.ndm, pitch), -7, dtype=tdtype, device="cuda")
+        h_out = torch.full((2, cfg.ndm, pitch), -7, dtype=tdtype).pin_memory()
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=variant) as p:
+            p.set_dm_list(cfg.dm_list()).set_output_stride(pitch * es)
+            p.set_batch(2, dev.stride(0), out.stride(0) * es)
+            p.execute(cfg.nsamps, dev, stride, out, code, torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, code)
+        for b in range(2):
+            ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab)
+            for o in (out[b].cpu(), h_out[b]):
+                assert np.array_equal(o[:, :cfg.nsamps].numpy().astype(np.int64), ref)
+                assert bool((o[:, cfg.nsamps:] == -7).all())          # the padding between rows was not written
+
+
+def test_output_row_stride_subband_and_all_killed():
+    cfg = W.CONFIGS[2].reduced(nsamps=1500, ndm=40, nchans=64)
+    dms = cfg.dm_list()
+    nominal, d1, d2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, 16, 16)
+    extent = oracle.subband_required_samples(cfg.nsamps, d1, d2, 16) - cfg.nsamps
+    packed, stride = W.gen_packed(cfg, max(extent, int(_oracle_table(cfg).max())))
+    pitch = cfg.nsamps + 20
+    out = torch.full((cfg.ndm, pitch), -7, dtype=torch.int32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms).set_output_stride(pitch * 4)
+        p.set_subband(16, 16)
+        p.execute(cfg.nsamps, packed[0].cuda(), stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ref = oracle.subband_dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, 16, 16)
+        assert np.array_equal(out[:, :cfg.nsamps].cpu().numpy().view(np.uint32), ref.astype(np.uint32))
+        assert bool((out[:, cfg.nsamps:] == -7).all())
+        p.set_subband(0, 0)
+        p.set_killmask(np.zeros(cfg.nchans, dtype=np.int32))      # every channel killed: zeros, padding untouched
+        out.fill_(-7)
+        p.execute(cfg.nsamps, packed[0].cuda(), stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert bool((out[:, :cfg.nsamps] == 0).all()) and bool((out[:, cfg.nsamps:] == -7).all())
+
+
 def test_execute_host_matches_oracle():
     cfg = W.CONFIGS[4].reduced(nsamps=2 * 640 + 100, ndm=40, nchans=256)
     tab = _oracle_table(cfg)
