@@ -566,3 +566,62 @@ def test_cfg4_full_size_sampled():
 
 def test_cfg5_full_size_sampled_batch():
     _full_size_sampled(W.CONFIGS[5], npoints=2000)
+
+
+def test_cfg2_full_size_subband_32_32_sampled():
+    # the sub-band method at the size bench.py --subband 32,32 times: sampled outputs against the direct sum with
+    # the summed delays delta1 + delta2 (the identity pinned by P13), evaluated one output at a time
+    cfg, sb, grp = W.CONFIGS[2], 32, 32
+    dms = cfg.dm_list()
+    nominal, d1, d2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb, grp)
+    summed = d1[np.arange(cfg.ndm) // grp] + np.repeat(d2, sb, axis=1)            # [ndm][nchans]
+    extent = oracle.subband_required_samples(cfg.nsamps, d1, d2, sb) - cfg.nsamps
+    assert int(summed.max()) <= extent
+    packed_dev, stride = W.gen_packed(cfg, max(extent, int(_oracle_table(cfg).max())), None, device="cuda", chan_chunk=16)
+    out = torch.full((cfg.ndm, cfg.nsamps), -1, dtype=torch.float32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        p.set_subband(sb, grp)
+        assert p.subband_extent == extent
+        p.execute(cfg.nsamps, packed_dev[0], stride, out, 32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert p.launch_info()["last_launches"] == 3
+    d_idx, t_idx = _sample_points(cfg, 3072, 3000, seed=321)
+    ref = oracle.dedisperse_points(lambda c, t: W.values_at(cfg, 0, c, t, None).numpy(), summed, d_idx, t_idx)
+    got = out[torch.as_tensor(d_idx, device="cuda"), torch.as_tensor(t_idx, device="cuda")].cpu().numpy().astype(np.int64)
+    bad = np.nonzero(got != ref)[0]
+    assert bad.size == 0, f"{bad.size}/{ref.size} differ; first d={d_idx[bad[0]]} t={t_idx[bad[0]]} got={got[bad[0]]} ref={ref[bad[0]]}"
+    assert bool((out >= 0).all())                                                  # every element was written
+    del out, packed_dev
+    torch.cuda.empty_cache()
+
+
+def test_cfg2_full_size_scrunched_sampled():
+    # the transform with time-scrunching at the size bench.py --scrunch 16 times: sampled outputs of every level,
+    # D_F[d][t] = sum_c sum_{i<F} A[c][F (t + delay_F[d][c]) + i], one output at a time
+    cfg = W.CONFIGS[2]
+    dms = np.asarray(cfg.dm_list())
+    with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, 16) as s:
+        lv = s.levels
+        assert [l["factor"] for l in lv] == [1, 2, 4, 8, 16]
+        need = s.required_bytes(cfg.nsamps)
+        packed_dev, stride = W.gen_packed(cfg, need * 8 // cfg.nbits - cfg.nsamps, None, device="cuda", chan_chunk=16)
+        outs = [torch.full((l["ndm"], cfg.nsamps // l["factor"]), -1, dtype=torch.float32, device="cuda") for l in lv]
+        s.execute(cfg.nsamps, packed_dev[0], stride, outs, 32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+    rng = np.random.default_rng(99)
+    for l, o in zip(lv, outs):
+        F, ns = l["factor"], cfg.nsamps // l["factor"]
+        tabF = oracle.delay_table(cfg.nchans, cfg.dt * F, cfg.f_top, cfg.df, dms[l["first_dm"]:l["first_dm"] + l["ndm"]])
+        assert int(tabF.max()) == l["max_delay"]
+        d_idx = np.concatenate([rng.integers(0, l["ndm"], 400), [0, l["ndm"] - 1, 0, l["ndm"] - 1]])
+        t_idx = np.concatenate([rng.integers(0, ns, 400), [0, 0, ns - 1, ns - 1]])
+        ref = np.zeros(d_idx.shape[0], dtype=np.int64)
+        for i in range(F):
+            ref += oracle.dedisperse_points(lambda c, t: W.values_at(cfg, 0, c, t, None).numpy(), tabF * F, d_idx, t_idx * F + i)
+        got = o[torch.as_tensor(d_idx, device="cuda"), torch.as_tensor(t_idx, device="cuda")].cpu().numpy().astype(np.int64)
+        bad = np.nonzero(got != ref)[0]
+        assert bad.size == 0, f"factor {F}: {bad.size}/{ref.size} differ; first d={d_idx[bad[0]]} t={t_idx[bad[0]]}"
+        assert bool((o >= 0).all())
+    del outs, packed_dev
+    torch.cuda.empty_cache()
