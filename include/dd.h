@@ -182,6 +182,8 @@ dd_status dd_set_batch(dd_plan plan, int nbeams, int64_t in_beam_stride, int64_t
  * Enqueues on `stream` and returns; does not synchronise and does not allocate (except that the first
  * call after a dd_set_dm_list made without a device uploads the tables).  The caller keeps in/out
  * alive until the stream has passed the enqueued work.  Launch errors are returned as DD_ERR_CUDA.
+ * After one warm-up call with the same arguments (tables uploaded, the bit-plane work buffer grown) a call only
+ * enqueues kernels, so it can be captured into a CUDA graph on `stream` and replayed (dd_scrunch_execute likewise).
  */
 dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
                      int out_nbits, void *stream);

@@ -625,3 +625,53 @@ def test_cfg2_full_size_scrunched_sampled():
         assert bool((o >= 0).all())
     del outs, packed_dev
     torch.cuda.empty_cache()
+
+
+def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
+    # dd_execute neither allocates nor synchronises after its first call, so a warmed-up call can be captured into
+    # a CUDA graph and replayed on new input (launch-bound cases: small transforms, the 14 launches of a scrunch set)
+    cfg = W.CONFIGS[2].reduced(nsamps=5120 + 77, ndm=21, nchans=64)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    cfg_b = W.CONFIGS[2].reduced(nsamps=5120 + 77, ndm=21, nchans=64, nbeams=2)
+    other, _ = W.gen_packed(cfg_b, int(tab.max()), beams=[1])          # a second, different input of the same shape
+    dev = packed[0].cuda()
+    out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.float32, device="cuda")
+    side = torch.cuda.Stream()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(cfg.dm_list())
+        with torch.cuda.stream(side):
+            p.execute(cfg.nsamps, dev, stride, out, 32, side)          # warm-up: tables uploaded, work buffer grown
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            p.execute(cfg.nsamps, dev, stride, out, 32, torch.cuda.current_stream())
+        for src in (packed[0], other[0], packed[0]):
+            dev.copy_(src.cuda())
+            out.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            ref = oracle.dedisperse(src.numpy(), cfg.nbits, cfg.nsamps, tab)
+            assert np.array_equal(out.cpu().numpy(), ref.astype(np.float32))
+    dms = np.array([0.0, 100.0, 300.0, 900.0])
+    with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, 8) as s:
+        lv = s.levels
+        need = s.required_bytes(cfg.nsamps)
+        nsamp_in = need * 8 // cfg.nbits
+        pk, st2 = W.gen_packed(cfg, nsamp_in - cfg.nsamps)
+        dev2 = pk[0].cuda()
+        outs = [torch.zeros((l["ndm"], cfg.nsamps // l["factor"]), dtype=torch.float32, device="cuda") for l in lv]
+        with torch.cuda.stream(side):
+            s.execute(cfg.nsamps, dev2, st2, outs, 32, side)
+        side.synchronize()
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=side):
+            s.execute(cfg.nsamps, dev2, st2, outs, 32, torch.cuda.current_stream())
+        for o in outs:
+            o.zero_()
+        g2.replay()
+        torch.cuda.synchronize()
+        ref = oracle.scrunched_dedisperse(pk[0].numpy(), cfg.nbits, cfg.nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, 8, nsamp_in)
+        assert len(ref) == len(outs) >= 3
+        for o, (F, first, want) in zip(outs, ref):
+            assert np.array_equal(o.cpu().numpy(), want.astype(np.float32)), f"factor {F}"
