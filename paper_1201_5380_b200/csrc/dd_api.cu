@@ -118,7 +118,8 @@ static int elem_size(int out_nbits)
         return 4;
     case DD_OUT_U16:
         return 2;
-    case kOutPlanes:   // internal (sub-band intermediate: bit planes, one byte per sample); rejected at the C ABI
+    case kOutU8:       // internal; check_execute rejects both at the C ABI
+    case kOutPlanes:   // (sub-band intermediate: bit planes, one byte per sample)
         return 1;
     }
     return 0;
@@ -130,7 +131,7 @@ static dd_status check_execute(const dd_plan_s *p, int64_t nsamps, int64_t in_st
     if (p->ndm <= 0)
         return DD_ERR_NO_DM_LIST;
     const int es = elem_size(out_nbits);
-    if (nsamps <= 0 || es == 0 || out_nbits == kOutPlanes)
+    if (nsamps <= 0 || es == 0 || out_nbits == kOutU8 || out_nbits == kOutPlanes)
         return DD_ERR_INVALID_ARG;
     if (in_stride <= 0 || in_stride % 16 != 0)
         return DD_ERR_ALIGNMENT;

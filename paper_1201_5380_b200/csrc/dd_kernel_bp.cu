@@ -338,6 +338,16 @@ __device__ __forceinline__ void store4(const KernelParams &p, uint8_t *orow, int
                 if (t + k < p.nsamps)
                     o[k] = q[k];
         }
+    } else if (p.out_code == kOutU8) {   // internal: the intermediate series of the sub-band method
+        uint8_t *o = orow + t;
+        if (whole) {
+            *reinterpret_cast<uint32_t *>(o) = q[0] | (q[1] << 8) | (q[2] << 16) | (q[3] << 24);
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (t + k < p.nsamps)
+                    o[k] = static_cast<uint8_t>(q[k]);
+        }
     } else {
         uint16_t *o = reinterpret_cast<uint16_t *>(orow) + t;
         if (whole) {
@@ -356,7 +366,7 @@ __device__ __forceinline__ void store4(const KernelParams &p, uint8_t *orow, int
 // the warp reads the patch back so that consecutive lanes hold consecutive chunks of the SAME unit and stores:
 // every STG.128 covers whole 128-byte lines (4 units of float32) instead of 32 scattered 16-byte pieces.
 // The chunk index is XOR-swizzled so that both the write and the read phase are free of bank conflicts.
-//   ES     bytes per output element (4, 2);  F32: convert to float32
+//   ES     bytes per output element (4, 2, 1);  F32: convert to float32
 //   gunit  address of this unit of lane 0;  lane s's unit is s * lane_pitch bytes further
 template <int ES, bool F32>
 __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], uint8_t *patch, int lane, uint8_t *gunit,
@@ -374,10 +384,15 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
                                __float_as_uint(__uint2float_rn(q[4 * c + 2])), __float_as_uint(__uint2float_rn(q[4 * c + 3])));
             else
                 v = make_uint4(q[4 * c], q[4 * c + 1], q[4 * c + 2], q[4 * c + 3]);
-        } else {
-            static_assert(ES == 2, "element sizes: 4 or 2 bytes");
+        } else if constexpr (ES == 2) {
             v = make_uint4(q[8 * c] | (q[8 * c + 1] << 16), q[8 * c + 2] | (q[8 * c + 3] << 16),
                            q[8 * c + 4] | (q[8 * c + 5] << 16), q[8 * c + 6] | (q[8 * c + 7] << 16));
+        } else {
+            uint32_t w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                w[k] = q[16 * c + 4 * k] | (q[16 * c + 4 * k + 1] << 8) | (q[16 * c + 4 * k + 2] << 16) | (q[16 * c + 4 * k + 3] << 24);
+            v = make_uint4(w[0], w[1], w[2], w[3]);
         }
         *reinterpret_cast<uint4 *>(patch + lane * (CH * 16) + ((c ^ swz) * 16)) = v;
     }
@@ -395,8 +410,8 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
 // Bp<NBITS>::FL stages (the plan pads the channel list to whole groups of FL stages), and for 8-bit input the
 // epilogue stores straight from registers (a deeper stage ring is worth more than coalesced stores there).
 // Otherwise: a flush after every stage, and the epilogue goes through per-warp shared-memory patches.
-// PIN < NBITS: only the low PIN planes of a sample can be set (sub-band step 2: the plan knows the largest sample of the
-// intermediate series; scrunched series: dd_set_input_max), the others are neither shifted nor added.
+// PIN < NBITS (short instantiation, 8-bit input): only the low PIN planes of a sample can be set (the plan knows the
+// largest sample of the sub-band intermediate), the others are neither shifted nor added.
 template <int NBITS, bool LONG, int PIN = NBITS>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
@@ -623,7 +638,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int d = blk * DB + warp;
     if (d >= p.ndm)
         return;
-    const int esize = (p.out_code == DD_OUT_U16) ? 2 : 4;
+    const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
     uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.out_dm_stride;
     const bool interior = PATCH && p.vec16_ok && (t0 + TB <= p.nsamps);   // 16-byte stores: rows must be 16-byte aligned
     uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
@@ -653,8 +668,10 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                 store_unit_coalesced<4, true>(q, patch, lane, gunit, W * 32 * 4);
             else if (p.out_code == DD_OUT_U32)
                 store_unit_coalesced<4, false>(q, patch, lane, gunit, W * 32 * 4);
-            else
+            else if (p.out_code == DD_OUT_U16)
                 store_unit_coalesced<2, false>(q, patch, lane, gunit, W * 32 * 2);
+            else
+                store_unit_coalesced<1, false>(q, patch, lane, gunit, W * 32);
         } else {
             const int64_t tunit = t0 + 32 * (W * lane + j);
 #pragma unroll

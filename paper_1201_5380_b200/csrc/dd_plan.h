@@ -135,6 +135,7 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
 
 constexpr int64_t kMaxDynSmem = 227 * 1024;   // usable shared memory per CTA on sm_100a
 constexpr int kBpPatchBytes = 4096;             // bit-plane kernel epilogue: shared memory per warp (32 lanes x 128 B)
+constexpr int kOutU8 = 8;                     // internal output code: uint8 sums, not in the C ABI
 constexpr int kOutPlanes = 9;                 // internal output code: the low 8 bit planes of the sums, written in the layout the
                                               // 8-bit bit-plane kernel stages (sub-band intermediate: step 2 needs no pre-pass)
 
