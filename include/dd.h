@@ -138,8 +138,7 @@ dd_status dd_set_input_max(dd_plan plan, int vmax);
  * Takes effect at once when a DM list is present (else at dd_set_dm_list); on error the plan is unchanged.  Honours
  * the kill mask and dd_set_batch.  dd_execute then needs input rows of nsamps + dd_get_subband_extent() samples,
  * allocates its temporary buffers on first use, and launches three kernels (bit-plane transpose of the input,
- * step 1 writing S as bit planes, step 2).  dd_execute_host returns
- * DD_ERR_INVALID_ARG while the sub-band method is selected.
+ * step 1 writing S as bit planes, step 2).  dd_execute_host runs the method on its staged copy as one time slab.
  */
 dd_status dd_set_subband(dd_plan plan, int sb_nchans, int dm_group);
 

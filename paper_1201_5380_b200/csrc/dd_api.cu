@@ -202,8 +202,10 @@ static KernelParams make_params(const dd_plan_s *p, int64_t nsamps, const void *
 // ARE the 8-bit series S[beam][sub-band][nominal DM][t], t < nsamps + largest step-2 delay, in the layout step 2
 // stages -- so that neither an output transpose, nor a byte buffer, nor a second pre-pass is needed; step 2
 // dedisperses, for every group of trials, the miniature filterbank of its nominal DM.  Three kernels.
+// dense_out: the output is a dense device slab [beam][d][nsamps] (the staging of dd_execute_host) instead of the
+// caller's strides.
 static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
-                                 int out_nbits, cudaStream_t st_)
+                                 int out_nbits, cudaStream_t st_, bool dense_out = false)
 {
     dd_plan_s *s1 = plan->s1, *s2 = plan->s2;
     if (!s1 || !s2)
@@ -218,8 +220,10 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
     const int64_t t1 = (nsamps + plan->sb_max_d2 + 31) / 32 * 32;
     cudaError_t e;
     // step 2's launch geometry first: N_SB channels; DM block blk reads the rows of nominal DM blk / (dm_group / 16)
-    const int64_t out_beam = nbeams > 1 ? plan->out_beam_stride : 0;
-    KernelParams k2 = make_params(s2, nsamps, nullptr, 16, out_ptr, out_nbits, nbeams, 0, out_beam, plan->out_dm_stride);
+    const int64_t out_beam = dense_out ? static_cast<int64_t>(plan->ndm) * nsamps * elem_size(out_nbits)
+                                       : (nbeams > 1 ? plan->out_beam_stride : 0);
+    KernelParams k2 = make_params(s2, nsamps, nullptr, 16, out_ptr, out_nbits, nbeams, 0, out_beam,
+                                  dense_out ? 0 : plan->out_dm_stride);
     k2.nrows = nsb * ngrp;
     k2.row_mul = ngrp;
     k2.in_blk_div = plan->dm_group / s2->var.DB;
@@ -599,8 +603,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     if (st != DD_OK)
         return st;
     const int es = elem_size(out_nbits);
-    if (plan->sb_nchans > 0)
-        return DD_ERR_INVALID_ARG;   // the sub-band method is offered on device buffers only (dd.h)
+    if (plan->sb_nchans > 0 && in_stride * 8 < (nsamps + plan->sb_extent) * plan->nbits)
+        return DD_ERR_STRIDE_TOO_SMALL;   // the two steps read sb_extent samples beyond nsamps
     const int64_t row_pitch = plan->out_dm_stride > 0 ? plan->out_dm_stride : nsamps * es;   // host rows (dd_set_output_stride)
     if (row_pitch % es != 0)
         return DD_ERR_ALIGNMENT;
@@ -632,8 +636,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     // length is a multiple of the tile so that slab starts stay 16-byte aligned in the packed rows.
     const int64_t TB = plan->var.TB;
     int64_t slab = ((int64_t(1) << 17) + TB - 1) / TB * TB;
-    if (slab > (nsamps + TB - 1) / TB * TB)
-        slab = (nsamps + TB - 1) / TB * TB;
+    if (slab > (nsamps + TB - 1) / TB * TB || plan->sb_nchans > 0)   // the sub-band method runs as one slab (its
+        slab = (nsamps + TB - 1) / TB * TB;                          // intermediate series span the whole call)
     const int64_t nslabs = (nsamps + slab - 1) / slab;
     const size_t in_bytes = static_cast<size_t>(in_beam) * nbeams;
     const size_t out_slab_bytes = static_cast<size_t>(nbeams) * plan->ndm * slab * es;
@@ -690,12 +694,22 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
         if (k >= 2)
             cudaStreamWaitEvent(S->compute, S->drained[b], 0);   // slab buffer b has been copied out
         const uint8_t *in_slab = S->d_in + (s0 * plan->nbits) / 8;
-        KernelParams kp = make_params(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, nbeams, in_beam,
-                                      static_cast<int64_t>(plan->ndm) * len * es);
-        kp.in_row_bytes = in_stride - (s0 * plan->nbits) / 8;
-        if ((e = launch_direct(plan, kp, S->compute)) != cudaSuccess)
-            return cuda_fail(e, "dd_execute_host launch");
-        launches += launches_per_execute(plan);
+        if (plan->sb_nchans > 0) {   // PAPER.md:317-321 on the staged copy (one slab)
+            const int64_t keep_beam = plan->in_beam_stride;
+            plan->in_beam_stride = in_beam;
+            const dd_status sst = execute_subband(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, S->compute, true);
+            plan->in_beam_stride = keep_beam;
+            if (sst != DD_OK)
+                return sst;
+            launches += plan->last_launches;
+        } else {
+            KernelParams kp = make_params(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, nbeams, in_beam,
+                                          static_cast<int64_t>(plan->ndm) * len * es);
+            kp.in_row_bytes = in_stride - (s0 * plan->nbits) / 8;
+            if ((e = launch_direct(plan, kp, S->compute)) != cudaSuccess)
+                return cuda_fail(e, "dd_execute_host launch");
+            launches += launches_per_execute(plan);
+        }
         cudaEventRecord(S->done[b], S->compute);
         cudaStreamWaitEvent(S->copy_out[b], S->done[b], 0);
         for (int beam = 0; beam < nbeams; ++beam) {

@@ -191,7 +191,10 @@ def test_subband_host_side():
         # the direct delay table is untouched, and rows shorter than nsamps + extent are refused
         assert np.array_equal(p.delay_table().astype(np.int64),
                               oracle.delay_table(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms))
-        assert L.dd_execute_host(h, 100, 16, 4096, 16, 32) == -2
+        ext = max(p.subband_extent, p.max_delay)
+        short = ((100 + ext) * 2 // 8) // 16 * 16          # 2-bit rows a few samples short of nsamps + extent
+        assert L.dd_execute_host(h, 100, 16, short, 16, 32) == -5
+        assert L.dd_execute(h, 100, 16, short, 16, 32, None) == -5
         p.set_subband(0, 0)
         assert L.dd_get_subband_extent(h) == -2
 

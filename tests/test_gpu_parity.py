@@ -271,6 +271,10 @@ def test_subband_method_matches_the_two_step_oracle(case, gpc, monkeypatch):
             ref = oracle.subband_dedisperse(packed[b].numpy(), cfg.nbits, nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df,
                                             dms, sb, grp, mask=mask)
             assert np.array_equal(got[b], ref), f"beam {b}"
+        if gpc == 0:      # the same through the host-buffer path (one time slab on the staged copy)
+            h_out = torch.full((nbeams, ndm, nsamps), -1, dtype=torch.int32).pin_memory()
+            p.execute_host(nsamps, packed.contiguous().pin_memory(), stride, h_out, -32)
+            assert np.array_equal(h_out.numpy().view(np.uint32), got)
         if sb == 1:       # and that IS the direct transform
             assert np.array_equal(got[0], oracle.dedisperse(packed[0].numpy(), cfg.nbits, nsamps, _oracle_table(cfg)))
         # back to the direct transform on the same plan
