@@ -232,6 +232,7 @@ dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int
  *
  * dd_scrunch_create: dm_list HOST, non-decreasing (DD_ERR_INVALID_ARG otherwise), ndm > 0; max_factor a power of two
  *   >= 1 (1 = no scrunching: one level, the plain transform).  The set owns one plan per level.
+ * dd_scrunch_set_killmask: the channel kill mask of dd_set_killmask applied to every level; NULL removes it.
  * dd_scrunch_levels: number of levels (>= 1), or a negative status.
  * dd_scrunch_level_info: HOST out, 6 int64: [0] factor F, [1] index of the level's first trial in dm_list,
  *   [2] trials in the level, [3] largest delay in samples of dt*F, [4] bits per sample of A_F, [5] DM_diag * 1e6 rounded.
@@ -246,6 +247,7 @@ dd_status dd_time_scrunch(int nrows, int64_t nsamps_out, const void *in_ptr, int
 typedef struct dd_scrunch_s *dd_scrunch;
 dd_status dd_scrunch_create(dd_scrunch *set, int nchans, double dt, double f_top, double df, int nbits,
                             const double *dm_list, int ndm, int max_factor);
+dd_status dd_scrunch_set_killmask(dd_scrunch set, const int32_t *mask);
 int dd_scrunch_levels(dd_scrunch set);
 dd_status dd_scrunch_level_info(dd_scrunch set, int level, int64_t *info);
 int64_t dd_scrunch_required_bytes(dd_scrunch set, int64_t nsamps);

@@ -139,11 +139,11 @@ def time_scrunch(packed: np.ndarray, nbits_in: int, nsamps_out: int) -> np.ndarr
 
 
 def scrunched_dedisperse(packed: np.ndarray, nbits: int, nsamps: int, nchans: int, dt: float, f_top: float, df: float,
-                         dm_list, max_factor: int, nsamp_in: int):
+                         dm_list, max_factor: int, nsamp_in: int, mask=None):
     """Direct transform with time-scrunching of packed rows holding nsamp_in samples:
     list of (factor, first trial, int64 sums [ndm_F][nsamps // factor]).  Readings T1-T4 (DESIGN.md section 11)."""
     return scrunched_dedisperse_np(unpack(packed, nbits, nsamp_in), nsamps, nchans, dt, f_top, df, dm_list, max_factor,
-                                   (1 << nbits) - 1)
+                                   (1 << nbits) - 1, mask=mask)
 
 
 def cast_out(sums: np.ndarray, kind: str) -> np.ndarray:

@@ -187,11 +187,12 @@ def scrunch_factors_np(dm_list, dm_diag: float, max_factor: int, vmax: int) -> n
 
 
 def scrunched_dedisperse_np(a: np.ndarray, nsamps: int, nchans: int, dt: float, f_top: float, df: float, dm_list,
-                            max_factor: int, vmax: int):
+                            max_factor: int, vmax: int, mask=None):
     """The direct transform with time-scrunching, step by step in the paper's order: for every
     factor F in use, the series at resolution F dt is made by adding adjacent pairs log2 F times; the trials of
     that factor are dedispersed with eq. 3-5 evaluated for the sampling interval F dt (reading T4), nsamps // F
-    output samples each.  a: unpacked samples [nchans][>= needed].  -> list of (F, first trial, int64 [ndm_F][nsamps//F])."""
+    output samples each.  a: unpacked samples [nchans][>= needed]; mask: optional kill mask (0/1 per channel).
+    -> list of (F, first trial, int64 [ndm_F][nsamps//F])."""
     dms = np.asarray(dm_list, dtype=np.float64)
     fac = scrunch_factors_np(dms, diagonal_dm_np(nchans, dt, f_top, df), max_factor, vmax)
     series = np.asarray(a).astype(np.int64)
@@ -208,6 +209,6 @@ def scrunched_dedisperse_np(a: np.ndarray, nsamps: int, nchans: int, dt: float, 
         for i in range(len(idx)):
             for c in range(nchans):
                 d = int(delays[i, c])
-                res[i] += series[c, d:d + ns]
+                res[i] += series[c, d:d + ns] * (1 if mask is None else int(mask[c] != 0))
         out.append((F, int(idx[0]), res))
     return out

@@ -22,7 +22,7 @@ __all__ = [
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
-    "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
+    "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
@@ -35,7 +35,7 @@ EXPORTED_SYMBOLS = (
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
-    "dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
+    "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy",
 )
 
@@ -101,12 +101,14 @@ def lib() -> ctypes.CDLL:
         L.dd_profile_read.argtypes = [vp, ctypes.POINTER(i32), vp, vp]
         L.dd_scrunch_create.argtypes = [ctypes.POINTER(vp), i32, dbl, dbl, dbl, i32, vp, i32, i32]
         L.dd_scrunch_levels.argtypes = [vp]
+        L.dd_scrunch_set_killmask.argtypes = [vp, vp]
+        L.dd_scrunch_set_killmask.restype = i32
         L.dd_scrunch_level_info.argtypes = [vp, i32, vp]
         L.dd_scrunch_required_bytes.argtypes = [vp, i64]
         L.dd_scrunch_required_bytes.restype = i64
         L.dd_scrunch_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_scrunch_destroy.argtypes = [vp]
-        for name in ("dd_scrunch_create", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_execute", "dd_scrunch_destroy"):
+        for name in ("dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_execute", "dd_scrunch_destroy"):
             getattr(L, name).restype = i32
         L.dd_strerror.argtypes = [i32]
         L.dd_strerror.restype = ctypes.c_char_p
@@ -293,6 +295,15 @@ def dd_scrunch_create(nchans: int, dt: float, f_top: float, df: float, nbits: in
     return int(h.value)
 
 
+def dd_scrunch_set_killmask(sset: int, mask) -> None:
+    """Kill mask for every level of the set; None removes it."""
+    if mask is None:
+        _check(lib().dd_scrunch_set_killmask(sset, None), "dd_scrunch_set_killmask")
+        return
+    m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.int32)
+    _check(lib().dd_scrunch_set_killmask(sset, ctypes.c_void_p(m.ctypes.data)), "dd_scrunch_set_killmask")
+
+
 def dd_scrunch_levels(sset: int) -> int:
     return _check(int(lib().dd_scrunch_levels(sset)), "dd_scrunch_levels")
 
@@ -330,6 +341,10 @@ class ScrunchSet:
     @property
     def levels(self):
         return [dd_scrunch_level_info(self.handle, l) for l in range(dd_scrunch_levels(self.handle))]
+
+    def set_killmask(self, mask) -> "ScrunchSet":
+        dd_scrunch_set_killmask(self.handle, mask)
+        return self
 
     def required_bytes(self, nsamps: int) -> int:
         return dd_scrunch_required_bytes(self.handle, nsamps)

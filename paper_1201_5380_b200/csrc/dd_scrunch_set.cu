@@ -162,6 +162,18 @@ dd_status dd_scrunch_create(dd_scrunch *set, int nchans, double dt, double f_top
     return DD_OK;
 }
 
+dd_status dd_scrunch_set_killmask(dd_scrunch set, const int32_t *mask)
+{
+    if (!set)
+        return DD_ERR_NULL;
+    for (Level &l : set->levels) {   // the same channels are left out at every resolution
+        const dd_status st = dd_set_killmask(l.plan, mask);
+        if (st != DD_OK)
+            return st;
+    }
+    return DD_OK;
+}
+
 int dd_scrunch_levels(dd_scrunch set) { return set ? static_cast<int>(set->levels.size()) : DD_ERR_NULL; }
 
 dd_status dd_scrunch_level_info(dd_scrunch set, int level, int64_t *info)

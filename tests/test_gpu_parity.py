@@ -354,6 +354,14 @@ def test_scrunched_transform_matches_the_oracle_level_by_level(case):
             assert np.array_equal(o.cpu().numpy(), want.astype(np.float32))
         with pytest.raises(dd.DDError):                    # rows shorter than the set needs
             s.execute(nsamps, dev, 16, outs, -32, None)
+        mask = (np.arange(cfg.nchans) % 6 != 4).astype(np.int32)         # kill mask at every level
+        s.set_killmask(mask)
+        s.execute(nsamps, dev, stride, outs, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ref_m = oracle.scrunched_dedisperse(packed[0].numpy(), cfg.nbits, nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df,
+                                            dms, max_factor, nsamp_in, mask=mask)
+        for o, (F, first, want) in zip(outs, ref_m):
+            assert np.array_equal(o.cpu().numpy().view(np.uint32), want.astype(np.uint32)), f"masked, factor {F}"
 
 
 @pytest.mark.parametrize("case", [(8, 160, 24), (8, 160, 48), (8, 136, 100), (8, 40, 30), (8, 40, 200), (4, 528, 6), (4, 48, 5)])

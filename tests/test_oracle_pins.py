@@ -503,6 +503,12 @@ def test_p15_levels_equal_the_full_resolution_loop_summed_over_f_outputs(nbits):
         dF = oracle.delay_table(nchans, base.dt * F, base.f_top, base.df, dms[idx])
         full = oracle.dedisperse_unpacked(a, (nsamps // F) * F, dF * F)
         assert np.array_equal(res, full.reshape(len(idx), nsamps // F, F).sum(axis=2))
+    # kill mask: the masked transform is the transform of the input with the killed rows zeroed
+    mask = (np.arange(nchans) % 5 != 2).astype(np.int32)
+    masked = oracle.scrunched_dedisperse_np(a, nsamps, nchans, base.dt, base.f_top, base.df, dms, 64, (1 << nbits) - 1, mask=mask)
+    zeroed = oracle.scrunched_dedisperse_np(a * mask[:, None], nsamps, nchans, base.dt, base.f_top, base.df, dms, 64, (1 << nbits) - 1)
+    assert all(np.array_equal(m[2], z[2]) and m[0] == z[0] for m, z in zip(masked, zeroed)) and len(masked) == len(levels)
+    assert not np.array_equal(masked[0][2], levels[0][2])
     # max_factor = 1: one level, the plain transform
     one = oracle.scrunched_dedisperse_np(a, nsamps, nchans, base.dt, base.f_top, base.df, dms[:5], 1, (1 << nbits) - 1)
     assert len(one) == 1 and one[0][0] == 1
