@@ -101,7 +101,8 @@ def info_after(plan) -> int:
     return int(plan.launch_info()["last_launches"])
 
 
-KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp<{nbits}>"}
+KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp<{nbits}>",
+                4: "dd_direct_bp<pair rows of {nbits}-bit input>"}
 
 
 def measured_peaks() -> dict:
@@ -252,7 +253,7 @@ def run_ours(args) -> None:
     nbeams = cfg.nbeams
     stream = torch.cuda.Stream()
 
-    plan = dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits).set_dm_list(cfg.dm_list())
+    plan = dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=args.variant).set_dm_list(cfg.dm_list())
     max_delay = plan.max_delay
     subband = None
     if args.subband:        # the approximate sub-band method instead of the direct transform
@@ -403,6 +404,7 @@ def main() -> None:
                     "nominal DM) instead of the direct transform; implies --no-e2e")
     ap.add_argument("--scrunch", type=int, default=0, help="MAXF: time the transform with time-scrunching up to this "
                     "factor (a power of two) instead -- a side measurement")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant (dd_set_kernel_variant); 0 = the library's choice")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")
     ap.add_argument("--cpu-nsamps", type=int, default=1 << 18, help="output samples of the bounded oracle sample")

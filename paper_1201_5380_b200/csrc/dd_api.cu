@@ -62,7 +62,9 @@ static void free_device_tables(dd_plan_s *p)
         cudaFree(p->d_rel);
     if (p->d_zero)
         cudaFree(p->d_zero);
-    p->d_span = p->d_rel = p->d_zero = nullptr;
+    if (p->d_prow)
+        cudaFree(p->d_prow);
+    p->d_span = p->d_rel = p->d_zero = p->d_prow = nullptr;
     p->uploaded = false;
 }
 
@@ -96,6 +98,14 @@ static dd_status upload_tables(dd_plan_s *p)
         (e = cudaMemcpy(p->d_rel, p->rel.data(), rel_bytes, cudaMemcpyHostToDevice)) != cudaSuccess) {
         free_device_tables(p);
         return cuda_fail(e, "cudaMemcpy(tables)");
+    }
+    if (p->pairs && !p->prow.empty()) {   // variant 4: {c0, c1, delta, 0} of every pair row
+        const size_t pb = p->prow.size() * sizeof(int32_t);
+        if ((e = cudaMalloc(&p->d_prow, pb)) != cudaSuccess ||
+            (e = cudaMemcpy(p->d_prow, p->prow.data(), pb, cudaMemcpyHostToDevice)) != cudaSuccess) {
+            free_device_tables(p);
+            return cuda_fail(e, "cudaMalloc/Memcpy(pair rows)");
+        }
     }
     p->uploaded = true;
     return DD_OK;
@@ -341,6 +351,12 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->final32 = scratch.final32;
     plan->span.swap(scratch.span);
     plan->rel.swap(scratch.rel);
+    plan->pairs = scratch.pairs;
+    plan->pair_nbits = scratch.pair_nbits;
+    plan->pair_planes = scratch.pair_planes;
+    plan->rows_per_chunk = scratch.rows_per_chunk;
+    plan->prow.swap(scratch.prow);
+    plan->n_prows = scratch.n_prows;
     plan->last_launches = 0;
     // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
     int ndev = 0;
@@ -393,6 +409,8 @@ dd_status dd_plan_destroy(dd_plan plan)
     free_device_tables(plan);
     if (plan->d_work)
         cudaFree(plan->d_work);
+    if (plan->d_pairwork)
+        cudaFree(plan->d_pairwork);
     if (plan->d_tmp)
         cudaFree(plan->d_tmp);
     destroy_subplan(plan->s1);
@@ -784,7 +802,7 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)
         return DD_ERR_NULL;
-    if (variant < 0 || variant > 3)
+    if (variant < 0 || variant > 4)
         return DD_ERR_INVALID_ARG;
     plan->force_variant = variant;
     return DD_OK;

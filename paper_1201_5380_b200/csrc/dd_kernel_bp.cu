@@ -412,7 +412,10 @@ __device__ __forceinline__ void store_unit_coalesced(const uint32_t (&q)[32], ui
 // Otherwise: a flush after every stage, and the epilogue goes through per-warp shared-memory patches.
 // PIN < NBITS (short instantiation, 8-bit input): only the low PIN planes of a sample can be set (the plan knows the
 // largest sample of the sub-band intermediate), the others are neither shifted nor added.
-template <int NBITS, bool LONG, int PIN = NBITS>
+// PAIRS (variant 4): the "channels" are pairs of channels; a stage holds, besides the offset entries of its CC pairs,
+// the p.rows_per_chunk pair rows those pairs need for the delay differences of this DM block (span list
+// [blk][chunk][rows_per_chunk]); every DM slot's offset entry points into the row of its own difference.
+template <int NBITS, bool LONG, int PIN = NBITS, bool PAIRS = false>
 __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelParams p)
 {
     using C = Bp<NBITS>;
@@ -424,10 +427,10 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     static_assert(PIN >= 1 && PIN <= NBITS, "planes in use");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
     constexpr int FL = LONG ? C::FL : 1;
-    constexpr bool PATCH = !LONG || NBITS < 8;
+    constexpr bool PATCH = !LONG || (NBITS < 8 && !PAIRS);   // pair rows: the ring needs the shared memory more
     constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;        // largest value one stage adds to a counter
     constexpr int NT = bit_length(FL * STAGE_SUM);                   // pending slots
-    static_assert((CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
+    static_assert(PAIRS || (CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
 
     extern __shared__ __align__(128) uint8_t smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -459,7 +462,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);      // [NS]
     uint64_t *empty = full + 8;                                 // [NS]
     const int rel_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * DB * 8));
-    const int raw_stage = static_cast<int>(align128(static_cast<int64_t>(CC) * p.raw_slot));
+    const int raw_stage = static_cast<int>(align128(static_cast<int64_t>(PAIRS ? p.rows_per_chunk : CC) * p.raw_slot));
     uint8_t *rel_base = smem + 128 + (PATCH ? BP_NWARPS * kBpPatchBytes : 0);   // after the warps' output patches
     uint8_t *raw_base = rel_base + NS * rel_stage;
 
@@ -476,18 +479,26 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                              (p.in_blk_div > 0 ? static_cast<int64_t>(blk / p.in_blk_div) * p.in_blk_stride : 0);
     const uint8_t *in_tile = in_beam + (t0 >> 5) * UB;   // this tile's first unit in every sub-row
     const int64_t col0 = static_cast<int64_t>(blk) * p.nchans_pad + static_cast<int64_t>(group) * p.group_cols;
-    const int4 *span_blk = p.span + col0;
+    const int4 *span_blk = PAIRS ? p.span + static_cast<int64_t>(blk) * p.nchunks * p.rows_per_chunk : p.span + col0;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + col0 * DB;
 
     // producers: EVERY warp stages CPW = CC * NSUB / NWARPS sub-rows of each chunk (its lane 0 issues the bulk
     // copies: a bulk copy takes its operands from uniform registers, so one warp issuing all copies of a chunk
     // serialises over its lanes and falls behind the others); warp 0 also stages the chunk's offset entries.
     // The span metadata of the next chunk to stage is fetched one step early.
-    constexpr int CPW = CC * NSUB / BP_NWARPS;
+    constexpr int CPW = PAIRS ? 3 : CC * NSUB / BP_NWARPS;   // PAIRS: rows per warp and stage (the plan keeps rows_per_chunk <= 48)
     auto load_meta = [&](int chunk, int4 (&m)[CPW]) {
 #pragma unroll
-        for (int k = 0; k < CPW; ++k)
-            m[k] = (lane == 0 && chunk < nchunks_cta()) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
+        for (int k = 0; k < CPW; ++k) {
+            if constexpr (PAIRS) {
+                const int slot = warp + BP_NWARPS * k;
+                m[k] = (lane == 0 && chunk < nchunks_cta() && slot < p.rows_per_chunk)
+                           ? __ldg(&span_blk[static_cast<int64_t>(chunk) * p.rows_per_chunk + slot])
+                           : make_int4(0, 0, 0, 0);
+            } else {
+                m[k] = (lane == 0 && chunk < nchunks_cta()) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
+            }
+        }
     };
     // chunk = round * NS + s: the ring position is carried along instead of divided out (NS is a run-time value)
     int prod_s = 0, prod_round = 0;
@@ -501,10 +512,23 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             uint32_t tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
 #pragma unroll
             for (int k = 0; k < CPW; ++k)
-                tx += static_cast<uint32_t>(m[k].y);
+                tx += static_cast<uint32_t>(m[k].y) * (PAIRS ? NSUB : 1);
             mbar_arrive_expect_tx(&full[s], tx);
+            if constexpr (PAIRS) {
 #pragma unroll
-            for (int k = 0; k < CPW; ++k) {
+                for (int k = 0; k < CPW; ++k) {
+                    if (m[k].y > 0) {
+                        const int slot = warp + BP_NWARPS * k;
+#pragma unroll
+                        for (int sub = 0; sub < NSUB; ++sub)
+                            tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
+                                         in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x,
+                                         static_cast<uint32_t>(m[k].y), &full[s]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < (PAIRS ? 0 : CPW); ++k) {
                 const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
                 const uint8_t *src = in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x;
                 tma_bulk_g2s(raw_base + s * raw_stage + cl * p.raw_slot + sub * p.sub_slot, src, static_cast<uint32_t>(m[k].y),
@@ -783,6 +807,143 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------ pair rows (variant 4)
+// S[t] = x[c0][t] + x[c1][t + delta] in bit planes, for every pair row {c0, c1, delta}: NBITS planes + NBITS planes ->
+// NBITS + 1 planes by a ripple of full adders (xor3 / maj3), written in the layout of the consumer kernel
+// (4 planes per unit and sub-row).  One thread per (row, unit).  in: bit-plane rows of the input [c][unit][NBITS
+// planes], in_units units per row, zero beyond the input; a killed partner (c1 < 0) contributes nothing.
+template <int NBITS>
+__global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restrict__ in, int64_t in_row_words, int64_t in_units,
+                                                         const int4 *__restrict__ prow, uint32_t *__restrict__ out,
+                                                         int64_t out_sub_words, int64_t out_units, int64_t ublocks)
+{
+    constexpr int NSUBO = NBITS == 2 ? 1 : 2;
+    const int64_t blk = blockIdx.x;
+    const int64_t r = blk / ublocks, u = (blk - r * ublocks) * blockDim.x + threadIdx.x;
+    if (u >= out_units)
+        return;
+    const int4 pr = __ldg(&prow[r]);
+    uint32_t a[NBITS], b[NBITS];
+    const uint32_t *ra = in + static_cast<int64_t>(pr.x) * in_row_words + u * NBITS;
+#pragma unroll
+    for (int k = 0; k < NBITS; ++k)
+        a[k] = u < in_units ? ra[k] : 0u;
+    if (pr.y >= 0) {
+        const int64_t ub = u + (pr.z >> 5);
+        const uint32_t sh = static_cast<uint32_t>(pr.z) & 31u;
+        const uint32_t *rb = in + static_cast<int64_t>(pr.y) * in_row_words + ub * NBITS;
+#pragma unroll
+        for (int k = 0; k < NBITS; ++k) {
+            const uint32_t lo = ub < in_units ? rb[k] : 0u, hi = ub + 1 < in_units ? rb[NBITS + k] : 0u;
+            b[k] = __funnelshift_r(lo, hi, sh);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < NBITS; ++k)
+            b[k] = 0u;
+    }
+    uint32_t sum[NBITS + 1], cy = 0u;
+#pragma unroll
+    for (int k = 0; k < NBITS; ++k) {
+        sum[k] = xor3(a[k], b[k], cy);
+        cy = maj3(a[k], b[k], cy);
+    }
+    sum[NBITS] = cy;
+    uint32_t *o = out + r * (NSUBO * out_sub_words) + u * 4;
+    if constexpr (NBITS == 2) {
+        *reinterpret_cast<uint4 *>(o) = make_uint4(sum[0], sum[1], sum[2], 0u);
+    } else {
+        *reinterpret_cast<uint4 *>(o) = make_uint4(sum[0], sum[1], sum[2], sum[3]);
+        *reinterpret_cast<uint4 *>(o + out_sub_words) = make_uint4(sum[4], 0u, 0u, 0u);
+    }
+}
+
+// NBITS: input width (2 or 4); the consumer is the bit-plane kernel of width ENB = 4 or 8 with NBITS + 1 planes in use
+template <int NBITS>
+cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
+{
+    constexpr int ENB = NBITS == 2 ? 4 : 8;
+    using C = Bp<ENB>;
+    constexpr int TB = 32 * 32 * C::W;
+    if (!plan->pairs || plan->pair_nbits != ENB || plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB ||
+        kp_in.ngroups != 1 || !plan->d_prow)
+        return cudaErrorInvalidValue;
+    KernelParams kp = kp_in;
+    int32_t max_delta = 0;
+    for (int64_t r = 0; r < plan->n_prows; ++r)
+        max_delta = plan->prow[4 * r + 2] > max_delta ? plan->prow[4 * r + 2] : max_delta;
+    // pair rows: as long as the longest span of the tiles needs; input bit planes: that plus the largest difference
+    const int64_t out_units = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + 31) / 32;
+    const int64_t conv_o = out_units * 16;
+    const int64_t rows_o = plan->n_prows + 1;                               // + the all-zero row of padded entries
+    const int64_t beam_o = rows_o * C::NSUB * conv_o;
+    const int64_t spg = (16 / (NBITS * 4)) * 32;                            // input samples per 16-byte group
+    const int64_t groups_i = (out_units * 32 + max_delta + 64 + spg - 1) / spg;
+    const int64_t conv_i = groups_i * 16, in_units = conv_i / (NBITS * 4);
+    const int64_t beam_i = static_cast<int64_t>(kp.nrows) * conv_i;
+    cudaError_t e;
+    const size_t need_i = static_cast<size_t>(kp.nbeams) * beam_i, need_o = static_cast<size_t>(kp.nbeams) * beam_o;
+    if (plan->work_bytes < need_i) {
+        if (plan->d_work)
+            cudaFree(plan->d_work);
+        plan->d_work = nullptr;
+        plan->work_bytes = 0;
+        if ((e = cudaMalloc(&plan->d_work, need_i)) != cudaSuccess)
+            return e;
+        plan->work_bytes = need_i;
+    }
+    plan->work_layout[0] = 0;   // the direct launcher must re-establish its zero rows if the plan goes back to it
+    if (plan->pairwork_bytes < need_o) {
+        if (plan->d_pairwork)
+            cudaFree(plan->d_pairwork);
+        plan->d_pairwork = nullptr;
+        plan->pairwork_bytes = 0;
+        if ((e = cudaMalloc(&plan->d_pairwork, need_o)) != cudaSuccess)
+            return e;
+        plan->pairwork_bytes = need_o;
+    }
+    // the zero row of every beam
+    if ((e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_pairwork) + plan->n_prows * C::NSUB * conv_o, static_cast<size_t>(beam_o),
+                               0, static_cast<size_t>(C::NSUB) * conv_o, kp.nbeams, stream)) != cudaSuccess)
+        return e;
+    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups_i + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
+        kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv_i, beam_i,
+        static_cast<int32_t>(groups_i));
+    if ((e = cudaGetLastError()) != cudaSuccess)
+        return e;
+    const int64_t ublocks = (out_units + 255) / 256;
+    if (plan->n_prows * ublocks > 0x7FFFFFFFLL)
+        return cudaErrorInvalidConfiguration;
+    for (int b = 0; b < kp.nbeams; ++b) {
+        dd_make_pair_rows<NBITS><<<dim3(static_cast<unsigned>(plan->n_prows * ublocks)), 256, 0, stream>>>(
+            reinterpret_cast<const uint32_t *>(static_cast<const uint8_t *>(plan->d_work) + b * beam_i), conv_i / 4, in_units,
+            static_cast<const int4 *>(plan->d_prow), reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(plan->d_pairwork) + b * beam_o),
+            conv_o / 4, out_units, ublocks);
+        if ((e = cudaGetLastError()) != cudaSuccess)
+            return e;
+    }
+    if (plan->prof_mid)
+        cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
+    kp.in = static_cast<const uint8_t *>(plan->d_pairwork);
+    kp.in_stride = C::NSUB * conv_o;
+    kp.in_blk_stride = 0;
+    kp.in_row_bytes = conv_o;
+    kp.in_beam_stride = beam_o;
+    kp.gpc = 1;
+    kp.rows_per_chunk = plan->rows_per_chunk;
+    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams;
+    if (ctas <= 0 || ctas > 0x7FFFFFFFLL || kp.out_code == kOutPlanes)
+        return cudaErrorInvalidConfiguration;
+    if (plan->long_mode && kp.nchunks % C::FL != 0)
+        return cudaErrorInvalidValue;
+    auto kernel = plan->long_mode ? dd_direct_bp<ENB, true, NBITS + 1, true> : dd_direct_bp<ENB, false, NBITS + 1, true>;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
+    if (e != cudaSuccess)
+        return e;
+    kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 // Two launches: the bit-plane transpose of the rows the tiles will read, then the dedispersion kernel.
@@ -797,6 +958,17 @@ cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_
         return launch_bp<4>(plan, kp, stream, planes_ready);
     case 8:
         return launch_bp<8>(plan, kp, stream, planes_ready);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_variant4(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
+{
+    switch (plan->nbits) {
+    case 2:
+        return launch_pairs<2>(plan, kp, stream);
+    case 4:
+        return launch_pairs<4>(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }

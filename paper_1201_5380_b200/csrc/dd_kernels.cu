@@ -58,11 +58,14 @@ cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t 
         return launch_variant2(plan, kp, stream);
     case 3:
         return launch_variant3(plan, kp, stream);
+    case 4:
+        return launch_variant4(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }
 
-int launches_per_execute(const dd_plan_s *plan) { return plan->var.bitplane ? 2 : 1; }
+// bit planes: transpose + transform; pair rows: transpose + one row builder per beam + transform
+int launches_per_execute(const dd_plan_s *plan) { return plan->pairs ? 2 + plan->nbeams : (plan->var.bitplane ? 2 : 1); }
 
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
 {

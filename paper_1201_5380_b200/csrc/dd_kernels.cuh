@@ -42,6 +42,7 @@ struct KernelParams {
     int64_t pl_beam;          // bytes between beams
     int32_t pl_units;         // units (32 samples) per sub-row
     int32_t gpc;              // channel groups summed one after the other by a CTA (>= 1; > 1 only with kOutPlanes)
+    int32_t rows_per_chunk;   // pair rows (variant 4): rows staged per stage; span is [nblk][nchunks][rows_per_chunk]
 };
 
 // Geometry of the bit-plane work buffer of a plan for one launch (dd_kernel_bp.cu).
@@ -61,6 +62,9 @@ cudaError_t launch_variant2(const dd_plan_s *plan, const KernelParams &kp, cudaS
 // planes_ready: plan->d_work already holds the bit planes (written by another launch with kOutPlanes after
 // bp_prepare_work): the transpose is skipped.
 cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool planes_ready = false);
+// variant 4 launches three kernels: bit-plane transpose, pair rows (one per delay difference of every channel pair),
+// transform over the pair rows.  May grow plan->d_work and plan->d_pairwork.
+cudaError_t launch_variant4(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 // Sizes (and grows) plan->d_work for the launch described by kp and keeps its all-zero rows; zero_all: the whole
 // buffer is cleared whenever it is new or its layout changed (for a producer that does not write every unit).
 cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w);

@@ -140,7 +140,7 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
     if (p->patch)   // one output patch per warp for the coalescing epilogue (kept apart from the stages,
         bytes += static_cast<int64_t>(v.threads / 32) * kBpPatchBytes;   // so that a warp can store while others still add); Bp<nbits>::PATCH
     bytes += p->nstages * align_up(static_cast<int64_t>(cc) * v.DB * v.rel_bytes, 128);           // offset-table stages
-    bytes += p->nstages * align_up(static_cast<int64_t>(cc) * p->raw_slot, 128);                  // packed / bit-plane stages
+    bytes += p->nstages * align_up(static_cast<int64_t>(p->pairs ? p->rows_per_chunk : cc) * p->raw_slot, 128);   // packed / bit-plane stages (pair rows: rows per stage)
     if (v.lane_bits != p->nbits)                                                                  // unpacked lanes
         bytes += v.lane_stages * align_up(static_cast<int64_t>(cc) * p->lane_slot, 128);
     return bytes;
@@ -168,8 +168,207 @@ static const Variant kVariants[] = {
     {1, 32, 640, 256, 4, 2, 8, 1, 2, {32, 16, 8, 4}, (1 << 2) | (1 << 4) | (1 << 8), 32, false, false, 0, 1},
 };
 
+// Variant 4 -- pair rows.  For two adjacent live channels (c0, c1) the difference delta = delay[d][c1] - delay[d][c0]
+// takes few values over the whole DM list (it grows slowly with DM and the two roundings make it jitter by one), so
+// the row S_delta[t] = x[c0][t] + x[c1][t + delta] is made ONCE per delta by a pre-pass (n + 1 bit planes), and every
+// trial adds the row of its own delta at the delay of c0: n + 1 plane words per pair instead of 2 n.  Exact: the
+// delay table is used as it stands.  The transform kernel is the bit-plane kernel of the next width (2-bit pairs:
+// the 4-plane layout with 3 planes in use; 4-bit pairs: the 2 x 4-plane layout with 5 in use); a stage holds CC
+// pairs and the rows of every delta the DM block needs for them.
+dd_status build_tiles_pairs(dd_plan_s *p)
+{
+    const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    if ((nbits != 2 && nbits != 4) || p->group_size > 0)
+        return DD_ERR_SMEM;
+    std::vector<int32_t> live;
+    for (int c = 0; c < nrows; ++c)
+        if (p->keep.empty() || p->keep[c])
+            live.push_back(c);
+    const int nlive = static_cast<int>(live.size());
+    if (nlive == 0)
+        return DD_ERR_SMEM;
+    const int npairs = (nlive + 1) / 2;
+    const int enb = nbits == 2 ? 4 : 8;                 // consumer layout
+    const Variant *vv = nullptr;
+    for (const Variant &v : kVariants)
+        if (v.id == 3 && (v.nbits_mask & (1 << enb)))
+            vv = &v;
+    if (!vv)
+        return DD_ERR_SMEM;
+    Variant v = *vv;
+    v.id = 4;
+    const int pin = nbits + 1;                          // planes of a pair sum
+    const int64_t top = static_cast<int64_t>(npairs) * ((1 << pin) - 1);   // structural weight the counters take
+    if (top >= (int64_t(1) << v.max_sum_bits))
+        return DD_ERR_SMEM;
+    const int DB = v.DB, cc = v.cc[0];
+    const int fl = kBpFlushStages(enb);
+    const int nblk = (ndm + DB - 1) / DB;
+    const bool long_mode = npairs >= 8 * cc * fl;
+    const int ents_pad = static_cast<int>(align_up(npairs, cc * (long_mode ? fl : 1)));
+    const int nchunks = ents_pad / cc;
+    // pair rows: every delta of every pair, in pair order
+    std::vector<int32_t> prow;
+    std::vector<int64_t> rowbase(npairs + 1, 0);
+    std::vector<std::vector<int32_t>> deltas(npairs);
+    for (int q = 0; q < npairs; ++q) {
+        const int c0 = live[2 * q], c1 = 2 * q + 1 < nlive ? live[2 * q + 1] : -1;
+        std::vector<int32_t> &u = deltas[q];
+        if (c1 < 0) {
+            u.push_back(0);
+        } else {
+            for (int d = 0; d < ndm; ++d)
+                u.push_back(p->delay[static_cast<size_t>(d) * nrows + c1] - p->delay[static_cast<size_t>(d) * nrows + c0]);
+            std::sort(u.begin(), u.end());
+            u.erase(std::unique(u.begin(), u.end()), u.end());
+        }
+        rowbase[q + 1] = rowbase[q] + static_cast<int64_t>(u.size());
+        for (int32_t dl : u) {
+            prow.push_back(c0);
+            prow.push_back(c1);
+            prow.push_back(dl);
+            prow.push_back(0);
+        }
+    }
+    const int64_t n_prows = rowbase[npairs];
+    if (n_prows > (int64_t(1) << 30))
+        return DD_ERR_SMEM;
+    // per (DM block, pair): the rows in use and the staged span (of the pair's first channel)
+    const int A = (16 / v.unit_bytes) * 32;
+    struct Use { int32_t start, nbytes; std::vector<int32_t> rows; };
+    std::vector<Use> use(static_cast<size_t>(nblk) * npairs);
+    int64_t max_bytes = 0, max_end = 0;
+    int rs = 0;
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            int rows_here = 0;
+            for (int e = k * cc; e < std::min((k + 1) * cc, npairs); ++e) {
+                const int c0 = live[2 * e], c1 = 2 * e + 1 < nlive ? live[2 * e + 1] : -1;
+                int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0;
+                Use &u = use[static_cast<size_t>(b) * npairs + e];
+                for (int i = 0; i < DB; ++i) {
+                    const int d = std::min(b * DB + i, ndm - 1);
+                    const int32_t d0 = p->delay[static_cast<size_t>(d) * nrows + c0];
+                    const int32_t dl = c1 < 0 ? 0 : p->delay[static_cast<size_t>(d) * nrows + c1] - d0;
+                    dmin = std::min(dmin, d0);
+                    dmax = std::max(dmax, d0);
+                    const int32_t r = static_cast<int32_t>(
+                        rowbase[e] + (std::lower_bound(deltas[e].begin(), deltas[e].end(), dl) - deltas[e].begin()));
+                    if (std::find(u.rows.begin(), u.rows.end(), r) == u.rows.end())
+                        u.rows.push_back(r);
+                }
+                const int32_t start = dmin / A * A;
+                const int64_t need = static_cast<int64_t>(v.TB) + (dmax - start) + v.tail;
+                const int64_t nbytes = align_up(need, A) / 32 * v.unit_bytes;
+                if (dmax - start > (int64_t(1) << 26) || nbytes > (1 << 19))
+                    return DD_ERR_SMEM;
+                u.start = start;
+                u.nbytes = static_cast<int32_t>(nbytes);
+                max_bytes = std::max(max_bytes, nbytes);
+                max_end = std::max<int64_t>(max_end, start + nbytes / v.unit_bytes * 32);
+                rows_here += static_cast<int>(u.rows.size());
+            }
+            if ((k + 1) * cc > npairs)
+                rows_here += 1;   // the all-zero row behind which the padded entries of this stage hide
+            rs = std::max(rs, rows_here);
+        }
+    }
+    rs = std::max(rs, 1);
+    if (rs > 48)   // the kernel's producers stage at most 3 rows per warp and stage
+        return DD_ERR_SMEM;
+    p->var = v;
+    p->pairs = true;
+    p->pair_nbits = enb;
+    p->pair_planes = pin;
+    p->long_mode = long_mode;
+    p->patch = !long_mode;   // long: no output patches, a deeper ring instead (must match PATCH in dd_kernel_bp.cu)
+    p->max_span_end = max_end;
+    p->sub_slot = static_cast<int>(max_bytes);
+    p->raw_slot = static_cast<int>(max_bytes) * v.nsub;
+    p->lane_slot = p->raw_slot;
+    p->rows_per_chunk = rs;
+    p->cc = cc;
+    int nst = 0;
+    for (int n = v.raw_stages; n >= 2 && nst == 0; --n) {
+        p->nstages = n;
+        const int64_t tx = static_cast<int64_t>(rs) * p->raw_slot + static_cast<int64_t>(cc) * DB * v.rel_bytes;
+        if (smem_layout_bytes(p, cc) <= kMaxDynSmem && tx < (1 << 20))
+            nst = n;
+    }
+    if (nst == 0) {
+        p->pairs = false;
+        return DD_ERR_SMEM;
+    }
+    p->nstages = nst;
+    // span list [nblk][nchunks][rs] and offsets [nblk][ents_pad][DB]
+    std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchunks * rs);
+    std::vector<uint8_t> rel(static_cast<size_t>(nblk) * ents_pad * DB * 8);
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            SpanMeta *sl = span.data() + (static_cast<size_t>(b) * nchunks + k) * rs;
+            int slot = 0;
+            for (int j = 0; j < rs; ++j)
+                sl[j] = SpanMeta{0, 0, 0, 0};
+            int zero_slot = -1;   // a stage with padded entries also stages the all-zero row (row n_prows)
+            for (int e = k * cc; e < (k + 1) * cc; ++e) {
+                const size_t base = (static_cast<size_t>(b) * ents_pad + e) * DB;
+                if (e >= npairs) {   // padded entry: every window at the start of the zero row's slot
+                    if (zero_slot < 0) {
+                        zero_slot = slot;
+                        sl[slot] = SpanMeta{0, p->sub_slot, static_cast<int32_t>(n_prows), 0};
+                        ++slot;
+                    }
+                    for (int i = 0; i < DB; ++i) {
+                        uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
+                        en[0] = static_cast<uint32_t>(zero_slot) * static_cast<uint32_t>(p->raw_slot);
+                        en[1] = 0;
+                    }
+                    continue;
+                }
+                const Use &u = use[static_cast<size_t>(b) * npairs + e];
+                const int first_slot = slot;
+                for (int32_t r : u.rows) {
+                    sl[slot] = SpanMeta{u.start / 32 * v.unit_bytes, u.nbytes, r, u.start};
+                    ++slot;
+                }
+                const int c0 = live[2 * e], c1 = 2 * e + 1 < nlive ? live[2 * e + 1] : -1;
+                for (int i = 0; i < DB; ++i) {
+                    const int d = std::min(b * DB + i, ndm - 1);
+                    const int32_t d0 = p->delay[static_cast<size_t>(d) * nrows + c0];
+                    const int32_t dl = c1 < 0 ? 0 : p->delay[static_cast<size_t>(d) * nrows + c1] - d0;
+                    const int32_t r = static_cast<int32_t>(
+                        rowbase[e] + (std::lower_bound(deltas[e].begin(), deltas[e].end(), dl) - deltas[e].begin()));
+                    const int which = static_cast<int>(std::find(u.rows.begin(), u.rows.end(), r) - u.rows.begin());
+                    const uint32_t off = static_cast<uint32_t>(d0 - u.start);
+                    uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
+                    en[0] = static_cast<uint32_t>(first_slot + which) * static_cast<uint32_t>(p->raw_slot) +
+                            (off >> 5) * static_cast<uint32_t>(v.unit_bytes);
+                    en[1] = off & 31u;
+                }
+            }
+        }
+    }
+    p->ngroups = 1;
+    p->group_cols = ents_pad;
+    p->nblk = nblk;
+    p->nchans_pad = ents_pad;
+    p->smem_bytes = smem_layout_bytes(p, cc);
+    p->span.swap(span);
+    p->rel.swap(rel);
+    p->live.swap(live);
+    p->nlive = nlive;
+    p->prow.swap(prow);
+    p->n_prows = n_prows;
+    const int64_t vmax = (1 << nbits) - 1;
+    p->final32 = static_cast<int64_t>(nlive) * vmax > 65535;
+    return DD_OK;
+}
+
 dd_status build_tiles(dd_plan_s *p)
 {
+    p->pairs = false;
+    if (p->force_variant == 4)
+        return build_tiles_pairs(p);
     const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
     // the channels that are summed (PAPER.md:113 kill mask): the kernels iterate over this list only
     std::vector<int32_t> live;

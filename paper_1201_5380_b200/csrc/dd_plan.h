@@ -95,6 +95,17 @@ struct dd_plan_s {
     int sub_slot = 0;      // bit planes: bytes per sub-row inside a channel slot (raw_slot / nsub)
     int lane_slot = 0;     // bytes per channel slot of the unpacked lane buffer
     int64_t smem_bytes = 0;
+    // pair rows (variant 4): the CTA adds, per pair of adjacent live channels, ONE row S = x[c0] + shift(x[c1], delta)
+    // made beforehand for every delay difference delta = delay[d][c1] - delay[d][c0] that occurs in the table
+    bool pairs = false;
+    int pair_nbits = 0;                   // width of the consumer layout (4 for 2-bit input, 8 for 4-bit input)
+    int pair_planes = 0;                  // planes of a pair sum (nbits + 1)
+    int rows_per_chunk = 0;               // pair rows staged per stage (the largest count of any stage, padded rows skipped)
+    std::vector<int32_t> prow;            // [n_prows][4] {c0 row, c1 row or -1, delta, 0}
+    int64_t n_prows = 0;
+    void *d_prow = nullptr;
+    void *d_pairwork = nullptr;           // pair rows as bit planes [n_prows + 1][sub][bytes]; the last row is all zero
+    size_t pairwork_bytes = 0;
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
     std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels (nchans_pad = ngroups * group_cols)
@@ -129,6 +140,8 @@ dd_status build_subband(const dd_plan_s *p, dd_plan_s *s1, dd_plan_s *s2, std::v
 
 // Chooses the kernel variant and builds span/rel metadata.  DD_ERR_SMEM if no tiling fits.
 dd_status build_tiles(dd_plan_s *p);
+// Variant 4 (pair rows): 2- and 4-bit input, one channel group.  DD_ERR_SMEM if it cannot serve the plan.
+dd_status build_tiles_pairs(dd_plan_s *p);
 
 // Shared-memory bytes the kernel needs for `cc` channels per stage (must match the kernel's carve-up).
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc);

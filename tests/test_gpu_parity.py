@@ -38,7 +38,7 @@ def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, var
         p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
         torch.cuda.synchronize()
         info = p.launch_info()
-        assert info["last_launches"] == (2 if info["variant"] == 3 else 1) and (variant == 0 or info["variant"] == variant)
+        assert info["last_launches"] == {3: 2, 4: 2 + nbeams}.get(info["variant"], 1) and (variant == 0 or info["variant"] == variant)
     return out.cpu().numpy().view(_NP_VIEW[out_kind])
 
 
@@ -68,7 +68,7 @@ def test_cfg1_full_u32_and_f32():
     _full_compare(W.CONFIGS[1], out_kinds=["u32", "f32", "u16"])
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 def test_cfg2_reduced_several_tiles_ragged_tail(variant):
     # 1024 channels, 2-bit, 70 DMs (3 DM blocks of 32 / 5 of 16, last ragged), 3 time tiles + ragged tail of 77 samples
     _full_compare(W.CONFIGS[2].reduced(nsamps=3 * 1280 + 77, ndm=70), variant=variant)
@@ -95,13 +95,45 @@ def test_variant3_extreme_values_fill_all_planes():
         assert np.array_equal(got[0], ref) and int(ref.max()) == want and int(ref.min()) == want
 
 
+@pytest.mark.parametrize("nbits", [2, 4])
+def test_variant4_pair_rows(nbits):
+    # pair rows: one pre-summed row per (channel pair, delay difference), every trial adds the row of its own
+    # difference -- exact.  Channel counts around the stage size (16 / 8 pairs), odd counts (a last single channel),
+    # several tiles with a ragged tail, all output types, unsorted DM list, two beams through device and host paths
+    base = W.CONFIGS[2 if nbits == 2 else 4]
+    _full_compare(base.reduced(nsamps=2 * 3072 + 333, ndm=37, nchans=200), out_kinds=["f32", "u32", "u16"], variant=4)
+    for nchans in (1, 2, 3, 15, 16, 17, 31, 33, 63, 65, 257):
+        _full_compare(base.reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=4)
+    cfg = base.reduced(nsamps=1000, ndm=24, nchans=96)
+    dms = np.asarray(cfg.dm_list())[np.random.default_rng(4).permutation(cfg.ndm)]
+    _full_compare(cfg, dms=dms, out_kinds=["u32"], variant=4)
+    cfg = base.reduced(nsamps=3072 + 500, ndm=19, nchans=70, nbeams=2)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    mask = (np.arange(cfg.nchans) % 4 != 1).astype(np.int32)
+    out = torch.full((2, cfg.ndm, cfg.nsamps), -1, dtype=torch.float32, device="cuda")
+    h_out = torch.zeros((2, cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=4) as p:
+        p.set_killmask(mask)
+        p.set_dm_list(cfg.dm_list())
+        assert p.launch_info()["variant"] == 4
+        p.set_batch(2, dev.stride(0), out.stride(0) * 4)
+        p.execute(cfg.nsamps, dev, stride, out, 32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, 32)
+    for b in range(2):
+        ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask).astype(np.float32)
+        assert np.array_equal(out[b].cpu().numpy(), ref) and np.array_equal(h_out[b].numpy(), ref)
+
+
 def test_variant2_channel_counts_around_group_and_flush_boundaries():
     # nchans not a multiple of 5 (group), of 40 (stage), beyond 85 (8-bit flush) and 17*5*k boundaries
     for nchans in (1, 4, 5, 6, 39, 41, 84, 85, 86, 171, 1023):
         _full_compare(W.CONFIGS[2].reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=2)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_cfg2_high_dm_end(variant):
     # the last DMs of config 2 (largest delays and spreads), nsamps not a multiple of 4
     cfg = W.CONFIGS[2].reduced(nsamps=1501, ndm=40)
@@ -119,7 +151,7 @@ def test_cfg3_high_dm_end_large_spread(variant):
     _full_compare(cfg, dms=W.CONFIGS[3].dm_list()[-32:], variant=variant)
 
 
-@pytest.mark.parametrize("variant", [1, 3])
+@pytest.mark.parametrize("variant", [1, 3, 4])
 def test_cfg4_reduced_4bit_u16(variant):
     _full_compare(W.CONFIGS[4].reduced(nsamps=2000, ndm=65), out_kinds=["u16", "u32", "f32"], variant=variant)
 
@@ -185,7 +217,7 @@ def test_many_channels_need_32bit_accumulators():
     _full_compare(cfg4)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])   # variant 4 with a kill mask: test_variant4_pair_rows
 def test_killmask_every_variant(variant):
     # PAPER.md:113 kill mask against the oracle's arithmetic form (sum += data * mask[c]); masks that kill
     # runs, single channels, the first and the last channel, so that the live list is ragged against the stage size
@@ -415,7 +447,7 @@ def test_u16_rows_that_are_not_16_byte_aligned(nbits):
     assert np.array_equal(h_out.numpy().view(np.uint16), ref.astype(np.uint16))
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])
 @pytest.mark.parametrize("pad", [16, 1])   # rows padded by 16 elements (16-byte aligned rows) / by one element
 def test_output_row_stride(variant, pad):
     # PAPER.md:388 "arbitrary strides through the ... output arrays": rows out_dm_stride bytes apart, padding untouched
