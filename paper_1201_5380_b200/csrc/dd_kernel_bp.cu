@@ -57,6 +57,10 @@ struct Bp<2> {
     static constexpr int NB = 2, NSUB = 1, NP = 12, W = DD_BP_W2, CC = 32, FL = DD_BP_FL2;
 };
 template <>
+struct Bp<3> {   // pair rows of 2-bit input (variant 4): 3 planes per unit (12 bytes, three LDS.32), 8 pairs per stage
+    static constexpr int NB = 3, NSUB = 1, NP = 12, W = DD_BP_W2, CC = 8, FL = 4;
+};
+template <>
 struct Bp<4> {
     static constexpr int NB = 4, NSUB = 1, NP = 16, W = 3, CC = 16, FL = DD_BP_FL4;
 };
@@ -208,6 +212,15 @@ struct PlaneVec<2> {
     {
         const uint2 v = *reinterpret_cast<const uint2 *>(p);
         w[0] = v.x, w[1] = v.y;
+    }
+};
+template <>
+struct PlaneVec<3> {
+    uint32_t w[3];
+    __device__ __forceinline__ void load(const uint8_t *p)
+    {
+        const uint32_t *q = reinterpret_cast<const uint32_t *>(p);
+        w[0] = q[0], w[1] = q[1], w[2] = q[2];
     }
 };
 template <>
@@ -427,7 +440,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     static_assert(PIN >= 1 && PIN <= NBITS, "planes in use");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
     constexpr int FL = LONG ? C::FL : 1;
-    constexpr bool PATCH = !LONG || (NBITS < 8 && !PAIRS);   // pair rows: the ring needs the shared memory more
+    constexpr bool PATCH = !LONG || (NBITS < 8 && (!PAIRS || NBITS == 3));   // 4-bit pair rows: the ring needs the shared memory more
     constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;        // largest value one stage adds to a counter
     constexpr int NT = bit_length(FL * STAGE_SUM);                   // pending slots
     static_assert(PAIRS || (CC * NSUB) % BP_NWARPS == 0, "every warp stages the same number of sub-rows");
@@ -810,7 +823,7 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
 // ------------------------------------------------------------------------------------------ pair rows (variant 4)
 // S[t] = x[c0][t] + x[c1][t + delta] in bit planes, for every pair row {c0, c1, delta}: NBITS planes + NBITS planes ->
 // NBITS + 1 planes by a ripple of full adders (xor3 / maj3), written in the layout of the consumer kernel
-// (4 planes per unit and sub-row).  One thread per (row, unit).  in: bit-plane rows of the input [c][unit][NBITS
+// (2-bit input: 3 planes per unit, 12 bytes; 4-bit input: 2 sub-rows of 4 planes, 5 in use).  One thread per (row, unit).  in: bit-plane rows of the input [c][unit][NBITS
 // planes], in_units units per row, zero beyond the input; a killed partner (c1 < 0) contributes nothing.
 template <int NBITS>
 __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restrict__ in, int64_t in_row_words, int64_t in_units,
@@ -850,8 +863,9 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
     }
     sum[NBITS] = cy;
     uint32_t *o = out + r * (NSUBO * out_sub_words) + u * 4;
-    if constexpr (NBITS == 2) {
-        *reinterpret_cast<uint4 *>(o) = make_uint4(sum[0], sum[1], sum[2], 0u);
+    if constexpr (NBITS == 2) {   // 3 planes per unit, 12 bytes (consecutive threads write consecutive units)
+        uint32_t *o3 = out + r * out_sub_words + u * 3;
+        o3[0] = sum[0], o3[1] = sum[1], o3[2] = sum[2];
     } else {
         *reinterpret_cast<uint4 *>(o) = make_uint4(sum[0], sum[1], sum[2], sum[3]);
         *reinterpret_cast<uint4 *>(o + out_sub_words) = make_uint4(sum[4], 0u, 0u, 0u);
@@ -862,9 +876,10 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
 template <int NBITS>
 cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
 {
-    constexpr int ENB = NBITS == 2 ? 4 : 8;
+    constexpr int ENB = NBITS == 2 ? 3 : 8;   // layout of the pair rows: 3 planes per unit / 2 x 4 planes (5 in use)
     using C = Bp<ENB>;
     constexpr int TB = 32 * 32 * C::W;
+    constexpr int UBO = C::NB * 4;            // bytes per unit of a pair-row sub-row
     if (!plan->pairs || plan->pair_nbits != ENB || plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB ||
         kp_in.ngroups != 1 || !plan->d_prow)
         return cudaErrorInvalidValue;
@@ -873,8 +888,8 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     for (int64_t r = 0; r < plan->n_prows; ++r)
         max_delta = plan->prow[4 * r + 2] > max_delta ? plan->prow[4 * r + 2] : max_delta;
     // pair rows: as long as the longest span of the tiles needs; input bit planes: that plus the largest difference
-    const int64_t out_units = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + 31) / 32;
-    const int64_t conv_o = out_units * 16;
+    const int64_t out_units = ((static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + 31) / 32 + 3) / 4 * 4;
+    const int64_t conv_o = out_units * UBO;   // a multiple of 16 bytes (whole groups of 4 units)
     const int64_t rows_o = plan->n_prows + 1;                               // + the all-zero row of padded entries
     const int64_t beam_o = rows_o * C::NSUB * conv_o;
     const int64_t spg = (16 / (NBITS * 4)) * 32;                            // input samples per 16-byte group
@@ -911,7 +926,7 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
         static_cast<int32_t>(groups_i));
     if ((e = cudaGetLastError()) != cudaSuccess)
         return e;
-    const int64_t ublocks = (out_units + 255) / 256;
+    const int64_t ublocks = (out_units + 255) / 256;   // (a 4-units-per-thread builder with 16-byte stores measured slower)
     if (plan->n_prows * ublocks > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
     for (int b = 0; b < kp.nbeams; ++b) {

@@ -188,21 +188,26 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     if (nlive == 0)
         return DD_ERR_SMEM;
     const int npairs = (nlive + 1) / 2;
-    const int enb = nbits == 2 ? 4 : 8;                 // consumer layout
-    const Variant *vv = nullptr;
-    for (const Variant &v : kVariants)
-        if (v.id == 3 && (v.nbits_mask & (1 << enb)))
-            vv = &v;
-    if (!vv)
-        return DD_ERR_SMEM;
-    Variant v = *vv;
-    v.id = 4;
+    const int enb = nbits == 2 ? 3 : 8;                 // layout of the pair rows (must match Bp<3> / Bp<8> in dd_kernel_bp.cu)
+    Variant v{};
+    if (nbits == 2) {   // 3 planes per unit (12 bytes), 5 units per lane, 8 pairs per stage, flush every 4 stages
+        v = Variant{4, 16, 1024 * DD_BP_W2, 512, 32, 8, 3, 0, 4, {8, 0, 0, 0}, 1 << 2, 12, true, true, 12, 1};
+    } else {
+        const Variant *vv = nullptr;
+        for (const Variant &k : kVariants)
+            if (k.id == 3 && (k.nbits_mask & (1 << enb)))
+                vv = &k;
+        if (!vv)
+            return DD_ERR_SMEM;
+        v = *vv;
+        v.id = 4;
+    }
     const int pin = nbits + 1;                          // planes of a pair sum
     const int64_t top = static_cast<int64_t>(npairs) * ((1 << pin) - 1);   // structural weight the counters take
     if (top >= (int64_t(1) << v.max_sum_bits))
         return DD_ERR_SMEM;
     const int DB = v.DB, cc = v.cc[0];
-    const int fl = kBpFlushStages(enb);
+    const int fl = nbits == 2 ? 4 : kBpFlushStages(enb);
     const int nblk = (ndm + DB - 1) / DB;
     const bool long_mode = npairs >= 8 * cc * fl;
     const int ents_pad = static_cast<int>(align_up(npairs, cc * (long_mode ? fl : 1)));
@@ -234,7 +239,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     if (n_prows > (int64_t(1) << 30))
         return DD_ERR_SMEM;
     // per (DM block, pair): the rows in use and the staged span (of the pair's first channel)
-    const int A = (16 / v.unit_bytes) * 32;
+    const int A = v.unit_bytes == 12 ? 128 : (16 / v.unit_bytes) * 32;   // samples per 16-byte aligned granule (12-byte units: 4 units)
     struct Use { int32_t start, nbytes; std::vector<int32_t> rows; };
     std::vector<Use> use(static_cast<size_t>(nblk) * npairs);
     int64_t max_bytes = 0, max_end = 0;
@@ -281,7 +286,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     p->pair_nbits = enb;
     p->pair_planes = pin;
     p->long_mode = long_mode;
-    p->patch = !long_mode;   // long: no output patches, a deeper ring instead (must match PATCH in dd_kernel_bp.cu)
+    p->patch = !long_mode || nbits == 2;   // 4-bit input, long: no output patches, a deeper ring (must match PATCH in dd_kernel_bp.cu)
     p->max_span_end = max_end;
     p->sub_slot = static_cast<int>(max_bytes);
     p->raw_slot = static_cast<int>(max_bytes) * v.nsub;
