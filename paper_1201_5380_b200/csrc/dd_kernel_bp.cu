@@ -65,6 +65,10 @@ struct Bp<4> {
     static constexpr int NB = 4, NSUB = 1, NP = 16, W = 3, CC = 16, FL = DD_BP_FL4;
 };
 template <>
+struct Bp<12> {   // pair rows of 8-bit input (variant 4): 9 planes in three 4-plane sub-rows, 4 pairs per stage
+    static constexpr int NB = 4, NSUB = 3, NP = 20, W = 3, CC = 4, FL = 2;
+};
+template <>
 struct Bp<8> {
     static constexpr int NB = 4, NSUB = 2, NP = 20, W = 3, CC = 8, FL = DD_BP_FL8;
 };
@@ -830,24 +834,27 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
                                                          const int4 *__restrict__ prow, uint32_t *__restrict__ out,
                                                          int64_t out_sub_words, int64_t out_units, int64_t ublocks)
 {
-    constexpr int NSUBO = NBITS == 2 ? 1 : 2;
+    constexpr int NBI = Bp<NBITS>::NB, NSUBI = Bp<NBITS>::NSUB;   // input layout: NSUBI sub-rows of NBI planes per unit
+    constexpr int NSUBO = NBITS == 2 ? 1 : (NBITS == 4 ? 2 : 3);
     const int64_t blk = blockIdx.x;
     const int64_t r = blk / ublocks, u = (blk - r * ublocks) * blockDim.x + threadIdx.x;
     if (u >= out_units)
         return;
     const int4 pr = __ldg(&prow[r]);
+    const int64_t in_sub_words = in_row_words / NSUBI;
     uint32_t a[NBITS], b[NBITS];
-    const uint32_t *ra = in + static_cast<int64_t>(pr.x) * in_row_words + u * NBITS;
+    const uint32_t *ra = in + static_cast<int64_t>(pr.x) * in_row_words;
 #pragma unroll
     for (int k = 0; k < NBITS; ++k)
-        a[k] = u < in_units ? ra[k] : 0u;
+        a[k] = u < in_units ? ra[(k / NBI) * in_sub_words + u * NBI + (k % NBI)] : 0u;
     if (pr.y >= 0) {
         const int64_t ub = u + (pr.z >> 5);
         const uint32_t sh = static_cast<uint32_t>(pr.z) & 31u;
-        const uint32_t *rb = in + static_cast<int64_t>(pr.y) * in_row_words + ub * NBITS;
+        const uint32_t *rb = in + static_cast<int64_t>(pr.y) * in_row_words;
 #pragma unroll
         for (int k = 0; k < NBITS; ++k) {
-            const uint32_t lo = ub < in_units ? rb[k] : 0u, hi = ub + 1 < in_units ? rb[NBITS + k] : 0u;
+            const uint32_t *q = rb + (k / NBI) * in_sub_words + ub * NBI + (k % NBI);
+            const uint32_t lo = ub < in_units ? q[0] : 0u, hi = ub + 1 < in_units ? q[NBI] : 0u;
             b[k] = __funnelshift_r(lo, hi, sh);
         }
     } else {
@@ -862,21 +869,23 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
         cy = maj3(a[k], b[k], cy);
     }
     sum[NBITS] = cy;
-    uint32_t *o = out + r * (NSUBO * out_sub_words) + u * 4;
     if constexpr (NBITS == 2) {   // 3 planes per unit, 12 bytes (consecutive threads write consecutive units)
         uint32_t *o3 = out + r * out_sub_words + u * 3;
         o3[0] = sum[0], o3[1] = sum[1], o3[2] = sum[2];
-    } else {
-        *reinterpret_cast<uint4 *>(o) = make_uint4(sum[0], sum[1], sum[2], sum[3]);
-        *reinterpret_cast<uint4 *>(o + out_sub_words) = make_uint4(sum[4], 0u, 0u, 0u);
+    } else {                      // sub-rows of 4 planes; the last one holds the carry plane alone
+        uint32_t *o = out + r * (NSUBO * out_sub_words) + u * 4;
+#pragma unroll
+        for (int q = 0; q < NSUBO - 1; ++q)
+            *reinterpret_cast<uint4 *>(o + q * out_sub_words) = make_uint4(sum[4 * q], sum[4 * q + 1], sum[4 * q + 2], sum[4 * q + 3]);
+        *reinterpret_cast<uint4 *>(o + (NSUBO - 1) * out_sub_words) = make_uint4(sum[NBITS], 0u, 0u, 0u);
     }
 }
 
-// NBITS: input width (2 or 4); the consumer is the bit-plane kernel of width ENB = 4 or 8 with NBITS + 1 planes in use
+// NBITS: input width; the consumer is the bit-plane kernel with the layout Bp<ENB> and NBITS + 1 planes in use
 template <int NBITS>
 cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
 {
-    constexpr int ENB = NBITS == 2 ? 3 : 8;   // layout of the pair rows: 3 planes per unit / 2 x 4 planes (5 in use)
+    constexpr int ENB = NBITS == 2 ? 3 : (NBITS == 4 ? 8 : 12);   // pair-row layout: 3 planes per unit / 2 x 4 planes (5 in use) / 3 x 4 (9 in use)
     using C = Bp<ENB>;
     constexpr int TB = 32 * 32 * C::W;
     constexpr int UBO = C::NB * 4;            // bytes per unit of a pair-row sub-row
@@ -892,10 +901,11 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     const int64_t conv_o = out_units * UBO;   // a multiple of 16 bytes (whole groups of 4 units)
     const int64_t rows_o = plan->n_prows + 1;                               // + the all-zero row of padded entries
     const int64_t beam_o = rows_o * C::NSUB * conv_o;
-    const int64_t spg = (16 / (NBITS * 4)) * 32;                            // input samples per 16-byte group
+    using CI = Bp<NBITS>;                                                   // layout of the input bit planes
+    const int64_t spg = (16 / (CI::NB * 4)) * 32;                           // input samples per 16-byte group of a sub-row
     const int64_t groups_i = (out_units * 32 + max_delta + 64 + spg - 1) / spg;
-    const int64_t conv_i = groups_i * 16, in_units = conv_i / (NBITS * 4);
-    const int64_t beam_i = static_cast<int64_t>(kp.nrows) * conv_i;
+    const int64_t conv_i = groups_i * 16, in_units = conv_i / (CI::NB * 4);  // bytes per sub-row, units per row
+    const int64_t beam_i = static_cast<int64_t>(kp.nrows) * CI::NSUB * conv_i;
     cudaError_t e;
     const size_t need_i = static_cast<size_t>(kp.nbeams) * beam_i, need_o = static_cast<size_t>(kp.nbeams) * beam_o;
     if (plan->work_bytes < need_i) {
@@ -931,7 +941,7 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
         return cudaErrorInvalidConfiguration;
     for (int b = 0; b < kp.nbeams; ++b) {
         dd_make_pair_rows<NBITS><<<dim3(static_cast<unsigned>(plan->n_prows * ublocks)), 256, 0, stream>>>(
-            reinterpret_cast<const uint32_t *>(static_cast<const uint8_t *>(plan->d_work) + b * beam_i), conv_i / 4, in_units,
+            reinterpret_cast<const uint32_t *>(static_cast<const uint8_t *>(plan->d_work) + b * beam_i), CI::NSUB * conv_i / 4, in_units,
             static_cast<const int4 *>(plan->d_prow), reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(plan->d_pairwork) + b * beam_o),
             conv_o / 4, out_units, ublocks);
         if ((e = cudaGetLastError()) != cudaSuccess)
@@ -984,6 +994,8 @@ cudaError_t launch_variant4(dd_plan_s *plan, const KernelParams &kp, cudaStream_
         return launch_pairs<2>(plan, kp, stream);
     case 4:
         return launch_pairs<4>(plan, kp, stream);
+    case 8:
+        return launch_pairs<8>(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }

@@ -178,7 +178,7 @@ static const Variant kVariants[] = {
 dd_status build_tiles_pairs(dd_plan_s *p)
 {
     const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
-    if ((nbits != 2 && nbits != 4) || p->group_size > 0)
+    if (p->group_size > 0)
         return DD_ERR_SMEM;
     std::vector<int32_t> live;
     for (int c = 0; c < nrows; ++c)
@@ -188,10 +188,12 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     if (nlive == 0)
         return DD_ERR_SMEM;
     const int npairs = (nlive + 1) / 2;
-    const int enb = nbits == 2 ? 3 : 8;                 // layout of the pair rows (must match Bp<3> / Bp<8> in dd_kernel_bp.cu)
+    const int enb = nbits == 2 ? 3 : (nbits == 4 ? 8 : 12);   // layout of the pair rows (must match Bp<3> / Bp<8> / Bp<12> in dd_kernel_bp.cu)
     Variant v{};
     if (nbits == 2) {   // 3 planes per unit (12 bytes), 5 units per lane, 8 pairs per stage, flush every 4 stages
         v = Variant{4, 16, 1024 * DD_BP_W2, 512, 32, 8, 3, 0, 4, {8, 0, 0, 0}, 1 << 2, 12, true, true, 12, 1};
+    } else if (nbits == 8) {   // 9 planes in three 4-plane sub-rows, 3 units per lane, 4 pairs per stage, flush every 2 stages
+        v = Variant{4, 16, 3072, 512, 32, 8, 12, 0, 4, {4, 0, 0, 0}, 1 << 8, 20, true, true, 16, 3};
     } else {
         const Variant *vv = nullptr;
         for (const Variant &k : kVariants)
@@ -207,7 +209,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     if (top >= (int64_t(1) << v.max_sum_bits))
         return DD_ERR_SMEM;
     const int DB = v.DB, cc = v.cc[0];
-    const int fl = nbits == 2 ? 4 : kBpFlushStages(enb);
+    const int fl = nbits == 2 ? 4 : (nbits == 8 ? 2 : kBpFlushStages(enb));
     const int nblk = (ndm + DB - 1) / DB;
     const bool long_mode = npairs >= 8 * cc * fl;
     const int ents_pad = static_cast<int>(align_up(npairs, cc * (long_mode ? fl : 1)));
@@ -286,7 +288,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     p->pair_nbits = enb;
     p->pair_planes = pin;
     p->long_mode = long_mode;
-    p->patch = !long_mode || nbits == 2;   // 4-bit input, long: no output patches, a deeper ring (must match PATCH in dd_kernel_bp.cu)
+    p->patch = !long_mode || nbits == 2;   // 4- and 8-bit input, long: no output patches, a deeper ring (must match PATCH in dd_kernel_bp.cu)
     p->max_span_end = max_end;
     p->sub_slot = static_cast<int>(max_bytes);
     p->raw_slot = static_cast<int>(max_bytes) * v.nsub;

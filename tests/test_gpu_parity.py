@@ -95,12 +95,19 @@ def test_variant3_extreme_values_fill_all_planes():
         assert np.array_equal(got[0], ref) and int(ref.max()) == want and int(ref.min()) == want
 
 
-@pytest.mark.parametrize("nbits", [2, 4])
+@pytest.mark.parametrize("nbits", [2, 4, 8])
 def test_variant4_pair_rows(nbits):
     # pair rows: one pre-summed row per (channel pair, delay difference), every trial adds the row of its own
     # difference -- exact.  Channel counts around the stage size (16 / 8 pairs), odd counts (a last single channel),
     # several tiles with a ragged tail, all output types, unsorted DM list, two beams through device and host paths
-    base = W.CONFIGS[2 if nbits == 2 else 4]
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+
+    class base:   # reduced copies of the config with one beam unless asked otherwise
+        @staticmethod
+        def reduced(**kw):
+            kw.setdefault("nbeams", 1)
+            return full.reduced(**kw)
+
     _full_compare(base.reduced(nsamps=2 * 3072 + 333, ndm=37, nchans=200), out_kinds=["f32", "u32", "u16"], variant=4)
     for nchans in (1, 2, 3, 15, 16, 17, 31, 33, 63, 65, 257):
         _full_compare(base.reduced(nsamps=1283, ndm=3, nchans=nchans), out_kinds=["u32"], variant=4)
