@@ -241,6 +241,7 @@ struct BpShared {
     const uint8_t *lane_base;   // stage base + this lane's byte offset (W units per lane)
     const uint2 *rel;           // this warp's offset entries of the stage: [cl * BP_DB]
     int sub_slot;               // bytes between the sub-rows of a channel slot
+    const uint8_t *lane_lone;   // LONE layouts: last sub-row of slot 0 + this lane's offset in it (4 bytes per unit)
 };
 
 // plane k of sub-row SUB of a channel, for every unit of the lane; CLS = channels added since the last flush
@@ -263,29 +264,43 @@ __device__ __forceinline__ void plane_step(const PlaneVec<Bp<NBITS>::NB> (&x)[Bp
 
 // channel CL of the stage: per sub-row one window of W+1 units serves W units; per unit and plane one funnel
 // shift + carry-save adds
-template <int NBITS, int PIN, int CLS, int SUB, int NP, int NT>
+// LONE (pair rows of 4- and 8-bit input): the last sub-row holds the carry plane alone, one word per unit; the offset
+// entry carries the window's unit offset in e.y >> 8 (the funnel shift takes e.y modulo 32)
+template <int NBITS, int PIN, bool LONE, int CLS, int SUB, int NP, int NT>
 __device__ __forceinline__ void subrow_step(const BpShared &sh, const uint2 e, uint32_t (&P)[Bp<NBITS>::W][NP],
                                             uint32_t (&T)[Bp<NBITS>::W][NT])
 {
     using C = Bp<NBITS>;
-    if constexpr (SUB < C::NSUB && SUB * C::NB < PIN) {
+    if constexpr (LONE && SUB == C::NSUB - 1) {
+        constexpr int L = SUB * C::NB;                                        // weight of the lone plane
+        static_assert(PIN == L + 1, "the lone plane is the top plane of a pair sum");
+        constexpr uint32_t S = ((1u << PIN) - 1u) * CLS + ((1u << L) - 1u);
+        const uint32_t *wp = reinterpret_cast<const uint32_t *>(sh.lane_lone + e.x - (e.y >> 8) * 12u);
+        uint32_t x[C::W + 1];
+#pragma unroll
+        for (int j = 0; j <= C::W; ++j)
+            x[j] = wp[j];
+#pragma unroll
+        for (int j = 0; j < C::W; ++j)
+            csa_add<S, L>(P[j], T[j], __funnelshift_r(x[j], x[j + 1], e.y));
+    } else if constexpr (SUB < C::NSUB && SUB * C::NB < PIN) {
         const uint8_t *wp = sh.lane_base + e.x + SUB * sh.sub_slot;
         PlaneVec<C::NB> x[C::W + 1];
 #pragma unroll
         for (int j = 0; j <= C::W; ++j)
             x[j].load(wp + j * (C::NB * 4));
         plane_step<NBITS, PIN, CLS, SUB, 0>(x, e.y, P, T);
-        subrow_step<NBITS, PIN, CLS, SUB + 1>(sh, e, P, T);
+        subrow_step<NBITS, PIN, LONE, CLS, SUB + 1>(sh, e, P, T);
     }
 }
 
 // PHASE: stages added since the last flush (the pending words are rippled into the planes every FL stages)
-template <int NBITS, int PIN, int PHASE, int NP, int NT, int... CLs>
+template <int NBITS, int PIN, bool LONE, int PHASE, int NP, int NT, int... CLs>
 __device__ __forceinline__ void stage_steps(std::integer_sequence<int, CLs...>, const BpShared &sh,
                                             uint32_t (&P)[Bp<NBITS>::W][NP], uint32_t (&T)[Bp<NBITS>::W][NT])
 {
     // rel entry: {byte offset in the stage, bit shift}
-    (subrow_step<NBITS, PIN, PHASE * Bp<NBITS>::CC + CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);
+    (subrow_step<NBITS, PIN, LONE, PHASE * Bp<NBITS>::CC + CLs, 0>(sh, sh.rel[CLs * BP_DB], P, T), ...);
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -443,6 +458,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     static_assert(LONG || static_cast<int64_t>(8 * CC * C::FL) * ((1 << NBITS) - 1) <= (int64_t(1) << NP), "short-mode sums must fit NP planes");
     static_assert(PIN >= 1 && PIN <= NBITS, "planes in use");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
+    constexpr bool LONE = PAIRS && (NBITS == 8 || NBITS == 12);      // the last sub-row holds one plane, 4 bytes per unit
     constexpr int FL = LONG ? C::FL : 1;
     constexpr bool PATCH = !LONG || (NBITS < 8 && (!PAIRS || NBITS == 3));   // 4-bit pair rows: the ring needs the shared memory more
     constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;        // largest value one stage adds to a counter
@@ -529,7 +545,9 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             uint32_t tx = (warp == 0) ? static_cast<uint32_t>(CC * DB * 8) : 0u;
 #pragma unroll
             for (int k = 0; k < CPW; ++k)
-                tx += static_cast<uint32_t>(m[k].y) * (PAIRS ? NSUB : 1);
+                tx += PAIRS ? (LONE ? static_cast<uint32_t>(m[k].y) * (NSUB - 1) + static_cast<uint32_t>(m[k].y) / 4u
+                                    : static_cast<uint32_t>(m[k].y) * NSUB)
+                            : static_cast<uint32_t>(m[k].y);
             mbar_arrive_expect_tx(&full[s], tx);
             if constexpr (PAIRS) {
 #pragma unroll
@@ -537,10 +555,17 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                     if (m[k].y > 0) {
                         const int slot = warp + BP_NWARPS * k;
 #pragma unroll
-                        for (int sub = 0; sub < NSUB; ++sub)
-                            tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
-                                         in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x,
-                                         static_cast<uint32_t>(m[k].y), &full[s]);
+                        for (int sub = 0; sub < NSUB; ++sub) {
+                            if (LONE && sub == NSUB - 1)   // the lone plane: a quarter of the bytes at a quarter of the offset
+                                tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
+                                             in_beam + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes +
+                                                 ((t0 >> 5) * UB + m[k].x) / 4,
+                                             static_cast<uint32_t>(m[k].y) / 4u, &full[s]);
+                            else
+                                tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
+                                             in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x,
+                                             static_cast<uint32_t>(m[k].y), &full[s]);
+                        }
                     }
                 }
             }
@@ -604,7 +629,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
         sh.lane_base = raw_base + s * raw_stage + lane * (W * UB);
         sh.rel = reinterpret_cast<const uint2 *>(rel_base + s * rel_stage) + warp;
         sh.sub_slot = p.sub_slot;
-        stage_steps<NBITS, PIN, PHASE>(std::make_integer_sequence<int, CC>{}, sh, P, T);
+        sh.lane_lone = raw_base + s * raw_stage + (NSUB - 1) * p.sub_slot + lane * (W * 4);
+        stage_steps<NBITS, PIN, LONE, PHASE>(std::make_integer_sequence<int, CC>{}, sh, P, T);
         if constexpr (FLUSH != 0u) {
 #pragma unroll
             for (int j = 0; j < W; ++j)
@@ -872,12 +898,12 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
     if constexpr (NBITS == 2) {   // 3 planes per unit, 12 bytes (consecutive threads write consecutive units)
         uint32_t *o3 = out + r * out_sub_words + u * 3;
         o3[0] = sum[0], o3[1] = sum[1], o3[2] = sum[2];
-    } else {                      // sub-rows of 4 planes; the last one holds the carry plane alone
-        uint32_t *o = out + r * (NSUBO * out_sub_words) + u * 4;
+    } else {                      // sub-rows of 4 planes, then the carry plane alone at 4 bytes per unit
+        uint32_t *o = out + r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + u * 4;
 #pragma unroll
         for (int q = 0; q < NSUBO - 1; ++q)
             *reinterpret_cast<uint4 *>(o + q * out_sub_words) = make_uint4(sum[4 * q], sum[4 * q + 1], sum[4 * q + 2], sum[4 * q + 3]);
-        *reinterpret_cast<uint4 *>(o + (NSUBO - 1) * out_sub_words) = make_uint4(sum[NBITS], 0u, 0u, 0u);
+        out[r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + (NSUBO - 1) * out_sub_words + u] = sum[NBITS];   // the lone carry plane
     }
 }
 
@@ -900,7 +926,9 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     const int64_t out_units = ((static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + 31) / 32 + 3) / 4 * 4;
     const int64_t conv_o = out_units * UBO;   // a multiple of 16 bytes (whole groups of 4 units)
     const int64_t rows_o = plan->n_prows + 1;                               // + the all-zero row of padded entries
-    const int64_t beam_o = rows_o * C::NSUB * conv_o;
+    constexpr bool LONEL = NBITS != 2;                                      // last sub-row: one plane, conv_o / 4 bytes
+    const int64_t pitch_o = LONEL ? (C::NSUB - 1) * conv_o + conv_o / 4 : C::NSUB * conv_o;   // bytes per pair row
+    const int64_t beam_o = rows_o * pitch_o;
     using CI = Bp<NBITS>;                                                   // layout of the input bit planes
     const int64_t spg = (16 / (CI::NB * 4)) * 32;                           // input samples per 16-byte group of a sub-row
     const int64_t groups_i = (out_units * 32 + max_delta + 64 + spg - 1) / spg;
@@ -928,8 +956,8 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
         plan->pairwork_bytes = need_o;
     }
     // the zero row of every beam
-    if ((e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_pairwork) + plan->n_prows * C::NSUB * conv_o, static_cast<size_t>(beam_o),
-                               0, static_cast<size_t>(C::NSUB) * conv_o, kp.nbeams, stream)) != cudaSuccess)
+    if ((e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_pairwork) + plan->n_prows * pitch_o, static_cast<size_t>(beam_o),
+                               0, static_cast<size_t>(pitch_o), kp.nbeams, stream)) != cudaSuccess)
         return e;
     dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups_i + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
         kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv_i, beam_i,
@@ -950,7 +978,7 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     kp.in = static_cast<const uint8_t *>(plan->d_pairwork);
-    kp.in_stride = C::NSUB * conv_o;
+    kp.in_stride = pitch_o;
     kp.in_blk_stride = 0;
     kp.in_row_bytes = conv_o;
     kp.in_beam_stride = beam_o;

@@ -241,7 +241,8 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     if (n_prows > (int64_t(1) << 30))
         return DD_ERR_SMEM;
     // per (DM block, pair): the rows in use and the staged span (of the pair's first channel)
-    const int A = v.unit_bytes == 12 ? 128 : (16 / v.unit_bytes) * 32;   // samples per 16-byte aligned granule (12-byte units: 4 units)
+    const bool lone = nbits != 2;   // last sub-row of a pair row: the carry plane alone, 4 bytes per unit (dd_kernel_bp.cu LONE)
+    const int A = 128;              // spans in whole groups of 4 units: 12-byte units and quarter-size lone sub-rows stay 16-byte aligned
     struct Use { int32_t start, nbytes; std::vector<int32_t> rows; };
     std::vector<Use> use(static_cast<size_t>(nblk) * npairs);
     int64_t max_bytes = 0, max_end = 0;
@@ -291,7 +292,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     p->patch = !long_mode || nbits == 2;   // 4- and 8-bit input, long: no output patches, a deeper ring (must match PATCH in dd_kernel_bp.cu)
     p->max_span_end = max_end;
     p->sub_slot = static_cast<int>(max_bytes);
-    p->raw_slot = static_cast<int>(max_bytes) * v.nsub;
+    p->raw_slot = lone ? static_cast<int>(max_bytes) * (v.nsub - 1) + static_cast<int>(max_bytes) / 4 : static_cast<int>(max_bytes) * v.nsub;
     p->lane_slot = p->raw_slot;
     p->rows_per_chunk = rs;
     p->cc = cc;
@@ -350,7 +351,7 @@ dd_status build_tiles_pairs(dd_plan_s *p)
                     uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (base + i) * 2;
                     en[0] = static_cast<uint32_t>(first_slot + which) * static_cast<uint32_t>(p->raw_slot) +
                             (off >> 5) * static_cast<uint32_t>(v.unit_bytes);
-                    en[1] = off & 31u;
+                    en[1] = (off & 31u) | ((off >> 5) << 8);   // shift; unit offset for the lone sub-row
                 }
             }
         }
