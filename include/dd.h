@@ -261,8 +261,10 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20);
  *            4 = pair rows (2/4/8-bit, opt-in): the same kernel over rows x[c0] + shift(x[c1], delta) made once per
  *                delay difference delta of every pair of adjacent summed channels -- exact, n + 1 plane words per
- *                pair instead of 2 n; costs device memory for the rows (16x / 26x / 12x the packed input on the
- *                2-bit / 4-bit / 8-bit survey-shaped configs: 2.3 GB / 14.5 GB / 46 GB) and a third kernel.
+ *                pair instead of 2 n; costs device memory for the rows of one beam (16x / 26x / 12x its packed
+ *                input on the 2-bit / 4-bit / 8-bit survey-shaped configs; twice that with several beams; the time
+ *                axis is split into groups if that exceeds 3/4 of the free memory) and two more kernels per group,
+ *                run on internal streams that are forked from and joined to the caller's stream.
  * Takes effect at the next dd_set_dm_list (which returns DD_ERR_SMEM if that variant cannot serve the plan).
  */
 dd_status dd_set_kernel_variant(dd_plan plan, int variant);

@@ -411,6 +411,12 @@ dd_status dd_plan_destroy(dd_plan plan)
         cudaFree(plan->d_work);
     if (plan->d_pairwork)
         cudaFree(plan->d_pairwork);
+    for (void *st : plan->pair_streams)
+        if (st)
+            cudaStreamDestroy(static_cast<cudaStream_t>(st));
+    for (void *ev : plan->pair_events)
+        if (ev)
+            cudaEventDestroy(static_cast<cudaEvent_t>(ev));
     if (plan->d_tmp)
         cudaFree(plan->d_tmp);
     destroy_subplan(plan->s1);

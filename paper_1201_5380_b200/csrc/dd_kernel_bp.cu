@@ -29,6 +29,7 @@
 //            into the upper planes;
 //   store  : bit-matrix transposes turn NP planes x 32 lanes into 32 integers; float32 / uint32 / uint16,
 //            128-bit stores, time contiguous.
+#include <cstdlib>
 #include <utility>
 
 #include "dd_common.cuh"
@@ -472,7 +473,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int64_t cta = blockIdx.x;
     const int blk = static_cast<int>(cta % p.nblk);
     const int64_t rest = cta / p.nblk;
-    const int tile = static_cast<int>(rest % p.ntiles);
+    const int tile = static_cast<int>(rest % p.ntiles) + (PAIRS ? p.tile0 : 0);
     const int batch = static_cast<int>(rest / p.ntiles);          // (beam, set of gpc channel groups); gpc = 1: (beam, group)
     int beam, group, nch_set = 0;   // group: the first one of the set; nch_set: stages this CTA works through
     if constexpr (LONG) {           // always one group per CTA
@@ -510,7 +511,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
 
     const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride +
                              (p.in_blk_div > 0 ? static_cast<int64_t>(blk / p.in_blk_div) * p.in_blk_stride : 0);
-    const uint8_t *in_tile = in_beam + (t0 >> 5) * UB;   // this tile's first unit in every sub-row
+    const int64_t unit_t0 = (t0 >> 5) - (PAIRS ? p.in_unit0 : 0);   // the tile's first unit inside the staged-from rows
+    const uint8_t *in_tile = in_beam + unit_t0 * UB;   // this tile's first unit in every sub-row
     const int64_t col0 = static_cast<int64_t>(blk) * p.nchans_pad + static_cast<int64_t>(group) * p.group_cols;
     const int4 *span_blk = PAIRS ? p.span + static_cast<int64_t>(blk) * p.nchunks * p.rows_per_chunk : p.span + col0;
     const uint2 *rel_blk = static_cast<const uint2 *>(p.rel) + col0 * DB;
@@ -559,7 +561,7 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                             if (LONE && sub == NSUB - 1)   // the lone plane: a quarter of the bytes at a quarter of the offset
                                 tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
                                              in_beam + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes +
-                                                 ((t0 >> 5) * UB + m[k].x) / 4,
+                                                 (unit_t0 * UB + m[k].x) / 4,
                                              static_cast<uint32_t>(m[k].y) / 4u, &full[s]);
                             else
                                 tma_bulk_g2s(raw_base + s * raw_stage + slot * p.raw_slot + sub * p.sub_slot,
@@ -858,14 +860,17 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
 template <int NBITS>
 __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restrict__ in, int64_t in_row_words, int64_t in_units,
                                                          const int4 *__restrict__ prow, uint32_t *__restrict__ out,
-                                                         int64_t out_sub_words, int64_t out_units, int64_t ublocks)
+                                                         int64_t out_sub_words, int64_t out_units, int64_t ublocks, int64_t unit0)
 {
+    // out holds the units unit0 .. unit0 + out_units - 1 of every row (a group of time tiles); out_sub_words is the
+    // pitch of a 4-plane sub-row of the buffer
     constexpr int NBI = Bp<NBITS>::NB, NSUBI = Bp<NBITS>::NSUB;   // input layout: NSUBI sub-rows of NBI planes per unit
     constexpr int NSUBO = NBITS == 2 ? 1 : (NBITS == 4 ? 2 : 3);
     const int64_t blk = blockIdx.x;
-    const int64_t r = blk / ublocks, u = (blk - r * ublocks) * blockDim.x + threadIdx.x;
-    if (u >= out_units)
+    const int64_t r = blk / ublocks, ul = (blk - r * ublocks) * blockDim.x + threadIdx.x;   // unit inside the buffer
+    if (ul >= out_units)
         return;
+    const int64_t u = unit0 + ul;                                                           // unit of the row
     const int4 pr = __ldg(&prow[r]);
     const int64_t in_sub_words = in_row_words / NSUBI;
     uint32_t a[NBITS], b[NBITS];
@@ -896,14 +901,14 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
     }
     sum[NBITS] = cy;
     if constexpr (NBITS == 2) {   // 3 planes per unit, 12 bytes (consecutive threads write consecutive units)
-        uint32_t *o3 = out + r * out_sub_words + u * 3;
+        uint32_t *o3 = out + r * out_sub_words + ul * 3;
         o3[0] = sum[0], o3[1] = sum[1], o3[2] = sum[2];
     } else {                      // sub-rows of 4 planes, then the carry plane alone at 4 bytes per unit
-        uint32_t *o = out + r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + u * 4;
+        uint32_t *o = out + r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + ul * 4;
 #pragma unroll
         for (int q = 0; q < NSUBO - 1; ++q)
             *reinterpret_cast<uint4 *>(o + q * out_sub_words) = make_uint4(sum[4 * q], sum[4 * q + 1], sum[4 * q + 2], sum[4 * q + 3]);
-        out[r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + (NSUBO - 1) * out_sub_words + u] = sum[NBITS];   // the lone carry plane
+        out[r * ((NSUBO - 1) * out_sub_words + out_sub_words / 4) + (NSUBO - 1) * out_sub_words + ul] = sum[NBITS];   // the lone carry plane
     }
 }
 
@@ -911,31 +916,62 @@ __global__ void __launch_bounds__(256) dd_make_pair_rows(const uint32_t *__restr
 template <int NBITS>
 cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t stream)
 {
-    constexpr int ENB = NBITS == 2 ? 3 : (NBITS == 4 ? 8 : 12);   // pair-row layout: 3 planes per unit / 2 x 4 planes (5 in use) / 3 x 4 (9 in use)
+    constexpr int ENB = NBITS == 2 ? 3 : (NBITS == 4 ? 8 : 12);   // pair-row layout: 3 planes per unit / 4 + 1 planes / 4 + 4 + 1
     using C = Bp<ENB>;
+    using CI = Bp<NBITS>;                      // layout of the input bit planes
     constexpr int TB = 32 * 32 * C::W;
-    constexpr int UBO = C::NB * 4;            // bytes per unit of a pair-row sub-row
+    constexpr int UBO = C::NB * 4;             // bytes per unit of a pair-row sub-row
+    constexpr bool LONEL = NBITS != 2;         // last sub-row: the carry plane alone, a quarter of the bytes
     if (!plan->pairs || plan->pair_nbits != ENB || plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB ||
-        kp_in.ngroups != 1 || !plan->d_prow)
+        kp_in.ngroups != 1 || !plan->d_prow || kp_in.out_code == kOutPlanes)
         return cudaErrorInvalidValue;
-    KernelParams kp = kp_in;
+    if (plan->long_mode && kp_in.nchunks % C::FL != 0)
+        return cudaErrorInvalidValue;
+    cudaError_t e;
     int32_t max_delta = 0;
     for (int64_t r = 0; r < plan->n_prows; ++r)
         max_delta = plan->prow[4 * r + 2] > max_delta ? plan->prow[4 * r + 2] : max_delta;
-    // pair rows: as long as the longest span of the tiles needs; input bit planes: that plus the largest difference
-    const int64_t out_units = ((static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + 31) / 32 + 3) / 4 * 4;
-    const int64_t conv_o = out_units * UBO;   // a multiple of 16 bytes (whole groups of 4 units)
-    const int64_t rows_o = plan->n_prows + 1;                               // + the all-zero row of padded entries
-    constexpr bool LONEL = NBITS != 2;                                      // last sub-row: one plane, conv_o / 4 bytes
-    const int64_t pitch_o = LONEL ? (C::NSUB - 1) * conv_o + conv_o / 4 : C::NSUB * conv_o;   // bytes per pair row
-    const int64_t beam_o = rows_o * pitch_o;
-    using CI = Bp<NBITS>;                                                   // layout of the input bit planes
-    const int64_t spg = (16 / (CI::NB * 4)) * 32;                           // input samples per 16-byte group of a sub-row
-    const int64_t groups_i = (out_units * 32 + max_delta + 64 + spg - 1) / spg;
+    // The pair rows are made per beam and per GROUP of time tiles into one of two buffers, on two internal streams that
+    // alternate between groups, so that the rows of one group are built while the other is transformed and the device
+    // memory taken is two groups' worth whatever the number of beams.  A group is the whole time axis unless its rows
+    // would exceed the budget below.  (Groups small enough to keep the rows in L2 -- 1 to 32 tiles on cfg2 -- were
+    // measured: 15.5 ... 9.07 ms against 8.77 ms for one group; the launches fragment the machine more than the saved
+    // DRAM round trip gives back.)
+    const int64_t tile_units = TB / 32;
+    const int64_t extra_units = ((plan->max_span_end + 31) / 32 - tile_units + 3) / 4 * 4;   // span beyond a tile's own units
+    const int64_t rows_o = plan->n_prows + 1;                                                  // + the all-zero row of padded entries
+    auto pitch_of = [&](int64_t units) { return LONEL ? (C::NSUB - 1) * units * UBO + units * UBO / 4 : C::NSUB * units * UBO; };
+    // budget of a group's rows: what the plan already holds, else 75 % of the free device memory (halved when two
+    // groups are alive: several beams, or a time axis that has to be split)
+    int64_t budget = static_cast<int64_t>(plan->pairwork_bytes);
+    {
+        const int64_t whole = rows_o * pitch_of(static_cast<int64_t>(kp_in.ntiles) * tile_units + extra_units);
+        const int64_t want = kp_in.nbeams > 1 ? 2 * whole : whole;
+        if (budget < want) {
+            size_t free_b = 0, total_b = 0;
+            if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) {
+                (void)cudaGetLastError();
+                free_b = size_t(8) << 30;
+            }
+            budget = static_cast<int64_t>((free_b + plan->pairwork_bytes) / 4 * 3);
+        }
+        budget = want <= budget ? whole : budget / 2;
+    }
+    int64_t G = (budget - rows_o * pitch_of(extra_units)) / (rows_o * pitch_of(tile_units));
+    if (const char *envv = std::getenv("DD_PAIR_COLS"))   // test / tuning hook: time tiles per group
+        G = std::atoll(envv);
+    G = G < 1 ? 1 : (G > kp_in.ntiles ? kp_in.ntiles : G);
+    const int64_t units_g = G * tile_units + extra_units, conv_g = units_g * UBO, pitch_g = pitch_of(units_g);
+    const int64_t buf_bytes = rows_o * pitch_g;
+    // input bit planes of the whole call (one transpose), long enough for the last group's rows plus the largest difference
+    const int64_t all_units = static_cast<int64_t>(kp_in.ntiles) * tile_units + extra_units;
+    const int64_t spg = (16 / (CI::NB * 4)) * 32;                            // input samples per 16-byte group of a sub-row
+    const int64_t groups_i = (all_units * 32 + max_delta + 64 + spg - 1) / spg;
     const int64_t conv_i = groups_i * 16, in_units = conv_i / (CI::NB * 4);  // bytes per sub-row, units per row
-    const int64_t beam_i = static_cast<int64_t>(kp.nrows) * CI::NSUB * conv_i;
-    cudaError_t e;
-    const size_t need_i = static_cast<size_t>(kp.nbeams) * beam_i, need_o = static_cast<size_t>(kp.nbeams) * beam_o;
+    const int64_t beam_i = static_cast<int64_t>(kp_in.nrows) * CI::NSUB * conv_i;
+    const int64_t ngroups_all = static_cast<int64_t>(kp_in.nbeams) * ((kp_in.ntiles + G - 1) / G);
+    const int nbuf = ngroups_all >= 2 ? 2 : 1;
+    const size_t need_i = static_cast<size_t>(kp_in.nbeams) * beam_i, need_o = static_cast<size_t>(nbuf) * static_cast<size_t>(buf_bytes);
     if (plan->work_bytes < need_i) {
         if (plan->d_work)
             cudaFree(plan->d_work);
@@ -955,46 +991,86 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
             return e;
         plan->pairwork_bytes = need_o;
     }
-    // the zero row of every beam
-    if ((e = cudaMemset2DAsync(static_cast<uint8_t *>(plan->d_pairwork) + plan->n_prows * pitch_o, static_cast<size_t>(beam_o),
-                               0, static_cast<size_t>(pitch_o), kp.nbeams, stream)) != cudaSuccess)
-        return e;
-    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups_i + 255) / 256), kp.nrows, kp.nbeams), 256, 0, stream>>>(
-        kp.in, kp.in_stride, kp.in_row_bytes, kp.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv_i, beam_i,
+    if (!plan->pair_streams[0]) {
+        cudaStream_t st2[2];
+        cudaEvent_t ev3[3];
+        for (int i = 0; i < 2; ++i)
+            if ((e = cudaStreamCreateWithFlags(&st2[i], cudaStreamNonBlocking)) != cudaSuccess)
+                return e;
+        for (int i = 0; i < 3; ++i)
+            if ((e = cudaEventCreateWithFlags(&ev3[i], cudaEventDisableTiming)) != cudaSuccess)
+                return e;
+        for (int i = 0; i < 2; ++i)
+            plan->pair_streams[i] = st2[i];
+        for (int i = 0; i < 3; ++i)
+            plan->pair_events[i] = ev3[i];
+    }
+    cudaStream_t ws[2] = {static_cast<cudaStream_t>(plan->pair_streams[0]), static_cast<cudaStream_t>(plan->pair_streams[1])};
+    cudaEvent_t fork = static_cast<cudaEvent_t>(plan->pair_events[0]);
+    uint8_t *buf[2] = {static_cast<uint8_t *>(plan->d_pairwork), static_cast<uint8_t *>(plan->d_pairwork) + (nbuf - 1) * buf_bytes};
+
+    dd_to_bitplanes<NBITS><<<dim3(static_cast<unsigned>((groups_i + 255) / 256), kp_in.nrows, kp_in.nbeams), 256, 0, stream>>>(
+        kp_in.in, kp_in.in_stride, kp_in.in_row_bytes, kp_in.in_beam_stride, static_cast<uint8_t *>(plan->d_work), conv_i, beam_i,
         static_cast<int32_t>(groups_i));
     if ((e = cudaGetLastError()) != cudaSuccess)
         return e;
-    const int64_t ublocks = (out_units + 255) / 256;   // (a 4-units-per-thread builder with 16-byte stores measured slower)
-    if (plan->n_prows * ublocks > 0x7FFFFFFFLL)
-        return cudaErrorInvalidConfiguration;
-    for (int b = 0; b < kp.nbeams; ++b) {
-        dd_make_pair_rows<NBITS><<<dim3(static_cast<unsigned>(plan->n_prows * ublocks)), 256, 0, stream>>>(
-            reinterpret_cast<const uint32_t *>(static_cast<const uint8_t *>(plan->d_work) + b * beam_i), CI::NSUB * conv_i / 4, in_units,
-            static_cast<const int4 *>(plan->d_prow), reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(plan->d_pairwork) + b * beam_o),
-            conv_o / 4, out_units, ublocks);
-        if ((e = cudaGetLastError()) != cudaSuccess)
-            return e;
-    }
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
-    kp.in = static_cast<const uint8_t *>(plan->d_pairwork);
-    kp.in_stride = pitch_o;
-    kp.in_blk_stride = 0;
-    kp.in_row_bytes = conv_o;
-    kp.in_beam_stride = beam_o;
-    kp.gpc = 1;
-    kp.rows_per_chunk = plan->rows_per_chunk;
-    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams;
-    if (ctas <= 0 || ctas > 0x7FFFFFFFLL || kp.out_code == kOutPlanes)
-        return cudaErrorInvalidConfiguration;
-    if (plan->long_mode && kp.nchunks % C::FL != 0)
-        return cudaErrorInvalidValue;
+    // fork: both work streams wait for the transpose (and for everything the caller enqueued before)
+    cudaEventRecord(fork, stream);
+    for (int i = 0; i < 2; ++i) {
+        cudaStreamWaitEvent(ws[i], fork, 0);
+        if (i < nbuf && (e = cudaMemsetAsync(buf[i] + plan->n_prows * pitch_g, 0, static_cast<size_t>(pitch_g), ws[i])) != cudaSuccess)
+            return e;   // the zero row
+    }
     auto kernel = plan->long_mode ? dd_direct_bp<ENB, true, NBITS + 1, true> : dd_direct_bp<ENB, false, NBITS + 1, true>;
-    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
-    if (e != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes))) != cudaSuccess)
         return e;
-    kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
-    return cudaGetLastError();
+    const int64_t ublocks = (units_g + 255) / 256;
+    if (plan->n_prows * ublocks > 0x7FFFFFFFLL)
+        return cudaErrorInvalidConfiguration;
+    int launches = 1, it = 0;
+    for (int b = 0; b < kp_in.nbeams; ++b) {
+        for (int64_t c0 = 0; c0 < kp_in.ntiles; c0 += G, ++it) {
+            const int sl = nbuf == 2 ? (it & 1) : 0;
+            const int64_t gc = (c0 + G <= kp_in.ntiles) ? G : kp_in.ntiles - c0;
+            const int64_t unit0 = c0 * tile_units;
+            dd_make_pair_rows<NBITS><<<dim3(static_cast<unsigned>(plan->n_prows * ublocks)), 256, 0, ws[sl]>>>(
+                reinterpret_cast<const uint32_t *>(static_cast<const uint8_t *>(plan->d_work) + b * beam_i), CI::NSUB * conv_i / 4,
+                in_units, static_cast<const int4 *>(plan->d_prow), reinterpret_cast<uint32_t *>(buf[sl]), conv_g / 4, units_g, ublocks,
+                unit0);
+            if ((e = cudaGetLastError()) != cudaSuccess)
+                return e;
+            KernelParams kp = kp_in;
+            kp.in = buf[sl];
+            kp.in_stride = pitch_g;
+            kp.in_blk_stride = 0;
+            kp.in_row_bytes = conv_g;
+            kp.in_beam_stride = 0;
+            kp.out = kp_in.out + static_cast<int64_t>(b) * kp_in.out_beam_stride;
+            kp.nbeams = 1;
+            kp.gpc = 1;
+            kp.rows_per_chunk = plan->rows_per_chunk;
+            kp.tile0 = static_cast<int32_t>(c0);
+            kp.ntiles = static_cast<int32_t>(gc);
+            kp.in_unit0 = unit0;
+            const int64_t ctas = static_cast<int64_t>(kp.nblk) * gc;
+            if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
+                return cudaErrorInvalidConfiguration;
+            kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, ws[sl]>>>(kp);
+            if ((e = cudaGetLastError()) != cudaSuccess)
+                return e;
+            launches += 2;
+        }
+    }
+    // join: the caller's stream continues when both work streams are done
+    for (int i = 0; i < 2; ++i) {
+        cudaEvent_t jn = static_cast<cudaEvent_t>(plan->pair_events[1 + i]);
+        cudaEventRecord(jn, ws[i]);
+        cudaStreamWaitEvent(stream, jn, 0);
+    }
+    plan->pair_launches = launches;
+    return cudaSuccess;
 }
 
 }  // namespace

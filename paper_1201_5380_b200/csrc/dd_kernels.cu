@@ -64,8 +64,8 @@ cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t 
     return cudaErrorInvalidValue;
 }
 
-// bit planes: transpose + transform; pair rows: transpose + one row builder per beam + transform
-int launches_per_execute(const dd_plan_s *plan) { return plan->pairs ? 2 + plan->nbeams : (plan->var.bitplane ? 2 : 1); }
+// bit planes: transpose + transform; pair rows: transpose + (row builder + transform) per group of time tiles
+int launches_per_execute(const dd_plan_s *plan) { return plan->pairs ? plan->pair_launches : (plan->var.bitplane ? 2 : 1); }
 
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
 {

@@ -106,6 +106,9 @@ struct dd_plan_s {
     void *d_prow = nullptr;
     void *d_pairwork = nullptr;           // pair rows as bit planes [n_prows + 1][sub][bytes]; the last row is all zero
     size_t pairwork_bytes = 0;
+    void *pair_streams[2] = {nullptr, nullptr};   // internal streams: groups of time tiles alternate between them
+    void *pair_events[3] = {nullptr, nullptr, nullptr};   // fork, join[2]
+    int pair_launches = 0;                // kernels of the last launch (depends on the number of tile groups)
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
     std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels (nchans_pad = ngroups * group_cols)
