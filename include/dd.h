@@ -259,7 +259,8 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
  *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20);
- *            4 = pair rows (2/4/8-bit, opt-in): the same kernel over rows x[c0] + shift(x[c1], delta) made once per
+ *            4 = pair rows (2/4/8-bit; the default for 4- and 8-bit plans of >= 128 channels): the same kernel
+ *                over rows x[c0] + shift(x[c1], delta) made once per
  *                delay difference delta of every pair of adjacent summed channels -- exact, n + 1 plane words per
  *                pair instead of 2 n; costs device memory for the rows of one beam (16x / 26x / 12x its packed
  *                input on the 2-bit / 4-bit / 8-bit survey-shaped configs; twice that with several beams; the time

@@ -296,6 +296,7 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     scratch.nbits = plan->nbits;
     scratch.ndm = static_cast<int>(dm.size());
     scratch.force_variant = plan->force_variant;
+    scratch.in_planes = plan->in_planes;   // dd_set_input_max: keeps the plan on the plane-skipping kernel
     scratch.dm.swap(dm);
     scratch.keep.swap(keep);
     dd_status st = compute_delay_table(&scratch);
