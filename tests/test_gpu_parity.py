@@ -705,6 +705,28 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
             torch.cuda.synchronize()
             ref = oracle.dedisperse(src.numpy(), cfg.nbits, cfg.nsamps, tab)
             assert np.array_equal(out.cpu().numpy(), ref.astype(np.float32))
+    # the pair-row launcher (8-bit input, >= 128 channels) forks onto internal streams and joins them: capturable too
+    cfg8 = W.CONFIGS[5].reduced(nsamps=3072 + 200, ndm=20, nchans=160, nbeams=2)
+    tab8 = _oracle_table(cfg8)
+    pk8, st8 = W.gen_packed(cfg8, int(tab8.max()))
+    dev8 = pk8.cuda()
+    out8 = torch.zeros((2, cfg8.ndm, cfg8.nsamps), dtype=torch.float32, device="cuda")
+    with dd.Plan(cfg8.nchans, cfg8.dt, cfg8.f_top, cfg8.df, cfg8.nbits) as p:
+        p.set_dm_list(cfg8.dm_list())
+        assert p.launch_info()["variant"] == 4
+        p.set_batch(2, dev8.stride(0), out8.stride(0) * 4)
+        with torch.cuda.stream(side):
+            p.execute(cfg8.nsamps, dev8, st8, out8, 32, side)
+        side.synchronize()
+        g8 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g8, stream=side):
+            p.execute(cfg8.nsamps, dev8, st8, out8, 32, torch.cuda.current_stream())
+        out8.zero_()
+        g8.replay()
+        torch.cuda.synchronize()
+        for b in range(2):
+            ref8 = oracle.dedisperse(pk8[b].numpy(), cfg8.nbits, cfg8.nsamps, tab8)
+            assert np.array_equal(out8[b].cpu().numpy(), ref8.astype(np.float32))
     dms = np.array([0.0, 100.0, 300.0, 900.0])
     with dd.ScrunchSet(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, dms, 8) as s:
         lv = s.levels
