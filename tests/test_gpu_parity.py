@@ -749,3 +749,29 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
         assert len(ref) == len(outs) >= 3
         for o, (F, first, want) in zip(outs, ref):
             assert np.array_equal(o.cpu().numpy(), want.astype(np.float32)), f"factor {F}"
+
+
+@pytest.mark.parametrize("case", [
+    # (config, nchans, ndm, nsamps, keep one channel in ..., expected variant)
+    (5, 512, 40, 3500, 3, 4), (4, 1024, 64, 4000, 4, 4), (5, 300, 1200, 2000, 2, 4), (3, 4096, 32, 1500, 7, 3),
+    (5, 64, 20, 1500, 1, 3),
+])
+def test_default_variant_for_4_and_8_bit_input_under_sparse_kill_masks(case):
+    # 4- and 8-bit plans of >= 128 channels take the pair-row variant by default, also when a sparse kill mask pairs
+    # channels that are far apart; when the pair planner cannot serve the table (cfg3's largest DMs, one channel
+    # in seven kept) or the plan is small, the library falls back to variant 3 -- the result is the same either way
+    idx, nchans, ndm, nsamps, mod, want_variant = case
+    cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=1)
+    dms = W.CONFIGS[3].dm_list()[-32:] if idx == 3 else cfg.dm_list()
+    tab = _oracle_table(cfg, dms)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    mask = (np.arange(nchans) % mod == 0).astype(np.int32)
+    ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, nsamps, tab, mask=mask)
+    out = torch.full((len(dms), nsamps), -1, dtype=torch.int32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        p.set_killmask(mask)
+        assert p.launch_info()["variant"] == want_variant
+        p.execute(nsamps, packed[0].cuda(), stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().view(np.uint32), ref.astype(np.uint32))
