@@ -42,6 +42,9 @@ constexpr int BP_DB = 16, BP_NWARPS = 16;
 
 // Tile shape per input width.  FL = stages between flushes of the pending words in the LONG instantiation
 // (dd_plan.cpp pads the channel list accordingly: kBpFlushStages there must agree).
+#ifndef DD_PAIR_FL
+#define DD_PAIR_FL 4   // stages between flushes of the pair-row kernels (dd_plan.cpp: the same)
+#endif
 #ifndef DD_BP_W2
 #define DD_BP_W2 5     // units per lane of the 2-bit kernel (dd_plan.cpp: the tile is 1024 * DD_BP_W2 samples)
 #endif
@@ -455,12 +458,13 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     constexpr int DB = BP_DB, W = C::W, TB = 32 * 32 * W, CC = C::CC, NSUB = C::NSUB;
     // the short instantiation serves fewer than 8 * CC * FL channels per group: 8-bit sums then fit 16 planes and the
     // epilogue transposes 16 x 16 bit matrices instead of 32 x 32
-    constexpr int NP = (NBITS == 8 && !LONG) ? 16 : C::NP;
+    // (pair rows of 4-bit input: at most 31 per pair and 2114 pairs by plan construction -> 16 planes as well)
+    constexpr int NP = (NBITS == 8 && (!LONG || PAIRS)) ? 16 : C::NP;
     static_assert(LONG || static_cast<int64_t>(8 * CC * C::FL) * ((1 << NBITS) - 1) <= (int64_t(1) << NP), "short-mode sums must fit NP planes");
     static_assert(PIN >= 1 && PIN <= NBITS, "planes in use");
     constexpr int UB = C::NB * 4;                                    // bytes per unit of a sub-row
     constexpr bool LONE = PAIRS && (NBITS == 8 || NBITS == 12);      // the last sub-row holds one plane, 4 bytes per unit
-    constexpr int FL = LONG ? C::FL : 1;
+    constexpr int FL = LONG ? (PAIRS ? DD_PAIR_FL : C::FL) : 1;   // pair rows: flush every DD_PAIR_FL stages (the plan pads alike)
     constexpr bool PATCH = !LONG || (NBITS < 8 && (!PAIRS || NBITS == 3));   // 4-bit pair rows: the ring needs the shared memory more
     constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;        // largest value one stage adds to a counter
     constexpr int NT = bit_length(FL * STAGE_SUM);                   // pending slots
@@ -925,7 +929,7 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     if (!plan->pairs || plan->pair_nbits != ENB || plan->cc != C::CC || plan->var.TB != TB || plan->var.DB != BP_DB ||
         kp_in.ngroups != 1 || !plan->d_prow || kp_in.out_code == kOutPlanes)
         return cudaErrorInvalidValue;
-    if (plan->long_mode && kp_in.nchunks % C::FL != 0)
+    if (plan->long_mode && kp_in.nchunks % DD_PAIR_FL != 0)
         return cudaErrorInvalidValue;
     cudaError_t e;
     int32_t max_delta = 0;

@@ -147,6 +147,9 @@ int64_t smem_layout_bytes(const dd_plan_s *p, int cc)
 }
 
 // Stages between flushes in the LONG bit-plane kernel: must agree with Bp<nbits>::FL (DD_BP_FL*) in dd_kernel_bp.cu.
+#ifndef DD_PAIR_FL
+#define DD_PAIR_FL 4
+#endif
 #ifndef DD_BP_W2
 #define DD_BP_W2 5
 #endif
@@ -206,10 +209,10 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     }
     const int pin = nbits + 1;                          // planes of a pair sum
     const int64_t top = static_cast<int64_t>(npairs) * ((1 << pin) - 1);   // structural weight the counters take
-    if (top >= (int64_t(1) << v.max_sum_bits))
+    if (top >= (int64_t(1) << (nbits == 4 ? 16 : v.max_sum_bits)))   // 4-bit pairs: the kernel keeps 16 sum planes
         return DD_ERR_SMEM;
     const int DB = v.DB, cc = v.cc[0];
-    const int fl = nbits == 2 ? 4 : (nbits == 8 ? 2 : kBpFlushStages(enb));
+    const int fl = DD_PAIR_FL;   // stages between flushes of the pair-row kernels (dd_kernel_bp.cu: the same)
     const int nblk = (ndm + DB - 1) / DB;
     const bool long_mode = npairs >= 8 * cc * fl;
     const int ents_pad = static_cast<int>(align_up(npairs, cc * (long_mode ? fl : 1)));
@@ -377,7 +380,7 @@ dd_status build_tiles(dd_plan_s *p)
     p->pairs = false;
     if (p->force_variant == 4)
         return build_tiles_pairs(p);
-    // Default for 4- and 8-bit input: pair rows (variant 4, 9-17 % faster on cfg3-5), unless the plan sums channel
+    // Default for 4- and 8-bit input: pair rows (variant 4, 15-17 % faster on cfg3-5), unless the plan sums channel
     // groups (sub-band steps), the caller promised small samples (dd_set_input_max: variant 3 then skips planes), or
     // the pair planner cannot serve the table (then variant 3 and the others are tried as before).  2-bit input
     // stays on variant 3: the pair rows gain nothing there.
