@@ -271,6 +271,21 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
 dd_status dd_set_kernel_variant(dd_plan plan, int variant);
 
 /*
+ * dd_set_tuning -- documented launch-geometry knobs for tests and tuning (the library reads no environment
+ * variables).  Results never depend on them.
+ *   key    DD_TUNE_SUBBAND_GPC: sub-bands summed one after the other by a CTA of sub-band step 1;
+ *            0 = chosen by the library.  Takes effect at the next dd_execute.
+ *          DD_TUNE_GROUP_SIZE: channels per group of variant 5 (2 or 4); 0 = chosen by the planner.
+ *          DD_TUNE_GROUPS_PER_STAGE: groups per pipeline stage of variant 5 (one of the compiled shapes: 2-bit 16 / 8
+ *            pairs or 8 / 4 groups of four, 4-bit 8 / 4 or 4 / 2, 8-bit 4 / 2 or 2 / 1); 0 = chosen by the planner.
+ *            Both take effect at the next dd_set_dm_list (DD_ERR_SMEM if no compiled shape matches or fits).
+ *   value  >= 0.
+ * DD_ERR_INVALID_ARG for an unknown key or a negative value.
+ */
+enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3 };
+dd_status dd_set_tuning(dd_plan plan, int key, int value);
+
+/*
  * dd_get_launch_info -- how the plan tiles the problem (for benchmarks and tests).  Host only.
  *   info  HOST out, 8 int64: [0] DMs per CTA (DB), [1] output samples per CTA (TB), [2] channels per
  *         pipeline stage, [3] dynamic shared memory bytes per CTA, [4] threads per CTA, [5] number of DM

@@ -21,7 +21,7 @@ __all__ = [
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
@@ -34,7 +34,7 @@ EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
+    "dd_set_kernel_variant", "dd_set_tuning", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy",
 )
@@ -96,6 +96,8 @@ def lib() -> ctypes.CDLL:
         L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
         L.dd_get_launch_info.argtypes = [vp, vp]
         L.dd_set_kernel_variant.argtypes = [vp, i32]
+        L.dd_set_tuning.argtypes = [vp, i32, i32]
+        L.dd_set_tuning.restype = i32
         L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
         L.dd_profile_enable.argtypes = [vp, i32]
         L.dd_profile_read.argtypes = [vp, ctypes.POINTER(i32), vp, vp]
@@ -256,6 +258,14 @@ def dd_set_kernel_variant(plan: int, variant: int) -> None:
     _check(lib().dd_set_kernel_variant(plan, int(variant)), "dd_set_kernel_variant")
 
 
+DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE = 1, 2, 3
+
+
+def dd_set_tuning(plan: int, key: int, value: int) -> None:
+    """Launch-geometry knobs (include/dd.h); results never depend on them."""
+    _check(lib().dd_set_tuning(plan, int(key), int(value)), "dd_set_tuning")
+
+
 def dd_get_launch_info(plan: int) -> dict:
     info = np.zeros(8, dtype=np.int64)
     _check(lib().dd_get_launch_info(plan, info.ctypes.data), "dd_get_launch_info")
@@ -402,6 +412,10 @@ class Plan:
 
     def set_input_max(self, vmax: int) -> "Plan":
         dd_set_input_max(self.handle, vmax)
+        return self
+
+    def set_tuning(self, key: int, value: int) -> "Plan":
+        dd_set_tuning(self.handle, key, value)
         return self
 
     def set_killmask(self, mask) -> "Plan":

@@ -64,7 +64,9 @@ static void free_device_tables(dd_plan_s *p)
         cudaFree(p->d_zero);
     if (p->d_prow)
         cudaFree(p->d_prow);
-    p->d_span = p->d_rel = p->d_zero = p->d_prow = nullptr;
+    if (p->d_gs_tab)
+        cudaFree(p->d_gs_tab);
+    p->d_span = p->d_rel = p->d_zero = p->d_prow = p->d_gs_tab = nullptr;
     p->uploaded = false;
 }
 
@@ -105,6 +107,14 @@ static dd_status upload_tables(dd_plan_s *p)
             (e = cudaMemcpy(p->d_prow, p->prow.data(), pb, cudaMemcpyHostToDevice)) != cudaSuccess) {
             free_device_tables(p);
             return cuda_fail(e, "cudaMalloc/Memcpy(pair rows)");
+        }
+    }
+    if (p->gs && !p->gs_tab.empty()) {   // variant 5: the build entries of every stage
+        const size_t tb = p->gs_tab.size() * sizeof(GsEntry);
+        if ((e = cudaMalloc(&p->d_gs_tab, tb)) != cudaSuccess ||
+            (e = cudaMemcpy(p->d_gs_tab, p->gs_tab.data(), tb, cudaMemcpyHostToDevice)) != cudaSuccess) {
+            free_device_tables(p);
+            return cuda_fail(e, "cudaMalloc/Memcpy(group-sum table)");
         }
     }
     p->uploaded = true;
@@ -255,8 +265,8 @@ static dd_status execute_subband(dd_plan_s *plan, int64_t nsamps, const void *in
     (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device >= 0 ? plan->device : 0);
     const int64_t ctas1 = static_cast<int64_t>(k1.nblk) * k1.ntiles * nbeams * k1.ngroups;
     int64_t gpc = ctas1 / (8 * static_cast<int64_t>(sms));   // measured on the cfg2 shape: flat from 4 to 16 sub-bands per CTA
-    if (const char *envv = std::getenv("DD_SB_GPC"))   // test hook: groups per CTA
-        gpc = std::atoi(envv);
+    if (plan->sb_gpc > 0)   // dd_set_tuning(DD_TUNE_SUBBAND_GPC)
+        gpc = plan->sb_gpc;
     k1.gpc = static_cast<int32_t>(std::max<int64_t>(1, std::min<int64_t>(gpc, k1.ngroups)));
     s1->prof_mid = nullptr;
     if ((e = launch_direct(s1, k1, st_)) != cudaSuccess)
@@ -297,6 +307,8 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     scratch.ndm = static_cast<int>(dm.size());
     scratch.force_variant = plan->force_variant;
     scratch.in_planes = plan->in_planes;   // dd_set_input_max: keeps the plan on the plane-skipping kernel
+    scratch.gs_force_G = plan->gs_force_G;
+    scratch.gs_force_cc = plan->gs_force_cc;
     scratch.dm.swap(dm);
     scratch.keep.swap(keep);
     dd_status st = compute_delay_table(&scratch);
@@ -358,6 +370,15 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->rows_per_chunk = scratch.rows_per_chunk;
     plan->prow.swap(scratch.prow);
     plan->n_prows = scratch.n_prows;
+    plan->gs = scratch.gs;
+    plan->gs_G = scratch.gs_G;
+    plan->gs_rows = scratch.gs_rows;
+    plan->gs_row_units = scratch.gs_row_units;
+    plan->gs_raw_sub = scratch.gs_raw_sub;
+    plan->gs_nsr = scratch.gs_nsr;
+    plan->gs_nsp = scratch.gs_nsp;
+    plan->gs_patch = scratch.gs_patch;
+    plan->gs_tab.swap(scratch.gs_tab);
     plan->last_launches = 0;
     // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
     int ndev = 0;
@@ -809,10 +830,32 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)
         return DD_ERR_NULL;
-    if (variant < 0 || variant > 4)
+    if (variant < 0 || variant > 5)
         return DD_ERR_INVALID_ARG;
     plan->force_variant = variant;
     return DD_OK;
+}
+
+dd_status dd_set_tuning(dd_plan plan, int key, int value)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (value < 0)
+        return DD_ERR_INVALID_ARG;
+    switch (key) {
+    case DD_TUNE_SUBBAND_GPC:
+        plan->sb_gpc = value;
+        return DD_OK;
+    case DD_TUNE_GROUP_SIZE:
+        if (value != 0 && value != 2 && value != 4)
+            return DD_ERR_INVALID_ARG;
+        plan->gs_force_G = value;
+        return DD_OK;
+    case DD_TUNE_GROUPS_PER_STAGE:
+        plan->gs_force_cc = value;
+        return DD_OK;
+    }
+    return DD_ERR_INVALID_ARG;
 }
 
 dd_status dd_get_launch_info(dd_plan plan, int64_t *info)

@@ -60,6 +60,8 @@ cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t 
         return launch_variant3(plan, kp, stream);
     case 4:
         return launch_variant4(plan, kp, stream);
+    case 5:
+        return launch_variant5(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }

@@ -45,6 +45,14 @@ struct KernelParams {
     int32_t rows_per_chunk;   // pair rows (variant 4): rows staged per stage; span is [nblk][nchunks][rows_per_chunk]
     int32_t tile0;            // pair rows: this launch covers the time tiles tile0 .. tile0 + ntiles - 1 ...
     int64_t in_unit0;         // ... and `in` holds the pair rows from unit in_unit0 (32 samples per unit) on
+    // group sums (variant 5, dd_kernel_gs.cu): span is [nblk][nchunks][channels per stage], rel [nblk][nchunks][cc][DB]
+    const int4 *gs_tab;       // [nblk][nchunks][gs_rows] build entries of 64 bytes each (dd_plan.h: GsEntry)
+    int32_t gs_rows;          // rows built per stage
+    int32_t gs_row_units;     // units (32 samples) per row slot, a multiple of 4
+    int32_t gs_raw_sub;       // bytes per sub-row of a channel slot of the raw stage
+    int32_t gs_nsr, gs_nsp;   // ring depths: raw stages, row stages
+    int32_t gs_nblk32;        // 32-unit blocks per row = ceil(gs_row_units / 32)
+    int32_t gs_magic;         // ceil(65536 / gs_nblk32): item / gs_nblk32 == (item * gs_magic) >> 16 for item < 4096
 };
 
 // Geometry of the bit-plane work buffer of a plan for one launch (dd_kernel_bp.cu).
@@ -67,9 +75,14 @@ cudaError_t launch_variant3(dd_plan_s *plan, const KernelParams &kp, cudaStream_
 // variant 4 launches three kernels: bit-plane transpose, pair rows (one per delay difference of every channel pair),
 // transform over the pair rows.  May grow plan->d_work and plan->d_pairwork.
 cudaError_t launch_variant4(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+// variant 5 (group sums made inside the CTA, dd_kernel_gs.cu): bit-plane transpose, then the transform.
+cudaError_t launch_variant5(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 // Sizes (and grows) plan->d_work for the launch described by kp and keeps its all-zero rows; zero_all: the whole
 // buffer is cleared whenever it is new or its layout changed (for a producer that does not write every unit).
 cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w);
+
+// The bit-plane transpose of the packed input into plan->d_work (geometry w from bp_prepare_work).
+cudaError_t launch_to_bitplanes(dd_plan_s *plan, const KernelParams &kp, const BpWork &w, cudaStream_t stream);
 
 // Time-scrunching of packed rows (dd_scrunch.cu).  out_bytes = bytes of every output row to produce (multiple of 16).
 cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t *in, int64_t in_stride, uint8_t *out,

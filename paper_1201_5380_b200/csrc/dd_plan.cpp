@@ -375,11 +375,253 @@ dd_status build_tiles_pairs(dd_plan_s *p)
     return DD_OK;
 }
 
+int64_t gs_smem_bytes(int nbits, int G, int cc, int rows, int row_units, int raw_sub, int nsr, int nsp, bool patch)
+{
+    const int nsubr = nbits == 8 ? 2 : 1, pin = nbits + (G == 2 ? 1 : 2);
+    int64_t b = 128 + (patch ? 16 * static_cast<int64_t>(kBpPatchBytes) : 0);
+    b += nsp * align_up(static_cast<int64_t>(cc) * 16 * 8, 128);                       // offset entries of the trials
+    b += nsr * align_up(static_cast<int64_t>(rows) * 64, 128);                         // build table
+    b += nsr * align_up(static_cast<int64_t>(G) * cc * nsubr * raw_sub, 128);          // staged bit-plane spans
+    b += nsp * align_up(static_cast<int64_t>(rows) * row_units * 4 * pin, 128);        // rows
+    return b;
+}
+
+// Variant 5 -- group sums made inside the CTA (dd_kernel_gs.cu).  Groups of G adjacent live channels; per (DM block,
+// group) the distinct patterns (delta_1 .. delta_{G-1}), delta_i = delay[d][c_i] - delay[d][c_0], of the block's 16
+// trials; the CTA builds one row R[t] = sum_i x[c_i][t + delta_i] per pattern from the staged spans of the G channels
+// and every trial adds the row of its own pattern at the delay of c_0.  Exact: the delay table is used as it stands.
+dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
+{
+    const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    if (p->group_size > 0 || p->in_planes > 0 || (G != 2 && G != 4) || !gs_instance_exists(nbits, G, cc))
+        return DD_ERR_SMEM;
+    std::vector<int32_t> live;
+    for (int c = 0; c < nrows; ++c)
+        if (p->keep.empty() || p->keep[c])
+            live.push_back(c);
+    const int nlive = static_cast<int>(live.size());
+    if (nlive == 0)
+        return DD_ERR_SMEM;
+    const int W = nbits == 2 ? DD_BP_W2 : 3, TB = 1024 * W, DB = 16;
+    const int nbr = nbits == 2 ? 2 : 4, nsubr = nbits / nbr, ubr = nbr * 4;   // raw layout: planes per unit, sub-rows, bytes per unit
+    const int pin = nbits + (G == 2 ? 1 : 2), np = nbits == 2 ? 12 : (nbits == 4 ? 16 : 20);
+    const int64_t vmax = (1 << nbits) - 1;
+    if (static_cast<int64_t>(nlive) * vmax >= (int64_t(1) << np))
+        return DD_ERR_SMEM;
+    const int ngr = (nlive + G - 1) / G, fl = kGsFlushStages;
+    const int ents_pad = static_cast<int>(align_up(ngr, cc * fl)), nchunks = ents_pad / cc;
+    const int nblk = (ndm + DB - 1) / DB;
+    const int A = 32 * (16 / ubr);   // samples per 16 bytes of a raw sub-row: the bulk-copy granularity
+
+    struct GInfo {
+        int cnt = 0;                 // channels present
+        int32_t ch[4] = {0, 0, 0, 0};
+        int32_t start0 = 0, U = 0;   // first sample of the rows (multiple of 32), units per row
+        int npat = 0;
+        int32_t pat[16][4];          // delay differences per pattern
+        uint8_t pat_of[16];          // pattern of every trial
+        int32_t off[16];             // delay[d][c_0] - start0
+        int32_t rawstart[4], RU[4];  // staged span per channel: first sample, units
+    };
+    auto analyse = [&](int b, int q, GInfo &g) -> bool {
+        g = GInfo();
+        if (q >= ngr) {   // padded group: one all-zero row
+            g.U = TB / 32 + 1;
+            g.npat = 1;
+            for (int i = 0; i < 4; ++i)
+                g.pat[0][i] = 0, g.rawstart[i] = 0, g.RU[i] = 0;
+            for (int i = 0; i < DB; ++i)
+                g.pat_of[i] = 0, g.off[i] = 0;
+            return true;
+        }
+        g.cnt = std::min(G, nlive - q * G);
+        for (int i = 0; i < g.cnt; ++i)
+            g.ch[i] = live[q * G + i];
+        int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0, d0s[16];
+        for (int i = 0; i < DB; ++i) {
+            const int d = std::min(b * DB + i, ndm - 1);   // the last block is padded with its last trial
+            const int32_t *row = p->delay.data() + static_cast<size_t>(d) * nrows;
+            d0s[i] = row[g.ch[0]];
+            dmin = std::min(dmin, d0s[i]);
+            dmax = std::max(dmax, d0s[i]);
+            int32_t dl[4] = {0, 0, 0, 0};
+            for (int k = 1; k < g.cnt; ++k)
+                dl[k] = row[g.ch[k]] - d0s[i];
+            int f = -1;
+            for (int k = 0; k < g.npat && f < 0; ++k)
+                if (std::equal(dl, dl + 4, g.pat[k]))
+                    f = k;
+            if (f < 0) {
+                f = g.npat++;
+                std::copy(dl, dl + 4, g.pat[f]);
+            }
+            g.pat_of[i] = static_cast<uint8_t>(f);
+        }
+        g.start0 = dmin / 32 * 32;
+        if (dmax - g.start0 > (1 << 20))
+            return false;
+        g.U = TB / 32 + (dmax - g.start0) / 32 + 1;
+        for (int i = 0; i < DB; ++i)
+            g.off[i] = d0s[i] - g.start0;
+        for (int k = 0; k < g.cnt; ++k) {
+            int32_t lo = std::numeric_limits<int32_t>::max(), hi = std::numeric_limits<int32_t>::min();
+            for (int j = 0; j < g.npat; ++j) {
+                lo = std::min(lo, g.pat[j][k]);
+                hi = std::max(hi, g.pat[j][k]);
+            }
+            if (g.start0 + lo < 0 || hi - lo > (1 << 20))   // (a difference can be negative only in a table that is not
+                return false;                                //  monotone in c, i.e. never for df < 0; refused all the same)
+            g.rawstart[k] = (g.start0 + lo) / A * A;
+            const int ru = ((g.start0 + hi - g.rawstart[k]) >> 5) + g.U + 1;   // the funnel shift reads one unit further
+            g.RU[k] = static_cast<int32_t>(align_up(ru, 16 / ubr));
+        }
+        return true;
+    };
+
+    // pass 1: sizes
+    int rows = 1, row_units = 0, raw_units = 16 / ubr;
+    int64_t max_end = 0;
+    GInfo g;
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            int rows_here = 0;
+            for (int q = k * cc; q < (k + 1) * cc; ++q) {
+                if (!analyse(b, q, g))
+                    return DD_ERR_SMEM;
+                rows_here += g.npat;
+                row_units = std::max(row_units, g.U);
+                for (int i = 0; i < g.cnt; ++i) {
+                    raw_units = std::max(raw_units, g.RU[i]);
+                    max_end = std::max<int64_t>(max_end, static_cast<int64_t>(g.rawstart[i]) + static_cast<int64_t>(g.RU[i]) * 32);
+                }
+            }
+            rows = std::max(rows, rows_here);
+        }
+    }
+    row_units = static_cast<int>(align_up(row_units, 4));
+    const int raw_sub = raw_units * ubr;
+    max_end = std::max<int64_t>(max_end, static_cast<int64_t>(raw_units) * 32);   // zero-row copies of padded channels
+    if (static_cast<int64_t>(rows) * ((row_units + 31) / 32) >= 4096 || raw_sub > (1 << 19))
+        return DD_ERR_SMEM;
+    // ring depths: the deepest that fits; output patches for 2- and 4-bit input when there is room for them
+    const bool want_patch = nbits < 8;
+    const int cand[6][3] = {{3, 3, 1}, {2, 3, 1}, {3, 3, 0}, {2, 3, 0}, {2, 2, 1}, {2, 2, 0}};
+    int nsr = 0, nsp = 0;
+    bool patch = false;
+    for (const auto &cd : cand) {
+        if (cd[2] && !want_patch)
+            continue;
+        if (gs_smem_bytes(nbits, G, cc, rows, row_units, raw_sub, cd[0], cd[1], cd[2] != 0) <= kMaxDynSmem) {
+            nsr = cd[0], nsp = cd[1], patch = cd[2] != 0;
+            break;
+        }
+    }
+    if (nsr == 0)
+        return DD_ERR_SMEM;
+
+    // pass 2: tables
+    const int CHS = G * cc, row_bytes = row_units * 4 * pin;
+    std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchunks * CHS);
+    std::vector<GsEntry> tab(static_cast<size_t>(nblk) * nchunks * rows);
+    std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nchunks * cc * DB * 8);
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            const size_t st = static_cast<size_t>(b) * nchunks + k;
+            GsEntry *te = tab.data() + st * rows;
+            for (int r = 0; r < rows; ++r)
+                te[r] = GsEntry{};
+            int row_idx = 0;
+            for (int gi = 0; gi < cc; ++gi) {
+                analyse(b, k * cc + gi, g);
+                for (int i = 0; i < G; ++i) {
+                    SpanMeta &m = span[st * CHS + gi * G + i];
+                    if (i < g.cnt)
+                        m = SpanMeta{g.rawstart[i] / 32 * ubr, g.RU[i] * ubr, g.ch[i], 0};
+                    else
+                        m = SpanMeta{0, raw_sub, nrows, 0};   // the all-zero row behind the input rows
+                }
+                for (int j = 0; j < g.npat; ++j) {
+                    GsEntry &e = te[row_idx + j];
+                    e.dst = (row_idx + j) * row_bytes;
+                    e.nunits = g.U;
+                    for (int i = 0; i < G; ++i) {
+                        const int32_t o = i < g.cnt ? g.start0 + g.pat[j][i] - g.rawstart[i] : 0;
+                        e.src[i] = (gi * G + i) * nsubr * raw_sub + (o >> 5) * ubr;
+                        e.sh[i] = o & 31;
+                    }
+                }
+                uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (st * cc + gi) * DB * 2;
+                for (int i = 0; i < DB; ++i) {
+                    const uint32_t off = static_cast<uint32_t>(g.off[i]);
+                    en[2 * i] = static_cast<uint32_t>(row_idx + g.pat_of[i]) * static_cast<uint32_t>(row_bytes);
+                    en[2 * i + 1] = ((off >> 5) << 8) | (off & 31u);
+                }
+                row_idx += g.npat;
+            }
+        }
+    }
+    p->var = Variant{5, DB, TB, 512, 32, 8, nbits, 0, 4, {cc, 0, 0, 0}, 1 << nbits, np, true, true, ubr, nsubr};
+    p->pairs = false;
+    p->gs = true;
+    p->gs_G = G;
+    p->gs_rows = rows;
+    p->gs_row_units = row_units;
+    p->gs_raw_sub = raw_sub;
+    p->gs_nsr = nsr;
+    p->gs_nsp = nsp;
+    p->gs_patch = patch;
+    p->long_mode = true;
+    p->patch = patch;
+    p->max_span_end = max_end;
+    p->sub_slot = raw_sub;
+    p->raw_slot = raw_sub * nsubr;
+    p->lane_slot = p->raw_slot;
+    p->cc = cc;
+    p->nstages = nsr;
+    p->ngroups = 1;
+    p->group_cols = ents_pad;
+    p->nblk = nblk;
+    p->nchans_pad = ents_pad;
+    p->smem_bytes = gs_smem_bytes(nbits, G, cc, rows, row_units, raw_sub, nsr, nsp, patch);
+    p->span.swap(span);
+    p->rel.swap(rel);
+    p->gs_tab.swap(tab);
+    p->live.swap(live);
+    p->nlive = nlive;
+    p->final32 = static_cast<int64_t>(nlive) * vmax > 65535;
+    return DD_OK;
+}
+
+// Variant 5 with the group size and the groups per stage of dd_set_tuning, else the first compiled shape that fits.
+static dd_status build_tiles_gs_auto(dd_plan_s *p)
+{
+    static const int shapes[3][2][2][2] = {
+        /* 2-bit */ {{{2, 16}, {2, 8}}, {{4, 8}, {4, 4}}},
+        /* 4-bit */ {{{2, 8}, {2, 4}}, {{4, 4}, {4, 2}}},
+        /* 8-bit */ {{{2, 4}, {2, 2}}, {{4, 2}, {4, 1}}},
+    };
+    const int wi = p->nbits == 2 ? 0 : (p->nbits == 4 ? 1 : 2);
+    for (int gi = 1; gi >= 0; --gi) {   // groups of four first
+        for (int ci = 0; ci < 2; ++ci) {
+            const int G = shapes[wi][gi][ci][0], cc = shapes[wi][gi][ci][1];
+            if ((p->gs_force_G && p->gs_force_G != G) || (p->gs_force_cc && p->gs_force_cc != cc))
+                continue;
+            if (build_tiles_gs(p, G, cc) == DD_OK)
+                return DD_OK;
+        }
+    }
+    p->gs = false;
+    return DD_ERR_SMEM;
+}
+
 dd_status build_tiles(dd_plan_s *p)
 {
     p->pairs = false;
+    p->gs = false;
     if (p->force_variant == 4)
         return build_tiles_pairs(p);
+    if (p->force_variant == 5)
+        return build_tiles_gs_auto(p);
     // Default for 4- and 8-bit input: pair rows (variant 4, 15-17 % faster on cfg3-5), unless the plan sums channel
     // groups (sub-band steps), the caller promised small samples (dd_set_input_max: variant 3 then skips planes), or
     // the pair planner cannot serve the table (then variant 3 and the others are tried as before).  2-bit input

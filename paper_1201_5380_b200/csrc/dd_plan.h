@@ -45,6 +45,18 @@ struct SpanMeta {   // per (DM block, live channel); mirrored on the device as i
     int32_t pad;
 };
 
+// Variant 5: one row to build in a stage (mirrored on the device as 4 x int4).  Row = sum over the group's channels i
+// of x[c_i][t + delta_i] for one pattern (delta_1 .. delta_{G-1}) of delay differences, over `nunits` units.
+struct GsEntry {
+    int32_t dst;      // byte offset of the row slot inside the row stage
+    int32_t nunits;   // units to build (0: unused entry)
+    int32_t src[4];   // per channel: byte offset, inside the raw stage, of the unit of sub-row 0 that holds the row's first
+                      // sample shifted by delta_i (channel slot + whole units of the offset)
+    int32_t sh[4];    // per channel: the offset's remainder, 0..31 (sh[0] == 0)
+    int32_t pad[6];
+};
+static_assert(sizeof(GsEntry) == 64, "GsEntry is staged as 4 x 16 bytes");
+
 struct HostStage;   // device staging for dd_execute_host (dd_api.cu)
 
 }  // namespace dd
@@ -109,6 +121,19 @@ struct dd_plan_s {
     void *pair_streams[2] = {nullptr, nullptr};   // internal streams: groups of time tiles alternate between them
     void *pair_events[3] = {nullptr, nullptr, nullptr};   // fork, join[2]
     int pair_launches = 0;                // kernels of the last launch (depends on the number of tile groups)
+    // group sums (variant 5): per group of G adjacent live channels and DM block, the CTA itself builds one row per
+    // pattern of delay differences in shared memory; every trial adds the row of its own pattern
+    bool gs = false;
+    int gs_G = 0;                         // channels per group (2 or 4); cc = groups per stage
+    int gs_force_G = 0, gs_force_cc = 0;  // dd_set_tuning: 0 = chosen by the planner
+    int gs_rows = 0;                      // rows built per stage (the largest count of any stage)
+    int gs_row_units = 0;                 // units per row slot
+    int gs_raw_sub = 0;                   // bytes per sub-row of a raw channel slot
+    int gs_nsr = 0, gs_nsp = 0;           // ring depths
+    bool gs_patch = false;                // epilogue through shared-memory patches
+    std::vector<dd::GsEntry> gs_tab;      // [nblk][nchunks][gs_rows]
+    void *d_gs_tab = nullptr;
+    int sb_gpc = 0;                       // dd_set_tuning: sub-bands per CTA of sub-band step 1 (0 = chosen by the library)
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
     std::vector<dd::SpanMeta> span;   // [nblk][nchans_pad] over the live channels (nchans_pad = ngroups * group_cols)
@@ -145,6 +170,12 @@ dd_status build_subband(const dd_plan_s *p, dd_plan_s *s1, dd_plan_s *s2, std::v
 dd_status build_tiles(dd_plan_s *p);
 // Variant 4 (pair rows): 2- and 4-bit input, one channel group.  DD_ERR_SMEM if it cannot serve the plan.
 dd_status build_tiles_pairs(dd_plan_s *p);
+// Variant 5 (group sums in shared memory), G channels per group, cc groups per stage (0 = the default for the width).
+dd_status build_tiles_gs(dd_plan_s *p, int G, int cc);
+// Shared-memory bytes of the variant-5 kernel for this geometry (must match the carve-up in dd_kernel_gs.cu).
+int64_t gs_smem_bytes(int nbits, int G, int cc, int rows, int row_units, int raw_sub, int nsr, int nsp, bool patch);
+bool gs_instance_exists(int nbits, int G, int cc);   // is dd_direct_gs<nbits, G, cc> compiled in?  (dd_kernel_gs.cu)
+constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 
 // Shared-memory bytes the kernel needs for `cc` channels per stage (must match the kernel's carve-up).
 int64_t smem_layout_bytes(const dd_plan_s *p, int cc);
