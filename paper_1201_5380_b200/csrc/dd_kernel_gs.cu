@@ -21,6 +21,7 @@
 // Every warp takes its share of both jobs, in this order per iteration k:
 //   issue the copies of stage k + 1 + DT  |  build its share of the rows of stage k + 1  |  add stage k
 // with full/empty mbarriers per ring slot (no CTA-wide barrier in the loop).
+#include <cstdio>
 #include <utility>
 
 #include "dd_bp_core.cuh"
@@ -29,6 +30,12 @@ namespace dd {
 namespace {
 
 constexpr int GS_DB = 16, GS_NWARPS = 16;
+#ifndef GS_X_SWAP
+#define GS_X_SWAP 1      // the two halves of the CTA build at different points of an iteration
+#endif
+#ifndef GS_X_ILP2
+#define GS_X_ILP2 1      // build items two at a time
+#endif
 constexpr int GS_FL = kGsFlushStages;   // stages between flushes of the pending words
 
 template <int NBITS, int G>
@@ -216,11 +223,12 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
     uint8_t *raw_base = tab_base + NSR * tab_slot;
     uint8_t *row_base = raw_base + NSR * raw_slot;
 
+    constexpr int NBUILD = GS_NWARPS;   // every warp builds its share of the rows of a stage
     if (tid == 0) {
         for (int s = 0; s < 4; ++s) {
             mbar_init(&raw_full[s], GS_NWARPS);
-            mbar_init(&raw_empty[s], GS_NWARPS);
-            mbar_init(&row_full[s], GS_NWARPS);
+            mbar_init(&raw_empty[s], NBUILD);
+            mbar_init(&row_full[s], NBUILD);
             mbar_init(&row_empty[s], GS_NWARPS);
         }
         mbar_fence_init();
@@ -234,53 +242,85 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
     const int4 *tab_blk = p.gs_tab + stage0 * p.gs_rows * 4;
     const uint8_t *rel_blk = static_cast<const uint8_t *>(p.rel) + stage0 * REL_BYTES;
 
+#ifdef GS_X_TIMING
+    uint32_t tm_issue = 0, tm_bwait = 0, tm_build = 0, tm_cwait = 0, tm_add = 0;
+#define GS_TICK(acc, t_) { const uint32_t now_ = clock(); acc += now_ - t_; t_ = now_; }
+#else
+#define GS_TICK(acc, t_)
+#endif
+    // ring position of a chunk: slot = chunk % depth, round = chunk / depth, by multiplication (depth is 2, 3 or 4 at
+    // run time; chunk < 8192 by plan construction), so that no counters are carried through the loop
+    const int magic_r = (65536 + NSR - 1) / NSR, magic_p = (65536 + NSP - 1) / NSP;
+    auto raw_pos = [&](int chunk, int &slot, int &round) {
+        round = (chunk * magic_r) >> 16;
+        slot = chunk - round * NSR;
+    };
+    auto row_pos = [&](int chunk, int &slot, int &round) {
+        round = (chunk * magic_p) >> 16;
+        slot = chunk - round * NSP;
+    };
+
     // ---- copies: every warp's lane 0 issues its share of the spans of a stage (a bulk copy takes uniform operands,
-    // so one warp issuing them all would fall behind); warp 0 also brings the build table
-    int prod_s = 0, prod_round = 0;
+    // so one warp issuing them all would fall behind); warp 0 also brings the build table.  The span entries of the
+    // next stage to issue are fetched one call early.
+    int4 meta[CPW];
+    auto load_meta = [&](int chunk) {
+#pragma unroll
+        for (int k = 0; k < CPW; ++k) {
+            const int i = warp + GS_NWARPS * k;   // copy index: channel slot i / NSUBR, sub-row i % NSUBR
+            meta[k] = (lane == 0 && i < NCOPY && chunk < nchunks) ? __ldg(&span_blk[static_cast<int64_t>(chunk) * CHS + i / C::NSUBR])
+                                                                  : make_int4(0, 0, 0, 0);
+        }
+    };
     auto issue = [&](int chunk) {
-        const int s = prod_s;
+        int s, round;
+        raw_pos(chunk, s, round);
         if (lane == 0) {
-            if (prod_round > 0)
-                mbar_wait(&raw_empty[s], (prod_round - 1) & 1);   // every warp has built its rows of chunk - NSR
-            int4 m[CPW];
+            if (round > 0)
+                mbar_wait(&raw_empty[s], (round - 1) & 1);   // the builders of chunk - NSR are done with the slot
             uint32_t tx = (warp == 0) ? static_cast<uint32_t>(p.gs_rows) * 64u : 0u;
 #pragma unroll
-            for (int k = 0; k < CPW; ++k) {
-                const int i = warp + GS_NWARPS * k;   // copy index: channel slot i / NSUBR, sub-row i % NSUBR
-                m[k] = i < NCOPY ? __ldg(&span_blk[static_cast<int64_t>(chunk) * CHS + i / C::NSUBR]) : make_int4(0, 0, 0, 0);
-                tx += static_cast<uint32_t>(m[k].y);
-            }
+            for (int k = 0; k < CPW; ++k)
+                tx += static_cast<uint32_t>(meta[k].y);
             mbar_arrive_expect_tx(&raw_full[s], tx);
 #pragma unroll
             for (int k = 0; k < CPW; ++k) {
                 const int i = warp + GS_NWARPS * k;
-                if (i < NCOPY && m[k].y > 0) {
+                if (i < NCOPY && meta[k].y > 0) {
                     const int sub = i % C::NSUBR;
                     // span entry: {byte offset inside a sub-row for tile 0, bytes, input row, -}; the work rows are long
                     // enough for every copy, and padded channels point at the all-zero row
                     tma_bulk_g2s(raw_base + s * raw_slot + i * p.gs_raw_sub,
-                                 in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x,
-                                 static_cast<uint32_t>(m[k].y), &raw_full[s]);
+                                 in_tile + static_cast<int64_t>(meta[k].z) * p.in_stride + sub * p.in_row_bytes + meta[k].x,
+                                 static_cast<uint32_t>(meta[k].y), &raw_full[s]);
                 }
             }
             if (warp == 0)
                 tma_bulk_g2s(tab_base + s * tab_slot, tab_blk + static_cast<int64_t>(chunk) * p.gs_rows * 4,
                              static_cast<uint32_t>(p.gs_rows) * 64u, &raw_full[s]);
         }
+        load_meta(chunk + 1);
         __syncwarp();
-        if (++prod_s == NSR) {
-            prod_s = 0;
-            ++prod_round;
-        }
     };
 
-    // ---- build: this warp's share of the rows of a chunk, (row, block of 32 units) items dealt round-robin
-    int bs = 0, bs_round = 0, bp = 0, bp_round = 0;
+    // ---- build: this warp's share of the rows of a chunk; items (row, block of 32 units) are dealt round-robin to the
+    // warps, two at a time for overlap.  The build is a chain of shared-memory round trips with little arithmetic, so
+    // the two halves of the CTA do it at different points of an iteration (see `stage` below): while one half builds,
+    // the other adds.
     const int nitems = p.gs_rows * p.gs_nblk32;
     auto build = [&](int chunk) {
+        int bs, bs_round, bp, bp_round;
+        raw_pos(chunk, bs, bs_round);
+        row_pos(chunk, bp, bp_round);
+#ifdef GS_X_TIMING
+        uint32_t tb = clock();
+#endif
         mbar_wait(&raw_full[bs], bs_round & 1);
         if (bp_round > 0)
             mbar_wait(&row_empty[bp], (bp_round - 1) & 1);   // every warp has added chunk - NSP
+#ifdef GS_X_TIMING
+        tm_bwait += clock() - tb;
+#endif
         if (warp == 0 && lane == 0) {   // the trials' offset entries travel with the row slot
             mbar_expect_tx(&row_full[bp], REL_BYTES);
             tma_bulk_g2s(rel_base + bp * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &row_full[bp]);
@@ -288,32 +328,34 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
         const uint8_t *raw = raw_base + bs * raw_slot;
         uint8_t *row = row_base + bp * row_slot;
         const int4 *tab = reinterpret_cast<const int4 *>(tab_base + bs * tab_slot);
-        for (int it = warp; it < nitems; it += GS_NWARPS) {
+        for (int it = warp; it < nitems; it += (GS_X_ILP2 ? 2 : 1) * NBUILD) {
+            const int it2 = GS_X_ILP2 ? it + NBUILD : nitems;
             const int r = (it * p.gs_magic) >> 16, b32 = it - r * p.gs_nblk32;
-            const int4 e0 = tab[4 * r], e1 = tab[4 * r + 1];
-            int4 e2 = make_int4(0, 0, 0, 0);
-            if constexpr (G == 4)
+            const int r2 = it2 < nitems ? (it2 * p.gs_magic) >> 16 : r, b32b = it2 - r2 * p.gs_nblk32;
+            const int4 e0 = tab[4 * r], e1 = tab[4 * r + 1], f0 = tab[4 * r2], f1 = tab[4 * r2 + 1];
+            int4 e2 = make_int4(0, 0, 0, 0), f2 = make_int4(0, 0, 0, 0);
+            if constexpr (G == 4) {
                 e2 = tab[4 * r + 2];
-            const int u = b32 * 32 + lane;
+                f2 = tab[4 * r2 + 2];
+            }
+            const int u = b32 * 32 + lane, u2 = b32b * 32 + lane;
+#ifndef GS_X_NOBUILD
             if (u < e0.y)
                 gs_build_unit<NBITS, G>(raw, row, e0, e1, e2, u, p.gs_raw_sub, p.gs_row_units);
+            if (it2 < nitems && u2 < f0.y)
+                gs_build_unit<NBITS, G>(raw, row, f0, f1, f2, u2, p.gs_raw_sub, p.gs_row_units);
+#endif
         }
         __syncwarp();
         if (lane == 0) {
             mbar_arrive(&row_full[bp]);
             mbar_arrive(&raw_empty[bs]);
         }
-        if (++bs == NSR) {
-            bs = 0;
-            ++bs_round;
-        }
-        if (++bp == NSP) {
-            bp = 0;
-            ++bp_round;
-        }
     };
 
     const int DT = NSR - 1;   // copies run DT stages ahead of the build
+    const bool early = !GS_X_SWAP || warp < GS_NWARPS / 2;   // this half builds stage k + 1 before it adds stage k, the other half after
+    load_meta(0);
     for (int k = 0; k <= DT && k < nchunks; ++k)
         issue(k);
     build(0);
@@ -329,20 +371,28 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
             T[j][k] = 0;
     }
 
-    int cs = 0;
-    uint32_t cs_parity = 0;
-    // one iteration: keep the copies flowing, build the next stage's rows, add this stage's rows
+    // one iteration: keep the copies flowing, build this warp's share of the next stage's rows, add this stage's rows
     auto stage = [&](int chunk, auto phase, auto flush) {
-        constexpr int PHASE = decltype(phase)::value;
+        constexpr int PHASE = decltype(phase)::value;   // == chunk % 4 (GS_FL == 4)
         constexpr uint32_t FLUSH = decltype(flush)::value;
+#ifdef GS_X_TIMING
+        uint32_t tk = clock();
+#endif
         if (chunk + 1 + DT < nchunks)
             issue(chunk + 1 + DT);
-        if (chunk + 1 < nchunks)
+        GS_TICK(tm_issue, tk)
+        if (early && chunk + 1 < nchunks)
             build(chunk + 1);
-        mbar_wait(&row_full[cs], cs_parity);
+        GS_TICK(tm_build, tk)
+        int cs, cs_round;
+        row_pos(chunk, cs, cs_round);
+        mbar_wait(&row_full[cs], cs_round & 1);
+        GS_TICK(tm_cwait, tk)
+#ifndef GS_X_NOADD
         gs_add_stage<NBITS, G, CC, PHASE>(std::make_integer_sequence<int, CC>{}, row_base + cs * row_slot,
                                           reinterpret_cast<const uint2 *>(rel_base + cs * rel_slot) + warp, lane, p.gs_row_units,
                                           P, T);
+#endif
         if constexpr (FLUSH != 0u) {
 #pragma unroll
             for (int j = 0; j < W; ++j)
@@ -351,10 +401,10 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
         __syncwarp();
         if (lane == 0)
             mbar_arrive(&row_empty[cs]);
-        if (++cs == NSP) {
-            cs = 0;
-            cs_parity ^= 1u;
-        }
+        GS_TICK(tm_add, tk)
+        if (!early && chunk + 1 < nchunks)
+            build(chunk + 1);
+        GS_TICK(tm_build, tk)
     };
     using NoFlush = std::integral_constant<uint32_t, 0u>;
     using FlushAll = std::integral_constant<uint32_t, GS_FL * STAGE_SUM>;
@@ -366,6 +416,11 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
         stage(chunk + 3, std::integral_constant<int, 3>{}, FlushAll{});
     }
 
+#ifdef GS_X_TIMING
+    if (lane == 0 && (cta == 5 || cta == 3000) && (warp == 0 || warp == 6 || warp == 15))
+        printf("cta %d warp %d stages %d: per stage issue %u build(total) %u of which waits %u, wait row_full %u, add %u\n", (int)cta, warp,
+               nchunks, tm_issue / nchunks, tm_build / nchunks, tm_bwait / nchunks, tm_cwait / nchunks, tm_add / nchunks);
+#endif
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp` (as in dd_kernel_bp.cu)
     const int d = blk * DB + warp;
     if (d >= p.ndm)
@@ -427,10 +482,14 @@ cudaError_t launch_gs_inst(dd_plan_s *plan, const KernelParams &kp, cudaStream_t
 }  // namespace
 
 // The instantiations compiled in: {nbits, G, groups per stage}; dd_plan.cpp::build_tiles_gs picks among them.
+#ifdef GS_X_ONLY
+#define DD_GS_INSTANCES(X) X(8, 2, 4)
+#else
 #define DD_GS_INSTANCES(X) \
     X(8, 2, 4) X(8, 2, 2) X(8, 4, 2) X(8, 4, 1) \
     X(4, 2, 8) X(4, 2, 4) X(4, 4, 4) X(4, 4, 2) \
     X(2, 2, 16) X(2, 2, 8) X(2, 4, 8) X(2, 4, 4)
+#endif
 
 bool gs_instance_exists(int nbits, int G, int cc)
 {
