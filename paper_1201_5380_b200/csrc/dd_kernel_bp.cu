@@ -548,7 +548,7 @@ template <int NBITS>
 cudaError_t prepare_bp(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w)
 {
     using C = Bp<NBITS>;
-    constexpr int TB = 32 * 32 * C::W;
+    const int64_t TB = plan->var.TB;   // (variant 5 has its own tile length)
     // 16-byte groups of every sub-row the tiles can touch (2 units of 2-bit input, 1 unit otherwise).  The bit-plane
     // rows are as long as the longest span needs, zero beyond the input, so that the kernel's copies need no
     // clamping; behind the nrows input rows of a beam lie row_mul all-zero rows, the source of padded channels.

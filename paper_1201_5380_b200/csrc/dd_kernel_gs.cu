@@ -15,12 +15,12 @@
 // and the rows never leave the SM (this is the sub-band idea of PAPER.md:311-321 without its approximation, and the
 // paper's "temporal caching" of PAPER.md:115 applied to partial sums).
 //
-// One CTA = 16 trials x 1024 W samples, 16 warps, as in dd_kernel_bp.cu.  Two rings in shared memory:
+// One CTA = 16 trials x 1024 W samples; 16 adder warps (warp = trial) and 4 builder warps.  Two rings in shared memory:
 //   raw ring  : per stage the bit-plane spans of its G * CC channels (TMA bulk copies) and the build table;
-//   row ring  : per stage the rows built from them and the offset entries of the trials.
-// Every warp takes its share of both jobs, in this order per iteration k:
-//   issue the copies of stage k + 1 + DT  |  build its share of the rows of stage k + 1  |  add stage k
-// with full/empty mbarriers per ring slot (no CTA-wide barrier in the loop).
+//   row ring  : per stage the rows built from them and the offset entries of the trials,
+// with full/empty mbarriers per ring slot (no CTA-wide barrier in the loop).  The builder warps copy and build, the
+// adder warps only add (measured with every warp doing all three jobs: per stage and warp ~1000 clocks issuing
+// copies, ~2400 building, ~2600 adding -- the latency chains of the first two stalled the adds).
 #include <cstdio>
 #include <utility>
 
@@ -30,11 +30,8 @@ namespace dd {
 namespace {
 
 constexpr int GS_DB = 16, GS_NWARPS = 16;
-#ifndef GS_X_SWAP
-#define GS_X_SWAP 1      // the two halves of the CTA build at different points of an iteration
-#endif
-#ifndef GS_X_ILP2
-#define GS_X_ILP2 1      // build items two at a time
+#ifndef GS_ILP
+#define GS_ILP 2         // items a builder warp takes at a time (their dependency chains interleave)
 #endif
 constexpr int GS_FL = kGsFlushStages;   // stages between flushes of the pending words
 
@@ -49,9 +46,26 @@ struct Gs {
     static constexpr int WF = PIN < 4 ? 2 : 4;          // planes per unit of the full sub-rows of a row
     static constexpr int NF = PIN / WF;                 // full sub-rows
     static constexpr int RW = PIN - NF * WF;            // planes of the last, narrower sub-row (0: none)
-    static constexpr int W = NBITS == 2 ? 5 : 3;        // units per lane
+    static constexpr int W = NBITS == 2 ? kGsW2 : kGsW48;   // units per lane (16 adder + 4 builder warps: 96 registers per thread)
     static constexpr int NP = NBITS == 2 ? 12 : (NBITS == 4 ? 16 : 20);   // sum planes
+    // Row layout in shared memory.  With W odd the lanes of a warp (W units apart) fall into distinct banks when the units
+    // of a sub-row lie one after the other.  With W = 2 they would collide two by two, so the units of a sub-row are
+    // DE-INTERLEAVED: even units in one array, odd units in a second array row_units / 2 units further -- a lane's units
+    // base + 2 l + {0, 1, 2} are then {A_p[h + l], A_(1-p)[h + p + l], A_p[h + l + 1]} (p = base & 1, h = base >> 1) and
+    // consecutive lanes read consecutive units of one array: no conflicts (measured without: the adds ran at the speed
+    // of the shared-memory pipe, every LDS.128 taking two passes).
+    static constexpr int DI = (W % 2 == 0) ? 2 : 1;
+    static_assert(W % 2 == 1 || W == 2, "even W: only the two-array layout is written out");
 };
+// position (in units) of unit u inside a sub-row of row_units units
+template <int DI>
+__device__ __forceinline__ int gs_unit_pos(int u, int row_units)
+{
+    if constexpr (DI == 2)
+        return (u & 1) * (row_units >> 1) + (u >> 1);
+    else
+        return u;
+}
 
 // ------------------------------------------------------------------------------------------ builder
 // One unit (32 samples) of one row: sum over the group's channels of the staged planes, channel i read at the bit
@@ -102,16 +116,17 @@ __device__ __forceinline__ void gs_build_unit(const uint8_t *raw, uint8_t *row, 
         o[NBITS + 1] = (c01 & c23) | (cs & (c01 ^ c23));
     }
     // row layout: NF sub-rows of WF planes per unit, then one sub-row of RW planes per unit
+    const int up = gs_unit_pos<C::DI>(u, row_units);
 #pragma unroll
     for (int s = 0; s < C::NF; ++s) {
-        uint8_t *q = row + e0.x + row_units * (4 * C::WF) * s + u * (4 * C::WF);
+        uint8_t *q = row + e0.x + row_units * (4 * C::WF) * s + up * (4 * C::WF);
         if constexpr (C::WF == 4)
             *reinterpret_cast<uint4 *>(q) = make_uint4(o[4 * s], o[4 * s + 1], o[4 * s + 2], o[4 * s + 3]);
         else
             *reinterpret_cast<uint2 *>(q) = make_uint2(o[2 * s], o[2 * s + 1]);
     }
     if constexpr (C::RW > 0) {
-        uint8_t *q = row + e0.x + row_units * (4 * C::WF) * C::NF + u * (4 * C::RW);
+        uint8_t *q = row + e0.x + row_units * (4 * C::WF) * C::NF + up * (4 * C::RW);
         if constexpr (C::RW == 1)
             *reinterpret_cast<uint32_t *>(q) = o[C::NF * C::WF];
         else
@@ -136,41 +151,51 @@ __device__ __forceinline__ void gs_add_planes(const PlaneVec<NW> (&x)[Gs<NBITS, 
     }
 }
 
-// W + 1 units loaded for W units, per unit and plane one funnel shift + carry-save adds
+// W + 1 units loaded for W units, per unit and plane one funnel shift + carry-save adds.  sub: the sub-row of this row;
+// v0, v1: positions (in units) of the lane's first and second unit inside it (DI == 1: v1 unused, units are consecutive)
 template <int NBITS, int G, int CLS, int L0, int NW, int NP, int NT>
-__device__ __forceinline__ void gs_add_subrow(const uint8_t *q, uint32_t shift, uint32_t (&P)[Gs<NBITS, G>::W][NP],
-                                              uint32_t (&T)[Gs<NBITS, G>::W][NT])
+__device__ __forceinline__ void gs_add_subrow(const uint8_t *sub, int v0, int v1, uint32_t shift,
+                                              uint32_t (&P)[Gs<NBITS, G>::W][NP], uint32_t (&T)[Gs<NBITS, G>::W][NT])
 {
     using C = Gs<NBITS, G>;
     PlaneVec<NW> x[C::W + 1];
+    if constexpr (C::DI == 2) {
+        x[0].load(sub + v0 * (4 * NW));
+        x[1].load(sub + v1 * (4 * NW));
+        x[2].load(sub + v0 * (4 * NW) + 4 * NW);
+    } else {
 #pragma unroll
-    for (int j = 0; j <= C::W; ++j)
-        x[j].load(q + j * (4 * NW));
+        for (int j = 0; j <= C::W; ++j)
+            x[j].load(sub + v0 * (4 * NW) + j * (4 * NW));
+    }
     gs_add_planes<NBITS, G, CLS, L0, NW, 0>(x, shift, P, T);
 }
 
 template <int NBITS, int G, int CLS, int S_, int NP, int NT>
-__device__ __forceinline__ void gs_add_full(const uint8_t *rowq, int ui, int row_units, uint32_t shift,
+__device__ __forceinline__ void gs_add_full(const uint8_t *rowq, int v0, int v1, int row_units, uint32_t shift,
                                             uint32_t (&P)[Gs<NBITS, G>::W][NP], uint32_t (&T)[Gs<NBITS, G>::W][NT])
 {
     using C = Gs<NBITS, G>;
     if constexpr (S_ < C::NF) {
-        gs_add_subrow<NBITS, G, CLS, S_ * C::WF, C::WF>(rowq + row_units * (4 * C::WF) * S_ + ui * (4 * C::WF), shift, P, T);
-        gs_add_full<NBITS, G, CLS, S_ + 1>(rowq, ui, row_units, shift, P, T);
+        gs_add_subrow<NBITS, G, CLS, S_ * C::WF, C::WF>(rowq + row_units * (4 * C::WF) * S_, v0, v1, shift, P, T);
+        gs_add_full<NBITS, G, CLS, S_ + 1>(rowq, v0, v1, row_units, shift, P, T);
     }
 }
 
-// one group of the stage for this warp's trial: e = {byte offset of the row slot, (unit offset << 8) | bit shift}
+// one group of the stage for this warp's trial: e = {byte offset of the row slot, bit shift | v0 << 8 | v1 << 20} with
+// v0, v1 the positions of the trial's first and second unit in a sub-row (DI == 1: v0 = the unit offset, v1 = 0)
 template <int NBITS, int G, int CLS, int NP, int NT>
 __device__ __forceinline__ void gs_add_group(const uint8_t *row_stage, const uint2 e, int lane, int row_units,
                                              uint32_t (&P)[Gs<NBITS, G>::W][NP], uint32_t (&T)[Gs<NBITS, G>::W][NT])
 {
     using C = Gs<NBITS, G>;
     const uint8_t *rowq = row_stage + e.x;
-    const int ui = static_cast<int>(e.y >> 8) + C::W * lane;
-    gs_add_full<NBITS, G, CLS, 0>(rowq, ui, row_units, e.y, P, T);
+    // lane l owns the units base + W l + j: with two arrays that is l positions further in both
+    const int v0 = static_cast<int>((e.y >> 8) & 0xFFFu) + (C::DI == 2 ? lane : C::W * lane);
+    const int v1 = static_cast<int>(e.y >> 20) + lane;
+    gs_add_full<NBITS, G, CLS, 0>(rowq, v0, v1, row_units, e.y, P, T);
     if constexpr (C::RW > 0)
-        gs_add_subrow<NBITS, G, CLS, C::NF * C::WF, C::RW>(rowq + row_units * (4 * C::WF) * C::NF + ui * (4 * C::RW), e.y, P, T);
+        gs_add_subrow<NBITS, G, CLS, C::NF * C::WF, C::RW>(rowq + row_units * (4 * C::WF) * C::NF, v0, v1, e.y, P, T);
 }
 
 template <int NBITS, int G, int CC, int PHASE, int NP, int NT, int... GIs>
@@ -182,18 +207,23 @@ __device__ __forceinline__ void gs_add_stage(std::integer_sequence<int, GIs...>,
 }
 
 // ------------------------------------------------------------------------------------------ the kernel
-// PATCH: the epilogue passes through per-warp shared-memory patches (whole 128-byte lines per store instruction)
-template <int NBITS, int G, int CC, bool PATCH>
-__global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelParams p)
+// Warps 0 .. 15 ADD: warp w owns trial w of the DM block, lane l the units W l .. W l + W - 1; per stage they wait for
+// the rows, add them, and release the slot -- nothing else.  Warps 16 .. 16 + NBW - 1 BUILD: they issue the bulk
+// copies of the spans (and of the build table and the trials' offset entries) DT stages ahead, and build the rows of
+// a stage as soon as its spans have landed and a row slot is free.  The latency chains of copying and building
+// (mbarrier round trips, dependent shared-memory loads, ripple carries) thus run beside the adders instead of in them.
+// PATCH: the epilogue passes through per-warp shared-memory patches (whole 128-byte lines per store instruction).
+template <int NBITS, int G, int CC, int NBW, bool PATCH>
+__global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const KernelParams p)
 {
     using C = Gs<NBITS, G>;
     constexpr int DB = GS_DB, W = C::W, TB = 32 * 32 * W, NP = C::NP, PIN = C::PIN;
     constexpr int CHS = G * CC;                                     // channels per stage
     constexpr int NCOPY = CHS * C::NSUBR;                           // bulk copies of spans per stage
-    constexpr int CPW = (NCOPY + GS_NWARPS - 1) / GS_NWARPS;        // ... per warp
     constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;         // weight one stage adds to a counter
     constexpr int NT = bit_length(GS_FL * STAGE_SUM);               // pending slots
     constexpr uint32_t REL_BYTES = CC * DB * 8;
+    static_assert(NCOPY + 2 <= 32 * NBW, "one lane per bulk copy");
 
     extern __shared__ __align__(128) uint8_t smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -223,143 +253,131 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
     uint8_t *raw_base = tab_base + NSR * tab_slot;
     uint8_t *row_base = raw_base + NSR * raw_slot;
 
-    constexpr int NBUILD = GS_NWARPS;   // every warp builds its share of the rows of a stage
     if (tid == 0) {
         for (int s = 0; s < 4; ++s) {
-            mbar_init(&raw_full[s], GS_NWARPS);
-            mbar_init(&raw_empty[s], NBUILD);
-            mbar_init(&row_full[s], NBUILD);
+            mbar_init(&raw_full[s], NBW);
+            mbar_init(&raw_empty[s], NBW);
+            mbar_init(&row_full[s], NBW);
             mbar_init(&row_empty[s], GS_NWARPS);
         }
         mbar_fence_init();
     }
-    __syncthreads();
+    __syncthreads();   // the only CTA-wide barrier: builders and adders part ways below
 
-    const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
-    const uint8_t *in_tile = in_beam + (t0 >> 5) * C::UBR;   // this tile's first unit in every sub-row
-    const int64_t stage0 = static_cast<int64_t>(blk) * nchunks;
-    const int4 *span_blk = p.span + stage0 * CHS;
-    const int4 *tab_blk = p.gs_tab + stage0 * p.gs_rows * 4;
-    const uint8_t *rel_blk = static_cast<const uint8_t *>(p.rel) + stage0 * REL_BYTES;
-
+    if (warp >= GS_NWARPS) {
+        // ================================================================== builders
+        const int bw = warp - GS_NWARPS;
+        const uint8_t *in_beam = p.in + static_cast<int64_t>(beam) * p.in_beam_stride;
+        const uint8_t *in_tile = in_beam + (t0 >> 5) * C::UBR;   // this tile's first unit in every sub-row
+        const int64_t stage0 = static_cast<int64_t>(blk) * nchunks;
+        const int4 *span_blk = p.span + stage0 * CHS;
+        const int4 *tab_blk = p.gs_tab + stage0 * p.gs_rows * 4;
+        const uint8_t *rel_blk = static_cast<const uint8_t *>(p.rel) + stage0 * REL_BYTES;
+        // Copies: lane i of builder warp bw issues copy bw + NBW i -- the spans 0 .. NCOPY - 1 (channel slot / NSUBR, sub-row
+        // % NSUBR), then the build table.  Bulk copies take uniform operands, so the lanes of a warp issue theirs one
+        // after the other (measured: ~300 clocks per copy; one warp issuing all 17 copies of a stage in turn with the
+        // others was slower still -- ~7000 clocks per turn), hence the copies of a stage are spread over all builder warps.
+        const int ci = bw + NBW * lane;
+        auto load_meta = [&](int chunk) -> int4 {
+            return (ci < NCOPY && chunk < nchunks) ? __ldg(&span_blk[static_cast<int64_t>(chunk) * CHS + ci / C::NSUBR])
+                                                   : make_int4(0, 0, 0, 0);
+        };
+        int is = 0, iround = 0;   // ring position of the next chunk to copy
+        int4 meta = load_meta(0);
+        auto issue = [&](int chunk) {
+            if (iround > 0)
+                mbar_wait(&raw_empty[is], (iround - 1) & 1);   // the builders are done with chunk - NSR
+            const uint32_t bytes = ci < NCOPY ? static_cast<uint32_t>(meta.y) : (ci == NCOPY ? static_cast<uint32_t>(p.gs_rows) * 64u : 0u);
+            const uint32_t tx = __reduce_add_sync(0xFFFFFFFFu, bytes);
+            if (lane == 0)
+                mbar_arrive_expect_tx(&raw_full[is], tx);
+            __syncwarp();
+            if (ci < NCOPY) {
+                // span entry: {byte offset inside a sub-row for tile 0, bytes, input row, -}; the work rows are long enough
+                // for every copy, and padded channels point at the all-zero row
+                if (meta.y > 0)
+                    tma_bulk_g2s(raw_base + is * raw_slot + ci * p.gs_raw_sub,
+                                 in_tile + static_cast<int64_t>(meta.z) * p.in_stride + (ci % C::NSUBR) * p.in_row_bytes + meta.x,
+                                 static_cast<uint32_t>(meta.y), &raw_full[is]);
+            } else if (ci == NCOPY) {
+                tma_bulk_g2s(tab_base + is * tab_slot, tab_blk + static_cast<int64_t>(chunk) * p.gs_rows * 4, bytes, &raw_full[is]);
+            }
+            meta = load_meta(chunk + 1);
+            if (++is == NSR) {
+                is = 0;
+                ++iround;
+            }
+        };
+        const int DT = NSR - 1;   // copies run DT stages ahead of the build
+        for (int k = 0; k < DT && k < nchunks; ++k)
+            issue(k);
+        int bs = 0, bs_round = 0, bp = 0, bp_round = 0;
 #ifdef GS_X_TIMING
-    uint32_t tm_issue = 0, tm_bwait = 0, tm_build = 0, tm_cwait = 0, tm_add = 0;
-#define GS_TICK(acc, t_) { const uint32_t now_ = clock(); acc += now_ - t_; t_ = now_; }
+        uint32_t tm_issue = 0, tm_wraw = 0, tm_wrow = 0, tm_items = 0, tk = clock();
+#define GS_TICK(acc) { const uint32_t now_ = clock(); acc += now_ - tk; tk = now_; }
 #else
-#define GS_TICK(acc, t_)
+#define GS_TICK(acc)
 #endif
-    // ring position of a chunk: slot = chunk % depth, round = chunk / depth, by multiplication (depth is 2, 3 or 4 at
-    // run time; chunk < 8192 by plan construction), so that no counters are carried through the loop
-    const int magic_r = (65536 + NSR - 1) / NSR, magic_p = (65536 + NSP - 1) / NSP;
-    auto raw_pos = [&](int chunk, int &slot, int &round) {
-        round = (chunk * magic_r) >> 16;
-        slot = chunk - round * NSR;
-    };
-    auto row_pos = [&](int chunk, int &slot, int &round) {
-        round = (chunk * magic_p) >> 16;
-        slot = chunk - round * NSP;
-    };
-
-    // ---- copies: every warp's lane 0 issues its share of the spans of a stage (a bulk copy takes uniform operands,
-    // so one warp issuing them all would fall behind); warp 0 also brings the build table.  The span entries of the
-    // next stage to issue are fetched one call early.
-    int4 meta[CPW];
-    auto load_meta = [&](int chunk) {
+        for (int chunk = 0; chunk < nchunks; ++chunk) {
+            if (chunk + DT < nchunks)
+                issue(chunk + DT);
+            GS_TICK(tm_issue)
+            mbar_wait(&raw_full[bs], bs_round & 1);
+            GS_TICK(tm_wraw)
+            if (bp_round > 0)
+                mbar_wait(&row_empty[bp], (bp_round - 1) & 1);   // every adder is done with chunk - NSP
+            GS_TICK(tm_wrow)
+            if (bw == 0 && lane == 0) {   // the trials' offset entries travel with the row slot
+                mbar_expect_tx(&row_full[bp], REL_BYTES);
+                tma_bulk_g2s(rel_base + bp * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &row_full[bp]);
+            }
+            const uint8_t *raw = raw_base + bs * raw_slot;
+            uint8_t *row = row_base + bp * row_slot;
+            const int4 *tab = reinterpret_cast<const int4 *>(tab_base + bs * tab_slot);
+            // items (row, block of 32 units) of the rows in use, dealt round-robin to the builder warps and taken GS_ILP at a
+            // time without branches (a lane past the end of a row redoes the row's last unit, a missing item redoes the
+            // first), so that their dependency chains interleave
+            const int nitems = tab[3].w * p.gs_nblk32;   // GsEntry::pad[5] of entry 0: rows in use in this stage
+            for (int it0 = bw; it0 < nitems; it0 += GS_ILP * NBW) {
+                int4 e0[GS_ILP], e1[GS_ILP], e2[GS_ILP];
+                int u[GS_ILP];
 #pragma unroll
-        for (int k = 0; k < CPW; ++k) {
-            const int i = warp + GS_NWARPS * k;   // copy index: channel slot i / NSUBR, sub-row i % NSUBR
-            meta[k] = (lane == 0 && i < NCOPY && chunk < nchunks) ? __ldg(&span_blk[static_cast<int64_t>(chunk) * CHS + i / C::NSUBR])
-                                                                  : make_int4(0, 0, 0, 0);
-        }
-    };
-    auto issue = [&](int chunk) {
-        int s, round;
-        raw_pos(chunk, s, round);
-        if (lane == 0) {
-            if (round > 0)
-                mbar_wait(&raw_empty[s], (round - 1) & 1);   // the builders of chunk - NSR are done with the slot
-            uint32_t tx = (warp == 0) ? static_cast<uint32_t>(p.gs_rows) * 64u : 0u;
-#pragma unroll
-            for (int k = 0; k < CPW; ++k)
-                tx += static_cast<uint32_t>(meta[k].y);
-            mbar_arrive_expect_tx(&raw_full[s], tx);
-#pragma unroll
-            for (int k = 0; k < CPW; ++k) {
-                const int i = warp + GS_NWARPS * k;
-                if (i < NCOPY && meta[k].y > 0) {
-                    const int sub = i % C::NSUBR;
-                    // span entry: {byte offset inside a sub-row for tile 0, bytes, input row, -}; the work rows are long
-                    // enough for every copy, and padded channels point at the all-zero row
-                    tma_bulk_g2s(raw_base + s * raw_slot + i * p.gs_raw_sub,
-                                 in_tile + static_cast<int64_t>(meta[k].z) * p.in_stride + sub * p.in_row_bytes + meta[k].x,
-                                 static_cast<uint32_t>(meta[k].y), &raw_full[s]);
+                for (int q = 0; q < GS_ILP; ++q) {
+                    const int it = it0 + q * NBW < nitems ? it0 + q * NBW : it0;
+                    const int r = (it * p.gs_magic) >> 16;
+                    e0[q] = tab[4 * r];
+                    e1[q] = tab[4 * r + 1];
+                    e2[q] = G == 4 ? tab[4 * r + 2] : make_int4(0, 0, 0, 0);
+                    u[q] = min((it - r * p.gs_nblk32) * 32 + lane, e0[q].y - 1);
                 }
+#pragma unroll
+                for (int q = 0; q < GS_ILP; ++q)
+                    gs_build_unit<NBITS, G>(raw, row, e0[q], e1[q], e2[q], u[q], p.gs_raw_sub, p.gs_row_units);
             }
-            if (warp == 0)
-                tma_bulk_g2s(tab_base + s * tab_slot, tab_blk + static_cast<int64_t>(chunk) * p.gs_rows * 4,
-                             static_cast<uint32_t>(p.gs_rows) * 64u, &raw_full[s]);
-        }
-        load_meta(chunk + 1);
-        __syncwarp();
-    };
-
-    // ---- build: this warp's share of the rows of a chunk; items (row, block of 32 units) are dealt round-robin to the
-    // warps, two at a time for overlap.  The build is a chain of shared-memory round trips with little arithmetic, so
-    // the two halves of the CTA do it at different points of an iteration (see `stage` below): while one half builds,
-    // the other adds.
-    const int nitems = p.gs_rows * p.gs_nblk32;
-    auto build = [&](int chunk) {
-        int bs, bs_round, bp, bp_round;
-        raw_pos(chunk, bs, bs_round);
-        row_pos(chunk, bp, bp_round);
-#ifdef GS_X_TIMING
-        uint32_t tb = clock();
-#endif
-        mbar_wait(&raw_full[bs], bs_round & 1);
-        if (bp_round > 0)
-            mbar_wait(&row_empty[bp], (bp_round - 1) & 1);   // every warp has added chunk - NSP
-#ifdef GS_X_TIMING
-        tm_bwait += clock() - tb;
-#endif
-        if (warp == 0 && lane == 0) {   // the trials' offset entries travel with the row slot
-            mbar_expect_tx(&row_full[bp], REL_BYTES);
-            tma_bulk_g2s(rel_base + bp * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &row_full[bp]);
-        }
-        const uint8_t *raw = raw_base + bs * raw_slot;
-        uint8_t *row = row_base + bp * row_slot;
-        const int4 *tab = reinterpret_cast<const int4 *>(tab_base + bs * tab_slot);
-        for (int it = warp; it < nitems; it += (GS_X_ILP2 ? 2 : 1) * NBUILD) {
-            const int it2 = GS_X_ILP2 ? it + NBUILD : nitems;
-            const int r = (it * p.gs_magic) >> 16, b32 = it - r * p.gs_nblk32;
-            const int r2 = it2 < nitems ? (it2 * p.gs_magic) >> 16 : r, b32b = it2 - r2 * p.gs_nblk32;
-            const int4 e0 = tab[4 * r], e1 = tab[4 * r + 1], f0 = tab[4 * r2], f1 = tab[4 * r2 + 1];
-            int4 e2 = make_int4(0, 0, 0, 0), f2 = make_int4(0, 0, 0, 0);
-            if constexpr (G == 4) {
-                e2 = tab[4 * r + 2];
-                f2 = tab[4 * r2 + 2];
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&row_full[bp]);
+                mbar_arrive(&raw_empty[bs]);
             }
-            const int u = b32 * 32 + lane, u2 = b32b * 32 + lane;
-#ifndef GS_X_NOBUILD
-            if (u < e0.y)
-                gs_build_unit<NBITS, G>(raw, row, e0, e1, e2, u, p.gs_raw_sub, p.gs_row_units);
-            if (it2 < nitems && u2 < f0.y)
-                gs_build_unit<NBITS, G>(raw, row, f0, f1, f2, u2, p.gs_raw_sub, p.gs_row_units);
+            if (++bs == NSR) {
+                bs = 0;
+                ++bs_round;
+            }
+            if (++bp == NSP) {
+                bp = 0;
+                ++bp_round;
+            }
+            GS_TICK(tm_items)
+        }
+#ifdef GS_X_TIMING
+        if (lane == 0 && (cta == 5 || cta == 3000) && (bw == 0 || bw == 3))
+            printf("cta %d builder %d stages %d: per stage issue %u wait raw_full %u wait row_empty %u items %u\n", (int)cta, bw, nchunks,
+                   tm_issue / nchunks, tm_wraw / nchunks, tm_wrow / nchunks, tm_items / nchunks);
 #endif
-        }
-        __syncwarp();
-        if (lane == 0) {
-            mbar_arrive(&row_full[bp]);
-            mbar_arrive(&raw_empty[bs]);
-        }
-    };
+        return;
+    }
 
-    const int DT = NSR - 1;   // copies run DT stages ahead of the build
-    const bool early = !GS_X_SWAP || warp < GS_NWARPS / 2;   // this half builds stage k + 1 before it adds stage k, the other half after
-    load_meta(0);
-    for (int k = 0; k <= DT && k < nchunks; ++k)
-        issue(k);
-    build(0);
-
+    // ====================================================================== adders
     uint32_t P[W][NP], T[W][NT];
 #pragma unroll
     for (int j = 0; j < W; ++j) {
@@ -370,29 +388,21 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
         for (int k = 0; k < NT; ++k)
             T[j][k] = 0;
     }
-
-    // one iteration: keep the copies flowing, build this warp's share of the next stage's rows, add this stage's rows
-    auto stage = [&](int chunk, auto phase, auto flush) {
-        constexpr int PHASE = decltype(phase)::value;   // == chunk % 4 (GS_FL == 4)
-        constexpr uint32_t FLUSH = decltype(flush)::value;
+    int cs = 0;
+    uint32_t cs_parity = 0;
 #ifdef GS_X_TIMING
-        uint32_t tk = clock();
+    uint32_t tm_wait = 0, tm_add = 0, tka = clock();
 #endif
-        if (chunk + 1 + DT < nchunks)
-            issue(chunk + 1 + DT);
-        GS_TICK(tm_issue, tk)
-        if (early && chunk + 1 < nchunks)
-            build(chunk + 1);
-        GS_TICK(tm_build, tk)
-        int cs, cs_round;
-        row_pos(chunk, cs, cs_round);
-        mbar_wait(&row_full[cs], cs_round & 1);
-        GS_TICK(tm_cwait, tk)
-#ifndef GS_X_NOADD
+    auto stage = [&](auto phase, auto flush) {
+        constexpr int PHASE = decltype(phase)::value;
+        constexpr uint32_t FLUSH = decltype(flush)::value;
+        mbar_wait(&row_full[cs], cs_parity);
+#ifdef GS_X_TIMING
+        { const uint32_t n_ = clock(); tm_wait += n_ - tka; tka = n_; }
+#endif
         gs_add_stage<NBITS, G, CC, PHASE>(std::make_integer_sequence<int, CC>{}, row_base + cs * row_slot,
                                           reinterpret_cast<const uint2 *>(rel_base + cs * rel_slot) + warp, lane, p.gs_row_units,
                                           P, T);
-#endif
         if constexpr (FLUSH != 0u) {
 #pragma unroll
             for (int j = 0; j < W; ++j)
@@ -401,25 +411,27 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
         __syncwarp();
         if (lane == 0)
             mbar_arrive(&row_empty[cs]);
-        GS_TICK(tm_add, tk)
-        if (!early && chunk + 1 < nchunks)
-            build(chunk + 1);
-        GS_TICK(tm_build, tk)
+        if (++cs == NSP) {
+            cs = 0;
+            cs_parity ^= 1u;
+        }
+#ifdef GS_X_TIMING
+        { const uint32_t n_ = clock(); tm_add += n_ - tka; tka = n_; }
+#endif
     };
     using NoFlush = std::integral_constant<uint32_t, 0u>;
     using FlushAll = std::integral_constant<uint32_t, GS_FL * STAGE_SUM>;
     static_assert(GS_FL == 4, "unroll the phases here");
     for (int chunk = 0; chunk < nchunks; chunk += GS_FL) {   // nchunks is a multiple of GS_FL by plan construction
-        stage(chunk, std::integral_constant<int, 0>{}, NoFlush{});
-        stage(chunk + 1, std::integral_constant<int, 1>{}, NoFlush{});
-        stage(chunk + 2, std::integral_constant<int, 2>{}, NoFlush{});
-        stage(chunk + 3, std::integral_constant<int, 3>{}, FlushAll{});
+        stage(std::integral_constant<int, 0>{}, NoFlush{});
+        stage(std::integral_constant<int, 1>{}, NoFlush{});
+        stage(std::integral_constant<int, 2>{}, NoFlush{});
+        stage(std::integral_constant<int, 3>{}, FlushAll{});
     }
 
 #ifdef GS_X_TIMING
-    if (lane == 0 && (cta == 5 || cta == 3000) && (warp == 0 || warp == 6 || warp == 15))
-        printf("cta %d warp %d stages %d: per stage issue %u build(total) %u of which waits %u, wait row_full %u, add %u\n", (int)cta, warp,
-               nchunks, tm_issue / nchunks, tm_build / nchunks, tm_bwait / nchunks, tm_cwait / nchunks, tm_add / nchunks);
+    if (lane == 0 && (cta == 5 || cta == 3000) && (warp == 0 || warp == 9))
+        printf("cta %d adder %d: per stage wait row_full %u add %u\n", (int)cta, warp, tm_wait / nchunks, tm_add / nchunks);
 #endif
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp` (as in dd_kernel_bp.cu)
     const int d = blk * DB + warp;
@@ -468,14 +480,16 @@ __global__ void __launch_bounds__(GS_NWARPS * 32, 1) dd_direct_gs(const KernelPa
     }
 }
 
+constexpr int GS_NBW = 4;   // builder warps
+
 template <int NBITS, int G, int CC, bool PATCH>
 cudaError_t launch_gs_inst(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, int64_t ctas)
 {
-    auto kernel = dd_direct_gs<NBITS, G, CC, PATCH>;
+    auto kernel = dd_direct_gs<NBITS, G, CC, GS_NBW, PATCH>;
     const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes));
     if (e != cudaSuccess)
         return e;
-    kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(GS_NWARPS * 32), plan->smem_bytes, stream>>>(kp);
+    kernel<<<dim3(static_cast<unsigned>(ctas)), dim3((GS_NWARPS + GS_NBW) * 32), plan->smem_bytes, stream>>>(kp);
     return cudaGetLastError();
 }
 

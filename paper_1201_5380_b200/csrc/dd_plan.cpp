@@ -402,7 +402,7 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
     const int nlive = static_cast<int>(live.size());
     if (nlive == 0)
         return DD_ERR_SMEM;
-    const int W = nbits == 2 ? DD_BP_W2 : 3, TB = 1024 * W, DB = 16;
+    const int W = nbits == 2 ? kGsW2 : kGsW48, TB = 1024 * W, DB = 16;
     const int nbr = nbits == 2 ? 2 : 4, nsubr = nbits / nbr, ubr = nbr * 4;   // raw layout: planes per unit, sub-rows, bytes per unit
     const int pin = nbits + (G == 2 ? 1 : 2), np = nbits == 2 ? 12 : (nbits == 4 ? 16 : 20);
     const int64_t vmax = (1 << nbits) - 1;
@@ -498,7 +498,9 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
             rows = std::max(rows, rows_here);
         }
     }
-    row_units = static_cast<int>(align_up(row_units, 4));
+    row_units = static_cast<int>(align_up(row_units, 8));   // (two arrays of whole 16-byte groups when W is even)
+    if (row_units >= 2048)
+        return DD_ERR_SMEM;                                 // unit positions travel in 12 bits
     const int raw_sub = raw_units * ubr;
     max_end = std::max<int64_t>(max_end, static_cast<int64_t>(raw_units) * 32);   // zero-row copies of padded channels
     if (static_cast<int64_t>(rows) * ((row_units + 31) / 32) >= 4096 || raw_sub > (1 << 19))
@@ -530,6 +532,7 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
             GsEntry *te = tab.data() + st * rows;
             for (int r = 0; r < rows; ++r)
                 te[r] = GsEntry{};
+            te[0].nunits = 1;   // (entry 0 is always in use; guards the builder's clamp if it were not)
             int row_idx = 0;
             for (int gi = 0; gi < cc; ++gi) {
                 analyse(b, k * cc + gi, g);
@@ -554,13 +557,19 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
                 for (int i = 0; i < DB; ++i) {
                     const uint32_t off = static_cast<uint32_t>(g.off[i]);
                     en[2 * i] = static_cast<uint32_t>(row_idx + g.pat_of[i]) * static_cast<uint32_t>(row_bytes);
-                    en[2 * i + 1] = ((off >> 5) << 8) | (off & 31u);
+                    // positions of the trial's first and second unit in a sub-row: consecutive when W is odd, in the even /
+                    // odd arrays when W is even (dd_kernel_gs.cu: Gs::DI)
+                    const uint32_t base = off >> 5, pp = base & 1u, hh = base >> 1;
+                    const uint32_t v0 = (W % 2) ? base : pp * (row_units / 2) + hh;
+                    const uint32_t v1 = (W % 2) ? 0u : (1u - pp) * (row_units / 2) + hh + pp;
+                    en[2 * i + 1] = (off & 31u) | (v0 << 8) | (v1 << 20);
                 }
                 row_idx += g.npat;
             }
+            te[0].pad[5] = row_idx;   // rows in use in this stage
         }
     }
-    p->var = Variant{5, DB, TB, 512, 32, 8, nbits, 0, 4, {cc, 0, 0, 0}, 1 << nbits, np, true, true, ubr, nsubr};
+    p->var = Variant{5, DB, TB, 640, 32, 8, nbits, 0, 4, {cc, 0, 0, 0}, 1 << nbits, np, true, true, ubr, nsubr};
     p->pairs = false;
     p->gs = true;
     p->gs_G = G;

@@ -175,6 +175,7 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc);
 // Shared-memory bytes of the variant-5 kernel for this geometry (must match the carve-up in dd_kernel_gs.cu).
 int64_t gs_smem_bytes(int nbits, int G, int cc, int rows, int row_units, int raw_sub, int nsr, int nsp, bool patch);
 bool gs_instance_exists(int nbits, int G, int cc);   // is dd_direct_gs<nbits, G, cc> compiled in?  (dd_kernel_gs.cu)
+constexpr int kGsW2 = 3, kGsW48 = 2;   // variant 5: units (32 samples) per lane for 2-bit / 4- and 8-bit input (tile = 1024 W samples)
 constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 
 // Shared-memory bytes the kernel needs for `cc` channels per stage (must match the kernel's carve-up).
