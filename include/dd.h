@@ -178,11 +178,13 @@ dd_status dd_set_batch(dd_plan plan, int nbeams, int64_t in_beam_stride, int64_t
  *   out_ptr    DEVICE.  out[beam][d][t], dense rows of nsamps elements, DM-major, time contiguous.
  *   out_nbits  DD_OUT_F32 (32), DD_OUT_U16 (16) or DD_OUT_U32 (-32).
  *   stream     a cudaStream_t (NULL = default stream).
- * Enqueues on `stream` and returns; does not synchronise and does not allocate (except that the first
- * call after a dd_set_dm_list made without a device uploads the tables).  The caller keeps in/out
- * alive until the stream has passed the enqueued work.  Launch errors are returned as DD_ERR_CUDA.
- * After one warm-up call with the same arguments (tables uploaded, the bit-plane work buffer grown) a call only
- * enqueues kernels, so it can be captured into a CUDA graph on `stream` and replayed (dd_scrunch_execute likewise).
+ * Enqueues on `stream` and returns.  The FIRST call for a given problem size allocates the plan's work buffers (see
+ * dd_set_workspace_limit; a call that needs larger ones frees and re-allocates, which synchronises the device), and
+ * the first call after a dd_set_dm_list made without a device uploads the tables.  Every later call with the same
+ * nsamps and batch only enqueues kernels -- it neither allocates, nor queries the device, nor synchronises -- so it
+ * can be captured into a CUDA graph on `stream` and replayed (dd_scrunch_execute likewise).  The caller keeps in/out
+ * alive until the stream has passed the enqueued work.  Launch errors are returned as DD_ERR_CUDA; variant 4 runs on
+ * two internal streams forked from `stream`, which are joined back to it before the call returns, also on error.
  */
 dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
                      int out_nbits, void *stream);
@@ -264,8 +266,12 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *                delay difference delta of every pair of adjacent summed channels -- exact, n + 1 plane words per
  *                pair instead of 2 n; costs device memory for the rows of one beam (16x / 26x / 12x its packed
  *                input on the 2-bit / 4-bit / 8-bit survey-shaped configs; twice that with several beams; the time
- *                axis is split into groups if that exceeds 3/4 of the free memory) and two more kernels per group,
- *                run on internal streams that are forked from and joined to the caller's stream.
+ *                axis is split into groups if that exceeds the limit of dd_set_workspace_limit) and two more kernels
+ *                per group, run on internal streams that are forked from and joined to the caller's stream;
+ *            5 = group sums made inside the CTA (2/4/8-bit, opt-in): per group of 2 or 4 adjacent summed channels and
+ *                block of 16 trials, one row per pattern of delay differences is built in shared memory from the staged
+ *                bit planes by builder warps, and every trial adds the row of its own pattern -- exact like variant 4,
+ *                but the rows never reach device memory.
  * Takes effect at the next dd_set_dm_list (which returns DD_ERR_SMEM if that variant cannot serve the plan).
  */
 dd_status dd_set_kernel_variant(dd_plan plan, int variant);
@@ -279,11 +285,29 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant);
  *          DD_TUNE_GROUPS_PER_STAGE: groups per pipeline stage of variant 5 (one of the compiled shapes: 2-bit 16 / 8
  *            pairs or 8 / 4 groups of four, 4-bit 8 / 4 or 4 / 2, 8-bit 4 / 2 or 2 / 1); 0 = chosen by the planner.
  *            Both take effect at the next dd_set_dm_list (DD_ERR_SMEM if no compiled shape matches or fits).
+ *          DD_TUNE_PAIR_TILES: time tiles per group of pair rows of variant 4 (its launcher builds and transforms the
+ *            rows group by group); 0 = as many as the workspace limit allows.  Takes effect at the next dd_execute.
  *   value  >= 0.
  * DD_ERR_INVALID_ARG for an unknown key or a negative value.
  */
-enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3 };
+enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3, DD_TUNE_PAIR_TILES = 4 };
 dd_status dd_set_tuning(dd_plan plan, int key, int value);
+
+/*
+ * dd_set_workspace_limit / dd_get_workspace_bytes -- device memory the plan takes beside its tables.
+ * Every bit-plane variant keeps a bit-plane copy of the packed input (same size as the input).  Variant 4 (the default
+ * for 4- and 8-bit plans of >= 128 channels) also keeps the pair rows of one group of time tiles (two groups when the
+ * call has several beams or the time axis is split): 12-26 x the packed input of a beam if the whole time axis is one
+ * group.  The buffers are allocated by the first dd_execute / dd_execute_host that needs them and re-used afterwards;
+ * they grow (cudaFree + cudaMalloc, which synchronise the device) only when a later call needs more.  The split of
+ * the time axis is worked out once per launch geometry (time tiles x beams) and kept.
+ *   bytes  limit for the pair rows of one group; 0 (default) = 3/4 of the device memory free at the first call.
+ *          A limit too small for one time tile's rows makes dd_execute return DD_ERR_CUDA (out of memory).
+ * dd_get_workspace_bytes returns the bytes the plan holds on the device right now (work buffers, pair rows, the
+ * staging buffers of dd_execute_host; tables not counted).
+ */
+dd_status dd_set_workspace_limit(dd_plan plan, int64_t bytes);
+int64_t dd_get_workspace_bytes(dd_plan plan);
 
 /*
  * dd_get_launch_info -- how the plan tiles the problem (for benchmarks and tests).  Host only.

@@ -21,7 +21,8 @@ __all__ = [
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE",
+    "DD_TUNE_PAIR_TILES", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
@@ -34,7 +35,8 @@ EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
-    "dd_set_kernel_variant", "dd_set_tuning", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error",
+    "dd_set_kernel_variant", "dd_set_tuning", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read",
+    "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy",
 )
@@ -98,6 +100,10 @@ def lib() -> ctypes.CDLL:
         L.dd_set_kernel_variant.argtypes = [vp, i32]
         L.dd_set_tuning.argtypes = [vp, i32, i32]
         L.dd_set_tuning.restype = i32
+        L.dd_set_workspace_limit.argtypes = [vp, i64]
+        L.dd_set_workspace_limit.restype = i32
+        L.dd_get_workspace_bytes.argtypes = [vp]
+        L.dd_get_workspace_bytes.restype = i64
         L.dd_int_add_peak.argtypes = [i32, ctypes.POINTER(dbl), vp]
         L.dd_profile_enable.argtypes = [vp, i32]
         L.dd_profile_read.argtypes = [vp, ctypes.POINTER(i32), vp, vp]
@@ -258,12 +264,23 @@ def dd_set_kernel_variant(plan: int, variant: int) -> None:
     _check(lib().dd_set_kernel_variant(plan, int(variant)), "dd_set_kernel_variant")
 
 
-DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE = 1, 2, 3
+DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE, DD_TUNE_PAIR_TILES = 1, 2, 3, 4
 
 
 def dd_set_tuning(plan: int, key: int, value: int) -> None:
     """Launch-geometry knobs (include/dd.h); results never depend on them."""
     _check(lib().dd_set_tuning(plan, int(key), int(value)), "dd_set_tuning")
+
+
+def dd_set_workspace_limit(plan: int, nbytes: int) -> None:
+    _check(lib().dd_set_workspace_limit(plan, int(nbytes)), "dd_set_workspace_limit")
+
+
+def dd_get_workspace_bytes(plan: int) -> int:
+    n = int(lib().dd_get_workspace_bytes(plan))
+    if n < 0:
+        _check(n, "dd_get_workspace_bytes")
+    return n
 
 
 def dd_get_launch_info(plan: int) -> dict:
@@ -413,6 +430,14 @@ class Plan:
     def set_input_max(self, vmax: int) -> "Plan":
         dd_set_input_max(self.handle, vmax)
         return self
+
+    def set_workspace_limit(self, nbytes: int) -> "Plan":
+        dd_set_workspace_limit(self.handle, nbytes)
+        return self
+
+    @property
+    def workspace_bytes(self) -> int:
+        return dd_get_workspace_bytes(self.handle)
 
     def set_tuning(self, key: int, value: int) -> "Plan":
         dd_set_tuning(self.handle, key, value)

@@ -1,7 +1,6 @@
 // dd_api.cu -- the C ABI of include/dd.h: argument checking, table upload, kernel launch.
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -379,6 +378,7 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->gs_nsp = scratch.gs_nsp;
     plan->gs_patch = scratch.gs_patch;
     plan->gs_tab.swap(scratch.gs_tab);
+    plan->pair_geom[2] = 0;
     plan->last_launches = 0;
     // upload now when a device exists; otherwise the first dd_execute retries (documented in dd.h)
     int ndev = 0;
@@ -854,8 +854,35 @@ dd_status dd_set_tuning(dd_plan plan, int key, int value)
     case DD_TUNE_GROUPS_PER_STAGE:
         plan->gs_force_cc = value;
         return DD_OK;
+    case DD_TUNE_PAIR_TILES:
+        plan->pair_tiles = value;
+        return DD_OK;
     }
     return DD_ERR_INVALID_ARG;
+}
+
+dd_status dd_set_workspace_limit(dd_plan plan, int64_t bytes)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    if (bytes < 0)
+        return DD_ERR_INVALID_ARG;
+    plan->ws_limit = bytes;
+    plan->pair_geom[2] = 0;   // worked out again at the next dd_execute
+    return DD_OK;
+}
+
+int64_t dd_get_workspace_bytes(dd_plan plan)
+{
+    if (!plan)
+        return DD_ERR_NULL;
+    int64_t b = static_cast<int64_t>(plan->work_bytes) + static_cast<int64_t>(plan->pairwork_bytes);
+    for (const dd_plan_s *q : {plan->s1, plan->s2})
+        if (q)
+            b += static_cast<int64_t>(q->work_bytes);
+    if (plan->stage)
+        b += static_cast<int64_t>(plan->stage->in_bytes) + 2 * static_cast<int64_t>(plan->stage->out_bytes);
+    return b;
 }
 
 dd_status dd_get_launch_info(dd_plan plan, int64_t *info)

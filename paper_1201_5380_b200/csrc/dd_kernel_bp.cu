@@ -29,7 +29,6 @@
 //            into the upper planes;
 //   store  : bit-matrix transposes turn NP planes x 32 lanes into 32 integers; float32 / uint32 / uint16,
 //            128-bit stores, time contiguous.
-#include <cstdlib>
 #include <utility>
 
 #include "dd_bp_core.cuh"
@@ -733,13 +732,20 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
     const int64_t extra_units = ((plan->max_span_end + 31) / 32 - tile_units + 3) / 4 * 4;   // span beyond a tile's own units
     const int64_t rows_o = plan->n_prows + 1;                                                  // + the all-zero row of padded entries
     auto pitch_of = [&](int64_t units) { return LONEL ? (C::NSUB - 1) * units * UBO + units * UBO / 4 : C::NSUB * units * UBO; };
-    // budget of a group's rows: what the plan already holds, else 75 % of the free device memory (halved when two
-    // groups are alive: several beams, or a time axis that has to be split)
-    int64_t budget = static_cast<int64_t>(plan->pairwork_bytes);
-    {
+    // Tiles per group: fixed when the plan first meets this launch geometry (time tiles x beams) and kept afterwards, so
+    // that later calls neither query the device nor re-allocate.  The budget of a group's rows is the caller's limit
+    // (dd_set_workspace_limit), else 3/4 of the device memory free at that moment; two groups are alive with several
+    // beams or a split time axis.  dd_set_tuning(DD_TUNE_PAIR_TILES) overrides the choice (tests).
+    int64_t G;
+    if (plan->pair_tiles > 0) {
+        G = plan->pair_tiles;
+    } else if (plan->pair_geom[0] == kp_in.ntiles && plan->pair_geom[1] == kp_in.nbeams && plan->pair_geom[2] > 0) {
+        G = plan->pair_geom[2];
+    } else {
         const int64_t whole = rows_o * pitch_of(static_cast<int64_t>(kp_in.ntiles) * tile_units + extra_units);
         const int64_t want = kp_in.nbeams > 1 ? 2 * whole : whole;
-        if (budget < want) {
+        int64_t budget = plan->ws_limit;
+        if (budget <= 0) {
             size_t free_b = 0, total_b = 0;
             if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) {
                 (void)cudaGetLastError();
@@ -748,10 +754,14 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
             budget = static_cast<int64_t>((free_b + plan->pairwork_bytes) / 4 * 3);
         }
         budget = want <= budget ? whole : budget / 2;
+        G = (budget - rows_o * pitch_of(extra_units)) / (rows_o * pitch_of(tile_units));
+        if (G < 1)
+            return cudaErrorMemoryAllocation;   // not even one tile's rows fit the limit
+        G = G > kp_in.ntiles ? kp_in.ntiles : G;
+        plan->pair_geom[0] = kp_in.ntiles;
+        plan->pair_geom[1] = kp_in.nbeams;
+        plan->pair_geom[2] = G;
     }
-    int64_t G = (budget - rows_o * pitch_of(extra_units)) / (rows_o * pitch_of(tile_units));
-    if (const char *envv = std::getenv("DD_PAIR_COLS"))   // test / tuning hook: time tiles per group
-        G = std::atoll(envv);
     G = G < 1 ? 1 : (G > kp_in.ntiles ? kp_in.ntiles : G);
     const int64_t units_g = G * tile_units + extra_units, conv_g = units_g * UBO, pitch_g = pitch_of(units_g);
     const int64_t buf_bytes = rows_o * pitch_g;
@@ -783,19 +793,21 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
             return e;
         plan->pairwork_bytes = need_o;
     }
-    if (!plan->pair_streams[0]) {
-        cudaStream_t st2[2];
-        cudaEvent_t ev3[3];
-        for (int i = 0; i < 2; ++i)
-            if ((e = cudaStreamCreateWithFlags(&st2[i], cudaStreamNonBlocking)) != cudaSuccess)
+    for (int i = 0; i < 2; ++i) {   // stored in the plan as they are created: dd_plan_destroy frees whatever exists
+        if (!plan->pair_streams[i]) {
+            cudaStream_t st;
+            if ((e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)) != cudaSuccess)
                 return e;
-        for (int i = 0; i < 3; ++i)
-            if ((e = cudaEventCreateWithFlags(&ev3[i], cudaEventDisableTiming)) != cudaSuccess)
+            plan->pair_streams[i] = st;
+        }
+    }
+    for (int i = 0; i < 3; ++i) {
+        if (!plan->pair_events[i]) {
+            cudaEvent_t ev;
+            if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess)
                 return e;
-        for (int i = 0; i < 2; ++i)
-            plan->pair_streams[i] = st2[i];
-        for (int i = 0; i < 3; ++i)
-            plan->pair_events[i] = ev3[i];
+            plan->pair_events[i] = ev;
+        }
     }
     cudaStream_t ws[2] = {static_cast<cudaStream_t>(plan->pair_streams[0]), static_cast<cudaStream_t>(plan->pair_streams[1])};
     cudaEvent_t fork = static_cast<cudaEvent_t>(plan->pair_events[0]);
@@ -808,22 +820,23 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
         return e;
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
-    // fork: both work streams wait for the transpose (and for everything the caller enqueued before)
-    cudaEventRecord(fork, stream);
-    for (int i = 0; i < 2; ++i) {
-        cudaStreamWaitEvent(ws[i], fork, 0);
-        if (i < nbuf && (e = cudaMemsetAsync(buf[i] + plan->n_prows * pitch_g, 0, static_cast<size_t>(pitch_g), ws[i])) != cudaSuccess)
-            return e;   // the zero row
-    }
     auto kernel = plan->long_mode ? dd_direct_bp<ENB, true, NBITS + 1, true> : dd_direct_bp<ENB, false, NBITS + 1, true>;
     if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes))) != cudaSuccess)
         return e;
     const int64_t ublocks = (units_g + 255) / 256;
-    if (plan->n_prows * ublocks > 0x7FFFFFFFLL)
+    if (plan->n_prows * ublocks > 0x7FFFFFFFLL || static_cast<int64_t>(kp_in.nblk) * G > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
+    // fork: both work streams wait for the transpose (and for everything the caller enqueued before).  From here on an
+    // error does not return before the join below, so that the caller's stream (and a capture in progress) stays whole.
+    cudaEventRecord(fork, stream);
+    for (int i = 0; i < 2; ++i)
+        cudaStreamWaitEvent(ws[i], fork, 0);
+    e = cudaSuccess;
+    for (int i = 0; i < nbuf && e == cudaSuccess; ++i)
+        e = cudaMemsetAsync(buf[i] + plan->n_prows * pitch_g, 0, static_cast<size_t>(pitch_g), ws[i]);   // the zero row
     int launches = 1, it = 0;
-    for (int b = 0; b < kp_in.nbeams; ++b) {
-        for (int64_t c0 = 0; c0 < kp_in.ntiles; c0 += G, ++it) {
+    for (int b = 0; b < kp_in.nbeams && e == cudaSuccess; ++b) {
+        for (int64_t c0 = 0; c0 < kp_in.ntiles && e == cudaSuccess; c0 += G, ++it) {
             const int sl = nbuf == 2 ? (it & 1) : 0;
             const int64_t gc = (c0 + G <= kp_in.ntiles) ? G : kp_in.ntiles - c0;
             const int64_t unit0 = c0 * tile_units;
@@ -832,7 +845,7 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
                 in_units, static_cast<const int4 *>(plan->d_prow), reinterpret_cast<uint32_t *>(buf[sl]), conv_g / 4, units_g, ublocks,
                 unit0);
             if ((e = cudaGetLastError()) != cudaSuccess)
-                return e;
+                break;
             KernelParams kp = kp_in;
             kp.in = buf[sl];
             kp.in_stride = pitch_g;
@@ -846,12 +859,8 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
             kp.tile0 = static_cast<int32_t>(c0);
             kp.ntiles = static_cast<int32_t>(gc);
             kp.in_unit0 = unit0;
-            const int64_t ctas = static_cast<int64_t>(kp.nblk) * gc;
-            if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
-                return cudaErrorInvalidConfiguration;
-            kernel<<<dim3(static_cast<unsigned>(ctas)), dim3(BP_NWARPS * 32), plan->smem_bytes, ws[sl]>>>(kp);
-            if ((e = cudaGetLastError()) != cudaSuccess)
-                return e;
+            kernel<<<dim3(static_cast<unsigned>(static_cast<int64_t>(kp.nblk) * gc)), dim3(BP_NWARPS * 32), plan->smem_bytes, ws[sl]>>>(kp);
+            e = cudaGetLastError();
             launches += 2;
         }
     }
@@ -861,6 +870,8 @@ cudaError_t launch_pairs(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_
         cudaEventRecord(jn, ws[i]);
         cudaStreamWaitEvent(stream, jn, 0);
     }
+    if (e != cudaSuccess)
+        return e;
     plan->pair_launches = launches;
     return cudaSuccess;
 }

@@ -121,6 +121,9 @@ struct dd_plan_s {
     void *pair_streams[2] = {nullptr, nullptr};   // internal streams: groups of time tiles alternate between them
     void *pair_events[3] = {nullptr, nullptr, nullptr};   // fork, join[2]
     int pair_launches = 0;                // kernels of the last launch (depends on the number of tile groups)
+    int pair_tiles = 0;                   // dd_set_tuning(DD_TUNE_PAIR_TILES): time tiles per group of pair rows; 0 = by budget
+    int64_t pair_geom[3] = {0, 0, 0};     // {time tiles, beams, tiles per group} the budget was last worked out for
+    int64_t ws_limit = 0;                 // dd_set_workspace_limit: bytes the pair rows of one group may take; 0 = 3/4 of free memory
     // group sums (variant 5): per group of G adjacent live channels and DM block, the CTA itself builds one row per
     // pattern of delay differences in shared memory; every trial adds the row of its own pattern
     bool gs = false;

@@ -38,7 +38,7 @@ def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, var
         p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
         torch.cuda.synchronize()
         info = p.launch_info()
-        assert (info["last_launches"] == {3: 2}.get(info["variant"], 1) or (info["variant"] == 4 and info["last_launches"] >= 3)) \
+        assert (info["last_launches"] == {3: 2, 5: 2}.get(info["variant"], 1) or (info["variant"] == 4 and info["last_launches"] >= 3)) \
             and (variant == 0 or info["variant"] == variant)
     return out.cpu().numpy().view(_NP_VIEW[out_kind])
 
@@ -133,6 +133,131 @@ def test_variant4_pair_rows(nbits):
     for b in range(2):
         ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask).astype(np.float32)
         assert np.array_equal(out[b].cpu().numpy(), ref) and np.array_equal(h_out[b].numpy(), ref)
+
+
+@pytest.mark.parametrize("nbeams", [1, 2])
+@pytest.mark.parametrize("tiles_per_group", [1, 2, 3])
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_variant4_time_axis_split_into_groups(nbits, tiles_per_group, nbeams):
+    # The pair-row launcher builds and transforms the rows per GROUP of time tiles (two buffers and two internal
+    # streams that alternate); with the whole time axis in one group -- the usual case -- the group offsets are all
+    # zero.  Here the split is forced (dd_set_tuning) to 1, 2 and 3 tiles over 7 tiles and a ragged 8th: first tile
+    # and first unit of a group != 0, a ragged last group, both buffers, one and two beams, device and host paths.
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    tb = 5120 if nbits == 2 else 3072
+    cfg = full.reduced(nsamps=7 * tb + 555, ndm=21, nchans=40, nbeams=nbeams)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    out = torch.full((nbeams, cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+    h_out = torch.full((nbeams, cfg.ndm, cfg.nsamps), -1, dtype=torch.int32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=4) as p:
+        p.set_tuning(dd.DD_TUNE_PAIR_TILES, tiles_per_group)
+        p.set_dm_list(cfg.dm_list())
+        if nbeams > 1:
+            p.set_batch(nbeams, dev.stride(0), out.stride(0) * 4)
+        p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        info = p.launch_info()
+        ngroups = -(-8 // tiles_per_group)
+        assert info["variant"] == 4 and info["time_block"] == tb and info["last_launches"] == 1 + 2 * ngroups * nbeams
+        assert p.workspace_bytes > 0
+        p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, -32)
+    for b in range(nbeams):
+        ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab)
+        got = out[b].cpu().numpy().view(np.uint32)
+        bad = np.nonzero(got != ref)
+        assert bad[0].size == 0, f"beam {b}: {bad[0].size} mismatches, first at d={bad[0][0]} t={bad[1][0]}"
+        assert np.array_equal(h_out[b].numpy().view(np.uint32), ref)
+
+
+def test_variant4_workspace_limit_splits_the_time_axis_and_is_worked_out_once():
+    # dd_set_workspace_limit: a limit below the rows of the whole time axis makes the launcher split it (more launches,
+    # same result); a limit below one tile's rows is an out-of-memory error, not a crash; the split is kept between calls
+    cfg = W.CONFIGS[4].reduced(nsamps=6 * 3072 + 100, ndm=20, nchans=64)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab)
+    out = torch.full((cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=4) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert p.launch_info()["last_launches"] == 3 and np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+        whole = p.workspace_bytes
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=4) as p:
+        p.set_dm_list(cfg.dm_list())
+        p.set_workspace_limit(whole // 3)
+        for _ in range(2):
+            out.fill_(-1)
+            p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            assert p.launch_info()["last_launches"] > 3 and np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+        assert p.workspace_bytes < whole
+        p.set_workspace_limit(1024)
+        with pytest.raises(dd.DDError):
+            p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        p.set_workspace_limit(0)     # and the plan still works afterwards
+        p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+
+
+_GS_SHAPES = {2: [(2, 16), (2, 8), (4, 8), (4, 4)], 4: [(2, 8), (2, 4), (4, 4), (4, 2)], 8: [(2, 4), (2, 2), (4, 2), (4, 1)]}
+
+
+def _gs_run(cfg, G, cc, dms=None, kind="u32", mask=None, host=False):
+    dms = cfg.dm_list() if dms is None else np.asarray(dms, dtype=np.float64)
+    tab = _oracle_table(cfg, dms)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    out = torch.full((cfg.nbeams, len(dms), cfg.nsamps), -1, dtype=_TORCH_OUT[kind], device="cuda")
+    h_out = torch.full((cfg.nbeams, len(dms), cfg.nsamps), -1, dtype=_TORCH_OUT[kind]).pin_memory() if host else None
+    code = {"f32": 32, "u32": -32, "u16": 16}[kind]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=5) as p:
+        p.set_tuning(dd.DD_TUNE_GROUP_SIZE, G).set_tuning(dd.DD_TUNE_GROUPS_PER_STAGE, cc)
+        p.set_killmask(mask)
+        p.set_dm_list(dms)
+        if cfg.nbeams > 1:
+            p.set_batch(cfg.nbeams, dev.stride(0), out.stride(0) * out.element_size())
+        p.execute(cfg.nsamps, dev, stride, out, code, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        info = p.launch_info()
+        assert info["variant"] == 5 and info["last_launches"] == 2 and info["chans_per_stage"] == cc
+        if host:
+            p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, code)
+    got = out.cpu().numpy().view(_NP_VIEW[kind])
+    for b in range(cfg.nbeams):
+        ref = oracle.cast_out(oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask), kind)
+        bad = np.nonzero(got[b] != ref)
+        assert bad[0].size == 0, (f"{cfg.name} G={G} cc={cc} {kind} beam {b}: {bad[0].size} mismatches, first at "
+                                  f"d={bad[0][0]} t={bad[1][0]} got={got[b][bad[0][0], bad[1][0]]} ref={ref[bad[0][0], bad[1][0]]}")
+        if host:
+            assert np.array_equal(h_out[b].numpy().view(_NP_VIEW[kind]), ref)
+
+
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_variant5_group_sums_in_shared_memory(nbits):
+    # group sums made inside the CTA: every compiled shape (pairs and groups of four, two stage sizes each) on several
+    # tiles with a ragged tail; channel counts that leave partial and padded groups; all output types; two beams
+    # through device and host paths; the high-DM end of the list (largest spreads, most patterns); a kill mask; an
+    # unsorted DM list (many patterns per block)
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    tb = 3072 if nbits == 2 else 2048
+    for G, cc in _GS_SHAPES[nbits]:
+        _gs_run(full.reduced(nsamps=2 * tb + 333, ndm=37, nchans=200, nbeams=1), G, cc)
+        for nchans in (1, 3, 17, 65):
+            _gs_run(full.reduced(nsamps=1283, ndm=3, nchans=nchans, nbeams=1), G, cc)
+    G, cc = _GS_SHAPES[nbits][2]
+    _gs_run(full.reduced(nsamps=3000, ndm=40, nbeams=2), G, cc, kind="f32", host=True)
+    cfg = full.reduced(nsamps=3000, ndm=40, nbeams=1)
+    _gs_run(cfg, G, cc, dms=np.asarray(full.dm_list())[-40:], kind="f32")
+    _gs_run(cfg, G, cc, mask=(np.arange(cfg.nchans) % 4 != 1).astype(np.int32), kind="u16" if nbits < 8 else "f32")
+    G, cc = _GS_SHAPES[nbits][0]
+    small = full.reduced(nsamps=1000, ndm=24, nchans=96, nbeams=1)
+    _gs_run(small, G, cc, dms=np.asarray(small.dm_list())[np.random.default_rng(4).permutation(small.ndm)])
 
 
 def test_variant2_channel_counts_around_group_and_flush_boundaries():
@@ -280,12 +405,8 @@ def test_killmask_4_and_8_bit_batch_and_host_path(nbits):
     (5, 48, 35, 900, 1, 32, 1, False),              # 8-bit input: only 1-channel sub-bands fit 8-bit intermediates
 ])
 @pytest.mark.parametrize("gpc", [0, 3])   # sub-bands summed per CTA in step 1: the library's choice / forced to 3
-def test_subband_method_matches_the_two_step_oracle(case, gpc, monkeypatch):
+def test_subband_method_matches_the_two_step_oracle(case, gpc):
     idx, nchans, ndm, nsamps, sb, grp, nbeams, masked = case
-    if gpc:
-        monkeypatch.setenv("DD_SB_GPC", str(gpc))
-    else:
-        monkeypatch.delenv("DD_SB_GPC", raising=False)
     cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=nbeams)
     dms = cfg.dm_list()
     nominal, d1, d2 = oracle.subband_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb, grp)
@@ -295,6 +416,7 @@ def test_subband_method_matches_the_two_step_oracle(case, gpc, monkeypatch):
     mask = (np.arange(nchans) % 7 != 3).astype(np.int32) if masked else None
     out = torch.full((nbeams, ndm, nsamps), -1, dtype=torch.int32, device="cuda")
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_tuning(dd.DD_TUNE_SUBBAND_GPC, gpc)
         p.set_dm_list(dms)
         p.set_killmask(mask)
         p.set_subband(sb, grp)
