@@ -420,6 +420,42 @@ def test_p13_subband_impulse_response():
                 assert np.array_equal(out[d], want)
 
 
+@pytest.mark.parametrize("sb,grp,nchans,ndm", [(4, 1, 24, 11), (4, 3, 24, 11), (8, 4, 24, 11), (24, 11, 24, 11), (1, 4, 24, 7), (6, 2, 36, 9)])
+def test_p13_subband_required_samples_is_exactly_the_largest_index_read(sb, grp, nchans, ndm):
+    """S4 pinned from both sides: step 2 reads S[b][g] at t + delta2[d][b] for t < nsamps,
+    step 1 makes S[b][g][t'] from a[c][t' + delta1[g][c]], c in sub-band b, for every nominal DM g.  The largest input
+    index the two steps read is therefore, by brute force over every (sub-band, nominal group, trial),
+    nsamps - 1 + max_d delta2[d][b] + max_{g, c in b} delta1[g][c]; `need` must be that + 1 -- an over-estimate would
+    pass every other pin (and the GPU's dd_get_subband_extent is compared with this function)."""
+    cfg = W.CONFIGS[1]
+    nsamps = 200
+    dms = np.arange(ndm, dtype=np.float64) * 7.5
+    nominal, d1, d2 = oracle.subband_tables(nchans, cfg.dt, cfg.f_top, -2.0, dms, sb, grp)
+    nsb, ngroups = nchans // sb, -(-ndm // grp)
+    largest = -1
+    for b in range(nsb):
+        top2 = -1
+        for d in range(ndm):
+            top2 = max(top2, int(d2[d][b]))
+        top1 = -1
+        for g in range(ngroups):
+            for c in range(b * sb, (b + 1) * sb):
+                top1 = max(top1, int(d1[g][c]))
+        largest = max(largest, nsamps - 1 + top2 + top1)
+    need = oracle.subband_required_samples(nsamps, d1, d2, sb)
+    assert need == largest + 1
+    # and the index is really read: a non-zero sample there reaches an output of the step-by-step transform when the
+    # trial whose delta2 is largest belongs to the nominal group whose delta1 is largest (always so on a band whose
+    # delays grow with DM: the last trial, the last group)
+    a = np.zeros((nchans, need), dtype=np.uint8)
+    a[nchans - 1, need - 1] = 1
+    out = oracle.subband_dedisperse_np(a, nsamps, nominal, d1, d2, sb, grp)
+    assert out[ndm - 1][nsamps - 1] == 1 and out[:, :nsamps - 1].sum() == 0
+    # one sample fewer is not enough for the step-by-step transform
+    with pytest.raises(ValueError):
+        oracle.subband_dedisperse_np(a[:, :need - 1], nsamps, nominal, d1, d2, sb, grp)
+
+
 # ----------------------------------------------------------------------------- P14
 def test_p14_time_scrunch():
     """adjacent pairs added.  Hand example: byte 0xE4 = 2-bit samples 0,1,2,3 -> sums 1, 5; totals are
