@@ -689,7 +689,27 @@ def _sample_points(cfg, tile, n, seed):
     return np.concatenate([d, dd_.ravel()]), np.concatenate([t, tt.ravel()])
 
 
-def _full_size_sampled(cfg, npoints, whole_rows=0):
+def _compare_block(cfg, out_b, packed_host, tab, rows, t0, length, what):
+    """Every output of the trials `rows` over the samples [t0, t0 + length) against the C oracle run on the packed rows
+    from sample t0 on (t0 * nbits is a whole number of bytes: tiles are multiples of 1024 samples)."""
+    rows = np.asarray(rows, dtype=np.int64)
+    byte0 = t0 * cfg.nbits // 8
+    byte1 = min(packed_host.shape[1], -(-(t0 + length + int(tab[rows].max())) * cfg.nbits // 8) + 16)
+    sub = packed_host if byte0 == 0 and byte1 == packed_host.shape[1] else np.ascontiguousarray(packed_host[:, byte0:byte1])
+    ref = oracle.cast_out(oracle.dedisperse(sub, cfg.nbits, length, tab[rows]), cfg.out)
+    got = out_b[torch.as_tensor(rows, device="cuda"), t0:t0 + length].cpu().numpy().view(_NP_VIEW[cfg.out])
+    bad = np.nonzero(got != ref)
+    assert bad[0].size == 0, (f"{cfg.name} {what}: {bad[0].size}/{ref.size} outputs differ; first d={rows[bad[0][0]]} "
+                              f"t={t0 + bad[1][0]} got={got[bad[0][0], bad[1][0]]} ref={ref[bad[0][0], bad[1][0]]}")
+    return ref.size
+
+
+def _full_size_sampled(cfg, npoints, whole_rows=0, everything=False, blocks_and_tiles=False):
+    """The transform at the full BASELINE.json size in the configuration bench.py times, against the oracle:
+    sampled outputs (random + tile / block edges) evaluated one by one; `whole_rows` whole DM rows; `everything`:
+    every output element (cfg2: ~16 s of oracle on 16 host threads); `blocks_and_tiles`: every output of three whole
+    16-trial DM blocks (first, middle, last -- the last has the largest delay spread) over the whole time axis, and
+    every trial over the first and the last (ragged or not) time tile, for the first and the last beam."""
     tab = _oracle_table(cfg)
     pulses = W.make_pulses(cfg, lambda idx: tab[idx])
     max_delay = int(tab.max())
@@ -719,6 +739,27 @@ def _full_size_sampled(cfg, npoints, whole_rows=0):
         ref_rows = oracle.cast_out(oracle.dedisperse(packed_host, cfg.nbits, nsamps, tab[rows]), cfg.out)
         got_rows = out[0][torch.as_tensor(rows, device="cuda")].cpu().numpy().view(_NP_VIEW[cfg.out])
         assert np.array_equal(got_rows, ref_rows)
+    compared = 0
+    if everything or blocks_and_tiles:
+        for b in sorted({0, nbeams - 1}):
+            packed_host = packed_dev[b].cpu().numpy()
+            if everything:
+                for r0 in range(0, ndm, 96):
+                    compared += _compare_block(cfg, out[b], packed_host, tab, np.arange(r0, min(r0 + 96, ndm)), 0, nsamps,
+                                               f"beam {b} trials {r0}..")
+            else:
+                nblk = -(-ndm // 16)
+                for blk in sorted({0, nblk // 2, nblk - 1}):
+                    compared += _compare_block(cfg, out[b], packed_host, tab, np.arange(blk * 16, min(blk * 16 + 16, ndm)), 0,
+                                               nsamps, f"beam {b} DM block {blk}")
+                ntiles = -(-nsamps // tile)
+                for tl in sorted({0, ntiles - 1}):
+                    t0 = tl * tile
+                    for r0 in range(0, ndm, 512):
+                        compared += _compare_block(cfg, out[b], packed_host, tab, np.arange(r0, min(r0 + 512, ndm)), t0,
+                                                   min(tile, nsamps - t0), f"beam {b} time tile {tl}")
+            del packed_host
+        print(f"{cfg.name}: {compared} outputs compared element by element")
     # every element was written (the buffer was pre-filled with -1 / NaN-like patterns)
     if cfg.out == "f32":
         assert bool((out >= 0).all())
@@ -726,20 +767,20 @@ def _full_size_sampled(cfg, npoints, whole_rows=0):
     torch.cuda.empty_cache()
 
 
-def test_cfg2_full_size_bench_configuration():
-    _full_size_sampled(W.CONFIGS[2], npoints=4000, whole_rows=12)
+def test_cfg2_full_size_bench_configuration_every_element():
+    _full_size_sampled(W.CONFIGS[2], npoints=4000, everything=True)
 
 
-def test_cfg3_full_size_sampled():
-    _full_size_sampled(W.CONFIGS[3], npoints=1500)
+def test_cfg3_full_size_blocks_tiles_and_samples():
+    _full_size_sampled(W.CONFIGS[3], npoints=1500, blocks_and_tiles=True)
 
 
-def test_cfg4_full_size_sampled():
-    _full_size_sampled(W.CONFIGS[4], npoints=3000)
+def test_cfg4_full_size_blocks_tiles_and_samples():
+    _full_size_sampled(W.CONFIGS[4], npoints=3000, blocks_and_tiles=True)
 
 
-def test_cfg5_full_size_sampled_batch():
-    _full_size_sampled(W.CONFIGS[5], npoints=2000)
+def test_cfg5_full_size_batch_blocks_tiles_and_samples():
+    _full_size_sampled(W.CONFIGS[5], npoints=2000, blocks_and_tiles=True)
 
 
 def test_cfg2_full_size_subband_32_32_sampled():
