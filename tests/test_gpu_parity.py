@@ -666,6 +666,55 @@ def test_execute_host_bitplane_8bit_two_slabs():
     assert np.array_equal(out.numpy(), ref)
 
 
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("nbits", [2, 8])
+def test_dm_slab_and_time_slab_shards_through_the_kernel(nbits, world):
+    # the two exchange-free splits besides beams, driven through dd_execute on one GPU,
+    # one "rank" after the other: DM slabs (own plan with the slab's DM sub-list, input replicated) and time slabs
+    # (input pointer advanced to the slab's first byte, nsamps = slab length, a halo of max_delay samples read by both
+    # neighbours); the shards are reassembled and compared with the oracle on every element.  Ragged last slabs.
+    from paper_1201_5380_b200 import multi
+    full = W.CONFIGS[{2: 2, 8: 5}[nbits]]
+    cfg = full.reduced(nsamps=5 * 1024 + 700, ndm=53, nchans=72, nbeams=1)
+    dms = cfg.dm_list()
+    tab = _oracle_table(cfg)
+    max_delay = int(tab.max())
+    packed, stride = W.gen_packed(cfg, max_delay)
+    ref = oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab)
+    # rows must be readable out to in_stride from the advanced pointer: one spare row behind the last channel
+    dev = torch.cat([packed[0], torch.zeros((1, stride), dtype=torch.uint8)]).cuda()
+    st = torch.cuda.current_stream()
+    # DM slabs
+    got = torch.full((cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+    covered = 0
+    for rank in range(world):
+        lo, hi = multi.shard_dm_slabs(cfg.ndm, world, rank)
+        assert lo % 16 == 0 and lo == covered
+        covered = hi
+        if hi == lo:
+            continue
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+            p.set_dm_list(dms[lo:hi])
+            p.execute(cfg.nsamps, dev, stride, got[lo:hi], -32, st)
+            torch.cuda.synchronize()
+    assert covered == cfg.ndm and np.array_equal(got.cpu().numpy().view(np.uint32), ref)
+    # time slabs, each written in place through the output row stride
+    got.fill_(-1)
+    covered = 0
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        p.set_dm_list(dms)
+        p.set_output_stride(cfg.nsamps * 4)
+        for rank in range(world):
+            t_lo, t_hi, in_lo, in_hi = multi.shard_time_slabs(cfg.nsamps, world, rank, max_delay)
+            assert t_lo == covered and in_lo == t_lo and in_hi == t_hi + max_delay and (t_lo * cfg.nbits) % 128 == 0
+            covered = t_hi
+            if t_hi == t_lo:
+                continue
+            p.execute(t_hi - t_lo, dev.data_ptr() + t_lo * cfg.nbits // 8, stride, got.data_ptr() + 4 * t_lo, -32, st)
+            torch.cuda.synchronize()
+    assert covered == cfg.nsamps and np.array_equal(got.cpu().numpy().view(np.uint32), ref)
+
+
 def test_device_generation_equals_host_generation():
     cfg = W.CONFIGS[2].reduced(nsamps=5000, ndm=8, nchans=64)
     a, s1 = W.gen_packed(cfg, 300)
