@@ -102,7 +102,7 @@ def info_after(plan) -> int:
 
 
 KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp<{nbits}>",
-                4: "dd_direct_bp<pair rows of {nbits}-bit input>"}
+                4: "dd_direct_bp<pair rows of {nbits}-bit input>", 5: "dd_direct_gs<{nbits}>"}
 
 
 def measured_peaks() -> dict:
@@ -115,17 +115,16 @@ def measured_peaks() -> dict:
     return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
 
 
-def committed_traffic(workload: str, variant: int):
-    """dram bytes per launch from the committed ncu capture (profiles/dram_traffic.csv), or None."""
+def committed_capture(workload: str, variant: int) -> dict:
+    """Counters of the committed ncu capture of this (workload, kernel variant): profiles/dram_traffic.csv, one line
+    each -- dram bytes per dd_execute, ALU-pipe utilisation of the dominant kernel (%), the summary file."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
-    if not os.path.exists(path):
-        return None
-    best = None
-    for line in open(path):
-        f = [x.strip() for x in line.split(",")]
-        if len(f) >= 3 and f[0] == workload and f[1] == str(variant):
-            best = float(f[2])
-    return best
+    if os.path.exists(path):
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 5 and not f[0].startswith("#") and f[0] == workload and f[1] == str(variant):
+                return {"traffic": float(f[2]), "alu_pipe_pct": float(f[3]) if f[3] else None, "capture": f[4]}
+    return {"traffic": None, "alu_pipe_pct": None, "capture": None}
 
 
 def cpu_sample(cfg, nsamps: int, dm_step: int):
@@ -152,6 +151,53 @@ def time_oracle(packed, tab, nbits, nsamps, reps: int = 1):
     return best
 
 
+def measure_config(dd, W, torch, cfg, stream, device_index, alu_peak, steps=5, warmup=3) -> dict:
+    """One full-size config timed like the headline line (no end-to-end, no oracle): for `other_configs`."""
+    plan = dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits).set_dm_list(cfg.dm_list())
+    max_delay = plan.max_delay
+    tab = plan.delay_table() if cfg.npulses else None
+    pulses = W.make_pulses(cfg, lambda idx: tab[idx]) if cfg.npulses else None
+    packed, stride = W.gen_packed(cfg, max_delay, pulses, device="cuda", beams=list(range(cfg.nbeams)), chan_chunk=16)
+    tdtype = {"f32": torch.float32, "u32": torch.int32, "u16": torch.int16}[cfg.out]
+    out = torch.empty((cfg.nbeams, cfg.ndm, cfg.nsamps), dtype=tdtype, device="cuda")
+    if cfg.nbeams > 1:
+        plan.set_batch(cfg.nbeams, packed.stride(0), out.stride(0) * out.element_size())
+    counts = algorithmic_counts(cfg, max_delay, cfg.nbeams)
+    for _ in range(warmup):
+        plan.execute(cfg.nsamps, packed, stride, out, cfg.out_nbits, stream)
+    torch.cuda.synchronize()
+    plan.profile_enable(steps)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    with ClockSampler(device_index) as clk:
+        with torch.cuda.stream(stream):
+            ev[0].record(stream)
+            for k in range(steps):
+                plan.execute(cfg.nsamps, packed, stride, out, cfg.out_nbits, stream)
+                ev[k + 1].record(stream)
+        torch.cuda.synchronize()
+    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    prepass_ms, main_ms = plan.profile_read()
+    plan.profile_enable(0)
+    info = plan.launch_info()
+    ms = float(np.mean(per_step))
+    cap = committed_capture(cfg.name, info["variant"])
+    res = {
+        "workload": cfg.name, "nchans": cfg.nchans, "nbits": cfg.nbits, "ndm": cfg.ndm, "nsamps": cfg.nsamps,
+        "nbeams": cfg.nbeams, "out": cfg.out, "steps": steps, "variant": info["variant"],
+        "kernel": KERNEL_NAMES[info["variant"]].format(nbits=cfg.nbits), "kernels_per_step": info["last_launches"],
+        "ms_per_step": ms, "step_ms_min_max": [float(min(per_step)), float(max(per_step))],
+        "kernel_ms": float(np.mean(main_ms)), "prepass_kernel_ms": float(np.mean(prepass_ms)),
+        "value": counts["units"] / (ms * 1e-3), "unit": UNIT,
+        "achieved_tadd_s": counts["adds"] / (ms * 1e-3) / 1e12, "frac": counts["adds"] / (ms * 1e-3) / alu_peak,   # of the whole step (every kernel of dd_execute)
+        "algorithmic_bytes": counts["bytes"], "traffic": cap["traffic"], "alu_pipe_pct": cap["alu_pipe_pct"],
+        "ncu_capture": cap["capture"], "workspace_bytes": plan.workspace_bytes, "clocks": clk.summary(),
+    }
+    plan.close()
+    del packed, out
+    torch.cuda.empty_cache()
+    return res
+
+
 # ------------------------------------------------------------------------------------------ reference arm
 def run_reference(args) -> None:
     import dd_workloads as W
@@ -161,7 +207,7 @@ def run_reference(args) -> None:
     if rank != 0:
         return
     cfg = W.CONFIGS[args.config]
-    packed, tab, nsamps, ndm, desc = cpu_sample(cfg, 1 << 15, 16)
+    packed, tab, nsamps, ndm, desc = cpu_sample(cfg, args.cpu_nsamps, args.cpu_dm_step)   # the sample cpu_baseline times
     cores = oracle.threads(0)
     for _ in range(args.warmup):
         oracle.dedisperse(packed, cfg.nbits, nsamps, tab)
@@ -345,10 +391,11 @@ def run_ours(args) -> None:
     peaks = measured_peaks()
     achieved_adds = counts["adds"] / (kernel_ms * 1e-3)
     achieved_gbs = counts["bytes"] / (kernel_ms * 1e-3) / 1e9
+    cap = committed_capture(cfg.name, info["variant"])
     roofline = {
         "bound": "alu", "achieved": achieved_adds / 1e12, "peak": alu_peak / 1e12, "unit": "Tadd/s",
         "frac": achieved_adds / alu_peak,
-        "traffic": committed_traffic(cfg.name, info["variant"]),
+        "traffic": cap["traffic"], "alu_pipe_pct": cap["alu_pipe_pct"], "ncu_capture": cap["capture"],
         "kernel": ("sub-band: dd_to_bitplanes + dd_direct_bp<{nbits}> (step 1), dd_to_bitplanes + dd_direct_bp<8> (step 2)"
                    if subband else KERNEL_NAMES[info["variant"]]).format(nbits=cfg.nbits), "kernel_ms": kernel_ms,
         "kernel_ms_p5_p50_p95": [float(np.percentile(main_ms, q)) for q in (5, 50, 95)],
@@ -356,6 +403,9 @@ def run_ours(args) -> None:
         "prepass_kernel_ms": float(np.mean(prepass_ms)),
         "step_ms_p5_p50_p95": [float(np.percentile(per_step, q)) for q in (5, 50, 95)],
         "algorithmic_adds_per_launch": counts["adds"], "algorithmic_bytes_per_launch": counts["bytes"],
+        "frac_note": "algorithmic channel-adds / measured scalar integer-add peak; the bit-plane kernels retire 32 "
+                     "channel-adds with ~6 ALU instructions, so frac may exceed 1 -- alu_pipe_pct (ncu, committed "
+                     "capture) says how busy the limiting pipe is",
         "peak_source": "measured in this run by dd_int_add_peak (32-bit integer additions/s, all SMs): "
                        f"2-input adds {peak_ind / 1e12:.2f}, 3-input IADD3 {peak_3in / 1e12:.2f}, IADD3+IMAD on both "
                        f"pipes {peak_mix / 1e12:.2f} Tadd/s; peak = the largest",
@@ -363,12 +413,21 @@ def run_ours(args) -> None:
                 "frac": achieved_gbs / peaks.get("hbm_gbs", float("nan")), "peak_source": peaks["source"]},
     }
 
+    # ---- the other full-size configs of BASELINE.json (cfg4, cfg5, cfg3), 5 timed steps each, same method: inputs
+    # generated in HBM, CUDA events on the launching stream, clocks sampled during that config's timed region
+    other_configs = None
+    if args.config == 2 and not subband and not args.no_others and world == 1 and not args.variant:
+        plan.close()
+        del packed, out
+        torch.cuda.empty_cache()
+        other_configs = [measure_config(dd, W, torch, W.CONFIGS[i], stream, local_rank, alu_peak, steps=5) for i in (4, 5, 3)]
+
     # ---- the oracle timed beside it on this box's host cores (bounded sample; a baseline, not the target)
     cpu_baseline = None
     if not args.no_cpu and world == 1:
         import oracle
         cpacked, ctab, cns, cndm, desc = cpu_sample(cfg, args.cpu_nsamps, args.cpu_dm_step)
-        el = time_oracle(cpacked, ctab, cfg.nbits, cns)
+        el = time_oracle(cpacked, ctab, cfg.nbits, cns, reps=4)
         cpu_baseline = {"value": cndm * cns / el, "unit": UNIT, "cores": oracle.threads(0), "kind": "oracle",
                         "sample": desc, "seconds": el}
 
@@ -385,7 +444,7 @@ def run_ours(args) -> None:
                    "parallelism": f"beam-per-gpu x{world}" if world > 1 else "single gpu",
                    **({"method": "sub-band (approximate)", **subband} if subband else {})},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": args.steps * kernels_per_step,
-        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "other_configs": other_configs,
         "wall_s_timed_region": wall,
     }
     print(json.dumps(line))
@@ -407,7 +466,9 @@ def main() -> None:
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (dd_set_kernel_variant); 0 = the library's choice")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")
-    ap.add_argument("--cpu-nsamps", type=int, default=1 << 18, help="output samples of the bounded oracle sample")
+    ap.add_argument("--no-others", action="store_true", help="skip the other full-size configs (other_configs)")
+    ap.add_argument("--cpu-nsamps", type=int, default=1 << 16, help="output samples of the bounded oracle sample (both the "
+                    "cpu_baseline of the main arm and every step of --impl reference time this sample)")
     ap.add_argument("--cpu-dm-step", type=int, default=1, help="the oracle sample takes every n-th DM trial")
     args = ap.parse_args()
     if args.subband:
