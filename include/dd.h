@@ -16,7 +16,9 @@
  * Conventions
  *   - Plain C types only.  Every pointer argument says whether it is HOST or DEVICE memory.
  *   - All functions return a dd_status (0 = DD_OK, negative = error) unless stated; none aborts.
- *     On error the plan is left unchanged.
+ *     On error the plan is left unchanged -- with one exception: when the planning of a new DM list / kill mask /
+ *     sub-band setting succeeds but the upload of its tables to the device fails (DD_ERR_CUDA), the plan holds the
+ *     new setting without device tables, and the next dd_execute* uploads them again.
  *   - A plan is not thread-safe; distinct plans are independent.  The library never frees or
  *     retains caller buffers.  The plan owns its DM list, delay table and tile metadata (host and
  *     device copies) until dd_plan_destroy.
@@ -116,7 +118,8 @@ dd_status dd_set_output_stride(dd_plan plan, int64_t out_dm_stride);
  * 2-bit samples: vmax = 3 * 2^k).  The bit-plane kernel then neither shifts nor adds the planes that
  * cannot be set (bit_length(vmax) of the nbits planes are used).  Results are undefined if the promise is broken.
  *   vmax  1 .. 2^nbits - 1, or 0 to withdraw the promise (DD_ERR_INVALID_ARG otherwise).  Takes effect at the
- *         next dd_execute; independent of the DM list, kill mask and batch.
+ *         next dd_execute.  With a DM list already set the tile metadata is planned again (the promise decides which
+ *         kernel serves the plan), so the call costs as much as dd_set_dm_list and can return its errors.
  */
 dd_status dd_set_input_max(dd_plan plan, int vmax);
 

@@ -733,6 +733,15 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     cudaEventRecord(S->in_ready, S->copy_in);
     cudaStreamWaitEvent(S->compute, S->in_ready, 0);
 
+    // an error below must not return while copies into the caller's buffers are still in flight
+    auto fail_drained = [&](dd_status code) {
+        cudaStreamSynchronize(S->copy_in);
+        cudaStreamSynchronize(S->compute);
+        cudaStreamSynchronize(S->copy_out[0]);
+        cudaStreamSynchronize(S->copy_out[1]);
+        (void)cudaGetLastError();
+        return code;
+    };
     int64_t launches = 0;
     for (int64_t k = 0; k < nslabs; ++k) {
         const int b = static_cast<int>(k & 1);
@@ -746,14 +755,14 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
             const dd_status sst = execute_subband(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, S->compute, true);
             plan->in_beam_stride = keep_beam;
             if (sst != DD_OK)
-                return sst;
+                return fail_drained(sst);
             launches += plan->last_launches;
         } else {
             KernelParams kp = make_params(plan, len, in_slab, in_stride, S->d_out[b], out_nbits, nbeams, in_beam,
                                           static_cast<int64_t>(plan->ndm) * len * es);
             kp.in_row_bytes = in_stride - (s0 * plan->nbits) / 8;
             if ((e = launch_direct(plan, kp, S->compute)) != cudaSuccess)
-                return cuda_fail(e, "dd_execute_host launch");
+                return fail_drained(cuda_fail(e, "dd_execute_host launch"));
             launches += launches_per_execute(plan);
         }
         cudaEventRecord(S->done[b], S->compute);
@@ -764,7 +773,7 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
             if ((e = cudaMemcpy2DAsync(dst, static_cast<size_t>(row_pitch), src, static_cast<size_t>(len) * es,
                                        static_cast<size_t>(len) * es, plan->ndm, cudaMemcpyDeviceToHost,
                                        S->copy_out[b])) != cudaSuccess)
-                return cuda_fail(e, "cudaMemcpy2DAsync(out)");
+                return fail_drained(cuda_fail(e, "cudaMemcpy2DAsync(out)"));
         }
         cudaEventRecord(S->drained[b], S->copy_out[b]);
     }
@@ -822,8 +831,22 @@ dd_status dd_set_input_max(dd_plan plan, int vmax)
     int planes = 0;
     while (vmax >> planes)
         ++planes;
+    if (planes == plan->in_planes)
+        return DD_OK;
+    const int before = plan->in_planes;
     plan->in_planes = planes;   // 0 = all nbits planes
-    return DD_OK;
+    if (plan->ndm <= 0)
+        return DD_OK;
+    // the promise decides which kernel serves the plan (variant 3 skips planes, variant 4 does not): plan again
+    try {
+        const dd_status st = replan(plan, plan->dm, plan->keep, plan->sb_nchans, plan->dm_group);
+        if (st != DD_OK)
+            plan->in_planes = before;
+        return st;
+    } catch (const std::bad_alloc &) {
+        plan->in_planes = before;
+        return DD_ERR_NOMEM;
+    }
 }
 
 dd_status dd_set_kernel_variant(dd_plan plan, int variant)
