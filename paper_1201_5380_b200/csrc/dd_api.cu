@@ -100,7 +100,7 @@ static dd_status upload_tables(dd_plan_s *p)
         free_device_tables(p);
         return cuda_fail(e, "cudaMemcpy(tables)");
     }
-    if (p->pairs && !p->prow.empty()) {   // variant 4: {c0, c1, delta, 0} of every pair row
+    if ((p->pairs || p->gr) && !p->prow.empty()) {   // variants 4 / 6: the channels and delay differences of every row
         const size_t pb = p->prow.size() * sizeof(int32_t);
         if ((e = cudaMalloc(&p->d_prow, pb)) != cudaSuccess ||
             (e = cudaMemcpy(p->d_prow, p->prow.data(), pb, cudaMemcpyHostToDevice)) != cudaSuccess) {
@@ -369,6 +369,7 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->rows_per_chunk = scratch.rows_per_chunk;
     plan->prow.swap(scratch.prow);
     plan->n_prows = scratch.n_prows;
+    plan->gr = scratch.gr;
     plan->gs = scratch.gs;
     plan->gs_G = scratch.gs_G;
     plan->gs_rows = scratch.gs_rows;
@@ -853,7 +854,7 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant)
 {
     if (!plan)
         return DD_ERR_NULL;
-    if (variant < 0 || variant > 5)
+    if (variant < 0 || variant > 6)
         return DD_ERR_INVALID_ARG;
     plan->force_variant = variant;
     return DD_OK;

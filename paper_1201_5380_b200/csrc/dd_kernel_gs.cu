@@ -480,7 +480,10 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
     }
 }
 
-constexpr int GS_NBW = 4;   // builder warps
+#ifndef GS_NBW_
+#define GS_NBW_ 4
+#endif
+constexpr int GS_NBW = GS_NBW_;   // builder warps
 
 template <int NBITS, int G, int CC, bool PATCH>
 cudaError_t launch_gs_inst(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, int64_t ctas)

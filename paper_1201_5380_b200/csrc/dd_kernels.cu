@@ -62,12 +62,17 @@ cudaError_t launch_direct(dd_plan_s *plan, const KernelParams &kp, cudaStream_t 
         return launch_variant4(plan, kp, stream);
     case 5:
         return launch_variant5(plan, kp, stream);
+    case 6:
+        return launch_variant6(plan, kp, stream);
     }
     return cudaErrorInvalidValue;
 }
 
 // bit planes: transpose + transform; pair rows: transpose + (row builder + transform) per group of time tiles
-int launches_per_execute(const dd_plan_s *plan) { return plan->pairs ? plan->pair_launches : (plan->var.bitplane ? 2 : 1); }
+int launches_per_execute(const dd_plan_s *plan)
+{
+    return (plan->pairs || plan->gr) ? plan->pair_launches : (plan->var.bitplane ? 2 : 1);
+}
 
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream)
 {

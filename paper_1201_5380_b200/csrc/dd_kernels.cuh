@@ -81,6 +81,8 @@ cudaError_t launch_variant5(dd_plan_s *plan, const KernelParams &kp, cudaStream_
 // buffer is cleared whenever it is new or its layout changed (for a producer that does not write every unit).
 cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream, bool zero_all, BpWork *w);
 
+// variant 6 (group rows in device memory, dd_kernel_gr.cu): transpose, then per group of time tiles row builder + transform.
+cudaError_t launch_variant6(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
 // The bit-plane transpose of the packed input into plan->d_work (geometry w from bp_prepare_work).
 cudaError_t launch_to_bitplanes(dd_plan_s *plan, const KernelParams &kp, const BpWork &w, cudaStream_t stream);
 

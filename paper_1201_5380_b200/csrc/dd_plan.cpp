@@ -601,6 +601,231 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
     return DD_OK;
 }
 
+int64_t gr_smem_bytes(int nbits, int G, int nstages, int stage_bytes, bool patch)
+{
+    int64_t b = 128 + (patch ? 16 * static_cast<int64_t>(kBpPatchBytes) : 0);
+    b += nstages * align_up(static_cast<int64_t>(gr_groups_per_stage(nbits, G)) * 16 * 8, 128);   // offset entries of the trials
+    b += static_cast<int64_t>(nstages) * stage_bytes;                                               // rows
+    return b;
+}
+
+// Variant 6 -- group rows in device memory (dd_kernel_gr.cu).  Groups of G adjacent live channels; per group the
+// distinct tuples (delta_1 .. delta_{G-1}), delta_i = delay[d][c_i] - delay[d][c_0], over the WHOLE DM list: one row
+// R[t] = sum_i x[c_i][t + delta_i] per tuple is made by a pre-pass, every trial adds the row of its own tuple at the
+// delay of c_0.  A stage holds, per DM block, the spans of the rows its 16 trials use, packed one after the other.
+dd_status build_tiles_gr(dd_plan_s *p, int G)
+{
+    const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
+    if (G == 0)
+        G = 4;
+    if (p->group_size > 0 || p->in_planes > 0 || (G != 2 && G != 4) || (nbits == 2 && G != 4))
+        return DD_ERR_SMEM;
+    std::vector<int32_t> live;
+    for (int c = 0; c < nrows; ++c)
+        if (p->keep.empty() || p->keep[c])
+            live.push_back(c);
+    const int nlive = static_cast<int>(live.size());
+    if (nlive == 0)
+        return DD_ERR_SMEM;
+    const int W = nbits == 2 ? DD_BP_W2 : 3, TB = 1024 * W, DB = 16;
+    const int np = nbits == 2 ? 12 : (nbits == 4 ? 16 : 20);
+    const int uw = gr_unit_words(nbits, G), ub = uw * 4, cc = gr_groups_per_stage(nbits, G);
+    const int au = (ub % 16 == 0) ? 1 : 2;   // spans start and end on whole 16 bytes: pairs of units when a unit is 8 (mod 16) bytes
+    const int64_t vmax = (1 << nbits) - 1;
+    if (static_cast<int64_t>(nlive) * vmax >= (int64_t(1) << np))
+        return DD_ERR_SMEM;
+    const int ngr = (nlive + G - 1) / G, fl = kGrFlushStages;
+    const int ents_pad = static_cast<int>(align_up(ngr, cc * fl)), nchunks = ents_pad / cc;
+    const int nblk = (ndm + DB - 1) / DB;
+    if (nchunks >= 8192)
+        return DD_ERR_SMEM;
+
+    // rows: every tuple of every group, in group order; per (trial, group) the row of the trial's tuple
+    struct Tuple {
+        int32_t d[4];
+        bool operator<(const Tuple &o) const { return std::lexicographical_compare(d, d + 4, o.d, o.d + 4); }
+        bool operator==(const Tuple &o) const { return std::equal(d, d + 4, o.d); }
+    };
+    std::vector<int32_t> prow;                                       // [n_rows][8] {c_0..c_3, delta_0..delta_3}
+    std::vector<int32_t> row_of(static_cast<size_t>(ndm) * ngr);     // [d][q] global row index
+    std::vector<Tuple> tup(ndm), uniq;
+    for (int q = 0; q < ngr; ++q) {
+        const int cnt = std::min(G, nlive - q * G);
+        int32_t ch[4] = {-1, -1, -1, -1};
+        for (int i = 0; i < cnt; ++i)
+            ch[i] = live[q * G + i];
+        for (int d = 0; d < ndm; ++d) {
+            const int32_t *row = p->delay.data() + static_cast<size_t>(d) * nrows;
+            Tuple t{{0, 0, 0, 0}};
+            for (int i = 1; i < cnt; ++i) {
+                t.d[i] = row[ch[i]] - row[ch[0]];
+                if (t.d[i] < 0 || t.d[i] > (1 << 26))   // (never for a descending band; refused all the same)
+                    return DD_ERR_SMEM;
+            }
+            tup[d] = t;
+        }
+        uniq = tup;
+        std::sort(uniq.begin(), uniq.end());
+        uniq.erase(std::unique(uniq.begin(), uniq.end()), uniq.end());
+        const int32_t base = static_cast<int32_t>(prow.size() / 8);
+        for (const Tuple &t : uniq) {
+            prow.insert(prow.end(), ch, ch + 4);
+            prow.insert(prow.end(), t.d, t.d + 4);
+        }
+        for (int d = 0; d < ndm; ++d)
+            row_of[static_cast<size_t>(d) * ngr + q] =
+                base + static_cast<int32_t>(std::lower_bound(uniq.begin(), uniq.end(), tup[d]) - uniq.begin());
+        if (prow.size() / 8 > (size_t(1) << 28))
+            return DD_ERR_SMEM;
+    }
+    const int64_t n_rows = static_cast<int64_t>(prow.size() / 8);
+    {   // behind the rows: the first row of every group, and the row count (the builder works group by group)
+        std::vector<int32_t> gbase;
+        int32_t last = -1;
+        for (int64_t r = 0; r < n_rows; ++r)
+            if (r == 0 || prow[8 * r] != last) {   // c_0 changes from group to group
+                gbase.push_back(static_cast<int32_t>(r));
+                last = prow[8 * r];
+            }
+        gbase.push_back(static_cast<int32_t>(n_rows));
+        prow.insert(prow.end(), gbase.begin(), gbase.end());
+    }
+
+    // per (DM block, group): the rows in use and the staged span of the group's first channel
+    struct Use {
+        int32_t start = 0, nbytes = 0, off[16];
+        int nrow = 0;
+        int32_t rows[16];
+        uint8_t which[16];
+    };
+    auto analyse = [&](int b, int q, Use &u) -> bool {
+        u = Use();
+        if (q >= ngr) {   // padded group: the all-zero row, every window at its start
+            u.nrow = 1;
+            u.rows[0] = static_cast<int32_t>(n_rows);
+            u.nbytes = static_cast<int32_t>(align_up(TB / 32 + 1, au)) * ub;
+            for (int i = 0; i < DB; ++i)
+                u.which[i] = 0, u.off[i] = 0;
+            return true;
+        }
+        const int c0 = live[q * G];
+        int32_t dmin = std::numeric_limits<int32_t>::max(), dmax = 0, d0s[16];
+        for (int i = 0; i < DB; ++i) {
+            const int d = std::min(b * DB + i, ndm - 1);   // the last block is padded with its last trial
+            d0s[i] = p->delay[static_cast<size_t>(d) * nrows + c0];
+            dmin = std::min(dmin, d0s[i]);
+            dmax = std::max(dmax, d0s[i]);
+            const int32_t r = row_of[static_cast<size_t>(d) * ngr + q];
+            int f = -1;
+            for (int k = 0; k < u.nrow && f < 0; ++k)
+                if (u.rows[k] == r)
+                    f = k;
+            if (f < 0) {
+                f = u.nrow++;
+                u.rows[f] = r;
+            }
+            u.which[i] = static_cast<uint8_t>(f);
+        }
+        u.start = dmin / (32 * au) * (32 * au);
+        if (dmax - u.start > (1 << 20))
+            return false;
+        const int64_t nunits = align_up(TB / 32 + (dmax - u.start) / 32 + 1, au);   // the funnel shift reads one unit further
+        u.nbytes = static_cast<int32_t>(nunits * ub);
+        for (int i = 0; i < DB; ++i)
+            u.off[i] = d0s[i] - u.start;
+        return true;
+    };
+    // pass 1: sizes
+    int rs = 1;
+    int64_t stage_bytes = 0, max_end = 0;
+    Use u;
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            int rows_here = 0;
+            int64_t bytes_here = 0;
+            for (int q = k * cc; q < (k + 1) * cc; ++q) {
+                if (!analyse(b, q, u))
+                    return DD_ERR_SMEM;
+                rows_here += u.nrow;
+                bytes_here += static_cast<int64_t>(u.nrow) * u.nbytes;
+                max_end = std::max<int64_t>(max_end, static_cast<int64_t>(u.start) + u.nbytes / ub * 32);
+            }
+            rs = std::max(rs, rows_here);
+            stage_bytes = std::max(stage_bytes, bytes_here);
+        }
+    }
+    if (rs > 48)   // the kernel's producers stage at most 3 rows per warp and stage
+        return DD_ERR_SMEM;
+    stage_bytes = align_up(stage_bytes, 128);
+    if (stage_bytes >= (1 << 20))
+        return DD_ERR_SMEM;
+    // the deepest ring that fits; output patches for 2- and 4-bit input when a ring of three still fits with them
+    int nst = 0;
+    bool patch = false;
+    for (int n = 4; n >= 2 && nst == 0; --n) {
+        if (nbits < 8 && n >= 3 && gr_smem_bytes(nbits, G, n, static_cast<int>(stage_bytes), true) <= kMaxDynSmem)
+            nst = n, patch = true;
+        else if (gr_smem_bytes(nbits, G, n, static_cast<int>(stage_bytes), false) <= kMaxDynSmem)
+            nst = n, patch = false;
+    }
+    if (nst == 0)
+        return DD_ERR_SMEM;
+
+    // pass 2: span list [nblk][nchunks][rs] and offsets [nblk][ents_pad][DB]
+    std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchunks * rs);
+    std::vector<uint8_t> rel(static_cast<size_t>(nblk) * ents_pad * DB * 8);
+    for (int b = 0; b < nblk; ++b) {
+        for (int k = 0; k < nchunks; ++k) {
+            SpanMeta *sl = span.data() + (static_cast<size_t>(b) * nchunks + k) * rs;
+            for (int j = 0; j < rs; ++j)
+                sl[j] = SpanMeta{0, 0, 0, 0};
+            int slot = 0;
+            int32_t dst = 0;
+            for (int gi = 0; gi < cc; ++gi) {
+                const int q = k * cc + gi;
+                analyse(b, q, u);
+                uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (static_cast<size_t>(b) * ents_pad + q) * DB * 2;
+                for (int i = 0; i < DB; ++i) {
+                    const uint32_t off = static_cast<uint32_t>(u.off[i]);
+                    en[2 * i] = static_cast<uint32_t>(dst + u.which[i] * u.nbytes) + (off >> 5) * static_cast<uint32_t>(ub);
+                    en[2 * i + 1] = off & 31u;
+                }
+                for (int j = 0; j < u.nrow; ++j) {
+                    sl[slot++] = SpanMeta{u.start / 32 * ub, u.nbytes, u.rows[j], dst};
+                    dst += u.nbytes;
+                }
+            }
+        }
+    }
+    p->var = Variant{6, DB, TB, 512, 32, 8, nbits, 0, 4, {cc, 0, 0, 0}, 1 << nbits, np, true, true, ub, 1};
+    p->pairs = false;
+    p->gs = false;
+    p->gr = true;
+    p->gs_G = G;
+    p->long_mode = true;
+    p->patch = patch;
+    p->max_span_end = max_end;
+    p->sub_slot = static_cast<int>(stage_bytes);
+    p->raw_slot = static_cast<int>(stage_bytes);
+    p->lane_slot = p->raw_slot;
+    p->rows_per_chunk = rs;
+    p->cc = cc;
+    p->nstages = nst;
+    p->ngroups = 1;
+    p->group_cols = ents_pad;
+    p->nblk = nblk;
+    p->nchans_pad = ents_pad;
+    p->smem_bytes = gr_smem_bytes(nbits, G, nst, static_cast<int>(stage_bytes), patch);
+    p->span.swap(span);
+    p->rel.swap(rel);
+    p->live.swap(live);
+    p->nlive = nlive;
+    p->prow.swap(prow);
+    p->n_prows = n_rows;
+    p->final32 = static_cast<int64_t>(nlive) * vmax > 65535;
+    return DD_OK;
+}
+
 // Variant 5 with the group size and the groups per stage of dd_set_tuning, else the first compiled shape that fits.
 static dd_status build_tiles_gs_auto(dd_plan_s *p)
 {
@@ -631,6 +856,9 @@ dd_status build_tiles(dd_plan_s *p)
         return build_tiles_pairs(p);
     if (p->force_variant == 5)
         return build_tiles_gs_auto(p);
+    p->gr = false;
+    if (p->force_variant == 6)
+        return build_tiles_gr(p, p->gs_force_G);
     // Default for 4- and 8-bit input: pair rows (variant 4, 15-17 % faster on cfg3-5), unless the plan sums channel
     // groups (sub-band steps), the caller promised small samples (dd_set_input_max: variant 3 then skips planes), or
     // the pair planner cannot serve the table (then variant 3 and the others are tried as before).  2-bit input

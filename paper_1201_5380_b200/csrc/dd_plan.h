@@ -136,6 +136,10 @@ struct dd_plan_s {
     bool gs_patch = false;                // epilogue through shared-memory patches
     std::vector<dd::GsEntry> gs_tab;      // [nblk][nchunks][gs_rows]
     void *d_gs_tab = nullptr;
+    // group rows (variant 6): like pair rows, for groups of gs_G = 4 (or 2) adjacent live channels, rows unit-interleaved;
+    // prow holds {c_0 .. c_3 (or -1), delta_0 .. delta_3} per row (8 ints), span [nblk][nchunks][rows_per_chunk]
+    // {byte offset in the row for tile 0, bytes, row, byte offset in the stage}, raw_slot = bytes of a stage's rows
+    bool gr = false;
     int sb_gpc = 0;                       // dd_set_tuning: sub-bands per CTA of sub-band step 1 (0 = chosen by the library)
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
@@ -178,6 +182,14 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc);
 // Shared-memory bytes of the variant-5 kernel for this geometry (must match the carve-up in dd_kernel_gs.cu).
 int64_t gs_smem_bytes(int nbits, int G, int cc, int rows, int row_units, int raw_sub, int nsr, int nsp, bool patch);
 bool gs_instance_exists(int nbits, int G, int cc);   // is dd_direct_gs<nbits, G, cc> compiled in?  (dd_kernel_gs.cu)
+// Variant 6 (group rows in device memory, dd_kernel_gr.cu): G channels per group (0 = 4).  DD_ERR_SMEM if it cannot serve.
+dd_status build_tiles_gr(dd_plan_s *p, int G);
+int64_t gr_smem_bytes(int nbits, int G, int nstages, int stage_bytes, bool patch);
+constexpr int kGrFlushStages = 4;
+// words per 32-sample unit of a group row: the planes (nbits + log2 G) padded so that the lanes of a warp read without
+// bank conflicts and units stay 8-byte aligned (dd_kernel_gr.cu)
+constexpr int gr_unit_words(int nbits, int G) { return nbits == 2 ? 4 : (nbits == 4 ? 6 : 10); }
+constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? 2 : 4) : (nbits == 8 ? 4 : 8); }
 constexpr int kGsW2 = 3, kGsW48 = 2;   // variant 5: units (32 samples) per lane for 2-bit / 4- and 8-bit input (tile = 1024 W samples)
 constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 
