@@ -347,52 +347,46 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     const int4 *span_blk = p.span + stage0 * p.rows_per_chunk;
     const uint8_t *rel_blk = static_cast<const uint8_t *>(p.rel) + stage0 * REL_BYTES;
 
-    // producers: every warp's lane 0 issues the copies of its rows of a stage (slots warp, warp + 16, warp + 32); warp 0
-    // also brings the trials' offset entries.  The span entries of the next stage to issue are fetched one step early.
-    auto load_meta = [&](int chunk, int4 (&m)[RPW]) {
-#pragma unroll
-        for (int k = 0; k < RPW; ++k) {
-            const int slot = warp + GR_NWARPS * k;
-            m[k] = (lane == 0 && chunk < nchunks && slot < p.rows_per_chunk)
-                       ? __ldg(&span_blk[static_cast<int64_t>(chunk) * p.rows_per_chunk + slot])
-                       : make_int4(0, 0, 0, 0);
-        }
+    // producers: lanes 0 .. RPW - 1 of every warp issue the copies of the warp's rows of a stage (lane k: slot warp +
+    // 16 k; one span entry per lane, so that the entries cost 8 registers instead of 24); warp 0 also brings the trials'
+    // offset entries.  The span entry of the next stage to issue is fetched one step early.
+    auto load_meta = [&](int chunk) -> int4 {
+        const int slot = warp + GR_NWARPS * lane;
+        return (lane < RPW && chunk < nchunks && slot < p.rows_per_chunk)
+                   ? __ldg(&span_blk[static_cast<int64_t>(chunk) * p.rows_per_chunk + slot])
+                   : make_int4(0, 0, 0, 0);
     };
     int prod_s = 0, prod_round = 0;
-    auto produce = [&](int chunk, const int4 (&m)[RPW]) {
+    auto produce = [&](int chunk, const int4 m) {
         const int s = prod_s;
+        // span entry: {byte offset inside the row for tile 0, bytes, row, byte offset inside the stage}
+        uint32_t tx = static_cast<uint32_t>(m.y);
+        tx += __shfl_down_sync(0xFFFFFFFFu, tx, 2);
+        tx += __shfl_down_sync(0xFFFFFFFFu, tx, 1);   // lane 0: bytes of lanes 0 .. 2 (RPW == 3; the other lanes hold 0)
         if (lane == 0) {
             if (prod_round > 0)
                 mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has added chunk - NS
-            // span entry: {byte offset inside the row for tile 0, bytes, row, byte offset inside the stage}
-            uint32_t tx = (warp == 0) ? REL_BYTES : 0u;
-#pragma unroll
-            for (int k = 0; k < RPW; ++k)
-                tx += static_cast<uint32_t>(m[k].y);
-            mbar_arrive_expect_tx(&full[s], tx);
-#pragma unroll
-            for (int k = 0; k < RPW; ++k)
-                if (m[k].y > 0)
-                    tma_bulk_g2s(row_base + s * row_slot + m[k].w, in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + m[k].x,
-                                 static_cast<uint32_t>(m[k].y), &full[s]);
+            mbar_arrive_expect_tx(&full[s], tx + (warp == 0 ? REL_BYTES : 0u));
             if (warp == 0)
                 tma_bulk_g2s(rel_base + s * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &full[s]);
         }
+        __syncwarp();
+        if (m.y > 0)
+            tma_bulk_g2s(row_base + s * row_slot + m.w, in_tile + static_cast<int64_t>(m.z) * p.in_stride + m.x,
+                         static_cast<uint32_t>(m.y), &full[s]);
         __syncwarp();
         if (++prod_s == NS) {
             prod_s = 0;
             ++prod_round;
         }
     };
+    static_assert(RPW == 3, "the byte count of a warp's copies is summed over lanes 0 .. 2");
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in stages
-    int4 meta[RPW], nxt[RPW];
-    load_meta(0, meta);
+    int4 meta = load_meta(0);
     for (int k = 0; k < dist && k < nchunks; ++k) {
-        load_meta(k + 1, nxt);
+        const int4 nxt = load_meta(k + 1);
         produce(k, meta);
-#pragma unroll
-        for (int i = 0; i < RPW; ++i)
-            meta[i] = nxt[i];
+        meta = nxt;
     }
 
     uint32_t P[W][NP], T[W][NT];
@@ -411,11 +405,9 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         constexpr int PHASE = decltype(phase)::value;
         constexpr uint32_t FLUSH = decltype(flush)::value;
         if (chunk + dist < nchunks) {
-            load_meta(chunk + dist + 1, nxt);
+            const int4 nxt = load_meta(chunk + dist + 1);
             produce(chunk + dist, meta);
-#pragma unroll
-            for (int i = 0; i < RPW; ++i)
-                meta[i] = nxt[i];
+            meta = nxt;
         }
         mbar_wait(&full[s], full_parity);
         gr_add_stage<NBITS, G, PHASE>(std::make_integer_sequence<int, CC>{}, row_base + s * row_slot + lane * (W * UB),
