@@ -40,7 +40,7 @@ struct Gr {
     static constexpr int PIN = NBITS + (G == 2 ? 1 : 2);   // planes of a row
     static constexpr int UW = gr_unit_words(NBITS, G);  // words per unit of a row (dd_plan.h)
     static constexpr int UB = UW * 4;
-    static constexpr int W = NBITS == 2 ? 5 : 3;        // units per lane
+    static constexpr int W = NBITS == 2 ? kGrW2 : 3;    // units per lane
     static constexpr int CC = gr_groups_per_stage(NBITS, G);
     static constexpr int NP = NBITS == 2 ? 12 : (NBITS == 4 ? 16 : 20);   // sum planes
     static_assert(UW >= PIN && (UW == 4 || UW % 2 == 0), "row unit");
@@ -269,31 +269,57 @@ __global__ void __launch_bounds__(GR_UBLK) dd_make_group_rows_staged(const uint3
 // ------------------------------------------------------------------------------------------ the transform
 // one group of the stage for this warp's trial: e = {byte offset, inside the stage, of the unit of the trial's row that
 // holds its first sample; bit shift}; W + 1 units loaded for W units, per unit and plane a funnel shift + carry-save adds
+// the planes K .. PIN - 1 of one unit: x0 / x1 hold the unit's words and those of the unit after it
 template <int NBITS, int G, int CLS, int K, int NP, int NT>
-__device__ __forceinline__ void gr_add_planes(const uint32_t (&x)[Gr<NBITS, G>::W + 1][Gr<NBITS, G>::PIN], uint32_t shift,
-                                              uint32_t (&P)[Gr<NBITS, G>::W][NP], uint32_t (&T)[Gr<NBITS, G>::W][NT])
+__device__ __forceinline__ void gr_add_planes(const uint32_t (&x0)[Gr<NBITS, G>::PIN], const uint32_t (&x1)[Gr<NBITS, G>::PIN], uint32_t shift,
+                                              uint32_t (&P)[NP], uint32_t (&T)[NT])
 {
     using C = Gr<NBITS, G>;
     if constexpr (K < C::PIN) {
         // weight the counter has taken since the last flush: CLS whole rows and the planes below this one
         constexpr uint32_t S = ((1u << C::PIN) - 1u) * CLS + ((1u << K) - 1u);
-#pragma unroll
-        for (int j = 0; j < C::W; ++j)
-            csa_add<S, K>(P[j], T[j], __funnelshift_r(x[j][K], x[j + 1][K], shift));
-        gr_add_planes<NBITS, G, CLS, K + 1>(x, shift, P, T);
+        csa_add<S, K>(P, T, __funnelshift_r(x0[K], x1[K], shift));
+        gr_add_planes<NBITS, G, CLS, K + 1>(x0, x1, shift, P, T);
     }
 }
 
+// plane K of every unit of the lane (the W counters advance side by side: most instruction-level parallelism)
+template <int NBITS, int G, int CLS, int K, int NP, int NT>
+__device__ __forceinline__ void gr_add_planes_all(const uint32_t (&x)[Gr<NBITS, G>::W + 1][Gr<NBITS, G>::PIN], uint32_t shift,
+                                                  uint32_t (&P)[Gr<NBITS, G>::W][NP], uint32_t (&T)[Gr<NBITS, G>::W][NT])
+{
+    using C = Gr<NBITS, G>;
+    if constexpr (K < C::PIN) {
+        constexpr uint32_t S = ((1u << C::PIN) - 1u) * CLS + ((1u << K) - 1u);
+#pragma unroll
+        for (int j = 0; j < C::W; ++j)
+            csa_add<S, K>(P[j], T[j], __funnelshift_r(x[j][K], x[j + 1][K], shift));
+        gr_add_planes_all<NBITS, G, CLS, K + 1>(x, shift, P, T);
+    }
+}
+
+// The counters of the W units are independent, so the order of the units is free.  Plane by plane over all units gives
+// the most parallelism (measured best for 2- and 4-bit input and 8-bit groups of four); unit by unit keeps only two
+// units' words live, which the 9-plane rows of 8-bit pairs need to stay clear of spills (cfg3: 196 -> 185 ms).
 template <int NBITS, int G, int CLS, int NP, int NT>
 __device__ __forceinline__ void gr_add_group(const uint8_t *lane_base, const uint2 e, uint32_t (&P)[Gr<NBITS, G>::W][NP],
                                              uint32_t (&T)[Gr<NBITS, G>::W][NT])
 {
     using C = Gr<NBITS, G>;
     uint32_t x[C::W + 1][C::PIN];
+    if constexpr (NBITS == 8 && G == 2) {
+        gr_load_unit<C::UW, C::PIN>(lane_base + e.x, x[0]);
 #pragma unroll
-    for (int j = 0; j <= C::W; ++j)
-        gr_load_unit<C::UW, C::PIN>(lane_base + e.x + j * C::UB, x[j]);
-    gr_add_planes<NBITS, G, CLS, 0>(x, e.y, P, T);
+        for (int j = 0; j < C::W; ++j) {
+            gr_load_unit<C::UW, C::PIN>(lane_base + e.x + (j + 1) * C::UB, x[j + 1]);
+            gr_add_planes<NBITS, G, CLS, 0>(x[j], x[j + 1], e.y, P[j], T[j]);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j <= C::W; ++j)
+            gr_load_unit<C::UW, C::PIN>(lane_base + e.x + j * C::UB, x[j]);
+        gr_add_planes_all<NBITS, G, CLS, 0>(x, e.y, P, T);
+    }
 }
 
 template <int NBITS, int G, int PHASE, int NP, int NT, int... GIs>

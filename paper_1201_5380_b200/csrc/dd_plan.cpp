@@ -627,7 +627,7 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
     const int nlive = static_cast<int>(live.size());
     if (nlive == 0)
         return DD_ERR_SMEM;
-    const int W = nbits == 2 ? DD_BP_W2 : 3, TB = 1024 * W, DB = 16;
+    const int W = nbits == 2 ? kGrW2 : 3, TB = 1024 * W, DB = 16;
     const int np = nbits == 2 ? 12 : (nbits == 4 ? 16 : 20);
     const int uw = gr_unit_words(nbits, G), ub = uw * 4, cc = gr_groups_per_stage(nbits, G);
     const int au = (ub % 16 == 0) ? 1 : 2;   // spans start and end on whole 16 bytes: pairs of units when a unit is 8 (mod 16) bytes

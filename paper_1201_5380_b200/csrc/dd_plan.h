@@ -189,7 +189,12 @@ constexpr int kGrFlushStages = 4;
 // words per 32-sample unit of a group row: the planes (nbits + log2 G) padded so that the lanes of a warp read without
 // bank conflicts and units stay 8-byte aligned (dd_kernel_gr.cu)
 constexpr int gr_unit_words(int nbits, int G) { return nbits == 2 ? 4 : (nbits == 4 ? 6 : 10); }
-constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? 2 : 4) : (nbits == 8 ? 4 : 8); }
+#ifndef DD_GR_W2
+#define DD_GR_W2 5
+#define DD_GR_CC2 4
+#endif
+constexpr int kGrW2 = DD_GR_W2;   // units per lane of the 2-bit group-row kernel
+constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? 2 : (nbits == 2 ? DD_GR_CC2 : 4)) : (nbits == 8 ? 4 : 8); }
 constexpr int kGsW2 = 3, kGsW48 = 2;   // variant 5: units (32 samples) per lane for 2-bit / 4- and 8-bit input (tile = 1024 W samples)
 constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 
