@@ -863,10 +863,33 @@ dd_status build_tiles(dd_plan_s *p)
     // groups (sub-band steps), the caller promised small samples (dd_set_input_max: variant 3 then skips planes), or
     // the pair planner cannot serve the table (then variant 3 and the others are tried as before).  2-bit input
     // stays on variant 3: the pair rows gain nothing there.
-    if (p->force_variant == 0 && (p->nbits == 4 || p->nbits == 8) && p->group_size == 0 && p->in_planes == 0 &&
-        p->nchans >= 128 &&   // small transforms are launch-bound: two kernels beat 1 + 2 per group
-        build_tiles_pairs(p) == DD_OK)
-        return DD_OK;
+    if (p->force_variant == 0 && p->group_size == 0 && p->in_planes == 0 && p->nchans >= 128) {
+        // Default: group rows (variant 6) when their cost model says so -- rows of four channels first, pairs if those do
+        // not fit shared memory (large delay spreads) -- else, for 4- and 8-bit input, the pair rows of variant 4.
+        for (int G : {4, 2}) {
+            if (p->gs_force_G && p->gs_force_G != G)
+                continue;
+            if (build_tiles_gr(p, G) != DD_OK)
+                continue;
+            // cost per 32 output samples, in ALU lane-operations: the bit-plane kernel adds nbits plane words per trial
+            // and channel (a shift + 2.13 LOP3 each); with group rows every trial adds pin words per group (15 % more
+            // overhead per word: smaller stages), every row costs its G shifted loads and ripple adders plus its bytes
+            // written (3.4 lane-operations per byte: 5.5 TB/s against 18.6e12 lane-operations/s; reading them back
+            // overlaps with the adds).  Calibrated on a B200: model 0.61 / 0.61 / 0.78 / 0.94 of the bit-plane kernel
+            // for cfg5 / cfg4 / cfg3 (pairs) / cfg2, measured 0.68 / 0.66 / 0.75 / 0.97.
+            const double pin = p->nbits + (G == 2 ? 1 : 2), ngr = (p->nlive + G - 1) / G;
+            const double direct = 3.13 * p->ndm * static_cast<double>(p->nlive) * p->nbits;
+            const double rows = static_cast<double>(p->n_prows) * (G * p->nbits + 2.0 * (G - 1) * (p->nbits + 1) +
+                                                                  3.4 * 4.0 * gr_unit_words(p->nbits, G));
+            const double grouped = 1.15 * 3.13 * p->ndm * ngr * pin + rows;
+            if (grouped < 0.9 * direct)
+                return DD_OK;
+            p->gr = false;
+        }
+        p->gr = false;
+        if ((p->nbits == 4 || p->nbits == 8) && p->gs_force_G == 0 && build_tiles_pairs(p) == DD_OK)
+            return DD_OK;
+    }
     p->pairs = false;
     const int nrows = p->nchans, ndm = p->ndm, nbits = p->nbits;
     // the channels that are summed (PAPER.md:113 kill mask): the kernels iterate over this list only

@@ -38,7 +38,7 @@ def _gpu_transform(cfg, packed_dev, stride, dms, out_kind=None, nsamps=None, var
         p.execute(nsamps, packed_dev, stride, out, code, torch.cuda.current_stream())
         torch.cuda.synchronize()
         info = p.launch_info()
-        assert (info["last_launches"] == {3: 2, 5: 2}.get(info["variant"], 1) or (info["variant"] == 4 and info["last_launches"] >= 3)) \
+        assert (info["last_launches"] == {3: 2, 5: 2}.get(info["variant"], 1) or (info["variant"] in (4, 6) and info["last_launches"] >= 3)) \
             and (variant == 0 or info["variant"] == variant)
     return out.cpu().numpy().view(_NP_VIEW[out_kind])
 
@@ -203,6 +203,77 @@ def test_variant4_workspace_limit_splits_the_time_axis_and_is_worked_out_once():
         p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
         torch.cuda.synchronize()
         assert np.array_equal(out.cpu().numpy().view(np.uint32), ref)
+
+
+@pytest.mark.parametrize("nbeams", [1, 2])
+@pytest.mark.parametrize("tiles_per_group", [1, 3])
+@pytest.mark.parametrize("nbits,G", [(2, 4), (4, 4), (4, 2), (8, 4), (8, 2)])
+def test_variant6_group_rows_and_time_axis_split(nbits, G, tiles_per_group, nbeams):
+    # group rows in device memory (the default for 4- and 8-bit plans): rows of four (or two) channels per tuple of
+    # delay differences, made group of time tiles by group on two internal streams.  The split is forced to 1 and 3
+    # tiles over 7 tiles and a ragged 8th (first tile / first unit of a group != 0, ragged last group, both buffers),
+    # one and two beams, device and host paths, every element against the oracle.
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    tb = 5120 if nbits == 2 else 3072
+    cfg = full.reduced(nsamps=7 * tb + 555, ndm=21, nchans=42, nbeams=nbeams)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    out = torch.full((nbeams, cfg.ndm, cfg.nsamps), -1, dtype=torch.int32, device="cuda")
+    h_out = torch.full((nbeams, cfg.ndm, cfg.nsamps), -1, dtype=torch.int32).pin_memory()
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=6) as p:
+        p.set_tuning(dd.DD_TUNE_GROUP_SIZE, G).set_tuning(dd.DD_TUNE_PAIR_TILES, tiles_per_group)
+        p.set_dm_list(cfg.dm_list())
+        if nbeams > 1:
+            p.set_batch(nbeams, dev.stride(0), out.stride(0) * 4)
+        p.execute(cfg.nsamps, dev, stride, out, -32, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        info = p.launch_info()
+        ngroups = -(-8 // tiles_per_group)
+        assert info["variant"] == 6 and info["time_block"] == tb and info["last_launches"] == 1 + 2 * ngroups * nbeams
+        p.execute_host(cfg.nsamps, packed.contiguous().pin_memory(), stride, h_out, -32)
+    for b in range(nbeams):
+        ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab)
+        got = out[b].cpu().numpy().view(np.uint32)
+        bad = np.nonzero(got != ref)
+        assert bad[0].size == 0, f"beam {b}: {bad[0].size} mismatches, first at d={bad[0][0]} t={bad[1][0]}"
+        assert np.array_equal(h_out[b].numpy().view(np.uint32), ref)
+
+
+@pytest.mark.parametrize("nbits,G", [(2, 4), (4, 4), (4, 2), (8, 4), (8, 2)])
+def test_variant6_group_rows_shapes_masks_and_dm_lists(nbits, G):
+    # several tiles with a ragged tail and all output types; channel counts that leave partial and padded groups; the
+    # high-DM end of the list (largest spreads, most tuples); a kill mask; an unsorted DM list
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    tb = 5120 if nbits == 2 else 3072
+
+    def run(cfg, dms=None, kinds=("u32",), mask=None):
+        dms = cfg.dm_list() if dms is None else np.asarray(dms, dtype=np.float64)
+        tab = _oracle_table(cfg, dms)
+        packed, stride = W.gen_packed(cfg, int(tab.max()))
+        dev = packed.cuda()
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=6) as p:
+            p.set_tuning(dd.DD_TUNE_GROUP_SIZE, G)
+            p.set_killmask(mask)
+            p.set_dm_list(dms)
+            for kind in kinds:
+                out = torch.full((1, len(dms), cfg.nsamps), -1, dtype=_TORCH_OUT[kind], device="cuda")
+                p.execute(cfg.nsamps, dev, stride, out, {"f32": 32, "u32": -32, "u16": 16}[kind], torch.cuda.current_stream())
+                torch.cuda.synchronize()
+                assert p.launch_info()["variant"] == 6
+                ref = oracle.cast_out(oracle.dedisperse(packed[0].numpy(), cfg.nbits, cfg.nsamps, tab, mask=mask), kind)
+                got = out[0].cpu().numpy().view(_NP_VIEW[kind])
+                bad = np.nonzero(got != ref)
+                assert bad[0].size == 0, f"{cfg.name} G={G} {kind}: {bad[0].size} mismatches, first d={bad[0][0]} t={bad[1][0]}"
+
+    run(full.reduced(nsamps=2 * tb + 333, ndm=37, nchans=200, nbeams=1), kinds=("f32", "u32") + (("u16",) if nbits < 8 else ()))
+    for nchans in (1, 3, 17, 65):
+        run(full.reduced(nsamps=1283, ndm=3, nchans=nchans, nbeams=1))
+    cfg = full.reduced(nsamps=3000, ndm=40, nbeams=1)
+    run(cfg, dms=np.asarray(full.dm_list())[-40:], kinds=("f32",))
+    run(cfg, mask=(np.arange(cfg.nchans) % 4 != 1).astype(np.int32))
+    small = full.reduced(nsamps=1000, ndm=24, nchans=96, nbeams=1)
+    run(small, dms=np.asarray(small.dm_list())[np.random.default_rng(4).permutation(small.ndm)])
 
 
 _GS_SHAPES = {2: [(2, 16), (2, 8), (4, 8), (4, 4)], 4: [(2, 8), (2, 4), (4, 4), (4, 2)], 8: [(2, 4), (2, 2), (4, 2), (4, 1)]}
@@ -917,7 +988,7 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
             torch.cuda.synchronize()
             ref = oracle.dedisperse(src.numpy(), cfg.nbits, cfg.nsamps, tab)
             assert np.array_equal(out.cpu().numpy(), ref.astype(np.float32))
-    # the pair-row launcher (8-bit input, >= 128 channels) forks onto internal streams and joins them: capturable too
+    # the group-row launcher (8-bit input, >= 128 channels) forks onto internal streams and joins them: capturable too
     cfg8 = W.CONFIGS[5].reduced(nsamps=3072 + 200, ndm=20, nchans=160, nbeams=2)
     tab8 = _oracle_table(cfg8)
     pk8, st8 = W.gen_packed(cfg8, int(tab8.max()))
@@ -925,7 +996,7 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
     out8 = torch.zeros((2, cfg8.ndm, cfg8.nsamps), dtype=torch.float32, device="cuda")
     with dd.Plan(cfg8.nchans, cfg8.dt, cfg8.f_top, cfg8.df, cfg8.nbits) as p:
         p.set_dm_list(cfg8.dm_list())
-        assert p.launch_info()["variant"] == 4
+        assert p.launch_info()["variant"] == 6
         p.set_batch(2, dev8.stride(0), out8.stride(0) * 4)
         with torch.cuda.stream(side):
             p.execute(cfg8.nsamps, dev8, st8, out8, 32, side)
@@ -965,13 +1036,14 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
 
 @pytest.mark.parametrize("case", [
     # (config, nchans, ndm, nsamps, keep one channel in ..., expected variant)
-    (5, 512, 40, 3500, 3, 4), (4, 1024, 64, 4000, 4, 4), (5, 300, 1200, 2000, 2, 4), (3, 4096, 32, 1500, 7, 3),
+    (5, 512, 40, 3500, 3, 6), (4, 1024, 64, 4000, 4, 4), (5, 300, 1200, 2000, 2, 6), (3, 4096, 32, 1500, 7, 3),
     (5, 64, 20, 1500, 1, 3),
 ])
 def test_default_variant_for_4_and_8_bit_input_under_sparse_kill_masks(case):
-    # 4- and 8-bit plans of >= 128 channels take the pair-row variant by default, also when a sparse kill mask pairs
-    # channels that are far apart; when the pair planner cannot serve the table (cfg3's largest DMs, one channel
-    # in seven kept) or the plan is small, the library falls back to variant 3 -- the result is the same either way
+    # plans of >= 128 channels take group rows (variant 6) by default when its cost model says they pay, else -- 4- and
+    # 8-bit input -- the pair rows of variant 4 (here: 64 trials of the 4-bit band under a one-in-four mask), also when a
+    # sparse kill mask groups channels that are far apart; when neither planner can serve the table (cfg3's largest
+    # DMs, one channel in seven kept) or the plan is small, the library falls back to variant 3 -- same result each way
     idx, nchans, ndm, nsamps, mod, want_variant = case
     cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=1)
     dms = W.CONFIGS[3].dm_list()[-32:] if idx == 3 else cfg.dm_list()
