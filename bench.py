@@ -102,7 +102,8 @@ def info_after(plan) -> int:
 
 
 KERNEL_NAMES = {1: "dd_direct_v1<{nbits}>", 2: "dd_direct_v2", 3: "dd_direct_bp<{nbits}>",
-                4: "dd_direct_bp<pair rows of {nbits}-bit input>", 5: "dd_direct_gs<{nbits}>"}
+                4: "dd_direct_bp<pair rows of {nbits}-bit input>", 5: "dd_direct_gs<{nbits}>",
+                6: "dd_make_group_rows_staged<{nbits}> + dd_direct_gr<{nbits}>"}
 
 
 def measured_peaks() -> dict:
