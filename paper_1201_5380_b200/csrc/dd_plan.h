@@ -193,8 +193,12 @@ constexpr int gr_unit_words(int nbits, int G) { return nbits == 2 ? 4 : (nbits =
 #define DD_GR_W2 5
 #define DD_GR_CC2 4
 #endif
+#ifndef DD_GR_CC8
+#define DD_GR_CC8 2
+#define DD_GR_CC4 4
+#endif
 constexpr int kGrW2 = DD_GR_W2;   // units per lane of the 2-bit group-row kernel
-constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? 2 : (nbits == 2 ? DD_GR_CC2 : 4)) : (nbits == 8 ? 4 : 8); }
+constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? DD_GR_CC8 : (nbits == 2 ? DD_GR_CC2 : DD_GR_CC4)) : (nbits == 8 ? 4 : 8); }
 constexpr int kGsW2 = 3, kGsW48 = 2;   // variant 5: units (32 samples) per lane for 2-bit / 4- and 8-bit input (tile = 1024 W samples)
 constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 
