@@ -370,6 +370,7 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     plan->prow.swap(scratch.prow);
     plan->n_prows = scratch.n_prows;
     plan->gr = scratch.gr;
+    plan->gr_stage_slots = scratch.gr_stage_slots;
     plan->gs = scratch.gs;
     plan->gs_G = scratch.gs_G;
     plan->gs_rows = scratch.gs_rows;

@@ -19,8 +19,9 @@
 // (5 x LDS.64, W = 3).
 //
 // Kernels: dd_make_group_rows<nbits, G> (pre-pass, one thread per row and unit) and dd_direct_gr<nbits, G> (16 trials
-// x 1024 W samples per CTA, 16 warps, warp = trial; ring of stages of CC groups with full/empty mbarriers, every
-// warp's lane 0 issues the copies of its share of a stage's rows, as in dd_kernel_bp.cu).
+// x 1024 W samples per CTA, 16 warps, warp = trial; ring of stages with full/empty mbarriers, each holding the rows of as
+// many consecutive groups as fit its byte budget; lanes 0-2 of every warp issue the copies of the warp's share of a
+// stage's rows).
 #include <utility>
 
 #include "dd_bp_core.cuh"
@@ -29,7 +30,6 @@ namespace dd {
 namespace {
 
 constexpr int GR_DB = 16, GR_NWARPS = 16;
-constexpr int GR_FL = kGrFlushStages;   // stages between flushes of the pending words
 
 template <int NBITS, int G>
 struct Gr {
@@ -41,8 +41,11 @@ struct Gr {
     static constexpr int UW = gr_unit_words(NBITS, G);  // words per unit of a row (dd_plan.h)
     static constexpr int UB = UW * 4;
     static constexpr int W = NBITS == 2 ? kGrW2 : 3;    // units per lane
-    static constexpr int CC = gr_groups_per_stage(NBITS, G);
     static constexpr int NP = NBITS == 2 ? 12 : (NBITS == 4 ? 16 : 20);   // sum planes
+    static constexpr int NF = gr_flush_groups(NBITS, G);              // groups between flushes of the pending words
+    static constexpr int GMAX = gr_max_groups_per_stage(NBITS, G);    // most groups a stage holds
+    static constexpr int GQ = gr_group_quantum(NBITS, G);             // stages begin on multiples of GQ groups
+    static_assert(NF % GQ == 0 && GMAX % GQ == 0, "group quantum");
     static_assert(UW >= PIN && (UW == 4 || UW % 2 == 0), "row unit");
 };
 
@@ -322,22 +325,27 @@ __device__ __forceinline__ void gr_add_group(const uint8_t *lane_base, const uin
     }
 }
 
-template <int NBITS, int G, int PHASE, int NP, int NT, int... GIs>
-__device__ __forceinline__ void gr_add_stage(std::integer_sequence<int, GIs...>, const uint8_t *lane_base, const uint2 *rel,
-                                             uint32_t (&P)[Gr<NBITS, G>::W][NP], uint32_t (&T)[Gr<NBITS, G>::W][NT])
+template <class F, int... Is>
+__device__ __forceinline__ void gr_for_each(F &&f, std::integer_sequence<int, Is...>)
 {
-    (gr_add_group<NBITS, G, PHASE * Gr<NBITS, G>::CC + GIs>(lane_base, rel[GIs * GR_DB], P, T), ...);
+    (f(std::integral_constant<int, Is>{}), ...);
 }
 
+// Stages hold a VARIABLE number of groups: the planner packs consecutive groups into a stage until the stage's byte
+// budget (or 48 rows, or GMAX groups) is reached -- the rows a DM block needs per group vary (1 .. 7 on the survey band,
+// 4.1 on average), so stages sized for the worst case of a fixed group count ran at 60 % of their capacity, and the fixed
+// cost of a stage (producer chain, barrier round trips: ~650-1200 clocks per SM sub-partition) weighed on too little work.
+// The pending words are flushed every NF groups, whatever the stage boundaries are.
 // PATCH: the epilogue passes through per-warp shared-memory patches (whole 128-byte lines per store instruction)
 template <int NBITS, int G, bool PATCH>
 __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelParams p)
 {
     using C = Gr<NBITS, G>;
-    constexpr int DB = GR_DB, W = C::W, TB = 32 * 32 * W, NP = C::NP, PIN = C::PIN, CC = C::CC, UB = C::UB;
-    constexpr uint32_t STAGE_SUM = ((1u << PIN) - 1u) * CC;   // weight one stage adds to a counter
-    constexpr int NT = bit_length(GR_FL * STAGE_SUM);         // pending slots
-    constexpr uint32_t REL_BYTES = CC * DB * 8;
+    constexpr int DB = GR_DB, W = C::W, TB = 32 * 32 * W, NP = C::NP, PIN = C::PIN, UB = C::UB;
+    constexpr int NF = C::NF, GMAX = C::GMAX;
+    constexpr uint32_t FLUSH_SUM = ((1u << PIN) - 1u) * NF;   // weight the counters take between flushes
+    constexpr int NT = bit_length(FLUSH_SUM);                 // pending slots
+    constexpr uint32_t REL_BYTES = (GMAX * DB + DB) * 8;      // offset entries of up to GMAX groups + a trailer: groups of the NEXT stage
     constexpr int RPW = 3;                                    // rows a warp stages per stage (the plan keeps rows_per_chunk <= 48)
 
     extern __shared__ __align__(128) uint8_t smem[];
@@ -348,12 +356,12 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     const int blk = static_cast<int>(cta % p.nblk);
     const int tile = static_cast<int>(cta / p.nblk) + p.tile0;   // this launch covers the tiles tile0 .. tile0 + ntiles - 1
     const int64_t t0 = static_cast<int64_t>(tile) * TB;
-    const int nchunks = p.nchunks, NS = p.nstages;
+    const int NS = p.nstages;
 
     // shared memory carve-up (must match dd::gr_smem_bytes)
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);   // [8]
     uint64_t *empty = full + 8;                              // [8]
-    const int rel_slot = static_cast<int>(align128(REL_BYTES));
+    constexpr int rel_slot = static_cast<int>((REL_BYTES + 127) / 128 * 128);
     const int row_slot = p.raw_slot;                         // bytes of a stage's rows (a multiple of 128)
     uint8_t *rel_base = smem + 128 + (PATCH ? GR_NWARPS * kBpPatchBytes : 0);
     uint8_t *row_base = rel_base + NS * rel_slot;
@@ -367,23 +375,26 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     }
     __syncthreads();
 
-    // rows of this launch: p.in holds, per row, the units in_unit0 .. of the time axis, rows in_stride bytes apart
+    // rows of this launch: p.in holds, per row, the units in_unit0 .. of the time axis, rows in_stride bytes apart.
+    // Tables per DM block: p.nchunks stage slots (the largest stage count of any block)
     const uint8_t *in_tile = p.in + ((t0 >> 5) - p.in_unit0) * UB;
-    const int64_t stage0 = static_cast<int64_t>(blk) * nchunks;
-    const int4 *span_blk = p.span + stage0 * p.rows_per_chunk;
+    const int64_t stage0 = static_cast<int64_t>(blk) * p.nchunks;
+    const int4 *span_blk = p.span + (stage0 * p.rows_per_chunk + blk) + 1;   // one header entry ahead of every block's list
     const uint8_t *rel_blk = static_cast<const uint8_t *>(p.rel) + stage0 * REL_BYTES;
+    const int4 hdr = __ldg(span_blk - 1);   // {stages of this block, groups of its first stage, -, -}
+    const int nstg = hdr.x;
 
     // producers: lanes 0 .. RPW - 1 of every warp issue the copies of the warp's rows of a stage (lane k: slot warp +
     // 16 k; one span entry per lane, so that the entries cost 8 registers instead of 24); warp 0 also brings the trials'
     // offset entries.  The span entry of the next stage to issue is fetched one step early.
-    auto load_meta = [&](int chunk) -> int4 {
+    auto load_meta = [&](int stg) -> int4 {
         const int slot = warp + GR_NWARPS * lane;
-        return (lane < RPW && chunk < nchunks && slot < p.rows_per_chunk)
-                   ? __ldg(&span_blk[static_cast<int64_t>(chunk) * p.rows_per_chunk + slot])
+        return (lane < RPW && stg < nstg && slot < p.rows_per_chunk)
+                   ? __ldg(&span_blk[static_cast<int64_t>(stg) * p.rows_per_chunk + slot])
                    : make_int4(0, 0, 0, 0);
     };
     int prod_s = 0, prod_round = 0;
-    auto produce = [&](int chunk, const int4 m) {
+    auto produce = [&](int stg, const int4 m) {
         const int s = prod_s;
         // span entry: {byte offset inside the row for tile 0, bytes, row, byte offset inside the stage}
         uint32_t tx = static_cast<uint32_t>(m.y);
@@ -391,10 +402,10 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         tx += __shfl_down_sync(0xFFFFFFFFu, tx, 1);   // lane 0: bytes of lanes 0 .. 2 (RPW == 3; the other lanes hold 0)
         if (lane == 0) {
             if (prod_round > 0)
-                mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has added chunk - NS
+                mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has added stage stg - NS
             mbar_arrive_expect_tx(&full[s], tx + (warp == 0 ? REL_BYTES : 0u));
             if (warp == 0)
-                tma_bulk_g2s(rel_base + s * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &full[s]);
+                tma_bulk_g2s(rel_base + s * rel_slot, rel_blk + static_cast<int64_t>(stg) * REL_BYTES, REL_BYTES, &full[s]);
         }
         __syncwarp();
         if (m.y > 0)
@@ -409,7 +420,7 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     static_assert(RPW == 3, "the byte count of a warp's copies is summed over lanes 0 .. 2");
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in stages
     int4 meta = load_meta(0);
-    for (int k = 0; k < dist && k < nchunks; ++k) {
+    for (int k = 0; k < dist && k < nstg; ++k) {
         const int4 nxt = load_meta(k + 1);
         produce(k, meta);
         meta = nxt;
@@ -425,41 +436,50 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         for (int k = 0; k < NT; ++k)
             T[j][k] = 0;
     }
-    int s = 0;
-    uint32_t full_parity = 0;
-    auto stage = [&](int chunk, auto phase, auto flush) {
-        constexpr int PHASE = decltype(phase)::value;
-        constexpr uint32_t FLUSH = decltype(flush)::value;
-        if (chunk + dist < nchunks) {
-            const int4 nxt = load_meta(chunk + dist + 1);
-            produce(chunk + dist, meta);
-            meta = nxt;
+    int s = -1, stg = -1, g_in = 0, n_in = 0, n_next = hdr.y;
+    uint32_t full_parity = 1u;
+    // the next stage: release the one just finished, keep the ring fed, wait for the rows
+    auto next_stage = [&]() {
+        if (stg >= 0) {
+            __syncwarp();
+            if (lane == 0)
+                mbar_arrive(&empty[s]);
         }
-        mbar_wait(&full[s], full_parity);
-        gr_add_stage<NBITS, G, PHASE>(std::make_integer_sequence<int, CC>{}, row_base + s * row_slot + lane * (W * UB),
-                                      reinterpret_cast<const uint2 *>(rel_base + s * rel_slot) + warp, P, T);
-        if constexpr (FLUSH != 0u) {
-#pragma unroll
-            for (int j = 0; j < W; ++j)
-                csa_flush<FLUSH, 0, false>(P[j], T[j], 0u);
-        }
-        __syncwarp();
-        if (lane == 0)
-            mbar_arrive(&empty[s]);
-        if (++s == NS) {
+        ++stg;
+        if (++s == NS || stg == 0) {
             s = 0;
             full_parity ^= 1u;
         }
+        if (stg + dist < nstg) {
+            const int4 nxt = load_meta(stg + dist + 1);
+            produce(stg + dist, meta);
+            meta = nxt;
+        }
+        mbar_wait(&full[s], full_parity);
+        n_in = n_next;
+        g_in = 0;
+        n_next = static_cast<int>(reinterpret_cast<const uint2 *>(rel_base + s * rel_slot)[GMAX * DB].x);   // the trailer
     };
-    using NoFlush = std::integral_constant<uint32_t, 0u>;
-    using FlushAll = std::integral_constant<uint32_t, GR_FL * STAGE_SUM>;
-    static_assert(GR_FL == 4, "unroll the phases here");
-    for (int chunk = 0; chunk < nchunks; chunk += GR_FL) {   // nchunks is a multiple of GR_FL by plan construction
-        stage(chunk, std::integral_constant<int, 0>{}, NoFlush{});
-        stage(chunk + 1, std::integral_constant<int, 1>{}, NoFlush{});
-        stage(chunk + 2, std::integral_constant<int, 2>{}, NoFlush{});
-        stage(chunk + 3, std::integral_constant<int, 3>{}, FlushAll{});
+    // one group: CLS = groups added since the last flush
+    auto group = [&](auto cls) {
+        constexpr int CLS = decltype(cls)::value;
+        if constexpr (CLS % C::GQ == 0) {
+            if (g_in == n_in)
+                next_stage();
+        }
+        gr_add_group<NBITS, G, CLS>(row_base + s * row_slot + lane * (W * UB),
+                                    reinterpret_cast<const uint2 *>(rel_base + s * rel_slot)[g_in * DB + warp], P, T);
+        ++g_in;
+    };
+    for (int g = 0; g < p.nchans_pad; g += NF) {   // the group count is a multiple of NF by plan construction
+        gr_for_each(group, std::make_integer_sequence<int, NF>{});
+#pragma unroll
+        for (int j = 0; j < W; ++j)
+            csa_flush<FLUSH_SUM, 0, false>(P[j], T[j], 0u);
     }
+    __syncwarp();
+    if (lane == 0 && stg >= 0)
+        mbar_arrive(&empty[s]);
 
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp` (as in dd_kernel_bp.cu)
     const int d = blk * DB + warp;
@@ -519,8 +539,9 @@ cudaError_t launch_group_rows(dd_plan_s *plan, const KernelParams &kp_in, cudaSt
 {
     using C = Gr<NBITS, G>;
     constexpr int TB = 32 * 32 * C::W, NBI = C::NBR, NSUBI = C::NSUBR;
-    if (!plan->gr || plan->gs_G != G || plan->cc != C::CC || plan->var.TB != TB || kp_in.ngroups != 1 || !plan->d_prow ||
-        kp_in.out_code == kOutPlanes || kp_in.out_code == kOutU8 || kp_in.nchunks % GR_FL != 0 || plan->rows_per_chunk > 48)
+    if (!plan->gr || plan->gs_G != G || plan->var.TB != TB || kp_in.ngroups != 1 || !plan->d_prow ||
+        kp_in.out_code == kOutPlanes || kp_in.out_code == kOutU8 || kp_in.nchans_pad % C::NF != 0 ||
+        plan->rows_per_chunk > 48)
         return cudaErrorInvalidValue;
     cudaError_t e;
     int32_t max_delta = 0;
@@ -657,6 +678,7 @@ cudaError_t launch_group_rows(dd_plan_s *plan, const KernelParams &kp_in, cudaSt
             kp.out = kp_in.out + static_cast<int64_t>(b) * kp_in.out_beam_stride;
             kp.nbeams = 1;
             kp.rows_per_chunk = plan->rows_per_chunk;
+            kp.nchunks = plan->gr_stage_slots;
             kp.tile0 = static_cast<int32_t>(c0);
             kp.ntiles = static_cast<int32_t>(gc);
             kp.in_unit0 = unit0;

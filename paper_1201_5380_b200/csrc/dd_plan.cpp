@@ -604,8 +604,8 @@ dd_status build_tiles_gs(dd_plan_s *p, int G, int cc)
 int64_t gr_smem_bytes(int nbits, int G, int nstages, int stage_bytes, bool patch)
 {
     int64_t b = 128 + (patch ? 16 * static_cast<int64_t>(kBpPatchBytes) : 0);
-    b += nstages * align_up(static_cast<int64_t>(gr_groups_per_stage(nbits, G)) * 16 * 8, 128);   // offset entries of the trials
-    b += static_cast<int64_t>(nstages) * stage_bytes;                                               // rows
+    b += nstages * align_up((static_cast<int64_t>(gr_max_groups_per_stage(nbits, G)) * 16 + 16) * 8, 128);   // offset entries + trailer
+    b += static_cast<int64_t>(nstages) * stage_bytes;                                                          // rows
     return b;
 }
 
@@ -629,16 +629,15 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
         return DD_ERR_SMEM;
     const int W = nbits == 2 ? kGrW2 : 3, TB = 1024 * W, DB = 16;
     const int np = nbits == 2 ? 12 : (nbits == 4 ? 16 : 20);
-    const int uw = gr_unit_words(nbits, G), ub = uw * 4, cc = gr_groups_per_stage(nbits, G);
+    const int uw = gr_unit_words(nbits, G), ub = uw * 4;
+    const int nfg = gr_flush_groups(nbits, G), gmax = gr_max_groups_per_stage(nbits, G), gq = gr_group_quantum(nbits, G);
     const int au = (ub % 16 == 0) ? 1 : 2;   // spans start and end on whole 16 bytes: pairs of units when a unit is 8 (mod 16) bytes
     const int64_t vmax = (1 << nbits) - 1;
     if (static_cast<int64_t>(nlive) * vmax >= (int64_t(1) << np))
         return DD_ERR_SMEM;
-    const int ngr = (nlive + G - 1) / G, fl = kGrFlushStages;
-    const int ents_pad = static_cast<int>(align_up(ngr, cc * fl)), nchunks = ents_pad / cc;
+    const int ngr = (nlive + G - 1) / G;
+    const int ents_pad = static_cast<int>(align_up(ngr, nfg));
     const int nblk = (ndm + DB - 1) / DB;
-    if (nchunks >= 8192)
-        return DD_ERR_SMEM;
 
     // rows: every tuple of every group, in group order; per (trial, group) the row of the trial's tuple
     struct Tuple {
@@ -735,60 +734,93 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
             u.off[i] = d0s[i] - u.start;
         return true;
     };
-    // pass 1: sizes
-    int rs = 1;
-    int64_t stage_bytes = 0, max_end = 0;
+    // pass 1: the largest group; then the byte budget of a stage: a ring of three (two if a single group needs more),
+    // output patches for 2- and 4-bit input when the ring still holds the largest group beside them
     Use u;
+    int64_t max_group = 0, max_end = 0;   // max_group: bytes of the largest quantum of gq consecutive groups
+    int max_qrows = 0;
     for (int b = 0; b < nblk; ++b) {
-        for (int k = 0; k < nchunks; ++k) {
-            int rows_here = 0;
-            int64_t bytes_here = 0;
-            for (int q = k * cc; q < (k + 1) * cc; ++q) {
+        for (int q0 = 0; q0 < ents_pad; q0 += gq) {
+            int64_t qb = 0;
+            int qr = 0;
+            for (int q = q0; q < q0 + gq; ++q) {
                 if (!analyse(b, q, u))
                     return DD_ERR_SMEM;
-                rows_here += u.nrow;
-                bytes_here += static_cast<int64_t>(u.nrow) * u.nbytes;
+                qb += static_cast<int64_t>(u.nrow) * u.nbytes;
+                qr += u.nrow;
                 max_end = std::max<int64_t>(max_end, static_cast<int64_t>(u.start) + u.nbytes / ub * 32);
             }
-            rs = std::max(rs, rows_here);
-            stage_bytes = std::max(stage_bytes, bytes_here);
+            max_group = std::max(max_group, qb);
+            max_qrows = std::max(max_qrows, qr);
         }
     }
-    if (rs > 48)   // the kernel's producers stage at most 3 rows per warp and stage
+    if (max_qrows > 48)
         return DD_ERR_SMEM;
-    stage_bytes = align_up(stage_bytes, 128);
-    if (stage_bytes >= (1 << 20))
-        return DD_ERR_SMEM;
-    // the deepest ring that fits; output patches for 2- and 4-bit input when a ring of three still fits with them
     int nst = 0;
     bool patch = false;
-    for (int n = 4; n >= 2 && nst == 0; --n) {
-        if (nbits < 8 && n >= 3 && gr_smem_bytes(nbits, G, n, static_cast<int>(stage_bytes), true) <= kMaxDynSmem)
-            nst = n, patch = true;
-        else if (gr_smem_bytes(nbits, G, n, static_cast<int>(stage_bytes), false) <= kMaxDynSmem)
-            nst = n, patch = false;
+    int64_t stage_bytes = 0;
+    // ring depth: two large stages beat three smaller ones except for the 9-plane rows of 8-bit pairs (measured with 2 / 3 /
+    // 4 stages: cfg2 7.63 / 8.11 / 8.94 ms, cfg4 69.9 / 72.8 / 79.7, cfg5 143.9 / 146.0 / 151.9, cfg3 193 / 185 / 194)
+    const int ns_pref = (nbits == 8 && G == 2) ? 3 : 2;
+    const int cand[3][2] = {{ns_pref, 1}, {ns_pref, 0}, {2, 0}};
+    for (const auto &cd : cand) {
+        if (cd[1] && nbits == 8)
+            continue;
+        const int64_t fixed = gr_smem_bytes(nbits, G, cd[0], 0, cd[1] != 0);
+        const int64_t budget = (kMaxDynSmem - fixed) / cd[0] / 128 * 128;
+        if (budget >= max_group && budget > 0) {
+            nst = cd[0], patch = cd[1] != 0, stage_bytes = std::min<int64_t>(budget, (1 << 20) - 128);
+            break;
+        }
     }
     if (nst == 0)
         return DD_ERR_SMEM;
-
-    // pass 2: span list [nblk][nchunks][rs] and offsets [nblk][ents_pad][DB]
-    std::vector<SpanMeta> span(static_cast<size_t>(nblk) * nchunks * rs);
-    std::vector<uint8_t> rel(static_cast<size_t>(nblk) * ents_pad * DB * 8);
+    // pass 2: consecutive groups are packed into a stage until its bytes, 48 rows (3 per producer warp) or gmax groups
+    // are reached; stage_of[b] lists the first group of every stage of block b
+    std::vector<std::vector<int32_t>> first(nblk);
+    int nstg_max = 0, rs = 1;
     for (int b = 0; b < nblk; ++b) {
-        for (int k = 0; k < nchunks; ++k) {
-            SpanMeta *sl = span.data() + (static_cast<size_t>(b) * nchunks + k) * rs;
-            for (int j = 0; j < rs; ++j)
-                sl[j] = SpanMeta{0, 0, 0, 0};
+        int64_t bytes = 0;
+        int rows = 0, groups = 0;
+        for (int q0 = 0; q0 < ents_pad; q0 += gq) {   // a quantum of gq groups at a time
+            int64_t gb = 0;
+            int gr_rows = 0;
+            for (int q = q0; q < q0 + gq; ++q) {
+                analyse(b, q, u);
+                gb += static_cast<int64_t>(u.nrow) * u.nbytes;
+                gr_rows += u.nrow;
+            }
+            if (q0 == 0 || groups + gq > gmax || rows + gr_rows > 48 || bytes + gb > stage_bytes) {
+                first[b].push_back(q0);
+                bytes = 0, rows = 0, groups = 0;
+            }
+            bytes += gb, rows += gr_rows, groups += gq;
+            rs = std::max(rs, rows);
+        }
+        first[b].push_back(ents_pad);
+        nstg_max = std::max(nstg_max, static_cast<int>(first[b].size()) - 1);
+    }
+    // pass 3: per block a header {stages, groups of the first stage} and the span list [nstg_max][rs]; offsets
+    // [nblk][nstg_max][gmax * DB entries + a trailer whose first word is the group count of the NEXT stage]
+    const size_t span_blk = static_cast<size_t>(nstg_max) * rs + 1, rel_stage = (static_cast<size_t>(gmax) * DB + DB) * 8;
+    std::vector<SpanMeta> span(static_cast<size_t>(nblk) * span_blk, SpanMeta{0, 0, 0, 0});
+    std::vector<uint8_t> rel(static_cast<size_t>(nblk) * nstg_max * rel_stage, 0);
+    for (int b = 0; b < nblk; ++b) {
+        const int nstg = static_cast<int>(first[b].size()) - 1;
+        span[b * span_blk] = SpanMeta{nstg, first[b][1] - first[b][0], 0, 0};
+        for (int k = 0; k < nstg; ++k) {
+            SpanMeta *sl = span.data() + b * span_blk + 1 + static_cast<size_t>(k) * rs;
+            uint32_t *en = reinterpret_cast<uint32_t *>(rel.data() + (static_cast<size_t>(b) * nstg_max + k) * rel_stage);
+            en[2 * gmax * DB] = k + 1 < nstg ? static_cast<uint32_t>(first[b][k + 2] - first[b][k + 1]) : 0u;   // the trailer
             int slot = 0;
             int32_t dst = 0;
-            for (int gi = 0; gi < cc; ++gi) {
-                const int q = k * cc + gi;
+            for (int q = first[b][k]; q < first[b][k + 1]; ++q) {
                 analyse(b, q, u);
-                uint32_t *en = reinterpret_cast<uint32_t *>(rel.data()) + (static_cast<size_t>(b) * ents_pad + q) * DB * 2;
+                uint32_t *eg = en + static_cast<size_t>(q - first[b][k]) * DB * 2;
                 for (int i = 0; i < DB; ++i) {
                     const uint32_t off = static_cast<uint32_t>(u.off[i]);
-                    en[2 * i] = static_cast<uint32_t>(dst + u.which[i] * u.nbytes) + (off >> 5) * static_cast<uint32_t>(ub);
-                    en[2 * i + 1] = off & 31u;
+                    eg[2 * i] = static_cast<uint32_t>(dst + u.which[i] * u.nbytes) + (off >> 5) * static_cast<uint32_t>(ub);
+                    eg[2 * i + 1] = off & 31u;
                 }
                 for (int j = 0; j < u.nrow; ++j) {
                     sl[slot++] = SpanMeta{u.start / 32 * ub, u.nbytes, u.rows[j], dst};
@@ -797,6 +829,7 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
             }
         }
     }
+    const int cc = gmax;
     p->var = Variant{6, DB, TB, 512, 32, 8, nbits, 0, 4, {cc, 0, 0, 0}, 1 << nbits, np, true, true, ub, 1};
     p->pairs = false;
     p->gs = false;
@@ -809,6 +842,7 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
     p->raw_slot = static_cast<int>(stage_bytes);
     p->lane_slot = p->raw_slot;
     p->rows_per_chunk = rs;
+    p->gr_stage_slots = nstg_max;
     p->cc = cc;
     p->nstages = nst;
     p->ngroups = 1;
@@ -872,17 +906,21 @@ dd_status build_tiles(dd_plan_s *p)
             if (build_tiles_gr(p, G) != DD_OK)
                 continue;
             // cost per 32 output samples, in ALU lane-operations: the bit-plane kernel adds nbits plane words per trial
-            // and channel (a shift + 2.13 LOP3 each); with group rows every trial adds pin words per group (15 % more
-            // overhead per word: smaller stages), every row costs its G shifted loads and ripple adders plus its bytes
-            // written (3.4 lane-operations per byte: 5.5 TB/s against 18.6e12 lane-operations/s; reading them back
-            // overlaps with the adds).  Calibrated on a B200: model 0.61 / 0.61 / 0.78 / 0.94 of the bit-plane kernel
-            // for cfg5 / cfg4 / cfg3 (pairs) / cfg2, measured 0.68 / 0.66 / 0.75 / 0.97.
+            // and channel (a shift + 2.13 LOP3 each); with group rows every trial adds pin words per group, every row
+            // costs its G shifted loads and ripple adders plus its bytes written (3.4 lane-operations per byte: 5.5 TB/s
+            // against 18.6e12 lane-operations/s; reading them back overlaps with the adds).  Calibrated on a B200: model
+            // 0.57 / 0.55 / 0.69 / 0.87 of the bit-plane kernel for cfg5 / cfg4 / cfg3 (pairs) / cfg2, measured 0.64 / 0.62 /
+            // 0.75 / 0.87.
             const double pin = p->nbits + (G == 2 ? 1 : 2), ngr = (p->nlive + G - 1) / G;
             const double direct = 3.13 * p->ndm * static_cast<double>(p->nlive) * p->nbits;
             const double rows = static_cast<double>(p->n_prows) * (G * p->nbits + 2.0 * (G - 1) * (p->nbits + 1) +
                                                                   3.4 * 4.0 * gr_unit_words(p->nbits, G));
-            const double grouped = 1.15 * 3.13 * p->ndm * ngr * pin + rows;
-            if (grouped < 0.9 * direct)
+            const double grouped = 3.13 * p->ndm * ngr * pin + rows;
+            // ... and the rows must not swamp the memory system: written once, read about 1.5 times at ~4 TB/s (11.6
+            // lane-operations per byte of row); cfg3 with rows of four (393 GB of rows, each used by 4 trials only)
+            // measured 590 ms against 185 ms with pairs
+            const double row_bytes = static_cast<double>(p->n_prows) * 4.0 * gr_unit_words(p->nbits, G);
+            if (grouped < 0.9 * direct && 11.6 * row_bytes < 0.9 * direct)
                 return DD_OK;
             p->gr = false;
         }

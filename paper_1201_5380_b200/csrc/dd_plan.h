@@ -140,6 +140,8 @@ struct dd_plan_s {
     // prow holds {c_0 .. c_3 (or -1), delta_0 .. delta_3} per row (8 ints), span [nblk][nchunks][rows_per_chunk]
     // {byte offset in the row for tile 0, bytes, row, byte offset in the stage}, raw_slot = bytes of a stage's rows
     bool gr = false;
+    int gr_stage_slots = 0;               // stage slots per DM block in span / rel (the largest stage count of any block); every
+                                          // block's span list starts with a header entry {stages, groups of the first stage, -, -}
     int sb_gpc = 0;                       // dd_set_tuning: sub-bands per CTA of sub-band step 1 (0 = chosen by the library)
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)
@@ -185,20 +187,22 @@ bool gs_instance_exists(int nbits, int G, int cc);   // is dd_direct_gs<nbits, G
 // Variant 6 (group rows in device memory, dd_kernel_gr.cu): G channels per group (0 = 4).  DD_ERR_SMEM if it cannot serve.
 dd_status build_tiles_gr(dd_plan_s *p, int G);
 int64_t gr_smem_bytes(int nbits, int G, int nstages, int stage_bytes, bool patch);
-constexpr int kGrFlushStages = 4;
+// groups between flushes of the pending words / most groups a stage may hold (its offset entries have a fixed slot)
+constexpr int gr_flush_groups(int nbits, int G) { return nbits == 8 ? 8 : 16; }
+constexpr int gr_max_groups_per_stage(int nbits, int G) { return nbits == 8 ? 8 : 16; }
+#ifndef DD_GR_Q4
+#define DD_GR_Q4 4
+#define DD_GR_Q2 2
+#endif
+// stages begin and end on multiples of this many groups (the kernel tests for a stage boundary once per quantum)
+constexpr int gr_group_quantum(int nbits, int G) { return nbits == 8 ? 1 : (nbits == 4 ? DD_GR_Q4 : DD_GR_Q2); }
 // words per 32-sample unit of a group row: the planes (nbits + log2 G) padded so that the lanes of a warp read without
 // bank conflicts and units stay 8-byte aligned (dd_kernel_gr.cu)
 constexpr int gr_unit_words(int nbits, int G) { return nbits == 2 ? 4 : (nbits == 4 ? 6 : 10); }
 #ifndef DD_GR_W2
 #define DD_GR_W2 5
-#define DD_GR_CC2 4
-#endif
-#ifndef DD_GR_CC8
-#define DD_GR_CC8 2
-#define DD_GR_CC4 4
 #endif
 constexpr int kGrW2 = DD_GR_W2;   // units per lane of the 2-bit group-row kernel
-constexpr int gr_groups_per_stage(int nbits, int G) { return G == 4 ? (nbits == 8 ? DD_GR_CC8 : (nbits == 2 ? DD_GR_CC2 : DD_GR_CC4)) : (nbits == 8 ? 4 : 8); }
 constexpr int kGsW2 = 3, kGsW48 = 2;   // variant 5: units (32 samples) per lane for 2-bit / 4- and 8-bit input (tile = 1024 W samples)
 constexpr int kGsFlushStages = 4;   // stages between flushes of the pending words (dd_kernel_gs.cu: GS_FL)
 

@@ -1036,14 +1036,13 @@ def test_dd_execute_and_scrunch_set_are_cuda_graph_capturable():
 
 @pytest.mark.parametrize("case", [
     # (config, nchans, ndm, nsamps, keep one channel in ..., expected variant)
-    (5, 512, 40, 3500, 3, 6), (4, 1024, 64, 4000, 4, 4), (5, 300, 1200, 2000, 2, 6), (3, 4096, 32, 1500, 7, 3),
+    (5, 512, 40, 3500, 3, 6), (4, 1024, 64, 4000, 4, 6), (5, 300, 1200, 2000, 2, 6), (3, 4096, 32, 1500, 7, 3),
     (5, 64, 20, 1500, 1, 3),
 ])
 def test_default_variant_for_4_and_8_bit_input_under_sparse_kill_masks(case):
-    # plans of >= 128 channels take group rows (variant 6) by default when its cost model says they pay, else -- 4- and
-    # 8-bit input -- the pair rows of variant 4 (here: 64 trials of the 4-bit band under a one-in-four mask), also when a
-    # sparse kill mask groups channels that are far apart; when neither planner can serve the table (cfg3's largest
-    # DMs, one channel in seven kept) or the plan is small, the library falls back to variant 3 -- same result each way
+    # plans of >= 128 channels take group rows (variant 6) by default when its cost model says they pay, also when a
+    # sparse kill mask groups channels that are far apart; when the rows do not pay or fit (cfg3's largest DMs, one
+    # channel in seven kept) or the plan is small, the library falls back to variant 3 -- the same result each way
     idx, nchans, ndm, nsamps, mod, want_variant = case
     cfg = W.CONFIGS[idx].reduced(nsamps=nsamps, ndm=ndm, nchans=nchans, nbeams=1)
     dms = W.CONFIGS[3].dm_list()[-32:] if idx == 3 else cfg.dm_list()
