@@ -188,7 +188,11 @@ bool gs_instance_exists(int nbits, int G, int cc);   // is dd_direct_gs<nbits, G
 dd_status build_tiles_gr(dd_plan_s *p, int G);
 int64_t gr_smem_bytes(int nbits, int G, int nstages, int stage_bytes, bool patch);
 // groups between flushes of the pending words / most groups a stage may hold (its offset entries have a fixed slot)
-constexpr int gr_flush_groups(int nbits, int G) { return nbits == 8 ? 8 : 16; }
+#ifndef DD_GR_NF2
+#define DD_GR_NF2 16
+#define DD_GR_NF8 8
+#endif
+constexpr int gr_flush_groups(int nbits, int G) { return nbits == 8 ? DD_GR_NF8 : (nbits == 2 ? DD_GR_NF2 : 16); }
 constexpr int gr_max_groups_per_stage(int nbits, int G) { return nbits == 8 ? 8 : 16; }
 #ifndef DD_GR_Q4
 #define DD_GR_Q4 4
