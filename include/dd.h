@@ -264,7 +264,7 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
  *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20);
- *            4 = pair rows (2/4/8-bit; the default for 4- and 8-bit plans of >= 128 channels): the same kernel
+ *            4 = pair rows (2/4/8-bit; opt-in, and the fallback of variant 6 for 4- and 8-bit plans): the same kernel
  *                over rows x[c0] + shift(x[c1], delta) made once per
  *                delay difference delta of every pair of adjacent summed channels -- exact, n + 1 plane words per
  *                pair instead of 2 n; costs device memory for the rows of one beam (16x / 26x / 12x its packed
@@ -274,7 +274,12 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *            5 = group sums made inside the CTA (2/4/8-bit, opt-in): per group of 2 or 4 adjacent summed channels and
  *                block of 16 trials, one row per pattern of delay differences is built in shared memory from the staged
  *                bit planes by builder warps, and every trial adds the row of its own pattern -- exact like variant 4,
- *                but the rows never reach device memory.
+ *                but the rows never reach device memory (slower than variants 3 / 6);
+ *            6 = group rows (2/4/8-bit; the DEFAULT for plans of >= 128 channels whenever the planner's cost model says
+ *                it pays): one pre-summed row per group of four (or two) adjacent summed channels and tuple of delay
+ *                differences of the DM list, n + 2 bit planes added per four channels instead of 4 n -- exact; costs device
+ *                memory for the rows (dd_set_workspace_limit) like variant 4 and runs on the same internal streams
+ *                (DESIGN.md section 5.5).
  * Takes effect at the next dd_set_dm_list (which returns DD_ERR_SMEM if that variant cannot serve the plan).
  */
 dd_status dd_set_kernel_variant(dd_plan plan, int variant);
@@ -284,12 +289,12 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant);
  * variables).  Results never depend on them.
  *   key    DD_TUNE_SUBBAND_GPC: sub-bands summed one after the other by a CTA of sub-band step 1;
  *            0 = chosen by the library.  Takes effect at the next dd_execute.
- *          DD_TUNE_GROUP_SIZE: channels per group of variant 5 (2 or 4); 0 = chosen by the planner.
- *          DD_TUNE_GROUPS_PER_STAGE: groups per pipeline stage of variant 5 (one of the compiled shapes: 2-bit 16 / 8
- *            pairs or 8 / 4 groups of four, 4-bit 8 / 4 or 4 / 2, 8-bit 4 / 2 or 2 / 1); 0 = chosen by the planner.
+ *          DD_TUNE_GROUP_SIZE: channels per group of variants 5 and 6 (2 or 4); 0 = chosen by the planner.
+ *          DD_TUNE_GROUPS_PER_STAGE: groups per pipeline stage of variant 5 (one of the compiled shapes: 2-bit 16 pairs
+ *            or 4 groups of four, 4-bit 8 or 4, 8-bit 4 / 2 or 2 / 1); 0 = chosen by the planner.
  *            Both take effect at the next dd_set_dm_list (DD_ERR_SMEM if no compiled shape matches or fits).
- *          DD_TUNE_PAIR_TILES: time tiles per group of pair rows of variant 4 (its launcher builds and transforms the
- *            rows group by group); 0 = as many as the workspace limit allows.  Takes effect at the next dd_execute.
+ *          DD_TUNE_PAIR_TILES: time tiles per group of rows of variants 4 and 6 (their launchers build and transform the
+ *            rows group of tiles by group); 0 = as many as the workspace limit allows.  Takes effect at the next dd_execute.
  *   value  >= 0.
  * DD_ERR_INVALID_ARG for an unknown key or a negative value.
  */
@@ -298,9 +303,10 @@ dd_status dd_set_tuning(dd_plan plan, int key, int value);
 
 /*
  * dd_set_workspace_limit / dd_get_workspace_bytes -- device memory the plan takes beside its tables.
- * Every bit-plane variant keeps a bit-plane copy of the packed input (same size as the input).  Variant 4 (the default
- * for 4- and 8-bit plans of >= 128 channels) also keeps the pair rows of one group of time tiles (two groups when the
- * call has several beams or the time axis is split): 12-26 x the packed input of a beam if the whole time axis is one
+ * Every bit-plane variant keeps a bit-plane copy of the packed input (same size as the input).  Variants 6 (the default
+ * for larger plans) and 4 also keep the rows of one group of time tiles (two groups when the call has several beams or
+ * the time axis is split): 25-105 x the packed input of a beam for variant 6 on the survey-shaped configs (9.6 GB for
+ * 1024 channels x 1200 trials x 2^19 2-bit samples, 12.5 GB per 8-bit beam of 2^18 samples) if the whole time axis is one
  * group.  The buffers are allocated by the first dd_execute / dd_execute_host that needs them and re-used afterwards;
  * they grow (cudaFree + cudaMalloc, which synchronise the device) only when a later call needs more.  The split of
  * the time axis is worked out once per launch geometry (time tiles x beams) and kept.

@@ -21,7 +21,6 @@
 // with full/empty mbarriers per ring slot (no CTA-wide barrier in the loop).  The builder warps copy and build, the
 // adder warps only add (measured with every warp doing all three jobs: per stage and warp ~1000 clocks issuing
 // copies, ~2400 building, ~2600 adding -- the latency chains of the first two stalled the adds).
-#include <cstdio>
 #include <utility>
 
 #include "dd_bp_core.cuh"
@@ -312,21 +311,12 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
         for (int k = 0; k < DT && k < nchunks; ++k)
             issue(k);
         int bs = 0, bs_round = 0, bp = 0, bp_round = 0;
-#ifdef GS_X_TIMING
-        uint32_t tm_issue = 0, tm_wraw = 0, tm_wrow = 0, tm_items = 0, tk = clock();
-#define GS_TICK(acc) { const uint32_t now_ = clock(); acc += now_ - tk; tk = now_; }
-#else
-#define GS_TICK(acc)
-#endif
         for (int chunk = 0; chunk < nchunks; ++chunk) {
             if (chunk + DT < nchunks)
                 issue(chunk + DT);
-            GS_TICK(tm_issue)
             mbar_wait(&raw_full[bs], bs_round & 1);
-            GS_TICK(tm_wraw)
             if (bp_round > 0)
                 mbar_wait(&row_empty[bp], (bp_round - 1) & 1);   // every adder is done with chunk - NSP
-            GS_TICK(tm_wrow)
             if (bw == 0 && lane == 0) {   // the trials' offset entries travel with the row slot
                 mbar_expect_tx(&row_full[bp], REL_BYTES);
                 tma_bulk_g2s(rel_base + bp * rel_slot, rel_blk + static_cast<int64_t>(chunk) * REL_BYTES, REL_BYTES, &row_full[bp]);
@@ -367,13 +357,7 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
                 bp = 0;
                 ++bp_round;
             }
-            GS_TICK(tm_items)
         }
-#ifdef GS_X_TIMING
-        if (lane == 0 && (cta == 5 || cta == 3000) && (bw == 0 || bw == 3))
-            printf("cta %d builder %d stages %d: per stage issue %u wait raw_full %u wait row_empty %u items %u\n", (int)cta, bw, nchunks,
-                   tm_issue / nchunks, tm_wraw / nchunks, tm_wrow / nchunks, tm_items / nchunks);
-#endif
         return;
     }
 
@@ -390,16 +374,10 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
     }
     int cs = 0;
     uint32_t cs_parity = 0;
-#ifdef GS_X_TIMING
-    uint32_t tm_wait = 0, tm_add = 0, tka = clock();
-#endif
     auto stage = [&](auto phase, auto flush) {
         constexpr int PHASE = decltype(phase)::value;
         constexpr uint32_t FLUSH = decltype(flush)::value;
         mbar_wait(&row_full[cs], cs_parity);
-#ifdef GS_X_TIMING
-        { const uint32_t n_ = clock(); tm_wait += n_ - tka; tka = n_; }
-#endif
         gs_add_stage<NBITS, G, CC, PHASE>(std::make_integer_sequence<int, CC>{}, row_base + cs * row_slot,
                                           reinterpret_cast<const uint2 *>(rel_base + cs * rel_slot) + warp, lane, p.gs_row_units,
                                           P, T);
@@ -415,9 +393,6 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
             cs = 0;
             cs_parity ^= 1u;
         }
-#ifdef GS_X_TIMING
-        { const uint32_t n_ = clock(); tm_add += n_ - tka; tka = n_; }
-#endif
     };
     using NoFlush = std::integral_constant<uint32_t, 0u>;
     using FlushAll = std::integral_constant<uint32_t, GS_FL * STAGE_SUM>;
@@ -429,10 +404,6 @@ __global__ void __launch_bounds__((GS_NWARPS + NBW) * 32, 1) dd_direct_gs(const 
         stage(std::integral_constant<int, 3>{}, FlushAll{});
     }
 
-#ifdef GS_X_TIMING
-    if (lane == 0 && (cta == 5 || cta == 3000) && (warp == 0 || warp == 9))
-        printf("cta %d adder %d: per stage wait row_full %u add %u\n", (int)cta, warp, tm_wait / nchunks, tm_add / nchunks);
-#endif
     // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp` (as in dd_kernel_bp.cu)
     const int d = blk * DB + warp;
     if (d >= p.ndm)
@@ -499,14 +470,10 @@ cudaError_t launch_gs_inst(dd_plan_s *plan, const KernelParams &kp, cudaStream_t
 }  // namespace
 
 // The instantiations compiled in: {nbits, G, groups per stage}; dd_plan.cpp::build_tiles_gs picks among them.
-#ifdef GS_X_ONLY
-#define DD_GS_INSTANCES(X) X(8, 2, 4)
-#else
 #define DD_GS_INSTANCES(X) \
     X(8, 2, 4) X(8, 2, 2) X(8, 4, 2) X(8, 4, 1) \
-    X(4, 2, 8) X(4, 2, 4) X(4, 4, 4) X(4, 4, 2) \
-    X(2, 2, 16) X(2, 2, 8) X(2, 4, 8) X(2, 4, 4)
-#endif
+    X(4, 2, 8) X(4, 4, 4) \
+    X(2, 2, 16) X(2, 4, 4)
 
 bool gs_instance_exists(int nbits, int G, int cc)
 {

@@ -864,8 +864,8 @@ dd_status build_tiles_gr(dd_plan_s *p, int G)
 static dd_status build_tiles_gs_auto(dd_plan_s *p)
 {
     static const int shapes[3][2][2][2] = {
-        /* 2-bit */ {{{2, 16}, {2, 8}}, {{4, 8}, {4, 4}}},
-        /* 4-bit */ {{{2, 8}, {2, 4}}, {{4, 4}, {4, 2}}},
+        /* 2-bit */ {{{2, 16}, {2, 16}}, {{4, 4}, {4, 4}}},
+        /* 4-bit */ {{{2, 8}, {2, 8}}, {{4, 4}, {4, 4}}},
         /* 8-bit */ {{{2, 4}, {2, 2}}, {{4, 2}, {4, 1}}},
     };
     const int wi = p->nbits == 2 ? 0 : (p->nbits == 4 ? 1 : 2);
