@@ -41,7 +41,7 @@ struct Gr {
     static constexpr int UW = gr_unit_words(NBITS, G);  // words per unit of a row (dd_plan.h)
     static constexpr int UB = UW * 4;
     static constexpr int W = NBITS == 2 ? kGrW2 : 3;    // units per lane
-    static constexpr int NP = NBITS == 2 ? 12 : (NBITS == 4 ? 16 : 20);   // sum planes
+    static constexpr int NP = NBITS == 2 ? 12 : (NBITS == 4 ? 16 : 20);   // sum planes (8-bit: 18 when the sums fit)
     static constexpr int NF = gr_flush_groups(NBITS, G);              // groups between flushes of the pending words
     static constexpr int GMAX = gr_max_groups_per_stage(NBITS, G);    // most groups a stage holds
     static constexpr int GQ = gr_group_quantum(NBITS, G);             // stages begin on multiples of GQ groups
@@ -286,24 +286,25 @@ __device__ __forceinline__ void gr_add_planes(const uint32_t (&x0)[Gr<NBITS, G>:
     }
 }
 
-// plane K of every unit of the lane (the W counters advance side by side: most instruction-level parallelism)
-template <int NBITS, int G, int CLS, int K, int NP, int NT>
-__device__ __forceinline__ void gr_add_planes_all(const uint32_t (&x)[Gr<NBITS, G>::W + 1][Gr<NBITS, G>::PIN], uint32_t shift,
-                                                  uint32_t (&P)[Gr<NBITS, G>::W][NP], uint32_t (&T)[Gr<NBITS, G>::W][NT])
+// plane K of the units [J0, J1) of the lane (their counters advance side by side: instruction-level parallelism)
+template <int NBITS, int G, int CLS, int K, int J0, int J1, int NP, int NT>
+__device__ __forceinline__ void gr_add_planes_some(const uint32_t (&x)[Gr<NBITS, G>::W + 1][Gr<NBITS, G>::PIN], uint32_t shift,
+                                                   uint32_t (&P)[Gr<NBITS, G>::W][NP], uint32_t (&T)[Gr<NBITS, G>::W][NT])
 {
     using C = Gr<NBITS, G>;
     if constexpr (K < C::PIN) {
         constexpr uint32_t S = ((1u << C::PIN) - 1u) * CLS + ((1u << K) - 1u);
 #pragma unroll
-        for (int j = 0; j < C::W; ++j)
+        for (int j = J0; j < J1; ++j)
             csa_add<S, K>(P[j], T[j], __funnelshift_r(x[j][K], x[j + 1][K], shift));
-        gr_add_planes_all<NBITS, G, CLS, K + 1>(x, shift, P, T);
+        gr_add_planes_some<NBITS, G, CLS, K + 1, J0, J1>(x, shift, P, T);
     }
 }
 
 // The counters of the W units are independent, so the order of the units is free.  Plane by plane over all units gives
-// the most parallelism (measured best for 2- and 4-bit input and 8-bit groups of four); unit by unit keeps only two
-// units' words live, which the 9-plane rows of 8-bit pairs need to stay clear of spills (cfg3: 196 -> 185 ms).
+// the most parallelism (measured best for 4-bit input and 8-bit groups of four); unit by unit keeps only two units'
+// words live, which the 9-plane rows of 8-bit pairs need to stay clear of spills (cfg3: 196 -> 185 ms).  (The five units
+// of 2-bit input in two runs of three and two: 7.91 ms against 7.66 ms on cfg2, no fewer spills.)
 template <int NBITS, int G, int CLS, int NP, int NT>
 __device__ __forceinline__ void gr_add_group(const uint8_t *lane_base, const uint2 e, uint32_t (&P)[Gr<NBITS, G>::W][NP],
                                              uint32_t (&T)[Gr<NBITS, G>::W][NT])
@@ -321,7 +322,7 @@ __device__ __forceinline__ void gr_add_group(const uint8_t *lane_base, const uin
 #pragma unroll
         for (int j = 0; j <= C::W; ++j)
             gr_load_unit<C::UW, C::PIN>(lane_base + e.x + j * C::UB, x[j]);
-        gr_add_planes_all<NBITS, G, CLS, 0>(x, e.y, P, T);
+        gr_add_planes_some<NBITS, G, CLS, 0, 0, C::W>(x, e.y, P, T);
     }
 }
 
@@ -337,11 +338,13 @@ __device__ __forceinline__ void gr_for_each(F &&f, std::integer_sequence<int, Is
 // cost of a stage (producer chain, barrier round trips: ~650-1200 clocks per SM sub-partition) weighed on too little work.
 // The pending words are flushed every NF groups, whatever the stage boundaries are.
 // PATCH: the epilogue passes through per-warp shared-memory patches (whole 128-byte lines per store instruction)
-template <int NBITS, int G, bool PATCH>
+// NP: sum planes (sums < 2^NP; 8-bit plans of up to 1028 channels run with 18 instead of 20: six registers fewer, cfg5
+// 144.2 -> 141.5 ms)
+template <int NBITS, int G, bool PATCH, int NP = Gr<NBITS, G>::NP>
 __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelParams p)
 {
     using C = Gr<NBITS, G>;
-    constexpr int DB = GR_DB, W = C::W, TB = 32 * 32 * W, NP = C::NP, PIN = C::PIN, UB = C::UB;
+    constexpr int DB = GR_DB, W = C::W, TB = 32 * 32 * W, PIN = C::PIN, UB = C::UB;
     constexpr int NF = C::NF, GMAX = C::GMAX;
     constexpr uint32_t FLUSH_SUM = ((1u << PIN) - 1u) * NF;   // weight the counters take between flushes
     constexpr int NT = bit_length(FLUSH_SUM);                 // pending slots
@@ -641,6 +644,10 @@ cudaError_t launch_group_rows(dd_plan_s *plan, const KernelParams &kp_in, cudaSt
     if (plan->prof_mid)
         cudaEventRecord(static_cast<cudaEvent_t>(plan->prof_mid), stream);
     auto kernel = plan->patch ? dd_direct_gr<NBITS, G, true> : dd_direct_gr<NBITS, G, false>;
+    if constexpr (NBITS == 8) {
+        if (static_cast<int64_t>(plan->nlive) * 255 < (int64_t(1) << 18))
+            kernel = dd_direct_gr<8, G, false, 18>;   // (8-bit plans never use the output patches)
+    }
     if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan->smem_bytes))) != cudaSuccess)
         return e;
     const int64_t ublocks = (units_g + GR_UBLK - 1) / GR_UBLK;
