@@ -295,10 +295,13 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant);
  *            Both take effect at the next dd_set_dm_list (DD_ERR_SMEM if no compiled shape matches or fits).
  *          DD_TUNE_PAIR_TILES: time tiles per group of rows of variants 4 and 6 (their launchers build and transform the
  *            rows group of tiles by group); 0 = as many as the workspace limit allows.  Takes effect at the next dd_execute.
+ *          DD_TUNE_TILES_PER_CTA: consecutive time tiles a CTA of the short bit-plane kernel walks (plans with few channels
+ *            per group: step 2 of the sub-band method, small transforms); 0 = as many as leave 8 waves of CTAs, at most 8.
+ *            Takes effect at the next dd_execute.
  *   value  >= 0.
  * DD_ERR_INVALID_ARG for an unknown key or a negative value.
  */
-enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3, DD_TUNE_PAIR_TILES = 4 };
+enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3, DD_TUNE_PAIR_TILES = 4, DD_TUNE_TILES_PER_CTA = 5 };
 dd_status dd_set_tuning(dd_plan plan, int key, int value);
 
 /*

@@ -22,7 +22,7 @@ __all__ = [
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE",
-    "DD_TUNE_PAIR_TILES", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
@@ -264,7 +264,7 @@ def dd_set_kernel_variant(plan: int, variant: int) -> None:
     _check(lib().dd_set_kernel_variant(plan, int(variant)), "dd_set_kernel_variant")
 
 
-DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE, DD_TUNE_PAIR_TILES = 1, 2, 3, 4
+DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE, DD_TUNE_PAIR_TILES, DD_TUNE_TILES_PER_CTA = 1, 2, 3, 4, 5
 
 
 def dd_set_tuning(plan: int, key: int, value: int) -> None:

@@ -334,6 +334,9 @@ static dd_status replan(dd_plan_s *plan, std::vector<double> dm, std::vector<uin
     destroy_subplan(plan->s2);
     plan->s1 = s1;
     plan->s2 = s2;
+    for (dd_plan_s *q : {s1, s2})
+        if (q)
+            q->bp_tpc = plan->bp_tpc;
     plan->sb_nchans = sb_nchans;
     plan->dm_group = dm_group;
     plan->sb_nominal.swap(scratch.sb_nominal);
@@ -881,6 +884,12 @@ dd_status dd_set_tuning(dd_plan plan, int key, int value)
         return DD_OK;
     case DD_TUNE_PAIR_TILES:
         plan->pair_tiles = value;
+        return DD_OK;
+    case DD_TUNE_TILES_PER_CTA:
+        plan->bp_tpc = value;
+        for (dd_plan_s *q : {plan->s1, plan->s2})
+            if (q)
+                q->bp_tpc = value;
         return DD_OK;
     }
     return DD_ERR_INVALID_ARG;

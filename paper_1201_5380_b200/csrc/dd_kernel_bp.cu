@@ -264,16 +264,22 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
     const int64_t cta = blockIdx.x;
     const int blk = static_cast<int>(cta % p.nblk);
     const int64_t rest = cta / p.nblk;
-    const int tile = static_cast<int>(rest % p.ntiles) + (PAIRS ? p.tile0 : 0);
-    const int batch = static_cast<int>(rest / p.ntiles);          // (beam, set of gpc channel groups); gpc = 1: (beam, group)
+    // Short instantiation without pair rows: a CTA walks p.tpc consecutive time tiles of its DM block (the ring of stages
+    // runs on across them, so the first copies of a tile and the drain of its output hide behind the tile before and
+    // after -- CTAs of a few stages, as in step 2 of the sub-band method, otherwise expose both once per tile)
+    constexpr bool MULTI = !LONG && !PAIRS;
+    const int ntile_slots = MULTI ? (p.ntiles + p.tpc - 1) / p.tpc : p.ntiles;
+    const int tile = MULTI ? static_cast<int>(rest % ntile_slots) * p.tpc : static_cast<int>(rest % p.ntiles) + (PAIRS ? p.tile0 : 0);
+    const int batch = static_cast<int>(rest / ntile_slots);       // (beam, set of gpc channel groups); gpc = 1: (beam, group)
     int beam, group, nch_set = 0;   // group: the first one of the set; nch_set: stages this CTA works through
     if constexpr (LONG) {           // always one group per CTA
         beam = batch / p.ngroups, group = batch - beam * p.ngroups;
     } else {
         const int nsets = (p.ngroups + p.gpc - 1) / p.gpc;
         beam = batch / nsets, group = (batch - beam * nsets) * p.gpc;
-        nch_set = min(p.gpc, p.ngroups - group) * p.nchunks;
+        nch_set = min(p.gpc, p.ngroups - group) * p.nchunks * (MULTI ? min(p.tpc, p.ntiles - tile) : 1);
     }
+    const bool walk = MULTI && p.tpc > 1;   // several tiles per CTA: stage k belongs to tile k / nchunks (gpc == 1 then)
     auto nchunks_cta = [&]() -> int {   // LONG: straight from the parameter bank, no register held across the loop
         if constexpr (LONG)
             return p.nchunks;
@@ -322,7 +328,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                            ? __ldg(&span_blk[static_cast<int64_t>(chunk) * p.rows_per_chunk + slot])
                            : make_int4(0, 0, 0, 0);
             } else {
-                m[k] = (lane == 0 && chunk < nchunks_cta()) ? __ldg(&span_blk[chunk * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
+                const int cm = walk ? chunk % p.nchunks : chunk;
+                m[k] = (lane == 0 && chunk < nchunks_cta()) ? __ldg(&span_blk[cm * CC + (warp * CPW + k) / NSUB]) : make_int4(0, 0, 0, 0);
             }
         }
     };
@@ -362,15 +369,18 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                     }
                 }
             }
+            // several tiles per CTA: the stage belongs to tile chunk / nchunks, its spans lie TB samples per tile further
+            const int ct = walk ? chunk / p.nchunks : 0, cm = walk ? chunk - ct * p.nchunks : chunk;
+            const uint8_t *in_here = in_tile + static_cast<int64_t>(ct) * (TB / 32) * UB;
 #pragma unroll
             for (int k = 0; k < (PAIRS ? 0 : CPW); ++k) {
                 const int cl = (warp * CPW + k) / NSUB, sub = (warp * CPW + k) % NSUB;
-                const uint8_t *src = in_tile + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x;
+                const uint8_t *src = in_here + static_cast<int64_t>(m[k].z) * p.in_stride + sub * p.in_row_bytes + m[k].x;
                 tma_bulk_g2s(raw_base + s * raw_stage + cl * p.raw_slot + sub * p.sub_slot, src, static_cast<uint32_t>(m[k].y),
                              &full[s]);
             }
             if (warp == 0)
-                tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(chunk) * CC * DB,
+                tma_bulk_g2s(rel_base + s * rel_stage, rel_blk + static_cast<int64_t>(cm) * CC * DB,
                              static_cast<uint32_t>(CC * DB * 8), &full[s]);
         }
         __syncwarp();
@@ -466,13 +476,75 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
                 P[j][k] = 0;
         }
     };
-    int cig = 0, gi = 0;   // stages done of the current group, groups done
+    // ---- epilogue of one tile: thread owns samples t0x + 32*(W*lane + j) + [0, 32) of DM slot `warp`
+    // Interior tiles (the whole time block inside the row, vector stores allowed) go through a per-warp patch of
+    // shared memory so that every store instruction writes whole 128-byte lines.  The patches lie outside the
+    // stage ring: a warp that is done stores while the others are still adding.
+    auto store_out = [&](int64_t t0x) {
+        const int d = blk * DB + warp;
+        if (d >= p.ndm)
+            return;
+        const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
+        uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.out_dm_stride;
+        const bool interior = PATCH && p.vec16_ok && (t0x + TB <= p.nsamps);   // 16-byte stores: rows must be 16-byte aligned
+        uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            uint32_t q[32];   // the 32 sums of the unit, in time order
+            if constexpr (NP <= 16) {
+                uint32_t R[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k)
+                    R[k] = k < NP ? P[j][k] : 0u;
+                transpose16x2(R);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    q[k] = R[k] & 0xFFFFu;
+                    q[16 + k] = R[k] >> 16;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                    q[k] = k < NP ? P[j][k] : 0u;
+                transpose32(q);
+            }
+            if (interior) {
+                uint8_t *gunit = orow + (t0x + 32 * j) * esize;   // unit j of lane 0; lane s is W * 32 samples further
+                if (p.out_code == DD_OUT_F32)
+                    store_unit_coalesced<4, true>(q, patch, lane, gunit, W * 32 * 4);
+                else if (p.out_code == DD_OUT_U32)
+                    store_unit_coalesced<4, false>(q, patch, lane, gunit, W * 32 * 4);
+                else if (p.out_code == DD_OUT_U16)
+                    store_unit_coalesced<2, false>(q, patch, lane, gunit, W * 32 * 2);
+                else
+                    store_unit_coalesced<1, false>(q, patch, lane, gunit, W * 32);
+            } else {
+                const int64_t tunit = t0x + 32 * (W * lane + j);
+#pragma unroll
+                for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
+                    const uint32_t q4[4] = {q[4 * h], q[4 * h + 1], q[4 * h + 2], q[4 * h + 3]};
+                    store4(p, orow, tunit + 4 * h, q4);
+                }
+            }
+        }
+    };
+    int cig = 0, gi = 0;   // stages done of the current group / tile, groups / tiles done
     for (int chunk = 0; chunk < nchunks_cta(); chunk += FL) {
         if constexpr (FL == 1) {
             stage(chunk, std::integral_constant<int, 0>{}, FlushAll{});
-            if (p.out_code == kOutPlanes && ++cig == p.nchunks) {
+            if (++cig == p.nchunks) {   // a channel group (bit-plane output) or a time tile is complete
                 cig = 0;
-                store_planes(group + gi);
+                if (p.out_code == kOutPlanes) {
+                    store_planes(group + gi);
+                } else {
+                    store_out(t0 + static_cast<int64_t>(gi) * TB);
+#pragma unroll
+                    for (int j = 0; j < W; ++j) {
+#pragma unroll
+                        for (int k = 0; k < NP; ++k)
+                            P[j][k] = 0;
+                    }
+                }
                 ++gi;
             }
         } else if constexpr (FL == 2) {
@@ -486,61 +558,8 @@ __global__ void __launch_bounds__(BP_NWARPS * 32, 1) dd_direct_bp(const KernelPa
             stage(chunk + 3, std::integral_constant<int, 3>{}, FlushAll{});
         }
     }
-
-    // ---- epilogue: thread owns samples t0 + 32*(W*lane + j) + [0, 32) of DM slot `warp`
-    // Interior tiles (the whole time block inside the row, vector stores allowed) go through a per-warp patch of
-    // shared memory so that every store instruction writes whole 128-byte lines.  The patches lie outside the
-    // stage ring: a warp that is done stores while the others are still adding.
-    if constexpr (!LONG) {
-        if (p.out_code == kOutPlanes)
-            return;
-    }
-    const int d = blk * DB + warp;
-    if (d >= p.ndm)
-        return;
-    const int esize = (p.out_code == DD_OUT_U16) ? 2 : (p.out_code == kOutU8 ? 1 : 4);
-    uint8_t *orow = p.out + static_cast<int64_t>(batch) * p.out_beam_stride + static_cast<int64_t>(d) * p.out_dm_stride;
-    const bool interior = PATCH && p.vec16_ok && (t0 + TB <= p.nsamps);   // 16-byte stores: rows must be 16-byte aligned
-    uint8_t *patch = smem + 128 + warp * kBpPatchBytes;
-#pragma unroll
-    for (int j = 0; j < W; ++j) {
-        uint32_t q[32];   // the 32 sums of the unit, in time order
-        if constexpr (NP <= 16) {
-            uint32_t R[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k)
-                R[k] = k < NP ? P[j][k] : 0u;
-            transpose16x2(R);
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                q[k] = R[k] & 0xFFFFu;
-                q[16 + k] = R[k] >> 16;
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < 32; ++k)
-                q[k] = k < NP ? P[j][k] : 0u;
-            transpose32(q);
-        }
-        if (interior) {
-            uint8_t *gunit = orow + (t0 + 32 * j) * esize;   // unit j of lane 0; lane s is W * 32 samples further
-            if (p.out_code == DD_OUT_F32)
-                store_unit_coalesced<4, true>(q, patch, lane, gunit, W * 32 * 4);
-            else if (p.out_code == DD_OUT_U32)
-                store_unit_coalesced<4, false>(q, patch, lane, gunit, W * 32 * 4);
-            else if (p.out_code == DD_OUT_U16)
-                store_unit_coalesced<2, false>(q, patch, lane, gunit, W * 32 * 2);
-            else
-                store_unit_coalesced<1, false>(q, patch, lane, gunit, W * 32);
-        } else {
-            const int64_t tunit = t0 + 32 * (W * lane + j);
-#pragma unroll
-            for (int h = 0; h < 8; ++h) {   // samples 4h .. 4h+3 of the unit
-                const uint32_t q4[4] = {q[4 * h], q[4 * h + 1], q[4 * h + 2], q[4 * h + 3]};
-                store4(p, orow, tunit + 4 * h, q4);
-            }
-        }
-    }
+    if constexpr (FL > 1)   // (with a flush after every stage the tiles were stored inside the loop)
+        store_out(t0);
 }
 
 template <int NBITS>
@@ -618,7 +637,18 @@ cudaError_t launch_bp(dd_plan_s *plan, const KernelParams &kp_in, cudaStream_t s
         kp.gpc = 1;
 
     const int64_t nsets = (kp.ngroups + kp.gpc - 1) / kp.gpc;
-    const int64_t ctas = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * nsets;
+    // short plans (few stages per tile: step 2 of the sub-band method, small transforms): a CTA walks several time tiles,
+    // as many as leave >= 8 waves of CTAs, at most 8 (dd_set_tuning(DD_TUNE_TILES_PER_CTA) overrides)
+    kp.tpc = 1;
+    if (!plan->long_mode && kp.out_code != kOutPlanes && kp.gpc == 1) {
+        int sms = 148;
+        (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, plan->device >= 0 ? plan->device : 0);
+        const int64_t all = static_cast<int64_t>(kp.nblk) * kp.ntiles * kp.nbeams * nsets;
+        int64_t t = plan->bp_tpc > 0 ? plan->bp_tpc : all / (8 * static_cast<int64_t>(sms));
+        t = t < 1 ? 1 : (t > 8 && plan->bp_tpc <= 0 ? 8 : t);
+        kp.tpc = static_cast<int32_t>(t > kp.ntiles ? kp.ntiles : t);
+    }
+    const int64_t ctas = static_cast<int64_t>(kp.nblk) * ((kp.ntiles + kp.tpc - 1) / kp.tpc) * kp.nbeams * nsets;
     if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
         return cudaErrorInvalidConfiguration;
     if (plan->long_mode && kp.nchunks % C::FL != 0)

@@ -42,6 +42,7 @@ struct KernelParams {
     int64_t pl_beam;          // bytes between beams
     int32_t pl_units;         // units (32 samples) per sub-row
     int32_t gpc;              // channel groups summed one after the other by a CTA (>= 1; > 1 only with kOutPlanes)
+    int32_t tpc;              // time tiles a CTA of the short bit-plane instantiation walks (>= 1; > 1 only with gpc == 1)
     int32_t rows_per_chunk;   // pair rows (variant 4): rows staged per stage; span is [nblk][nchunks][rows_per_chunk]
     int32_t tile0;            // pair rows: this launch covers the time tiles tile0 .. tile0 + ntiles - 1 ...
     int64_t in_unit0;         // ... and `in` holds the pair rows from unit in_unit0 (32 samples per unit) on

@@ -377,6 +377,35 @@ def test_variant3_bitplane_4_and_8_bit_tiles_and_channel_padding(nbits):
     _full_compare(base.reduced(nsamps=3072 + 8, ndm=2, nchans=5), out_kinds=["u32"], variant=3)
 
 
+@pytest.mark.parametrize("tpc", [0, 1, 2, 3, 8])
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_variant3_short_plans_walk_several_time_tiles_per_cta(nbits, tpc):
+    # plans with few channels (the short instantiation of the bit-plane kernel: step 2 of the sub-band method, small
+    # transforms) let a CTA walk several consecutive time tiles with the ring of stages running on across them:
+    # 7 tiles and a ragged 8th, 1 / 2 / 3 / 8 tiles per CTA (ragged last CTA), the library's own choice, two beams,
+    # all output types, every element against the oracle
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    tb = 5120 if nbits == 2 else 3072
+    cfg = full.reduced(nsamps=7 * tb + 555, ndm=21, nchans=40, nbeams=2)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    dev = packed.cuda()
+    for kind in (["u32", "f32"] + (["u16"] if nbits < 8 else [])):
+        out = torch.full((2, cfg.ndm, cfg.nsamps), -1, dtype=_TORCH_OUT[kind], device="cuda")
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
+            p.set_tuning(dd.DD_TUNE_TILES_PER_CTA, tpc)
+            p.set_dm_list(cfg.dm_list())
+            p.set_batch(2, dev.stride(0), out.stride(0) * out.element_size())
+            p.execute(cfg.nsamps, dev, stride, out, {"f32": 32, "u32": -32, "u16": 16}[kind], torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            assert p.launch_info()["variant"] == 3
+        got = out.cpu().numpy().view(_NP_VIEW[kind])
+        for b in range(2):
+            ref = oracle.cast_out(oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab), kind)
+            bad = np.nonzero(got[b] != ref)
+            assert bad[0].size == 0, f"{kind} beam {b}: {bad[0].size} mismatches, first at d={bad[0][0]} t={bad[1][0]}"
+
+
 @pytest.mark.parametrize("nbits", [4, 8])
 def test_variant3_bitplane_4_and_8_bit_extreme_values(nbits):
     # every sample at its maximum with the largest channel count the planes hold: 4369 * 15 = 65535 (all 16
