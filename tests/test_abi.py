@@ -248,3 +248,49 @@ def test_scrunch_set_host_side():
             dd.ScrunchSet(64, 64e-6, 1500.0, -1.0, 2, bad["dm"], bad["mf"])
     with pytest.raises(dd.DDError):
         dd.ScrunchSet(64, 64e-6, 1500.0, +1.0, 2, [0.0], 2)                 # observing parameters are validated too
+
+
+def test_tuning_and_workspace_knobs_host_side():
+    """dd_set_tuning / dd_set_workspace_limit / dd_get_workspace_bytes: argument checks and what the planner makes of the
+    knobs, without a device (the library reads no environment variables: these calls are the only launch-geometry knobs)."""
+    L = dd.lib()
+    assert L.dd_set_tuning(None, dd.DD_TUNE_GROUP_SIZE, 4) == -1
+    assert L.dd_set_workspace_limit(None, 0) == -1
+    assert L.dd_get_workspace_bytes(None) == -1
+    cfg = W.CONFIGS[5]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        for key, value in ((0, 1), (99, 1), (dd.DD_TUNE_GROUP_SIZE, 3), (dd.DD_TUNE_GROUP_SIZE, -1), (dd.DD_TUNE_PAIR_TILES, -2)):
+            assert L.dd_set_tuning(p.handle, key, value) == -2, (key, value)
+        assert L.dd_set_workspace_limit(p.handle, -1) == -2
+        assert p.workspace_bytes == 0                       # nothing is allocated before the first dd_execute
+        p.set_dm_list(cfg.dm_list())
+        info = p.launch_info()
+        assert info["variant"] == 6 and info["smem_bytes"] <= 227 * 1024 and info["time_block"] == 3072   # rows of four by default
+        p.set_tuning(dd.DD_TUNE_GROUP_SIZE, 2).set_dm_list(cfg.dm_list())
+        assert p.launch_info()["variant"] == 6              # pairs serve this plan too
+        p.set_tuning(dd.DD_TUNE_GROUP_SIZE, 0)
+    # the default choice per config: group rows where the cost model says they pay, the bit-plane kernel for the tiny one
+    for idx, want in ((1, 3), (2, 6), (3, 6), (4, 6)):
+        c = W.CONFIGS[idx]
+        with dd.Plan(c.nchans, c.dt, c.f_top, c.df, c.nbits) as p:
+            p.set_dm_list(c.dm_list())
+            assert p.launch_info()["variant"] == want, idx
+    # a promise about the samples keeps the plan on the plane-skipping bit-plane kernel, also when made after the DM list
+    c = W.CONFIGS[5]
+    with dd.Plan(c.nchans, c.dt, c.f_top, c.df, c.nbits) as p:
+        p.set_dm_list(c.dm_list())
+        assert p.launch_info()["variant"] == 6
+        p.set_input_max(31)
+        assert p.launch_info()["variant"] == 3
+        p.set_input_max(0)
+        assert p.launch_info()["variant"] == 6
+    # every variant can be forced; 2-bit input has no rows of two in variant 6
+    c = W.CONFIGS[2].reduced(nsamps=4096, ndm=40)
+    for variant in (1, 2, 3, 4, 5, 6):
+        with dd.Plan(c.nchans, c.dt, c.f_top, c.df, c.nbits, variant=variant) as p:
+            p.set_dm_list(c.dm_list())
+            assert p.launch_info()["variant"] == variant
+    with dd.Plan(c.nchans, c.dt, c.f_top, c.df, c.nbits, variant=6) as p:
+        p.set_tuning(dd.DD_TUNE_GROUP_SIZE, 2)
+        with pytest.raises(dd.DDError):
+            p.set_dm_list(c.dm_list())
