@@ -420,15 +420,23 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
                    : make_int4(0, 0, 0, 0);
     };
     int prod_s = 0, prod_round = 0;
-    auto produce = [&](int stg, const int4 m) {
+    // blocking: wait for the slot to be released; otherwise give up (return false) if it has not been yet
+    auto produce = [&](int stg, const int4 m, bool blocking) -> bool {
         const int s = prod_s;
+        uint32_t ready = 1u;
+        if (lane == 0 && prod_round > 0) {   // every warp has added stage stg - NS?
+            if (blocking)
+                mbar_wait(&empty[s], (prod_round - 1) & 1);
+            else
+                ready = mbar_test(&empty[s], (prod_round - 1) & 1) ? 1u : 0u;
+        }
+        if (!__shfl_sync(0xFFFFFFFFu, ready, 0))
+            return false;
         // span entry: {byte offset inside the row for tile 0, bytes, row, byte offset inside the stage}
         uint32_t tx = static_cast<uint32_t>(m.y);
         tx += __shfl_down_sync(0xFFFFFFFFu, tx, 2);
         tx += __shfl_down_sync(0xFFFFFFFFu, tx, 1);   // lane 0: bytes of lanes 0 .. 2 (RPW == 3; the other lanes hold 0)
         if (lane == 0) {
-            if (prod_round > 0)
-                mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has added stage stg - NS
             mbar_arrive_expect_tx(&full[s], tx + (warp == 0 ? REL_BYTES : 0u));
             if (warp == 0)
                 tma_bulk_g2s(rel_base + s * rel_slot, rel_blk + static_cast<int64_t>(stg) * REL_BYTES, REL_BYTES, &full[s]);
@@ -442,13 +450,14 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
             prod_s = 0;
             ++prod_round;
         }
+        return true;
     };
     static_assert(RPW == 3, "the byte count of a warp's copies is summed over lanes 0 .. 2");
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in stages
     int4 meta = load_meta(0);
     for (int k = 0; k < dist && k < nstg; ++k) {
         const int4 nxt = load_meta(k + 1);
-        produce(k, meta);
+        produce(k, meta, true);
         meta = nxt;
     }
 
@@ -465,6 +474,16 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     int s = -1, stg = -1, g_in = 0, n_in = 0, n_next = hdr.y;
     uint32_t full_parity = 1u;
     // the next stage: release the one just finished, keep the ring fed, wait for the rows
+    // The copies of stage stg + dist are issued as soon as the slot is free, but a warp does not WAIT for that: it tries at
+    // every group quantum and goes on adding meanwhile (the slot is free when the slowest warp has left the stage before;
+    // waiting there made every warp as slow as the slowest plus the wait -- a fifth of the warp instructions were spins).
+    int pend_stg = -1;   // stage whose copies are still to be issued (its span entry is in `meta`), or -1
+    auto try_produce = [&](bool blocking) {
+        if (produce(pend_stg, meta, blocking)) {
+            meta = load_meta(pend_stg + 1);
+            pend_stg = -1;
+        }
+    };
     auto next_stage = [&]() {
         if (stg >= 0) {
             __syncwarp();
@@ -476,11 +495,10 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
             s = 0;
             full_parity ^= 1u;
         }
-        if (stg + dist < nstg) {
-            const int4 nxt = load_meta(stg + dist + 1);
-            produce(stg + dist, meta);
-            meta = nxt;
-        }
+        if (pend_stg >= 0)   // (only if it is the stage needed next or the ring is deeper than the backlog: issue it now)
+            try_produce(true);
+        if (stg + dist < nstg)
+            pend_stg = stg + dist;
         mbar_wait(&full[s], full_parity);
         n_in = n_next;
         g_in = 0;
@@ -492,6 +510,8 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         if constexpr (CLS % C::GQ == 0) {
             if (g_in == n_in)
                 next_stage();
+            if (pend_stg >= 0)
+                try_produce(false);
         }
         gr_add_group<NBITS, G, CLS>(row_base + s * row_slot + lane * (W * UB),
                                     reinterpret_cast<const uint2 *>(rel_base + s * rel_slot)[g_in * DB + warp], P, T);
