@@ -421,22 +421,25 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     };
     int prod_s = 0, prod_round = 0;
     // blocking: wait for the slot to be released; otherwise give up (return false) if it has not been yet
-    auto produce = [&](int stg, const int4 m, bool blocking) -> bool {
+    auto produce = [&](int stg, const int4 m, auto blocking_) -> bool {
+        constexpr bool BLOCKING = decltype(blocking_)::value;
         const int s = prod_s;
-        uint32_t ready = 1u;
-        if (lane == 0 && prod_round > 0) {   // every warp has added stage stg - NS?
-            if (blocking)
-                mbar_wait(&empty[s], (prod_round - 1) & 1);
-            else
+        if constexpr (!BLOCKING) {
+            uint32_t ready = 1u;
+            if (lane == 0 && prod_round > 0)   // every warp has added stage stg - NS?
                 ready = mbar_test(&empty[s], (prod_round - 1) & 1) ? 1u : 0u;
+            if (!__shfl_sync(0xFFFFFFFFu, ready, 0))
+                return false;
         }
-        if (!__shfl_sync(0xFFFFFFFFu, ready, 0))
-            return false;
         // span entry: {byte offset inside the row for tile 0, bytes, row, byte offset inside the stage}
         uint32_t tx = static_cast<uint32_t>(m.y);
         tx += __shfl_down_sync(0xFFFFFFFFu, tx, 2);
         tx += __shfl_down_sync(0xFFFFFFFFu, tx, 1);   // lane 0: bytes of lanes 0 .. 2 (RPW == 3; the other lanes hold 0)
         if (lane == 0) {
+            if constexpr (BLOCKING) {
+                if (prod_round > 0)
+                    mbar_wait(&empty[s], (prod_round - 1) & 1);   // every warp has added stage stg - NS
+            }
             mbar_arrive_expect_tx(&full[s], tx + (warp == 0 ? REL_BYTES : 0u));
             if (warp == 0)
                 tma_bulk_g2s(rel_base + s * rel_slot, rel_blk + static_cast<int64_t>(stg) * REL_BYTES, REL_BYTES, &full[s]);
@@ -452,12 +455,14 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         }
         return true;
     };
+    using Blocking = std::true_type;
+    using NonBlocking = std::false_type;
     static_assert(RPW == 3, "the byte count of a warp's copies is summed over lanes 0 .. 2");
     const int dist = NS > 2 ? NS - 2 : 1;   // prefetch distance in stages
     int4 meta = load_meta(0);
     for (int k = 0; k < dist && k < nstg; ++k) {
         const int4 nxt = load_meta(k + 1);
-        produce(k, meta, true);
+        produce(k, meta, Blocking{});
         meta = nxt;
     }
 
@@ -477,8 +482,12 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
     // The copies of stage stg + dist are issued as soon as the slot is free, but a warp does not WAIT for that: it tries at
     // every group quantum and goes on adding meanwhile (the slot is free when the slowest warp has left the stage before;
     // waiting there made every warp as slow as the slowest plus the wait -- a fifth of the warp instructions were spins).
+    // (Not for 8-bit input: there the warps -- and with them the CTAs of adjacent DM blocks -- drifting apart cost L2 hits:
+    // cfg3 read 250 GB instead of 169 GB from DRAM and took 178 ms instead of 168 ms, cfg5 124 ms instead of 122 ms; cfg4 gained
+    // 6.5 %, cfg2 1 %.)
+    constexpr bool DEFER = NBITS < 8;
     int pend_stg = -1;   // stage whose copies are still to be issued (its span entry is in `meta`), or -1
-    auto try_produce = [&](bool blocking) {
+    auto try_produce = [&](auto blocking) {
         if (produce(pend_stg, meta, blocking)) {
             meta = load_meta(pend_stg + 1);
             pend_stg = -1;
@@ -495,10 +504,16 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
             s = 0;
             full_parity ^= 1u;
         }
-        if (pend_stg >= 0)   // (only if it is the stage needed next or the ring is deeper than the backlog: issue it now)
-            try_produce(true);
-        if (stg + dist < nstg)
-            pend_stg = stg + dist;
+        if constexpr (DEFER) {
+            if (pend_stg >= 0)   // still not issued, and it is the stage needed next: wait for the slot now
+                try_produce(Blocking{});
+            if (stg + dist < nstg)
+                pend_stg = stg + dist;
+        } else if (stg + dist < nstg) {
+            const int4 nxt = load_meta(stg + dist + 1);
+            produce(stg + dist, meta, Blocking{});
+            meta = nxt;
+        }
         mbar_wait(&full[s], full_parity);
         n_in = n_next;
         g_in = 0;
@@ -510,8 +525,10 @@ __global__ void __launch_bounds__(GR_NWARPS * 32, 1) dd_direct_gr(const KernelPa
         if constexpr (CLS % C::GQ == 0) {
             if (g_in == n_in)
                 next_stage();
-            if (pend_stg >= 0)
-                try_produce(false);
+            if constexpr (DEFER) {
+                if (pend_stg >= 0)
+                    try_produce(NonBlocking{});
+            }
         }
         gr_add_group<NBITS, G, CLS>(row_base + s * row_slot + lane * (W * UB),
                                     reinterpret_cast<const uint2 *>(rel_base + s * rel_slot)[g_in * DB + warp], P, T);
