@@ -18,7 +18,7 @@
 // read conflict-free: 2-bit groups of four 4 words (LDS.128, W = 5), 4-bit 6 words (3 x LDS.64, W = 3), 8-bit 10 words
 // (5 x LDS.64, W = 3).
 //
-// Kernels: dd_make_group_rows<nbits, G> (pre-pass, one thread per row and unit) and dd_direct_gr<nbits, G> (16 trials
+// Kernels: dd_make_group_rows_staged<nbits, G> (pre-pass, one block per group and 256 units) and dd_direct_gr<nbits, G> (16 trials
 // x 1024 W samples per CTA, 16 warps, warp = trial; ring of stages with full/empty mbarriers, each holding the rows of as
 // many consecutive groups as fit its byte budget; lanes 0-2 of every warp issue the copies of the warp's share of a
 // stage's rows).
@@ -71,95 +71,14 @@ __device__ __forceinline__ void gr_load_unit(const uint8_t *q, uint32_t (&w)[PIN
 }
 
 // ------------------------------------------------------------------------------------------ pre-pass
-// One thread per (row, unit).  in: bit planes of the input [c][sub-row][unit][NBR planes] (dd_to_bitplanes), in_units
-// units per row, zero beyond the input.  grow: per row {c_0 .. c_3 (or -1), delta_0 = 0 .. delta_3}.  out holds the units
-// unit0 .. unit0 + out_units - 1 of every row (a group of time tiles), out_pitch_words words per row.
-template <int NBITS, int G>
-__global__ void __launch_bounds__(256) dd_make_group_rows(const uint32_t *__restrict__ in, int64_t in_row_words, int64_t in_units,
-                                                          const int4 *__restrict__ grow, uint32_t *__restrict__ out,
-                                                          int64_t out_pitch_words, int64_t out_units, int64_t ublocks, int64_t unit0)
-{
-    using C = Gr<NBITS, G>;
-    const int64_t blk = blockIdx.x;
-    const int64_t r = blk / ublocks, ul = (blk - r * ublocks) * blockDim.x + threadIdx.x;   // unit inside the buffer
-    if (ul >= out_units)
-        return;
-    const int64_t u = unit0 + ul;   // unit of the row
-    const int4 gc = __ldg(&grow[2 * r]), gd = __ldg(&grow[2 * r + 1]);
-    const int ch[4] = {gc.x, gc.y, gc.z, gc.w};
-    const int dl[4] = {gd.x, gd.y, gd.z, gd.w};
-    const int64_t in_sub_words = in_row_words / C::NSUBR;
-    uint32_t x[G][NBITS];
-#pragma unroll
-    for (int i = 0; i < G; ++i) {
-        if (ch[i] >= 0) {
-            const int64_t ub = u + (dl[i] >> 5);
-            const uint32_t sh = static_cast<uint32_t>(dl[i]) & 31u;
-            const uint32_t *rb = in + static_cast<int64_t>(ch[i]) * in_row_words;
-#pragma unroll
-            for (int sub = 0; sub < C::NSUBR; ++sub) {   // all planes of a sub-row unit in one vector load (lo and hi unit)
-                const uint32_t *q = rb + sub * in_sub_words + ub * C::NBR;
-                uint32_t lo[C::NBR], hi[C::NBR];
-                if constexpr (C::NBR == 4) {
-                    const uint4 a = ub < in_units ? __ldg(reinterpret_cast<const uint4 *>(q)) : make_uint4(0, 0, 0, 0);
-                    const uint4 b = ub + 1 < in_units ? __ldg(reinterpret_cast<const uint4 *>(q + 4)) : make_uint4(0, 0, 0, 0);
-                    lo[0] = a.x, lo[1] = a.y, lo[2] = a.z, lo[3] = a.w;
-                    hi[0] = b.x, hi[1] = b.y, hi[2] = b.z, hi[3] = b.w;
-                } else {
-                    const uint2 a = ub < in_units ? __ldg(reinterpret_cast<const uint2 *>(q)) : make_uint2(0, 0);
-                    const uint2 b = ub + 1 < in_units ? __ldg(reinterpret_cast<const uint2 *>(q + 2)) : make_uint2(0, 0);
-                    lo[0] = a.x, lo[1] = a.y;
-                    hi[0] = b.x, hi[1] = b.y;
-                }
-#pragma unroll
-                for (int kk = 0; kk < C::NBR; ++kk)
-                    x[i][sub * C::NBR + kk] = __funnelshift_r(lo[kk], hi[kk], sh);
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < NBITS; ++k)
-                x[i][k] = 0u;
-        }
-    }
-    uint32_t o[C::UW];
-#pragma unroll
-    for (int k = 0; k < C::UW; ++k)
-        o[k] = 0u;
-    uint32_t c01 = 0u, c23 = 0u, cs = 0u;
-#pragma unroll
-    for (int k = 0; k < NBITS; ++k) {
-        const uint32_t s01 = x[0][k] ^ x[1][k] ^ c01;
-        c01 = (x[0][k] & x[1][k]) | (c01 & (x[0][k] ^ x[1][k]));
-        if constexpr (G == 2) {
-            o[k] = s01;
-        } else {
-            const uint32_t s23 = x[2][k] ^ x[3][k] ^ c23;
-            c23 = (x[2][k] & x[3][k]) | (c23 & (x[2][k] ^ x[3][k]));
-            o[k] = s01 ^ s23 ^ cs;
-            cs = (s01 & s23) | (cs & (s01 ^ s23));
-        }
-    }
-    if constexpr (G == 2) {
-        o[NBITS] = c01;
-    } else {
-        o[NBITS] = c01 ^ c23 ^ cs;
-        o[NBITS + 1] = (c01 & c23) | (cs & (c01 ^ c23));
-    }
-    uint32_t *dst = out + r * out_pitch_words + ul * C::UW;
-    if constexpr (C::UW == 4) {
-        *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
-    } else {
-#pragma unroll
-        for (int h = 0; h < C::UW / 2; ++h)
-            *reinterpret_cast<uint2 *>(dst + 2 * h) = make_uint2(o[2 * h], o[2 * h + 1]);
-    }
-}
-
-// The same rows, one thread block per (group, block of GR_UBLK units): the spans of the group's G channels are staged
-// in shared memory ONCE and every row (tuple) of the group is made from them -- the group's ~140 rows differ only in
-// their bit offsets into the same data, which the one-thread-per-(row, unit) kernel above fetched again per row through
-// L1/L2 (measured on cfg5: 5.96 ms per beam for 12.5 GB of rows; L2-bound).  Rows leave through a per-warp
-// shared-memory patch as whole 16-byte vectors of consecutive addresses.
+// in: bit planes of the input [c][sub-row][unit][NBR planes] (dd_to_bitplanes), in_units units per row, zero beyond the
+// input.  grow: per row {c_0 .. c_3 (or -1), delta_0 = 0 .. delta_3}.  out holds the units unit0 .. unit0 + out_units - 1 of
+// every row (a group of time tiles), out_pitch_words words per row.
+// One thread block per (group, block of GR_UBLK units): the spans of the group's G channels are staged in shared memory
+// ONCE and every row (tuple) of the group is made from them -- the group's ~140 rows differ only in their bit offsets
+// into the same data, which a first kernel with one thread per (row, unit) fetched again per row through L1/L2 (measured
+// on cfg5: 5.96 ms per beam for 12.5 GB of rows; L2-bound).  Rows leave through a per-warp shared-memory patch as whole
+// 16-byte vectors of consecutive addresses.
 //   gbase  [ngroups + 1] first row of every group;  span_units: units staged per channel (GR_UBLK + the largest
 //   difference of the plan in units + 2)
 constexpr int GR_UBLK = 256;
@@ -222,7 +141,7 @@ __global__ void __launch_bounds__(GR_UBLK) dd_make_group_rows_staged(const uint3
     // The rows of a group are sorted by (delta_1, delta_2, delta_3): consecutive rows mostly share delta_1 and often
     // delta_2, so x0 is read once, x0 + x1 is kept while delta_1 stays, the shifted x2 while delta_2 stays, and only x3
     // is shifted for every row -- a third of the shared-memory loads and half the ripple adders of making every row anew
-    // (cfg5: 3.88 -> ms per beam; the builder was bound by the shared-memory pipe).
+    // (cfg5: 3.88 -> 2.31 ms per beam; the builder was bound by the shared-memory pipe and now writes at the HBM rate).
     uint32_t x0[NBITS];
 #pragma unroll
     for (int sub = 0; sub < C::NSUBR; ++sub) {   // channel 0 has no shift
