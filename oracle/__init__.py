@@ -25,7 +25,8 @@ from . import build as _build
 from .oracle_np import (delay_table_np, dedisperse_gather_np, dedisperse_points,  # noqa: F401
                         unpack_np, dedisperse_loops_py, subband_tables, subband_required_samples,
                         subband_dedisperse_np, time_scrunch_np, diagonal_dm_np, scrunch_factors_np,
-                        scrunched_dedisperse_np)
+                        scrunched_dedisperse_np, tree_theta, tree_phi, tree_np, tree_delays_np, piecewise_tree_tables,
+                        piecewise_tree_required_samples, piecewise_tree_np)
 
 _LIB: Optional[ctypes.CDLL] = None
 
@@ -160,3 +161,19 @@ def cast_out(sums: np.ndarray, kind: str) -> np.ndarray:
         assert mx < (1 << 24), "sum is not exactly representable in float32"
         return s.astype(np.float32)
     raise ValueError(kind)
+
+
+def tree(packed: np.ndarray, nbits: int, nsamps: int) -> np.ndarray:
+    """The basic tree transform (eq. 7-15) of one packed beam uint8 [N][stride], N a power of two:
+    int64 D'[d'][t], d' < N."""
+    n = packed.shape[0]
+    return tree_np(unpack(packed, nbits, nsamps + n - 1), nsamps)
+
+
+def piecewise_tree(packed: np.ndarray, nbits: int, nsamps: int, nchans: int, dt: float, f_top: float, df: float, dm_list,
+                   sb_nchans: int) -> np.ndarray:
+    """The piecewise linear tree method (eq. 16-23; readings X1-X5 in oracle_np.py) of one packed beam:
+    int64 [ndm][nsamps]."""
+    dprime, dt2 = piecewise_tree_tables(nchans, dt, f_top, df, dm_list, sb_nchans)
+    need = piecewise_tree_required_samples(nsamps, dprime, dt2, sb_nchans)
+    return piecewise_tree_np(unpack(packed, nbits, need), nsamps, dprime, dt2, sb_nchans)

@@ -212,3 +212,115 @@ def scrunched_dedisperse_np(a: np.ndarray, nsamps: int, nchans: int, dt: float, 
                 res[i] += series[c, d:d + ns] * (1 if mask is None else int(mask[c] != 0))
         out.append((F, int(idx[0]), res))
     return out
+
+
+# ------------------------------------------------------------------------------------------ tree dedispersion
+# PAPER.md:125-167 (section 3.1, eq. 7-15) and PAPER.md:181-222 (section 3.1.1, eq. 16-23).  Readings:
+#   X1  The tree IS its recursion (eq. 10-13 with Theta of eq. 14 and the shuffle Phi of eq. 15 as printed; "division is
+#       taken to be truncated integer division").  Eq. 7-8 describe it: the recursion's delays equal round(d' nu / (N - 1))
+#       exactly for N <= 8 and deviate by at most one sample for larger N (pinned), so eq. 8 is not used to compute.
+#   X2  Eq. 11-12 read: A^{i+1}[2 nu + b][t] = A^i[Phi(r, 2 nu)][t] + A^i[Phi(r, 2 nu + 1)][t + Theta(i, 2 nu + b)], r = 2^i.
+#   X3  Eq. 19 (difference of two rounded delays) and eq. 20 (the difference rounded once) disagree by one sample now and
+#       then; eq. 20 is taken: d'_n(d) = round(DM_d [DeltaT(nu_{n+1}) - DeltaT(nu_n)]), DeltaT(c) = k_DM (f_c^-2 - f_top^-2)/dt
+#       also at c = N (one channel past the band, for the last sub-band).
+#   X4  Eq. 23's sum runs over the sub-bands before n, so it telescopes: Dt''_n(d) = round(DM_d DeltaT(nu_n)) -- the direct
+#       delay (eq. 5) of the sub-band's first channel.
+#   X5  Eq. 16 reads N'_nu = N_nu / N_s; a trial with some d'_n(d) >= N'_nu lies beyond the diagonal DM (eq. 21) and is an
+#       error of the basic method.
+def tree_theta(i: int, nu: int) -> int:
+    """Eq. 14: Theta(i, nu) = [(nu mod 2^(i+1)) + 1] / 2, truncated."""
+    return ((nu % (1 << (i + 1))) + 1) // 2
+
+
+def tree_phi(r: int, nu: int) -> int:
+    """Eq. 15: Phi(r, nu) = (nu mod 2) r + nu / 2 + (nu / 2r) r, truncated divisions, r = 2^i."""
+    return (nu % 2) * r + nu // 2 + (nu // (2 * r)) * r
+
+
+def tree_np(a: np.ndarray, nsamps: int) -> np.ndarray:
+    """Eq. 10-13 step by step on unpacked samples a [N][>= nsamps + N - 1], N a power of two: int64 D'[d'][t], d' < N,
+    t < nsamps.  Samples read past the end of a row count as zero (they never reach an output t < nsamps)."""
+    a = np.asarray(a).astype(np.int64)
+    n = a.shape[0]
+    steps = n.bit_length() - 1
+    assert n == 1 << steps and a.shape[1] >= nsamps + n - 1
+    length = a.shape[1]
+    cur = a
+    for i in range(steps):
+        r = 1 << i
+        nxt = np.zeros_like(cur)
+        for nu in range(n // 2):
+            for b in (0, 1):
+                th = tree_theta(i, 2 * nu + b)
+                first, second = cur[tree_phi(r, 2 * nu)], cur[tree_phi(r, 2 * nu + 1)]
+                nxt[2 * nu + b] = first
+                nxt[2 * nu + b, :length - th] += second[th:]
+        cur = nxt
+    return cur[:, :nsamps]
+
+
+def tree_delays_np(n: int) -> np.ndarray:
+    """The delays the recursion applies: int64 [d'][channel], found by running eq. 10-15 on index sets (every output must
+    hold every channel exactly once)."""
+    steps = n.bit_length() - 1
+    assert n == 1 << steps
+    cur = [{c: 0} for c in range(n)]
+    for i in range(steps):
+        r = 1 << i
+        nxt = []
+        for o in range(n):
+            nu, th = o // 2, tree_theta(i, o)
+            d = dict(cur[tree_phi(r, 2 * nu)])
+            for c, dl in cur[tree_phi(r, 2 * nu + 1)].items():
+                assert c not in d
+                d[c] = dl + th
+            nxt.append(d)
+        cur = nxt
+    out = np.zeros((n, n), dtype=np.int64)
+    for dp in range(n):
+        assert sorted(cur[dp]) == list(range(n))
+        for c, dl in cur[dp].items():
+            out[dp, c] = dl
+    return out
+
+
+def piecewise_tree_tables(nchans: int, dt: float, f_top: float, df: float, dm_list, sb_nchans: int):
+    """Eq. 19-23 (readings X3, X4): (d'_n(d) [ndm][Ns], Dt''_n(d) [ndm][Ns]) for sub-bands of sb_nchans channels, float64."""
+    dm = np.asarray(dm_list, dtype=np.float64)
+    assert nchans % sb_nchans == 0
+    ns = nchans // sb_nchans
+    edges = f_top + (np.arange(ns + 1) * sb_nchans).astype(np.float64) * df          # nu_0 .. nu_Ns
+    big_t = K_DM * (1.0 / edges ** 2 - 1.0 / (f_top * f_top)) / dt                  # DeltaT(nu_n), eq. 4
+    dprime = np.floor(dm[:, None] * (big_t[1:] - big_t[:-1])[None, :] + 0.5).astype(np.int64)     # eq. 20
+    dt2 = np.floor(dm[:, None] * big_t[:-1][None, :] + 0.5).astype(np.int64)                      # eq. 23
+    return dprime, dt2
+
+
+def piecewise_tree_required_samples(nsamps: int, dprime: np.ndarray, dt2: np.ndarray, sb_nchans: int) -> int:
+    """Input samples per row the two stages read: stage 2 reads S_n at t + Dt''_n(d) for t < nsamps, stage 1 makes
+    S_n[d'][t'] from samples up to t' + d' (the tree's delays reach d' at the sub-band's last channel); stage 1 is run on
+    whole rows of nsamps + max Dt'' + sb_nchans - 1 samples."""
+    return int(nsamps + dt2.max() + sb_nchans - 1)
+
+
+def piecewise_tree_np(a: np.ndarray, nsamps: int, dprime: np.ndarray, dt2: np.ndarray, sb_nchans: int) -> np.ndarray:
+    """Stage 1 (eq. 18: the tree on every sub-band) then stage 2 (eq. 22) on unpacked samples a [nchans][>= required];
+    int64 [ndm][nsamps].  A trial beyond the diagonal (some d'_n >= sb_nchans) is an error (reading X5)."""
+    a = np.asarray(a).astype(np.int64)
+    nchans = a.shape[0]
+    ndm, ns = dprime.shape
+    assert ns * sb_nchans == nchans
+    if dprime.max() >= sb_nchans:
+        raise ValueError("a trial lies beyond the diagonal DM of the piecewise linear tree")
+    t1 = nsamps + int(dt2.max())
+    need = t1 + sb_nchans - 1
+    assert a.shape[1] >= need
+    s = np.zeros((ns, sb_nchans, t1), dtype=np.int64)
+    for n in range(ns):                                                              # stage 1
+        s[n] = tree_np(a[n * sb_nchans:(n + 1) * sb_nchans, :need], t1)
+    out = np.zeros((ndm, nsamps), dtype=np.int64)
+    for d in range(ndm):                                                             # stage 2
+        for n in range(ns):
+            o = int(dt2[d][n])
+            out[d] += s[n, int(dprime[d][n]), o:o + nsamps]
+    return out

@@ -549,3 +549,114 @@ def test_p15_levels_equal_the_full_resolution_loop_summed_over_f_outputs(nbits):
     one = oracle.scrunched_dedisperse_np(a, nsamps, nchans, base.dt, base.f_top, base.df, dms[:5], 1, (1 << nbits) - 1)
     assert len(one) == 1 and one[0][0] == 1
     assert np.array_equal(one[0][2], oracle.dedisperse_unpacked(a, nsamps, oracle.delay_table(nchans, base.dt, base.f_top, base.df, dms[:5])))
+
+
+# ----------------------------------------------------------------------------- P16: tree dedispersion
+def test_p16_theta_phi_hand_values_and_four_channel_tree():
+    """Eq. 14-15 as printed, worked by hand for N = 4: step 0 (r = 1) pairs the channels as they stand with delays 0 / 1,
+    step 1 (r = 2) takes Phi(2, .) = 0, 2, 1, 3 and Theta(1, .) = 0, 1, 1, 2 -- which gives the delays of eq. 8,
+    round(d' nu / 3): d' = 1: 0 0 1 1, d' = 2: 0 1 1 2, d' = 3: 0 1 2 3."""
+    assert [oracle.tree_phi(1, v) for v in range(4)] == [0, 1, 2, 3]
+    assert [oracle.tree_theta(0, v) for v in range(4)] == [0, 1, 0, 1]
+    assert [oracle.tree_phi(2, v) for v in range(4)] == [0, 2, 1, 3]
+    assert [oracle.tree_theta(1, v) for v in range(4)] == [0, 1, 1, 2]
+    assert oracle.tree_delays_np(4).tolist() == [[0, 0, 0, 0], [0, 0, 1, 1], [0, 1, 1, 2], [0, 1, 2, 3]]
+    # N = 2 by hand: D'_0 = A0 + A1, D'_1[t] = A0[t] + A1[t + 1]
+    a = np.array([[1, 2, 3, 9], [4, 5, 6, 7]])
+    assert oracle.tree_np(a, 3).tolist() == [[5, 7, 9], [6, 8, 10]]
+
+
+@pytest.mark.parametrize("n", [2, 4, 8, 16, 32, 64, 128])
+def test_p16_tree_delays_are_linear_trails(n):
+    """"the delay function is now a linear function of nu that ranges from 0 to exactly d' across the
+    band" -- every output holds every channel once (asserted inside), the delays start at 0, end at d', never decrease,
+    equal eq. 8's round(d' nu / (N - 1)) exactly for N <= 8 and within one sample beyond (reading X1)."""
+    dl = oracle.tree_delays_np(n)
+    nu = np.arange(n)
+    for dp in range(n):
+        assert dl[dp, 0] == 0 and dl[dp, n - 1] == dp and (np.diff(dl[dp]) >= 0).all()
+        eq8 = np.floor(dp * nu / (n - 1) + 0.5) if n > 1 else np.zeros(n)
+        assert np.abs(dl[dp] - eq8).max() <= (0 if n <= 8 else 1)
+
+
+@pytest.mark.parametrize("n,nbits", [(4, 8), (8, 2), (32, 4), (64, 8)])
+def test_p16_tree_equals_the_direct_sum_with_its_delays(n, nbits):
+    """Eq. 7: the tree's output IS a shifted channel sum; run through the pinned C loop (eq. 3) with the tree's delay table
+    -- for N <= 8 that table is eq. 8 itself, written out here by its formula."""
+    nsamps = 300
+    rng = np.random.default_rng(160 + n)
+    a = rng.integers(0, 1 << nbits, size=(n, nsamps + n - 1)).astype(np.uint8)
+    got = oracle.tree_np(a, nsamps)
+    table = (np.floor(np.arange(n)[:, None] * np.arange(n)[None, :] / (n - 1) + 0.5).astype(np.int64) if n <= 8
+             else oracle.tree_delays_np(n))
+    assert np.array_equal(got, oracle.dedisperse_unpacked(a, nsamps, table))
+    assert np.array_equal(got[0], a[:, :nsamps].astype(np.int64).sum(axis=0))          # d' = 0: the channel sum
+    # impulse response: one sample at (c*, tau) shows up in trial d' at t = tau - delay[d'][c*] and nowhere else
+    dl = oracle.tree_delays_np(n)
+    z = np.zeros_like(a)
+    z[n - 2, 57 + n] = 1
+    out = oracle.tree_np(z, nsamps)
+    for dp in range(n):
+        want = np.zeros(nsamps, dtype=np.int64)
+        want[57 + n - dl[dp, n - 2]] = 1
+        assert np.array_equal(out[dp], want)
+    # and through the packed path
+    packed = W.pack_rows(torch.from_numpy(np.pad(a, ((0, 0), (0, (-a.shape[1]) % 64)))), nbits).numpy()
+    assert np.array_equal(oracle.tree(packed, nbits, nsamps), got)
+
+
+# ----------------------------------------------------------------------------- P17: piecewise linear tree (PAPER.md:181-222)
+def _pw_case(nbits, sb, nchans=64, ndm=9, nsamps=160, dm_top=20.0, seed=170):
+    cfg = W.CONFIGS[1]
+    dms = np.linspace(0.0, dm_top, ndm)
+    dprime, dt2 = oracle.piecewise_tree_tables(nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb)
+    need = oracle.piecewise_tree_required_samples(nsamps, dprime, dt2, sb)
+    rng = np.random.default_rng(seed)
+    a = rng.integers(0, 1 << nbits, size=(nchans, -(-need // 64) * 64)).astype(np.uint8)
+    return cfg, dms, dprime, dt2, need, a
+
+
+def test_p17_piecewise_tables():
+    """Eq. 20 and 23 (readings X3, X4): the stage-2 delays telescope to the direct delays (eq. 5, the pinned table) of the
+    sub-bands' first channels; d'_n(d) is the rounded delay across the sub-band, checked in exact rational arithmetic."""
+    from fractions import Fraction
+    cfg, dms, dprime, dt2, need, a = _pw_case(8, 16)
+    full = oracle.delay_table(64, cfg.dt, cfg.f_top, cfg.df, dms)
+    assert np.array_equal(dt2, full[:, ::16])
+    k, dt_ = Fraction(4148808, 1000), Fraction(cfg.dt)
+    for d in (1, 4, 8):
+        for n in range(4):
+            f0, f1 = Fraction(cfg.f_top) + n * 16 * Fraction(cfg.df), Fraction(cfg.f_top) + (n + 1) * 16 * Fraction(cfg.df)
+            x = Fraction(dms[d]) * k * (1 / f1 ** 2 - 1 / f0 ** 2) / dt_
+            assert dprime[d][n] == (x + Fraction(1, 2)).__floor__()
+    assert dprime[0].tolist() == [0, 0, 0, 0] and (np.diff(dprime, axis=0) >= 0).all()
+
+
+@pytest.mark.parametrize("nbits,sb", [(8, 16), (2, 8), (4, 64), (8, 4)])
+def test_p17_piecewise_tree_equals_the_direct_sum_with_its_delays_and_error_bound(nbits, sb):
+    """Both stages are shifted sums, so the result is eq. 3 with delay  tree_delay[d'_n(d)][c - nu_n] + Dt''_n(d)  (run
+    through the pinned C loop); that delay misses eq. 5's by at most the chord error of the linear trail inside the
+    sub-band plus three roundings ("approximating the quadratic dispersion curve with a piecewise
+    linear one").  N'nu = N with one sub-band is the basic tree; a trial beyond the diagonal is refused."""
+    nchans, nsamps = 64, 160
+    cfg, dms, dprime, dt2, need, a = _pw_case(nbits, sb, dm_top=20.0 if sb > 4 else 6.0)
+    got = oracle.piecewise_tree_np(a, nsamps, dprime, dt2, sb)
+    tdl = oracle.tree_delays_np(sb)
+    c = np.arange(nchans)
+    eff = tdl[dprime[:, c // sb], (c % sb)[None, :]] + dt2[:, c // sb]
+    assert np.array_equal(got, oracle.dedisperse_unpacked(a, nsamps, eff))
+    f = cfg.f_top + np.arange(nchans + 1) * cfg.df
+    big_t = 4.148808e3 / cfg.dt * (1.0 / f ** 2 - 1.0 / cfg.f_top ** 2)
+    first = c // sb * sb
+    chord = (big_t[first + sb] - big_t[first]) * (c - first) / max(sb - 1, 1)
+    bound = 2.0 + np.abs(dms[:, None] * (chord - (big_t[c] - big_t[first]))[None, :])
+    assert np.all(np.abs(eff - dms[:, None] * big_t[c][None, :]) <= bound + 1e-9)
+    assert np.array_equal(got[0], a[:, :nsamps].astype(np.int64).sum(axis=0))          # DM 0: the channel sum
+    if sb == 64:      # one sub-band: stage 2 only picks the row d'_0(d) of the basic tree
+        assert np.array_equal(got, oracle.tree_np(a[:, :nsamps + int(dt2.max()) + 63], nsamps)[dprime[:, 0]])
+    # packed path, and the diagonal limit (reading X5)
+    packed = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+    assert np.array_equal(oracle.piecewise_tree(packed, nbits, nsamps, nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb), got)
+    with pytest.raises(ValueError):
+        far, far2 = oracle.piecewise_tree_tables(nchans, cfg.dt, cfg.f_top, cfg.df, [400.0], sb)
+        oracle.piecewise_tree_np(np.zeros((nchans, 100000), np.uint8), nsamps, far, far2, sb)
