@@ -52,7 +52,10 @@ enum {
     DD_ERR_DELAY_OVERFLOW = -7,   /* a delay does not fit int32                                           */
     DD_ERR_SMEM = -8,             /* the delay spread of one DM block does not fit shared memory          */
     DD_ERR_CUDA = -9,             /* a CUDA call failed / no device; text via dd_last_cuda_error          */
-    DD_ERR_NOMEM = -10            /* host allocation failed                                               */
+    DD_ERR_NOMEM = -10,           /* host allocation failed                                               */
+    DD_ERR_TOO_LARGE = -11,       /* dd_execute_static: the call needs more scratch than
+                                     DD_STATIC_WORKSPACE_BYTES; text via dd_last_cuda_error               */
+    DD_ERR_UNSUPPORTED = -12      /* dd_execute_static: the plan is not one this entry point serves       */
 };
 
 /* Output element type codes for `out_nbits` (reading R12 of DESIGN.md): raw sums, no scaling. */
@@ -191,6 +194,32 @@ dd_status dd_set_batch(dd_plan plan, int nbeams, int64_t in_beam_stride, int64_t
  */
 dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
                      int out_nbits, void *stream);
+
+/*
+ * dd_execute_static -- dd_execute for callers that may not allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the same transform (eq. 3) by the bit-plane
+ * kernel (variant 3), with the kernel's scratch -- the bit-plane copy of the input that dd_execute keeps
+ * in a buffer it allocates on first use -- in a fixed device array of DD_STATIC_WORKSPACE_BYTES bytes that is part of
+ * the library image (every GPU that loads the library holds it until the process exits).  Arguments, layouts,
+ * alignment rules and the status codes of the argument checks are those of dd_execute.  In addition:
+ *   - the plan must run the bit-plane kernel: dd_set_kernel_variant(plan, 3) before dd_set_dm_list, no sub-band
+ *     method, and its tables on the CURRENT device (dd_set_dm_list made with that device current); anything else
+ *     returns DD_ERR_UNSUPPORTED.  This call never uploads tables.
+ *   - the scratch the call needs, about  nbeams * (nchans + 1) * ceil16((nsamps + largest delay of a DM block) * nbits / 8)
+ *     bytes, must fit the array: DD_ERR_TOO_LARGE otherwise, with both numbers in dd_last_cuda_error(); nothing is
+ *     enqueued.  Larger problems: split the time axis over several calls (each call's input rows start where its
+ *     outputs start), or use dd_execute.
+ *   - it calls no cudaMalloc, cudaFree or allocating library routine, and does not touch the plan's own work buffers.
+ *     The first call on each device looks the array's address up (cudaGetSymbolAddress): make that one call outside
+ *     a stream capture; later calls only enqueue two kernels and one memset on `stream`.
+ *   - ALL calls, from all plans and threads, share the one array per device, and it keeps what the last call wrote:
+ *     each call rewrites every byte it reads (the all-zero rows included), so calls that are ordered on the GPU
+ *     (same stream, or joined by events) are independent of one another; calls whose kernels OVERLAP on the GPU
+ *     (different streams, no ordering) race on the array and their outputs are undefined.
+ */
+#define DD_STATIC_WORKSPACE_BYTES (64 * 1024 * 1024)
+dd_status dd_execute_static(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
+                            int out_nbits, void *stream);
 
 /*
  * dd_execute_host -- the same transform with HOST buffers (end-to-end path).

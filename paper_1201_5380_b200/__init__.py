@@ -20,7 +20,7 @@ __all__ = [
     "DDError", "DDLibraryError", "lib", "library_path",
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
-    "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_time_scrunch", "dd_execute", "dd_execute_static", "DD_STATIC_WORKSPACE_BYTES", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE",
     "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
@@ -29,12 +29,13 @@ __all__ = [
 ]
 
 DD_OUT_F32, DD_OUT_U16, DD_OUT_U32 = 32, 16, -32
+DD_STATIC_WORKSPACE_BYTES = 64 * 1024 * 1024   # include/dd.h: the scratch array of dd_execute_static
 
 # every symbol include/dd.h declares (tests check the library exports exactly these)
 EXPORTED_SYMBOLS = (
     "dd_plan_create", "dd_plan_destroy", "dd_set_dm_list", "dd_get_delay_table", "dd_get_max_delay",
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
-    "dd_time_scrunch", "dd_execute", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
+    "dd_time_scrunch", "dd_execute", "dd_execute_static", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_set_tuning", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read",
     "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
@@ -51,7 +52,7 @@ class DDError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
         msg = f"{where}: {dd_strerror(status)} (status {status})"
-        if status == -9:
+        if status in (-9, -11, -12):
             msg += f" [{dd_last_cuda_error()}]"
         super().__init__(msg)
 
@@ -95,6 +96,7 @@ def lib() -> ctypes.CDLL:
         L.dd_get_subband_tables.argtypes = [vp, vp, vp, vp]
         L.dd_get_subband_tables.restype = i32
         L.dd_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
+        L.dd_execute_static.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_execute_host.argtypes = [vp, i64, vp, i64, vp, i32]
         L.dd_get_launch_info.argtypes = [vp, vp]
         L.dd_set_kernel_variant.argtypes = [vp, i32]
@@ -251,6 +253,12 @@ def dd_execute(plan: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbit
     """Asynchronous; in_ptr/out_ptr are DEVICE buffers (tensors or addresses)."""
     _check(lib().dd_execute(plan, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits),
                             _stream(stream)), "dd_execute")
+
+
+def dd_execute_static(plan: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbits: int, stream=None) -> None:
+    """dd_execute that allocates nothing: kernel variant 3 on the library's fixed scratch array (include/dd.h)."""
+    _check(lib().dd_execute_static(plan, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits),
+                                   _stream(stream)), "dd_execute_static")
 
 
 def dd_execute_host(plan: int, nsamps: int, in_host, in_stride: int, out_host, out_nbits: int) -> None:
@@ -461,6 +469,9 @@ class Plan:
 
     def execute(self, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream=None) -> None:
         dd_execute(self.handle, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream)
+
+    def execute_static(self, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream=None) -> None:
+        dd_execute_static(self.handle, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream)
 
     def profile_enable(self, max_executes: int) -> None:
         self._prof_cap = int(max_executes)

@@ -645,6 +645,72 @@ dd_status dd_execute(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t i
     return DD_OK;
 }
 
+// dd_execute without allocations (include/dd.h): the argument checks of dd_execute, then the bit-plane kernel on the
+// library's fixed scratch array.  Nothing here, or below it, calls cudaMalloc / cudaFree.
+dd_status dd_execute_static(dd_plan plan, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr,
+                            int out_nbits, void *stream)
+{
+    if (!plan || !in_ptr || !out_ptr)
+        return DD_ERR_NULL;
+    dd_status st = check_execute(plan, nsamps, in_stride, out_nbits);
+    if (st != DD_OK)
+        return st;
+    const int es = elem_size(out_nbits);
+    if (reinterpret_cast<uintptr_t>(in_ptr) % 16 != 0 || reinterpret_cast<uintptr_t>(out_ptr) % es != 0)
+        return DD_ERR_ALIGNMENT;
+    const int64_t pitch = plan->out_dm_stride > 0 ? plan->out_dm_stride : nsamps * es;
+    if (pitch % es != 0)
+        return DD_ERR_ALIGNMENT;
+    if (pitch < nsamps * es)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    if (plan->nbeams > 1) {
+        if (plan->out_beam_stride % es != 0)
+            return DD_ERR_ALIGNMENT;
+        if (plan->in_beam_stride < static_cast<int64_t>(plan->nchans) * in_stride ||
+            plan->out_beam_stride < static_cast<int64_t>(plan->ndm - 1) * pitch + nsamps * es)
+            return DD_ERR_STRIDE_TOO_SMALL;
+    }
+    cudaStream_t st_ = static_cast<cudaStream_t>(stream);
+    if (plan->nlive == 0) {   // every channel killed: zeros, no scratch
+        for (int b = 0; b < plan->nbeams; ++b) {
+            uint8_t *o = static_cast<uint8_t *>(out_ptr) + static_cast<int64_t>(b) * (plan->nbeams > 1 ? plan->out_beam_stride : 0);
+            const cudaError_t me = cudaMemset2DAsync(o, static_cast<size_t>(pitch), 0, static_cast<size_t>(nsamps) * es,
+                                                     static_cast<size_t>(plan->ndm), st_);
+            if (me != cudaSuccess)
+                return cuda_fail(me, "dd_execute_static memset");
+        }
+        plan->last_launches = 0;
+        return DD_OK;
+    }
+    if (plan->sb_nchans > 0 || plan->var.id != 3 || !plan->var.bitplane) {
+        g_cuda_error = "dd_execute_static: the plan must run kernel variant 3 (dd_set_kernel_variant(plan, 3) before dd_set_dm_list) "
+                       "without the sub-band method";
+        return DD_ERR_UNSUPPORTED;
+    }
+    int dev = -1;
+    const cudaError_t de = cudaGetDevice(&dev);
+    if (de != cudaSuccess)
+        return cuda_fail(de, "dd_execute_static cudaGetDevice");
+    if (!plan->uploaded || plan->device != dev) {   // (uploading would allocate)
+        g_cuda_error = "dd_execute_static: the plan's tables are not on the current device (call dd_set_dm_list with this device current)";
+        return DD_ERR_UNSUPPORTED;
+    }
+    const KernelParams kp = make_params(plan, nsamps, in_ptr, in_stride, out_ptr, out_nbits, plan->nbeams,
+                                        plan->in_beam_stride, plan->out_beam_stride, plan->out_dm_stride);
+    const size_t need = static_work_need(plan, kp);
+    if (need > static_cast<size_t>(DD_STATIC_WORKSPACE_BYTES)) {
+        g_cuda_error = "dd_execute_static: the call needs " + std::to_string(need) + " bytes of scratch, the static array holds " +
+                       std::to_string(static_cast<size_t>(DD_STATIC_WORKSPACE_BYTES)) + " (DD_STATIC_WORKSPACE_BYTES)";
+        return DD_ERR_TOO_LARGE;
+    }
+    plan->prof_mid = nullptr;
+    const cudaError_t e = launch_variant3_static(plan, kp, st_);
+    if (e != cudaSuccess)
+        return cuda_fail(e, "dd_execute_static launch");
+    plan->last_launches = 2;
+    return DD_OK;
+}
+
 dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int64_t in_stride, void *out_host,
                           int out_nbits)
 {
@@ -1013,6 +1079,8 @@ const char *dd_strerror(dd_status s)
     case DD_ERR_SMEM: return "delay spread of a DM block does not fit shared memory";
     case DD_ERR_CUDA: return "CUDA error (see dd_last_cuda_error)";
     case DD_ERR_NOMEM: return "host allocation failed";
+    case DD_ERR_TOO_LARGE: return "needs more scratch than the static array holds (see dd_last_cuda_error)";
+    case DD_ERR_UNSUPPORTED: return "plan not served by this entry point (see dd_last_cuda_error)";
     }
     return "unknown status";
 }

@@ -29,6 +29,7 @@
 //            into the upper planes;
 //   store  : bit-matrix transposes turn NP planes x 32 lanes into 32 integers; float32 / uint32 / uint16,
 //            128-bit stores, time contiguous.
+#include <mutex>
 #include <utility>
 
 #include "dd_bp_core.cuh"
@@ -973,6 +974,92 @@ cudaError_t bp_prepare_work(dd_plan_s *plan, const KernelParams &kp, cudaStream_
         return prepare_bp<8>(plan, kp, stream, zero_all, w);
     }
     return cudaErrorInvalidValue;
+}
+
+}  // namespace dd
+
+// ------------------------------------------------------------------------------------------ dd_execute_static
+// Variant 3 for callers that may not allocate (include/dd.h: dd_execute_static): the bit-plane copy of the input
+// lives in this array instead of plan->d_work.  One array per device that loads the library, shared by every call;
+// it keeps the last call's contents, so each call writes everything it reads (dd_to_bitplanes every unit of every
+// input row, the memset the all-zero rows of the padded channels).  In host code the NAME below is only a handle:
+// the device address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char dd_static_work[DD_STATIC_WORKSPACE_BYTES];
+
+namespace dd {
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+uint8_t *g_static_addr[kStaticMaxDevices] = {};   // device address of dd_static_work on device i, once looked up
+
+// the geometry prepare_bp computes, without its allocation
+template <int NBITS>
+size_t static_need(const dd_plan_s *plan, const KernelParams &kp)
+{
+    using C = Bp<NBITS>;
+    const int64_t TB = plan->var.TB;
+    const int64_t spg = (16 / (C::NB * 4)) * 32;
+    const int64_t units = (static_cast<int64_t>(kp.ntiles - 1) * TB + plan->max_span_end + spg - 1) / spg;
+    const int64_t rows = static_cast<int64_t>(kp.nrows) + kp.row_mul;
+    return static_cast<size_t>(kp.nbeams) * static_cast<size_t>(rows * C::NSUB * units * 16);
+}
+
+}  // namespace
+
+size_t static_work_need(const dd_plan_s *plan, const KernelParams &kp)
+{
+    switch (plan->nbits) {
+    case 2:
+        return static_need<2>(plan, kp);
+    case 4:
+        return static_need<4>(plan, kp);
+    case 8:
+        return static_need<8>(plan, kp);
+    }
+    return ~static_cast<size_t>(0);
+}
+
+cudaError_t launch_variant3_static(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream)
+{
+    if (plan->var.id != 3 || !plan->var.bitplane)
+        return cudaErrorInvalidValue;
+    if (static_work_need(plan, kp) > static_cast<size_t>(DD_STATIC_WORKSPACE_BYTES))
+        return cudaErrorInvalidValue;   // (dd_execute_static has reported DD_ERR_TOO_LARGE before it gets here)
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess)
+        return e;
+    if (dev < 0 || dev >= kStaticMaxDevices)
+        return cudaErrorInvalidDevice;
+    uint8_t *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_addr[dev]) {
+            void *q = nullptr;
+            if ((e = cudaGetSymbolAddress(&q, dd_static_work)) != cudaSuccess)
+                return e;
+            g_static_addr[dev] = static_cast<uint8_t *>(q);
+        }
+        scratch = g_static_addr[dev];
+    }
+    // The launcher of variant 3 as it stands, with the plan's work buffer swapped for the array for the length of the
+    // call: the buffer is large enough, so prepare_bp neither frees nor allocates, and a cleared layout record makes
+    // it rewrite the all-zero rows (another plan's call may have left its data there).
+    void *const own_work = plan->d_work;
+    const size_t own_bytes = plan->work_bytes;
+    int64_t own_layout[4];
+    for (int i = 0; i < 4; ++i)
+        own_layout[i] = plan->work_layout[i];
+    plan->d_work = scratch;
+    plan->work_bytes = static_cast<size_t>(DD_STATIC_WORKSPACE_BYTES);
+    plan->work_layout[0] = 0;
+    e = launch_variant3(plan, kp, stream, false);
+    plan->d_work = own_work;
+    plan->work_bytes = own_bytes;
+    for (int i = 0; i < 4; ++i)
+        plan->work_layout[i] = own_layout[i];
+    return e;
 }
 
 }  // namespace dd

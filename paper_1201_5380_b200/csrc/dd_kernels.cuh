@@ -87,6 +87,11 @@ cudaError_t launch_variant6(dd_plan_s *plan, const KernelParams &kp, cudaStream_
 // The bit-plane transpose of the packed input into plan->d_work (geometry w from bp_prepare_work).
 cudaError_t launch_to_bitplanes(dd_plan_s *plan, const KernelParams &kp, const BpWork &w, cudaStream_t stream);
 
+// dd_execute_static (dd_kernel_bp.cu): variant 3 with its bit-plane work buffer in a file-scope device array of
+// DD_STATIC_WORKSPACE_BYTES; no allocation.  static_work_need: bytes of that buffer the launch described by kp takes.
+size_t static_work_need(const dd_plan_s *plan, const KernelParams &kp);
+cudaError_t launch_variant3_static(dd_plan_s *plan, const KernelParams &kp, cudaStream_t stream);
+
 // Time-scrunching of packed rows (dd_scrunch.cu).  out_bytes = bytes of every output row to produce (multiple of 16).
 cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t *in, int64_t in_stride, uint8_t *out,
                            int64_t out_stride, int64_t out_bytes, cudaStream_t stream);

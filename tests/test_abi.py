@@ -30,7 +30,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_strerror_and_status_codes():
     assert dd.dd_strerror(0) == "success"
-    for s in range(-10, 0):
+    for s in range(-12, 0):
         assert dd.dd_strerror(s) not in ("", "unknown status")
     assert dd.dd_strerror(-99) == "unknown status"
 
@@ -52,6 +52,7 @@ def test_null_pointers():
     assert L.dd_plan_destroy(None) == 0
     assert L.dd_set_dm_list(None, None, 1) == -1
     assert L.dd_get_max_delay(None) == -1
+    assert L.dd_execute_static(None, 1, None, 16, None, 32, None) == -1
 
 
 def test_dm_list_validation_leaves_plan_unchanged():
@@ -138,6 +139,27 @@ def test_execute_argument_checks_need_no_gpu():
         assert dd.lib().dd_set_batch(p.handle, 0, 0, 0) == -2
         assert dd.lib().dd_set_batch(p.handle, 2, 24, 0) == -4
         assert dd.lib().dd_set_batch(p.handle, 2, 4096 * 64, 1 << 20) == 0
+
+
+def test_execute_static_argument_checks_need_no_gpu():
+    # the argument checks of dd_execute, then DD_ERR_UNSUPPORTED for a plan that does not run the bit-plane kernel --
+    # all before the first CUDA call
+    cfg = W.CONFIGS[4]
+    with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+        L, h = dd.lib(), p.handle
+        assert L.dd_execute_static(h, 100, 16, 1024, 16, 32, None) == -3
+        p.set_dm_list([0.0, 5.0])
+        good_stride = ((100 + p.max_delay) * 4 // 8 + 15) // 16 * 16
+        assert L.dd_execute_static(h, 100, None, good_stride, 16, 32, None) == -1
+        assert L.dd_execute_static(h, 0, 16, good_stride, 16, 32, None) == -2
+        assert L.dd_execute_static(h, 100, 16, good_stride + 8, 16, 32, None) == -4
+        assert L.dd_execute_static(h, 100, 24, good_stride, 16, 32, None) == -4
+        assert L.dd_execute_static(h, 100, 16, 16, 16, 32, None) == -5
+        assert p.launch_info()["variant"] != 3
+        assert L.dd_execute_static(h, 100, 16, good_stride, 16, 32, None) == -12
+        assert "variant 3" in dd.dd_last_cuda_error()
+    assert dd.DD_STATIC_WORKSPACE_BYTES == 64 << 20
+    assert "#define DD_STATIC_WORKSPACE_BYTES (64 * 1024 * 1024)" in open(os.path.join(ROOT, "include", "dd.h")).read()
 
 
 def test_killmask_host_side():
