@@ -290,6 +290,59 @@ dd_status dd_scrunch_execute(dd_scrunch set, int64_t nsamps, const void *in_ptr,
 dd_status dd_scrunch_destroy(dd_scrunch set);
 
 /*
+ * dd_tree_* -- the tree dedispersion algorithm (section 3.1, eq. 7-15) and the piecewise linear tree
+ * method (section 3.1.1, eq. 16-23).  Readings X1-X5 of DESIGN.md section 12.
+ *
+ * The tree transforms N = 2^k channel rows into N series along LINEAR trails, D'[d'][t] = sum_c A[c][t + delay(d', c)],
+ * d' = 0 .. N - 1, in N log2 N row additions.  The delays are those the recursion of eq. 10-13 applies with Theta
+ * (eq. 14) and the shuffle Phi (eq. 15) exactly as printed; they equal eq. 8's round(d' c / (N - 1)) for N <= 8 and
+ * lie within one sample of it beyond (reading X1) -- dd_tree_get_delays returns them.  The piecewise linear tree runs
+ * the tree on every sub-band of sb_nchans = N' channels (stage 1, eq. 18) and then, for every trial of a DM list, adds
+ * one row per sub-band (stage 2, eq. 22):
+ *     out[d][t] = sum_n S_n[d'_n(d)][t + Dt''_n(d)],   d'_n(d) = round(DM_d [DeltaT(nu_{n+1}) - DeltaT(nu_n)])  (eq. 20, X3),
+ *                                                       Dt''_n(d) = round(DM_d DeltaT(nu_n))                     (eq. 23, X4),
+ * DeltaT(c) = k_DM ((f_top + c df)^-2 - f_top^-2) / dt (eq. 4), nu_n = n N'.  An APPROXIMATION of the direct transform
+ * (the trail inside a sub-band is a straight line); it is exact in the sense of the paper's own definition, which the
+ * tests check element by element.
+ *
+ * dd_tree_create   nchans a power of two, 2 .. 4096; sb_nchans a power of two, 2 .. nchans (== nchans: the whole band is
+ *                  one tree); nbits 2, 4 or 8; sb_nchans * (2^nbits - 1) <= 65535 (the stages add in 16-bit lanes), else
+ *                  DD_ERR_OUT_RANGE; other values DD_ERR_INVALID_ARG.  No device needed.
+ * dd_tree_set_dm_list  selects stage 2 for dm_list (HOST, ndm > 0 finite values >= 0) on the band (dt, f_top, df as in
+ *                  dd_plan_create).  A trial with some d'_n(d) >= sb_nchans lies beyond the "diagonal" DM (eq. 21,
+ *                  PAPER.md:205-211; reading X5): DD_ERR_OUT_RANGE, the tree unchanged (scrunch the input with
+ *                  dd_time_scrunch and make a tree with 2 dt for those trials, as the paper prescribes).
+ *                  nchans * (2^nbits - 1) must fit the output type at execute, as for dd_execute.
+ * dd_tree_get_tables   HOST arrays [ndm][nchans / sb_nchans] of d'_n(d) and Dt''_n(d) (either may be NULL).
+ * dd_tree_get_delays   HOST int32 [sb_nchans][sb_nchans]: delay(d', c) of the tree of one sub-band.
+ * dd_tree_required_samples  samples every input row must hold for nsamps outputs: nsamps + sb_nchans - 1 without a DM
+ *                  list, nsamps + max Dt'' + sb_nchans - 1 with one; negative status on error.
+ * dd_tree_execute  in_ptr DEVICE packed rows as for dd_execute (16-byte aligned, in_stride a multiple of 16 with
+ *                  in_stride * 8 >= required samples * nbits, readable out to in_stride).  out_ptr DEVICE dense rows of
+ *                  nsamps elements of out_nbits (DD_OUT_*): without a DM list out[n N' + d'][t] = S_n[d'][t] (nchans rows:
+ *                  the trees of all sub-bands; with sb_nchans == nchans the tree transform D'[d'][t]); with a DM list
+ *                  out[d][t] (ndm rows).  Asynchronous on `stream`; the first call for a given nsamps allocates the
+ *                  intermediate rows (16-bit, about 4 nchans (nsamps + sb_nchans) bytes, plus the stage-1 output with a
+ *                  DM list), later calls only enqueue kernels.  DD_ERR_CUDA without a device.
+ * dd_tree_set_tuning   test knob: key 1 = steps fused by the first pass (1 .. 6, 0 = default), key 2 = steps fused by
+ *                  later passes (1 .. 6, 0 = as many as keep the overlap of neighbouring tiles below half a tile),
+ *                  key 3 = items per thread of the first pass (4 or 8, 0 = default).  Takes effect at the next execute.
+ * dd_tree_get_info info[0] = passes, info[1] = kernels enqueued by the last execute, info[2] = device bytes held,
+ *                  info[3 + 2 p] / info[4 + 2 p] = steps fused by pass p / columns stored per tile (p < 6); int64 x 16.
+ */
+typedef struct dd_tree_s *dd_tree;
+dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits);
+dd_status dd_tree_set_dm_list(dd_tree tree, double dt, double f_top, double df, const double *dm_list, int ndm);
+dd_status dd_tree_get_tables(dd_tree tree, int32_t *dprime, int32_t *dt2);
+dd_status dd_tree_get_delays(dd_tree tree, int32_t *delays);
+int64_t dd_tree_required_samples(dd_tree tree, int64_t nsamps);
+dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr, int out_nbits,
+                          void *stream);
+dd_status dd_tree_set_tuning(dd_tree tree, int key, int value);
+dd_status dd_tree_get_info(dd_tree tree, int64_t *info);
+dd_status dd_tree_destroy(dd_tree tree);
+
+/*
  * dd_set_kernel_variant -- tuning/testing knob: restrict the plan to one kernel variant.
  *   variant  0 = automatic (default); 1 = generic byte-lane kernel (2/4/8-bit); 2 = 2-bit nibble-lane kernel;
  *            3 = bit-plane carry-save kernel (2/4/8-bit; needs nchans*(2^nbits-1) < 2^12 / 2^16 / 2^20);

@@ -25,6 +25,8 @@ __all__ = [
     "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
+    "dd_tree_create", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
+    "dd_tree_set_tuning", "dd_tree_get_info", "dd_tree_destroy", "Tree",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
 
@@ -40,6 +42,8 @@ EXPORTED_SYMBOLS = (
     "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy",
+    "dd_tree_create", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
+    "dd_tree_set_tuning", "dd_tree_get_info", "dd_tree_destroy",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -118,6 +122,19 @@ def lib() -> ctypes.CDLL:
         L.dd_scrunch_required_bytes.restype = i64
         L.dd_scrunch_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
         L.dd_scrunch_destroy.argtypes = [vp]
+        L.dd_tree_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32]
+        L.dd_tree_set_dm_list.argtypes = [vp, dbl, dbl, dbl, vp, i32]
+        L.dd_tree_get_tables.argtypes = [vp, vp, vp]
+        L.dd_tree_get_delays.argtypes = [vp, vp]
+        L.dd_tree_required_samples.argtypes = [vp, i64]
+        L.dd_tree_required_samples.restype = i64
+        L.dd_tree_execute.argtypes = [vp, i64, vp, i64, vp, i32, vp]
+        L.dd_tree_set_tuning.argtypes = [vp, i32, i32]
+        L.dd_tree_get_info.argtypes = [vp, vp]
+        L.dd_tree_destroy.argtypes = [vp]
+        for f in (L.dd_tree_create, L.dd_tree_set_dm_list, L.dd_tree_get_tables, L.dd_tree_get_delays, L.dd_tree_execute,
+                  L.dd_tree_set_tuning, L.dd_tree_get_info, L.dd_tree_destroy):
+            f.restype = i32
         for name in ("dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_execute", "dd_scrunch_destroy"):
             getattr(L, name).restype = i32
         L.dd_strerror.argtypes = [i32]
@@ -397,6 +414,108 @@ class ScrunchSet:
 
     def __exit__(self, *exc):
         self.close()
+
+
+# ------------------------------------------------------------------ tree / piecewise linear tree (include/dd.h: dd_tree_*)
+def dd_tree_create(nchans: int, sb_nchans: int, nbits: int) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().dd_tree_create(ctypes.byref(h), int(nchans), int(sb_nchans), int(nbits)), "dd_tree_create")
+    return h.value
+
+
+def dd_tree_destroy(tree: int) -> None:
+    _check(lib().dd_tree_destroy(tree), "dd_tree_destroy")
+
+
+def dd_tree_set_dm_list(tree: int, dt: float, f_top: float, df: float, dm_list: Sequence[float]) -> None:
+    dm = np.ascontiguousarray(np.asarray(dm_list, dtype=np.float64))
+    _check(lib().dd_tree_set_dm_list(tree, float(dt), float(f_top), float(df), ctypes.c_void_p(dm.ctypes.data), int(dm.size)),
+           "dd_tree_set_dm_list")
+
+
+def dd_tree_get_tables(tree: int, ndm: int, nsub: int):
+    dprime = np.empty((ndm, nsub), dtype=np.int32)
+    dt2 = np.empty((ndm, nsub), dtype=np.int32)
+    _check(lib().dd_tree_get_tables(tree, ctypes.c_void_p(dprime.ctypes.data), ctypes.c_void_p(dt2.ctypes.data)), "dd_tree_get_tables")
+    return dprime, dt2
+
+
+def dd_tree_get_delays(tree: int, sb_nchans: int) -> np.ndarray:
+    out = np.empty((sb_nchans, sb_nchans), dtype=np.int32)
+    _check(lib().dd_tree_get_delays(tree, ctypes.c_void_p(out.ctypes.data)), "dd_tree_get_delays")
+    return out
+
+
+def dd_tree_required_samples(tree: int, nsamps: int) -> int:
+    return _check(lib().dd_tree_required_samples(tree, int(nsamps)), "dd_tree_required_samples")
+
+
+def dd_tree_execute(tree: int, nsamps: int, in_ptr, in_stride: int, out_ptr, out_nbits: int, stream=None) -> None:
+    """Asynchronous; in_ptr/out_ptr are DEVICE buffers (tensors or addresses)."""
+    _check(lib().dd_tree_execute(tree, int(nsamps), _addr(in_ptr), int(in_stride), _addr(out_ptr), int(out_nbits), _stream(stream)),
+           "dd_tree_execute")
+
+
+def dd_tree_set_tuning(tree: int, key: int, value: int) -> None:
+    _check(lib().dd_tree_set_tuning(tree, int(key), int(value)), "dd_tree_set_tuning")
+
+
+def dd_tree_get_info(tree: int) -> dict:
+    info = (ctypes.c_int64 * 16)()
+    _check(lib().dd_tree_get_info(tree, info), "dd_tree_get_info")
+    n = int(info[0])
+    return {"passes": n, "last_launches": int(info[1]), "device_bytes": int(info[2]),
+            "steps": [int(info[3 + 2 * p]) for p in range(min(n, 6))], "tile": [int(info[4 + 2 * p]) for p in range(min(n, 6))]}
+
+
+class Tree:
+    """The tree transform of sub-bands of sb_nchans channels (sb_nchans == nchans: the whole band), optionally followed by
+    stage 2 of the piecewise linear tree for a DM list."""
+
+    def __init__(self, nchans: int, sb_nchans: int, nbits: int):
+        self.nchans, self.sb_nchans, self.nbits, self.ndm = int(nchans), int(sb_nchans), int(nbits), 0
+        self.handle = dd_tree_create(nchans, sb_nchans, nbits)
+
+    def set_dm_list(self, dt: float, f_top: float, df: float, dm_list) -> "Tree":
+        dd_tree_set_dm_list(self.handle, dt, f_top, df, dm_list)
+        self.ndm = len(dm_list)
+        return self
+
+    def tables(self):
+        return dd_tree_get_tables(self.handle, self.ndm, self.nchans // self.sb_nchans)
+
+    def delays(self) -> np.ndarray:
+        return dd_tree_get_delays(self.handle, self.sb_nchans)
+
+    def required_samples(self, nsamps: int) -> int:
+        return dd_tree_required_samples(self.handle, nsamps)
+
+    def set_tuning(self, key: int, value: int) -> "Tree":
+        dd_tree_set_tuning(self.handle, key, value)
+        return self
+
+    def info(self) -> dict:
+        return dd_tree_get_info(self.handle)
+
+    def execute(self, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream=None) -> None:
+        dd_tree_execute(self.handle, nsamps, in_ptr, in_stride, out_ptr, out_nbits, stream)
+
+    def close(self) -> None:
+        if self.handle:
+            dd_tree_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class Plan:

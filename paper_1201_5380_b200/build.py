@@ -19,7 +19,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdd_b200.so")
 OBJ = os.path.join(os.path.dirname(_HERE), "build", "obj")
 SOURCES = ["dd_api.cu", "dd_kernels.cu", "dd_kernel_v1.cu", "dd_kernel_v2.cu", "dd_kernel_bp.cu", "dd_kernel_gs.cu", "dd_kernel_gr.cu",
-           "dd_scrunch.cu", "dd_scrunch_set.cu", "dd_plan.cpp"]
+           "dd_scrunch.cu", "dd_scrunch_set.cu", "dd_tree.cu", "dd_plan.cpp"]
 HEADERS = ["dd_plan.h", "dd_kernels.cuh", "dd_common.cuh", "dd_bp_core.cuh", os.path.join("..", "..", "include", "dd.h")]
 
 NVCC_FLAGS = [

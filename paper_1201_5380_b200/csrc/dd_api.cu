@@ -22,6 +22,10 @@ static dd_status cuda_fail(cudaError_t e, const char *what)
     return DD_ERR_CUDA;
 }
 
+// for the other files of the library that return statuses (dd_tree.cu)
+dd_status report_cuda_error(cudaError_t e, const char *what) { return cuda_fail(e, what); }
+void set_error_text(const std::string &text) { g_cuda_error = text; }
+
 // Device staging of dd_execute_host: the whole packed input plus two output slabs.
 struct HostStage {
     uint8_t *d_in = nullptr;

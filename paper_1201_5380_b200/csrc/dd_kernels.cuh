@@ -99,6 +99,10 @@ cudaError_t launch_scrunch(int nbits_in, int nbits_out, int nrows, const uint8_t
 // Kernels one launch_direct call enqueues for this plan.
 int launches_per_execute(const dd_plan_s *plan);
 
+// DD_ERR_CUDA with the text dd_last_cuda_error returns; the text alone (dd_api.cu).
+dd_status report_cuda_error(cudaError_t e, const char *what);
+void set_error_text(const std::string &text);
+
 // Integer-add throughput microbenchmark (roofline denominator).  Synchronises `stream`.
 cudaError_t int_add_peak(int mode, double *adds_per_sec, cudaStream_t stream);
 

@@ -1,0 +1,708 @@
+// dd_tree.cu -- the tree dedispersion algorithm (eq. 7-15) and the piecewise linear tree method
+// (eq. 16-23); include/dd.h "dd_tree_*"; readings X1-X5 of DESIGN.md section 12.
+//
+// The recursion of eq. 10-13, with Theta (eq. 14) and the shuffle Phi (eq. 15) written out for one step i (r = 2^i):
+// the rows of level i lie in blocks of r rows (the tree of r adjacent channels, row m' = trial d' = m' of that block);
+// two neighbouring blocks L, U combine into one block of 2r rows,
+//
+//     out[2 m' + b][t] = L[m'][t] + U[m'][t + m' + b],      m' < r, b = 0, 1                      (eq. 11-12)
+//
+// (Phi(r, 2 nu) = L's row m', Phi(r, 2 nu + 1) = U's row m', Theta(i, 2 nu + b) = m' + b for nu = r k + m').  log2 N such
+// steps over N rows of T samples are N T log2 N additions -- 5.4e9 for 1024 channels and 2^19 samples, 0.1 ms of the
+// integer pipes -- against N T (nbits / 8 + 4) bytes in and out: the tree is bound by memory, not by arithmetic, so the
+// steps are FUSED in shared memory.  The outputs {2^Q x + o', o' < 2^Q} of Q consecutive steps i0 .. i0 + Q - 1 depend on
+// exactly 2^Q rows of level i0 (row x of each of 2^Q neighbouring blocks): a radix-2^Q butterfly, as in an FFT.  One
+// kernel, dd_tree_pass<Q>, runs one such pass: a CTA stages R = 2^Q rows x C columns (16-bit lanes, 128 KB) of one
+// butterfly and one time tile, runs the Q steps in place (every thread keeps the 2 x 8 sums of its items in registers
+// across the barrier between reading and writing a level), and stores TT = C - H columns, H = 2^i0 (2^Q - 1) being the
+// largest delay the pass applies.  1024 channels take two passes (Q = 6, then Q = 4: H = 960 of C = 4096 columns).
+//
+// The piecewise linear tree (section 3.1.1) is the same passes over sub-bands of N' channels (the blocks simply stop
+// growing at N' rows: stage 1, eq. 18) followed by dd_tree_stage2 (eq. 22): out[d][t] = sum_n S_n[d'_n(d)][t + Dt''_n(d)].
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "dd_kernels.cuh"
+
+namespace dd {
+namespace {
+
+constexpr int TR_THREADS = 512;
+constexpr int TR_SMEM_ELEMS = 65536;   // 16-bit lanes staged by a CTA with ITEMS = 8 (128 KB); ITEMS = 4: half
+
+struct TreePassParams {
+    const uint8_t *in;     // FIRST: packed rows; else 16-bit rows
+    int64_t in_stride;     // bytes between input rows (FIRST: also the bytes readable per row; zero beyond)
+    uint8_t *out;          // 16-bit rows, or rows of the caller's type (LAST)
+    int64_t out_stride;    // bytes between output rows
+    int64_t out_cols;      // LAST: columns below this are stored; else whole tiles are stored
+    int32_t nbits;         // FIRST: 2, 4, 8
+    int32_t out_code;      // LAST: DD_OUT_*
+    int32_t vec_ok;        // LAST: rows allow 16-byte stores
+    int32_t i0;            // first step of the pass
+    int32_t tt;            // columns a tile stores (multiple of 64)
+    int32_t ntiles;
+};
+
+// words k .. k + 3 of the 16-bit lane stream w[0..7] (two aligned 16-byte loads) taken from lane 2 E + (amount / 16) on:
+// amount = 0 / 16 gives the window for b = 0 at an even / odd lane offset, + 16 the window for b = 1
+template <int E>
+__device__ __forceinline__ void tree_window(const uint32_t (&w)[8], uint32_t amount, uint32_t (&x0)[4], uint32_t (&x1)[4])
+{
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        x0[k] = __funnelshift_rc(w[k + E], w[k + E + 1], amount);
+        x1[k] = __funnelshift_rc(w[k + E], w[k + E + 1], amount + 16);
+    }
+}
+
+// the 8 lanes from lane offset e (0..7, the same for every thread of a warp) on, and the 8 lanes from e + 1 on
+__device__ __forceinline__ void tree_windows(const uint4 a, const uint4 b, int e, uint32_t (&x0)[4], uint32_t (&x1)[4])
+{
+    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    const uint32_t amount = (e & 1) * 16;
+    switch (e >> 1) {
+    case 0:
+        tree_window<0>(w, amount, x0, x1);
+        break;
+    case 1:
+        tree_window<1>(w, amount, x0, x1);
+        break;
+    case 2:
+        tree_window<2>(w, amount, x0, x1);
+        break;
+    default:
+        tree_window<3>(w, amount, x0, x1);
+        break;
+    }
+}
+
+__device__ __forceinline__ uint32_t sel4(const uint4 v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
+
+// One pass: steps i0 .. i0 + Q - 1 for one butterfly (R = 2^Q rows) and one time tile.
+//   group g = k 2^i0 + x: butterfly x of block k (blocks of B = R 2^i0 rows after the pass)
+//   staged row b' (level i0) = global row k B + b' 2^i0 + x;   stored row o' = global row k B + x R + o'
+// In local terms step q combines the local blocks of 2^q rows pairwise exactly as the whole tree does, with x 2^q added to
+// every delay: out[c][2 o + b] = in[2c][o] + in[2c + 1][o] at + (x 2^q + o + b).
+template <int Q, int ITEMS, bool FIRST, bool LAST>
+__global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(const TreePassParams p)
+{
+    constexpr int R = 1 << Q;
+    constexpr int C = ITEMS * TR_THREADS * 8 / (R / 2);   // columns staged per row
+    constexpr int CH = C / 8;                             // 16-byte chunks per row (>= 64: a warp stays inside one row)
+    static_assert(CH >= 32 && (CH & (CH - 1)) == 0, "a warp's items must share their row");
+    extern __shared__ __align__(16) uint16_t sm[];        // [R][C] + one chunk of padding
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int tile = blockIdx.x % p.ntiles, g = blockIdx.x / p.ntiles;
+    const int x = g & ((1 << p.i0) - 1), k = g >> p.i0;
+    const int64_t row0 = (static_cast<int64_t>(k) << (p.i0 + Q));
+    const int64_t t0 = static_cast<int64_t>(tile) * p.tt;
+
+    // ---- stage R rows x C columns
+    if constexpr (FIRST) {
+        // packed samples, LSB first: 16 bytes hold SUB chunks of 8 samples; the chunks are taken in an order rotated by
+        // the lane so that the 16-byte stores of a quarter warp fall into distinct banks
+        const int nb = p.nbits;
+        const int sub = 16 / nb;                         // 8-sample chunks per 16 bytes: 8, 4, 2
+        const int per_row = C / (8 * sub);               // 16-byte loads per row
+        const int rot = (lane * sub) >> 3;
+        const uint32_t vmask = (1u << nb) - 1u;
+        const int64_t byte0 = t0 * nb / 8;               // (t0 is a multiple of 64)
+        for (int id = tid; id < R * per_row; id += TR_THREADS) {
+            const int r = id / per_row, c16 = id - r * per_row;
+            const int64_t off = byte0 + static_cast<int64_t>(c16) * 16;
+            const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + off;
+            const uint4 v = off + 16 <= p.in_stride ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
+            uint16_t *dst = sm + r * C + c16 * (8 * sub);
+            for (int kk0 = 0; kk0 < sub; ++kk0) {
+                const int kk = (kk0 + rot) & (sub - 1);
+                // the 8 samples of chunk kk: 8 nb bits from bit 8 nb kk on
+                const int bit = 8 * nb * kk;
+                const uint32_t lo = sel4(v, bit >> 5), hi = sel4(v, (bit >> 5) + (nb == 8 ? 1 : 0));
+                uint32_t o[4];
+                if (nb == 8) {
+#pragma unroll
+                    for (int h = 0; h < 4; ++h) {
+                        const uint32_t word = h < 2 ? lo : hi;
+                        o[h] = ((word >> (16 * (h & 1))) & 0xFFu) | (((word >> (16 * (h & 1) + 8)) & 0xFFu) << 16);
+                    }
+                } else {
+                    const uint32_t word = lo >> (bit & 31);
+#pragma unroll
+                    for (int h = 0; h < 4; ++h)
+                        o[h] = ((word >> (2 * h * nb)) & vmask) | (((word >> ((2 * h + 1) * nb)) & vmask) << 16);
+                }
+                *reinterpret_cast<uint4 *>(dst + kk * 8) = make_uint4(o[0], o[1], o[2], o[3]);
+            }
+        }
+    } else {
+        for (int id = tid; id < R * CH; id += TR_THREADS) {
+            const int r = id / CH, ch = id & (CH - 1);
+            const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + (t0 + ch * 8) * 2;
+            *reinterpret_cast<uint4 *>(sm + r * C + ch * 8) = __ldg(reinterpret_cast<const uint4 *>(src));
+        }
+    }
+    if (tid < 4)
+        reinterpret_cast<uint32_t *>(sm + R * C)[tid] = 0u;
+
+    // ---- Q steps in place
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        uint32_t s0[ITEMS][4], s1[ITEMS][4];
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const int id = it * TR_THREADS + tid;
+            const int ch = id & (CH - 1), pair = id / CH;
+            const int o = pair & ((1 << q) - 1), c = pair >> q;
+            const int lrow = ((2 * c) << q) + o;
+            const int shift = (x << q) + o;
+            int uch = ch + (shift >> 3);
+            uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
+            const uint4 l = *reinterpret_cast<const uint4 *>(sm + lrow * C + ch * 8);
+            const uint16_t *u = sm + (lrow + (1 << q)) * C + uch * 8;
+            const uint4 ua = *reinterpret_cast<const uint4 *>(u), ub = *reinterpret_cast<const uint4 *>(u + 8);
+            uint32_t x0[4], x1[4];
+            tree_windows(ua, ub, shift & 7, x0, x1);
+            const uint32_t lw[4] = {l.x, l.y, l.z, l.w};
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                s0[it][h] = lw[h] + x0[h];   // two 16-bit lanes per word; the sums stay below 2^16
+                s1[it][h] = lw[h] + x1[h];
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const int id = it * TR_THREADS + tid;
+            const int ch = id & (CH - 1), pair = id / CH;
+            const int o = pair & ((1 << q) - 1), c = pair >> q;
+            uint16_t *dst = sm + ((c << (q + 1)) + 2 * o) * C + ch * 8;
+            *reinterpret_cast<uint4 *>(dst) = make_uint4(s0[it][0], s0[it][1], s0[it][2], s0[it][3]);
+            *reinterpret_cast<uint4 *>(dst + C) = make_uint4(s1[it][0], s1[it][1], s1[it][2], s1[it][3]);
+        }
+    }
+    __syncthreads();
+
+    // ---- store the first tt columns of every row
+    const int tch = p.tt / 8;
+    for (int id = tid; id < R * tch; id += TR_THREADS) {
+        const int r = id / tch, ch = id - r * tch;
+        const uint4 v = *reinterpret_cast<const uint4 *>(sm + r * C + ch * 8);
+        const int64_t col = t0 + ch * 8;
+        uint8_t *orow = p.out + (row0 + (static_cast<int64_t>(x) << Q) + r) * p.out_stride;
+        if constexpr (!LAST) {
+            *reinterpret_cast<uint4 *>(orow + col * 2) = v;
+        } else {
+            if (col >= p.out_cols)
+                continue;
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+            uint32_t e[8];
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                e[2 * h] = w[h] & 0xFFFFu;
+                e[2 * h + 1] = w[h] >> 16;
+            }
+            const bool whole = p.vec_ok && col + 8 <= p.out_cols;
+            if (p.out_code == DD_OUT_U16) {
+                if (whole) {
+                    *reinterpret_cast<uint4 *>(orow + col * 2) = v;
+                } else {
+                    for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
+                        reinterpret_cast<uint16_t *>(orow)[col + h] = static_cast<uint16_t>(e[h]);
+                }
+            } else {
+                if (p.out_code == DD_OUT_F32) {
+#pragma unroll
+                    for (int h = 0; h < 8; ++h)
+                        e[h] = __float_as_uint(static_cast<float>(e[h]));
+                }
+                if (whole) {
+                    reinterpret_cast<uint4 *>(orow + col * 4)[0] = make_uint4(e[0], e[1], e[2], e[3]);
+                    reinterpret_cast<uint4 *>(orow + col * 4)[1] = make_uint4(e[4], e[5], e[6], e[7]);
+                } else {
+                    for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
+                        reinterpret_cast<uint32_t *>(orow)[col + h] = e[h];
+                }
+            }
+        }
+    }
+}
+
+// Stage 2 of the piecewise linear tree (eq. 22): out[d][t] = sum_n S[n N' + d'_n(d)][t + Dt''_n(d)] over 16-bit rows S.
+// One thread per 8 consecutive samples of one trial; tab[d][n] = {row, offset}.  The offsets of a (trial, sub-band) are
+// the same for the whole block, so the windows are cut out of two aligned 16-byte loads as in the passes.
+constexpr int TR2_THREADS = 256;
+__global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint16_t *__restrict__ S, int64_t pitch, const int2 *__restrict__ tab,
+                                                              int ns, uint8_t *__restrict__ out, int64_t out_stride, int64_t nsamps,
+                                                              int out_code, int vec_ok)
+{
+    extern __shared__ int2 stab[];
+    const int d = blockIdx.y;
+    for (int n = threadIdx.x; n < ns; n += TR2_THREADS)
+        stab[n] = __ldg(&tab[static_cast<int64_t>(d) * ns + n]);
+    __syncthreads();
+    const int64_t col = (static_cast<int64_t>(blockIdx.x) * TR2_THREADS + threadIdx.x) * 8;
+    if (col >= nsamps)
+        return;
+    uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int n = 0; n < ns; ++n) {
+        const int2 e = stab[n];
+        const int64_t at = col + e.y;
+        const uint16_t *src = S + static_cast<int64_t>(e.x) * pitch + (at & ~int64_t(7));
+        const uint4 a = __ldg(reinterpret_cast<const uint4 *>(src)), b = __ldg(reinterpret_cast<const uint4 *>(src + 8));
+        uint32_t x0[4], x1[4];
+        tree_windows(a, b, static_cast<int>(at & 7), x0, x1);
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            acc[2 * h] += x0[h] & 0xFFFFu;
+            acc[2 * h + 1] += x0[h] >> 16;
+        }
+    }
+    uint8_t *orow = out + static_cast<int64_t>(d) * out_stride;
+    const bool whole = vec_ok && col + 8 <= nsamps;
+    if (out_code == DD_OUT_U16) {
+        if (whole) {
+            *reinterpret_cast<uint4 *>(orow + col * 2) =
+                make_uint4(acc[0] | acc[1] << 16, acc[2] | acc[3] << 16, acc[4] | acc[5] << 16, acc[6] | acc[7] << 16);
+        } else {
+            for (int h = 0; h < 8 && col + h < nsamps; ++h)
+                reinterpret_cast<uint16_t *>(orow)[col + h] = static_cast<uint16_t>(acc[h]);
+        }
+    } else {
+        if (out_code == DD_OUT_F32) {
+#pragma unroll
+            for (int h = 0; h < 8; ++h)
+                acc[h] = __float_as_uint(static_cast<float>(acc[h]));
+        }
+        if (whole) {
+            reinterpret_cast<uint4 *>(orow + col * 4)[0] = make_uint4(acc[0], acc[1], acc[2], acc[3]);
+            reinterpret_cast<uint4 *>(orow + col * 4)[1] = make_uint4(acc[4], acc[5], acc[6], acc[7]);
+        } else {
+            for (int h = 0; h < 8 && col + h < nsamps; ++h)
+                reinterpret_cast<uint32_t *>(orow)[col + h] = acc[h];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host side
+struct TreePass {
+    int i0 = 0, q = 0, items = 8;
+    int cols = 0, halo = 0, tt = 0;   // columns staged / largest delay applied / columns stored per tile
+    int64_t out_cols = 0;             // columns the pass produces for the current nsamps
+    int64_t ntiles = 0;
+};
+
+template <int Q, int ITEMS>
+cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64_t groups, cudaStream_t stream)
+{
+    constexpr int R = 1 << Q;
+    constexpr int C = ITEMS * TR_THREADS * 8 / (R / 2);
+    const size_t smem = (static_cast<size_t>(R) * C + 8) * 2;
+    const int64_t ctas = groups * p.ntiles;
+    if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
+        return cudaErrorInvalidConfiguration;
+    auto go = [&](auto kernel) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        if (e != cudaSuccess)
+            return e;
+        kernel<<<static_cast<unsigned>(ctas), TR_THREADS, smem, stream>>>(p);
+        return cudaGetLastError();
+    };
+    if (first)
+        return last ? go(dd_tree_pass<Q, ITEMS, true, true>) : go(dd_tree_pass<Q, ITEMS, true, false>);
+    return last ? go(dd_tree_pass<Q, ITEMS, false, true>) : go(dd_tree_pass<Q, ITEMS, false, false>);
+}
+
+template <int Q>
+cudaError_t launch_pass_q(const TreePassParams &p, int items, bool first, bool last, int64_t groups, cudaStream_t stream)
+{
+    return items == 4 ? launch_pass_qi<Q, 4>(p, first, last, groups, stream) : launch_pass_qi<Q, 8>(p, first, last, groups, stream);
+}
+
+cudaError_t launch_pass(const TreePassParams &p, int q, int items, bool first, bool last, int64_t groups, cudaStream_t stream)
+{
+    switch (q) {
+    case 1:
+        return launch_pass_q<1>(p, items, first, last, groups, stream);
+    case 2:
+        return launch_pass_q<2>(p, items, first, last, groups, stream);
+    case 3:
+        return launch_pass_q<3>(p, items, first, last, groups, stream);
+    case 4:
+        return launch_pass_q<4>(p, items, first, last, groups, stream);
+    case 5:
+        return launch_pass_q<5>(p, items, first, last, groups, stream);
+    case 6:
+        return launch_pass_q<6>(p, items, first, last, groups, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
+int pass_cols(int q, int items) { return items * TR_THREADS * 8 / ((1 << q) / 2); }
+
+}  // namespace
+}  // namespace dd
+
+struct dd_tree_s {
+    int nchans = 0, sb = 0, nbits = 0, steps = 0;
+    int tune[3] = {0, 0, 0};   // steps of the first pass, steps of later passes, items per thread of the first pass
+    // stage 2 (piecewise linear tree)
+    int ndm = 0, ns = 0;
+    std::vector<int32_t> dprime, dt2;   // [ndm][ns]
+    int64_t max_dt2 = 0;
+    void *d_tab = nullptr;              // int2 [ndm][ns] {row of S, offset}
+    bool tab_uploaded = false;
+    // passes and intermediate rows, sized for `sized_for` output samples with the tuning `sized_tune`
+    std::vector<dd::TreePass> passes;
+    int64_t sized_for = -1;
+    int sized_tune[3] = {-1, -1, -1};
+    int sized_ndm = -1;
+    void *buf[2] = {nullptr, nullptr};
+    size_t buf_bytes[2] = {0, 0};
+    int64_t pitch[8] = {};              // columns per row of the output of pass p (16-bit rows)
+    int64_t last_launches = 0;
+};
+
+namespace dd {
+namespace {
+
+const double kTreeDm = 4.148808e3;   // k_DM in MHz^2 pc^-1 cm^3 s
+
+int log2_exact(int v)
+{
+    int k = 0;
+    while ((1 << k) < v)
+        ++k;
+    return (1 << k) == v ? k : -1;
+}
+
+// The passes for t_out output columns of the last pass; false if the tuning leaves a pass without room for a tile.
+bool plan_passes(dd_tree_s *t, int64_t t_out)
+{
+    t->passes.clear();
+    for (int i0 = 0; i0 < t->steps;) {
+        const int left = t->steps - i0;
+        const int items = (i0 == 0 && t->tune[2] == 4) ? 4 : 8;
+        int q = std::min(left, 6);
+        if (i0 == 0 && t->tune[0] > 0)
+            q = std::min(q, t->tune[0]);
+        if (i0 > 0 && t->tune[1] > 0)
+            q = std::min(q, t->tune[1]);
+        // later passes: the overlap of neighbouring tiles (the largest delay of the pass) at most half the columns staged
+        // (the first pass: whatever leaves a tile; 63 of 1024 columns for six steps)
+        for (; q > 1; --q) {
+            const int64_t halo = (int64_t(1) << i0) * ((1 << q) - 1), cols = pass_cols(q, items);
+            if ((i0 == 0 || t->tune[1] > 0 || 2 * halo <= cols) && halo + 64 <= cols)
+                break;
+        }
+        TreePass ps;
+        ps.i0 = i0, ps.q = q, ps.items = items;
+        ps.cols = pass_cols(q, items);
+        ps.halo = static_cast<int>((int64_t(1) << i0) * ((1 << q) - 1));
+        ps.tt = (ps.cols - ps.halo) & ~63;
+        if (ps.tt < 64)
+            return false;
+        t->passes.push_back(ps);
+        i0 += q;
+    }
+    if (t->passes.size() > 6)
+        return false;
+    // columns every pass has to produce, backwards: a pass stages (ntiles - 1) tt + cols columns of the one before
+    int64_t need = t_out;
+    for (int p = static_cast<int>(t->passes.size()) - 1; p >= 0; --p) {
+        TreePass &ps = t->passes[p];
+        ps.out_cols = need;
+        ps.ntiles = (need + ps.tt - 1) / ps.tt;
+        t->pitch[p] = ps.ntiles * ps.tt + 32;   // whole tiles are stored; stage 2 reads up to 23 columns past its last sample
+        need = (ps.ntiles - 1) * ps.tt + ps.cols;
+    }
+    return true;
+}
+
+void tree_free_buffers(dd_tree_s *t)
+{
+    for (int i = 0; i < 2; ++i) {
+        if (t->buf[i])
+            cudaFree(t->buf[i]);
+        t->buf[i] = nullptr;
+        t->buf_bytes[i] = 0;
+    }
+    t->sized_for = -1;
+}
+
+}  // namespace
+}  // namespace dd
+
+extern "C" {
+
+dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    *tree = nullptr;
+    const int kn = dd::log2_exact(nchans), ks = dd::log2_exact(sb_nchans);
+    if (nchans < 2 || nchans > 4096 || kn < 0 || sb_nchans < 2 || sb_nchans > nchans || ks < 0 || (nbits != 2 && nbits != 4 && nbits != 8))
+        return DD_ERR_INVALID_ARG;
+    if (static_cast<int64_t>(sb_nchans) * ((1 << nbits) - 1) > 65535)
+        return DD_ERR_OUT_RANGE;
+    dd_tree_s *t = new (std::nothrow) dd_tree_s;
+    if (!t)
+        return DD_ERR_NOMEM;
+    t->nchans = nchans, t->sb = sb_nchans, t->nbits = nbits, t->steps = ks;
+    *tree = t;
+    return DD_OK;
+}
+
+dd_status dd_tree_destroy(dd_tree tree)
+{
+    if (!tree)
+        return DD_OK;
+    dd::tree_free_buffers(tree);
+    if (tree->d_tab)
+        cudaFree(tree->d_tab);
+    delete tree;
+    return DD_OK;
+}
+
+dd_status dd_tree_set_dm_list(dd_tree tree, double dt, double f_top, double df, const double *dm_list, int ndm)
+{
+    if (!tree || !dm_list)
+        return DD_ERR_NULL;
+    if (ndm <= 0 || !(dt > 0) || !(f_top > 0) || !(df < 0) || !std::isfinite(dt) || !std::isfinite(f_top) || !std::isfinite(df) ||
+        !(f_top + static_cast<double>(tree->nchans) * df > 0))   // (eq. 20 evaluates DeltaT one channel past the band: X3)
+        return DD_ERR_INVALID_ARG;
+    for (int d = 0; d < ndm; ++d)
+        if (!(dm_list[d] >= 0) || !std::isfinite(dm_list[d]))
+            return DD_ERR_INVALID_ARG;
+    const int ns = tree->nchans / tree->sb;
+    std::vector<int32_t> dprime, dt2;
+    int64_t max_dt2 = 0;
+    try {
+        // DeltaT(nu_n) in samples at the sub-band edges nu_n = n N', n = 0 .. ns (eq. 4)
+        std::vector<double> big_t(ns + 1);
+        for (int n = 0; n <= ns; ++n) {
+            const double edge = f_top + static_cast<double>(n * tree->sb) * df;
+            big_t[n] = dd::kTreeDm * (1.0 / (edge * edge) - 1.0 / (f_top * f_top)) / dt;
+        }
+        dprime.resize(static_cast<size_t>(ndm) * ns);
+        dt2.resize(static_cast<size_t>(ndm) * ns);
+        for (int d = 0; d < ndm; ++d) {
+            for (int n = 0; n < ns; ++n) {
+                const double a = std::floor(dm_list[d] * (big_t[n + 1] - big_t[n]) + 0.5);   // eq. 20 (X3): rounded once
+                const double b = std::floor(dm_list[d] * big_t[n] + 0.5);                    // eq. 23 (X4): the sum telescopes
+                if (!(a >= 0) || !(b >= 0) || b > 2147483000.0)
+                    return DD_ERR_DELAY_OVERFLOW;
+                if (a >= static_cast<double>(tree->sb))
+                    return DD_ERR_OUT_RANGE;   // beyond the diagonal DM (eq. 21, X5)
+                dprime[static_cast<size_t>(d) * ns + n] = static_cast<int32_t>(a);
+                dt2[static_cast<size_t>(d) * ns + n] = static_cast<int32_t>(b);
+                max_dt2 = std::max<int64_t>(max_dt2, static_cast<int64_t>(b));
+            }
+        }
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+    tree->dprime.swap(dprime);
+    tree->dt2.swap(dt2);
+    tree->ndm = ndm, tree->ns = ns, tree->max_dt2 = max_dt2;
+    tree->tab_uploaded = false;
+    return DD_OK;
+}
+
+dd_status dd_tree_get_tables(dd_tree tree, int32_t *dprime, int32_t *dt2)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    if (tree->ndm <= 0)
+        return DD_ERR_NO_DM_LIST;
+    if (dprime)
+        std::copy(tree->dprime.begin(), tree->dprime.end(), dprime);
+    if (dt2)
+        std::copy(tree->dt2.begin(), tree->dt2.end(), dt2);
+    return DD_OK;
+}
+
+// The delays the steps apply, by running them on delay lists: a row of level i holds one delay per channel of its block.
+dd_status dd_tree_get_delays(dd_tree tree, int32_t *delays)
+{
+    if (!tree || !delays)
+        return DD_ERR_NULL;
+    try {
+        const int n = tree->sb;
+        std::vector<std::vector<int32_t>> cur(n, std::vector<int32_t>(1, 0)), nxt(n);
+        for (int r = 1; r < n; r *= 2) {
+            for (int k = 0; k < n / (2 * r); ++k) {
+                for (int m = 0; m < r; ++m) {
+                    const std::vector<int32_t> &lo = cur[2 * r * k + m], &up = cur[2 * r * k + r + m];
+                    for (int b = 0; b < 2; ++b) {
+                        std::vector<int32_t> &o = nxt[2 * r * k + 2 * m + b];
+                        o = lo;
+                        for (int32_t v : up)
+                            o.push_back(v + m + b);
+                    }
+                }
+            }
+            cur.swap(nxt);
+        }
+        for (int d = 0; d < n; ++d)
+            std::copy(cur[d].begin(), cur[d].end(), delays + static_cast<size_t>(d) * n);
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+    return DD_OK;
+}
+
+int64_t dd_tree_required_samples(dd_tree tree, int64_t nsamps)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    if (nsamps <= 0 || nsamps > (int64_t(1) << 40))
+        return DD_ERR_INVALID_ARG;
+    return nsamps + (tree->ndm > 0 ? tree->max_dt2 : 0) + tree->sb - 1;
+}
+
+dd_status dd_tree_set_tuning(dd_tree tree, int key, int value)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    if (key < 1 || key > 3 || value < 0 || (key <= 2 && value > 6) || (key == 3 && value != 0 && value != 4 && value != 8))
+        return DD_ERR_INVALID_ARG;
+    tree->tune[key - 1] = value;
+    return DD_OK;
+}
+
+dd_status dd_tree_get_info(dd_tree tree, int64_t *info)
+{
+    if (!tree || !info)
+        return DD_ERR_NULL;
+    for (int i = 0; i < 16; ++i)
+        info[i] = 0;
+    info[0] = static_cast<int64_t>(tree->passes.size());
+    info[1] = tree->last_launches;
+    info[2] = static_cast<int64_t>(tree->buf_bytes[0] + tree->buf_bytes[1]) +
+              (tree->d_tab ? static_cast<int64_t>(tree->ndm) * tree->ns * 8 : 0);
+    for (size_t p = 0; p < tree->passes.size() && p < 6; ++p) {
+        info[3 + 2 * p] = tree->passes[p].q;
+        info[4 + 2 * p] = tree->passes[p].tt;
+    }
+    return DD_OK;
+}
+
+dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int64_t in_stride, void *out_ptr, int out_nbits,
+                          void *stream)
+{
+    using namespace dd;
+    if (!tree || !in_ptr || !out_ptr)
+        return DD_ERR_NULL;
+    const int es = out_nbits == DD_OUT_U16 ? 2 : ((out_nbits == DD_OUT_U32 || out_nbits == DD_OUT_F32) ? 4 : 0);
+    if (nsamps <= 0 || nsamps > (int64_t(1) << 40) || es == 0)
+        return DD_ERR_INVALID_ARG;
+    if (in_stride <= 0 || in_stride % 16 != 0 || reinterpret_cast<uintptr_t>(in_ptr) % 16 != 0 ||
+        reinterpret_cast<uintptr_t>(out_ptr) % es != 0)
+        return DD_ERR_ALIGNMENT;
+    const bool stage2 = tree->ndm > 0;
+    const int64_t t_out = nsamps + (stage2 ? tree->max_dt2 : 0);   // columns of the stage-1 rows
+    const int64_t required = t_out + tree->sb - 1;
+    if (in_stride > INT64_MAX / 8 || in_stride * 8 < required * tree->nbits)
+        return DD_ERR_STRIDE_TOO_SMALL;
+    const int64_t top = static_cast<int64_t>(stage2 ? tree->nchans : tree->sb) * ((1 << tree->nbits) - 1);
+    if (out_nbits == DD_OUT_U16 && top > 65535)
+        return DD_ERR_OUT_RANGE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+
+    // ---- passes and intermediate rows for this size (first call, or the size / tuning / DM list changed)
+    if (tree->sized_for != t_out || tree->sized_ndm != tree->ndm || tree->sized_tune[0] != tree->tune[0] ||
+        tree->sized_tune[1] != tree->tune[1] || tree->sized_tune[2] != tree->tune[2]) {
+        tree->sized_for = -1;
+        if (!plan_passes(tree, t_out)) {
+            set_error_text("dd_tree_execute: the tuning leaves a pass without room for a tile");
+            return DD_ERR_INVALID_ARG;
+        }
+        const int np = static_cast<int>(tree->passes.size());
+        size_t need[2] = {0, 0};
+        for (int p = 0; p < np; ++p)
+            if (p + 1 < np || stage2)   // (the last pass of the plain tree writes the caller's rows)
+                need[p & 1] = std::max(need[p & 1], static_cast<size_t>(tree->nchans) * static_cast<size_t>(tree->pitch[p]) * 2);
+        for (int i = 0; i < 2; ++i) {
+            if (tree->buf_bytes[i] < need[i]) {
+                if (tree->buf[i])
+                    cudaFree(tree->buf[i]);   // synchronises with kernels still using the old rows
+                tree->buf[i] = nullptr;
+                tree->buf_bytes[i] = 0;
+                if ((e = cudaMalloc(&tree->buf[i], need[i])) != cudaSuccess)
+                    return report_cuda_error(e, "dd_tree_execute cudaMalloc(rows)");
+                tree->buf_bytes[i] = need[i];
+                // columns no pass writes (past the last tile) are staged by the next pass but reach no output: defined all the same
+                if ((e = cudaMemsetAsync(tree->buf[i], 0, need[i], st)) != cudaSuccess)
+                    return report_cuda_error(e, "dd_tree_execute memset(rows)");
+            }
+        }
+        tree->sized_for = t_out;
+        tree->sized_ndm = tree->ndm;
+        for (int i = 0; i < 3; ++i)
+            tree->sized_tune[i] = tree->tune[i];
+    }
+    if (stage2 && !tree->tab_uploaded) {
+        std::vector<int2> tab(static_cast<size_t>(tree->ndm) * tree->ns);
+        for (int d = 0; d < tree->ndm; ++d)
+            for (int n = 0; n < tree->ns; ++n) {
+                const size_t i = static_cast<size_t>(d) * tree->ns + n;
+                tab[i] = make_int2(n * tree->sb + tree->dprime[i], tree->dt2[i]);
+            }
+        if (tree->d_tab)
+            cudaFree(tree->d_tab);
+        tree->d_tab = nullptr;
+        if ((e = cudaMalloc(&tree->d_tab, tab.size() * sizeof(int2))) != cudaSuccess ||
+            (e = cudaMemcpy(tree->d_tab, tab.data(), tab.size() * sizeof(int2), cudaMemcpyHostToDevice)) != cudaSuccess)
+            return report_cuda_error(e, "dd_tree_execute upload(stage-2 table)");
+        tree->tab_uploaded = true;
+    }
+
+    // ---- stage 1: the passes
+    const int np = static_cast<int>(tree->passes.size());
+    const int64_t out_pitch_bytes = nsamps * es;
+    const bool rows16 = reinterpret_cast<uintptr_t>(out_ptr) % 16 == 0 && out_pitch_bytes % 16 == 0;
+    int64_t launches = 0;
+    for (int p = 0; p < np; ++p) {
+        const TreePass &ps = tree->passes[p];
+        const bool first = p == 0, last = p + 1 == np && !stage2;
+        TreePassParams kp{};
+        kp.in = first ? static_cast<const uint8_t *>(in_ptr) : static_cast<const uint8_t *>(tree->buf[(p - 1) & 1]);
+        kp.in_stride = first ? in_stride : tree->pitch[p - 1] * 2;
+        kp.out = last ? static_cast<uint8_t *>(out_ptr) : static_cast<uint8_t *>(tree->buf[p & 1]);
+        kp.out_stride = last ? out_pitch_bytes : tree->pitch[p] * 2;
+        kp.out_cols = last ? nsamps : ps.out_cols;
+        kp.nbits = tree->nbits;
+        kp.out_code = out_nbits;
+        kp.vec_ok = rows16 ? 1 : 0;
+        kp.i0 = ps.i0;
+        kp.tt = ps.tt;
+        kp.ntiles = static_cast<int32_t>(ps.ntiles);
+        const int64_t groups = tree->nchans >> ps.q;
+        if ((e = launch_pass(kp, ps.q, ps.items, first, last, groups, st)) != cudaSuccess)
+            return report_cuda_error(e, "dd_tree_execute pass");
+        ++launches;
+    }
+    // ---- stage 2
+    if (stage2) {
+        const dim3 grid(static_cast<unsigned>((nsamps + TR2_THREADS * 8 - 1) / (TR2_THREADS * 8)), static_cast<unsigned>(tree->ndm));
+        dd_tree_stage2<<<grid, TR2_THREADS, static_cast<size_t>(tree->ns) * sizeof(int2), st>>>(
+            static_cast<const uint16_t *>(tree->buf[(np - 1) & 1]), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
+            static_cast<uint8_t *>(out_ptr), out_pitch_bytes, nsamps, out_nbits, rows16 ? 1 : 0);
+        if ((e = cudaGetLastError()) != cudaSuccess)
+            return report_cuda_error(e, "dd_tree_execute stage 2");
+        ++launches;
+    }
+    tree->last_launches = launches;
+    return DD_OK;
+}
+
+}  // extern "C"

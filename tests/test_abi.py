@@ -316,3 +316,51 @@ def test_tuning_and_workspace_knobs_host_side():
         p.set_tuning(dd.DD_TUNE_GROUP_SIZE, 2)
         with pytest.raises(dd.DDError):
             p.set_dm_list(c.dm_list())
+
+
+def test_tree_host_side():
+    # dd_tree_* without a GPU: argument checks, the delays of the recursion and the stage-2 tables against the oracle
+    from oracle.oracle_np import piecewise_tree_required_samples, piecewise_tree_tables, tree_delays_np
+    L = dd.lib()
+    h = ctypes.c_void_p()
+    for args in ((1000, 1000, 2), (1024, 48, 2), (1024, 2048, 2), (8192, 64, 2), (1, 1, 2), (64, 64, 3)):
+        assert L.dd_tree_create(ctypes.byref(h), *args) == -2
+    assert L.dd_tree_create(ctypes.byref(h), 1024, 512, 8) == -6          # 512 * 255 does not fit the 16-bit lanes
+    assert L.dd_tree_create(None, 64, 64, 2) == -1 and L.dd_tree_destroy(None) == 0
+    for n in (2, 4, 8, 32, 128, 1024):
+        with dd.Tree(n, n, 2) as t:
+            assert np.array_equal(t.delays(), tree_delays_np(n))
+            assert t.required_samples(100) == 100 + n - 1
+    cfg = W.CONFIGS[2]
+    dms = np.linspace(0.0, 30.0, 37)
+    for sb in (16, 32, 64, 1024):
+        with dd.Tree(cfg.nchans, sb, cfg.nbits) as t:
+            assert L.dd_tree_get_tables(t.handle, None, None) == -3          # no DM list yet
+            if sb == 1024:
+                with pytest.raises(dd.DDError) as e:
+                    t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, [1000.0, 2000.0])   # 40 k samples across the band
+                assert e.value.status == -6
+                continue
+            t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
+            dprime, dt2 = t.tables()
+            o1, o2 = piecewise_tree_tables(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb)
+            assert np.array_equal(dprime, o1) and np.array_equal(dt2, o2)
+            assert t.required_samples(5000) == piecewise_tree_required_samples(5000, o1, o2, sb)
+            for bad in ([], [-1.0], [float("nan")]):
+                assert L.dd_tree_set_dm_list(t.handle, cfg.dt, cfg.f_top, cfg.df,
+                                             np.asarray(bad + [0.0], dtype=np.float64).ctypes.data_as(ctypes.c_void_p), len(bad)) == -2
+            assert L.dd_tree_set_dm_list(t.handle, cfg.dt, cfg.f_top, 0.4, dms.ctypes.data_as(ctypes.c_void_p), 3) == -2
+            assert np.array_equal(t.tables()[0], o1)                          # failures left the tables alone
+            # execute: argument checks come before the first CUDA call
+            need_bytes = (t.required_samples(5000) * 2 // 8 + 15) // 16 * 16
+            assert L.dd_tree_execute(t.handle, 5000, None, need_bytes, 16, 32, None) == -1
+            assert L.dd_tree_execute(t.handle, 0, 16, need_bytes, 16, 32, None) == -2
+            assert L.dd_tree_execute(t.handle, 5000, 16, need_bytes, 16, 8, None) == -2
+            assert L.dd_tree_execute(t.handle, 5000, 24, need_bytes, 16, 32, None) == -4
+            assert L.dd_tree_execute(t.handle, 5000, 16, need_bytes - 16, 16, 32, None) == -5
+            assert L.dd_tree_set_tuning(t.handle, 1, 7) == -2 and L.dd_tree_set_tuning(t.handle, 3, 5) == -2
+            assert L.dd_tree_set_tuning(t.handle, 4, 1) == -2 and L.dd_tree_set_tuning(t.handle, 2, 3) == 0
+    with dd.Tree(1024, 256, 8) as t8:
+        big = (1 << 20)
+        t8.set_dm_list(cfg.dt, cfg.f_top, cfg.df, [0.0, 1.0])
+        assert L.dd_tree_execute(t8.handle, 100, 16, big, 16, 16, None) == -6          # 1024 * 255 does not fit uint16

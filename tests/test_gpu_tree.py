@@ -1,0 +1,155 @@
+"""GPU parity of the tree dedispersion algorithm and the piecewise linear tree method
+(PAPER.md:181-222): dd_tree_execute through the C ABI against oracle.tree / oracle.piecewise_tree, element by element,
+bit-exact.  The oracle follows eq. 10-15 / 18-23 step by step and is pinned by P16 / P17 (tests/test_oracle_pins.py).
+All inputs are seeded and synthetic (dd_workloads); no expected value comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+import torch
+
+import dd_workloads as W
+import oracle
+import paper_1201_5380_b200 as dd
+
+pytestmark = pytest.mark.gpu
+
+_CODE = {"f32": 32, "u32": -32, "u16": 16}
+_TORCH_OUT = {"f32": torch.float32, "u32": torch.int32, "u16": torch.int16}
+_NP_VIEW = {"f32": np.float32, "u32": np.uint32, "u16": np.uint16}
+
+
+def _band(nbits, nchans, nsamps):
+    """A one-beam config on the survey band (cfg2's) with the value distribution of the config of that width."""
+    base = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    return base.reduced(nsamps=nsamps, ndm=2, nchans=nchans, nbeams=1)
+
+
+def _run(tree, nsamps, packed_dev, stride, nrows, kind):
+    out = torch.full((nrows, nsamps), -1, dtype=_TORCH_OUT[kind], device="cuda")
+    tree.execute(nsamps, packed_dev, stride, out, _CODE[kind], torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    return out.cpu().numpy().view(_NP_VIEW[kind])
+
+
+def _assert_equal(got, ref, what):
+    assert got.shape == ref.shape, what
+    bad = np.nonzero(got != ref)
+    assert bad[0].size == 0, (f"{what}: {bad[0].size} mismatches, first at row {bad[0][0]} t {bad[1][0]}: "
+                              f"got {got[bad[0][0], bad[1][0]]} ref {ref[bad[0][0], bad[1][0]]}")
+
+
+def _tree_case(nbits, n, nsamps, kinds=("u32",), tuning=()):
+    cfg = _band(nbits, n, nsamps)
+    packed, stride = W.gen_packed(cfg, n - 1, None)
+    ref = oracle.tree(packed[0].numpy(), nbits, nsamps)
+    dev = packed.cuda()
+    with dd.Tree(n, n, nbits) as t:
+        for key, value in tuning:
+            t.set_tuning(key, value)
+        assert t.required_samples(nsamps) == nsamps + n - 1
+        for kind in kinds:
+            got = _run(t, nsamps, dev, stride, n, kind)
+            _assert_equal(got, oracle.cast_out(ref, kind), f"tree N={n} {nbits}-bit {kind} tuning {tuning}")
+        info = t.info()
+        assert info["last_launches"] == info["passes"] >= 1 and sum(info["steps"]) == n.bit_length() - 1
+    return info
+
+
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_tree_every_size_one_to_three_passes(nbits):
+    # N = 2 .. 64: one pass; 128 .. 1024: two; 2048 / 4096: three.  Two tiles of the first pass and a ragged tail; a row
+    # length that allows 16-byte stores and one that does not; all output types
+    for n in (2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096):
+        if n * ((1 << nbits) - 1) > 65535:
+            with pytest.raises(dd.DDError) as err:
+                dd.Tree(n, n, nbits)
+            assert err.value.status == -6
+            continue
+        kinds = ("u16", "u32", "f32") if n in (4, 64, 256) else ("u32",)
+        info = _tree_case(nbits, n, 2 * 960 + 77, kinds)
+        assert info["passes"] == (1 if n <= 64 else 2 if n <= 1024 else 3)
+    _tree_case(nbits, 64, 2048, ("u16", "f32"))
+
+
+def test_tree_later_passes_over_several_tiles():
+    # 256 channels: the second pass (two steps) stores 16192 columns per tile; 40000 samples are three of its tiles
+    info = _tree_case(2, 256, 40000)
+    assert info["passes"] == 2 and info["tile"][1] < 20000
+    info = _tree_case(4, 1024, 7000)       # second pass (four steps): tiles of 3136
+    assert info["steps"] == [6, 4] and info["tile"] == [960, 3136]
+
+
+@pytest.mark.parametrize("first", [1, 2, 3, 4, 5, 6])
+def test_tree_pass_shapes(first):
+    # every radix of the pass kernel as first pass (packed input) and as later pass (16-bit rows), both thread loads
+    for later in (1, 2, 3):
+        for items in (4, 8):
+            info = _tree_case(4, 64, 1500, tuning=((1, first), (2, later), (3, items)))
+            assert info["steps"][0] == first and all(s <= later for s in info["steps"][1:])
+    for later in (4, 5, 6):
+        if first + later <= 8:
+            _tree_case(2, 256, 1100, tuning=((1, first), (2, later)))
+
+
+def _piecewise_case(nbits, nchans, sb, ndm, dm_hi, nsamps, kind="u32"):
+    cfg = _band(nbits, nchans, nsamps)
+    dms = np.linspace(0.0, dm_hi, ndm)
+    with dd.Tree(nchans, sb, nbits) as t:
+        t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
+        dprime, dt2 = t.tables()
+        need = t.required_samples(nsamps)
+        assert need == nsamps + int(dt2.max()) + sb - 1 and int(dprime.max()) < sb
+        packed, stride = W.gen_packed(cfg, need - nsamps, None)
+        got = _run(t, nsamps, packed.cuda(), stride, ndm, kind)
+        info = t.info()
+        assert info["last_launches"] == info["passes"] + 1
+    ref = oracle.piecewise_tree(packed[0].numpy(), nbits, nsamps, nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb)
+    _assert_equal(got, oracle.cast_out(ref, kind), f"piecewise tree {nchans}/{sb} {nbits}-bit {kind}")
+    return dprime, dt2
+
+
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_piecewise_linear_tree_small_bands(nbits):
+    # sub-bands of 8 .. 64 channels, trials up to just below the diagonal DM of the last sub-band, several tiles of both stages
+    dprime, _ = _piecewise_case(nbits, 256, 32, 23, 45.0, 2 * 960 + 501, "u32")
+    assert dprime.max() >= 20                      # the trials do reach far into the trees
+    _piecewise_case(nbits, 256, 8, 9, 50.0, 3000, "f32")
+    _piecewise_case(nbits, 128, 64, 17, 68.0, 2111, "u16" if nbits < 8 else "u32")
+    _piecewise_case(nbits, 64, 64, 5, 70.0, 1000)   # one sub-band: stage 2 only picks rows
+
+
+def test_piecewise_linear_tree_survey_band_and_the_diagonal():
+    # cfg2's band (1024 channels, 2-bit) in sub-bands of 32: the trials of its DM list below the diagonal DM
+    cfg = W.CONFIGS[2]
+    step = cfg.dm_max / (cfg.ndm - 1)
+    dprime, dt2 = _piecewise_case(2, 1024, 32, 40, 39 * step, 5000, "f32")
+    assert dprime.max() < 32 and dt2.max() > 500
+    with dd.Tree(1024, 32, 2) as t:                 # one trial beyond the diagonal: an error, the tree unchanged
+        t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, [0.0, 10.0])
+        with pytest.raises(dd.DDError) as err:
+            t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, [0.0, 10.0, 200.0])
+        assert err.value.status == -6
+        assert t.tables()[0].shape == (2, 32)
+
+
+def test_tree_full_size_survey_band_windows():
+    # cfg2's shape: 1024 channels, 2-bit, 2^19 samples, float32 rows.  The transform is invariant under time shifts, so the
+    # oracle is run on windows of the input: the start, the joints of the tiles of both passes, the end
+    n, nbits, nsamps, win = 1024, 2, 1 << 19, 1536
+    cfg = _band(nbits, n, nsamps)
+    packed, stride = W.gen_packed(cfg, n - 1, None)
+    dev = packed.cuda()
+    with dd.Tree(n, n, nbits) as t:
+        got = _run(t, nsamps, dev, stride, n, "f32")
+        info = t.info()
+        torch.cuda.synchronize()
+    assert info["steps"] == [6, 4]
+    starts = [0, 960 - 64, 3136 - 128, 100 * 3136 - 700, 273 * 960 - 512, nsamps - win]
+    host = packed[0].numpy()
+    for a in starts:
+        assert a % 4 == 0
+        rows = host[:, a // 4:(a + win + n - 1 + 3) // 4 + 1]
+        ref = oracle.tree(np.ascontiguousarray(rows), nbits, win)
+        _assert_equal(got[:, a:a + win], oracle.cast_out(ref, "f32"), f"window at {a}")
+    # every row sums every channel once: the mean level of a row is the mean level of the band
+    assert abs(float(got.mean()) - float(got[0].mean())) < 1.0
