@@ -284,6 +284,85 @@ def run_scrunch(args) -> None:
     sset.close()
 
 
+# ------------------------------------------------------------------------------------------ tree dedispersion (side measurement)
+def run_tree(args) -> None:
+    """`--tree SB`: the tree algorithm (dd_tree_*) on the config's band and length.  SB = channels per
+    tree: the config's channel count gives the whole-band tree (nchans linear trials); a smaller power of two gives the
+    piecewise linear tree for the trials of the config's DM list below its diagonal DM.  Timed like the
+    main arm (CUDA events on the launching stream); a side measurement, not the headline line.  The path is bound by memory:
+    the roofline counts the packed input read once and the output rows written once."""
+    import numpy as np
+    import torch
+
+    import dd_workloads as W
+    import oracle
+    import paper_1201_5380_b200 as dd
+
+    torch.cuda.set_device(0)
+    cfg = W.CONFIGS[args.config]
+    sb = args.tree
+    stream = torch.cuda.Stream()
+    tree = dd.Tree(cfg.nchans, sb, cfg.nbits)
+    dms = None
+    if sb < cfg.nchans:   # the leading trials of the DM list whose sub-band trails stay inside their trees (eq. 21)
+        all_dms = cfg.dm_list()
+        lo, hi = 1, len(all_dms)
+        while lo < hi:
+            mid = (lo + hi + 1) // 2
+            try:
+                tree.set_dm_list(cfg.dt, cfg.f_top, cfg.df, all_dms[:mid])
+                lo = mid
+            except dd.DDError:
+                hi = mid - 1
+        dms = all_dms[:lo]
+        tree.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
+    nrows = len(dms) if dms is not None else cfg.nchans
+    need = tree.required_samples(cfg.nsamps)
+    packed, stride = W.gen_packed(cfg, need - cfg.nsamps, None, device="cuda", beams=[0], chan_chunk=16)
+    out = torch.empty((nrows, cfg.nsamps), dtype=torch.float32, device="cuda")
+    for _ in range(max(args.warmup, 3)):
+        tree.execute(cfg.nsamps, packed[0], stride, out, 32, stream)
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    with ClockSampler(0) as clk:
+        with torch.cuda.stream(stream):
+            ev[0].record(stream)
+            for _ in range(args.steps):
+                tree.execute(cfg.nsamps, packed[0], stride, out, 32, stream)
+            ev[1].record(stream)
+        torch.cuda.synchronize()
+    ms = ev[0].elapsed_time(ev[1]) / args.steps
+    info = tree.info()
+    peaks = measured_peaks()
+    alg_bytes = cfg.nchans * need * cfg.nbits / 8 + nrows * cfg.nsamps * 4
+    achieved = alg_bytes / (ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC + " -- tree algorithm (side measurement)", "value": nrows * cfg.nsamps / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+        "dtype": "u16", "data": "synthetic", "gpu_launches": info["last_launches"] * args.steps,
+        "config": {"workload": cfg.name, "method": "tree" if dms is None else "piecewise linear tree", "sb_nchans": sb,
+                   "trials": nrows, "dm_max": None if dms is None else float(dms[-1]), "passes": info["steps"],
+                   "tile_columns": info["tile"], "device_bytes": info["device_bytes"], "l2": "inputs and outputs larger than L2"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                     "traffic": None, "peak_source": peaks["source"],
+                     "algorithmic_bytes": alg_bytes, "note": "packed input read once + float32 rows written once; the 16-bit rows "
+                     "between the passes (written and read once each) are not counted"},
+        "clocks": clk.summary()}
+    if not args.no_cpu:   # the oracle on a bounded sample: the same band, the first cpu_nsamps outputs
+        sub = cfg.reduced(nsamps=args.cpu_nsamps, nbeams=1)
+        hp, _ = W.gen_packed(sub, need - cfg.nsamps, None)
+        t0 = time.perf_counter()
+        if dms is None:
+            oracle.tree(hp[0].numpy(), cfg.nbits, args.cpu_nsamps)
+        else:
+            oracle.piecewise_tree(hp[0].numpy(), cfg.nbits, args.cpu_nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": nrows * args.cpu_nsamps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{cfg.name}: all channels, first {args.cpu_nsamps} output samples, {nrows} trials"}
+    print(json.dumps(line))
+    tree.close()
+
+
 # ------------------------------------------------------------------------------------------ our arm
 def run_ours(args) -> None:
     import torch
@@ -464,6 +543,8 @@ def main() -> None:
                     "nominal DM) instead of the direct transform; implies --no-e2e")
     ap.add_argument("--scrunch", type=int, default=0, help="MAXF: time the transform with time-scrunching up to this "
                     "factor (a power of two) instead -- a side measurement")
+    ap.add_argument("--tree", type=int, default=0, help="SB: time the tree algorithm on trees of SB channels (the config's channel "
+                    "count: the whole band; smaller: the piecewise linear tree below the diagonal DM) (side measurement)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (dd_set_kernel_variant); 0 = the library's choice")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")
@@ -478,6 +559,8 @@ def main() -> None:
         run_reference(args)
     elif args.scrunch:
         run_scrunch(args)
+    elif args.tree:
+        run_tree(args)
     else:
         run_ours(args)
 

@@ -28,6 +28,7 @@
 
 #include <cuda_runtime.h>
 
+#include "dd_common.cuh"
 #include "dd_kernels.cuh"
 
 namespace dd {
@@ -41,13 +42,11 @@ struct TreePassParams {
     int64_t in_stride;     // bytes between input rows (FIRST: also the bytes readable per row; zero beyond)
     uint8_t *out;          // 16-bit rows, or rows of the caller's type (LAST)
     int64_t out_stride;    // bytes between output rows
-    int64_t out_cols;      // LAST: columns below this are stored; else whole tiles are stored
+    int64_t out_cols;      // columns to produce: LAST stores exactly these, else whole tiles (up to tt - 1 columns more)
     int32_t nbits;         // FIRST: 2, 4, 8
     int32_t out_code;      // LAST: DD_OUT_*
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
-    int32_t tt;            // columns a tile stores (multiple of 64)
-    int32_t ntiles;
 };
 
 // words k .. k + 3 of the 16-bit lane stream w[0..7] (two aligned 16-byte loads) taken from lane 2 E + (amount / 16) on:
@@ -99,54 +98,80 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     static_assert(CH >= 32 && (CH & (CH - 1)) == 0, "a warp's items must share their row");
     extern __shared__ __align__(16) uint16_t sm[];        // [R][C] + one chunk of padding
     const int tid = threadIdx.x, lane = tid & 31;
-    const int tile = blockIdx.x % p.ntiles, g = blockIdx.x / p.ntiles;
+    const int tile = blockIdx.x, g = blockIdx.y;
     const int x = g & ((1 << p.i0) - 1), k = g >> p.i0;
     const int64_t row0 = (static_cast<int64_t>(k) << (p.i0 + Q));
-    const int64_t t0 = static_cast<int64_t>(tile) * p.tt;
+    // the delays of butterfly x add up to at most (x + 1)(R - 1) over the pass: it stores tt columns per tile and needs fewer
+    // tiles than the last butterfly of the block, for which the grid is sized
+    const int tt = (C - (x + 1) * (R - 1)) & ~63;
+    const int64_t t0 = static_cast<int64_t>(tile) * tt;
+    if (t0 >= p.out_cols)
+        return;
 
     // ---- stage R rows x C columns
     if constexpr (FIRST) {
         // packed samples, LSB first: 16 bytes hold SUB chunks of 8 samples; the chunks are taken in an order rotated by
-        // the lane so that the 16-byte stores of a quarter warp fall into distinct banks
+        // the lane so that the 16-byte stores of a quarter warp fall into distinct banks.  Two loads in flight per thread.
         const int nb = p.nbits;
         const int sub = 16 / nb;                         // 8-sample chunks per 16 bytes: 8, 4, 2
-        const int per_row = C / (8 * sub);               // 16-byte loads per row
+        const int lg_per_row = 31 - __clz(C / (8 * sub));   // 16-byte loads per row, a power of two
         const int rot = (lane * sub) >> 3;
-        const uint32_t vmask = (1u << nb) - 1u;
         const int64_t byte0 = t0 * nb / 8;               // (t0 is a multiple of 64)
-        for (int id = tid; id < R * per_row; id += TR_THREADS) {
-            const int r = id / per_row, c16 = id - r * per_row;
+        auto fetch = [&](int id) {
+            const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
             const int64_t off = byte0 + static_cast<int64_t>(c16) * 16;
             const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + off;
-            const uint4 v = off + 16 <= p.in_stride ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
+            return off + 16 <= p.in_stride ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
+        };
+        auto unpack = [&](int id, const uint4 v) {
+            const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
             uint16_t *dst = sm + r * C + c16 * (8 * sub);
             for (int kk0 = 0; kk0 < sub; ++kk0) {
                 const int kk = (kk0 + rot) & (sub - 1);
-                // the 8 samples of chunk kk: 8 nb bits from bit 8 nb kk on
-                const int bit = 8 * nb * kk;
-                const uint32_t lo = sel4(v, bit >> 5), hi = sel4(v, (bit >> 5) + (nb == 8 ? 1 : 0));
                 uint32_t o[4];
-                if (nb == 8) {
-#pragma unroll
-                    for (int h = 0; h < 4; ++h) {
-                        const uint32_t word = h < 2 ? lo : hi;
-                        o[h] = ((word >> (16 * (h & 1))) & 0xFFu) | (((word >> (16 * (h & 1) + 8)) & 0xFFu) << 16);
-                    }
-                } else {
-                    const uint32_t word = lo >> (bit & 31);
+                if (nb == 8) {       // chunk kk: words 2 kk, 2 kk + 1
+                    const uint32_t lo = sel4(v, 2 * kk), hi = sel4(v, 2 * kk + 1);
+                    o[0] = __byte_perm(lo, 0u, 0x4140), o[1] = __byte_perm(lo, 0u, 0x4342);
+                    o[2] = __byte_perm(hi, 0u, 0x4140), o[3] = __byte_perm(hi, 0u, 0x4342);
+                } else if (nb == 4) {   // chunk kk: word kk, 8 nibbles
+                    const uint32_t word = sel4(v, kk);
 #pragma unroll
                     for (int h = 0; h < 4; ++h)
-                        o[h] = ((word >> (2 * h * nb)) & vmask) | (((word >> ((2 * h + 1) * nb)) & vmask) << 16);
+                        o[h] = ((word >> (8 * h)) & 0xFu) | (((word >> (8 * h + 4)) & 0xFu) << 16);
+                } else {                // chunk kk: half kk & 1 of word kk >> 1, 8 pairs of bits
+                    const uint32_t word = sel4(v, kk >> 1) >> (16 * (kk & 1));
+#pragma unroll
+                    for (int h = 0; h < 4; ++h)
+                        o[h] = ((word >> (4 * h)) & 0x3u) | (((word >> (4 * h + 2)) & 0x3u) << 16);
                 }
                 *reinterpret_cast<uint4 *>(dst + kk * 8) = make_uint4(o[0], o[1], o[2], o[3]);
             }
+        };
+        const int total = R << lg_per_row;   // a multiple of the threads (C >= 512 columns of >= 2 bits: >= 8 loads per row ... R rows)
+        for (int id = tid; id < total; id += 2 * TR_THREADS) {
+            const bool two = id + TR_THREADS < total;
+            const uint4 va = fetch(id);
+            const uint4 vb = two ? fetch(id + TR_THREADS) : make_uint4(0, 0, 0, 0);
+            unpack(id, va);
+            if (two)
+                unpack(id + TR_THREADS, vb);
         }
     } else {
-        for (int id = tid; id < R * CH; id += TR_THREADS) {
-            const int r = id / CH, ch = id & (CH - 1);
-            const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + (t0 + ch * 8) * 2;
-            *reinterpret_cast<uint4 *>(sm + r * C + ch * 8) = __ldg(reinterpret_cast<const uint4 *>(src));
+        // 16-bit rows: one bulk copy per row, issued by the first lane of the warps in turn
+        __shared__ uint64_t full;
+        if (tid == 0) {
+            mbar_init(&full, 1);
+            mbar_fence_init();
+            mbar_arrive_expect_tx(&full, static_cast<uint32_t>(R * C * 2));
         }
+        __syncthreads();
+        if (lane == 0) {
+            for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
+                const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + t0 * 2;
+                tma_bulk_g2s(sm + r * C, src, static_cast<uint32_t>(C * 2), &full);
+            }
+        }
+        mbar_wait(&full, 0);
     }
     if (tid < 4)
         reinterpret_cast<uint32_t *>(sm + R * C)[tid] = 0u;
@@ -190,46 +215,40 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     }
     __syncthreads();
 
-    // ---- store the first tt columns of every row
-    const int tch = p.tt / 8;
-    for (int id = tid; id < R * tch; id += TR_THREADS) {
-        const int r = id / tch, ch = id - r * tch;
-        const uint4 v = *reinterpret_cast<const uint4 *>(sm + r * C + ch * 8);
-        const int64_t col = t0 + ch * 8;
+    // ---- store the first tt columns of every row: a warp per row, consecutive lanes consecutive 16 bytes
+    for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
         uint8_t *orow = p.out + (row0 + (static_cast<int64_t>(x) << Q) + r) * p.out_stride;
-        if constexpr (!LAST) {
-            *reinterpret_cast<uint4 *>(orow + col * 2) = v;
-        } else {
-            if (col >= p.out_cols)
-                continue;
-            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-            uint32_t e[8];
-#pragma unroll
-            for (int h = 0; h < 4; ++h) {
-                e[2 * h] = w[h] & 0xFFFFu;
-                e[2 * h + 1] = w[h] >> 16;
-            }
-            const bool whole = p.vec_ok && col + 8 <= p.out_cols;
-            if (p.out_code == DD_OUT_U16) {
-                if (whole) {
-                    *reinterpret_cast<uint4 *>(orow + col * 2) = v;
-                } else {
+        const uint16_t *srow = sm + r * C;
+        if (!LAST || (p.out_code == DD_OUT_U16 && p.vec_ok)) {
+            for (int ch = lane; ch < tt / 8; ch += 32) {
+                const int64_t col = t0 + ch * 8;
+                if (!LAST || col + 8 <= p.out_cols)
+                    *reinterpret_cast<uint4 *>(orow + col * 2) = *reinterpret_cast<const uint4 *>(srow + ch * 8);
+                else
                     for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
-                        reinterpret_cast<uint16_t *>(orow)[col + h] = static_cast<uint16_t>(e[h]);
-                }
-            } else {
-                if (p.out_code == DD_OUT_F32) {
+                        reinterpret_cast<uint16_t *>(orow)[col + h] = srow[ch * 8 + h];
+            }
+        } else if (p.out_code == DD_OUT_U16) {
+            for (int c = lane; c < tt && t0 + c < p.out_cols; c += 32)
+                reinterpret_cast<uint16_t *>(orow)[t0 + c] = srow[c];
+        } else {
+            const bool f32 = p.out_code == DD_OUT_F32;
+            for (int c4 = lane; c4 < tt / 4; c4 += 32) {
+                const int64_t col = t0 + c4 * 4;
+                if (col >= p.out_cols)
+                    break;
+                const uint2 v = *reinterpret_cast<const uint2 *>(srow + c4 * 4);
+                uint32_t e[4] = {v.x & 0xFFFFu, v.x >> 16, v.y & 0xFFFFu, v.y >> 16};
+                if (f32) {
 #pragma unroll
-                    for (int h = 0; h < 8; ++h)
+                    for (int h = 0; h < 4; ++h)
                         e[h] = __float_as_uint(static_cast<float>(e[h]));
                 }
-                if (whole) {
-                    reinterpret_cast<uint4 *>(orow + col * 4)[0] = make_uint4(e[0], e[1], e[2], e[3]);
-                    reinterpret_cast<uint4 *>(orow + col * 4)[1] = make_uint4(e[4], e[5], e[6], e[7]);
-                } else {
-                    for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
+                if (p.vec_ok && col + 4 <= p.out_cols)
+                    *reinterpret_cast<uint4 *>(orow + col * 4) = make_uint4(e[0], e[1], e[2], e[3]);
+                else
+                    for (int h = 0; h < 4 && col + h < p.out_cols; ++h)
                         reinterpret_cast<uint32_t *>(orow)[col + h] = e[h];
-                }
             }
         }
     }
@@ -300,19 +319,18 @@ struct TreePass {
 };
 
 template <int Q, int ITEMS>
-cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64_t groups, cudaStream_t stream)
+cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
     constexpr int R = 1 << Q;
     constexpr int C = ITEMS * TR_THREADS * 8 / (R / 2);
     const size_t smem = (static_cast<size_t>(R) * C + 8) * 2;
-    const int64_t ctas = groups * p.ntiles;
-    if (ctas <= 0 || ctas > 0x7FFFFFFFLL)
+    if (ntiles <= 0 || ntiles > 0x7FFFFFFFLL || groups <= 0 || groups > 65535)
         return cudaErrorInvalidConfiguration;
     auto go = [&](auto kernel) {
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
         if (e != cudaSuccess)
             return e;
-        kernel<<<static_cast<unsigned>(ctas), TR_THREADS, smem, stream>>>(p);
+        kernel<<<dim3(static_cast<unsigned>(ntiles), static_cast<unsigned>(groups)), TR_THREADS, smem, stream>>>(p);
         return cudaGetLastError();
     };
     if (first)
@@ -321,26 +339,27 @@ cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64
 }
 
 template <int Q>
-cudaError_t launch_pass_q(const TreePassParams &p, int items, bool first, bool last, int64_t groups, cudaStream_t stream)
+cudaError_t launch_pass_q(const TreePassParams &p, int items, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
-    return items == 4 ? launch_pass_qi<Q, 4>(p, first, last, groups, stream) : launch_pass_qi<Q, 8>(p, first, last, groups, stream);
+    return items == 4 ? launch_pass_qi<Q, 4>(p, first, last, groups, ntiles, stream)
+                      : launch_pass_qi<Q, 8>(p, first, last, groups, ntiles, stream);
 }
 
-cudaError_t launch_pass(const TreePassParams &p, int q, int items, bool first, bool last, int64_t groups, cudaStream_t stream)
+cudaError_t launch_pass(const TreePassParams &p, int q, int items, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
     switch (q) {
     case 1:
-        return launch_pass_q<1>(p, items, first, last, groups, stream);
+        return launch_pass_q<1>(p, items, first, last, groups, ntiles, stream);
     case 2:
-        return launch_pass_q<2>(p, items, first, last, groups, stream);
+        return launch_pass_q<2>(p, items, first, last, groups, ntiles, stream);
     case 3:
-        return launch_pass_q<3>(p, items, first, last, groups, stream);
+        return launch_pass_q<3>(p, items, first, last, groups, ntiles, stream);
     case 4:
-        return launch_pass_q<4>(p, items, first, last, groups, stream);
+        return launch_pass_q<4>(p, items, first, last, groups, ntiles, stream);
     case 5:
-        return launch_pass_q<5>(p, items, first, last, groups, stream);
+        return launch_pass_q<5>(p, items, first, last, groups, ntiles, stream);
     case 6:
-        return launch_pass_q<6>(p, items, first, last, groups, stream);
+        return launch_pass_q<6>(p, items, first, last, groups, ntiles, stream);
     }
     return cudaErrorInvalidValue;
 }
@@ -352,7 +371,7 @@ int pass_cols(int q, int items) { return items * TR_THREADS * 8 / ((1 << q) / 2)
 
 struct dd_tree_s {
     int nchans = 0, sb = 0, nbits = 0, steps = 0;
-    int tune[3] = {0, 0, 0};   // steps of the first pass, steps of later passes, items per thread of the first pass
+    int tune[4] = {0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later passes
     // stage 2 (piecewise linear tree)
     int ndm = 0, ns = 0;
     std::vector<int32_t> dprime, dt2;   // [ndm][ns]
@@ -362,7 +381,7 @@ struct dd_tree_s {
     // passes and intermediate rows, sized for `sized_for` output samples with the tuning `sized_tune`
     std::vector<dd::TreePass> passes;
     int64_t sized_for = -1;
-    int sized_tune[3] = {-1, -1, -1};
+    int sized_tune[4] = {-1, -1, -1, -1};
     int sized_ndm = -1;
     void *buf[2] = {nullptr, nullptr};
     size_t buf_bytes[2] = {0, 0};
@@ -389,14 +408,14 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
     t->passes.clear();
     for (int i0 = 0; i0 < t->steps;) {
         const int left = t->steps - i0;
-        const int items = (i0 == 0 && t->tune[2] == 4) ? 4 : 8;
+        const int items = (i0 == 0 ? t->tune[2] : t->tune[3]) == 8 ? 8 : 4;   // 4: two CTAs per SM (measured faster on every pass)
         int q = std::min(left, 6);
         if (i0 == 0 && t->tune[0] > 0)
             q = std::min(q, t->tune[0]);
         if (i0 > 0 && t->tune[1] > 0)
             q = std::min(q, t->tune[1]);
         // later passes: the overlap of neighbouring tiles (the largest delay of the pass) at most half the columns staged
-        // (the first pass: whatever leaves a tile; 63 of 1024 columns for six steps)
+        // (the first pass: whatever leaves a tile; 63 of 512 columns for six steps)
         for (; q > 1; --q) {
             const int64_t halo = (int64_t(1) << i0) * ((1 << q) - 1), cols = pass_cols(q, items);
             if ((i0 == 0 || t->tune[1] > 0 || 2 * halo <= cols) && halo + 64 <= cols)
@@ -419,9 +438,9 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
     for (int p = static_cast<int>(t->passes.size()) - 1; p >= 0; --p) {
         TreePass &ps = t->passes[p];
         ps.out_cols = need;
-        ps.ntiles = (need + ps.tt - 1) / ps.tt;
-        t->pitch[p] = ps.ntiles * ps.tt + 32;   // whole tiles are stored; stage 2 reads up to 23 columns past its last sample
-        need = (ps.ntiles - 1) * ps.tt + ps.cols;
+        ps.ntiles = (need + ps.tt - 1) / ps.tt;   // of the butterfly with the largest delays (tt columns per tile); the others need fewer
+        t->pitch[p] = (need + ps.cols + 32 + 63) & ~int64_t(63);   // whole tiles are stored; stage 2 reads up to 23 columns past its last sample
+        need = (need + ps.cols + 63) & ~int64_t(63);   // the last tile of a butterfly starts below `need` and stages cols columns
     }
     return true;
 }
@@ -572,7 +591,7 @@ dd_status dd_tree_set_tuning(dd_tree tree, int key, int value)
 {
     if (!tree)
         return DD_ERR_NULL;
-    if (key < 1 || key > 3 || value < 0 || (key <= 2 && value > 6) || (key == 3 && value != 0 && value != 4 && value != 8))
+    if (key < 1 || key > 4 || value < 0 || (key <= 2 && value > 6) || (key >= 3 && value != 0 && value != 4 && value != 8))
         return DD_ERR_INVALID_ARG;
     tree->tune[key - 1] = value;
     return DD_OK;
@@ -620,7 +639,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
 
     // ---- passes and intermediate rows for this size (first call, or the size / tuning / DM list changed)
     if (tree->sized_for != t_out || tree->sized_ndm != tree->ndm || tree->sized_tune[0] != tree->tune[0] ||
-        tree->sized_tune[1] != tree->tune[1] || tree->sized_tune[2] != tree->tune[2]) {
+        tree->sized_tune[1] != tree->tune[1] || tree->sized_tune[2] != tree->tune[2] || tree->sized_tune[3] != tree->tune[3]) {
         tree->sized_for = -1;
         if (!plan_passes(tree, t_out)) {
             set_error_text("dd_tree_execute: the tuning leaves a pass without room for a tile");
@@ -647,7 +666,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         }
         tree->sized_for = t_out;
         tree->sized_ndm = tree->ndm;
-        for (int i = 0; i < 3; ++i)
+        for (int i = 0; i < 4; ++i)
             tree->sized_tune[i] = tree->tune[i];
     }
     if (stage2 && !tree->tab_uploaded) {
@@ -684,10 +703,8 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.out_code = out_nbits;
         kp.vec_ok = rows16 ? 1 : 0;
         kp.i0 = ps.i0;
-        kp.tt = ps.tt;
-        kp.ntiles = static_cast<int32_t>(ps.ntiles);
         const int64_t groups = tree->nchans >> ps.q;
-        if ((e = launch_pass(kp, ps.q, ps.items, first, last, groups, st)) != cudaSuccess)
+        if ((e = launch_pass(kp, ps.q, ps.items, first, last, groups, ps.ntiles, st)) != cudaSuccess)
             return report_cuda_error(e, "dd_tree_execute pass");
         ++launches;
     }
