@@ -35,68 +35,117 @@ namespace dd {
 namespace {
 
 constexpr int TR_THREADS = 512;
-constexpr int TR_SMEM_ELEMS = 65536;   // 16-bit lanes staged by a CTA with ITEMS = 8 (128 KB); ITEMS = 4: half
 
 struct TreePassParams {
-    const uint8_t *in;     // FIRST: packed rows; else 16-bit rows
-    int64_t in_stride;     // bytes between input rows (FIRST: also the bytes readable per row; zero beyond)
-    uint8_t *out;          // 16-bit rows, or rows of the caller's type (LAST)
+    const uint8_t *in;     // PACKED: rows of nbits-wide samples (nbits = 8: the 8-bit rows of a first pass); else 16-bit rows
+    int64_t in_stride;     // bytes between input rows (PACKED: also the bytes readable per row; zero beyond)
+    uint8_t *out;          // rows of LB-bit lanes, or rows of the caller's type (LAST)
     int64_t out_stride;    // bytes between output rows
     int64_t out_cols;      // columns to produce: LAST stores exactly these, else whole tiles (up to tt - 1 columns more)
-    int32_t nbits;         // FIRST: 2, 4, 8
+    int32_t nbits;         // PACKED: 2, 4, 8
     int32_t out_code;      // LAST: DD_OUT_*
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
 };
 
-// words k .. k + 3 of the 16-bit lane stream w[0..7] (two aligned 16-byte loads) taken from lane 2 E + (amount / 16) on:
-// amount = 0 / 16 gives the window for b = 0 at an even / odd lane offset, + 16 the window for b = 1
-template <int E>
+// words k .. k + 3 of the lane stream w[0..7] (two aligned 16-byte loads) from word E, bit `amount` on, and one lane further
+template <int E, int LB>
 __device__ __forceinline__ void tree_window(const uint32_t (&w)[8], uint32_t amount, uint32_t (&x0)[4], uint32_t (&x1)[4])
 {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         x0[k] = __funnelshift_rc(w[k + E], w[k + E + 1], amount);
-        x1[k] = __funnelshift_rc(w[k + E], w[k + E + 1], amount + 16);
+        x1[k] = __funnelshift_rc(w[k + E], w[k + E + 1], amount + LB);   // (32: the next word)
     }
 }
 
-// the 8 lanes from lane offset e (0..7, the same for every thread of a warp) on, and the 8 lanes from e + 1 on
+// the 128 / LB lanes from lane offset e (0 .. 128 / LB - 1, the same for every thread of a warp) on (x0), and those from
+// e + 1 on (x1), of LB-bit lanes
+template <int LB>
 __device__ __forceinline__ void tree_windows(const uint4 a, const uint4 b, int e, uint32_t (&x0)[4], uint32_t (&x1)[4])
 {
+    constexpr int LPW = 32 / LB;   // lanes per word
     const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-    const uint32_t amount = (e & 1) * 16;
-    switch (e >> 1) {
+    const uint32_t amount = (e & (LPW - 1)) * LB;
+    switch (e / LPW) {
     case 0:
-        tree_window<0>(w, amount, x0, x1);
+        tree_window<0, LB>(w, amount, x0, x1);
         break;
     case 1:
-        tree_window<1>(w, amount, x0, x1);
+        tree_window<1, LB>(w, amount, x0, x1);
         break;
     case 2:
-        tree_window<2>(w, amount, x0, x1);
+        tree_window<2, LB>(w, amount, x0, x1);
         break;
     default:
-        tree_window<3>(w, amount, x0, x1);
+        tree_window<3, LB>(w, amount, x0, x1);
         break;
     }
 }
 
 __device__ __forceinline__ uint32_t sel4(const uint4 v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
 
+// 16 bytes of lanes (one chunk: 128 / LB samples) from packed samples, LSB first; kk = index of the chunk inside the 16
+// packed bytes v
+template <int LB>
+__device__ __forceinline__ uint4 tree_unpack_chunk(const uint4 v, int nb, int kk)
+{
+    uint32_t o[4];
+    if constexpr (LB == 16) {   // 8 samples
+        if (nb == 8) {          // words 2 kk, 2 kk + 1
+            const uint32_t lo = sel4(v, 2 * kk), hi = sel4(v, 2 * kk + 1);
+            o[0] = __byte_perm(lo, 0u, 0x4140), o[1] = __byte_perm(lo, 0u, 0x4342);
+            o[2] = __byte_perm(hi, 0u, 0x4140), o[3] = __byte_perm(hi, 0u, 0x4342);
+        } else if (nb == 4) {   // word kk, 8 nibbles
+            const uint32_t word = sel4(v, kk);
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                o[h] = ((word >> (8 * h)) & 0xFu) | (((word >> (8 * h + 4)) & 0xFu) << 16);
+        } else {                // half kk & 1 of word kk >> 1, 8 pairs of bits
+            const uint32_t word = sel4(v, kk >> 1) >> (16 * (kk & 1));
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                o[h] = ((word >> (4 * h)) & 0x3u) | (((word >> (4 * h + 2)) & 0x3u) << 16);
+        }
+    } else {                    // 16 samples into bytes
+        if (nb == 4) {          // words 2 kk, 2 kk + 1: 4 nibbles per output word
+            const uint32_t lo = sel4(v, 2 * kk), hi = sel4(v, 2 * kk + 1);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const uint32_t hw = ((h < 2 ? lo : hi) >> (16 * (h & 1))) & 0xFFFFu;
+                const uint32_t t = (hw | (hw << 8)) & 0x00FF00FFu;
+                o[h] = (t | (t << 4)) & 0x0F0F0F0Fu;
+            }
+        } else {                // word kk: 4 pairs of bits per output word
+            const uint32_t word = sel4(v, kk);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const uint32_t b = (word >> (8 * h)) & 0xFFu;
+                const uint32_t t = (b | (b << 12)) & 0x000F000Fu;
+                o[h] = (t | (t << 6)) & 0x03030303u;
+            }
+        }
+    }
+    return make_uint4(o[0], o[1], o[2], o[3]);
+}
+
 // One pass: steps i0 .. i0 + Q - 1 for one butterfly (R = 2^Q rows) and one time tile.
 //   group g = k 2^i0 + x: butterfly x of block k (blocks of B = R 2^i0 rows after the pass)
 //   staged row b' (level i0) = global row k B + b' 2^i0 + x;   stored row o' = global row k B + x R + o'
 // In local terms step q combines the local blocks of 2^q rows pairwise exactly as the whole tree does, with x 2^q added to
 // every delay: out[c][2 o + b] = in[2c][o] + in[2c + 1][o] at + (x 2^q + o + b).
-template <int Q, int ITEMS, bool FIRST, bool LAST>
+// LB = bits per lane in shared memory: 16, or 8 for a first pass whose sums stay below 256 (2-bit samples: up to 64
+// channels) -- half the shared-memory traffic per sample, which bounds the pass, and half the bytes written.
+template <int Q, int ITEMS, bool PACKED, bool LAST, int LB>
 __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(const TreePassParams p)
 {
     constexpr int R = 1 << Q;
-    constexpr int C = ITEMS * TR_THREADS * 8 / (R / 2);   // columns staged per row
-    constexpr int CH = C / 8;                             // 16-byte chunks per row (>= 64: a warp stays inside one row)
+    constexpr int CPC = 128 / LB;                           // columns per 16-byte chunk
+    constexpr int CH = ITEMS * TR_THREADS / (R / 2);        // 16-byte chunks per row (>= 32: a warp stays inside one row)
+    constexpr int C = CH * CPC;                             // columns staged per row
     static_assert(CH >= 32 && (CH & (CH - 1)) == 0, "a warp's items must share their row");
-    extern __shared__ __align__(16) uint16_t sm[];        // [R][C] + one chunk of padding
+    static_assert(LB == 16 || (LB == 8 && PACKED), "8-bit lanes: first pass only");
+    extern __shared__ uint4 smv[];                          // [R][CH] + one chunk of padding
     const int tid = threadIdx.x, lane = tid & 31;
     const int tile = blockIdx.x, g = blockIdx.y;
     const int x = g & ((1 << p.i0) - 1), k = g >> p.i0;
@@ -109,14 +158,14 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         return;
 
     // ---- stage R rows x C columns
-    if constexpr (FIRST) {
-        // packed samples, LSB first: 16 bytes hold SUB chunks of 8 samples; the chunks are taken in an order rotated by
-        // the lane so that the 16-byte stores of a quarter warp fall into distinct banks.  Two loads in flight per thread.
+    if constexpr (PACKED) {
+        // 16 packed bytes hold SUB chunks; they are taken in an order rotated by the lane so that the 16-byte stores of a
+        // quarter warp fall into distinct banks.  Two loads in flight per thread.
         const int nb = p.nbits;
-        const int sub = 16 / nb;                         // 8-sample chunks per 16 bytes: 8, 4, 2
-        const int lg_per_row = 31 - __clz(C / (8 * sub));   // 16-byte loads per row, a power of two
+        const int sub = 128 / (CPC * nb);                   // chunks per 16 packed bytes: 8, 4, 2 (16-bit lanes) / 4, 2 (8-bit)
+        const int lg_per_row = 31 - __clz(CH / sub);        // 16-byte loads per row, a power of two
         const int rot = (lane * sub) >> 3;
-        const int64_t byte0 = t0 * nb / 8;               // (t0 is a multiple of 64)
+        const int64_t byte0 = t0 * nb / 8;                  // (t0 is a multiple of 64)
         auto fetch = [&](int id) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
             const int64_t off = byte0 + static_cast<int64_t>(c16) * 16;
@@ -125,29 +174,13 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         };
         auto unpack = [&](int id, const uint4 v) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
-            uint16_t *dst = sm + r * C + c16 * (8 * sub);
+            uint4 *dst = smv + r * CH + c16 * sub;
             for (int kk0 = 0; kk0 < sub; ++kk0) {
                 const int kk = (kk0 + rot) & (sub - 1);
-                uint32_t o[4];
-                if (nb == 8) {       // chunk kk: words 2 kk, 2 kk + 1
-                    const uint32_t lo = sel4(v, 2 * kk), hi = sel4(v, 2 * kk + 1);
-                    o[0] = __byte_perm(lo, 0u, 0x4140), o[1] = __byte_perm(lo, 0u, 0x4342);
-                    o[2] = __byte_perm(hi, 0u, 0x4140), o[3] = __byte_perm(hi, 0u, 0x4342);
-                } else if (nb == 4) {   // chunk kk: word kk, 8 nibbles
-                    const uint32_t word = sel4(v, kk);
-#pragma unroll
-                    for (int h = 0; h < 4; ++h)
-                        o[h] = ((word >> (8 * h)) & 0xFu) | (((word >> (8 * h + 4)) & 0xFu) << 16);
-                } else {                // chunk kk: half kk & 1 of word kk >> 1, 8 pairs of bits
-                    const uint32_t word = sel4(v, kk >> 1) >> (16 * (kk & 1));
-#pragma unroll
-                    for (int h = 0; h < 4; ++h)
-                        o[h] = ((word >> (4 * h)) & 0x3u) | (((word >> (4 * h + 2)) & 0x3u) << 16);
-                }
-                *reinterpret_cast<uint4 *>(dst + kk * 8) = make_uint4(o[0], o[1], o[2], o[3]);
+                dst[kk] = tree_unpack_chunk<LB>(v, nb, kk);
             }
         };
-        const int total = R << lg_per_row;   // a multiple of the threads (C >= 512 columns of >= 2 bits: >= 8 loads per row ... R rows)
+        const int total = R << lg_per_row;
         for (int id = tid; id < total; id += 2 * TR_THREADS) {
             const bool two = id + TR_THREADS < total;
             const uint4 va = fetch(id);
@@ -162,19 +195,19 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         if (tid == 0) {
             mbar_init(&full, 1);
             mbar_fence_init();
-            mbar_arrive_expect_tx(&full, static_cast<uint32_t>(R * C * 2));
+            mbar_arrive_expect_tx(&full, static_cast<uint32_t>(R * CH * 16));
         }
         __syncthreads();
         if (lane == 0) {
             for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
                 const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + t0 * 2;
-                tma_bulk_g2s(sm + r * C, src, static_cast<uint32_t>(C * 2), &full);
+                tma_bulk_g2s(smv + r * CH, src, static_cast<uint32_t>(CH * 16), &full);
             }
         }
         mbar_wait(&full, 0);
     }
-    if (tid < 4)
-        reinterpret_cast<uint32_t *>(sm + R * C)[tid] = 0u;
+    if (tid == 0)
+        smv[R * CH] = make_uint4(0, 0, 0, 0);
 
     // ---- Q steps in place
 #pragma unroll
@@ -188,17 +221,17 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             const int o = pair & ((1 << q) - 1), c = pair >> q;
             const int lrow = ((2 * c) << q) + o;
             const int shift = (x << q) + o;
-            int uch = ch + (shift >> 3);
+            int uch = ch + shift / CPC;
             uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
-            const uint4 l = *reinterpret_cast<const uint4 *>(sm + lrow * C + ch * 8);
-            const uint16_t *u = sm + (lrow + (1 << q)) * C + uch * 8;
-            const uint4 ua = *reinterpret_cast<const uint4 *>(u), ub = *reinterpret_cast<const uint4 *>(u + 8);
+            const uint4 l = smv[lrow * CH + ch];
+            const uint4 *u = smv + (lrow + (1 << q)) * CH + uch;
+            const uint4 ua = u[0], ub = u[1];
             uint32_t x0[4], x1[4];
-            tree_windows(ua, ub, shift & 7, x0, x1);
+            tree_windows<LB>(ua, ub, shift & (CPC - 1), x0, x1);
             const uint32_t lw[4] = {l.x, l.y, l.z, l.w};
 #pragma unroll
             for (int h = 0; h < 4; ++h) {
-                s0[it][h] = lw[h] + x0[h];   // two 16-bit lanes per word; the sums stay below 2^16
+                s0[it][h] = lw[h] + x0[h];   // 32 / LB lanes per word; the sums stay below 2^LB
                 s1[it][h] = lw[h] + x1[h];
             }
         }
@@ -208,9 +241,9 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             const int id = it * TR_THREADS + tid;
             const int ch = id & (CH - 1), pair = id / CH;
             const int o = pair & ((1 << q) - 1), c = pair >> q;
-            uint16_t *dst = sm + ((c << (q + 1)) + 2 * o) * C + ch * 8;
-            *reinterpret_cast<uint4 *>(dst) = make_uint4(s0[it][0], s0[it][1], s0[it][2], s0[it][3]);
-            *reinterpret_cast<uint4 *>(dst + C) = make_uint4(s1[it][0], s1[it][1], s1[it][2], s1[it][3]);
+            uint4 *dst = smv + ((c << (q + 1)) + 2 * o) * CH + ch;
+            dst[0] = make_uint4(s0[it][0], s0[it][1], s0[it][2], s0[it][3]);
+            dst[CH] = make_uint4(s1[it][0], s1[it][1], s1[it][2], s1[it][3]);
         }
     }
     __syncthreads();
@@ -218,27 +251,47 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     // ---- store the first tt columns of every row: a warp per row, consecutive lanes consecutive 16 bytes
     for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
         uint8_t *orow = p.out + (row0 + (static_cast<int64_t>(x) << Q) + r) * p.out_stride;
-        const uint16_t *srow = sm + r * C;
-        if (!LAST || (p.out_code == DD_OUT_U16 && p.vec_ok)) {
-            for (int ch = lane; ch < tt / 8; ch += 32) {
-                const int64_t col = t0 + ch * 8;
-                if (!LAST || col + 8 <= p.out_cols)
-                    *reinterpret_cast<uint4 *>(orow + col * 2) = *reinterpret_cast<const uint4 *>(srow + ch * 8);
-                else
-                    for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
-                        reinterpret_cast<uint16_t *>(orow)[col + h] = srow[ch * 8 + h];
-            }
+        const uint4 *srow = smv + r * CH;
+        if constexpr (!LAST) {
+            for (int ch = lane; ch < tt / CPC; ch += 32)
+                *reinterpret_cast<uint4 *>(orow + (t0 + ch * CPC) * (LB / 8)) = srow[ch];
         } else if (p.out_code == DD_OUT_U16) {
-            for (int c = lane; c < tt && t0 + c < p.out_cols; c += 32)
-                reinterpret_cast<uint16_t *>(orow)[t0 + c] = srow[c];
+            // 8 columns per thread: 16 bytes of 16-bit lanes as they are, or 8 bytes of 8-bit lanes widened
+            for (int c8 = lane; c8 < tt / 8; c8 += 32) {
+                const int64_t col = t0 + c8 * 8;
+                if (col >= p.out_cols)
+                    break;
+                uint4 v;
+                if constexpr (LB == 16) {
+                    v = srow[c8];
+                } else {
+                    const uint2 b = reinterpret_cast<const uint2 *>(srow)[c8];
+                    v = make_uint4(__byte_perm(b.x, 0u, 0x4140), __byte_perm(b.x, 0u, 0x4342), __byte_perm(b.y, 0u, 0x4140),
+                                   __byte_perm(b.y, 0u, 0x4342));
+                }
+                if (p.vec_ok && col + 8 <= p.out_cols) {
+                    *reinterpret_cast<uint4 *>(orow + col * 2) = v;
+                } else {
+                    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+                    for (int h = 0; h < 8 && col + h < p.out_cols; ++h)
+                        reinterpret_cast<uint16_t *>(orow)[col + h] = static_cast<uint16_t>(w[h >> 1] >> (16 * (h & 1)));
+                }
+            }
         } else {
+            // 4 columns per thread: one 16-byte store of 32-bit elements
             const bool f32 = p.out_code == DD_OUT_F32;
             for (int c4 = lane; c4 < tt / 4; c4 += 32) {
                 const int64_t col = t0 + c4 * 4;
                 if (col >= p.out_cols)
                     break;
-                const uint2 v = *reinterpret_cast<const uint2 *>(srow + c4 * 4);
-                uint32_t e[4] = {v.x & 0xFFFFu, v.x >> 16, v.y & 0xFFFFu, v.y >> 16};
+                uint32_t e[4];
+                if constexpr (LB == 16) {
+                    const uint2 v = reinterpret_cast<const uint2 *>(srow)[c4];
+                    e[0] = v.x & 0xFFFFu, e[1] = v.x >> 16, e[2] = v.y & 0xFFFFu, e[3] = v.y >> 16;
+                } else {
+                    const uint32_t v = reinterpret_cast<const uint32_t *>(srow)[c4];
+                    e[0] = v & 0xFFu, e[1] = (v >> 8) & 0xFFu, e[2] = (v >> 16) & 0xFFu, e[3] = v >> 24;
+                }
                 if (f32) {
 #pragma unroll
                     for (int h = 0; h < 4; ++h)
@@ -254,57 +307,73 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     }
 }
 
-// Stage 2 of the piecewise linear tree (eq. 22): out[d][t] = sum_n S[n N' + d'_n(d)][t + Dt''_n(d)] over 16-bit rows S.
-// One thread per 8 consecutive samples of one trial; tab[d][n] = {row, offset}.  The offsets of a (trial, sub-band) are
-// the same for the whole block, so the windows are cut out of two aligned 16-byte loads as in the passes.
+// Stage 2 of the piecewise linear tree (eq. 22): out[d][t] = sum_n S[n N' + d'_n(d)][t + Dt''_n(d)] over rows S of LB-bit
+// lanes.  One thread per 128 / LB consecutive samples of one trial; tab[d][n] = {row, offset}.  The offsets of a (trial,
+// sub-band) are the same for the whole block, so the windows are cut out of two aligned 16-byte loads as in the passes.
 constexpr int TR2_THREADS = 256;
-__global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint16_t *__restrict__ S, int64_t pitch, const int2 *__restrict__ tab,
+template <int LB>
+__global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint8_t *__restrict__ S, int64_t pitch, const int2 *__restrict__ tab,
                                                               int ns, uint8_t *__restrict__ out, int64_t out_stride, int64_t nsamps,
                                                               int out_code, int vec_ok)
 {
+    constexpr int CPC = 128 / LB;
     extern __shared__ int2 stab[];
     const int d = blockIdx.y;
     for (int n = threadIdx.x; n < ns; n += TR2_THREADS)
         stab[n] = __ldg(&tab[static_cast<int64_t>(d) * ns + n]);
     __syncthreads();
-    const int64_t col = (static_cast<int64_t>(blockIdx.x) * TR2_THREADS + threadIdx.x) * 8;
+    const int64_t col = (static_cast<int64_t>(blockIdx.x) * TR2_THREADS + threadIdx.x) * CPC;
     if (col >= nsamps)
         return;
-    uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    uint32_t acc[CPC];
+#pragma unroll
+    for (int h = 0; h < CPC; ++h)
+        acc[h] = 0u;
     for (int n = 0; n < ns; ++n) {
         const int2 e = stab[n];
         const int64_t at = col + e.y;
-        const uint16_t *src = S + static_cast<int64_t>(e.x) * pitch + (at & ~int64_t(7));
-        const uint4 a = __ldg(reinterpret_cast<const uint4 *>(src)), b = __ldg(reinterpret_cast<const uint4 *>(src + 8));
+        const uint8_t *src = S + (static_cast<int64_t>(e.x) * pitch + (at & ~int64_t(CPC - 1))) * (LB / 8);
+        const uint4 a = __ldg(reinterpret_cast<const uint4 *>(src)), b = __ldg(reinterpret_cast<const uint4 *>(src + 16));
         uint32_t x0[4], x1[4];
-        tree_windows(a, b, static_cast<int>(at & 7), x0, x1);
+        tree_windows<LB>(a, b, static_cast<int>(at & (CPC - 1)), x0, x1);
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
-            acc[2 * h] += x0[h] & 0xFFFFu;
-            acc[2 * h + 1] += x0[h] >> 16;
+            if constexpr (LB == 16) {
+                acc[2 * h] += x0[h] & 0xFFFFu;
+                acc[2 * h + 1] += x0[h] >> 16;
+            } else {
+                acc[4 * h] += x0[h] & 0xFFu;
+                acc[4 * h + 1] += (x0[h] >> 8) & 0xFFu;
+                acc[4 * h + 2] += (x0[h] >> 16) & 0xFFu;
+                acc[4 * h + 3] += x0[h] >> 24;
+            }
         }
     }
     uint8_t *orow = out + static_cast<int64_t>(d) * out_stride;
-    const bool whole = vec_ok && col + 8 <= nsamps;
+    const bool whole = vec_ok && col + CPC <= nsamps;
     if (out_code == DD_OUT_U16) {
         if (whole) {
-            *reinterpret_cast<uint4 *>(orow + col * 2) =
-                make_uint4(acc[0] | acc[1] << 16, acc[2] | acc[3] << 16, acc[4] | acc[5] << 16, acc[6] | acc[7] << 16);
+#pragma unroll
+            for (int v = 0; v < CPC / 8; ++v)
+                reinterpret_cast<uint4 *>(orow + col * 2)[v] =
+                    make_uint4(acc[8 * v] | acc[8 * v + 1] << 16, acc[8 * v + 2] | acc[8 * v + 3] << 16,
+                               acc[8 * v + 4] | acc[8 * v + 5] << 16, acc[8 * v + 6] | acc[8 * v + 7] << 16);
         } else {
-            for (int h = 0; h < 8 && col + h < nsamps; ++h)
+            for (int h = 0; h < CPC && col + h < nsamps; ++h)
                 reinterpret_cast<uint16_t *>(orow)[col + h] = static_cast<uint16_t>(acc[h]);
         }
     } else {
         if (out_code == DD_OUT_F32) {
 #pragma unroll
-            for (int h = 0; h < 8; ++h)
+            for (int h = 0; h < CPC; ++h)
                 acc[h] = __float_as_uint(static_cast<float>(acc[h]));
         }
         if (whole) {
-            reinterpret_cast<uint4 *>(orow + col * 4)[0] = make_uint4(acc[0], acc[1], acc[2], acc[3]);
-            reinterpret_cast<uint4 *>(orow + col * 4)[1] = make_uint4(acc[4], acc[5], acc[6], acc[7]);
+#pragma unroll
+            for (int v = 0; v < CPC / 4; ++v)
+                reinterpret_cast<uint4 *>(orow + col * 4)[v] = make_uint4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
         } else {
-            for (int h = 0; h < 8 && col + h < nsamps; ++h)
+            for (int h = 0; h < CPC && col + h < nsamps; ++h)
                 reinterpret_cast<uint32_t *>(orow)[col + h] = acc[h];
         }
     }
@@ -312,18 +381,21 @@ __global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint16_t *__
 
 // ------------------------------------------------------------------------------------------ host side
 struct TreePass {
-    int i0 = 0, q = 0, items = 8;
-    int cols = 0, halo = 0, tt = 0;   // columns staged / largest delay applied / columns stored per tile
+    int i0 = 0, q = 0, items = 4;
+    int lane_bits = 16;               // lanes of the pass in shared memory and of the rows it stores (unless it is the last)
+    bool packed = true;               // input: packed samples (the first pass), or the 8-bit rows of the pass before; else 16-bit rows
+    int in_bits = 0;                  // packed: bits per sample of the input
+    int cols = 0, halo = 0, tt = 0;   // columns staged / largest delay applied / fewest columns a tile stores
     int64_t out_cols = 0;             // columns the pass produces for the current nsamps
     int64_t ntiles = 0;
 };
 
+// kind: 0 = 16-bit rows in, 16-bit lanes; 1 = packed in, 16-bit lanes; 2 = packed in, 8-bit lanes
 template <int Q, int ITEMS>
-cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
+cudaError_t launch_pass_qi(const TreePassParams &p, int kind, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
     constexpr int R = 1 << Q;
-    constexpr int C = ITEMS * TR_THREADS * 8 / (R / 2);
-    const size_t smem = (static_cast<size_t>(R) * C + 8) * 2;
+    const size_t smem = (static_cast<size_t>(R) * (ITEMS * TR_THREADS / (R / 2)) + 1) * 16;
     if (ntiles <= 0 || ntiles > 0x7FFFFFFFLL || groups <= 0 || groups > 65535)
         return cudaErrorInvalidConfiguration;
     auto go = [&](auto kernel) {
@@ -333,45 +405,48 @@ cudaError_t launch_pass_qi(const TreePassParams &p, bool first, bool last, int64
         kernel<<<dim3(static_cast<unsigned>(ntiles), static_cast<unsigned>(groups)), TR_THREADS, smem, stream>>>(p);
         return cudaGetLastError();
     };
-    if (first)
-        return last ? go(dd_tree_pass<Q, ITEMS, true, true>) : go(dd_tree_pass<Q, ITEMS, true, false>);
-    return last ? go(dd_tree_pass<Q, ITEMS, false, true>) : go(dd_tree_pass<Q, ITEMS, false, false>);
+    if (kind == 2)
+        return last ? go(dd_tree_pass<Q, ITEMS, true, true, 8>) : go(dd_tree_pass<Q, ITEMS, true, false, 8>);
+    if (kind == 1)
+        return last ? go(dd_tree_pass<Q, ITEMS, true, true, 16>) : go(dd_tree_pass<Q, ITEMS, true, false, 16>);
+    return last ? go(dd_tree_pass<Q, ITEMS, false, true, 16>) : go(dd_tree_pass<Q, ITEMS, false, false, 16>);
 }
 
 template <int Q>
-cudaError_t launch_pass_q(const TreePassParams &p, int items, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
+cudaError_t launch_pass_q(const TreePassParams &p, int items, int kind, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
-    return items == 4 ? launch_pass_qi<Q, 4>(p, first, last, groups, ntiles, stream)
-                      : launch_pass_qi<Q, 8>(p, first, last, groups, ntiles, stream);
+    return items == 4 ? launch_pass_qi<Q, 4>(p, kind, last, groups, ntiles, stream)
+                      : launch_pass_qi<Q, 8>(p, kind, last, groups, ntiles, stream);
 }
 
-cudaError_t launch_pass(const TreePassParams &p, int q, int items, bool first, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
+cudaError_t launch_pass(const TreePassParams &p, int q, int items, int kind, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
     switch (q) {
     case 1:
-        return launch_pass_q<1>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<1>(p, items, kind, last, groups, ntiles, stream);
     case 2:
-        return launch_pass_q<2>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<2>(p, items, kind, last, groups, ntiles, stream);
     case 3:
-        return launch_pass_q<3>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<3>(p, items, kind, last, groups, ntiles, stream);
     case 4:
-        return launch_pass_q<4>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<4>(p, items, kind, last, groups, ntiles, stream);
     case 5:
-        return launch_pass_q<5>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<5>(p, items, kind, last, groups, ntiles, stream);
     case 6:
-        return launch_pass_q<6>(p, items, first, last, groups, ntiles, stream);
+        return launch_pass_q<6>(p, items, kind, last, groups, ntiles, stream);
     }
     return cudaErrorInvalidValue;
 }
 
-int pass_cols(int q, int items) { return items * TR_THREADS * 8 / ((1 << q) / 2); }
+int pass_cols(int q, int items, int lane_bits) { return items * TR_THREADS * (128 / lane_bits) / ((1 << q) / 2); }
 
 }  // namespace
 }  // namespace dd
 
 struct dd_tree_s {
     int nchans = 0, sb = 0, nbits = 0, steps = 0;
-    int tune[4] = {0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later passes
+    int tune[5] = {0, 0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later
+                                     // passes, lanes of the first pass (16: never 8-bit lanes)
     // stage 2 (piecewise linear tree)
     int ndm = 0, ns = 0;
     std::vector<int32_t> dprime, dt2;   // [ndm][ns]
@@ -381,11 +456,11 @@ struct dd_tree_s {
     // passes and intermediate rows, sized for `sized_for` output samples with the tuning `sized_tune`
     std::vector<dd::TreePass> passes;
     int64_t sized_for = -1;
-    int sized_tune[4] = {-1, -1, -1, -1};
+    int sized_tune[5] = {-1, -1, -1, -1, -1};
     int sized_ndm = -1;
     void *buf[2] = {nullptr, nullptr};
     size_t buf_bytes[2] = {0, 0};
-    int64_t pitch[8] = {};              // columns per row of the output of pass p (16-bit rows)
+    int64_t pitch[8] = {};              // columns per row of the output of pass p
     int64_t last_launches = 0;
 };
 
@@ -406,6 +481,7 @@ int log2_exact(int v)
 bool plan_passes(dd_tree_s *t, int64_t t_out)
 {
     t->passes.clear();
+    const int vmax = (1 << t->nbits) - 1;
     for (int i0 = 0; i0 < t->steps;) {
         const int left = t->steps - i0;
         const int items = (i0 == 0 ? t->tune[2] : t->tune[3]) == 8 ? 8 : 4;   // 4: two CTAs per SM (measured faster on every pass)
@@ -414,16 +490,21 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
             q = std::min(q, t->tune[0]);
         if (i0 > 0 && t->tune[1] > 0)
             q = std::min(q, t->tune[1]);
+        // the first pass adds in 8-bit lanes when its sums stay below 256 (2-bit samples: any first pass; 4-bit: up to 4 steps)
+        auto lanes = [&](int qq) { return (i0 == 0 && t->tune[4] != 16 && vmax * (1 << qq) <= 255) ? 8 : 16; };
         // later passes: the overlap of neighbouring tiles (the largest delay of the pass) at most half the columns staged
-        // (the first pass: whatever leaves a tile; 63 of 512 columns for six steps)
+        // (the first pass: whatever leaves a tile; 63 of 512 or 1024 columns for six steps)
         for (; q > 1; --q) {
-            const int64_t halo = (int64_t(1) << i0) * ((1 << q) - 1), cols = pass_cols(q, items);
+            const int64_t halo = (int64_t(1) << i0) * ((1 << q) - 1), cols = pass_cols(q, items, lanes(q));
             if ((i0 == 0 || t->tune[1] > 0 || 2 * halo <= cols) && halo + 64 <= cols)
                 break;
         }
         TreePass ps;
         ps.i0 = i0, ps.q = q, ps.items = items;
-        ps.cols = pass_cols(q, items);
+        ps.lane_bits = lanes(q);
+        ps.packed = i0 == 0 || t->passes.back().lane_bits == 8;
+        ps.in_bits = i0 == 0 ? t->nbits : 8;
+        ps.cols = pass_cols(q, items, ps.lane_bits);
         ps.halo = static_cast<int>((int64_t(1) << i0) * ((1 << q) - 1));
         ps.tt = (ps.cols - ps.halo) & ~63;
         if (ps.tt < 64)
@@ -433,13 +514,13 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
     }
     if (t->passes.size() > 6)
         return false;
-    // columns every pass has to produce, backwards: a pass stages (ntiles - 1) tt + cols columns of the one before
+    // columns every pass has to produce, backwards
     int64_t need = t_out;
     for (int p = static_cast<int>(t->passes.size()) - 1; p >= 0; --p) {
         TreePass &ps = t->passes[p];
         ps.out_cols = need;
         ps.ntiles = (need + ps.tt - 1) / ps.tt;   // of the butterfly with the largest delays (tt columns per tile); the others need fewer
-        t->pitch[p] = (need + ps.cols + 32 + 63) & ~int64_t(63);   // whole tiles are stored; stage 2 reads up to 23 columns past its last sample
+        t->pitch[p] = (need + ps.cols + 32 + 63) & ~int64_t(63);   // whole tiles are stored; stage 2 reads up to 47 columns past its last sample
         need = (need + ps.cols + 63) & ~int64_t(63);   // the last tile of a butterfly starts below `need` and stages cols columns
     }
     return true;
@@ -591,7 +672,8 @@ dd_status dd_tree_set_tuning(dd_tree tree, int key, int value)
 {
     if (!tree)
         return DD_ERR_NULL;
-    if (key < 1 || key > 4 || value < 0 || (key <= 2 && value > 6) || (key >= 3 && value != 0 && value != 4 && value != 8))
+    if (key < 1 || key > 5 || value < 0 || (key <= 2 && value > 6) || ((key == 3 || key == 4) && value != 0 && value != 4 && value != 8) ||
+        (key == 5 && value != 0 && value != 16))
         return DD_ERR_INVALID_ARG;
     tree->tune[key - 1] = value;
     return DD_OK;
@@ -639,7 +721,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
 
     // ---- passes and intermediate rows for this size (first call, or the size / tuning / DM list changed)
     if (tree->sized_for != t_out || tree->sized_ndm != tree->ndm || tree->sized_tune[0] != tree->tune[0] ||
-        tree->sized_tune[1] != tree->tune[1] || tree->sized_tune[2] != tree->tune[2] || tree->sized_tune[3] != tree->tune[3]) {
+        tree->sized_tune[1] != tree->tune[1] || tree->sized_tune[2] != tree->tune[2] || tree->sized_tune[3] != tree->tune[3] || tree->sized_tune[4] != tree->tune[4]) {
         tree->sized_for = -1;
         if (!plan_passes(tree, t_out)) {
             set_error_text("dd_tree_execute: the tuning leaves a pass without room for a tile");
@@ -649,7 +731,8 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         size_t need[2] = {0, 0};
         for (int p = 0; p < np; ++p)
             if (p + 1 < np || stage2)   // (the last pass of the plain tree writes the caller's rows)
-                need[p & 1] = std::max(need[p & 1], static_cast<size_t>(tree->nchans) * static_cast<size_t>(tree->pitch[p]) * 2);
+                need[p & 1] = std::max(need[p & 1], static_cast<size_t>(tree->nchans) * static_cast<size_t>(tree->pitch[p]) *
+                                                static_cast<size_t>(tree->passes[p].lane_bits / 8));
         for (int i = 0; i < 2; ++i) {
             if (tree->buf_bytes[i] < need[i]) {
                 if (tree->buf[i])
@@ -666,7 +749,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         }
         tree->sized_for = t_out;
         tree->sized_ndm = tree->ndm;
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 5; ++i)
             tree->sized_tune[i] = tree->tune[i];
     }
     if (stage2 && !tree->tab_uploaded) {
@@ -695,24 +778,28 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         const bool first = p == 0, last = p + 1 == np && !stage2;
         TreePassParams kp{};
         kp.in = first ? static_cast<const uint8_t *>(in_ptr) : static_cast<const uint8_t *>(tree->buf[(p - 1) & 1]);
-        kp.in_stride = first ? in_stride : tree->pitch[p - 1] * 2;
+        kp.in_stride = first ? in_stride : tree->pitch[p - 1] * (tree->passes[p - 1].lane_bits / 8);
         kp.out = last ? static_cast<uint8_t *>(out_ptr) : static_cast<uint8_t *>(tree->buf[p & 1]);
-        kp.out_stride = last ? out_pitch_bytes : tree->pitch[p] * 2;
+        kp.out_stride = last ? out_pitch_bytes : tree->pitch[p] * (ps.lane_bits / 8);
         kp.out_cols = last ? nsamps : ps.out_cols;
-        kp.nbits = tree->nbits;
+        kp.nbits = ps.in_bits;
         kp.out_code = out_nbits;
         kp.vec_ok = rows16 ? 1 : 0;
         kp.i0 = ps.i0;
         const int64_t groups = tree->nchans >> ps.q;
-        if ((e = launch_pass(kp, ps.q, ps.items, first, last, groups, ps.ntiles, st)) != cudaSuccess)
+        const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
+        if ((e = launch_pass(kp, ps.q, ps.items, kind, last, groups, ps.ntiles, st)) != cudaSuccess)
             return report_cuda_error(e, "dd_tree_execute pass");
         ++launches;
     }
     // ---- stage 2
     if (stage2) {
-        const dim3 grid(static_cast<unsigned>((nsamps + TR2_THREADS * 8 - 1) / (TR2_THREADS * 8)), static_cast<unsigned>(tree->ndm));
-        dd_tree_stage2<<<grid, TR2_THREADS, static_cast<size_t>(tree->ns) * sizeof(int2), st>>>(
-            static_cast<const uint16_t *>(tree->buf[(np - 1) & 1]), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
+        const int lb = tree->passes[np - 1].lane_bits;
+        const int cpt = 128 / lb;   // columns per thread
+        const dim3 grid(static_cast<unsigned>((nsamps + TR2_THREADS * cpt - 1) / (TR2_THREADS * cpt)), static_cast<unsigned>(tree->ndm));
+        auto s2 = lb == 8 ? dd_tree_stage2<8> : dd_tree_stage2<16>;
+        s2<<<grid, TR2_THREADS, static_cast<size_t>(tree->ns) * sizeof(int2), st>>>(
+            static_cast<const uint8_t *>(tree->buf[(np - 1) & 1]), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
             static_cast<uint8_t *>(out_ptr), out_pitch_bytes, nsamps, out_nbits, rows16 ? 1 : 0);
         if ((e = cudaGetLastError()) != cudaSuccess)
             return report_cuda_error(e, "dd_tree_execute stage 2");

@@ -84,19 +84,22 @@ def test_tree_later_passes_over_several_tiles():
 @pytest.mark.parametrize("first", [1, 2, 3, 4, 5, 6])
 def test_tree_pass_shapes(first):
     # every radix of the pass kernel as first pass (packed input) and as later pass (16-bit rows), both thread loads
+    # (2-bit samples: 8-bit lanes in the first pass unless told otherwise; 4-bit: only while 15 * 2^first < 256)
     for later in (1, 2, 3):
-        for items in (4, 8):
-            info = _tree_case(4, 64, 1500, tuning=((1, first), (2, later), (3, items), (4, items)))
+        for items, nbits, lanes in ((4, 4, 0), (8, 2, 0), (4, 2, 16), (8, 4, 16)):
+            info = _tree_case(nbits, 64, 1500, tuning=((1, first), (2, later), (3, items), (4, items), (5, lanes)))
             assert info["steps"][0] == first and all(s <= later for s in info["steps"][1:])
     for later in (4, 5, 6):
         if first + later <= 8:
             _tree_case(2, 256, 1100, tuning=((1, first), (2, later)))
 
 
-def _piecewise_case(nbits, nchans, sb, ndm, dm_hi, nsamps, kind="u32"):
+def _piecewise_case(nbits, nchans, sb, ndm, dm_hi, nsamps, kind="u32", tuning=()):
     cfg = _band(nbits, nchans, nsamps)
     dms = np.linspace(0.0, dm_hi, ndm)
     with dd.Tree(nchans, sb, nbits) as t:
+        for key, value in tuning:
+            t.set_tuning(key, value)
         t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
         dprime, dt2 = t.tables()
         need = t.required_samples(nsamps)
@@ -118,6 +121,9 @@ def test_piecewise_linear_tree_small_bands(nbits):
     _piecewise_case(nbits, 256, 8, 9, 50.0, 3000, "f32")
     _piecewise_case(nbits, 128, 64, 17, 68.0, 2111, "u16" if nbits < 8 else "u32")
     _piecewise_case(nbits, 64, 64, 5, 70.0, 1000)   # one sub-band: stage 2 only picks rows
+    # stage-1 rows in 16-bit lanes where the default is 8-bit lanes (2-bit samples), and two passes of stage 1
+    _piecewise_case(nbits, 256, 32, 23, 45.0, 2000, "u16" if nbits < 8 else "u32", tuning=((5, 16),))
+    _piecewise_case(nbits, 128, 64, 17, 68.0, 1500, "f32", tuning=((1, 3), (2, 3)))
 
 
 def test_piecewise_linear_tree_survey_band_and_the_diagonal():
