@@ -26,7 +26,8 @@ from .oracle_np import (delay_table_np, dedisperse_gather_np, dedisperse_points,
                         unpack_np, dedisperse_loops_py, subband_tables, subband_required_samples,
                         subband_dedisperse_np, time_scrunch_np, diagonal_dm_np, scrunch_factors_np,
                         scrunched_dedisperse_np, tree_theta, tree_phi, tree_np, tree_delays_np, piecewise_tree_tables,
-                        piecewise_tree_required_samples, piecewise_tree_np)
+                        piecewise_tree_required_samples, piecewise_tree_np, padded_tree_map, padded_tree_np,
+                        padded_tree_dm)
 
 _LIB: Optional[ctypes.CDLL] = None
 
@@ -177,3 +178,10 @@ def piecewise_tree(packed: np.ndarray, nbits: int, nsamps: int, nchans: int, dt:
     dprime, dt2 = piecewise_tree_tables(nchans, dt, f_top, df, dm_list, sb_nchans)
     need = piecewise_tree_required_samples(nsamps, dprime, dt2, sb_nchans)
     return piecewise_tree_np(unpack(packed, nbits, need), nsamps, dprime, dt2, sb_nchans)
+
+
+def padded_tree(packed: np.ndarray, nbits: int, nsamps: int, f_top: float, df: float) -> np.ndarray:
+    """The frequency-padded tree (eq. 25; readings X6-X8 in oracle_np.py) of one packed beam
+    uint8 [nchans][stride]: int64 D'[d'][t], d' < N_pad."""
+    pos, npad = padded_tree_map(packed.shape[0], f_top, df)
+    return padded_tree_np(unpack(packed, nbits, nsamps + npad - 1), nsamps, pos, npad)

@@ -324,3 +324,42 @@ def piecewise_tree_np(a: np.ndarray, nsamps: int, dprime: np.ndarray, dt2: np.nd
             o = int(dt2[d][n])
             out[d] += s[n, int(dprime[d][n]), o:o + nsamps]
     return out
+
+
+# ------------------------------------------------------------------------------------------ frequency-padded tree
+# PAPER.md:224-242 (section 3.1.2, eq. 24-26) and PAPER.md:307 (how the paper applies it).  Readings:
+#   X6  Eq. 25 gives the row of real channel nu in the stretched band, nu' = round(x(nu)),
+#       x(nu) = 1/2 (nu0 / dnu) [1 - (1 + (dnu / nu0) nu)^-2], rounded as everywhere else (floor(x + 0.5), reading R1).  x is
+#       exactly DeltaT(nu) / s with s = d DeltaT / d nu at nu = 0 (eq. 24): the quadratic delays become s nu', a straight line.
+#   X7  "Evaluating at nu = N_nu gives the total number of frequency channels in the linearised coordinates ... rounded up
+#       to a power of two": N_pad = the smallest power of two >= nu'(N_nu).  The blank rows are zero (the
+#       array is initialised to zero and the input is scattered into it) and the basic tree runs on the N_pad rows.
+#   X8  The trials are those of the basic tree on the stretched band (eq. 9 with eq. 26): trial d' = N_pad - 1 is
+#       DM_diag(padded) = 1 / DeltaT(1), and DM(d') = d' / ((N_pad - 1) DeltaT(1)).
+def padded_tree_map(nchans: int, f_top: float, df: float):
+    """Eq. 25 (X6, X7): (row of every real channel in the stretched band, int64 [nchans]; N_pad)."""
+    nu = np.arange(nchans + 1, dtype=np.float64)
+    y = 1.0 + (df / f_top) * nu
+    x = 0.5 * (f_top / df) * (1.0 - 1.0 / (y * y))
+    pos = np.floor(x + 0.5).astype(np.int64)
+    npad = 1
+    while npad < int(pos[nchans]):
+        npad *= 2
+    return pos[:nchans], npad
+
+
+def padded_tree_np(a: np.ndarray, nsamps: int, pos: np.ndarray, npad: int) -> np.ndarray:
+    """scatter the rows of a [nchans][>= nsamps + npad - 1] into a zero array of npad rows at pos, then the
+    basic tree (eq. 10-13): int64 D'[d'][t], d' < npad."""
+    a = np.asarray(a).astype(np.int64)
+    assert a.shape[1] >= nsamps + npad - 1 and len(pos) == a.shape[0]
+    padded = np.zeros((npad, nsamps + npad - 1), dtype=np.int64)
+    for c in range(a.shape[0]):
+        padded[int(pos[c])] = a[c, :nsamps + npad - 1]
+    return tree_np(padded, nsamps)
+
+
+def padded_tree_dm(dprime, npad: int, dt: float, f_top: float, df: float):
+    """Eq. 9 on the stretched band with eq. 26 (X8): the DM of trial d'."""
+    big_t1 = K_DM * (1.0 / ((f_top + df) * (f_top + df)) - 1.0 / (f_top * f_top)) / dt      # DeltaT(1), eq. 4
+    return np.asarray(dprime, dtype=np.float64) / ((npad - 1) * big_t1)

@@ -660,3 +660,73 @@ def test_p17_piecewise_tree_equals_the_direct_sum_with_its_delays_and_error_boun
     with pytest.raises(ValueError):
         far, far2 = oracle.piecewise_tree_tables(nchans, cfg.dt, cfg.f_top, cfg.df, [400.0], sb)
         oracle.piecewise_tree_np(np.zeros((nchans, 100000), np.uint8), nsamps, far, far2, sb)
+
+
+# ------------------------------------------------------------------ P18: the frequency-padded tree
+def test_p18_padding_map_hand_values():
+    """Eq. 25 by hand for nu0 = 1000, dnu = -100, four channels: x = -5 (1 - (1 - 0.1 nu)^-2) = 0, 1.1728, 2.8125, 5.2041
+    and 8.8889 at nu = 4: rows 0, 1, 3, 5 of a band of 9 -> 16 rows."""
+    from oracle.oracle_np import padded_tree_map
+    pos, npad = padded_tree_map(4, 1000.0, -100.0)
+    assert pos.tolist() == [0, 1, 3, 5] and npad == 16
+    pos, npad = padded_tree_map(2, 1000.0, -1e-6)          # a band so narrow that nothing stretches
+    assert pos.tolist() == [0, 1] and npad == 2
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_p18_padding_map_exact_and_linearising(idx):
+    """Eq. 25 in exact rational arithmetic; the real channels keep their order and never share a row; N_pad is the power
+    of two above nu'(N_nu) and at most twice the channel count; and the map does what eq. 24 wants: the
+    quadratic delay DeltaT(nu) (eq. 4, the pinned delay table's formula) equals s nu' within half a row, s = dDeltaT/dnu at 0."""
+    from fractions import Fraction
+    from oracle.oracle_np import K_DM, padded_tree_map
+    cfg = W.CONFIGS[idx]
+    pos, npad = padded_tree_map(cfg.nchans, cfg.f_top, cfg.df)
+    f0, d = Fraction(cfg.f_top), Fraction(cfg.df)
+    for c in list(range(0, cfg.nchans, 37)) + [cfg.nchans - 1]:
+        y = 1 + d / f0 * c
+        x = Fraction(1, 2) * (f0 / d) * (1 - 1 / (y * y))
+        if abs((x + Fraction(1, 2)) - round(x + Fraction(1, 2))) > Fraction(1, 10**9):     # (not within rounding noise of a tie)
+            assert int(pos[c]) == (x + Fraction(1, 2)).__floor__(), c
+    assert np.all(np.diff(pos) >= 1) and pos[0] == 0
+    assert npad & (npad - 1) == 0 and pos[-1] < npad <= 2 * cfg.nchans and npad // 2 < pos[-1] + 2
+    c = np.arange(cfg.nchans, dtype=np.float64)
+    big_t = K_DM * (1.0 / (cfg.f_top + c * cfg.df) ** 2 - 1.0 / cfg.f_top ** 2) / cfg.dt                  # eq. 4
+    s = K_DM / cfg.dt * (-2.0 * cfg.df / cfg.f_top ** 3)
+    assert np.max(np.abs(big_t - s * pos)) <= 0.5 * s * (1 + 1e-9)
+
+
+@pytest.mark.parametrize("nbits", [2, 8])
+def test_p18_padded_tree_equals_the_direct_sum_with_its_delays(nbits):
+    """The scatter only renames rows and blank rows add nothing: the result is eq. 3 (the pinned C loop) over the REAL
+    channels with the delays of the N_pad-row tree taken at the rows eq. 25 assigns; trial 0 is the plain channel sum."""
+    from oracle.oracle_np import padded_tree_map, padded_tree_np, tree_delays_np
+    nchans, f_top, df, nsamps = 24, 1500.0, -8.0, 200
+    pos, npad = padded_tree_map(nchans, f_top, df)
+    assert npad == 32 and pos[-1] > nchans
+    rng = np.random.default_rng(18 + nbits)
+    a = rng.integers(0, 1 << nbits, size=(nchans, (nsamps + npad - 1 + 3) // 4 * 4), dtype=np.uint8)   # (whole bytes at 2 bits)
+    got = padded_tree_np(a, nsamps, pos, npad)
+    delays = tree_delays_np(npad)[:, pos]
+    ref = oracle.dedisperse_unpacked(a, nsamps, delays)
+    assert np.array_equal(got, ref.astype(np.int64))
+    assert np.array_equal(got[0], a[:, :nsamps].astype(np.int64).sum(axis=0))
+    # through the packed entry point
+    packed = W.pack_rows(torch.from_numpy(a), nbits).numpy()
+    rows = np.zeros((nchans, (packed.shape[1] + 15) // 16 * 16), dtype=np.uint8)
+    rows[:, :packed.shape[1]] = packed
+    assert np.array_equal(oracle.padded_tree(rows, nbits, nsamps, f_top, df), got)
+
+
+def test_p18_trials_of_the_padded_tree():
+    """Eq. 26 / X8: at DM(d') the quadratic delay of every real channel (eq. 4-5) stays within two samples and a half of
+    the delay the tree applies to its row; the last trial is 1 / DeltaT(1)."""
+    from oracle.oracle_np import K_DM, padded_tree_dm, padded_tree_map, tree_delays_np
+    cfg = W.CONFIGS[2].reduced(nsamps=64, nchans=256)
+    pos, npad = padded_tree_map(cfg.nchans, cfg.f_top, cfg.df)
+    c = np.arange(cfg.nchans, dtype=np.float64)
+    big_t = K_DM * (1.0 / (cfg.f_top + c * cfg.df) ** 2 - 1.0 / cfg.f_top ** 2) / cfg.dt
+    dms = padded_tree_dm(np.arange(npad), npad, cfg.dt, cfg.f_top, cfg.df)
+    assert dms[0] == 0 and abs(dms[-1] * big_t[1] - 1.0) < 1e-12
+    tree = tree_delays_np(npad)[:, pos]
+    assert np.max(np.abs(dms[:, None] * big_t[None, :] - tree)) <= 2.5
