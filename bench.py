@@ -302,9 +302,12 @@ def run_tree(args) -> None:
     cfg = W.CONFIGS[args.config]
     sb = args.tree
     stream = torch.cuda.Stream()
-    tree = dd.Tree(cfg.nchans, sb, cfg.nbits)
+    padded = sb < 0   # --tree -1: the frequency-padded tree over the stretched band
+    tree = dd.Tree.padded(cfg.nchans, cfg.f_top, cfg.df, cfg.nbits) if padded else dd.Tree(cfg.nchans, sb, cfg.nbits)
     dms = None
-    if sb < cfg.nchans:   # the leading trials of the DM list whose sub-band trails stay inside their trees (eq. 21)
+    if padded:
+        sb = tree.nchans
+    elif sb < cfg.nchans:   # the leading trials of the DM list whose sub-band trails stay inside their trees (eq. 21)
         all_dms = cfg.dm_list()
         lo, hi = 1, len(all_dms)
         while lo < hi:
@@ -316,7 +319,7 @@ def run_tree(args) -> None:
                 hi = mid - 1
         dms = all_dms[:lo]
         tree.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
-    nrows = len(dms) if dms is not None else cfg.nchans
+    nrows = len(dms) if dms is not None else tree.nchans
     need = tree.required_samples(cfg.nsamps)
     packed, stride = W.gen_packed(cfg, need - cfg.nsamps, None, device="cuda", beams=[0], chan_chunk=16)
     out = torch.empty((nrows, cfg.nsamps), dtype=torch.float32, device="cuda")
@@ -340,7 +343,7 @@ def run_tree(args) -> None:
         "metric": METRIC + " -- tree algorithm (side measurement)", "value": nrows * cfg.nsamps / (ms * 1e-3), "unit": UNIT,
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
         "dtype": "u16", "data": "synthetic", "gpu_launches": info["last_launches"] * args.steps,
-        "config": {"workload": cfg.name, "method": "tree" if dms is None else "piecewise linear tree", "sb_nchans": sb,
+        "config": {"workload": cfg.name, "method": "frequency-padded tree" if padded else ("tree" if dms is None else "piecewise linear tree"), "sb_nchans": sb,
                    "trials": nrows, "dm_max": None if dms is None else float(dms[-1]), "passes": info["steps"],
                    "tile_columns": info["tile"], "device_bytes": info["device_bytes"], "l2": "inputs and outputs larger than L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
@@ -352,7 +355,9 @@ def run_tree(args) -> None:
         sub = cfg.reduced(nsamps=args.cpu_nsamps, nbeams=1)
         hp, _ = W.gen_packed(sub, need - cfg.nsamps, None)
         t0 = time.perf_counter()
-        if dms is None:
+        if padded:
+            oracle.padded_tree(hp[0].numpy(), cfg.nbits, args.cpu_nsamps, cfg.f_top, cfg.df)
+        elif dms is None:
             oracle.tree(hp[0].numpy(), cfg.nbits, args.cpu_nsamps)
         else:
             oracle.piecewise_tree(hp[0].numpy(), cfg.nbits, args.cpu_nsamps, cfg.nchans, cfg.dt, cfg.f_top, cfg.df, dms, sb)
@@ -544,7 +549,8 @@ def main() -> None:
     ap.add_argument("--scrunch", type=int, default=0, help="MAXF: time the transform with time-scrunching up to this "
                     "factor (a power of two) instead -- a side measurement")
     ap.add_argument("--tree", type=int, default=0, help="SB: time the tree algorithm on trees of SB channels (the config's channel "
-                    "count: the whole band; smaller: the piecewise linear tree below the diagonal DM) (side measurement)")
+                    "count: the whole band; smaller: the piecewise linear tree below the diagonal DM; -1: the frequency-padded "
+                    "tree) (side measurement)")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (dd_set_kernel_variant); 0 = the library's choice")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle baseline")

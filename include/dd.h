@@ -308,6 +308,16 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  * dd_tree_create   nchans a power of two, 2 .. 4096; sb_nchans a power of two, 2 .. nchans (== nchans: the whole band is
  *                  one tree); nbits 2, 4 or 8; sb_nchans * (2^nbits - 1) <= 65535 (the stages add in 16-bit lanes), else
  *                  DD_ERR_OUT_RANGE; other values DD_ERR_INVALID_ARG.  No device needed.
+ * dd_tree_create_padded  the frequency-padded tree (section 3.1.2; readings X6-X8): the nchans real channels
+ *                  of the band (f_top, df as in dd_plan_create) are placed at the rows nu'(c) of eq. 25 of a stretched band
+ *                  of N_pad rows (nu'(nchans) rounded up to a power of two; the other rows are blank), in which the
+ *                  quadratic dispersion curves are straight lines, and ONE tree runs over the N_pad rows (the paper scatters
+ *                  the input into a zero array; here the first pass reads through the row map and nothing is
+ *                  copied).  Trial d' of N_pad is DM(d') = d' / ((N_pad - 1) DeltaT(1)) (eq. 26).  N_pad <= 4096 and
+ *                  N_pad * (2^nbits - 1) <= 65535 as for dd_tree_create.  dd_tree_execute then takes nchans input rows of
+ *                  nsamps + N_pad - 1 samples and writes N_pad rows; dd_tree_set_dm_list is DD_ERR_UNSUPPORTED.
+ * dd_tree_get_padding  returns N_pad (negative status on error; DD_ERR_INVALID_ARG for a tree that is not padded) and, if
+ *                  pos is not NULL, writes nu'(c) for the nchans real channels (HOST int32).
  * dd_tree_set_dm_list  selects stage 2 for dm_list (HOST, ndm > 0 finite values >= 0) on the band (dt, f_top, df as in
  *                  dd_plan_create).  A trial with some d'_n(d) >= sb_nchans lies beyond the "diagonal" DM (eq. 21,
  *                  PAPER.md:205-211; reading X5): DD_ERR_OUT_RANGE, the tree unchanged (scrunch the input with
@@ -335,6 +345,8 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  */
 typedef struct dd_tree_s *dd_tree;
 dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits);
+dd_status dd_tree_create_padded(dd_tree *tree, int nchans, double f_top, double df, int nbits);
+int dd_tree_get_padding(dd_tree tree, int32_t *pos);
 dd_status dd_tree_set_dm_list(dd_tree tree, double dt, double f_top, double df, const double *dm_list, int ndm);
 dd_status dd_tree_get_tables(dd_tree tree, int32_t *dprime, int32_t *dt2);
 dd_status dd_tree_get_delays(dd_tree tree, int32_t *delays);

@@ -25,7 +25,7 @@ __all__ = [
     "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
-    "dd_tree_create", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
+    "dd_tree_create", "dd_tree_create_padded", "dd_tree_get_padding", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
     "dd_tree_set_tuning", "dd_tree_get_info", "dd_tree_destroy", "Tree",
     "DD_OUT_F32", "DD_OUT_U16", "DD_OUT_U32", "EXPORTED_SYMBOLS",
 ]
@@ -42,7 +42,7 @@ EXPORTED_SYMBOLS = (
     "dd_strerror", "dd_last_cuda_error",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy",
-    "dd_tree_create", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
+    "dd_tree_create", "dd_tree_create_padded", "dd_tree_get_padding", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
     "dd_tree_set_tuning", "dd_tree_get_info", "dd_tree_destroy",
 )
 
@@ -124,6 +124,10 @@ def lib() -> ctypes.CDLL:
         L.dd_scrunch_destroy.argtypes = [vp]
         L.dd_tree_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32]
         L.dd_tree_set_dm_list.argtypes = [vp, dbl, dbl, dbl, vp, i32]
+        L.dd_tree_create_padded.argtypes = [ctypes.POINTER(vp), i32, dbl, dbl, i32]
+        L.dd_tree_create_padded.restype = i32
+        L.dd_tree_get_padding.argtypes = [vp, vp]
+        L.dd_tree_get_padding.restype = i32
         L.dd_tree_get_tables.argtypes = [vp, vp, vp]
         L.dd_tree_get_delays.argtypes = [vp, vp]
         L.dd_tree_required_samples.argtypes = [vp, i64]
@@ -423,6 +427,19 @@ def dd_tree_create(nchans: int, sb_nchans: int, nbits: int) -> int:
     return h.value
 
 
+def dd_tree_create_padded(nchans: int, f_top: float, df: float, nbits: int) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().dd_tree_create_padded(ctypes.byref(h), int(nchans), float(f_top), float(df), int(nbits)), "dd_tree_create_padded")
+    return h.value
+
+
+def dd_tree_get_padding(tree: int, nchans: int):
+    """(rows of the nchans real channels in the stretched band, N_pad)."""
+    pos = np.empty(nchans, dtype=np.int32)
+    npad = _check(lib().dd_tree_get_padding(tree, ctypes.c_void_p(pos.ctypes.data)), "dd_tree_get_padding")
+    return pos, npad
+
+
 def dd_tree_destroy(tree: int) -> None:
     _check(lib().dd_tree_destroy(tree), "dd_tree_destroy")
 
@@ -472,9 +489,19 @@ class Tree:
     """The tree transform of sub-bands of sb_nchans channels (sb_nchans == nchans: the whole band), optionally followed by
     stage 2 of the piecewise linear tree for a DM list."""
 
-    def __init__(self, nchans: int, sb_nchans: int, nbits: int):
+    def __init__(self, nchans: int, sb_nchans: int, nbits: int, _handle=None):
         self.nchans, self.sb_nchans, self.nbits, self.ndm = int(nchans), int(sb_nchans), int(nbits), 0
-        self.handle = dd_tree_create(nchans, sb_nchans, nbits)
+        self.handle = _handle if _handle is not None else dd_tree_create(nchans, sb_nchans, nbits)
+        self.padding = None
+
+    @classmethod
+    def padded(cls, nchans: int, f_top: float, df: float, nbits: int) -> "Tree":
+        """The frequency-padded tree: `nchans` is then N_pad, `padding` the rows of the real channels."""
+        h = dd_tree_create_padded(nchans, f_top, df, nbits)
+        pos, npad = dd_tree_get_padding(h, nchans)
+        t = cls(npad, npad, nbits, _handle=h)
+        t.padding = pos
+        return t
 
     def set_dm_list(self, dt: float, f_top: float, df: float, dm_list) -> "Tree":
         dd_tree_set_dm_list(self.handle, dt, f_top, df, dm_list)

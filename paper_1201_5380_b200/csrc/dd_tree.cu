@@ -46,6 +46,7 @@ struct TreePassParams {
     int32_t out_code;      // LAST: DD_OUT_*
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
+    const int32_t *row_map;   // first pass of a frequency-padded tree: input row of every tree row, -1 = blank; else NULL
 };
 
 // words k .. k + 3 of the lane stream w[0..7] (two aligned 16-byte loads) from word E, bit `amount` on, and one lane further
@@ -169,8 +170,11 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         auto fetch = [&](int id) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
             const int64_t off = byte0 + static_cast<int64_t>(c16) * 16;
-            const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + off;
-            return off + 16 <= p.in_stride ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
+            int64_t row = row0 + (static_cast<int64_t>(r) << p.i0) + x;
+            if (p.row_map)
+                row = __ldg(&p.row_map[row]);   // (the stretched band of eq. 25: most rows are blank)
+            const uint8_t *src = p.in + row * p.in_stride + off;
+            return (row >= 0 && off + 16 <= p.in_stride) ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
         };
         auto unpack = [&](int id, const uint4 v) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
@@ -444,7 +448,11 @@ int pass_cols(int q, int items, int lane_bits) { return items * TR_THREADS * (12
 }  // namespace dd
 
 struct dd_tree_s {
-    int nchans = 0, sb = 0, nbits = 0, steps = 0;
+    int nchans = 0, sb = 0, nbits = 0, steps = 0;   // nchans: rows of the tree (the stretched band when padded)
+    // frequency-padded tree: the real channels lie at rows pad_pos of a band of nchans rows
+    int nchans_in = 0;                  // real channels (0: not padded)
+    std::vector<int32_t> pad_pos;       // [nchans_in]
+    void *d_row_map = nullptr;          // int32 [nchans]: input row or -1
     int tune[5] = {0, 0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later
                                      // passes, lanes of the first pass (16: never 8-bit lanes)
     // stage 2 (piecewise linear tree)
@@ -567,14 +575,72 @@ dd_status dd_tree_destroy(dd_tree tree)
     dd::tree_free_buffers(tree);
     if (tree->d_tab)
         cudaFree(tree->d_tab);
+    if (tree->d_row_map)
+        cudaFree(tree->d_row_map);
     delete tree;
     return DD_OK;
+}
+
+// Eq. 25: the row of real channel nu in the stretched band, nu' = round(1/2 (nu0 / dnu) [1 - (1 + (dnu / nu0) nu)^-2]); the
+// band has nu'(N_nu) rows, rounded up to a power of two (readings X6, X7).
+dd_status dd_tree_create_padded(dd_tree *tree, int nchans, double f_top, double df, int nbits)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    *tree = nullptr;
+    if (nchans < 2 || nchans > 4096 || !(f_top > 0) || !(df < 0) || !std::isfinite(f_top) || !std::isfinite(df) ||
+        !(f_top + static_cast<double>(nchans) * df > 0) || (nbits != 2 && nbits != 4 && nbits != 8))
+        return DD_ERR_INVALID_ARG;
+    std::vector<int32_t> pos;
+    int64_t total = 0;
+    try {
+        pos.resize(nchans);
+        for (int c = 0; c <= nchans; ++c) {
+            const double y = 1.0 + (df / f_top) * static_cast<double>(c);
+            const double x = 0.5 * (f_top / df) * (1.0 - 1.0 / (y * y));
+            const double r = std::floor(x + 0.5);
+            if (!(r >= 0) || r > 1e9)
+                return DD_ERR_INVALID_ARG;
+            if (c < nchans)
+                pos[c] = static_cast<int32_t>(r);
+            else
+                total = static_cast<int64_t>(r);
+        }
+    } catch (const std::bad_alloc &) {
+        return DD_ERR_NOMEM;
+    }
+    int64_t npad = 2;
+    while (npad < total)
+        npad *= 2;
+    if (npad > 4096)
+        return DD_ERR_INVALID_ARG;   // (the stretched band does not fit the largest tree)
+    dd_tree t = nullptr;
+    const dd_status st = dd_tree_create(&t, static_cast<int>(npad), static_cast<int>(npad), nbits);
+    if (st != DD_OK)
+        return st;
+    t->nchans_in = nchans;
+    t->pad_pos.swap(pos);
+    *tree = t;
+    return DD_OK;
+}
+
+int dd_tree_get_padding(dd_tree tree, int32_t *pos)
+{
+    if (!tree)
+        return DD_ERR_NULL;
+    if (tree->nchans_in == 0)
+        return DD_ERR_INVALID_ARG;
+    if (pos)
+        std::copy(tree->pad_pos.begin(), tree->pad_pos.end(), pos);
+    return tree->nchans;
 }
 
 dd_status dd_tree_set_dm_list(dd_tree tree, double dt, double f_top, double df, const double *dm_list, int ndm)
 {
     if (!tree || !dm_list)
         return DD_ERR_NULL;
+    if (tree->nchans_in > 0)
+        return DD_ERR_UNSUPPORTED;   // (the padded tree is one tree over the stretched band: its trials are fixed, eq. 26)
     if (ndm <= 0 || !(dt > 0) || !(f_top > 0) || !(df < 0) || !std::isfinite(dt) || !std::isfinite(f_top) || !std::isfinite(df) ||
         !(f_top + static_cast<double>(tree->nchans) * df > 0))   // (eq. 20 evaluates DeltaT one channel past the band: X3)
         return DD_ERR_INVALID_ARG;
@@ -713,7 +779,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
     const int64_t required = t_out + tree->sb - 1;
     if (in_stride > INT64_MAX / 8 || in_stride * 8 < required * tree->nbits)
         return DD_ERR_STRIDE_TOO_SMALL;
-    const int64_t top = static_cast<int64_t>(stage2 ? tree->nchans : tree->sb) * ((1 << tree->nbits) - 1);
+    const int64_t top = static_cast<int64_t>(tree->nchans_in > 0 ? tree->nchans_in : (stage2 ? tree->nchans : tree->sb)) * ((1 << tree->nbits) - 1);
     if (out_nbits == DD_OUT_U16 && top > 65535)
         return DD_ERR_OUT_RANGE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -752,6 +818,18 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         for (int i = 0; i < 5; ++i)
             tree->sized_tune[i] = tree->tune[i];
     }
+    if (tree->nchans_in > 0 && !tree->d_row_map) {
+        std::vector<int32_t> map(tree->nchans, -1);
+        for (int c = 0; c < tree->nchans_in; ++c)
+            map[tree->pad_pos[c]] = c;
+        if ((e = cudaMalloc(&tree->d_row_map, map.size() * sizeof(int32_t))) != cudaSuccess ||
+            (e = cudaMemcpy(tree->d_row_map, map.data(), map.size() * sizeof(int32_t), cudaMemcpyHostToDevice)) != cudaSuccess) {
+            if (tree->d_row_map)
+                cudaFree(tree->d_row_map);
+            tree->d_row_map = nullptr;
+            return report_cuda_error(e, "dd_tree_execute upload(row map)");
+        }
+    }
     if (stage2 && !tree->tab_uploaded) {
         std::vector<int2> tab(static_cast<size_t>(tree->ndm) * tree->ns);
         for (int d = 0; d < tree->ndm; ++d)
@@ -786,6 +864,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.out_code = out_nbits;
         kp.vec_ok = rows16 ? 1 : 0;
         kp.i0 = ps.i0;
+        kp.row_map = first ? static_cast<const int32_t *>(tree->d_row_map) : nullptr;
         const int64_t groups = tree->nchans >> ps.q;
         const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
         if ((e = launch_pass(kp, ps.q, ps.items, kind, last, groups, ps.ntiles, st)) != cudaSuccess)

@@ -360,6 +360,18 @@ def test_tree_host_side():
             assert L.dd_tree_execute(t.handle, 5000, 16, need_bytes - 16, 16, 32, None) == -5
             assert L.dd_tree_set_tuning(t.handle, 1, 7) == -2 and L.dd_tree_set_tuning(t.handle, 3, 5) == -2
             assert L.dd_tree_set_tuning(t.handle, 4, 1) == -2 and L.dd_tree_set_tuning(t.handle, 2, 3) == 0
+    # the frequency-padded tree: eq. 25 against the oracle; its trials are fixed (no DM list)
+    from oracle.oracle_np import padded_tree_map
+    for nchans, f_top, df in ((cfg.nchans, cfg.f_top, cfg.df), (24, 1500.0, -8.0), (100, 1581.8, -4.0), (2, 1000.0, -1e-6)):
+        with dd.Tree.padded(nchans, f_top, df, 2) as t:
+            pos, npad = padded_tree_map(nchans, f_top, df)
+            assert np.array_equal(t.padding, pos) and t.nchans == max(npad, 2)
+            assert L.dd_tree_set_dm_list(t.handle, cfg.dt, f_top, df, dms.ctypes.data_as(ctypes.c_void_p), 3) == -12
+            assert t.required_samples(10) == 10 + t.nchans - 1
+    assert L.dd_tree_create_padded(ctypes.byref(h), 4096, 400.0, -0.0244140625, 2) == -2      # 8192 rows: beyond the largest tree
+    assert L.dd_tree_create_padded(ctypes.byref(h), 64, 400.0, 0.1, 2) == -2
+    with dd.Tree(8, 8, 2) as t:
+        assert L.dd_tree_get_padding(t.handle, None) == -2
     with dd.Tree(1024, 256, 8) as t8:
         big = (1 << 20)
         t8.set_dm_list(cfg.dt, cfg.f_top, cfg.df, [0.0, 1.0])

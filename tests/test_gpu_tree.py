@@ -161,3 +161,25 @@ def test_tree_full_size_survey_band_windows():
         _assert_equal(got[:, a:a + win], oracle.cast_out(ref, "f32"), f"window at {a}")
     # every row sums every channel once: the mean level of a row is the mean level of the band
     assert abs(float(got.mean()) - float(got[0].mean())) < 1.0
+
+
+@pytest.mark.parametrize("nbits", [2, 4, 8])
+def test_frequency_padded_tree(nbits):
+    # the real channels at the rows of eq. 25 of a stretched band of N_pad rows, blank rows between them,
+    # one tree over all of it.  Bands that stretch by a few per cent and by 1.56 (the survey band's ratio), one to three passes
+    for nchans, f_top, df, nsamps, kind in ((24, 1500.0, -8.0, 1111, "u32"), (100, 1581.8, -0.390625, 2 * 960 + 77, "u16"),
+                                            (100, 1581.8, -4.0, 3000, "f32"), (1024, 1581.8, -0.390625, 2500, "f32")):
+        cfg = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]].reduced(nsamps=nsamps, ndm=2, nchans=nchans, nbeams=1)
+        try:
+            t = dd.Tree.padded(nchans, f_top, df, nbits)
+        except dd.DDError as err:                      # 8-bit: the 16-bit lanes hold trees of up to 256 rows
+            assert nbits == 8 and err.status == -6
+            continue
+        with t:
+            npad = t.nchans
+            assert t.required_samples(nsamps) == nsamps + npad - 1 and npad >= nchans
+            packed, stride = W.gen_packed(cfg, npad - 1, None)
+            got = _run(t, nsamps, packed.cuda(), stride, npad, kind)
+            assert t.info()["last_launches"] == t.info()["passes"]
+        ref = oracle.padded_tree(packed[0].numpy(), nbits, nsamps, f_top, df)
+        _assert_equal(got, oracle.cast_out(ref, kind), f"padded tree {nchans} -> {npad} rows, {nbits}-bit {kind}")
