@@ -200,6 +200,52 @@ def measure_config(dd, W, torch, cfg, stream, device_index, alu_peak, steps=5, w
 
 
 # ------------------------------------------------------------------------------------------ reference arm
+def measure_trees(dd, torch, cfg, packed_dev, stride, stream, steps=5, warmup=3):
+    """`other_methods` of the headline line: the tree algorithm over the whole band and the piecewise linear tree (sub-bands
+    of 32 channels, the leading trials of the DM list below the diagonal DM) on the SAME device-resident input as the
+    headline measurement, when its rows are long enough; ms per call by CUDA events.  `bench.py --tree` is the full
+    side measurement (roofline, oracle timing)."""
+    out = []
+    for sb in (cfg.nchans, 32):
+        if cfg.nchans & (cfg.nchans - 1) or cfg.nchans * ((1 << cfg.nbits) - 1) > 65535:
+            break
+        tree = dd.Tree(cfg.nchans, sb, cfg.nbits)
+        ndm = 0
+        if sb < cfg.nchans:
+            dms = cfg.dm_list()
+            lo, hi = 1, len(dms)
+            while lo < hi:
+                mid = (lo + hi + 1) // 2
+                try:
+                    tree.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms[:mid])
+                    lo = mid
+                except dd.DDError:
+                    hi = mid - 1
+            tree.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms[:lo])
+            ndm = lo
+        nrows = ndm if ndm else cfg.nchans
+        nsamps = cfg.nsamps
+        if stride * 8 < tree.required_samples(nsamps) * cfg.nbits:      # (the rows were sized for the direct transform)
+            nsamps = (stride * 8 // cfg.nbits - (tree.required_samples(nsamps) - nsamps)) // 64 * 64
+        o = torch.empty((nrows, nsamps), dtype=torch.float32, device="cuda")
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        with torch.cuda.stream(stream):
+            for _ in range(warmup):
+                tree.execute(nsamps, packed_dev, stride, o, 32, stream)
+            ev[0].record(stream)
+            for _ in range(steps):
+                tree.execute(nsamps, packed_dev, stride, o, 32, stream)
+            ev[1].record(stream)
+        torch.cuda.synchronize()
+        ms = ev[0].elapsed_time(ev[1]) / steps
+        out.append({"method": "tree" if not ndm else "piecewise linear tree", "sb_nchans": sb, "trials": nrows, "nsamps": nsamps,
+                    "ms_per_step": ms, "value": nrows * nsamps / (ms * 1e-3), "unit": UNIT, "passes": tree.info()["steps"],
+                    "gpu_launches": tree.info()["last_launches"] * steps})
+        tree.close()
+        del o
+    return out
+
+
 def run_reference(args) -> None:
     import dd_workloads as W
     import oracle
@@ -501,9 +547,13 @@ def run_ours(args) -> None:
     # ---- the other full-size configs of BASELINE.json (cfg4, cfg5, cfg3), 5 timed steps each, same method: inputs
     # generated in HBM, CUDA events on the launching stream, clocks sampled during that config's timed region
     other_configs = None
+    other_methods = None
     if args.config == 2 and not subband and not args.no_others and world == 1 and not args.variant:
         plan.close()
-        del packed, out
+        del out
+        torch.cuda.empty_cache()
+        other_methods = measure_trees(dd, torch, cfg, packed[0], stride, stream, steps=5)   # (on the headline's input rows)
+        del packed
         torch.cuda.empty_cache()
         other_configs = [measure_config(dd, W, torch, W.CONFIGS[i], stream, local_rank, alu_peak, steps=5) for i in (4, 5, 3)]
 
@@ -529,7 +579,7 @@ def run_ours(args) -> None:
                    "parallelism": f"beam-per-gpu x{world}" if world > 1 else "single gpu",
                    **({"method": "sub-band (approximate)", **subband} if subband else {})},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": args.steps * kernels_per_step,
-        "roofline": roofline, "cpu_baseline": cpu_baseline, "other_configs": other_configs,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "other_configs": other_configs, "other_methods": other_methods,
         "wall_s_timed_region": wall,
     }
     print(json.dumps(line))
