@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     // ---- stage R rows x C columns
     if constexpr (PACKED) {
         // 16 packed bytes hold SUB chunks; they are taken in an order rotated by the lane so that the 16-byte stores of a
-        // quarter warp fall into distinct banks.  Two loads in flight per thread.
+        // quarter warp fall into distinct banks.  Up to four loads in flight per thread.
         const int nb = p.nbits;
         const int sub = 128 / (CPC * nb);                   // chunks per 16 packed bytes: 8, 4, 2 (16-bit lanes) / 4, 2 (8-bit)
         const int lg_per_row = 31 - __clz(CH / sub);        // 16-byte loads per row, a power of two
@@ -184,14 +184,26 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
                 dst[kk] = tree_unpack_chunk<LB>(v, nb, kk);
             }
         };
-        const int total = R << lg_per_row;
-        for (int id = tid; id < total; id += 2 * TR_THREADS) {
-            const bool two = id + TR_THREADS < total;
-            const uint4 va = fetch(id);
-            const uint4 vb = two ? fetch(id + TR_THREADS) : make_uint4(0, 0, 0, 0);
-            unpack(id, va);
-            if (two)
-                unpack(id + TR_THREADS, vb);
+        const int total = R << lg_per_row;   // (a power of two)
+        if (total >= 4 * TR_THREADS) {       // four loads in flight per thread
+            for (int id = tid; id < total; id += 4 * TR_THREADS) {
+                uint4 v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    v[j] = fetch(id + j * TR_THREADS);
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    unpack(id + j * TR_THREADS, v[j]);
+            }
+        } else {
+            for (int id = tid; id < total; id += 2 * TR_THREADS) {
+                const bool two = id + TR_THREADS < total;
+                const uint4 va = fetch(id);
+                const uint4 vb = two ? fetch(id + TR_THREADS) : make_uint4(0, 0, 0, 0);
+                unpack(id, va);
+                if (two)
+                    unpack(id + TR_THREADS, vb);
+            }
         }
     } else {
         // 16-bit rows: one bulk copy per row, issued by the first lane of the warps in turn
