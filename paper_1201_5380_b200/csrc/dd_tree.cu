@@ -38,7 +38,8 @@ constexpr int TR_THREADS = 512;
 
 struct TreePassParams {
     const uint8_t *in;     // PACKED: rows of nbits-wide samples (nbits = 8: the 8-bit rows of a first pass); else 16-bit rows
-    int64_t in_stride;     // bytes between input rows (PACKED: also the bytes readable per row; zero beyond)
+    int64_t in_stride;     // bytes between input rows
+    int64_t in_bytes;      // PACKED: bytes readable from the start of a row (zero beyond)
     uint8_t *out;          // rows of LB-bit lanes, or rows of the caller's type (LAST)
     int64_t out_stride;    // bytes between output rows
     int64_t out_cols;      // columns to produce: LAST stores exactly these, else whole tiles (up to tt - 1 columns more)
@@ -46,6 +47,7 @@ struct TreePassParams {
     int32_t out_code;      // LAST: DD_OUT_*
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
+    int32_t tt;            // columns a tile stores (multiple of 64)
     const int32_t *row_map;   // first pass of a frequency-padded tree: input row of every tree row, -1 = blank; else NULL
 };
 
@@ -151,12 +153,19 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     const int tile = blockIdx.x, g = blockIdx.y;
     const int x = g & ((1 << p.i0) - 1), k = g >> p.i0;
     const int64_t row0 = (static_cast<int64_t>(k) << (p.i0 + Q));
-    // the delays of butterfly x add up to at most (x + 1)(R - 1) over the pass: it stores tt columns per tile and needs fewer
-    // tiles than the last butterfly of the block, for which the grid is sized
-    const int tt = (C - (x + 1) * (R - 1)) & ~63;
+    // SKEWED STAGING (passes after the first).  Step q reads U at t + x 2^q + o + b: the part x 2^q is the same for every
+    // row of the step, and over the pass it adds up to x r for staged row r (bit q of r says whether the row is on the U
+    // side at step q).  So row r is staged from column t0 + x r instead of t0 -- rounded down to the 16-byte granule AL of
+    // the rows, and AL columns earlier per set bit of r so that what is left of every shift stays non-negative:
+    //     staged row r starts at column t0 + A(x r) - AL popcount(r),   A(v) = v - v mod AL,
+    //     shift at step q between L = block 2c and U = block 2c + 1:  o + b + AL + (x r_U) mod AL - (x r_L) mod AL.
+    // The overlap of neighbouring tiles falls from x (R - 1) columns (up to 960 of 2048 for the second pass of 1024
+    // channels) to at most (R - 1) + 2 AL Q, for every butterfly alike, and column t of a stored row is column t0 + t.
+    const bool skew = p.i0 > 0;
+    constexpr int AL = PACKED ? 16 : 8;   // columns per 16 bytes of the rows staged: 8-bit rows / 16-bit rows
+    const int tt = p.tt;
     const int64_t t0 = static_cast<int64_t>(tile) * tt;
-    if (t0 >= p.out_cols)
-        return;
+    auto first_col = [&](int r) -> int64_t { return skew ? t0 + ((x * r) & ~(AL - 1)) - AL * __popc(r) : t0; };
 
     // ---- stage R rows x C columns
     if constexpr (PACKED) {
@@ -166,15 +175,14 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         const int sub = 128 / (CPC * nb);                   // chunks per 16 packed bytes: 8, 4, 2 (16-bit lanes) / 4, 2 (8-bit)
         const int lg_per_row = 31 - __clz(CH / sub);        // 16-byte loads per row, a power of two
         const int rot = (lane * sub) >> 3;
-        const int64_t byte0 = t0 * nb / 8;                  // (t0 is a multiple of 64)
         auto fetch = [&](int id) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
-            const int64_t off = byte0 + static_cast<int64_t>(c16) * 16;
+            const int64_t off = first_col(r) * nb / 8 + static_cast<int64_t>(c16) * 16;   // (a multiple of 16)
             int64_t row = row0 + (static_cast<int64_t>(r) << p.i0) + x;
             if (p.row_map)
                 row = __ldg(&p.row_map[row]);   // (the stretched band of eq. 25: most rows are blank)
             const uint8_t *src = p.in + row * p.in_stride + off;
-            return (row >= 0 && off + 16 <= p.in_stride) ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
+            return (row >= 0 && off >= 0 && off + 16 <= p.in_bytes) ? __ldg(reinterpret_cast<const uint4 *>(src)) : make_uint4(0, 0, 0, 0);
         };
         auto unpack = [&](int id, const uint4 v) {
             const int r = id >> lg_per_row, c16 = id & ((1 << lg_per_row) - 1);
@@ -216,7 +224,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         __syncthreads();
         if (lane == 0) {
             for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
-                const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + t0 * 2;
+                const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + first_col(r) * 2;
                 tma_bulk_g2s(smv + r * CH, src, static_cast<uint32_t>(CH * 16), &full);
             }
         }
@@ -236,7 +244,8 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             const int ch = id & (CH - 1), pair = id / CH;
             const int o = pair & ((1 << q) - 1), c = pair >> q;
             const int lrow = ((2 * c) << q) + o;
-            const int shift = (x << q) + o;
+            const int ru = lrow - o + (1 << q);   // first staged row of U's block (L's: lrow - o)
+            const int shift = skew ? o + AL + ((x * ru) & (AL - 1)) - ((x * (lrow - o)) & (AL - 1)) : o;
             int uch = ch + shift / CPC;
             uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
             const uint4 l = smv[lrow * CH + ch];
@@ -488,6 +497,7 @@ namespace dd {
 namespace {
 
 const double kTreeDm = 4.148808e3;   // k_DM in MHz^2 pc^-1 cm^3 s
+constexpr int64_t kTreeMargin = 128;  // zero columns in front of every row between the passes
 
 int log2_exact(int v)
 {
@@ -512,11 +522,14 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
             q = std::min(q, t->tune[1]);
         // the first pass adds in 8-bit lanes when its sums stay below 256 (2-bit samples: any first pass; 4-bit: up to 4 steps)
         auto lanes = [&](int qq) { return (i0 == 0 && t->tune[4] != 16 && vmax * (1 << qq) <= 255) ? 8 : 16; };
-        // later passes: the overlap of neighbouring tiles (the largest delay of the pass) at most half the columns staged
-        // (the first pass: whatever leaves a tile; 63 of 512 or 1024 columns for six steps)
+        // the overlap of neighbouring tiles: the first pass applies delays up to 2^q - 1; later passes stage their rows skewed
+        // (dd_tree_pass) and keep 2^q - 1 plus two 16-byte granules of the staged rows per step.  Later passes take as many
+        // steps as keep it within a quarter of the columns staged.
+        const int al = (i0 > 0 && t->passes.back().lane_bits == 8) ? 16 : 8;
+        auto overlap = [&](int qq) { return ((1 << qq) - 1) + (i0 > 0 ? 2 * al * qq : 0); };
         for (; q > 1; --q) {
-            const int64_t halo = (int64_t(1) << i0) * ((1 << q) - 1), cols = pass_cols(q, items, lanes(q));
-            if ((i0 == 0 || t->tune[1] > 0 || 2 * halo <= cols) && halo + 64 <= cols)
+            const int cols = pass_cols(q, items, lanes(q));
+            if ((i0 == 0 || t->tune[1] > 0 || 4 * overlap(q) <= cols) && overlap(q) + 64 <= cols)
                 break;
         }
         TreePass ps;
@@ -525,7 +538,7 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
         ps.packed = i0 == 0 || t->passes.back().lane_bits == 8;
         ps.in_bits = i0 == 0 ? t->nbits : 8;
         ps.cols = pass_cols(q, items, ps.lane_bits);
-        ps.halo = static_cast<int>((int64_t(1) << i0) * ((1 << q) - 1));
+        ps.halo = overlap(q);
         ps.tt = (ps.cols - ps.halo) & ~63;
         if (ps.tt < 64)
             return false;
@@ -534,14 +547,17 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
     }
     if (t->passes.size() > 6)
         return false;
-    // columns every pass has to produce, backwards
+    // columns every pass has to produce, backwards: a later pass stages row r of butterfly x from column t0 + x r on
+    // (x r < the rows of a block after the pass), cols columns of it
     int64_t need = t_out;
     for (int p = static_cast<int>(t->passes.size()) - 1; p >= 0; --p) {
         TreePass &ps = t->passes[p];
         ps.out_cols = need;
-        ps.ntiles = (need + ps.tt - 1) / ps.tt;   // of the butterfly with the largest delays (tt columns per tile); the others need fewer
-        t->pitch[p] = (need + ps.cols + 32 + 63) & ~int64_t(63);   // whole tiles are stored; stage 2 reads up to 47 columns past its last sample
-        need = (need + ps.cols + 63) & ~int64_t(63);   // the last tile of a butterfly starts below `need` and stages cols columns
+        ps.ntiles = (need + ps.tt - 1) / ps.tt;
+        // whole tiles are stored; stage 2 reads up to 47 columns past its last sample; kTreeMargin zero columns in front
+        // (a skewed row starts up to 16 columns per step before t0)
+        t->pitch[p] = (kTreeMargin + ps.ntiles * ps.tt + 64 + 63) & ~int64_t(63);
+        need = (ps.ntiles * ps.tt + (ps.i0 > 0 ? (int64_t(1) << (ps.i0 + ps.q)) : 0) + ps.cols + 63) & ~int64_t(63);
     }
     return true;
 }
@@ -867,15 +883,19 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         const TreePass &ps = tree->passes[p];
         const bool first = p == 0, last = p + 1 == np && !stage2;
         TreePassParams kp{};
-        kp.in = first ? static_cast<const uint8_t *>(in_ptr) : static_cast<const uint8_t *>(tree->buf[(p - 1) & 1]);
-        kp.in_stride = first ? in_stride : tree->pitch[p - 1] * (tree->passes[p - 1].lane_bits / 8);
-        kp.out = last ? static_cast<uint8_t *>(out_ptr) : static_cast<uint8_t *>(tree->buf[p & 1]);
-        kp.out_stride = last ? out_pitch_bytes : tree->pitch[p] * (ps.lane_bits / 8);
+        // (rows between the passes: column 0 lies kTreeMargin columns into the row)
+        const int in_lb = first ? 0 : tree->passes[p - 1].lane_bits / 8, out_lb = ps.lane_bits / 8;
+        kp.in = first ? static_cast<const uint8_t *>(in_ptr) : static_cast<const uint8_t *>(tree->buf[(p - 1) & 1]) + kTreeMargin * in_lb;
+        kp.in_stride = first ? in_stride : tree->pitch[p - 1] * in_lb;
+        kp.in_bytes = first ? in_stride : (tree->pitch[p - 1] - kTreeMargin) * in_lb;
+        kp.out = last ? static_cast<uint8_t *>(out_ptr) : static_cast<uint8_t *>(tree->buf[p & 1]) + kTreeMargin * out_lb;
+        kp.out_stride = last ? out_pitch_bytes : tree->pitch[p] * out_lb;
         kp.out_cols = last ? nsamps : ps.out_cols;
         kp.nbits = ps.in_bits;
         kp.out_code = out_nbits;
         kp.vec_ok = rows16 ? 1 : 0;
         kp.i0 = ps.i0;
+        kp.tt = ps.tt;
         kp.row_map = first ? static_cast<const int32_t *>(tree->d_row_map) : nullptr;
         const int64_t groups = tree->nchans >> ps.q;
         const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
@@ -890,7 +910,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         const dim3 grid(static_cast<unsigned>((nsamps + TR2_THREADS * cpt - 1) / (TR2_THREADS * cpt)), static_cast<unsigned>(tree->ndm));
         auto s2 = lb == 8 ? dd_tree_stage2<8> : dd_tree_stage2<16>;
         s2<<<grid, TR2_THREADS, static_cast<size_t>(tree->ns) * sizeof(int2), st>>>(
-            static_cast<const uint8_t *>(tree->buf[(np - 1) & 1]), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
+            static_cast<const uint8_t *>(tree->buf[(np - 1) & 1]) + kTreeMargin * (lb / 8), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
             static_cast<uint8_t *>(out_ptr), out_pitch_bytes, nsamps, out_nbits, rows16 ? 1 : 0);
         if ((e = cudaGetLastError()) != cudaSuccess)
             return report_cuda_error(e, "dd_tree_execute stage 2");
