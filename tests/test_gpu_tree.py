@@ -185,3 +185,38 @@ def test_frequency_padded_tree(nbits):
             assert t.info()["last_launches"] == t.info()["passes"]
         ref = oracle.padded_tree(packed[0].numpy(), nbits, nsamps, f_top, df)
         _assert_equal(got, oracle.cast_out(ref, kind), f"padded tree {nchans} -> {npad} rows, {nbits}-bit {kind}")
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_tree_time_slab_shards_reassemble(world):
+    # PAPER.md:456 ("time-division multiplexing"): the tree is invariant under time shifts, so ranks take time
+    # slabs with a halo of the samples the trails reach into (N - 1; max Dt'' + N' - 1 for the piecewise method), no
+    # exchange.  One "rank" after the other on one GPU: input pointer advanced to the slab's first byte, nsamps = the slab's
+    # length; the slabs side by side are the whole transform (ragged last slab).
+    from paper_1201_5380_b200 import multi
+    st = torch.cuda.current_stream()
+    n, nbits, nsamps = 256, 2, 5 * 1024 + 700
+    cfg = _band(nbits, n, nsamps)
+    for piecewise in (False, True):
+        with (dd.Tree(n, 32, nbits) if piecewise else dd.Tree(n, n, nbits)) as t:
+            dms = np.linspace(0.0, 45.0, 19)
+            if piecewise:
+                t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
+            halo = t.required_samples(nsamps) - nsamps
+            packed, stride = W.gen_packed(cfg, halo, None)
+            ref = (oracle.piecewise_tree(packed[0].numpy(), nbits, nsamps, n, cfg.dt, cfg.f_top, cfg.df, dms, 32) if piecewise
+                   else oracle.tree(packed[0].numpy(), nbits, nsamps))
+            dev = torch.cat([packed[0], torch.zeros((1, stride), dtype=torch.uint8)]).cuda()   # (rows readable out to in_stride)
+            parts, covered = [], 0
+            for rank in range(world):
+                t_lo, t_hi, in_lo, in_hi = multi.shard_time_slabs(nsamps, world, rank, halo)
+                assert t_lo == covered and in_lo == t_lo and in_hi == t_hi + halo and (t_lo * nbits) % 128 == 0
+                covered = t_hi
+                if t_hi == t_lo:
+                    continue
+                out = torch.full((ref.shape[0], t_hi - t_lo), -1, dtype=torch.int32, device="cuda")
+                t.execute(t_hi - t_lo, dev.data_ptr() + t_lo * nbits // 8, stride, out, _CODE["u32"], st)
+                torch.cuda.synchronize()
+                parts.append(out.cpu().numpy().view(np.uint32))
+            assert covered == nsamps
+            _assert_equal(np.concatenate(parts, axis=1), oracle.cast_out(ref, "u32"), f"time slabs, piecewise={piecewise}, world {world}")
