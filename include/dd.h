@@ -335,13 +335,12 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *                  rows between the passes (8- or 16-bit, at most 4 nchans (nsamps + sb_nchans) bytes; with a DM list they
  *                  include the stage-1 output), later calls only enqueue kernels.  DD_ERR_CUDA without a device.
  * dd_tree_set_tuning   test knob: key 1 = steps fused by the first pass (1 .. 6, 0 = default), key 2 = steps fused by
- *                  later passes (1 .. 6, 0 = as many as keep the overlap of neighbouring tiles below half a tile),
+ *                  later passes (1 .. 6, 0 = as many as keep the overlap of neighbouring tiles within a quarter of a tile),
  *                  key 3 / 4 = items per thread of the first / of later passes (4: two CTAs per SM, 8: one; 0 = default),
  *                  key 5 = 16: the first pass adds in 16-bit lanes even where 8-bit lanes hold its sums (0 = default).
  *                  Takes effect at the next execute.
  * dd_tree_get_info info[0] = passes, info[1] = kernels enqueued by the last execute, info[2] = device bytes held,
- *                  info[3 + 2 p] / info[4 + 2 p] = steps fused by pass p / fewest columns a tile of it stores (p < 6);
- *                  int64 x 16.
+ *                  info[3 + 2 p] / info[4 + 2 p] = steps fused by pass p / columns a tile of it stores (p < 6); int64 x 16.
  */
 typedef struct dd_tree_s *dd_tree;
 dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits);
