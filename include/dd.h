@@ -394,10 +394,13 @@ dd_status dd_set_kernel_variant(dd_plan plan, int variant);
  *          DD_TUNE_TILES_PER_CTA: consecutive time tiles a CTA of the short bit-plane kernel walks (plans with few channels
  *            per group: step 2 of the sub-band method, small transforms); 0 = as many as leave 8 waves of CTAs, at most 8.
  *            Takes effect at the next dd_execute.
+ *          DD_TUNE_HOST_SLAB: output samples per time slab of dd_execute_host (rounded up to whole time tiles); 0 = 2^15.
+ *            Takes effect at the next dd_execute_host.
  *   value  >= 0.
  * DD_ERR_INVALID_ARG for an unknown key or a negative value.
  */
-enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3, DD_TUNE_PAIR_TILES = 4, DD_TUNE_TILES_PER_CTA = 5 };
+enum { DD_TUNE_SUBBAND_GPC = 1, DD_TUNE_GROUP_SIZE = 2, DD_TUNE_GROUPS_PER_STAGE = 3, DD_TUNE_PAIR_TILES = 4, DD_TUNE_TILES_PER_CTA = 5,
+       DD_TUNE_HOST_SLAB = 6 };
 dd_status dd_set_tuning(dd_plan plan, int key, int value);
 
 /*

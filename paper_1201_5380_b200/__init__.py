@@ -22,7 +22,7 @@ __all__ = [
     "dd_set_batch", "dd_set_killmask", "dd_set_output_stride", "dd_set_input_max", "dd_set_subband", "dd_get_subband_extent", "dd_get_subband_tables",
     "dd_time_scrunch", "dd_execute", "dd_execute_static", "DD_STATIC_WORKSPACE_BYTES", "dd_execute_host", "dd_get_launch_info", "dd_int_add_peak",
     "dd_set_kernel_variant", "dd_set_tuning", "DD_TUNE_SUBBAND_GPC", "DD_TUNE_GROUP_SIZE", "DD_TUNE_GROUPS_PER_STAGE",
-    "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
+    "DD_TUNE_PAIR_TILES", "DD_TUNE_TILES_PER_CTA", "DD_TUNE_HOST_SLAB", "dd_set_workspace_limit", "dd_get_workspace_bytes", "dd_profile_enable", "dd_profile_read", "dd_strerror", "dd_last_cuda_error", "Plan",
     "dd_scrunch_create", "dd_scrunch_set_killmask", "dd_scrunch_levels", "dd_scrunch_level_info", "dd_scrunch_required_bytes", "dd_scrunch_execute",
     "dd_scrunch_destroy", "ScrunchSet",
     "dd_tree_create", "dd_tree_create_padded", "dd_tree_get_padding", "dd_tree_set_dm_list", "dd_tree_get_tables", "dd_tree_get_delays", "dd_tree_required_samples", "dd_tree_execute",
@@ -294,6 +294,7 @@ def dd_set_kernel_variant(plan: int, variant: int) -> None:
 
 
 DD_TUNE_SUBBAND_GPC, DD_TUNE_GROUP_SIZE, DD_TUNE_GROUPS_PER_STAGE, DD_TUNE_PAIR_TILES, DD_TUNE_TILES_PER_CTA = 1, 2, 3, 4, 5
+DD_TUNE_HOST_SLAB = 6
 
 
 def dd_set_tuning(plan: int, key: int, value: int) -> None:

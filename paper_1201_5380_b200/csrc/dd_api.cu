@@ -33,7 +33,7 @@ struct HostStage {
     uint8_t *d_out[2] = {nullptr, nullptr};
     size_t out_bytes = 0;
     cudaStream_t copy_in = nullptr, compute = nullptr, copy_out[2] = {nullptr, nullptr};
-    cudaEvent_t in_ready = nullptr, done[2] = {nullptr, nullptr}, drained[2] = {nullptr, nullptr};
+    cudaEvent_t in_ready = nullptr, in_rest = nullptr, done[2] = {nullptr, nullptr}, drained[2] = {nullptr, nullptr};
     bool streams = false;
 };
 
@@ -53,6 +53,8 @@ static void free_stage(HostStage *s)
             cudaEventDestroy(s->drained[i]);
         }
         cudaEventDestroy(s->in_ready);
+        if (s->in_rest)
+            cudaEventDestroy(s->in_rest);
     }
     delete s;
 }
@@ -756,7 +758,7 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     // Time slabs: the input slab of output samples [s0, s0+len) is rows [s0, s0+len+max_delay); the slab
     // length is a multiple of the tile so that slab starts stay 16-byte aligned in the packed rows.
     const int64_t TB = plan->var.TB;
-    int64_t slab = ((int64_t(1) << 17) + TB - 1) / TB * TB;
+    int64_t slab = ((plan->host_slab > 0 ? static_cast<int64_t>(plan->host_slab) : (int64_t(1) << 15)) + TB - 1) / TB * TB;
     if (slab > (nsamps + TB - 1) / TB * TB || plan->sb_nchans > 0)   // the sub-band method runs as one slab (its
         slab = (nsamps + TB - 1) / TB * TB;                          // intermediate series span the whole call)
     const int64_t nslabs = (nsamps + slab - 1) / slab;
@@ -776,6 +778,7 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
             (e = cudaStreamCreateWithFlags(&S->copy_out[1], cudaStreamNonBlocking)) != cudaSuccess)
             return cuda_fail(e, "cudaStreamCreate");
         cudaEventCreateWithFlags(&S->in_ready, cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&S->in_rest, cudaEventDisableTiming);
         for (int i = 0; i < 2; ++i) {
             cudaEventCreateWithFlags(&S->done[i], cudaEventDisableTiming);
             cudaEventCreateWithFlags(&S->drained[i], cudaEventDisableTiming);
@@ -802,10 +805,34 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
         S->out_bytes = out_slab_bytes;
     }
 
-    // input: one H2D copy of the whole packed filterbank (it is 5-30x smaller than the output)
-    if ((e = cudaMemcpyAsync(S->d_in, in_host, in_bytes, cudaMemcpyHostToDevice, S->copy_in)) != cudaSuccess)
-        return cuda_fail(e, "cudaMemcpyAsync(in)");
-    cudaEventRecord(S->in_ready, S->copy_in);
+    // input (5-30x smaller than the output): first the bytes of every row that the first slab reads, so that its kernels --
+    // and, behind them, the first copy out, which is what the call is bound by -- start early; then the rest of the rows
+    const int64_t nrows_all = static_cast<int64_t>(nbeams) * plan->nchans;
+    const bool rows_dense = nbeams == 1 || in_beam == static_cast<int64_t>(plan->nchans) * in_stride;
+    // (the kernels of a slab of n tiles read n - 1 tiles + max_span_end samples of every row, in whole 16-byte groups)
+    const int64_t reach = std::max<int64_t>(plan->max_span_end, TB + plan->max_delay);
+    int64_t head = ((slab - TB + reach + 256) * plan->nbits / 8 + 15) / 16 * 16;
+    if (!rows_dense || nslabs < 2 || head >= in_stride)
+        head = 0;   // (one copy of everything)
+    if (head > 0) {
+        if ((e = cudaMemcpy2DAsync(S->d_in, static_cast<size_t>(in_stride), in_host, static_cast<size_t>(in_stride),
+                                   static_cast<size_t>(head), static_cast<size_t>(nrows_all), cudaMemcpyHostToDevice,
+                                   S->copy_in)) != cudaSuccess)
+            return cuda_fail(e, "cudaMemcpy2DAsync(in, head)");
+        cudaEventRecord(S->in_ready, S->copy_in);
+        if ((e = cudaMemcpy2DAsync(S->d_in + head, static_cast<size_t>(in_stride), static_cast<const uint8_t *>(in_host) + head,
+                                   static_cast<size_t>(in_stride), static_cast<size_t>(in_stride - head),
+                                   static_cast<size_t>(nrows_all), cudaMemcpyHostToDevice, S->copy_in)) != cudaSuccess) {
+            cudaStreamSynchronize(S->copy_in);
+            return cuda_fail(e, "cudaMemcpy2DAsync(in, rest)");
+        }
+        cudaEventRecord(S->in_rest, S->copy_in);
+    } else {
+        if ((e = cudaMemcpyAsync(S->d_in, in_host, in_bytes, cudaMemcpyHostToDevice, S->copy_in)) != cudaSuccess)
+            return cuda_fail(e, "cudaMemcpyAsync(in)");
+        cudaEventRecord(S->in_ready, S->copy_in);
+        cudaEventRecord(S->in_rest, S->copy_in);
+    }
     cudaStreamWaitEvent(S->compute, S->in_ready, 0);
 
     // an error below must not return while copies into the caller's buffers are still in flight
@@ -821,6 +848,8 @@ dd_status dd_execute_host(dd_plan plan, int64_t nsamps, const void *in_host, int
     for (int64_t k = 0; k < nslabs; ++k) {
         const int b = static_cast<int>(k & 1);
         const int64_t s0 = k * slab, len = (s0 + slab <= nsamps) ? slab : nsamps - s0;
+        if (k == 1)
+            cudaStreamWaitEvent(S->compute, S->in_rest, 0);      // the rest of the input rows
         if (k >= 2)
             cudaStreamWaitEvent(S->compute, S->drained[b], 0);   // slab buffer b has been copied out
         const uint8_t *in_slab = S->d_in + (s0 * plan->nbits) / 8;
@@ -954,6 +983,9 @@ dd_status dd_set_tuning(dd_plan plan, int key, int value)
         return DD_OK;
     case DD_TUNE_PAIR_TILES:
         plan->pair_tiles = value;
+        return DD_OK;
+    case DD_TUNE_HOST_SLAB:
+        plan->host_slab = value;
         return DD_OK;
     case DD_TUNE_TILES_PER_CTA:
         plan->bp_tpc = value;

@@ -143,6 +143,7 @@ struct dd_plan_s {
     int gr_stage_slots = 0;               // stage slots per DM block in span / rel (the largest stage count of any block); every
                                           // block's span list starts with a header entry {stages, groups of the first stage, -, -}
     int bp_tpc = 0;                       // dd_set_tuning: time tiles per CTA of the short bit-plane kernel (0 = chosen by the launcher)
+    int host_slab = 0;                    // dd_set_tuning: output samples per time slab of dd_execute_host (0 = the default)
     int sb_gpc = 0;                       // dd_set_tuning: sub-bands per CTA of sub-band step 1 (0 = chosen by the library)
     int in_planes = 0;     // > 0: no input sample reaches 2^in_planes (sub-band step 2: sums of N'nu samples); 0 = nbits
     bool final32 = false;  // sums need 32-bit accumulators (nchans*(2^nbits-1) > 65535)

@@ -281,9 +281,11 @@ def test_tuning_and_workspace_knobs_host_side():
     assert L.dd_get_workspace_bytes(None) == -1
     cfg = W.CONFIGS[5]
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
-        for key, value in ((0, 1), (99, 1), (dd.DD_TUNE_GROUP_SIZE, 3), (dd.DD_TUNE_GROUP_SIZE, -1), (dd.DD_TUNE_PAIR_TILES, -2)):
+        for key, value in ((0, 1), (99, 1), (dd.DD_TUNE_GROUP_SIZE, 3), (dd.DD_TUNE_GROUP_SIZE, -1), (dd.DD_TUNE_PAIR_TILES, -2),
+                           (dd.DD_TUNE_HOST_SLAB, -1), (7, 1)):
             assert L.dd_set_tuning(p.handle, key, value) == -2, (key, value)
         assert L.dd_set_workspace_limit(p.handle, -1) == -2
+        assert L.dd_set_tuning(p.handle, dd.DD_TUNE_HOST_SLAB, 1 << 16) == 0 and L.dd_set_tuning(p.handle, dd.DD_TUNE_HOST_SLAB, 0) == 0
         assert p.workspace_bytes == 0                       # nothing is allocated before the first dd_execute
         p.set_dm_list(cfg.dm_list())
         info = p.launch_info()

@@ -747,9 +747,41 @@ def test_execute_host_bitplane_variant_two_slabs():
     out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
+        p.set_tuning(dd.DD_TUNE_HOST_SLAB, 1 << 17)
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
         assert p.launch_info()["last_launches"] == 4
+        assert np.array_equal(out.numpy(), ref)
+        # the default slabs (2^15 samples rounded up to 7 tiles of 5120: four slabs); the bytes of every row the first
+        # slab reads are copied in first, the rest of the rows behind them
+        out.zero_()
+        p.set_tuning(dd.DD_TUNE_HOST_SLAB, 0)
+        p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
+        assert p.launch_info()["last_launches"] == 8
     assert np.array_equal(out.numpy(), ref)
+
+
+@pytest.mark.parametrize("nbits,dense", [(2, True), (4, False), (8, True)])
+def test_execute_host_many_slabs_fresh_staging(nbits, dense):
+    # first call of a fresh plan (its staging buffer has never held the input): slabs of one and of three tiles, so that
+    # the first slab's kernels run while most of the rows are still on their way; two beams whose rows lie back to back
+    # (the head of all rows is one strided copy) or apart (one copy of everything); the library's default kernel
+    full = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]]
+    cfg = full.reduced(nsamps=60000, ndm=21, nchans=160, nbeams=2)
+    tab = _oracle_table(cfg)
+    packed, stride = W.gen_packed(cfg, int(tab.max()))
+    gap = 0 if dense else 4 * stride
+    h_in = torch.zeros((cfg.nbeams, cfg.nchans * stride + gap), dtype=torch.uint8).pin_memory()
+    h_in[:, :cfg.nchans * stride] = packed.reshape(cfg.nbeams, -1)
+    for slab in (1, 15000):
+        h_out = torch.full((cfg.nbeams, cfg.ndm, cfg.nsamps), -1, dtype=torch.int32).pin_memory()
+        with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits) as p:
+            p.set_dm_list(cfg.dm_list())
+            p.set_batch(cfg.nbeams, h_in.stride(0), h_out.stride(0) * 4)
+            p.set_tuning(dd.DD_TUNE_HOST_SLAB, slab)
+            p.execute_host(cfg.nsamps, h_in, stride, h_out, -32)
+        for b in range(cfg.nbeams):
+            ref = oracle.dedisperse(packed[b].numpy(), cfg.nbits, cfg.nsamps, tab)
+            assert np.array_equal(h_out[b].numpy().view(np.uint32), ref), (nbits, dense, slab, b)
 
 
 def test_execute_host_bitplane_8bit_two_slabs():
@@ -761,6 +793,7 @@ def test_execute_host_bitplane_8bit_two_slabs():
     out = torch.zeros((cfg.ndm, cfg.nsamps), dtype=torch.float32).pin_memory()
     with dd.Plan(cfg.nchans, cfg.dt, cfg.f_top, cfg.df, cfg.nbits, variant=3) as p:
         p.set_dm_list(cfg.dm_list())
+        p.set_tuning(dd.DD_TUNE_HOST_SLAB, 1 << 17)
         p.execute_host(cfg.nsamps, packed[0].contiguous().pin_memory(), stride, out, 32)
         assert p.launch_info()["last_launches"] == 4
     assert np.array_equal(out.numpy(), ref)
