@@ -50,6 +50,7 @@ struct TreePassParams {
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
     int32_t tt;            // columns a tile stores (multiple of 64)
+    int32_t fuse2;         // first pass: steps 0 and 1 are made while the rows are staged (the step loop starts at 2)
     const int32_t *row_map;   // first pass of a frequency-padded tree: input row of every tree row, -1 = blank; else NULL
 };
 
@@ -134,6 +135,16 @@ __device__ __forceinline__ uint4 tree_unpack_chunk(const uint4 v, int nb, int kk
     return make_uint4(o[0], o[1], o[2], o[3]);
 }
 
+// words 0 .. 3 of the lane stream l[0..7] taken S lanes further on (S = 1, 2, 3: the delays of the first two steps)
+template <int LB, int S>
+__device__ __forceinline__ void tree_lanes_from(const uint32_t (&l)[8], uint32_t (&o)[4])
+{
+    constexpr int WO = (S * LB) / 32, AM = (S * LB) % 32;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        o[k] = AM == 0 ? l[k + WO] : __funnelshift_r(l[k + WO], l[k + WO + 1], AM);
+}
+
 // One pass: steps i0 .. i0 + Q - 1 for one butterfly (R = 2^Q rows) and one time tile.
 //   group g = k 2^i0 + x: butterfly x of block k (blocks of B = R 2^i0 rows after the pass)
 //   staged row b' (level i0) = global row k B + b' 2^i0 + x;   stored row o' = global row k B + x R + o'
@@ -170,7 +181,71 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     auto first_col = [&](int r) -> int64_t { return skew ? t0 + ((x * r) & ~(AL - 1)) - AL * __popc(r) : t0; };
 
     // ---- stage R rows x C columns
-    if constexpr (PACKED) {
+    if (PACKED && p.fuse2) {
+        // FIRST TWO STEPS IN REGISTERS.  Their delays are 0 .. 3 samples (eq. 8 for four channels: 0000 / 0011 / 0112 /
+        // 0123), so a thread that unpacks one 16-byte chunk of lanes of four adjacent rows, and the three lanes after it,
+        // can write the four rows of level 2 straight away: two of the pass's steps never go through shared memory.
+        const int nb = p.nbits;
+        const int wpc = CPC * nb / 32;                      // packed words per chunk: 1 or 2 (the host checks)
+        for (int id = tid; id < (R / 4) * CH; id += TR_THREADS) {
+            const int j = id / CH, ch = id & (CH - 1);
+            const int64_t off = (t0 + static_cast<int64_t>(ch) * CPC) * nb / 8;   // a multiple of 4
+            uint32_t w[4][3];   // all loads first, then row by row (few registers live: two CTAs per SM leave 64)
+#pragma unroll
+            for (int rr = 0; rr < 4; ++rr) {
+                int64_t row = row0 + 4 * j + rr;
+                if (p.row_map)
+                    row = __ldg(&p.row_map[row]);
+                const uint8_t *src = p.in + row * p.in_stride + off;
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    w[rr][k] = (row >= 0 && k <= wpc && off + 4 * (k + 1) <= p.in_bytes) ? __ldg(reinterpret_cast<const uint32_t *>(src) + k) : 0u;
+            }
+            uint32_t o[4][4];
+            auto lanes_of = [&](int rr, uint32_t (&l)[8]) {   // the chunk, then the lanes that follow it (three are used)
+                const uint4 a = tree_unpack_chunk<LB>(make_uint4(w[rr][0], w[rr][1], 0u, 0u), nb, 0);
+                const uint4 b = tree_unpack_chunk<LB>(make_uint4(wpc == 1 ? w[rr][1] : w[rr][2], 0u, 0u, 0u), nb, 0);
+                l[0] = a.x, l[1] = a.y, l[2] = a.z, l[3] = a.w, l[4] = b.x, l[5] = b.y, l[6] = b.z, l[7] = b.w;
+            };
+            {   // row 0: delay 0 in all four
+                uint32_t l[8];
+                lanes_of(0, l);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    o[0][k] = o[1][k] = o[2][k] = o[3][k] = l[k];
+            }
+            {   // row 1: delays 0 0 1 1
+                uint32_t l[8], s1[4];
+                lanes_of(1, l);
+                tree_lanes_from<LB, 1>(l, s1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    o[0][k] += l[k], o[1][k] += l[k], o[2][k] += s1[k], o[3][k] += s1[k];
+            }
+            {   // row 2: delays 0 1 1 2
+                uint32_t l[8], s1[4], s2[4];
+                lanes_of(2, l);
+                tree_lanes_from<LB, 1>(l, s1);
+                tree_lanes_from<LB, 2>(l, s2);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    o[0][k] += l[k], o[1][k] += s1[k], o[2][k] += s1[k], o[3][k] += s2[k];
+            }
+            {   // row 3: delays 0 1 2 3
+                uint32_t l[8], s1[4], s2[4], s3[4];
+                lanes_of(3, l);
+                tree_lanes_from<LB, 1>(l, s1);
+                tree_lanes_from<LB, 2>(l, s2);
+                tree_lanes_from<LB, 3>(l, s3);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    o[0][k] += l[k], o[1][k] += s1[k], o[2][k] += s2[k], o[3][k] += s3[k];
+            }
+#pragma unroll
+            for (int rr = 0; rr < 4; ++rr)
+                smv[(4 * j + rr) * CH + ch] = make_uint4(o[rr][0], o[rr][1], o[rr][2], o[rr][3]);
+        }
+    } else if constexpr (PACKED) {
         // 16 packed bytes hold SUB chunks; they are taken in an order rotated by the lane so that the 16-byte stores of a
         // quarter warp fall into distinct banks.  Up to four loads in flight per thread.
         const int nb = p.nbits;
@@ -238,6 +313,8 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     // ---- Q steps in place
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
+        if (PACKED && p.fuse2 && q < 2)
+            continue;
         uint32_t s0[ITEMS][4], s1[ITEMS][4];
         __syncthreads();
 #pragma unroll
@@ -476,8 +553,8 @@ struct dd_tree_s {
     int nchans_in = 0;                  // real channels (0: not padded)
     std::vector<int32_t> pad_pos;       // [nchans_in]
     void *d_row_map = nullptr;          // int32 [nchans]: input row or -1
-    int tune[5] = {0, 0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later
-                                     // passes, lanes of the first pass (16: never 8-bit lanes)
+    int tune[6] = {0, 0, 0, 0, 0, 0};   // steps of the first pass / of later passes, items per thread of the first pass / of later
+                                     // passes, lanes of the first pass (16: never 8-bit lanes), 1: no steps fused into staging
     // stage 2 (piecewise linear tree)
     int ndm = 0, ns = 0;
     std::vector<int32_t> dprime, dt2;   // [ndm][ns]
@@ -768,7 +845,7 @@ dd_status dd_tree_set_tuning(dd_tree tree, int key, int value)
 {
     if (!tree)
         return DD_ERR_NULL;
-    if (key < 1 || key > 5 || value < 0 || (key <= 2 && value > 6) || ((key == 3 || key == 4) && value != 0 && value != 4 && value != 8) ||
+    if (key < 1 || key > 6 || value < 0 || (key == 6 && value > 1) || (key <= 2 && value > 6) || ((key == 3 || key == 4) && value != 0 && value != 4 && value != 8) ||
         (key == 5 && value != 0 && value != 16))
         return DD_ERR_INVALID_ARG;
     tree->tune[key - 1] = value;
@@ -899,6 +976,8 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.i0 = ps.i0;
         kp.tt = ps.tt;
         kp.row_map = first ? static_cast<const int32_t *>(tree->d_row_map) : nullptr;
+        // steps 0 and 1 while staging: the chunk of a thread must be whole packed words (not 2-bit samples in 16-bit lanes)
+        kp.fuse2 = (first && ps.q >= 2 && tree->tune[5] == 0 && (128 / ps.lane_bits) * tree->nbits >= 32) ? 1 : 0;
         const int64_t groups = tree->nchans >> ps.q;
         const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
         if ((e = launch_pass(kp, ps.q, ps.items, kind, last, groups, ps.ntiles, st)) != cudaSuccess)
