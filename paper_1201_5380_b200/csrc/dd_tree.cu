@@ -1,5 +1,6 @@
 // dd_tree.cu -- the tree dedispersion algorithm (eq. 7-15) and the piecewise linear tree method
-// (eq. 16-23); include/dd.h "dd_tree_*"; readings X1-X5 of DESIGN.md section 12.
+// (eq. 16-23), and the frequency-padded tree (eq. 25); include/dd.h "dd_tree_*";
+// readings X1-X8 of DESIGN.md section 12.
 //
 // The recursion of eq. 10-13, with Theta (eq. 14) and the shuffle Phi (eq. 15) written out for one step i (r = 2^i):
 // the rows of level i lie in blocks of r rows (the tree of r adjacent channels, row m' = trial d' = m' of that block);
@@ -12,8 +13,8 @@
 // integer pipes -- against N T (nbits / 8 + 4) bytes in and out: the tree is bound by memory, not by arithmetic, so the
 // steps are FUSED in shared memory.  The outputs {2^Q x + o', o' < 2^Q} of Q consecutive steps i0 .. i0 + Q - 1 depend on
 // exactly 2^Q rows of level i0 (row x of each of 2^Q neighbouring blocks): a radix-2^Q butterfly, as in an FFT.  One
-// kernel, dd_tree_pass<Q>, runs one such pass: a CTA stages R = 2^Q rows x C columns (16-bit lanes, 128 KB) of one
-// butterfly and one time tile, runs the Q steps in place (every thread keeps the 2 x 8 sums of its items in registers
+// kernel, dd_tree_pass<Q>, runs one such pass: a CTA stages R = 2^Q rows x C columns (8- or 16-bit lanes, 64 KB, two CTAs
+// per SM) of one butterfly and one time tile, runs the Q steps in place (every thread keeps the sums of its items in registers
 // across the barrier between reading and writing a level), and stores the first C - overlap columns.  The first pass
 // overlaps its neighbours by 2^Q - 1 columns; later passes stage their rows SKEWED by the delay the pass will apply to
 // them (see dd_tree_pass), which keeps the overlap at 2^Q - 1 plus two 16-byte granules per step instead of
@@ -21,6 +22,7 @@
 //
 // The piecewise linear tree (section 3.1.1) is the same passes over sub-bands of N' channels (the blocks simply stop
 // growing at N' rows: stage 1, eq. 18) followed by dd_tree_stage2 (eq. 22): out[d][t] = sum_n S_n[d'_n(d)][t + Dt''_n(d)].
+// The frequency-padded tree is one tree over a stretched band whose first pass reads its rows through a row map.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -489,7 +491,7 @@ struct TreePass {
     int lane_bits = 16;               // lanes of the pass in shared memory and of the rows it stores (unless it is the last)
     bool packed = true;               // input: packed samples (the first pass), or the 8-bit rows of the pass before; else 16-bit rows
     int in_bits = 0;                  // packed: bits per sample of the input
-    int cols = 0, halo = 0, tt = 0;   // columns staged / largest delay applied / fewest columns a tile stores
+    int cols = 0, halo = 0, tt = 0;   // columns staged / overlap of neighbouring tiles / columns a tile stores
     int64_t out_cols = 0;             // columns the pass produces for the current nsamps
     int64_t ntiles = 0;
 };
