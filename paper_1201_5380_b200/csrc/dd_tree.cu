@@ -52,7 +52,9 @@ struct TreePassParams {
     int32_t vec_ok;        // LAST: rows allow 16-byte stores
     int32_t i0;            // first step of the pass
     int32_t tt;            // columns a tile stores (multiple of 64)
-    int32_t fuse2;         // first pass: steps 0 and 1 are made while the rows are staged (the step loop starts at 2)
+    int32_t fuse2;         // packed rows: steps 0 and 1 are made while the rows are staged (the step loop starts at 2)
+    int32_t next_i0;       // not LAST: the pass that reads these rows starts at step next_i0 and takes next_q steps
+    int32_t next_q;        //   (0: no pass follows -- stage 2 reads the rows as they are)
     const int32_t *row_map;   // first pass of a frequency-padded tree: input row of every tree row, -1 = blank; else NULL
 };
 
@@ -170,17 +172,17 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     const int64_t row0 = (static_cast<int64_t>(k) << (p.i0 + Q));
     // SKEWED STAGING (passes after the first).  Step q reads U at t + x 2^q + o + b: the part x 2^q is the same for every
     // row of the step, and over the pass it adds up to x r for staged row r (bit q of r says whether the row is on the U
-    // side at step q).  So row r is staged from column t0 + x r instead of t0 -- rounded down to the 16-byte granule AL of
-    // the rows, and AL columns earlier per set bit of r so that what is left of every shift stays non-negative:
-    //     staged row r starts at column t0 + A(x r) - AL popcount(r),   A(v) = v - v mod AL,
-    //     shift at step q between L = block 2c and U = block 2c + 1:  o + b + AL + (x r_U) mod AL - (x r_L) mod AL.
-    // The overlap of neighbouring tiles falls from x (R - 1) columns (up to 960 of 2048 for the second pass of 1024
-    // channels) to at most (R - 1) + 2 AL Q, for every butterfly alike, and column t of a stored row is column t0 + t.
+    // side at step q).  So row r is staged from column t0 + x r instead of t0, and what is left of every shift is o + b --
+    // a later pass is the first pass again, for every butterfly alike: the overlap of neighbouring tiles falls from
+    // x (R - 1) columns (up to 960 of 2048 for the second pass of 1024 channels) to R - 1, and its first two steps can be
+    // made in registers too.  Staging copies whole 16-byte granules (AL columns of the rows read), so the PRODUCER of the
+    // rows stores each one (x r) mod AL columns early (its store phase below): column t of the row as stored is column
+    // t + (x r) mod AL of the row, and staging from the granule A(x r) = x r - (x r) mod AL on lands on column t0 + x r.
     const bool skew = p.i0 > 0;
     constexpr int AL = PACKED ? 16 : 8;   // columns per 16 bytes of the rows staged: 8-bit rows / 16-bit rows
     const int tt = p.tt;
     const int64_t t0 = static_cast<int64_t>(tile) * tt;
-    auto first_col = [&](int r) -> int64_t { return skew ? t0 + ((x * r) & ~(AL - 1)) - AL * __popc(r) : t0; };
+    auto first_col = [&](int r) -> int64_t { return skew ? t0 + ((x * r) & ~(AL - 1)) : t0; };
 
     // ---- stage R rows x C columns
     if (PACKED && p.fuse2) {
@@ -191,13 +193,13 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         const int wpc = CPC * nb / 32;                      // packed words per chunk: 1 or 2 (the host checks)
         for (int id = tid; id < (R / 4) * CH; id += TR_THREADS) {
             const int j = id / CH, ch = id & (CH - 1);
-            const int64_t off = (t0 + static_cast<int64_t>(ch) * CPC) * nb / 8;   // a multiple of 4
             uint32_t w[4][3];   // all loads first, then row by row (few registers live: two CTAs per SM leave 64)
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr) {
-                int64_t row = row0 + 4 * j + rr;
+                int64_t row = row0 + (static_cast<int64_t>(4 * j + rr) << p.i0) + x;
                 if (p.row_map)
                     row = __ldg(&p.row_map[row]);
+                const int64_t off = (first_col(4 * j + rr) + static_cast<int64_t>(ch) * CPC) * nb / 8;   // a multiple of 4
                 const uint8_t *src = p.in + row * p.in_stride + off;
 #pragma unroll
                 for (int k = 0; k < 3; ++k)
@@ -325,8 +327,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             const int ch = id & (CH - 1), pair = id / CH;
             const int o = pair & ((1 << q) - 1), c = pair >> q;
             const int lrow = ((2 * c) << q) + o;
-            const int ru = lrow - o + (1 << q);   // first staged row of U's block (L's: lrow - o)
-            const int shift = skew ? o + AL + ((x * ru) & (AL - 1)) - ((x * (lrow - o)) & (AL - 1)) : o;
+            const int shift = o;   // (+ b for the second sum; the x 2^q of a later pass is in the staging)
             int uch = ch + shift / CPC;
             uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
             const uint4 l = smv[lrow * CH + ch];
@@ -359,8 +360,24 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         uint8_t *orow = p.out + (row0 + (static_cast<int64_t>(x) << Q) + r) * p.out_stride;
         const uint4 *srow = smv + r * CH;
         if constexpr (!LAST) {
-            for (int ch = lane; ch < tt / CPC; ch += 32)
-                *reinterpret_cast<uint4 *>(orow + (t0 + ch * CPC) * (LB / 8)) = srow[ch];
+            // rows that a later pass stages skewed are stored (x' r') mod CPC columns early, x' and r' being the butterfly
+            // and the staged row this row is in that pass (see SKEWED STAGING): 0 .. CPC - 1 lanes, the same for the row
+            int early = 0;
+            if (p.next_q > 0) {
+                const int64_t grow = row0 + (static_cast<int64_t>(x) << Q) + r;
+                const int xn = static_cast<int>(grow & ((int64_t(1) << p.next_i0) - 1));
+                const int rn = static_cast<int>((grow >> p.next_i0) & ((1 << p.next_q) - 1));
+                early = (xn * rn) & (CPC - 1);
+            }
+            for (int ch = lane; ch < tt / CPC; ch += 32) {
+                uint4 v = srow[ch];
+                if (early) {
+                    uint32_t x0[4], x1[4];
+                    tree_windows<LB>(v, srow[ch + 1], early, x0, x1);
+                    v = make_uint4(x0[0], x0[1], x0[2], x0[3]);
+                }
+                *reinterpret_cast<uint4 *>(orow + (t0 + ch * CPC) * (LB / 8)) = v;
+            }
         } else if (p.out_code == DD_OUT_U16) {
             // 8 columns per thread: 16 bytes of 16-bit lanes as they are, or 8 bytes of 8-bit lanes widened
             for (int c8 = lane; c8 < tt / 8; c8 += 32) {
@@ -603,14 +620,12 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
             q = std::min(q, t->tune[1]);
         // the first pass adds in 8-bit lanes when its sums stay below 256 (2-bit samples: any first pass; 4-bit: up to 4 steps)
         auto lanes = [&](int qq) { return (i0 == 0 && t->tune[4] != 16 && vmax * (1 << qq) <= 255) ? 8 : 16; };
-        // the overlap of neighbouring tiles: the first pass applies delays up to 2^q - 1; later passes stage their rows skewed
-        // (dd_tree_pass) and keep 2^q - 1 plus two 16-byte granules of the staged rows per step.  Later passes take as many
-        // steps as keep it within a quarter of the columns staged.
-        const int al = (i0 > 0 && t->passes.back().lane_bits == 8) ? 16 : 8;
-        auto overlap = [&](int qq) { return ((1 << qq) - 1) + (i0 > 0 ? 2 * al * qq : 0); };
+        // the overlap of neighbouring tiles is 2^q - 1 columns in every pass (later passes stage their rows skewed:
+        // dd_tree_pass); later passes take as many steps as keep it within a quarter of the columns staged
+        auto overlap = [&](int qq) { return (1 << qq) - 1; };
         for (; q > 1; --q) {
             const int cols = pass_cols(q, items, lanes(q));
-            if ((i0 == 0 || t->tune[1] > 0 || 4 * overlap(q) <= cols) && overlap(q) + 64 <= cols)
+            if ((i0 == 0 || t->tune[1] > 0 || 4 * overlap(q) <= cols) && overlap(q) + 16 + 64 <= cols)
                 break;
         }
         TreePass ps;
@@ -620,14 +635,20 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
         ps.in_bits = i0 == 0 ? t->nbits : 8;
         ps.cols = pass_cols(q, items, ps.lane_bits);
         ps.halo = overlap(q);
-        ps.tt = (ps.cols - ps.halo) & ~63;
-        if (ps.tt < 64)
-            return false;
         t->passes.push_back(ps);
         i0 += q;
     }
     if (t->passes.size() > 6)
         return false;
+    for (size_t p = 0; p < t->passes.size(); ++p) {
+        TreePass &ps = t->passes[p];
+        // rows that a later pass stages skewed are stored up to one 16-byte granule of lanes early: that many more columns
+        // of the tile have to be complete
+        const int early = p + 1 < t->passes.size() ? 128 / ps.lane_bits - 1 : 0;
+        ps.tt = (ps.cols - ps.halo - early) & ~63;
+        if (ps.tt < 64)
+            return false;
+    }
     // columns every pass has to produce, backwards: a later pass stages row r of butterfly x from column t0 + x r on
     // (x r < the rows of a block after the pass), cols columns of it
     int64_t need = t_out;
@@ -635,8 +656,7 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
         TreePass &ps = t->passes[p];
         ps.out_cols = need;
         ps.ntiles = (need + ps.tt - 1) / ps.tt;
-        // whole tiles are stored; stage 2 reads up to 47 columns past its last sample; kTreeMargin zero columns in front
-        // (a skewed row starts up to 16 columns per step before t0)
+        // whole tiles are stored; stage 2 reads up to 47 columns past its last sample; kTreeMargin spare columns in front
         t->pitch[p] = (kTreeMargin + ps.ntiles * ps.tt + 64 + 63) & ~int64_t(63);
         need = (ps.ntiles * ps.tt + (ps.i0 > 0 ? (int64_t(1) << (ps.i0 + ps.q)) : 0) + ps.cols + 63) & ~int64_t(63);
     }
@@ -978,8 +998,11 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.i0 = ps.i0;
         kp.tt = ps.tt;
         kp.row_map = first ? static_cast<const int32_t *>(tree->d_row_map) : nullptr;
-        // steps 0 and 1 while staging: the chunk of a thread must be whole packed words (not 2-bit samples in 16-bit lanes)
-        kp.fuse2 = (first && ps.q >= 2 && tree->tune[5] == 0 && (128 / ps.lane_bits) * tree->nbits >= 32) ? 1 : 0;
+        // steps 0 and 1 while staging packed rows (the input, or 8-bit rows): the chunk of a thread must be whole packed words
+        // (not 2-bit samples in 16-bit lanes)
+        kp.fuse2 = (ps.packed && ps.q >= 2 && tree->tune[5] == 0 && (128 / ps.lane_bits) * ps.in_bits >= 32) ? 1 : 0;
+        kp.next_i0 = p + 1 < np ? tree->passes[p + 1].i0 : 0;
+        kp.next_q = p + 1 < np ? tree->passes[p + 1].q : 0;
         const int64_t groups = tree->nchans >> ps.q;
         const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
         if ((e = launch_pass(kp, ps.q, ps.items, kind, last, groups, ps.ntiles, st)) != cudaSuccess)

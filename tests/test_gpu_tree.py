@@ -56,8 +56,8 @@ def _tree_case(nbits, n, nsamps, kinds=("u32",), tuning=()):
 
 
 @pytest.mark.parametrize("nbits", [2, 4, 8])
-def test_tree_every_size_one_to_three_passes(nbits):
-    # N = 2 .. 64: one pass; 128 .. 2048: two; 4096: three.  Four tiles of the first pass and a ragged tail; a row
+def test_tree_every_size_one_and_two_passes(nbits):
+    # N = 2 .. 64: one pass; 128 .. 4096: two.  Four tiles of the first pass and a ragged tail; a row
     # length that allows 16-byte stores and one that does not; all output types
     for n in (2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096):
         if n * ((1 << nbits) - 1) > 65535:
@@ -67,22 +67,24 @@ def test_tree_every_size_one_to_three_passes(nbits):
             continue
         kinds = ("u16", "u32", "f32") if n in (4, 64, 256) else ("u32",)
         info = _tree_case(nbits, n, 4 * 448 + 77, kinds)
-        assert info["passes"] == (1 if n <= 64 else 2 if n <= 2048 else 3)
+        assert info["passes"] == (1 if n <= 64 else 2)
     _tree_case(nbits, 64, 2048, ("u16", "f32"))
     _tree_case(nbits, 64, 2048, ("u32",), tuning=((6, 1),))
     _tree_case(nbits, 256, 3000, ("u32",), tuning=((6, 1),))
 
 
 def test_tree_later_passes_over_several_tiles():
-    # 256 channels: the second pass (two steps) stores 8064 columns per tile; 40000 samples are five of its tiles
+    # 256 channels: the second pass (two steps) stores 8128 columns per tile; 40000 samples are five of its tiles
     info = _tree_case(2, 256, 40000)
     assert info["passes"] == 2 and info["tile"][1] < 10000
-    info = _tree_case(4, 1024, 7000)       # second pass (four steps, rows staged skewed): tiles of 1920 of 2048 columns
-    assert info["steps"] == [6, 4] and info["tile"] == [448, 1920]
+    info = _tree_case(4, 1024, 7000)       # second pass (four steps, rows staged skewed): tiles of 1984 of 2048 columns
+    assert info["steps"] == [6, 4] and info["tile"] == [384, 1984]
     info = _tree_case(4, 1024, 7000, tuning=((3, 8), (4, 8)))   # one CTA per SM: twice the columns
-    assert info["steps"] == [6, 4] and info["tile"] == [960, 3968]
-    info = _tree_case(2, 2048, 9000)       # 8-bit rows between the passes, five steps in the second: 832 of 1024 columns
-    assert info["steps"] == [6, 5] and info["tile"] == [960, 832]
+    assert info["steps"] == [6, 4] and info["tile"] == [896, 4032]
+    info = _tree_case(2, 2048, 9000)       # 8-bit rows between the passes, five steps in the second: 960 of 1024 columns
+    assert info["steps"] == [6, 5] and info["tile"] == [896, 960]
+    info = _tree_case(4, 4096, 3000, tuning=((1, 3), (2, 3)))   # four passes: every row is stored early for the next one
+    assert info["steps"] == [3, 3, 3, 3]
 
 
 @pytest.mark.parametrize("first", [1, 2, 3, 4, 5, 6])
@@ -157,7 +159,7 @@ def test_tree_full_size_survey_band_windows():
         info = t.info()
         torch.cuda.synchronize()
     assert info["steps"] == [6, 4]
-    starts = [0, 960 - 64, 1856 - 128, 100 * 1856 - 700, 273 * 960 - 512, nsamps - win]
+    starts = [0, 896 - 64, 1984 - 128, 100 * 1984 - 700, 273 * 896 - 512, nsamps - win]
     host = packed[0].numpy()
     for a in starts:
         assert a % 4 == 0
