@@ -17,8 +17,9 @@
 // per SM) of one butterfly and one time tile, runs the Q steps in place (every thread keeps the sums of its items in registers
 // across the barrier between reading and writing a level), and stores the first C - overlap columns.  The first pass
 // overlaps its neighbours by 2^Q - 1 columns; later passes stage their rows SKEWED by the delay the pass will apply to
-// them (see dd_tree_pass), which keeps the overlap at 2^Q - 1 plus two 16-byte granules per step instead of
-// 2^i0 (2^Q - 1).  1024 channels take two passes (Q = 6 in 8-bit lanes for 2-bit samples, then Q = 4).
+// them (see dd_tree_pass; the pass before stores every row early by what 16-byte staging cannot express), which keeps
+// their overlap at 2^Q - 1 as well instead of 2^i0 (2^Q - 1).  The first two steps of a pass over packed rows are made in
+// registers while staging.  1024 channels take two passes (Q = 6 in 8-bit lanes for 2-bit samples, then Q = 4).
 //
 // The piecewise linear tree (section 3.1.1) is the same passes over sub-bands of N' channels (the blocks simply stop
 // growing at N' rows: stage 1, eq. 18) followed by dd_tree_stage2 (eq. 22): out[d][t] = sum_n S_n[d'_n(d)][t + Dt''_n(d)].
