@@ -192,9 +192,9 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         // can write the four rows of level 2 straight away: two of the pass's steps never go through shared memory.
         const int nb = p.nbits;
         const int wpc = CPC * nb / 32;                      // packed words per chunk: 1 or 2 (the host checks)
-        for (int id = tid; id < (R / 4) * CH; id += TR_THREADS) {
+        // (the loads of two items first, then their sums row by row: few registers live -- two CTAs per SM leave 64)
+        auto load_item = [&](int id, uint32_t (&w)[4][3]) {
             const int j = id / CH, ch = id & (CH - 1);
-            uint32_t w[4][3];   // all loads first, then row by row (few registers live: two CTAs per SM leave 64)
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr) {
                 int64_t row = row0 + (static_cast<int64_t>(4 * j + rr) << p.i0) + x;
@@ -206,6 +206,9 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
                 for (int k = 0; k < 3; ++k)
                     w[rr][k] = (row >= 0 && k <= wpc && off + 4 * (k + 1) <= p.in_bytes) ? __ldg(reinterpret_cast<const uint32_t *>(src) + k) : 0u;
             }
+        };
+        auto make_item = [&](int id, const uint32_t (&w)[4][3]) {
+            const int j = id / CH, ch = id & (CH - 1);
             uint32_t o[4][4];
             auto lanes_of = [&](int rr, uint32_t (&l)[8]) {   // the chunk, then the lanes that follow it (three are used)
                 const uint4 a = tree_unpack_chunk<LB>(make_uint4(w[rr][0], w[rr][1], 0u, 0u), nb, 0);
@@ -249,6 +252,17 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr)
                 smv[(4 * j + rr) * CH + ch] = make_uint4(o[rr][0], o[rr][1], o[rr][2], o[rr][3]);
+        };
+        constexpr int NIT = (R / 4) * CH;
+        for (int id = tid; id < NIT; id += 2 * TR_THREADS) {
+            uint32_t wa[4][3], wb[4][3];
+            const bool two = id + TR_THREADS < NIT;
+            load_item(id, wa);
+            if (two)
+                load_item(id + TR_THREADS, wb);
+            make_item(id, wa);
+            if (two)
+                make_item(id + TR_THREADS, wb);
         }
     } else if constexpr (PACKED) {
         // 16 packed bytes hold SUB chunks; they are taken in an order rotated by the lane so that the 16-byte stores of a
