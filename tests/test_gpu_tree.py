@@ -3,6 +3,8 @@
 bit-exact.  The oracle follows eq. 10-15 / 18-23 step by step and is pinned by P16 / P17 (tests/test_oracle_pins.py).
 All inputs are seeded and synthetic (dd_workloads); no expected value comes from the CUDA path.
 """
+from dataclasses import replace
+
 import numpy as np
 import pytest
 import torch
@@ -225,3 +227,36 @@ def test_tree_time_slab_shards_reassemble(world):
                 parts.append(out.cpu().numpy().view(np.uint32))
             assert covered == nsamps
             _assert_equal(np.concatenate(parts, axis=1), oracle.cast_out(ref, "u32"), f"time slabs, piecewise={piecewise}, world {world}")
+
+
+def test_tree_execute_is_cuda_graph_capturable():
+    # after its first call for a size dd_tree_execute only enqueues kernels (no allocation, no synchronisation): a warmed-up
+    # call is captured into a CUDA graph and replayed on new input -- the tree (two passes) and the piecewise method
+    n, nbits, nsamps = 256, 2, 3000
+    cfg = _band(nbits, n, nsamps)
+    side = torch.cuda.Stream()
+    dms = np.linspace(0.0, 45.0, 11)
+    for piecewise in (False, True):
+        with (dd.Tree(n, 32, nbits) if piecewise else dd.Tree(n, n, nbits)) as t:
+            if piecewise:
+                t.set_dm_list(cfg.dt, cfg.f_top, cfg.df, dms)
+            halo = t.required_samples(nsamps) - nsamps
+            inputs = [W.gen_packed(replace(cfg, seed=cfg.seed + k), halo, None) for k in range(2)]
+            stride = inputs[0][1]
+            dev = inputs[0][0][0].cuda()
+            out = torch.zeros((len(dms) if piecewise else n, nsamps), dtype=torch.float32, device="cuda")
+            with torch.cuda.stream(side):
+                t.execute(nsamps, dev, stride, out, _CODE["f32"], side)      # warm-up: rows between the passes, tables
+            side.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                t.execute(nsamps, dev, stride, out, _CODE["f32"], torch.cuda.current_stream())
+            for k in (0, 1, 0):
+                dev.copy_(inputs[k][0][0].cuda())
+                out.zero_()
+                g.replay()
+                torch.cuda.synchronize()
+                host = inputs[k][0][0].numpy()
+                ref = (oracle.piecewise_tree(host, nbits, nsamps, n, cfg.dt, cfg.f_top, cfg.df, dms, 32) if piecewise
+                       else oracle.tree(host, nbits, nsamps))
+                _assert_equal(out.cpu().numpy(), oracle.cast_out(ref, "f32"), f"graph replay {k}, piecewise={piecewise}")
