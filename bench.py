@@ -384,6 +384,7 @@ def run_tree(args) -> None:
     info = tree.info()
     peaks = measured_peaks()
     alg_bytes = cfg.nchans * need * cfg.nbits / 8 + nrows * cfg.nsamps * 4
+    cap = committed_capture(cfg.name, f"tree{args.tree}")   # dram bytes of one execute from the committed ncu capture, if any
     achieved = alg_bytes / (ms * 1e-3) / 1e9
     line = {
         "metric": METRIC + " -- tree algorithm (side measurement)", "value": nrows * cfg.nsamps / (ms * 1e-3), "unit": UNIT,
@@ -393,7 +394,7 @@ def run_tree(args) -> None:
                    "trials": nrows, "dm_max": None if dms is None else float(dms[-1]), "passes": info["steps"],
                    "tile_columns": info["tile"], "device_bytes": info["device_bytes"], "l2": "inputs and outputs larger than L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                     "traffic": None, "peak_source": peaks["source"],
+                     "traffic": cap["traffic"], "ncu_capture": cap["capture"], "peak_source": peaks["source"],
                      "algorithmic_bytes": alg_bytes, "note": "packed input read once + float32 rows written once; the 16-bit rows "
                      "between the passes (written and read once each) are not counted"},
         "clocks": clk.summary()}
