@@ -389,7 +389,8 @@ def run_tree(args) -> None:
     line = {
         "metric": METRIC + " -- tree algorithm (side measurement)", "value": nrows * cfg.nsamps / (ms * 1e-3), "unit": UNIT,
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
-        "dtype": "u16", "data": "synthetic", "gpu_launches": info["last_launches"] * args.steps,
+        "dtype": "u16" if sb * ((1 << cfg.nbits) - 1) <= 65535 else "u32", "data": "synthetic",
+        "gpu_launches": info["last_launches"] * args.steps,
         "config": {"workload": cfg.name, "method": "frequency-padded tree" if padded else ("tree" if dms is None else "piecewise linear tree"), "sb_nchans": sb,
                    "trials": nrows, "dm_max": None if dms is None else float(dms[-1]), "passes": info["steps"],
                    "tile_columns": info["tile"], "device_bytes": info["device_bytes"], "l2": "inputs and outputs larger than L2"},

@@ -306,15 +306,15 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  * tests check element by element.
  *
  * dd_tree_create   nchans a power of two, 2 .. 4096; sb_nchans a power of two, 2 .. nchans (== nchans: the whole band is
- *                  one tree); nbits 2, 4 or 8; sb_nchans * (2^nbits - 1) <= 65535 (the stages add in 16-bit lanes), else
- *                  DD_ERR_OUT_RANGE; other values DD_ERR_INVALID_ARG.  No device needed.
+ *                  one tree); nbits 2, 4 or 8; other values DD_ERR_INVALID_ARG.  No device needed.  (The stages add in
+ *                  8- or 16-bit lanes while sb_nchans * (2^nbits - 1) <= 65535, in 32-bit lanes beyond.)
  * dd_tree_create_padded  the frequency-padded tree (section 3.1.2; readings X6-X8): the nchans real channels
  *                  of the band (f_top, df as in dd_plan_create) are placed at the rows nu'(c) of eq. 25 of a stretched band
  *                  of N_pad rows (nu'(nchans) rounded up to a power of two; the other rows are blank), in which the
  *                  quadratic dispersion curves are straight lines, and ONE tree runs over the N_pad rows (the paper scatters
  *                  the input into a zero array; here the first pass reads through the row map and nothing is
- *                  copied).  Trial d' of N_pad is DM(d') = d' / ((N_pad - 1) DeltaT(1)) (eq. 26).  N_pad <= 4096 and
- *                  N_pad * (2^nbits - 1) <= 65535 as for dd_tree_create.  dd_tree_execute then takes nchans input rows of
+ *                  copied).  Trial d' of N_pad is DM(d') = d' / ((N_pad - 1) DeltaT(1)) (eq. 26).  N_pad <= 4096, else
+ *                  DD_ERR_INVALID_ARG.  dd_tree_execute then takes nchans input rows of
  *                  nsamps + N_pad - 1 samples and writes N_pad rows; dd_tree_set_dm_list is DD_ERR_UNSUPPORTED.
  * dd_tree_get_padding  returns N_pad (negative status on error; DD_ERR_INVALID_ARG for a tree that is not padded) and, if
  *                  pos is not NULL, writes nu'(c) for the nchans real channels (HOST int32).
@@ -332,7 +332,7 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *                  nsamps elements of out_nbits (DD_OUT_*): without a DM list out[n N' + d'][t] = S_n[d'][t] (nchans rows:
  *                  the trees of all sub-bands; with sb_nchans == nchans the tree transform D'[d'][t]); with a DM list
  *                  out[d][t] (ndm rows).  Asynchronous on `stream`; the first call for a given nsamps allocates the
- *                  rows between the passes (8- or 16-bit, at most 4 nchans (nsamps + sb_nchans) bytes; with a DM list they
+ *                  rows between the passes (8-, 16- or 32-bit, at most 8 nchans (nsamps + sb_nchans) bytes; with a DM list they
  *                  include the stage-1 output), later calls only enqueue kernels.  DD_ERR_CUDA without a device.
  * dd_tree_set_tuning   test knob: key 1 = steps fused by the first pass (1 .. 6, 0 = default), key 2 = steps fused by
  *                  later passes (1 .. 6, 0 = as many as keep the overlap of neighbouring tiles within a quarter of a tile),

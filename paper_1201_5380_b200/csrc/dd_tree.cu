@@ -102,7 +102,12 @@ template <int LB>
 __device__ __forceinline__ uint4 tree_unpack_chunk(const uint4 v, int nb, int kk)
 {
     uint32_t o[4];
-    if constexpr (LB == 16) {   // 8 samples
+    if constexpr (LB == 32) {   // 4 samples of 8 bits (wider lanes are for sums beyond 65535: 8-bit input only): word kk
+        const uint32_t word = sel4(v, kk);
+#pragma unroll
+        for (int h = 0; h < 4; ++h)
+            o[h] = (word >> (8 * h)) & 0xFFu;
+    } else if constexpr (LB == 16) {   // 8 samples
         if (nb == 8) {          // words 2 kk, 2 kk + 1
             const uint32_t lo = sel4(v, 2 * kk), hi = sel4(v, 2 * kk + 1);
             o[0] = __byte_perm(lo, 0u, 0x4140), o[1] = __byte_perm(lo, 0u, 0x4342);
@@ -165,7 +170,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     constexpr int CH = ITEMS * TR_THREADS / (R / 2);        // 16-byte chunks per row (>= 32: a warp stays inside one row)
     constexpr int C = CH * CPC;                             // columns staged per row
     static_assert(CH >= 32 && (CH & (CH - 1)) == 0, "a warp's items must share their row");
-    static_assert(LB == 16 || (LB == 8 && PACKED), "8-bit lanes: first pass only");
+    static_assert(LB == 16 || LB == 32 || (LB == 8 && PACKED), "8-bit lanes: first pass only");
     extern __shared__ uint4 smv[];                          // [R][CH] + one chunk of padding
     const int tid = threadIdx.x, lane = tid & 31;
     const int tile = blockIdx.x, g = blockIdx.y;
@@ -180,7 +185,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
     // rows stores each one (x r) mod AL columns early (its store phase below): column t of the row as stored is column
     // t + (x r) mod AL of the row, and staging from the granule A(x r) = x r - (x r) mod AL on lands on column t0 + x r.
     const bool skew = p.i0 > 0;
-    constexpr int AL = PACKED ? 16 : 8;   // columns per 16 bytes of the rows staged: 8-bit rows / 16-bit rows
+    constexpr int AL = PACKED ? 16 : CPC;   // columns per 16 bytes of the rows staged: 8-bit rows / rows of the pass's own lanes
     const int tt = p.tt;
     const int64_t t0 = static_cast<int64_t>(tile) * tt;
     auto first_col = [&](int r) -> int64_t { return skew ? t0 + ((x * r) & ~(AL - 1)) : t0; };
@@ -320,7 +325,7 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         __syncthreads();
         if (lane == 0) {
             for (int r = tid >> 5; r < R; r += TR_THREADS / 32) {
-                const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + first_col(r) * 2;
+                const uint8_t *src = p.in + (row0 + (static_cast<int64_t>(r) << p.i0) + x) * p.in_stride + first_col(r) * (LB / 8);
                 tma_bulk_g2s(smv + r * CH, src, static_cast<uint32_t>(CH * 16), &full);
             }
         }
@@ -400,7 +405,10 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
                 if (col >= p.out_cols)
                     break;
                 uint4 v;
-                if constexpr (LB == 16) {
+                if constexpr (LB == 32) {     // (sums beyond 65535 have no uint16 output: dd_tree_execute refuses it)
+                    const uint4 a = srow[2 * c8], b = srow[2 * c8 + 1];
+                    v = make_uint4(a.x | a.y << 16, a.z | a.w << 16, b.x | b.y << 16, b.z | b.w << 16);
+                } else if constexpr (LB == 16) {
                     v = srow[c8];
                 } else {
                     const uint2 b = reinterpret_cast<const uint2 *>(srow)[c8];
@@ -423,7 +431,10 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
                 if (col >= p.out_cols)
                     break;
                 uint32_t e[4];
-                if constexpr (LB == 16) {
+                if constexpr (LB == 32) {
+                    const uint4 v = srow[c4];
+                    e[0] = v.x, e[1] = v.y, e[2] = v.z, e[3] = v.w;
+                } else if constexpr (LB == 16) {
                     const uint2 v = reinterpret_cast<const uint2 *>(srow)[c4];
                     e[0] = v.x & 0xFFFFu, e[1] = v.x >> 16, e[2] = v.y & 0xFFFFu, e[3] = v.y >> 16;
                 } else {
@@ -476,7 +487,9 @@ __global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint8_t *__r
         tree_windows<LB>(a, b, static_cast<int>(at & (CPC - 1)), x0, x1);
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
-            if constexpr (LB == 16) {
+            if constexpr (LB == 32) {
+                acc[h] += x0[h];
+            } else if constexpr (LB == 16) {
                 acc[2 * h] += x0[h] & 0xFFFFu;
                 acc[2 * h + 1] += x0[h] >> 16;
             } else {
@@ -490,7 +503,7 @@ __global__ void __launch_bounds__(TR2_THREADS) dd_tree_stage2(const uint8_t *__r
     uint8_t *orow = out + static_cast<int64_t>(d) * out_stride;
     const bool whole = vec_ok && col + CPC <= nsamps;
     if (out_code == DD_OUT_U16) {
-        if (whole) {
+        if (whole && CPC >= 8) {
 #pragma unroll
             for (int v = 0; v < CPC / 8; ++v)
                 reinterpret_cast<uint4 *>(orow + col * 2)[v] =
@@ -528,7 +541,8 @@ struct TreePass {
     int64_t ntiles = 0;
 };
 
-// kind: 0 = 16-bit rows in, 16-bit lanes; 1 = packed in, 16-bit lanes; 2 = packed in, 8-bit lanes
+// kind: 0 = 16-bit rows in, 16-bit lanes; 1 = packed in, 16-bit lanes; 2 = packed in, 8-bit lanes; 3 = packed in, 32-bit
+// lanes; 4 = 32-bit rows in, 32-bit lanes
 template <int Q, int ITEMS>
 cudaError_t launch_pass_qi(const TreePassParams &p, int kind, bool last, int64_t groups, int64_t ntiles, cudaStream_t stream)
 {
@@ -543,6 +557,10 @@ cudaError_t launch_pass_qi(const TreePassParams &p, int kind, bool last, int64_t
         kernel<<<dim3(static_cast<unsigned>(ntiles), static_cast<unsigned>(groups)), TR_THREADS, smem, stream>>>(p);
         return cudaGetLastError();
     };
+    if (kind == 4)
+        return last ? go(dd_tree_pass<Q, ITEMS, false, true, 32>) : go(dd_tree_pass<Q, ITEMS, false, false, 32>);
+    if (kind == 3)
+        return last ? go(dd_tree_pass<Q, ITEMS, true, true, 32>) : go(dd_tree_pass<Q, ITEMS, true, false, 32>);
     if (kind == 2)
         return last ? go(dd_tree_pass<Q, ITEMS, true, true, 8>) : go(dd_tree_pass<Q, ITEMS, true, false, 8>);
     if (kind == 1)
@@ -634,13 +652,17 @@ bool plan_passes(dd_tree_s *t, int64_t t_out)
         if (i0 > 0 && t->tune[1] > 0)
             q = std::min(q, t->tune[1]);
         // the first pass adds in 8-bit lanes when its sums stay below 256 (2-bit samples: any first pass; 4-bit: up to 4 steps)
-        auto lanes = [&](int qq) { return (i0 == 0 && t->tune[4] != 16 && vmax * (1 << qq) <= 255) ? 8 : 16; };
+        // (and in 32-bit lanes throughout when the sums of a tree go beyond 16 bits: 8-bit samples, more than 256 channels)
+        const bool wide = static_cast<int64_t>(t->sb) * vmax > 65535;
+        auto lanes = [&](int qq) { return wide ? 32 : ((i0 == 0 && t->tune[4] != 16 && vmax * (1 << qq) <= 255) ? 8 : 16); };
         // the overlap of neighbouring tiles is 2^q - 1 columns in every pass (later passes stage their rows skewed:
-        // dd_tree_pass); later passes take as many steps as keep it within a quarter of the columns staged
+        // dd_tree_pass); later passes, and a first pass in 32-bit lanes, take as many steps as keep it (and the columns a
+        // row may be stored early) within a quarter of the columns staged
         auto overlap = [&](int qq) { return (1 << qq) - 1; };
         for (; q > 1; --q) {
             const int cols = pass_cols(q, items, lanes(q));
-            if ((i0 == 0 || t->tune[1] > 0 || 4 * overlap(q) <= cols) && overlap(q) + 16 + 64 <= cols)
+            if (((i0 == 0 && !wide) || (i0 == 0 ? t->tune[0] : t->tune[1]) > 0 || 4 * (overlap(q) + 128 / lanes(q) - 1) <= cols) &&
+                overlap(q) + 16 + 64 <= cols)
                 break;
         }
         TreePass ps;
@@ -702,8 +724,6 @@ dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits)
     const int kn = dd::log2_exact(nchans), ks = dd::log2_exact(sb_nchans);
     if (nchans < 2 || nchans > 4096 || kn < 0 || sb_nchans < 2 || sb_nchans > nchans || ks < 0 || (nbits != 2 && nbits != 4 && nbits != 8))
         return DD_ERR_INVALID_ARG;
-    if (static_cast<int64_t>(sb_nchans) * ((1 << nbits) - 1) > 65535)
-        return DD_ERR_OUT_RANGE;
     dd_tree_s *t = new (std::nothrow) dd_tree_s;
     if (!t)
         return DD_ERR_NOMEM;
@@ -1019,7 +1039,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.next_i0 = p + 1 < np ? tree->passes[p + 1].i0 : 0;
         kp.next_q = p + 1 < np ? tree->passes[p + 1].q : 0;
         const int64_t groups = tree->nchans >> ps.q;
-        const int kind = ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0);
+        const int kind = ps.lane_bits == 32 ? (ps.packed ? 3 : 4) : (ps.lane_bits == 8 ? 2 : (ps.packed ? 1 : 0));
         if ((e = launch_pass(kp, ps.q, ps.items, kind, last, groups, ps.ntiles, st)) != cudaSuccess)
             return report_cuda_error(e, "dd_tree_execute pass");
         ++launches;
@@ -1029,7 +1049,7 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         const int lb = tree->passes[np - 1].lane_bits;
         const int cpt = 128 / lb;   // columns per thread
         const dim3 grid(static_cast<unsigned>((nsamps + TR2_THREADS * cpt - 1) / (TR2_THREADS * cpt)), static_cast<unsigned>(tree->ndm));
-        auto s2 = lb == 8 ? dd_tree_stage2<8> : dd_tree_stage2<16>;
+        auto s2 = lb == 8 ? dd_tree_stage2<8> : (lb == 16 ? dd_tree_stage2<16> : dd_tree_stage2<32>);
         s2<<<grid, TR2_THREADS, static_cast<size_t>(tree->ns) * sizeof(int2), st>>>(
             static_cast<const uint8_t *>(tree->buf[(np - 1) & 1]) + kTreeMargin * (lb / 8), tree->pitch[np - 1], static_cast<const int2 *>(tree->d_tab), tree->ns,
             static_cast<uint8_t *>(out_ptr), out_pitch_bytes, nsamps, out_nbits, rows16 ? 1 : 0);

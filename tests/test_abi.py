@@ -327,7 +327,8 @@ def test_tree_host_side():
     h = ctypes.c_void_p()
     for args in ((1000, 1000, 2), (1024, 48, 2), (1024, 2048, 2), (8192, 64, 2), (1, 1, 2), (64, 64, 3)):
         assert L.dd_tree_create(ctypes.byref(h), *args) == -2
-    assert L.dd_tree_create(ctypes.byref(h), 1024, 512, 8) == -6          # 512 * 255 does not fit the 16-bit lanes
+    assert L.dd_tree_create(ctypes.byref(h), 1024, 512, 8) == 0           # (sums beyond 16 bits: 32-bit lanes)
+    assert L.dd_tree_destroy(h) == 0
     assert L.dd_tree_create(None, 64, 64, 2) == -1 and L.dd_tree_destroy(None) == 0
     for n in (2, 4, 8, 32, 128, 1024):
         with dd.Tree(n, n, 2) as t:

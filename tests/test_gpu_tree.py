@@ -62,14 +62,14 @@ def test_tree_every_size_one_and_two_passes(nbits):
     # N = 2 .. 64: one pass; 128 .. 4096: two.  Four tiles of the first pass and a ragged tail; a row
     # length that allows 16-byte stores and one that does not; all output types
     for n in (2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096):
-        if n * ((1 << nbits) - 1) > 65535:
-            with pytest.raises(dd.DDError) as err:
-                dd.Tree(n, n, nbits)
-            assert err.value.status == -6
-            continue
-        kinds = ("u16", "u32", "f32") if n in (4, 64, 256) else ("u32",)
+        wide = n * ((1 << nbits) - 1) > 65535        # 8-bit samples, 512 channels and more: 32-bit lanes throughout
+        kinds = ("u16", "u32", "f32") if n in (4, 64, 256) else (("u32", "f32") if n == 1024 else ("u32",))
         info = _tree_case(nbits, n, 4 * 448 + 77, kinds)
-        assert info["passes"] == (1 if n <= 64 else 2)
+        assert info["passes"] == (1 if n <= (32 if wide else 64) else 2 if n <= (1024 if wide else 4096) else 3)
+        if wide:                                     # sums that do not fit uint16 rows are refused at execute
+            with dd.Tree(n, n, nbits) as t, pytest.raises(dd.DDError) as err:
+                t.execute(64, torch.zeros(16, dtype=torch.uint8, device="cuda"), 1 << 20, torch.zeros(16, device="cuda"), 16)
+            assert err.value.status == -6
     _tree_case(nbits, 64, 2048, ("u16", "f32"))
     _tree_case(nbits, 64, 2048, ("u32",), tuning=((6, 1),))
     _tree_case(nbits, 256, 3000, ("u32",), tuning=((6, 1),))
@@ -130,6 +130,8 @@ def test_piecewise_linear_tree_small_bands(nbits):
     _piecewise_case(nbits, 256, 8, 9, 50.0, 3000, "f32")
     _piecewise_case(nbits, 128, 64, 17, 68.0, 2111, "u16" if nbits < 8 else "u32")
     _piecewise_case(nbits, 64, 64, 5, 70.0, 1000)   # one sub-band: stage 2 only picks rows
+    if nbits == 8:                                  # sub-bands of 512 eight-bit channels: 32-bit lanes in both stages
+        _piecewise_case(8, 1024, 512, 9, 40.0, 1500, "f32")
     # stage-1 rows in 16-bit lanes where the default is 8-bit lanes (2-bit samples), and two passes of stage 1
     _piecewise_case(nbits, 256, 32, 23, 45.0, 2000, "u16" if nbits < 8 else "u32", tuning=((5, 16),))
     _piecewise_case(nbits, 128, 64, 17, 68.0, 1500, "f32", tuning=((1, 3), (2, 3)))
@@ -179,12 +181,7 @@ def test_frequency_padded_tree(nbits):
     for nchans, f_top, df, nsamps, kind in ((24, 1500.0, -8.0, 1111, "u32"), (100, 1581.8, -0.390625, 2 * 960 + 77, "u16"),
                                             (100, 1581.8, -4.0, 3000, "f32"), (1024, 1581.8, -0.390625, 2500, "f32")):
         cfg = W.CONFIGS[{2: 2, 4: 4, 8: 5}[nbits]].reduced(nsamps=nsamps, ndm=2, nchans=nchans, nbeams=1)
-        try:
-            t = dd.Tree.padded(nchans, f_top, df, nbits)
-        except dd.DDError as err:                      # 8-bit: the 16-bit lanes hold trees of up to 256 rows
-            assert nbits == 8 and err.status == -6
-            continue
-        with t:
+        with dd.Tree.padded(nchans, f_top, df, nbits) as t:
             npad = t.nchans
             assert t.required_samples(nsamps) == nsamps + npad - 1 and npad >= nchans
             packed, stride = W.gen_packed(cfg, npad - 1, None)
