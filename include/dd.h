@@ -305,8 +305,11 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  * (the trail inside a sub-band is a straight line); it is exact in the sense of the paper's own definition, which the
  * tests check element by element.
  *
- * dd_tree_create   nchans a power of two, 2 .. 4096; sb_nchans a power of two, 2 .. nchans (== nchans: the whole band is
- *                  one tree); nbits 2, 4 or 8; other values DD_ERR_INVALID_ARG.  No device needed.  (The stages add in
+ * dd_tree_create   sb_nchans a power of two, 2 .. 4096: the channels of one tree; nchans a multiple of it, up to 65536: the
+ *                  rows are nchans / sb_nchans trees one after the other -- the sub-bands of one band (== 1: the whole band
+ *                  is one tree), or the bands of several beams whose rows lie back to back (without a DM list: stage 2
+ *                  sums ALL sub-bands of the rows, so it serves one beam); nbits 2, 4 or 8; other values
+ *                  DD_ERR_INVALID_ARG.  No device needed.  (The stages add in
  *                  8- or 16-bit lanes while sb_nchans * (2^nbits - 1) <= 65535, in 32-bit lanes beyond.)
  * dd_tree_create_padded  the frequency-padded tree (section 3.1.2; readings X6-X8): the nchans real channels
  *                  of the band (f_top, df as in dd_plan_create) are placed at the rows nu'(c) of eq. 25 of a stretched band

@@ -721,8 +721,10 @@ dd_status dd_tree_create(dd_tree *tree, int nchans, int sb_nchans, int nbits)
     if (!tree)
         return DD_ERR_NULL;
     *tree = nullptr;
-    const int kn = dd::log2_exact(nchans), ks = dd::log2_exact(sb_nchans);
-    if (nchans < 2 || nchans > 4096 || kn < 0 || sb_nchans < 2 || sb_nchans > nchans || ks < 0 || (nbits != 2 && nbits != 4 && nbits != 8))
+    // (the rows are nchans / sb_nchans trees one after the other: sub-bands of one band, or the bands of several beams)
+    const int ks = dd::log2_exact(sb_nchans);
+    if (nchans < 2 || nchans > 65536 || sb_nchans < 2 || sb_nchans > 4096 || sb_nchans > nchans || ks < 0 || nchans % sb_nchans != 0 ||
+        (nbits != 2 && nbits != 4 && nbits != 8))
         return DD_ERR_INVALID_ARG;
     dd_tree_s *t = new (std::nothrow) dd_tree_s;
     if (!t)

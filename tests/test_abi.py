@@ -325,7 +325,7 @@ def test_tree_host_side():
     from oracle.oracle_np import piecewise_tree_required_samples, piecewise_tree_tables, tree_delays_np
     L = dd.lib()
     h = ctypes.c_void_p()
-    for args in ((1000, 1000, 2), (1024, 48, 2), (1024, 2048, 2), (8192, 64, 2), (1, 1, 2), (64, 64, 3)):
+    for args in ((1000, 1000, 2), (1024, 48, 2), (1024, 2048, 2), (8192, 8192, 2), (1000, 64, 2), (1 << 17, 64, 2), (1, 1, 2), (64, 64, 3)):
         assert L.dd_tree_create(ctypes.byref(h), *args) == -2
     assert L.dd_tree_create(ctypes.byref(h), 1024, 512, 8) == 0           # (sums beyond 16 bits: 32-bit lanes)
     assert L.dd_tree_destroy(h) == 0

@@ -257,3 +257,15 @@ def test_tree_execute_is_cuda_graph_capturable():
                 ref = (oracle.piecewise_tree(host, nbits, nsamps, n, cfg.dt, cfg.f_top, cfg.df, dms, 32) if piecewise
                        else oracle.tree(host, nbits, nsamps))
                 _assert_equal(out.cpu().numpy(), oracle.cast_out(ref, "f32"), f"graph replay {k}, piecewise={piecewise}")
+
+
+def test_trees_of_several_beams_in_one_call():
+    # the rows of three beams back to back (768 rows, trees of 256: not a power of two in all): one call, one tree per beam
+    nbits, n, nbeams, nsamps = 2, 256, 3, 3000
+    cfg = W.CONFIGS[2].reduced(nsamps=nsamps, ndm=2, nchans=n, nbeams=nbeams)
+    packed, stride = W.gen_packed(cfg, n - 1, None)
+    with dd.Tree(nbeams * n, n, nbits) as t:
+        got = _run(t, nsamps, packed.cuda(), stride, nbeams * n, "u32")
+    for b in range(nbeams):
+        ref = oracle.tree(packed[b].numpy(), nbits, nsamps)
+        _assert_equal(got[b * n:(b + 1) * n], oracle.cast_out(ref, "u32"), f"beam {b}")
