@@ -341,8 +341,9 @@ dd_status dd_scrunch_destroy(dd_scrunch set);
  *                  later passes (1 .. 6, 0 = as many as keep the overlap of neighbouring tiles within a quarter of a tile),
  *                  key 3 / 4 = items per thread of the first / of later passes (4: two CTAs per SM, 8: one; 0 = default),
  *                  key 5 = 16: the first pass adds in 16-bit lanes even where 8-bit lanes hold its sums (0 = default),
- *                  key 6 = 1: the first pass makes its first two steps in shared memory like the others instead of
- *                  in registers while it stages its rows (0 = default).
+ *                  key 6 = bit 0: the first two steps of a pass over packed rows are made in shared memory like the
+ *                  others instead of in registers while the rows are staged; bit 1: every step makes its own trip through
+ *                  shared memory instead of two steps per trip (0 = default).
  *                  Takes effect at the next execute.
  * dd_tree_get_info info[0] = passes, info[1] = kernels enqueued by the last execute, info[2] = device bytes held,
  *                  info[3 + 2 p] / info[4 + 2 p] = steps fused by pass p / columns a tile of it stores (p < 6); int64 x 16.

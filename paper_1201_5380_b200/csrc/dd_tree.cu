@@ -54,6 +54,7 @@ struct TreePassParams {
     int32_t i0;            // first step of the pass
     int32_t tt;            // columns a tile stores (multiple of 64)
     int32_t fuse2;         // packed rows: steps 0 and 1 are made while the rows are staged (the step loop starts at 2)
+    int32_t radix4;        // pairs of steps in one trip through shared memory (0: every step on its own)
     int32_t next_i0;       // not LAST: the pass that reads these rows starts at step next_i0 and takes next_q steps
     int32_t next_q;        //   (0: no pass follows -- stage 2 reads the rows as they are)
     const int32_t *row_map;   // first pass of a frequency-padded tree: input row of every tree row, -1 = blank; else NULL
@@ -335,10 +336,16 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
         smv[R * CH] = make_uint4(0, 0, 0, 0);
 
     // ---- Q steps in place
-#pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        if (PACKED && p.fuse2 && q < 2)
-            continue;
+    // the window of U: CPC lanes of staged row `row` from lane ch CPC + shift on (x0), and from one lane further on (x1)
+    auto windows_at = [&](int row, int ch, int shift, uint32_t (&x0)[4], uint32_t (&x1)[4]) {
+        int uch = ch + shift / CPC;
+        uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
+        const uint4 *u = smv + row * CH + uch;
+        const uint4 ua = u[0], ub = u[1];
+        tree_windows<LB>(ua, ub, shift & (CPC - 1), x0, x1);
+    };
+    // one step (eq. 11-12): out[c][2 o + b] = L[o] + U[o] at + (o + b); an item is one pair (L row, U row) x one chunk
+    auto radix2 = [&](const int q) {
         uint32_t s0[ITEMS][4], s1[ITEMS][4];
         __syncthreads();
 #pragma unroll
@@ -347,14 +354,9 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             const int ch = id & (CH - 1), pair = id / CH;
             const int o = pair & ((1 << q) - 1), c = pair >> q;
             const int lrow = ((2 * c) << q) + o;
-            const int shift = o;   // (+ b for the second sum; the x 2^q of a later pass is in the staging)
-            int uch = ch + shift / CPC;
-            uch = uch < CH - 1 ? uch : CH - 1;   // (columns whose window leaves the tile are never stored)
             const uint4 l = smv[lrow * CH + ch];
-            const uint4 *u = smv + (lrow + (1 << q)) * CH + uch;
-            const uint4 ua = u[0], ub = u[1];
             uint32_t x0[4], x1[4];
-            tree_windows<LB>(ua, ub, shift & (CPC - 1), x0, x1);
+            windows_at(lrow + (1 << q), ch, o, x0, x1);   // (+ b for the second sum; the x 2^q of a later pass is in the staging)
             const uint32_t lw[4] = {l.x, l.y, l.z, l.w};
 #pragma unroll
             for (int h = 0; h < 4; ++h) {
@@ -371,6 +373,71 @@ __global__ void __launch_bounds__(TR_THREADS, ITEMS <= 4 ? 2 : 1) dd_tree_pass(c
             uint4 *dst = smv + ((c << (q + 1)) + 2 * o) * CH + ch;
             dst[0] = make_uint4(s0[it][0], s0[it][1], s0[it][2], s0[it][3]);
             dst[CH] = make_uint4(s1[it][0], s1[it][1], s1[it][2], s1[it][3]);
+        }
+    };
+    // TWO steps q, q + 1 in one trip through shared memory: four blocks A, B, C, D of 2^q rows merge into one of 2^(q+2),
+    //     out[4 o + 2 b1 + b2] = A[o] + B[o] at + (o + b1) + C[o] at + (2 o + b1 + b2) + D[o] at + (3 o + 2 b1 + b2)
+    // (step q makes A + B at o + b1 and C + D at o + b1, step q + 1 adds the second to the first at 2 o + b1 + b2): 11
+    // 16-byte loads and 4 stores per item of four rows instead of 2 x (6 + 4) -- the passes are bound by shared memory.
+    auto radix4 = [&](const int q) {
+        constexpr int NI = ITEMS / 2;
+        uint32_t res[NI][4][4];
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < NI; ++it) {
+            const int id = it * TR_THREADS + tid;
+            const int ch = id & (CH - 1), quad = id / CH;
+            const int o = quad & ((1 << q) - 1), c = quad >> q;
+            const int arow = ((4 * c) << q) + o;
+            const uint4 a = smv[arow * CH + ch];
+            const uint32_t aw[4] = {a.x, a.y, a.z, a.w};
+            uint32_t x0[4], x1[4];
+            windows_at(arow + (1 << q), ch, o, x0, x1);                 // B at o, o + 1
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                res[it][0][h] = res[it][1][h] = aw[h] + x0[h];
+                res[it][2][h] = res[it][3][h] = aw[h] + x1[h];
+            }
+            windows_at(arow + (2 << q), ch, 2 * o, x0, x1);             // C at 2 o, 2 o + 1
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                res[it][0][h] += x0[h], res[it][1][h] += x1[h], res[it][2][h] += x1[h];
+            windows_at(arow + (2 << q), ch, 2 * o + 2, x0, x1);         // C at 2 o + 2
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                res[it][3][h] += x0[h];
+            windows_at(arow + (3 << q), ch, 3 * o, x0, x1);             // D at 3 o, 3 o + 1
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                res[it][0][h] += x0[h], res[it][1][h] += x1[h];
+            windows_at(arow + (3 << q), ch, 3 * o + 2, x0, x1);         // D at 3 o + 2, 3 o + 3
+#pragma unroll
+            for (int h = 0; h < 4; ++h)
+                res[it][2][h] += x0[h], res[it][3][h] += x1[h];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < NI; ++it) {
+            const int id = it * TR_THREADS + tid;
+            const int ch = id & (CH - 1), quad = id / CH;
+            const int o = quad & ((1 << q) - 1), c = quad >> q;
+            uint4 *dst = smv + ((c << (q + 2)) + 4 * o) * CH + ch;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                dst[k * CH] = make_uint4(res[it][k][0], res[it][k][1], res[it][k][2], res[it][k][3]);
+        }
+    };
+    const int q0 = (PACKED && p.fuse2) ? 2 : 0;   // (steps 0 and 1 were made while staging)
+#pragma unroll
+    for (int q = 0; q < Q; q += 2) {
+        if (q < q0)
+            continue;
+        if (q + 1 < Q && p.radix4) {
+            radix4(q);
+        } else {
+            radix2(q);
+            if (q + 1 < Q)
+                radix2(q + 1);
         }
     }
     __syncthreads();
@@ -904,7 +971,7 @@ dd_status dd_tree_set_tuning(dd_tree tree, int key, int value)
 {
     if (!tree)
         return DD_ERR_NULL;
-    if (key < 1 || key > 6 || value < 0 || (key == 6 && value > 1) || (key <= 2 && value > 6) || ((key == 3 || key == 4) && value != 0 && value != 4 && value != 8) ||
+    if (key < 1 || key > 6 || value < 0 || (key == 6 && value > 3) || (key <= 2 && value > 6) || ((key == 3 || key == 4) && value != 0 && value != 4 && value != 8) ||
         (key == 5 && value != 0 && value != 16))
         return DD_ERR_INVALID_ARG;
     tree->tune[key - 1] = value;
@@ -1037,7 +1104,8 @@ dd_status dd_tree_execute(dd_tree tree, int64_t nsamps, const void *in_ptr, int6
         kp.row_map = first ? static_cast<const int32_t *>(tree->d_row_map) : nullptr;
         // steps 0 and 1 while staging packed rows (the input, or 8-bit rows): the chunk of a thread must be whole packed words
         // (not 2-bit samples in 16-bit lanes)
-        kp.fuse2 = (ps.packed && ps.q >= 2 && tree->tune[5] == 0 && (128 / ps.lane_bits) * ps.in_bits >= 32) ? 1 : 0;
+        kp.fuse2 = (ps.packed && ps.q >= 2 && (tree->tune[5] & 1) == 0 && (128 / ps.lane_bits) * ps.in_bits >= 32) ? 1 : 0;
+        kp.radix4 = (tree->tune[5] & 2) ? 0 : 1;
         kp.next_i0 = p + 1 < np ? tree->passes[p + 1].i0 : 0;
         kp.next_q = p + 1 < np ? tree->passes[p + 1].q : 0;
         const int64_t groups = tree->nchans >> ps.q;

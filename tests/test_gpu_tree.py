@@ -71,8 +71,9 @@ def test_tree_every_size_one_and_two_passes(nbits):
                 t.execute(64, torch.zeros(16, dtype=torch.uint8, device="cuda"), 1 << 20, torch.zeros(16, device="cuda"), 16)
             assert err.value.status == -6
     _tree_case(nbits, 64, 2048, ("u16", "f32"))
-    _tree_case(nbits, 64, 2048, ("u32",), tuning=((6, 1),))
-    _tree_case(nbits, 256, 3000, ("u32",), tuning=((6, 1),))
+    for k6 in (1, 2, 3):
+        _tree_case(nbits, 64, 2048, ("u32",), tuning=((6, k6),))
+        _tree_case(nbits, 512, 3000, ("u32",), tuning=((6, k6),))
 
 
 def test_tree_later_passes_over_several_tiles():
@@ -95,8 +96,9 @@ def test_tree_pass_shapes(first):
     # (2-bit samples: 8-bit lanes in the first pass unless told otherwise; 4-bit: only while 15 * 2^first < 256)
     for later in (1, 2, 3):
         for items, nbits, lanes in ((4, 4, 0), (8, 2, 0), (4, 2, 16), (8, 4, 16)):
-            # (key 6: the first two steps in shared memory instead of in registers while staging)
-            info = _tree_case(nbits, 64, 1500, tuning=((1, first), (2, later), (3, items), (4, items), (5, lanes), (6, later % 2)))
+            # (key 6: bit 0 = the first two steps in shared memory instead of in registers while staging, bit 1 = one step
+            # per trip through shared memory instead of two)
+            info = _tree_case(nbits, 64, 1500, tuning=((1, first), (2, later), (3, items), (4, items), (5, lanes), (6, (first + later) % 4)))
             assert info["steps"][0] == first and all(s <= later for s in info["steps"][1:])
     for later in (4, 5, 6):
         if first + later <= 8:
